@@ -1,0 +1,164 @@
+/*
+ * md_b200.h -- C ABI of libmd_b200.so: the short-range force hot path of arXiv 1401.4350
+ * ("A comparison between parallelization approaches in molecular dynamics simulations on GPUs")
+ * written for one NVIDIA B200 (sm_100a).
+ *
+ * Citations: P:<n> = PAPER.md line n of the paper text; B:<n> = BASELINE.json line n;
+ *            S:<x> = SURVEY.md section 8 item x; D:<x> = DESIGN.md section x.
+ *
+ * The library implements, as hand-written CUDA kernels only (no CPU fallback, no library kernels):
+ *   - the "standard cell algorithm" + Verlet lists L_i of radius r_v = r_c + r_s
+ *   - VERTEX: one thread per particle loops over L_i, every pair computed twice, no atomics
+ *   - EDGE:   one thread per potentially interacting pair, F_ij = -F_ji, scatter to both
+ *   - velocity-Verlet NVE with a skin-triggered rebuild, energies                          (B:5)
+ *
+ * Conventions
+ *   Units        reduced LJ units, epsilon = sigma = m = k_B = 1 in all configs (B:7).
+ *   Memory       the CALLER owns all device memory: six state arrays and one workspace blob sized by
+ *                md_workspace_bytes().  The library never allocates device memory; md_destroy frees
+ *                only the host handle.  "device" / "host" is stated for every pointer below.
+ *   State layout float4 per particle (16-byte aligned device pointers), S:A1:
+ *                  pos   = (x, y, z, unused)        vel    = (vx, vy, vz, unused)
+ *                  force = (fx, fy, fz, pe_i)       pe_i = half of every pair/bond energy of i
+ *                  quat  = (w, x, y, z) unit        angmom = (Lx, Ly, Lz, unused) space frame
+ *                  torque= (tx, ty, tz, unused)     space frame
+ *                The arrays are borrowed from md_bind_state() until md_destroy().  When an order
+ *                other than MD_ORDER_NONE is set, md_build_cells() PERMUTES them in place: slot s
+ *                then holds the particle whose original id is ids[s] (md_get_ids).
+ *   Stream       every call enqueues on the CUDA stream given to md_create and returns without
+ *                synchronising, except md_energy, md_stats, md_get_pairs, md_get_ids,
+ *                md_step_host (they synchronise that stream).
+ *   Errors       every function returns an md_status (0 = success, negative = failure); the
+ *                text is available from md_last_error().  Device-detected conditions (neighbour
+ *                capacity overflow, FENE bond >= R0) are latched in a device flag and reported by
+ *                the next synchronising call.  No partial results are defined after a failure.
+ *   Determinism  VERTEX and MD_SCATTER_SEGMENTED are run-to-run bitwise reproducible; the
+ *                atomic scatter variants are not.
+ */
+#ifndef MD_B200_H
+#define MD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct md_system md_system; /* opaque host handle */
+
+typedef enum {
+    MD_OK = 0,
+    MD_ERR_INVALID = -1,  /* bad argument or geometry (box too small for r_v, N <= 0, ...) */
+    MD_ERR_STATE = -2,    /* call order: forces before lists, no state bound, ...            */
+    MD_ERR_CAPACITY = -3, /* a particle has more than max_neigh Verlet neighbours            */
+    MD_ERR_CUDA = -4,     /* CUDA runtime error (sticky)                                     */
+    MD_ERR_NUMERIC = -5   /* FENE bond length >= R0                                          */
+} md_status;
+
+typedef enum { MD_POT_LJ = 0, MD_POT_FENE_WCA = 1, MD_POT_PATCHY = 2 } md_pot_kind;
+typedef enum { MD_VERTEX = 0, MD_EDGE = 1 } md_strategy;
+/* EDGE scatter alternatives (B:5, S:A7); ignored for MD_VERTEX. */
+typedef enum {
+    MD_SCATTER_RED = 0,      /* red.global.add.f32, one per component                           */
+    MD_SCATTER_RED_V4 = 1,   /* red.global.add.v4.f32, one per particle and output array        */
+    MD_SCATTER_WARP = 2,     /* runs of equal owner i combined by warp shuffles, then one red.v4 */
+    MD_SCATTER_SEGMENTED = 3 /* per-edge store + atomic-free segmented reduction         */
+} md_scatter;
+typedef enum { MD_ORDER_NONE = 0, MD_ORDER_CELL = 1, MD_ORDER_HILBERT = 2 } md_order;
+
+/* Pair potential and rigid-body parameters.
+ *   MD_POT_LJ        Eq. (1), cut at rcut and energy-shifted by V(rcut) if shift_energy.
+ *   MD_POT_FENE_WCA  B:9: WCA (LJ cut at rcut = 2^(1/6) sigma, shifted by +epsilon) on all pairs, plus
+ *                    FENE bonds U = -1/2 K R0^2 ln(1 - r^2/R0^2) between ids (i, i+1) inside chains of
+ *                    chain_len consecutive ids.
+ *   MD_POT_PATCHY    B:10: WCA core cut at rcut_core plus n_patches x n_patches patch terms
+ *                    -eps_patch exp(-(r-sigma)^2/(2 patch_sigma_r^2)) exp(-(1-cos th_i)/patch_sigma_ang^2)
+ *                    exp(-(1-cos th_j)/patch_sigma_ang^2), truncated (not shifted) at rcut. */
+typedef struct {
+    int32_t kind; /* md_pot_kind */
+    float epsilon, sigma, mass;
+    int32_t shift_energy;
+    float fene_K, fene_R0;
+    int32_t chain_len;
+    int32_t n_patches; /* <= 8 */
+    float patch_dir[8][3]; /* body-frame unit vectors */
+    float eps_patch, patch_sigma_r, patch_sigma_ang;
+    float rcut_core;
+    float inertia; /* scalar moment of inertia of the spherical top (S:O7) */
+} md_potential;
+
+/* Bytes of device workspace md_create needs for these parameters.  host pointers. */
+md_status md_workspace_bytes(int64_t N, const double box[3], double rcut, double skin,
+                             const md_potential* pot, int32_t max_neigh, size_t* bytes);
+
+/* Create a system of N particles in the periodic orthorhombic box[3] (cells of width >= r_v =
+ * rcut + skin, Verlet lists of radius r_v).  box, pot: host.  workspace: DEVICE pointer, 256-byte
+ * aligned, workspace_bytes >= md_workspace_bytes(...), owned by the caller and borrowed until
+ * md_destroy.  cuda_stream: a cudaStream_t (may be NULL for the legacy default stream).
+ * max_neigh: capacity of every L_i (rounded up to a multiple of 4).
+ * MD_ERR_INVALID if N <= 0, N*max_neigh >= 2^31, box[k] < 2 (rcut + 2 skin), bad potential. */
+md_status md_create(md_system** out, int64_t N, const double box[3], double rcut, double skin,
+                    const md_potential* pot, int32_t max_neigh, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream);
+
+/* Bind the state arrays (DEVICE pointers to float4[N]; quat/angmom/torque may be NULL unless
+ * kind == MD_POT_PATCHY), taken to be in ORIGINAL id order: binding resets the slot map to the identity and
+ * invalidates cells, lists and forces.  Positions may lie anywhere; md_build_cells wraps them into [0, box_k). */
+md_status md_bind_state(md_system*, void* pos, void* vel, void* force, void* quat, void* angmom, void* torque);
+
+/* Storage order applied at every list build ("sorted along a Hilbert curve"). Default NONE. */
+md_status md_set_order(md_system*, int32_t order);
+
+/* S:A2/A3 ("cell filling ... one-particle-per-thread"): wrap positions into [0, box), bin into
+ * cells, counting sort; with an order set, permute all bound state arrays into cell / Hilbert order. */
+md_status md_build_cells(md_system*);
+
+/* S:A4: L_i = { j != i : |r_ij|^2 < r_v^2 }, predicate evaluated in fp64 on the fp32 positions in
+ * the fixed order of S:O0 (bit-exact pair set).  Emits the full list (VERTEX) and the half list i<j
+ * sorted by i (EDGE, "number of threads = sum_i |L_i| / 2"), and records the reference
+ * positions of the skin criterion.  Requires md_build_cells since the last position change. */
+md_status md_build_verlet(md_system*);
+
+/* S:A6/A7: forces, per-particle energies (force.w) and torques for the current positions.
+ * Lists must be valid (no particle moved more than skin/2 since md_build_verlet). */
+md_status md_forces(md_system*, int32_t strategy, int32_t scatter);
+
+/* S:A10 (B:5): nsteps of NVE velocity-Verlet (S:O6; rigid bodies S:O7) in fp32 state.  Each step:
+ * half kick, drift, skin check max_i |x_i - x_i^ref|^2 > (skin/2)^2 -> rebuild cells + lists on the
+ * device without host synchronisation, forces, half kick.  Requires valid forces on entry. */
+md_status md_integrate(md_system*, double dt, int64_t nsteps, int32_t strategy, int32_t scatter);
+
+/* S:A9: U = sum_i pe_i, K_t = 1/2 m sum |v|^2, K_r = sum |L|^2 / (2 I), accumulated in fp64.
+ * Host output pointers.  Synchronises; reports latched device errors. */
+md_status md_energy(md_system*, double* e_pot, double* e_kin_trans, double* e_kin_rot);
+
+/* Counters (host pointers, any may be NULL).  n_edges = E = 1/2 sum |L_i|. Synchronises. */
+md_status md_stats(md_system*, int64_t* n_edges, int64_t* n_full_entries, int32_t* max_neigh_seen,
+                   int64_t* n_rebuilds);
+
+/* Copy the half list to the HOST as pairs of ORIGINAL ids (lo, hi), unsorted. pairs_host has room for
+ * `capacity` pairs (2 int32 each); *n receives the pair count (even if > capacity). Synchronises. */
+md_status md_get_pairs(md_system*, int32_t* pairs_host, int64_t capacity, int64_t* n);
+
+/* ids_host[s] = original id of the particle stored in slot s (identity for MD_ORDER_NONE). Synchronises. */
+md_status md_get_ids(md_system*, int32_t* ids_host);
+
+/* End-to-end entry with HOST buffers (float4[N] each; quat/angmom/torque NULL unless patchy):
+ * copies pos, vel (quat, angmom) host->device into the bound arrays, builds cells and lists,
+ * evaluates forces, runs nsteps of md_integrate, and copies pos, vel, force (quat, angmom, torque)
+ * back to the host in ORIGINAL id order.  Synchronises. */
+md_status md_step_host(md_system*, void* pos_host, void* vel_host, void* force_host, void* quat_host,
+                       void* angmom_host, void* torque_host, double dt, int64_t nsteps, int32_t strategy,
+                       int32_t scatter);
+
+/* Number of kernels this library has launched on behalf of the handle (for bench.py's gpu_launches). */
+int64_t md_launch_count(const md_system*);
+
+const char* md_last_error(const md_system*);
+void md_destroy(md_system*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MD_B200_H */

@@ -1,0 +1,273 @@
+"""ctypes binding of libmd_b200.so: argument marshalling only (same names as include/md_b200.h)."""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import Optional
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libmd_b200.so"
+
+STRATEGY = {"vertex": 0, "edge": 1}
+SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3}
+ORDER = {"none": 0, "cell": 1, "hilbert": 2}
+POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2}
+STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPACITY", -4: "MD_ERR_CUDA",
+          -5: "MD_ERR_NUMERIC"}
+
+# every symbol include/md_b200.h declares (checked by tests/test_abi.py against the header and the .so)
+EXPORTED_SYMBOLS = ["md_workspace_bytes", "md_create", "md_bind_state", "md_set_order", "md_build_cells",
+                    "md_build_verlet", "md_forces", "md_integrate", "md_energy", "md_stats", "md_get_pairs",
+                    "md_get_ids", "md_step_host", "md_launch_count", "md_last_error", "md_destroy"]
+
+
+class MDError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class MDPotential(C.Structure):
+    _fields_ = [
+        ("kind", C.c_int32),
+        ("epsilon", C.c_float), ("sigma", C.c_float), ("mass", C.c_float),
+        ("shift_energy", C.c_int32),
+        ("fene_K", C.c_float), ("fene_R0", C.c_float),
+        ("chain_len", C.c_int32),
+        ("n_patches", C.c_int32),
+        ("patch_dir", (C.c_float * 3) * 8),
+        ("eps_patch", C.c_float), ("patch_sigma_r", C.c_float), ("patch_sigma_ang", C.c_float),
+        ("rcut_core", C.c_float),
+        ("inertia", C.c_float),
+    ]
+
+
+def make_potential(d: dict) -> MDPotential:
+    p = MDPotential()
+    p.kind = POT_KIND[d["kind"]]
+    p.epsilon = d.get("epsilon", 1.0)
+    p.sigma = d.get("sigma", 1.0)
+    p.mass = d.get("mass", 1.0)
+    p.shift_energy = int(d.get("shift_energy", 1))
+    p.fene_K = d.get("fene_K", 30.0)
+    p.fene_R0 = d.get("fene_R0", 1.5)
+    p.chain_len = int(d.get("chain_len", 1))
+    dirs = np.asarray(d.get("patch_dir", np.zeros((0, 3))), dtype=np.float64)
+    p.n_patches = int(d.get("n_patches", dirs.shape[0]))
+    for a in range(min(8, dirs.shape[0])):
+        for k in range(3):
+            p.patch_dir[a][k] = float(dirs[a, k])
+    p.eps_patch = d.get("eps_patch", 0.0)
+    p.patch_sigma_r = d.get("patch_sigma_r", 0.1)
+    p.patch_sigma_ang = d.get("patch_sigma_ang", 0.3)
+    p.rcut_core = d.get("rcut_core", 2.0 ** (1.0 / 6.0))
+    p.inertia = d.get("inertia", 0.1)
+    return p
+
+
+def library_path() -> Path:
+    return _LIB_PATH
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """Load libmd_b200.so (built in-tree by paper_1401_4350_b200/build.py). Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_1401_4350_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(str(_LIB_PATH))
+    dp3 = C.POINTER(C.c_double)
+    vp = C.c_void_p
+    L.md_workspace_bytes.restype = C.c_int
+    L.md_workspace_bytes.argtypes = [C.c_int64, dp3, C.c_double, C.c_double, C.POINTER(MDPotential), C.c_int32,
+                                     C.POINTER(C.c_size_t)]
+    L.md_create.restype = C.c_int
+    L.md_create.argtypes = [C.POINTER(vp), C.c_int64, dp3, C.c_double, C.c_double, C.POINTER(MDPotential), C.c_int32,
+                            vp, C.c_size_t, vp]
+    L.md_bind_state.restype = C.c_int
+    L.md_bind_state.argtypes = [vp] * 7
+    L.md_set_order.restype = C.c_int
+    L.md_set_order.argtypes = [vp, C.c_int32]
+    for name in ("md_build_cells", "md_build_verlet"):
+        getattr(L, name).restype = C.c_int
+        getattr(L, name).argtypes = [vp]
+    L.md_forces.restype = C.c_int
+    L.md_forces.argtypes = [vp, C.c_int32, C.c_int32]
+    L.md_integrate.restype = C.c_int
+    L.md_integrate.argtypes = [vp, C.c_double, C.c_int64, C.c_int32, C.c_int32]
+    L.md_energy.restype = C.c_int
+    L.md_energy.argtypes = [vp, dp3, dp3, dp3]
+    L.md_stats.restype = C.c_int
+    L.md_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
+    L.md_get_pairs.restype = C.c_int
+    L.md_get_pairs.argtypes = [vp, C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int64)]
+    L.md_get_ids.restype = C.c_int
+    L.md_get_ids.argtypes = [vp, C.POINTER(C.c_int32)]
+    L.md_step_host.restype = C.c_int
+    L.md_step_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_double, C.c_int64, C.c_int32, C.c_int32]
+    L.md_launch_count.restype = C.c_int64
+    L.md_launch_count.argtypes = [vp]
+    L.md_last_error.restype = C.c_char_p
+    L.md_last_error.argtypes = [vp]
+    L.md_destroy.restype = None
+    L.md_destroy.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def _code(x) -> int:
+    return x if isinstance(x, int) else (STRATEGY.get(x, None) if x in STRATEGY else SCATTER[x])
+
+
+class MDSystem:
+    """One system on one GPU. State lives in torch CUDA tensors ([N,4] float32) owned by this object and
+    borrowed by the library; the workspace is one torch uint8 tensor."""
+
+    def __init__(self, N: int, box, rcut: float, skin: float, potential: dict, max_neigh: int,
+                 device: str = "cuda:0", order: str = "none", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1401_4350_b200 needs a CUDA device (no CPU fallback)")
+        self.torch = torch
+        self.lib = load_library()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.N = int(N)
+        self.box = np.ascontiguousarray(box, dtype=np.float64)
+        self.rcut, self.skin = float(rcut), float(skin)
+        self.pot = make_potential(potential)
+        self.rigid = potential["kind"] == "patchy"
+        self.max_neigh = int(max_neigh)
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        nbytes = C.c_size_t(0)
+        boxp = self.box.ctypes.data_as(C.POINTER(C.c_double))
+        rc = self.lib.md_workspace_bytes(self.N, boxp, self.rcut, self.skin, C.byref(self.pot), self.max_neigh,
+                                         C.byref(nbytes))
+        if rc != 0:
+            raise MDError(rc, "md_workspace_bytes: invalid parameters")
+        self.workspace_bytes = int(nbytes.value)
+        self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        self._ws_ptr = (base + 255) // 256 * 256
+        h = C.c_void_p(None)
+        rc = self.lib.md_create(C.byref(h), self.N, boxp, self.rcut, self.skin, C.byref(self.pot), self.max_neigh,
+                                C.c_void_p(self._ws_ptr), self.workspace_bytes, C.c_void_p(self._stream.cuda_stream))
+        if rc != 0:
+            raise MDError(rc, "md_create failed (invalid geometry / parameters)")
+        self.h = h
+        z = lambda: torch.zeros((self.N, 4), dtype=torch.float32, device=self.device)
+        self.pos, self.vel, self.force = z(), z(), z()
+        self.quat = self.angmom = self.torque = None
+        if self.rigid:
+            self.quat, self.angmom, self.torque = z(), z(), z()
+            self.quat[:, 0] = 1.0
+        self._check(self.lib.md_bind_state(self.h, *[C.c_void_p(t.data_ptr()) if t is not None else None for t in
+                                                    (self.pos, self.vel, self.force, self.quat, self.angmom,
+                                                     self.torque)]))
+        if order != "none":
+            self.set_order(order)
+
+    # ---- plumbing ----
+    def _check(self, rc: int):
+        if rc != 0:
+            raise MDError(rc, self.lib.md_last_error(self.h).decode())
+
+    def close(self):
+        if getattr(self, "h", None) is not None and self.h:
+            self.torch.cuda.synchronize(self.device)
+            self.lib.md_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @classmethod
+    def from_workload(cls, w, device="cuda:0", order="none", max_neigh=None):
+        s = cls(w.N, w.box, w.rcut, w.skin, w.potential, max_neigh or w.max_neigh, device=device, order=order)
+        s.set_state(w.pos, w.vel, w.quat, w.angmom)
+        return s
+
+    def set_state(self, pos, vel=None, quat=None, angmom=None):
+        """Upload state given in ORIGINAL id order (resets the slot map: call build_cells afterwards)."""
+        t = self.torch
+        up = lambda a: t.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(self.device)
+        self.pos.copy_(up(pos))
+        if vel is not None:
+            self.vel.copy_(up(vel))
+        if self.rigid and quat is not None:
+            self.quat.copy_(up(quat))
+        if self.rigid and angmom is not None:
+            self.angmom.copy_(up(angmom))
+        # a fresh bind resets the validity flags; slot map is identity only for a new handle or order none
+        self._check(self.lib.md_bind_state(self.h, *[C.c_void_p(x.data_ptr()) if x is not None else None for x in
+                                                    (self.pos, self.vel, self.force, self.quat, self.angmom,
+                                                     self.torque)]))
+
+    # ---- the C ABI, same names ----
+    def set_order(self, order):
+        self._check(self.lib.md_set_order(self.h, ORDER[order] if isinstance(order, str) else int(order)))
+
+    def build_cells(self):
+        self._check(self.lib.md_build_cells(self.h))
+
+    def build_verlet(self):
+        self._check(self.lib.md_build_verlet(self.h))
+
+    def forces(self, strategy="vertex", scatter="red_v4"):
+        self._check(self.lib.md_forces(self.h, STRATEGY[strategy], SCATTER[scatter]))
+
+    def integrate(self, dt, nsteps, strategy="vertex", scatter="red_v4"):
+        self._check(self.lib.md_integrate(self.h, float(dt), int(nsteps), STRATEGY[strategy], SCATTER[scatter]))
+
+    def energy(self):
+        u, kt, kr = C.c_double(0), C.c_double(0), C.c_double(0)
+        self._check(self.lib.md_energy(self.h, C.byref(u), C.byref(kt), C.byref(kr)))
+        return u.value, kt.value, kr.value
+
+    def stats(self):
+        ne, nf, nr = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        mx = C.c_int32(0)
+        self._check(self.lib.md_stats(self.h, C.byref(ne), C.byref(nf), C.byref(mx), C.byref(nr)))
+        return dict(n_edges=ne.value, n_full_entries=nf.value, max_neigh_seen=mx.value, n_rebuilds=nr.value)
+
+    def get_pairs(self) -> np.ndarray:
+        """Half list as ORIGINAL-id pairs (lo, hi), int32 [E,2], unsorted."""
+        n = C.c_int64(0)
+        self._check(self.lib.md_get_pairs(self.h, None, 0, C.byref(n)))
+        out = np.empty((max(int(n.value), 1), 2), dtype=np.int32)
+        self._check(self.lib.md_get_pairs(self.h, out.ctypes.data_as(C.POINTER(C.c_int32)), int(n.value), C.byref(n)))
+        return out[:int(n.value)]
+
+    def get_ids(self) -> np.ndarray:
+        ids = np.empty(self.N, dtype=np.int32)
+        self._check(self.lib.md_get_ids(self.h, ids.ctypes.data_as(C.POINTER(C.c_int32))))
+        return ids
+
+    def step_host(self, pos, vel, force, dt, nsteps, strategy="vertex", scatter="red_v4", quat=None, angmom=None,
+                  torque=None):
+        """End-to-end call on HOST (pinned or pageable) torch/numpy float32 [N,4] buffers, updated in place."""
+        ptr = lambda a: None if a is None else C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+        self._check(self.lib.md_step_host(self.h, ptr(pos), ptr(vel), ptr(force), ptr(quat), ptr(angmom), ptr(torque),
+                                          float(dt), int(nsteps), STRATEGY[strategy], SCATTER[scatter]))
+
+    def launch_count(self) -> int:
+        return int(self.lib.md_launch_count(self.h))
+
+    # ---- helpers (not part of the path) ----
+    def in_id_order(self, tensor) -> np.ndarray:
+        """Copy a state tensor to the host in ORIGINAL id order."""
+        ids = self.get_ids()
+        a = tensor.detach().cpu().numpy()
+        out = np.empty_like(a)
+        out[ids] = a
+        return out

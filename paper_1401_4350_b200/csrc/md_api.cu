@@ -1,0 +1,489 @@
+// md_api.cu -- the C ABI of include/md_b200.h: argument checks, workspace carving, call order, error latching.
+// Host logic only; every step of the path runs in the kernels of md_build.cu / md_forces.cu / md_integrate.cu.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <algorithm>
+#include <vector>
+#include "md_internal.cuh"
+
+namespace {
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Geometry {
+    int nc[3];
+    int64_t ncell;
+    int cap, ntiles;
+    size_t ecap;
+};
+
+// S:Q8: n_k = max(1, floor(L_k / (r_v (1 + 1e-5)))) cells per axis, width >= r_v
+bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int max_neigh, Geometry* g) {
+    if (N <= 0 || N > (1ll << 30) || !(rcut > 0) || !(skin >= 0) || max_neigh <= 0) return false;
+    double rv = rcut + skin;
+    g->ncell = 1;
+    for (int k = 0; k < 3; ++k) {
+        if (!(box[k] > 0) || box[k] < 2.0 * (rcut + 2.0 * skin)) return false;
+        int n = (int)floor(box[k] / (rv * (1.0 + 1e-5)));
+        g->nc[k] = n < 1 ? 1 : n;
+        g->ncell *= g->nc[k];
+    }
+    if (g->ncell > (1ll << 30)) return false;
+    g->cap = (max_neigh + 3) / 4 * 4;
+    g->ntiles = (int)((N + MD_TILE - 1) / MD_TILE);
+    if ((int64_t)g->ntiles * MD_TILE * g->cap >= (1ll << 31)) return false;
+    g->ecap = (size_t)N * g->cap / 2 + 64;
+    return true;
+}
+
+// carve the workspace; with base == nullptr only the size is computed
+size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> char* {
+        char* p = base ? base + off : nullptr;
+        off = align_up(off + bytes, 256);
+        return p;
+    };
+    DevBuffers b;
+    memset(&b, 0, sizeof(b));
+    const size_t Npad = (size_t)g.ntiles * MD_TILE;
+    b.ctrl = (DevCtrl*)take(sizeof(DevCtrl));
+    b.cell_of = (int*)take(4 * Npad);
+    b.cell_count = (int*)take(4 * (size_t)(g.ncell + 1));
+    b.cell_start = (int*)take(4 * (size_t)(g.ncell + 1));
+    b.cell_rank = (int*)take(4 * (size_t)g.ncell);
+    b.items_tmp = (int*)take(4 * Npad);
+    b.items = (int*)take(4 * Npad);
+    b.ids = (int*)take(4 * Npad);
+    b.ids_tmp = (int*)take(4 * Npad);
+    b.slot_of_id = (int*)take(4 * Npad);
+    b.tmp4 = (float4*)take(16 * Npad);
+    b.pos_ref = (float4*)take(16 * Npad);
+    b.nl_count = (int*)take(4 * Npad);
+    b.nl_full = (int*)take(4 * Npad * g.cap);
+    b.tile_info = (int2*)take(8 * (size_t)g.ntiles);
+    b.half_count = (int*)take(4 * Npad);
+    b.edge_off = (unsigned int*)take(4 * (Npad + 1));
+    b.edges = (int2*)take(8 * g.ecap);
+    b.in_off = (unsigned int*)take(4 * (Npad + 1));
+    b.in_edge = (unsigned int*)take(4 * g.ecap);
+    b.edge_f = (float4*)take(16 * g.ecap);
+    if (rigid) {
+        b.edge_ti = (float4*)take(16 * g.ecap);
+        b.edge_tj = (float4*)take(16 * g.ecap);
+    }
+    size_t nscan = (std::max<size_t>(Npad, (size_t)g.ncell + 1) + 4095) / 4096 + 8;
+    b.scan_blk = (unsigned int*)take(4 * nscan);
+    b.e_part = (double*)take(8 * 3 * 2048);
+    b.e_out = (double*)take(8 * 4);
+    b.stage4 = (float4*)take(16 * Npad);
+    if (B) *B = b;
+    return off;
+}
+
+bool check_pot(const md_potential* p, double rcut) {
+    if (!p) return false;
+    if (p->kind < MD_POT_LJ || p->kind > MD_POT_PATCHY) return false;
+    if (!(p->epsilon > 0) || !(p->sigma > 0) || !(p->mass > 0)) return false;
+    if (p->kind == MD_POT_FENE_WCA && (p->chain_len < 1 || !(p->fene_K > 0) || !(p->fene_R0 > 0))) return false;
+    if (p->kind == MD_POT_PATCHY) {
+        if (p->n_patches < 1 || p->n_patches > MD_MAX_PATCH) return false;
+        if (!(p->inertia > 0) || !(p->patch_sigma_r > 0) || !(p->patch_sigma_ang > 0) || !(p->rcut_core > 0)) return false;
+        if (p->rcut_core > rcut) return false;
+        for (int a = 0; a < p->n_patches; ++a) {
+            double n2 = 0;
+            for (int k = 0; k < 3; ++k) n2 += (double)p->patch_dir[a][k] * p->patch_dir[a][k];
+            if (fabs(n2 - 1.0) > 1e-4) return false;   // S:8(b): non-unit patch vectors are invalid
+        }
+    }
+    return true;
+}
+
+// 3-D Hilbert index of cell (x,y,z) on a 2^bits grid ("8-vertex Hilbert curve" = 2x2x2 recursion).
+// Skilling's transpose construction ("Programming the Hilbert curve", AIP Conf. Proc. 707, 2004), restated.
+uint64_t hilbert3(uint32_t x, uint32_t y, uint32_t z, int bits) {
+    uint32_t X[3] = { x, y, z };
+    const uint32_t M = 1u << (bits - 1);
+    for (uint32_t Q = M; Q > 1; Q >>= 1) {          // inverse undo excess work
+        uint32_t Pm = Q - 1;
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) X[0] ^= Pm;
+            else { uint32_t t = (X[0] ^ X[i]) & Pm; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    for (int i = 1; i < 3; ++i) X[i] ^= X[i - 1];   // Gray encode
+    uint32_t t = 0;
+    for (uint32_t Q = M; Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
+    for (int i = 0; i < 3; ++i) X[i] ^= t;
+    uint64_t h = 0;                                  // interleave the transposed bits, X[0] most significant
+    for (int b = bits - 1; b >= 0; --b)
+        for (int i = 0; i < 3; ++i) h = (h << 1) | ((X[i] >> b) & 1u);
+    return h;
+}
+
+void make_cell_rank(const int nc[3], int order, std::vector<int>& rank) {
+    const int64_t ncell = (int64_t)nc[0] * nc[1] * nc[2];
+    rank.resize((size_t)ncell);
+    if (order != MD_ORDER_HILBERT) {
+        for (int64_t c = 0; c < ncell; ++c) rank[(size_t)c] = (int)c;
+        return;
+    }
+    int bits = 1;
+    while ((1 << bits) < std::max(nc[0], std::max(nc[1], nc[2]))) ++bits;
+    std::vector<std::pair<uint64_t, int>> keys((size_t)ncell);
+    for (int x = 0; x < nc[0]; ++x)
+        for (int y = 0; y < nc[1]; ++y)
+            for (int z = 0; z < nc[2]; ++z) {
+                int lin = (x * nc[1] + y) * nc[2] + z;
+                keys[(size_t)lin] = { hilbert3((uint32_t)x, (uint32_t)y, (uint32_t)z, bits), lin };
+            }
+    std::sort(keys.begin(), keys.end());
+    for (int64_t r = 0; r < ncell; ++r) rank[(size_t)keys[(size_t)r].second] = (int)r;
+}
+
+md_status fail(md_system* s, md_status code, const char* msg) {
+    if (s) snprintf(s->errmsg, sizeof(s->errmsg), "%s", msg);
+    return code;
+}
+
+md_status check_cuda(md_system* s, const char* where) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(s->errmsg, sizeof(s->errmsg), "CUDA error at %s: %s", where, cudaGetErrorString(e));
+        s->sticky = MD_ERR_CUDA;
+        return MD_ERR_CUDA;
+    }
+    return MD_OK;
+}
+
+// slot s holds original id s (state arrays given in original id order)
+void reset_ids(md_system* s) {
+    std::vector<int> iden((size_t)s->N);
+    for (int64_t i = 0; i < s->N; ++i) iden[(size_t)i] = (int)i;
+    cudaMemcpyAsync(s->B.ids, iden.data(), 4 * (size_t)s->N, cudaMemcpyHostToDevice, s->stream);
+    cudaMemcpyAsync(s->B.slot_of_id, iden.data(), 4 * (size_t)s->N, cudaMemcpyHostToDevice, s->stream);
+    cudaStreamSynchronize(s->stream);   // iden is a host temporary
+}
+
+// synchronise and surface latched device errors
+md_status sync_and_check(md_system* s, const char* where) {
+    DevCtrl c;
+    cudaError_t e = cudaMemcpyAsync(&c, s->B.ctrl, sizeof(c), cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) {
+        snprintf(s->errmsg, sizeof(s->errmsg), "CUDA error at %s: %s", where, cudaGetErrorString(e));
+        s->sticky = MD_ERR_CUDA;
+        return MD_ERR_CUDA;
+    }
+    if (c.err & MD_DEVERR_CAPACITY) {
+        snprintf(s->errmsg, sizeof(s->errmsg), "neighbour capacity exceeded: a particle has %d Verlet neighbours, max_neigh = %d", c.max_seen, s->P.cap);
+        s->lists_valid = false;
+        return MD_ERR_CAPACITY;
+    }
+    if (c.err & MD_DEVERR_FENE) {
+        snprintf(s->errmsg, sizeof(s->errmsg), "FENE bond length reached R0");
+        return MD_ERR_NUMERIC;
+    }
+    return MD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+md_status md_workspace_bytes(int64_t N, const double box[3], double rcut, double skin, const md_potential* pot,
+                             int32_t max_neigh, size_t* bytes) {
+    Geometry g;
+    if (!bytes || !box || !check_pot(pot, rcut) || !make_geometry(N, box, rcut, skin, max_neigh, &g)) return MD_ERR_INVALID;
+    *bytes = carve(nullptr, N, g, pot->kind == MD_POT_PATCHY, nullptr);
+    return MD_OK;
+}
+
+md_status md_create(md_system** out, int64_t N, const double box[3], double rcut, double skin, const md_potential* pot,
+                    int32_t max_neigh, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!out) return MD_ERR_INVALID;
+    *out = nullptr;
+    Geometry g;
+    if (!box || !check_pot(pot, rcut) || !make_geometry(N, box, rcut, skin, max_neigh, &g)) return MD_ERR_INVALID;
+    const bool rigid = pot->kind == MD_POT_PATCHY;
+    size_t need = carve(nullptr, N, g, rigid, nullptr);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return MD_ERR_INVALID;
+
+    md_system* s = (md_system*)calloc(1, sizeof(md_system));
+    if (!s) return MD_ERR_INVALID;
+    s->N = N;
+    s->stream = (cudaStream_t)cuda_stream;
+    s->rcut = rcut; s->skin = skin;
+    s->pot = *pot;
+    s->rigid = rigid;
+    s->order = MD_ORDER_NONE;
+    s->workspace = workspace; s->workspace_bytes = workspace_bytes;
+    s->ecap = g.ecap;
+    carve((char*)workspace, N, g, rigid, &s->B);
+
+    DevParams& P = s->P;
+    P.N = (int)N; P.ntiles = g.ntiles; P.cap = g.cap; P.capg = g.cap / 4;
+    P.dLx = box[0]; P.dLy = box[1]; P.dLz = box[2];
+    P.Lx = (float)box[0]; P.Ly = (float)box[1]; P.Lz = (float)box[2];
+    P.hLx = 0.5f * P.Lx; P.hLy = 0.5f * P.Ly; P.hLz = 0.5f * P.Lz;
+    const double rv = rcut + skin;
+    P.rv2d = rv * rv;
+    P.rc2d = rcut * rcut;
+    P.ncx = g.nc[0]; P.ncy = g.nc[1]; P.ncz = g.nc[2]; P.ncell = (int)g.ncell;
+    P.cscale_x = g.nc[0] / box[0]; P.cscale_y = g.nc[1] / box[1]; P.cscale_z = g.nc[2] / box[2];
+    P.rc2 = (float)P.rc2d;
+    P.rc2_lo = (float)(P.rc2d * (1.0 - 1e-6));   // S:H10 band; the fp32 d2 is accurate to ~3e-7 relative
+    P.rc2_hi = (float)(P.rc2d * (1.0 + 1e-6));
+    P.half_skin2 = (float)(0.25 * skin * skin);
+    P.kind = pot->kind;
+    P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
+    P.sigma = pot->sigma;
+    P.c48 = 48.0f * pot->epsilon; P.c24 = 24.0f * pot->epsilon; P.c4 = 4.0f * pot->epsilon;
+    {
+        double s2 = (double)pot->sigma * pot->sigma / (rcut * rcut), s6 = s2 * s2 * s2;
+        double vc = 4.0 * pot->epsilon * s6 * (s6 - 1.0);
+        bool shift = pot->shift_energy != 0 || pot->kind == MD_POT_FENE_WCA;   // WCA is always shifted (B:9)
+        P.vshift = (pot->kind == MD_POT_PATCHY || !shift) ? 0.0f : (float)vc;
+    }
+    if (rigid) {
+        double rc = pot->rcut_core;
+        double s2 = (double)pot->sigma * pot->sigma / (rc * rc), s6 = s2 * s2 * s2;
+        P.core_rc2 = (float)(rc * rc);
+        P.core_vshift = (float)(4.0 * pot->epsilon * s6 * (s6 - 1.0));
+        P.n_patches = pot->n_patches;
+        for (int a = 0; a < MD_MAX_PATCH; ++a)
+            for (int k = 0; k < 3; ++k) P.pdir[a][k] = a < pot->n_patches ? pot->patch_dir[a][k] : 0.0f;
+        P.eps_patch = pot->eps_patch;
+        P.inv_sr2 = 1.0f / (pot->patch_sigma_r * pot->patch_sigma_r);
+        P.inv_2sr2 = 0.5f * P.inv_sr2;
+        P.inv_w2 = 1.0f / (pot->patch_sigma_ang * pot->patch_sigma_ang);
+        P.inv_inertia = 1.0f / pot->inertia;
+    }
+    if (pot->kind == MD_POT_FENE_WCA) {
+        P.fene_K = pot->fene_K;
+        P.fene_R02 = pot->fene_R0 * pot->fene_R0;
+        P.fene_invR02 = 1.0f / P.fene_R02;
+        P.chain_len = pot->chain_len;
+    } else {
+        P.chain_len = 1;
+    }
+
+    // device-side initial state: control block zero, ids = identity, cell rank table
+    cudaMemsetAsync(s->B.ctrl, 0, sizeof(DevCtrl), s->stream);
+    {
+        reset_ids(s);
+        std::vector<int> rank;
+        make_cell_rank(g.nc, MD_ORDER_NONE, rank);
+        cudaMemcpyAsync(s->B.cell_rank, rank.data(), 4 * rank.size(), cudaMemcpyHostToDevice, s->stream);
+        cudaStreamSynchronize(s->stream);
+    }
+    if (check_cuda(s, "md_create") != MD_OK) { free(s); return MD_ERR_CUDA; }
+    *out = s;
+    return MD_OK;
+}
+
+md_status md_bind_state(md_system* s, void* pos, void* vel, void* force, void* quat, void* angmom, void* torque) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!pos || !vel || !force) return fail(s, MD_ERR_INVALID, "md_bind_state: pos, vel and force are required");
+    if (s->rigid && (!quat || !angmom || !torque)) return fail(s, MD_ERR_INVALID, "md_bind_state: rigid bodies need quat, angmom and torque");
+    void* all[6] = { pos, vel, force, quat, angmom, torque };
+    for (int k = 0; k < 6; ++k)
+        if (all[k] && ((uintptr_t)all[k] & 15)) return fail(s, MD_ERR_INVALID, "md_bind_state: pointers must be 16-byte aligned");
+    s->pos = (float4*)pos; s->vel = (float4*)vel; s->force = (float4*)force;
+    s->quat = s->rigid ? (float4*)quat : nullptr;
+    s->angmom = s->rigid ? (float4*)angmom : nullptr;
+    s->torque = s->rigid ? (float4*)torque : nullptr;
+    s->bound = true;
+    s->cells_valid = s->lists_valid = s->forces_valid = s->seg_valid = false;
+    reset_ids(s);   // the arrays are taken to be in original id order
+    return check_cuda(s, "md_bind_state");
+}
+
+md_status md_set_order(md_system* s, int32_t order) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (order < MD_ORDER_NONE || order > MD_ORDER_HILBERT) return fail(s, MD_ERR_INVALID, "md_set_order: unknown order");
+    s->order = order;
+    std::vector<int> rank;
+    int nc[3] = { s->P.ncx, s->P.ncy, s->P.ncz };
+    make_cell_rank(nc, order, rank);
+    cudaMemcpyAsync(s->B.cell_rank, rank.data(), 4 * rank.size(), cudaMemcpyHostToDevice, s->stream);
+    cudaStreamSynchronize(s->stream);   // rank is a host temporary
+    s->cells_valid = s->lists_valid = s->seg_valid = false;
+    return check_cuda(s, "md_set_order");
+}
+
+md_status md_build_cells(md_system* s) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->bound) return fail(s, MD_ERR_STATE, "md_build_cells: no state bound");
+    md_launch_build_cells(s, false);
+    s->cells_valid = true;
+    s->lists_valid = s->seg_valid = false;
+    return check_cuda(s, "md_build_cells");
+}
+
+md_status md_build_verlet(md_system* s) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->bound || !s->cells_valid) return fail(s, MD_ERR_STATE, "md_build_verlet: call md_build_cells first");
+    md_launch_build_verlet(s, false);
+    md_launch_build_end(s, false);
+    s->lists_valid = true;
+    s->seg_valid = false;
+    s->cells_valid = false;   // cells describe the positions at build time only
+    return check_cuda(s, "md_build_verlet");
+}
+
+static md_status check_strategy(md_system* s, int32_t strategy, int32_t scatter) {
+    if (strategy != MD_VERTEX && strategy != MD_EDGE) return fail(s, MD_ERR_INVALID, "unknown strategy");
+    if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_SEGMENTED)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
+    return MD_OK;
+}
+
+md_status md_forces(md_system* s, int32_t strategy, int32_t scatter) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->bound || !s->lists_valid) return fail(s, MD_ERR_STATE, "md_forces: lists are not built (md_build_cells, md_build_verlet)");
+    md_status st = check_strategy(s, strategy, scatter);
+    if (st != MD_OK) return st;
+    if (strategy == MD_EDGE && scatter == MD_SCATTER_SEGMENTED && !s->seg_valid) {
+        md_launch_seg_index(s, false);
+        s->seg_valid = true;
+    }
+    md_launch_forces(s, strategy, scatter);
+    s->forces_valid = true;
+    return check_cuda(s, "md_forces");
+}
+
+md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy, int32_t scatter) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->bound || !s->lists_valid || !s->forces_valid) return fail(s, MD_ERR_STATE, "md_integrate: needs built lists and valid forces on entry");
+    if (!(dt > 0) || nsteps < 0) return fail(s, MD_ERR_INVALID, "md_integrate: dt > 0 and nsteps >= 0 required");
+    md_status st = check_strategy(s, strategy, scatter);
+    if (st != MD_OK) return st;
+    const bool seg = strategy == MD_EDGE && scatter == MD_SCATTER_SEGMENTED;
+    if (seg && !s->seg_valid) { md_launch_seg_index(s, false); s->seg_valid = true; }
+    const float fdt = (float)dt;
+    for (int64_t k = 0; k < nsteps; ++k) {
+        md_launch_kick_drift(s, fdt);            // sets the device rebuild flag (S:A5)
+        md_launch_build_cells(s, true);          // gated on the flag: no host synchronisation (S:H6)
+        md_launch_build_verlet(s, true);
+        if (seg) md_launch_seg_index(s, true);
+        md_launch_build_end(s, true);
+        md_launch_forces(s, strategy, scatter);
+        md_launch_kick(s, fdt);
+    }
+    if (!seg) s->seg_valid = false;   // a device-side rebuild may have happened without the index
+    return check_cuda(s, "md_integrate");
+}
+
+md_status md_energy(md_system* s, double* e_pot, double* e_kin_trans, double* e_kin_rot) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->bound || !s->forces_valid) return fail(s, MD_ERR_STATE, "md_energy: needs valid forces (md_forces)");
+    md_launch_energy(s);
+    double e[3];
+    cudaMemcpyAsync(e, s->B.e_out, sizeof(e), cudaMemcpyDeviceToHost, s->stream);
+    md_status st = sync_and_check(s, "md_energy");
+    if (st != MD_OK) return st;
+    if (e_pot) *e_pot = e[0];
+    if (e_kin_trans) *e_kin_trans = e[1];
+    if (e_kin_rot) *e_kin_rot = s->rigid ? e[2] : 0.0;
+    return MD_OK;
+}
+
+md_status md_stats(md_system* s, int64_t* n_edges, int64_t* n_full_entries, int32_t* max_neigh_seen, int64_t* n_rebuilds) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    DevCtrl c;
+    cudaMemcpyAsync(&c, s->B.ctrl, sizeof(c), cudaMemcpyDeviceToHost, s->stream);
+    md_status st = sync_and_check(s, "md_stats");
+    if (n_edges) *n_edges = c.n_edges;
+    if (n_full_entries) *n_full_entries = (int64_t)c.n_full;
+    if (max_neigh_seen) *max_neigh_seen = c.max_seen;
+    if (n_rebuilds) *n_rebuilds = c.n_rebuilds;
+    return st;
+}
+
+md_status md_get_ids(md_system* s, int32_t* ids_host) {
+    if (!s || !ids_host) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    cudaMemcpyAsync(ids_host, s->B.ids, 4 * (size_t)s->N, cudaMemcpyDeviceToHost, s->stream);
+    cudaStreamSynchronize(s->stream);
+    return check_cuda(s, "md_get_ids");
+}
+
+md_status md_get_pairs(md_system* s, int32_t* pairs_host, int64_t capacity, int64_t* n) {
+    if (!s || !n) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->lists_valid) return fail(s, MD_ERR_STATE, "md_get_pairs: lists are not built");
+    DevCtrl c;
+    cudaMemcpyAsync(&c, s->B.ctrl, sizeof(c), cudaMemcpyDeviceToHost, s->stream);
+    md_status st = sync_and_check(s, "md_get_pairs");
+    if (st != MD_OK) return st;
+    *n = c.n_edges;
+    int64_t m = std::min<int64_t>(capacity, c.n_edges);
+    if (m <= 0 || !pairs_host) return MD_OK;
+    std::vector<int> ids((size_t)s->N);
+    cudaMemcpyAsync(ids.data(), s->B.ids, 4 * (size_t)s->N, cudaMemcpyDeviceToHost, s->stream);
+    cudaMemcpyAsync(pairs_host, s->B.edges, 8 * (size_t)m, cudaMemcpyDeviceToHost, s->stream);
+    cudaStreamSynchronize(s->stream);
+    for (int64_t e = 0; e < m; ++e) {   // slots -> original ids, (lo, hi); drop the image flag
+        int a = ids[(size_t)pairs_host[2 * e]];
+        int b = ids[(size_t)(pairs_host[2 * e + 1] & 0x7fffffff)];
+        pairs_host[2 * e] = a < b ? a : b;
+        pairs_host[2 * e + 1] = a < b ? b : a;
+    }
+    return check_cuda(s, "md_get_pairs");
+}
+
+md_status md_step_host(md_system* s, void* pos_host, void* vel_host, void* force_host, void* quat_host, void* angmom_host,
+                       void* torque_host, double dt, int64_t nsteps, int32_t strategy, int32_t scatter) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->bound) return fail(s, MD_ERR_STATE, "md_step_host: no state bound");
+    if (!pos_host || !vel_host || !force_host) return fail(s, MD_ERR_INVALID, "md_step_host: pos, vel, force host buffers required");
+    if (s->rigid && (!quat_host || !angmom_host || !torque_host)) return fail(s, MD_ERR_INVALID, "md_step_host: rigid bodies need quat, angmom, torque");
+    md_status st = check_strategy(s, strategy, scatter);
+    if (st != MD_OK) return st;
+    const size_t bytes = 16 * (size_t)s->N;
+    reset_ids(s);   // host buffers are in ORIGINAL id order
+    cudaMemcpyAsync(s->pos, pos_host, bytes, cudaMemcpyHostToDevice, s->stream);
+    cudaMemcpyAsync(s->vel, vel_host, bytes, cudaMemcpyHostToDevice, s->stream);
+    if (s->rigid) {
+        cudaMemcpyAsync(s->quat, quat_host, bytes, cudaMemcpyHostToDevice, s->stream);
+        cudaMemcpyAsync(s->angmom, angmom_host, bytes, cudaMemcpyHostToDevice, s->stream);
+    }
+    if ((st = md_build_cells(s)) != MD_OK) return st;
+    if ((st = md_build_verlet(s)) != MD_OK) return st;
+    if ((st = md_forces(s, strategy, scatter)) != MD_OK) return st;
+    if (nsteps > 0 && (st = md_integrate(s, dt, nsteps, strategy, scatter)) != MD_OK) return st;
+    struct { float4* dev; void* host; } outs[6] = { { s->pos, pos_host }, { s->vel, vel_host }, { s->force, force_host },
+                                                    { s->quat, quat_host }, { s->angmom, angmom_host }, { s->torque, torque_host } };
+    for (int k = 0; k < 6; ++k) {
+        if (!outs[k].dev || !outs[k].host) continue;
+        if (s->order == MD_ORDER_NONE) {
+            cudaMemcpyAsync(outs[k].host, outs[k].dev, bytes, cudaMemcpyDeviceToHost, s->stream);
+        } else {
+            md_launch_unpermute(s, outs[k].dev, s->B.stage4);
+            cudaMemcpyAsync(outs[k].host, s->B.stage4, bytes, cudaMemcpyDeviceToHost, s->stream);
+        }
+    }
+    return sync_and_check(s, "md_step_host");
+}
+
+int64_t md_launch_count(const md_system* s) { return s ? s->launches : 0; }
+
+const char* md_last_error(const md_system* s) { return s ? s->errmsg : "null handle"; }
+
+void md_destroy(md_system* s) {
+    if (!s) return;
+    free(s);
+}
+
+}  // extern "C"

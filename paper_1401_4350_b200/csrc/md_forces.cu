@@ -1,0 +1,516 @@
+// md_forces.cu -- the two thread mappings of arXiv 1401.4350 for the short-range force/torque evaluation.
+//   VERTEX: one thread per particle i loops over its Verlet list L_i, accumulates F_i (tau_i, pe_i)
+//                  in registers, one 128-bit store per output array; every pair evaluated twice; no atomics.
+//   EDGE: one thread per unordered pair of the list, the pair function evaluated once,
+//                  F_ij = -F_ji scattered to both particles only when the pair is inside the cutoff
+//                  ("only if the force is actually non-zero").  Four scatter paths (B:5, S:A7).
+// fp32 arithmetic; the in-cutoff decision is the fp64 predicate of S:O0/S:Q5, taken in fp32 with an fp64
+// recheck inside a relative band of 1e-6 around r_c^2 (S:H10), so it always equals the oracle's decision.
+#include <stdio.h>
+#include "md_internal.cuh"
+
+static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ------------------------------------------------------------------------------------------------
+// small device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ void red_add_v4(float4* addr, float a, float b, float c, float d) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+__device__ __forceinline__ void red_add_f32(float* addr, float a) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
+}
+__device__ __forceinline__ float4 ldg4(const float4* p) { return __ldg(p); }
+
+// S:H9 robust fp32 minimum image: subtract L from the larger coordinate before differencing (both inner
+// subtractions are exact), used only by warps that hold a pair crossing a periodic face.
+__device__ __forceinline__ float min_image(float xj, float xi, float L, float hL) {
+    float t = xj - xi;
+    if (t > hL) t = (xj - L) - xi;
+    else if (t < -hL) t = xj - (xi - L);
+    return t;
+}
+
+// S:O0 / S:Q5 predicate in fp64, fixed operation order, no FMA contraction.
+__device__ __noinline__ bool inside_fp64(float4 xi, float4 xj, double Lx, double Ly, double Lz, double thr2) {
+    double dx = (double)xj.x - (double)xi.x;
+    if (dx > 0.5 * Lx) dx -= Lx; else if (dx < -0.5 * Lx) dx += Lx;
+    double dy = (double)xj.y - (double)xi.y;
+    if (dy > 0.5 * Ly) dy -= Ly; else if (dy < -0.5 * Ly) dy += Ly;
+    double dz = (double)xj.z - (double)xi.z;
+    if (dz > 0.5 * Lz) dz -= Lz; else if (dz < -0.5 * Lz) dz += Lz;
+    double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    return d2 < thr2;
+}
+
+// in-cutoff decision: fp32 away from the threshold, fp64 inside the band
+__device__ __forceinline__ bool in_cutoff(const DevParams& P, float d2, float4 xi, float4 xj) {
+    bool in = d2 < P.rc2;
+    if (d2 > P.rc2_lo && d2 < P.rc2_hi) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rc2d);
+    return in;
+}
+
+// ------------------------------------------------------------------------------------------------
+// pair functions.  d = r_j - r_i (minimum image).  They return the force ON j:  F_j = g*d (+ ...),
+// F_i = -F_j, and the pair energy V; the callers split V in halves (S:O1).
+// ------------------------------------------------------------------------------------------------
+// O1 Eq.(1), cut + energy shift P:99;  O2 WCA is the same with rc = 2^(1/6) sigma, V_c = -eps.
+__device__ __forceinline__ void lj_pair(const DevParams& P, float d2, float& g, float& V) {
+    float inv = rcp_approx(d2);
+    float s2 = P.sig2 * inv;
+    float s6 = s2 * s2 * s2;
+    g = inv * s6 * fmaf(P.c48, s6, -P.c24);          // 24 eps s6 (2 s6 - 1) / d2
+    V = fmaf(s6, fmaf(P.c4, s6, -P.c4), -P.vshift);   // 4 eps s6 (s6 - 1) - V_c
+}
+
+struct Rot { float m[3][3]; };
+__device__ __forceinline__ Rot quat_to_rot(float4 q) {   // q = (w,x,y,z) stored as (.x,.y,.z,.w) = (w,x,y,z)
+    float w = q.x, x = q.y, y = q.z, z = q.w;
+    Rot R;
+    R.m[0][0] = 1.f - 2.f * (y * y + z * z); R.m[0][1] = 2.f * (x * y - w * z);       R.m[0][2] = 2.f * (x * z + w * y);
+    R.m[1][0] = 2.f * (x * y + w * z);       R.m[1][1] = 1.f - 2.f * (x * x + z * z); R.m[1][2] = 2.f * (y * z - w * x);
+    R.m[2][0] = 2.f * (x * z - w * y);       R.m[2][1] = 2.f * (y * z + w * x);       R.m[2][2] = 1.f - 2.f * (x * x + y * y);
+    return R;
+}
+
+// angular factor of one particle (S:O4, factorised form): with v = R^T * dir (dir = +u for i, -u for j)
+//   A = sum_a exp((b_a.v - 1)/w^2),   S = (1/w^2) R sum_a e_a b_a
+__device__ __forceinline__ void patch_factor(const DevParams& P, float4 q, float ux, float uy, float uz,
+                                             float& A, float& Sx, float& Sy, float& Sz) {
+    Rot R = quat_to_rot(q);
+    float vx = R.m[0][0] * ux + R.m[1][0] * uy + R.m[2][0] * uz;
+    float vy = R.m[0][1] * ux + R.m[1][1] * uy + R.m[2][1] * uz;
+    float vz = R.m[0][2] * ux + R.m[1][2] * uy + R.m[2][2] * uz;
+    const float k = P.inv_w2 * 1.4426950408889634f;   // exp(x) = 2^(x log2 e)
+    float a = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
+    for (int p = 0; p < P.n_patches; ++p) {
+        float c = P.pdir[p][0] * vx + P.pdir[p][1] * vy + P.pdir[p][2] * vz;
+        float e = ex2_approx((c - 1.0f) * k);
+        a += e;
+        bx = fmaf(e, P.pdir[p][0], bx); by = fmaf(e, P.pdir[p][1], by); bz = fmaf(e, P.pdir[p][2], bz);
+    }
+    A = a;
+    Sx = P.inv_w2 * (R.m[0][0] * bx + R.m[0][1] * by + R.m[0][2] * bz);
+    Sy = P.inv_w2 * (R.m[1][0] * bx + R.m[1][1] * by + R.m[1][2] * bz);
+    Sz = P.inv_w2 * (R.m[2][0] * bx + R.m[2][1] * by + R.m[2][2] * bz);
+}
+
+// O4 (B:10): WCA core + patch term.  Outputs force on j (fx,fy,fz), V, torque on i, torque on j.
+template <bool NEED_TJ>
+__device__ __forceinline__ void patchy_pair(const DevParams& P, float dx, float dy, float dz, float d2, float4 qi, float4 qj,
+                                            float& fx, float& fy, float& fz, float& V,
+                                            float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
+    float rinv = rsqrt_approx(d2);
+    float r = d2 * rinv;
+    float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+    float Ai, Six, Siy, Siz, Aj, Sjx, Sjy, Sjz;
+    patch_factor(P, qi, ux, uy, uz, Ai, Six, Siy, Siz);
+    patch_factor(P, qj, -ux, -uy, -uz, Aj, Sjx, Sjy, Sjz);
+    float dr = r - P.sigma;
+    float G = ex2_approx(-dr * dr * P.inv_2sr2 * 1.4426950408889634f);
+    float dG = -dr * P.inv_sr2 * G;
+    float eG = P.eps_patch * G;
+    V = -eG * Ai * Aj;
+    // dA_i/dr_vec = (S_i - (S_i.u)u)/r ; dA_j/dr_vec = -(S_j - (S_j.u)u)/r
+    float siu = Six * ux + Siy * uy + Siz * uz;
+    float sju = Sjx * ux + Sjy * uy + Sjz * uz;
+    float ci = eG * Aj * rinv, cj = eG * Ai * rinv;
+    float rad = P.eps_patch * dG * Ai * Aj;
+    // dV/dr_vec = -[ rad*u + ci*(S_i - siu u) - cj*(S_j - sju u) ] ; F_j = -dV/dr_vec
+    fx = rad * ux + ci * (Six - siu * ux) - cj * (Sjx - sju * ux);
+    fy = rad * uy + ci * (Siy - siu * uy) - cj * (Sjy - sju * uy);
+    fz = rad * uz + ci * (Siz - siu * uz) - cj * (Sjz - sju * uz);
+    // tau_i = eps_p G A_j (S_i x u)
+    float ti = eG * Aj;
+    tix = ti * (Siy * uz - Siz * uy); tiy = ti * (Siz * ux - Six * uz); tiz = ti * (Six * uy - Siy * ux);
+    if (NEED_TJ) {   // tau_j = eps_p G A_i (S_j x (-u))
+        float tj = -eG * Ai;
+        tjx = tj * (Sjy * uz - Sjz * uy); tjy = tj * (Sjz * ux - Sjx * uz); tjz = tj * (Sjx * uy - Sjy * ux);
+    }
+    if (d2 < P.core_rc2) {   // WCA core (force continuous at its cut: plain fp32 test)
+        float inv = rinv * rinv;
+        float s2 = P.sig2 * inv, s6 = s2 * s2 * s2;
+        float g = inv * s6 * fmaf(P.c48, s6, -P.c24);
+        V += fmaf(s6, fmaf(P.c4, s6, -P.c4), -P.core_vshift);
+        fx = fmaf(g, dx, fx); fy = fmaf(g, dy, fy); fz = fmaf(g, dz, fz);
+    }
+}
+
+// O3 FENE (B:9): U = -1/2 K R0^2 ln(1 - d2/R0^2); force on j = -K d / (1 - d2/R0^2)
+__device__ __forceinline__ bool fene_pair(const DevParams& P, float d2, float& g, float& V) {
+    float q = 1.0f - d2 * P.fene_invR02;
+    if (!(q > 0.0f)) { g = 0.f; V = 0.f; return false; }
+    g = -P.fene_K / q;
+    V = -0.5f * P.fene_K * P.fene_R02 * __logf(q);
+    return true;
+}
+
+// FENE partners of slot i (ids id-1 and id+1 inside its chain) -> accumulates into (f, pe)
+__device__ __forceinline__ void fene_vertex(const DevParams& P, const DevBuffers& B, const float4* __restrict__ pos,
+                                            int i, float4 xi, float& fx, float& fy, float& fz, float& pe) {
+    int id = B.ids[i];
+    int m = id % P.chain_len;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        int pid = s == 0 ? id - 1 : id + 1;
+        bool ok = s == 0 ? (m != 0) : (m != P.chain_len - 1 && pid < P.N);
+        if (!ok) continue;
+        float4 xj = pos[B.slot_of_id[pid]];
+        float dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
+        float dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
+        float dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+        float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        float g, V;
+        if (!fene_pair(P, d2, g, V)) atomicOr(&B.ctrl->err, MD_DEVERR_FENE);
+        fx -= g * dx; fy -= g * dy; fz -= g * dz;   // force on i = -(force on j)
+        pe += V;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// VERTEX kernels (S:A6).  List layout: tile of 32 particles, int4 groups: entry k of lane l at
+// ((tile*capg + k/4)*32 + l)*4 + k%4  -> one coalesced 128-bit load per 4 visits.
+// ------------------------------------------------------------------------------------------------
+template <bool IMG>
+__device__ __forceinline__ void vertex_lj_visit(const DevParams& P, const float4* __restrict__ pos, float4 xi, int j, bool valid,
+                                                float& fx, float& fy, float& fz, float& pe) {
+    float4 xj = ldg4(pos + j);
+    float dx, dy, dz;
+    if (IMG) {
+        dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
+        dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
+        dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+    } else {
+        dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+    }
+    float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    bool in = in_cutoff(P, d2, xi, xj) && valid;
+    float g, V;
+    lj_pair(P, d2, g, V);
+    g = in ? g : 0.0f;
+    V = in ? V : 0.0f;
+    fx = fmaf(-g, dx, fx); fy = fmaf(-g, dy, fy); fz = fmaf(-g, dz, fz);
+    pe += V;
+}
+
+template <bool BONDS>
+__global__ void __launch_bounds__(128) k_vertex_lj(DevParams P, DevBuffers B, const float4* __restrict__ pos, float4* __restrict__ force) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31, tile = i >> 5;
+    if (tile >= P.ntiles) return;
+    const bool live = i < P.N;
+    const int cnt = live ? B.nl_count[i] : 0;
+    const int2 info = B.tile_info[tile];
+    const float4 xi = live ? pos[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const int4* __restrict__ row = reinterpret_cast<const int4*>(B.nl_full) + (size_t)tile * P.capg * MD_TILE + lane;
+    const int ngroups = (info.x + 3) >> 2;
+    const int self = live ? i : 0;   // padding entries point at a harmless address and are masked by `valid`
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f;
+    if (info.y) {
+        for (int g = 0; g < ngroups; ++g) {
+            int4 jj = row[g * MD_TILE];
+            int k = g * 4;
+            bool v0 = k < cnt, v1 = k + 1 < cnt, v2 = k + 2 < cnt, v3 = k + 3 < cnt;
+            vertex_lj_visit<true>(P, pos, xi, v0 ? jj.x : self, v0, fx, fy, fz, pe);
+            vertex_lj_visit<true>(P, pos, xi, v1 ? jj.y : self, v1, fx, fy, fz, pe);
+            vertex_lj_visit<true>(P, pos, xi, v2 ? jj.z : self, v2, fx, fy, fz, pe);
+            vertex_lj_visit<true>(P, pos, xi, v3 ? jj.w : self, v3, fx, fy, fz, pe);
+        }
+    } else {
+#pragma unroll 2
+        for (int g = 0; g < ngroups; ++g) {
+            int4 jj = row[g * MD_TILE];
+            int k = g * 4;
+            bool v0 = k < cnt, v1 = k + 1 < cnt, v2 = k + 2 < cnt, v3 = k + 3 < cnt;
+            vertex_lj_visit<false>(P, pos, xi, v0 ? jj.x : self, v0, fx, fy, fz, pe);
+            vertex_lj_visit<false>(P, pos, xi, v1 ? jj.y : self, v1, fx, fy, fz, pe);
+            vertex_lj_visit<false>(P, pos, xi, v2 ? jj.z : self, v2, fx, fy, fz, pe);
+            vertex_lj_visit<false>(P, pos, xi, v3 ? jj.w : self, v3, fx, fy, fz, pe);
+        }
+    }
+    if (!live) return;
+    pe *= 0.5f;
+    if (BONDS) {
+        float bpe = 0.f;
+        fene_vertex(P, B, pos, i, xi, fx, fy, fz, bpe);
+        pe += 0.5f * bpe;
+    }
+    force[i] = make_float4(fx, fy, fz, pe);
+}
+
+template <bool IMG>
+__device__ __forceinline__ void vertex_patchy_visit(const DevParams& P, const float4* __restrict__ pos, const float4* __restrict__ quat,
+                                                    float4 xi, float4 qi, int j, float& fx, float& fy, float& fz, float& pe,
+                                                    float& tx, float& ty, float& tz) {
+    float4 xj = ldg4(pos + j);
+    float dx, dy, dz;
+    if (IMG) {
+        dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
+        dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
+        dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+    } else {
+        dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+    }
+    float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (in_cutoff(P, d2, xi, xj)) {
+        float4 qj = ldg4(quat + j);
+        float gx, gy, gz, V, a, b, c, u, v, w;
+        patchy_pair<false>(P, dx, dy, dz, d2, qi, qj, gx, gy, gz, V, a, b, c, u, v, w);
+        fx -= gx; fy -= gy; fz -= gz;
+        tx += a; ty += b; tz += c;
+        pe += V;
+    }
+}
+
+__global__ void __launch_bounds__(128) k_vertex_patchy(DevParams P, DevBuffers B, const float4* __restrict__ pos,
+                                                       const float4* __restrict__ quat, float4* __restrict__ force,
+                                                       float4* __restrict__ torque) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31, tile = i >> 5;
+    if (i >= P.N) return;
+    const int cnt = B.nl_count[i];
+    const int2 info = B.tile_info[tile];
+    const float4 xi = pos[i], qi = quat[i];
+    const int* __restrict__ row = B.nl_full + ((size_t)tile * P.capg * MD_TILE + lane) * 4;
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
+    for (int k = 0; k < cnt; ++k) {
+        int j = row[(k >> 2) * (MD_TILE * 4) + (k & 3)];
+        if (info.y) vertex_patchy_visit<true>(P, pos, quat, xi, qi, j, fx, fy, fz, pe, tx, ty, tz);
+        else vertex_patchy_visit<false>(P, pos, quat, xi, qi, j, fx, fy, fz, pe, tx, ty, tz);
+    }
+    force[i] = make_float4(fx, fy, fz, 0.5f * pe);
+    torque[i] = make_float4(tx, ty, tz, 0.f);
+}
+
+// ------------------------------------------------------------------------------------------------
+// EDGE kernels (S:A7)
+// ------------------------------------------------------------------------------------------------
+__global__ void k_zero4(DevParams P, float4* a, float4* b) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < P.N) {
+        a[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (b) b[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+// evaluate one edge: returns true if inside the cutoff; F_j = (fx,fy,fz), V full pair energy
+template <int KIND>
+__device__ __forceinline__ bool edge_eval(const DevParams& P, const float4* __restrict__ pos, const float4* __restrict__ quat,
+                                          int i, int jw, float& fx, float& fy, float& fz, float& V,
+                                          float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
+    const int j = jw & 0x7fffffff;
+    float4 xi = ldg4(pos + i), xj = ldg4(pos + j);
+    float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
+    if (jw < 0) {   // the pair crosses a periodic face (flag set at build time)
+        dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
+        dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
+        dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+    }
+    float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (!in_cutoff(P, d2, xi, xj)) return false;
+    if (KIND == MD_POT_PATCHY) {
+        float4 qi = ldg4(quat + i), qj = ldg4(quat + j);
+        patchy_pair<true>(P, dx, dy, dz, d2, qi, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
+    } else {
+        float g;
+        lj_pair(P, d2, g, V);
+        fx = g * dx; fy = g * dy; fz = g * dz;
+    }
+    return true;
+}
+
+// (a) red.global.add.f32 per component / (b) red.global.add.v4.f32 per particle and array
+template <int KIND, bool V4>
+__global__ void __launch_bounds__(256) k_edge_red(DevParams P, DevBuffers B, const float4* __restrict__ pos,
+                                                  const float4* __restrict__ quat, float4* force, float4* torque) {
+    const unsigned int E = B.ctrl->n_edges;
+    const unsigned int stride = gridDim.x * blockDim.x;
+    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < E; e += stride) {
+        int2 ij = B.edges[e];
+        float fx, fy, fz, V, tix = 0.f, tiy = 0.f, tiz = 0.f, tjx = 0.f, tjy = 0.f, tjz = 0.f;
+        if (!edge_eval<KIND>(P, pos, quat, ij.x, ij.y, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz)) continue;
+        const int j = ij.y & 0x7fffffff;
+        const float hV = 0.5f * V;
+        if (V4) {
+            red_add_v4(force + ij.x, -fx, -fy, -fz, hV);
+            red_add_v4(force + j, fx, fy, fz, hV);
+            if (KIND == MD_POT_PATCHY) {
+                red_add_v4(torque + ij.x, tix, tiy, tiz, 0.f);
+                red_add_v4(torque + j, tjx, tjy, tjz, 0.f);
+            }
+        } else {
+            float* fi = reinterpret_cast<float*>(force + ij.x);
+            float* fj = reinterpret_cast<float*>(force + j);
+            red_add_f32(fi + 0, -fx); red_add_f32(fi + 1, -fy); red_add_f32(fi + 2, -fz); red_add_f32(fi + 3, hV);
+            red_add_f32(fj + 0, fx);  red_add_f32(fj + 1, fy);  red_add_f32(fj + 2, fz);  red_add_f32(fj + 3, hV);
+            if (KIND == MD_POT_PATCHY) {
+                float* ti = reinterpret_cast<float*>(torque + ij.x);
+                float* tj = reinterpret_cast<float*>(torque + j);
+                red_add_f32(ti + 0, tix); red_add_f32(ti + 1, tiy); red_add_f32(ti + 2, tiz);
+                red_add_f32(tj + 0, tjx); red_add_f32(tj + 1, tjy); red_add_f32(tj + 2, tjz);
+            }
+        }
+    }
+}
+
+// (c) warp-aggregated by the owning particle: SLICE lanes walk the half row of particle i (edges sorted by
+// i), keep the i-side sum in registers, combine it with __shfl_xor and issue ONE red per particle and array;
+// the j side is scattered with red.v4.
+#define EDGE_SLICE 8
+template <int KIND>
+__global__ void __launch_bounds__(256) k_edge_warp(DevParams P, DevBuffers B, const float4* __restrict__ pos,
+                                                   const float4* __restrict__ quat, float4* force, float4* torque) {
+    const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int sl = threadIdx.x & (EDGE_SLICE - 1);
+    const int per_warp = 32 / EDGE_SLICE;
+    const int nslices = (gridDim.x * blockDim.x) / EDGE_SLICE;
+    // warp-uniform outer loop (the shuffles below need all 32 lanes); each aligned group of EDGE_SLICE lanes owns one i
+    for (int i0 = (gtid >> 5) * per_warp; i0 < P.N; i0 += nslices) {
+        const int i = i0 + ((threadIdx.x & 31) / EDGE_SLICE);
+        const bool act = i < P.N;
+        const unsigned int e0 = act ? B.edge_off[i] : 0u, e1 = act ? B.edge_off[i + 1] : 0u;
+        float ax = 0.f, ay = 0.f, az = 0.f, ape = 0.f, atx = 0.f, aty = 0.f, atz = 0.f;
+        for (unsigned int e = e0 + sl; e < e1; e += EDGE_SLICE) {
+            int2 ij = B.edges[e];
+            float fx, fy, fz, V, tix = 0.f, tiy = 0.f, tiz = 0.f, tjx = 0.f, tjy = 0.f, tjz = 0.f;
+            if (!edge_eval<KIND>(P, pos, quat, i, ij.y, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz)) continue;
+            const int j = ij.y & 0x7fffffff;
+            const float hV = 0.5f * V;
+            ax -= fx; ay -= fy; az -= fz; ape += hV;
+            red_add_v4(force + j, fx, fy, fz, hV);
+            if (KIND == MD_POT_PATCHY) {
+                atx += tix; aty += tiy; atz += tiz;
+                red_add_v4(torque + j, tjx, tjy, tjz, 0.f);
+            }
+        }
+        // slices of a warp may own different particles: reduce inside aligned groups of EDGE_SLICE lanes
+#pragma unroll
+        for (int o = EDGE_SLICE / 2; o > 0; o >>= 1) {
+            ax += __shfl_xor_sync(0xffffffffu, ax, o);
+            ay += __shfl_xor_sync(0xffffffffu, ay, o);
+            az += __shfl_xor_sync(0xffffffffu, az, o);
+            ape += __shfl_xor_sync(0xffffffffu, ape, o);
+            if (KIND == MD_POT_PATCHY) {
+                atx += __shfl_xor_sync(0xffffffffu, atx, o);
+                aty += __shfl_xor_sync(0xffffffffu, aty, o);
+                atz += __shfl_xor_sync(0xffffffffu, atz, o);
+            }
+        }
+        if (sl == 0 && e1 > e0) {   // one reduction per owning particle
+            red_add_v4(force + i, ax, ay, az, ape);
+            if (KIND == MD_POT_PATCHY) red_add_v4(torque + i, atx, aty, atz, 0.f);
+        }
+    }
+}
+
+// (d) per-edge store, then an atomic-free per-particle sum over own edges (+) and incoming edges (-)
+template <int KIND>
+__global__ void __launch_bounds__(256) k_edge_store(DevParams P, DevBuffers B, const float4* __restrict__ pos,
+                                                    const float4* __restrict__ quat) {
+    const unsigned int E = B.ctrl->n_edges;
+    const unsigned int stride = gridDim.x * blockDim.x;
+    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < E; e += stride) {
+        int2 ij = B.edges[e];
+        float fx = 0.f, fy = 0.f, fz = 0.f, V = 0.f, tix = 0.f, tiy = 0.f, tiz = 0.f, tjx = 0.f, tjy = 0.f, tjz = 0.f;
+        if (!edge_eval<KIND>(P, pos, quat, ij.x, ij.y, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz)) {
+            fx = fy = fz = V = 0.f; tix = tiy = tiz = tjx = tjy = tjz = 0.f;
+        }
+        B.edge_f[e] = make_float4(fx, fy, fz, V);
+        if (KIND == MD_POT_PATCHY) {
+            B.edge_ti[e] = make_float4(tix, tiy, tiz, 0.f);
+            B.edge_tj[e] = make_float4(tjx, tjy, tjz, 0.f);
+        }
+    }
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(128) k_edge_segsum(DevParams P, DevBuffers B, float4* __restrict__ force, float4* __restrict__ torque) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P.N) return;
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
+    for (unsigned int e = B.edge_off[p]; e < B.edge_off[p + 1]; ++e) {   // p is the first member: F_i = -F_j
+        float4 f = B.edge_f[e];
+        fx -= f.x; fy -= f.y; fz -= f.z; pe += f.w;
+        if (KIND == MD_POT_PATCHY) { float4 t = B.edge_ti[e]; tx += t.x; ty += t.y; tz += t.z; }
+    }
+    for (unsigned int t = B.in_off[p]; t < B.in_off[p + 1]; ++t) {       // p is the second member
+        unsigned int e = B.in_edge[t];
+        float4 f = B.edge_f[e];
+        fx += f.x; fy += f.y; fz += f.z; pe += f.w;
+        if (KIND == MD_POT_PATCHY) { float4 q = B.edge_tj[e]; tx += q.x; ty += q.y; tz += q.z; }
+    }
+    force[p] = make_float4(fx, fy, fz, 0.5f * pe);
+    if (KIND == MD_POT_PATCHY) torque[p] = make_float4(tx, ty, tz, 0.f);
+}
+
+// S:A8 bonded pass for EDGE (C3): one thread per static bond (id, id+1), FENE only, scatter with red.v4
+__global__ void k_edge_bonds(DevParams P, DevBuffers B, const float4* __restrict__ pos, float4* force) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= P.N - 1 || (id % P.chain_len) == P.chain_len - 1) return;
+    const int i = B.slot_of_id[id], j = B.slot_of_id[id + 1];
+    float4 xi = pos[i], xj = pos[j];
+    float dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
+    float dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
+    float dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+    float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    float g, V;
+    if (!fene_pair(P, d2, g, V)) atomicOr(&B.ctrl->err, MD_DEVERR_FENE);
+    red_add_v4(force + i, -g * dx, -g * dy, -g * dz, 0.5f * V);
+    red_add_v4(force + j, g * dx, g * dy, g * dz, 0.5f * V);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-side dispatch
+// ------------------------------------------------------------------------------------------------
+template <int KIND>
+static void launch_edge(md_system* s, int scatter) {
+    const DevParams& P = s->P;
+    const int nbN = cdiv(P.N, 256);
+    const int persistent = 148 * 8;   // 8 CTAs of 256 threads per SM, grid-stride over the device-resident edge count
+    float4* tq = KIND == MD_POT_PATCHY ? s->torque : nullptr;
+    if (scatter == MD_SCATTER_SEGMENTED) {
+        k_edge_store<KIND><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat);
+        k_edge_segsum<KIND><<<cdiv(P.N, 128), 128, 0, s->stream>>>(P, s->B, s->force, tq);
+        s->launches += 2;
+    } else {
+        k_zero4<<<nbN, 256, 0, s->stream>>>(P, s->force, tq);
+        s->launches += 1;
+        if (scatter == MD_SCATTER_RED) k_edge_red<KIND, false><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+        else if (scatter == MD_SCATTER_RED_V4) k_edge_red<KIND, true><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+        else k_edge_warp<KIND><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+        s->launches += 1;
+    }
+    if (P.kind == MD_POT_FENE_WCA) {
+        k_edge_bonds<<<nbN, 256, 0, s->stream>>>(P, s->B, s->pos, s->force);
+        s->launches += 1;
+    }
+}
+
+void md_launch_forces(md_system* s, int strategy, int scatter) {
+    const DevParams& P = s->P;
+    if (strategy == MD_VERTEX) {
+        int nb = cdiv((int64_t)P.ntiles * MD_TILE, 128);
+        if (P.kind == MD_POT_PATCHY) k_vertex_patchy<<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, s->torque);
+        else if (P.kind == MD_POT_FENE_WCA) k_vertex_lj<true><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->force);
+        else k_vertex_lj<false><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->force);
+        s->launches += 1;
+    } else {
+        if (P.kind == MD_POT_PATCHY) launch_edge<MD_POT_PATCHY>(s, scatter);
+        else launch_edge<MD_POT_LJ>(s, scatter);
+    }
+}

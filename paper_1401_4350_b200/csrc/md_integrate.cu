@@ -1,0 +1,143 @@
+// md_integrate.cu -- velocity-Verlet NVE in fp32 state (S:A10, S:O6; rigid bodies S:O7), the skin
+// criterion (S:A5, S:Q4) and the energy reduction (S:A9).
+#include <stdio.h>
+#include "md_internal.cuh"
+
+static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// first half: v += dt/2 F/m ; [L += dt/2 tau ; q <- dq (x) q] ; x += dt v ; skin check
+template <bool RIGID>
+__global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, float dt, float4* __restrict__ pos, float4* __restrict__ vel,
+                                                    const float4* __restrict__ force, float4* __restrict__ quat,
+                                                    float4* __restrict__ angmom, const float4* __restrict__ torque) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i < P.N) {
+        const float hk = 0.5f * dt * P.inv_mass;
+        float4 v = vel[i], f = force[i], x = pos[i];
+        v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z);
+        x.x = fmaf(dt, v.x, x.x); x.y = fmaf(dt, v.y, x.y); x.z = fmaf(dt, v.z, x.z);
+        vel[i] = v;
+        pos[i] = x;
+        if (RIGID) {
+            float4 L = angmom[i], t = torque[i], q = quat[i];
+            const float hd = 0.5f * dt;
+            L.x = fmaf(hd, t.x, L.x); L.y = fmaf(hd, t.y, L.y); L.z = fmaf(hd, t.z, L.z);
+            angmom[i] = L;
+            float wx = L.x * P.inv_inertia, wy = L.y * P.inv_inertia, wz = L.z * P.inv_inertia;
+            float wn = sqrtf(wx * wx + wy * wy + wz * wz);
+            if (wn > 0.0f) {   // exact free rotation of a spherical top about the space-frame axis omega (S:O7)
+                float h = 0.5f * wn * dt, sn, c;
+                sincosf(h, &sn, &c);
+                sn /= wn;
+                float a0 = c, a1 = sn * wx, a2 = sn * wy, a3 = sn * wz;
+                float q0 = q.x, q1 = q.y, q2 = q.z, q3 = q.w;   // (w,x,y,z)
+                float r0 = a0 * q0 - a1 * q1 - a2 * q2 - a3 * q3;
+                float r1 = a0 * q1 + a1 * q0 + a2 * q3 - a3 * q2;
+                float r2 = a0 * q2 - a1 * q3 + a2 * q0 + a3 * q1;
+                float r3 = a0 * q3 + a1 * q2 - a2 * q1 + a3 * q0;
+                float nrm = rsqrtf(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3);
+                quat[i] = make_float4(r0 * nrm, r1 * nrm, r2 * nrm, r3 * nrm);
+            }
+        }
+        float4 r = B.pos_ref[i];
+        float dx = x.x - r.x, dy = x.y - r.y, dz = x.z - r.z;
+        moved = (dx * dx + dy * dy + dz * dz) > P.half_skin2;   // S:Q4 strict '>'
+    }
+    if (__any_sync(0xffffffffu, moved) && (threadIdx.x & 31) == 0) B.ctrl->rebuild = 1;
+}
+
+// second half: v += dt/2 F/m ; L += dt/2 tau
+template <bool RIGID>
+__global__ void __launch_bounds__(256) k_kick(DevParams P, float dt, float4* __restrict__ vel, const float4* __restrict__ force,
+                                              float4* __restrict__ angmom, const float4* __restrict__ torque) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const float hk = 0.5f * dt * P.inv_mass;
+    float4 v = vel[i], f = force[i];
+    v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z);
+    vel[i] = v;
+    if (RIGID) {
+        float4 L = angmom[i], t = torque[i];
+        const float hd = 0.5f * dt;
+        L.x = fmaf(hd, t.x, L.x); L.y = fmaf(hd, t.y, L.y); L.z = fmaf(hd, t.z, L.z);
+        angmom[i] = L;
+    }
+}
+
+void md_launch_kick_drift(md_system* s, float dt) {
+    int nb = cdiv(s->P.N, 256);
+    if (s->rigid) k_kick_drift<true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
+    else k_kick_drift<false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
+    s->launches += 1;
+}
+
+void md_launch_kick(md_system* s, float dt) {
+    int nb = cdiv(s->P.N, 256);
+    if (s->rigid) k_kick<true><<<nb, 256, 0, s->stream>>>(s->P, dt, s->vel, s->force, s->angmom, s->torque);
+    else k_kick<false><<<nb, 256, 0, s->stream>>>(s->P, dt, s->vel, s->force, nullptr, nullptr);
+    s->launches += 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S:A9 energies: fp32 per-particle terms accumulated in fp64, two deterministic stages
+// ------------------------------------------------------------------------------------------------
+#define E_THREADS 256
+#define E_BLOCKS 1184   // 148 SMs x 8
+
+__device__ __forceinline__ double block_sum(double v, double* sh) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) sh[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (w == 0) {
+        r = lane < (blockDim.x >> 5) ? sh[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
+    }
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(E_THREADS) k_energy_partial(DevParams P, DevBuffers B, const float4* __restrict__ vel,
+                                                             const float4* __restrict__ force, const float4* __restrict__ angmom) {
+    __shared__ double sh[32];
+    double u = 0.0, kt = 0.0, kr = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
+        u += (double)force[i].w;
+        float4 v = vel[i];
+        kt += (double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z;
+        if (angmom) {
+            float4 L = angmom[i];
+            kr += (double)L.x * L.x + (double)L.y * L.y + (double)L.z * L.z;
+        }
+    }
+    u = block_sum(u, sh); kt = block_sum(kt, sh); kr = block_sum(kr, sh);
+    if (threadIdx.x == 0) {
+        B.e_part[3 * blockIdx.x + 0] = u;
+        B.e_part[3 * blockIdx.x + 1] = kt;
+        B.e_part[3 * blockIdx.x + 2] = kr;
+    }
+}
+
+__global__ void __launch_bounds__(E_THREADS) k_energy_final(DevParams P, DevBuffers B, int nblocks) {
+    __shared__ double sh[32];
+    double u = 0.0, kt = 0.0, kr = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
+        u += B.e_part[3 * b + 0]; kt += B.e_part[3 * b + 1]; kr += B.e_part[3 * b + 2];
+    }
+    u = block_sum(u, sh); kt = block_sum(kt, sh); kr = block_sum(kr, sh);
+    if (threadIdx.x == 0) {
+        B.e_out[0] = u;
+        B.e_out[1] = 0.5 * (double)P.mass * kt;
+        B.e_out[2] = 0.5 * (double)P.inv_inertia * kr;
+    }
+}
+
+void md_launch_energy(md_system* s) {
+    int nb = cdiv(s->P.N, E_THREADS);
+    if (nb > E_BLOCKS) nb = E_BLOCKS;
+    k_energy_partial<<<nb, E_THREADS, 0, s->stream>>>(s->P, s->B, s->vel, s->force, s->rigid ? s->angmom : nullptr);
+    k_energy_final<<<1, E_THREADS, 0, s->stream>>>(s->P, s->B, nb);
+    s->launches += 2;
+}
