@@ -128,6 +128,12 @@ class Oracle:
         n = self.lib.orc_pair_set(N, _f(p3), _d(box), rcut, skin, int(use_cells), out.ctypes.data_as(_ip), int(cap))
         return out[:min(n, cap)]
 
+    def pair_count(self, pos, box, rcut, skin, use_cells=True) -> int:
+        """O0: number of pairs only (E = 1/2 sum |L_i|)."""
+        p3 = self._pos3(pos)
+        box = np.ascontiguousarray(box, dtype=np.float64)
+        return int(self.lib.orc_pair_set(p3.shape[0], _f(p3), _d(box), rcut, skin, int(use_cells), None, 0))
+
     def forces(self, pos, box, pot, quat=None, use_cells=True):
         """O1-O5: returns dict(F [N,3], T [N,3] or None, pe [N], n_in_cut, bad) in fp64."""
         p3 = self._pos3(pos)

@@ -1,0 +1,236 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the same
+seeded inputs.  Bars (BASELINE.json north_star): pair sets bit-exact as sorted pair sets; forces and torques
+|dF| <= 1e-4 max|F_oracle| + 1e-6 per component; energies 1e-5 relative."""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = [("vertex", "red_v4"), ("edge", "red"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented")]
+FTOL_REL, FTOL_ABS, ETOL = 1e-4, 1e-6, 1e-5
+
+
+@pytest.fixture(scope="module")
+def MD():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1401_4350_b200 import MDSystem
+    return MDSystem
+
+
+def sorted_pairs(p):
+    return p[np.lexsort((p[:, 1], p[:, 0]))]
+
+
+def assert_pairs(s, oracle, pos, box, rcut, skin):
+    got = sorted_pairs(s.get_pairs())
+    ref = oracle.pair_set(pos, box, rcut, skin)
+    assert got.shape == ref.shape, (got.shape, ref.shape)
+    assert np.array_equal(got, ref)
+    st = s.stats()
+    assert st["n_edges"] == ref.shape[0] and st["n_full_entries"] == 2 * ref.shape[0]   # E = 1/2 sum |L_i|
+    return ref.shape[0]
+
+
+def assert_forces(s, o, rigid, ftol_scale=1.0):
+    fmax = np.abs(o["F"]).max()
+    F = s.in_id_order(s.force)
+    tol = ftol_scale * (FTOL_REL * fmax + FTOL_ABS)
+    assert np.abs(F[:, :3] - o["F"]).max() <= tol
+    # per-particle energies feed md_energy: compare the total to 1e-5 relative
+    U, Kt, Kr = s.energy()
+    Uo = o["pe"].sum()
+    assert abs(U - Uo) <= ETOL * max(abs(Uo), 1e-30) or abs(U - Uo) <= ETOL * (abs(Uo) + Kt + Kr)   # S:Q17
+    if rigid:
+        tmax = np.abs(o["T"]).max()
+        T = s.in_id_order(s.torque)
+        assert np.abs(T[:, :3] - o["T"]).max() <= ftol_scale * (FTOL_REL * tmax + FTOL_ABS)
+    return F
+
+
+CASES = {
+    "C1_lj2048": lambda: W.config("C1"),
+    "lj256_two_cells_per_axis": lambda: W.lj_fluid(256),
+    "lj16384_rc4_many_neighbours": lambda: W.lj_fluid(2 ** 14, rcut=4.0),
+    "lj4096_rc1.5_orthorhombic": lambda: W.lj_fluid(2 ** 12, rcut=1.5),
+    "dimers_lj_ragged_N": lambda: W.dimer_gas(1001, "lj"),
+    "dimers_fene": lambda: W.dimer_gas(4096, "fene_wca"),
+    "dimers_patchy": lambda: W.dimer_gas(4096, "patchy"),
+    "polymer_64x64": lambda: W.polymer_melt(64, 64),
+    "patchy4096": lambda: W.patchy_fluid(2 ** 12),
+    "tiny_16": lambda: W.dimer_gas(8, "lj"),
+}
+
+
+@pytest.mark.parametrize("order", ["none", "cell", "hilbert"])
+@pytest.mark.parametrize("case", list(CASES))
+def test_step0_parity(MD, oracle, case, order):
+    w = CASES[case]()
+    s = MD.from_workload(w, order=order)
+    s.build_cells(); s.build_verlet()
+    assert_pairs(s, oracle, w.pos, w.box, w.rcut, w.skin)
+    o = oracle.forces(w.pos, w.box, dict(w.potential), quat=w.quat)
+    assert o["bad"] == 0
+    results = {}
+    for strat, sc in VARIANTS:
+        s.forces(strat, sc)
+        results[(strat, sc)] = assert_forces(s, o, w.quat is not None)
+    # P11: the strategies agree with each other within twice the oracle tolerance
+    fmax = np.abs(o["F"]).max()
+    ref = results[("vertex", "red_v4")]
+    for k, F in results.items():
+        assert np.abs(F[:, :3] - ref[:, :3]).max() <= 2 * (FTOL_REL * fmax + FTOL_ABS)
+    # P7: Newton's third law survives fp32 accumulation
+    N = w.N
+    rms = np.sqrt((o["F"] ** 2).mean()) + 1e-30
+    assert np.abs(ref[:, :3].astype(np.float64).sum(axis=0)).max() <= 1e-6 * N * rms + 1e-4
+    s.close()
+
+
+def test_ids_are_a_permutation_and_state_follows(MD):
+    w = W.config("C1")
+    s = MD.from_workload(w, order="hilbert")
+    s.build_cells()
+    ids = s.get_ids()
+    assert np.array_equal(np.sort(ids), np.arange(w.N))
+    assert not np.array_equal(ids, np.arange(w.N))
+    assert np.array_equal(s.in_id_order(s.pos), w.pos)          # positions already in [0,L): wrap is the identity
+    assert np.array_equal(s.in_id_order(s.vel), w.vel)
+    s.close()
+
+
+def test_vertex_and_segmented_are_bitwise_reproducible(MD):
+    w = W.lj_fluid(2 ** 14)
+    out = {}
+    for rep in range(2):
+        s = MD.from_workload(w, order="cell")
+        s.build_cells(); s.build_verlet()
+        for strat, sc in [("vertex", "red_v4"), ("edge", "segmented")]:
+            s.forces(strat, sc)
+            F = s.in_id_order(s.force)
+            if rep:
+                assert np.array_equal(F, out[(strat, sc)])
+            out[(strat, sc)] = F
+        s.close()
+
+
+def test_error_paths(MD):
+    from paper_1401_4350_b200 import MDError
+    w = W.config("C1")
+    s = MD.from_workload(w)
+    with pytest.raises(MDError) as e:
+        s.forces("vertex")                      # forces before lists
+    assert e.value.code == -2
+    with pytest.raises(MDError) as e:
+        s.build_verlet()                        # verlet before cells
+    assert e.value.code == -2
+    s.build_cells(); s.build_verlet()
+    with pytest.raises(MDError) as e:
+        s.integrate(0.002, 1)                   # integrate before forces
+    assert e.value.code == -2
+    with pytest.raises(MDError) as e:
+        s.lib.md_forces(s.h, 7, 0) and None
+        s._check(s.lib.md_forces(s.h, 7, 0))    # unknown strategy
+    assert e.value.code == -1
+    s.close()
+    # capacity overflow is an error, never a silent truncation
+    s = MD.from_workload(w, max_neigh=40)
+    s.build_cells(); s.build_verlet()
+    with pytest.raises(MDError) as e:
+        s.stats()
+    assert e.value.code == -3
+    s.close()
+    # FENE bond stretched to R0
+    d = W.dimer_gas(64, "fene_wca")
+    d.pos[1, :3] = d.pos[0, :3] + np.array([1.6, 0, 0], dtype=np.float32)
+    s = MD.from_workload(d)
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    with pytest.raises(MDError) as e:
+        s.energy()
+    assert e.value.code == -5
+    s.close()
+
+
+@pytest.mark.parametrize("strat,sc", [("vertex", "red_v4"), ("edge", "warp"), ("edge", "segmented")])
+def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
+    """C1 (BASELINE.json configs[0]): 100 velocity-Verlet steps at dt = 0.002; fp32 GPU state against the fp64
+    oracle trajectory from the same fp32 input.  SURVEY 8(d): the two stay within the force tolerance for 100 steps."""
+    w = W.config("C1")
+    o = oracle.integrate(w.pos, w.vel, w.box, dict(w.potential), w.skin, w.dt, 100, every=100)
+    s = MD.from_workload(w, order="cell")
+    s.build_cells(); s.build_verlet(); s.forces(strat, sc)
+    e0 = s.energy()
+    assert abs(sum(e0) - o["e0"].sum()) <= ETOL * abs(o["e0"].sum())
+    s.integrate(w.dt, 100, strat, sc)
+    assert s.stats()["n_rebuilds"] >= 1                      # the skin criterion fired on the device
+    fmax = np.abs(o["F"]).max()
+    F = s.in_id_order(s.force)
+    assert np.abs(F[:, :3] - o["F"]).max() <= FTOL_REL * fmax + FTOL_ABS
+    x = s.in_id_order(s.pos)[:, :3].astype(np.float64)
+    dx = x - o["pos"]
+    dx -= w.box * np.round(dx / w.box)
+    assert np.abs(dx).max() < 1e-4
+    e1 = s.energy()
+    assert abs(sum(e1) - o["energies"][-1].sum()) <= ETOL * abs(o["energies"][-1].sum())
+    s.close()
+
+
+@pytest.mark.parametrize("case,steps,strat,sc", [
+    ("lj", 300, "vertex", "red_v4"), ("lj", 300, "edge", "red_v4"),
+    ("polymer", 200, "vertex", "red_v4"), ("polymer", 200, "edge", "warp"),
+    ("patchy", 300, "vertex", "red_v4"), ("patchy", 300, "edge", "segmented")])
+def test_snapshot_parity_after_device_side_rebuilds(MD, oracle, case, steps, strat, sc):
+    """Run md_integrate long enough for several skin-triggered rebuilds, then compare the forces the path holds
+    (computed from lists rebuilt on the device) with the oracle's plain definition on the SAME positions, and the
+    list of a fresh build with the oracle pair set (S:Q6: list parity on given positions, never along trajectories)."""
+    w = {"lj": lambda: W.lj_fluid(2 ** 14), "polymer": lambda: W.polymer_melt(128, 64),
+         "patchy": lambda: W.patchy_fluid(2 ** 12, T=1.0)}[case]()
+    s = MD.from_workload(w, order="hilbert")
+    s.build_cells(); s.build_verlet(); s.forces(strat, sc)
+    s.integrate(w.dt, steps, strat, sc)
+    assert s.stats()["n_rebuilds"] >= 2
+    pos = s.in_id_order(s.pos)
+    quat = s.in_id_order(s.quat) if w.quat is not None else None
+    o = oracle.forces(pos, w.box, dict(w.potential), quat=quat)
+    assert_forces(s, o, quat is not None)
+    s.build_cells(); s.build_verlet()
+    pos2 = s.in_id_order(s.pos)                               # wrapped by the build
+    assert_pairs(s, oracle, pos2, w.box, w.rcut, w.skin)
+    s.close()
+
+
+def test_nve_drift_c1_10k_steps(MD):
+    """P9 / north_star: NVE energy drift of C1 over 10^4 steps stays below 5e-5 relative."""
+    w = W.config("C1")
+    s = MD.from_workload(w, order="cell")
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    e0 = sum(s.energy())
+    worst = 0.0
+    for _ in range(20):
+        s.integrate(w.dt, 500, "vertex")
+        worst = max(worst, abs(sum(s.energy()) - e0) / abs(e0))
+    assert worst <= 5e-5
+    st = s.stats()
+    assert 300 <= st["n_rebuilds"] <= 600                     # a rebuild every ~25 steps
+    v = s.vel.double().sum(dim=0).cpu().numpy()[:3]
+    assert np.abs(v).max() < 1e-2                             # momentum stays ~0
+    s.close()
+
+
+def test_step_host_end_to_end(MD, oracle):
+    import torch
+    w = W.config("C1")
+    s = MD.from_workload(w, order="hilbert")
+    pos = torch.from_numpy(w.pos.copy()).pin_memory()
+    vel = torch.from_numpy(w.vel.copy()).pin_memory()
+    force = torch.zeros_like(pos).pin_memory()
+    s.step_host(pos, vel, force, w.dt, 0, "vertex")
+    o = oracle.forces(w.pos, w.box, dict(w.potential))
+    assert np.abs(force.numpy()[:, :3] - o["F"]).max() <= FTOL_REL * np.abs(o["F"]).max() + FTOL_ABS
+    assert np.array_equal(pos.numpy(), w.pos)
+    s.step_host(pos, vel, force, w.dt, 10, "edge", "red_v4")
+    o10 = oracle.integrate(w.pos, w.vel, w.box, dict(w.potential), w.skin, w.dt, 10)
+    assert np.abs(force.numpy()[:, :3] - o10["F"]).max() <= FTOL_REL * np.abs(o10["F"]).max() + FTOL_ABS
+    s.close()
