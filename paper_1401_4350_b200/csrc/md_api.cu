@@ -234,13 +234,17 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.ncx = g.nc[0]; P.ncy = g.nc[1]; P.ncz = g.nc[2]; P.ncell = (int)g.ncell;
     P.cscale_x = g.nc[0] / box[0]; P.cscale_y = g.nc[1] / box[1]; P.cscale_z = g.nc[2] / box[2];
     P.rc2 = (float)P.rc2d;
-    P.rc2_lo = (float)(P.rc2d * (1.0 - 1e-6));   // S:H10 band; the fp32 d2 is accurate to ~3e-7 relative
-    P.rc2_hi = (float)(P.rc2d * (1.0 + 1e-6));
+    P.band_abs = (float)(P.rc2d * 1e-6);   // S:H10 band; the fp32 d2 is accurate to ~3e-7 relative
     P.half_skin2 = (float)(0.25 * skin * skin);
     P.kind = pot->kind;
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
     P.sigma = pot->sigma;
     P.c48 = 48.0f * pot->epsilon; P.c24 = 24.0f * pot->epsilon; P.c4 = 4.0f * pot->epsilon;
+    {
+        const double s6 = pow((double)pot->sigma, 6.0), e = pot->epsilon;
+        P.lj_a = (float)(48.0 * e * s6 * s6); P.lj_b = (float)(24.0 * e * s6);
+        P.lj_c = (float)(4.0 * e * s6 * s6);  P.lj_d = (float)(4.0 * e * s6);
+    }
     {
         double s2 = (double)pot->sigma * pot->sigma / (rcut * rcut), s6 = s2 * s2 * s2;
         double vc = 4.0 * pot->epsilon * s6 * (s6 - 1.0);

@@ -290,11 +290,18 @@ __global__ void __launch_bounds__(128) k_build_verlet(DevParams P, DevBuffers B,
     }
     int c2 = cnt < P.cap ? cnt : P.cap;
     int kmax = __reduce_max_sync(0xffffffffu, c2);
+    int kmin = __reduce_min_sync(0xffffffffu, i < P.N ? c2 : 0);   // a tile with dead lanes takes the checked loop
     int tot = __reduce_add_sync(0xffffffffu, c2);
     int seen = __reduce_max_sync(0xffffffffu, cnt);
     int anyimg = __any_sync(0xffffffffu, img);
+    // pad every row of the tile up to the tile's rounded-up length with the particle's own slot (masked by the
+    // force kernels' validity test; keeps the gathers of the ragged tail in bounds)
+    if (tile < P.ntiles) {
+        const int self = i < P.N ? i : 0;
+        for (int k = c2; k < ((kmax + 3) & ~3); ++k) B.nl_full[full_index(tile, lane, k, P.capg)] = self;
+    }
     if (lane == 0 && tile < P.ntiles) {
-        B.tile_info[tile] = make_int2(kmax, anyimg);
+        B.tile_info[tile] = make_int2(kmax | (anyimg << 30), kmin);
         atomicMax(&B.ctrl->max_seen, seen);
         atomicAdd(&B.ctrl->n_full, (unsigned long long)tot);
     }

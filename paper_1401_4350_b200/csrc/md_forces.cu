@@ -60,8 +60,9 @@ __device__ __noinline__ bool inside_fp64(float4 xi, float4 xj, double Lx, double
 
 // in-cutoff decision: fp32 away from the threshold, fp64 inside the band
 __device__ __forceinline__ bool in_cutoff(const DevParams& P, float d2, float4 xi, float4 xj) {
-    bool in = d2 < P.rc2;
-    if (d2 > P.rc2_lo && d2 < P.rc2_hi) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rc2d);
+    const float t = d2 - P.rc2;
+    bool in = t < 0.0f;
+    if (fabsf(t) < P.band_abs) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rc2d);
     return in;
 }
 
@@ -72,10 +73,9 @@ __device__ __forceinline__ bool in_cutoff(const DevParams& P, float d2, float4 x
 // O1 Eq.(1), cut + energy shift P:99;  O2 WCA is the same with rc = 2^(1/6) sigma, V_c = -eps.
 __device__ __forceinline__ void lj_pair(const DevParams& P, float d2, float& g, float& V) {
     float inv = rcp_approx(d2);
-    float s2 = P.sig2 * inv;
-    float s6 = s2 * s2 * s2;
-    g = inv * s6 * fmaf(P.c48, s6, -P.c24);          // 24 eps s6 (2 s6 - 1) / d2
-    V = fmaf(s6, fmaf(P.c4, s6, -P.c4), -P.vshift);   // 4 eps s6 (s6 - 1) - V_c
+    float inv3 = inv * inv * inv;
+    g = inv * inv3 * fmaf(P.lj_a, inv3, -P.lj_b);            // 24 eps s6 (2 s6 - 1) / d2, s6 = sigma^6 / d2^3
+    V = fmaf(inv3, fmaf(P.lj_c, inv3, -P.lj_d), -P.vshift);   // 4 eps s6 (s6 - 1) - V_c
 }
 
 struct Rot { float m[3][3]; };
@@ -186,10 +186,13 @@ __device__ __forceinline__ void fene_vertex(const DevParams& P, const DevBuffers
 // VERTEX kernels (S:A6).  List layout: tile of 32 particles, int4 groups: entry k of lane l at
 // ((tile*capg + k/4)*32 + l)*4 + k%4  -> one coalesced 128-bit load per 4 visits.
 // ------------------------------------------------------------------------------------------------
-template <bool IMG>
-__device__ __forceinline__ void vertex_lj_visit(const DevParams& P, const float4* __restrict__ pos, float4 xi, int j, bool valid,
-                                                float& fx, float& fy, float& fz, float& pe) {
-    float4 xj = ldg4(pos + j);
+// Per-thread accumulators of the LJ VERTEX loop.  `band` tracks min |d2 - rc^2|: if any visit came within the
+// fp64-recheck band (S:H10) the particle is recomputed by vertex_lj_careful after the loop, which keeps the
+// hot loop free of calls and branches.
+struct LJAcc { float fx, fy, fz, pe, band; int nin; };
+
+template <bool IMG, bool TAIL>
+__device__ __forceinline__ void vertex_lj_visit(const DevParams& P, float4 xi, float4 xj, bool valid, LJAcc& a) {
     float dx, dy, dz;
     if (IMG) {
         dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
@@ -199,58 +202,102 @@ __device__ __forceinline__ void vertex_lj_visit(const DevParams& P, const float4
         dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
     }
     float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    bool in = in_cutoff(P, d2, xi, xj) && valid;
-    float g, V;
-    lj_pair(P, d2, g, V);
-    g = in ? g : 0.0f;
-    V = in ? V : 0.0f;
-    fx = fmaf(-g, dx, fx); fy = fmaf(-g, dy, fy); fz = fmaf(-g, dz, fz);
-    pe += V;
+    if (TAIL) d2 = fmaxf(d2, 1e-12f);           // padding entries point at the particle itself
+    const float t = d2 - P.rc2;
+    bool in = t < 0.0f;
+    if (TAIL) in = in && valid;
+    a.band = fminf(a.band, fabsf(t));
+    const float inv = rcp_approx(d2);
+    float inv3 = inv * inv * inv;
+    inv3 = in ? inv3 : 0.0f;
+    const float g = inv * inv3 * fmaf(P.lj_a, inv3, -P.lj_b);     // 24 eps s6 (2 s6 - 1) / d2
+    a.fx = fmaf(-g, dx, a.fx); a.fy = fmaf(-g, dy, a.fy); a.fz = fmaf(-g, dz, a.fz);
+    a.pe = fmaf(inv3, fmaf(P.lj_c, inv3, -P.lj_d), a.pe);        // 4 eps s6 (s6 - 1); the shift is nin * V_c
+    a.nin += in ? 1 : 0;
+}
+
+template <bool IMG>
+__device__ __forceinline__ void vertex_lj_loop(const DevParams& P, const float4* __restrict__ pos, const int4* __restrict__ row,
+                                               float4 xi, int cnt, int gmin, int gmax, LJAcc& a) {
+    int g = 0;
+#pragma unroll 2
+    for (; g < gmin; ++g) {                        // every lane of the warp has 4 real neighbours here
+        const int4 jj = row[g * MD_TILE];
+        const float4 x0 = ldg4(pos + jj.x), x1 = ldg4(pos + jj.y), x2 = ldg4(pos + jj.z), x3 = ldg4(pos + jj.w);
+        vertex_lj_visit<IMG, false>(P, xi, x0, true, a);
+        vertex_lj_visit<IMG, false>(P, xi, x1, true, a);
+        vertex_lj_visit<IMG, false>(P, xi, x2, true, a);
+        vertex_lj_visit<IMG, false>(P, xi, x3, true, a);
+    }
+    for (; g < gmax; ++g) {                        // ragged tail: entries k >= cnt are padding
+        const int4 jj = row[g * MD_TILE];
+        const int k = g * 4;
+        const float4 x0 = ldg4(pos + jj.x), x1 = ldg4(pos + jj.y), x2 = ldg4(pos + jj.z), x3 = ldg4(pos + jj.w);
+        vertex_lj_visit<IMG, true>(P, xi, x0, k < cnt, a);
+        vertex_lj_visit<IMG, true>(P, xi, x1, k + 1 < cnt, a);
+        vertex_lj_visit<IMG, true>(P, xi, x2, k + 2 < cnt, a);
+        vertex_lj_visit<IMG, true>(P, xi, x3, k + 3 < cnt, a);
+    }
+}
+
+// Rare path: some visit of this particle fell inside the recheck band -> redo the particle with the fp64
+// decision of S:O0 / S:Q5 for every banded pair (same accumulation order as the fast loop).  Scalar arguments
+// only (a by-value parameter block would live on the stack); the result goes through `out` (global memory).
+__device__ __noinline__ void vertex_lj_careful(const float4* __restrict__ pos, const int* __restrict__ row_i, int cnt, float4 xi,
+                                              float Lx, float Ly, float Lz, float rc2, float band_abs,
+                                              float lj_a, float lj_b, float lj_c, float lj_d, float vshift,
+                                              double dLx, double dLy, double dLz, double rc2d, float4* out) {
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f;
+    int nin = 0;
+    for (int k = 0; k < cnt; ++k) {
+        const int j = row_i[(k >> 2) * (MD_TILE * 4) + (k & 3)];
+        const float4 xj = pos[j];
+        const float dx = min_image(xj.x, xi.x, Lx, 0.5f * Lx);
+        const float dy = min_image(xj.y, xi.y, Ly, 0.5f * Ly);
+        const float dz = min_image(xj.z, xi.z, Lz, 0.5f * Lz);
+        const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        const float t = d2 - rc2;
+        bool in = t < 0.0f;
+        if (fabsf(t) < band_abs) in = inside_fp64(xi, xj, dLx, dLy, dLz, rc2d);
+        const float inv = rcp_approx(d2);
+        float inv3 = inv * inv * inv;
+        inv3 = in ? inv3 : 0.0f;
+        const float g = inv * inv3 * fmaf(lj_a, inv3, -lj_b);
+        fx = fmaf(-g, dx, fx); fy = fmaf(-g, dy, fy); fz = fmaf(-g, dz, fz);
+        pe = fmaf(inv3, fmaf(lj_c, inv3, -lj_d), pe);
+        nin += in ? 1 : 0;
+    }
+    *out = make_float4(fx, fy, fz, fmaf(-(float)nin, vshift, pe));
 }
 
 template <bool BONDS>
-__global__ void __launch_bounds__(128) k_vertex_lj(DevParams P, DevBuffers B, const float4* __restrict__ pos, float4* __restrict__ force) {
+__global__ void __launch_bounds__(128, 8) k_vertex_lj(DevParams P, DevBuffers B, const float4* __restrict__ pos, float4* __restrict__ force) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, tile = i >> 5;
     if (tile >= P.ntiles) return;
     const bool live = i < P.N;
     const int cnt = live ? B.nl_count[i] : 0;
-    const int2 info = B.tile_info[tile];
-    const float4 xi = live ? pos[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const int2 info = B.tile_info[tile];                 // (kmax | img << 30, kmin)
+    const int kmax = info.x & 0x3fffffff;
+    const float4 xi = pos[live ? i : 0];
     const int4* __restrict__ row = reinterpret_cast<const int4*>(B.nl_full) + (size_t)tile * P.capg * MD_TILE + lane;
-    const int ngroups = (info.x + 3) >> 2;
-    const int self = live ? i : 0;   // padding entries point at a harmless address and are masked by `valid`
-    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f;
-    if (info.y) {
-        for (int g = 0; g < ngroups; ++g) {
-            int4 jj = row[g * MD_TILE];
-            int k = g * 4;
-            bool v0 = k < cnt, v1 = k + 1 < cnt, v2 = k + 2 < cnt, v3 = k + 3 < cnt;
-            vertex_lj_visit<true>(P, pos, xi, v0 ? jj.x : self, v0, fx, fy, fz, pe);
-            vertex_lj_visit<true>(P, pos, xi, v1 ? jj.y : self, v1, fx, fy, fz, pe);
-            vertex_lj_visit<true>(P, pos, xi, v2 ? jj.z : self, v2, fx, fy, fz, pe);
-            vertex_lj_visit<true>(P, pos, xi, v3 ? jj.w : self, v3, fx, fy, fz, pe);
-        }
-    } else {
-#pragma unroll 2
-        for (int g = 0; g < ngroups; ++g) {
-            int4 jj = row[g * MD_TILE];
-            int k = g * 4;
-            bool v0 = k < cnt, v1 = k + 1 < cnt, v2 = k + 2 < cnt, v3 = k + 3 < cnt;
-            vertex_lj_visit<false>(P, pos, xi, v0 ? jj.x : self, v0, fx, fy, fz, pe);
-            vertex_lj_visit<false>(P, pos, xi, v1 ? jj.y : self, v1, fx, fy, fz, pe);
-            vertex_lj_visit<false>(P, pos, xi, v2 ? jj.z : self, v2, fx, fy, fz, pe);
-            vertex_lj_visit<false>(P, pos, xi, v3 ? jj.w : self, v3, fx, fy, fz, pe);
-        }
-    }
+    LJAcc a = { 0.f, 0.f, 0.f, 0.f, 3.0e38f, 0 };
+    if (info.x >> 30) vertex_lj_loop<true>(P, pos, row, xi, cnt, info.y >> 2, (kmax + 3) >> 2, a);
+    else vertex_lj_loop<false>(P, pos, row, xi, cnt, info.y >> 2, (kmax + 3) >> 2, a);
     if (!live) return;
-    pe *= 0.5f;
+    if (a.band < P.band_abs) {
+        vertex_lj_careful(pos, reinterpret_cast<const int*>(row), cnt, xi, P.Lx, P.Ly, P.Lz, P.rc2, P.band_abs,
+                          P.lj_a, P.lj_b, P.lj_c, P.lj_d, P.vshift, P.dLx, P.dLy, P.dLz, P.rc2d, force + i);
+        const float4 r = force[i];
+        a.fx = r.x; a.fy = r.y; a.fz = r.z; a.pe = r.w; a.nin = 0;
+    }
+    float pe = 0.5f * fmaf(-(float)a.nin, P.vshift, a.pe);
     if (BONDS) {
         float bpe = 0.f;
-        fene_vertex(P, B, pos, i, xi, fx, fy, fz, bpe);
+        fene_vertex(P, B, pos, i, xi, a.fx, a.fy, a.fz, bpe);
         pe += 0.5f * bpe;
     }
-    force[i] = make_float4(fx, fy, fz, pe);
+    force[i] = make_float4(a.fx, a.fy, a.fz, pe);
 }
 
 template <bool IMG>
@@ -290,7 +337,7 @@ __global__ void __launch_bounds__(128) k_vertex_patchy(DevParams P, DevBuffers B
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
     for (int k = 0; k < cnt; ++k) {
         int j = row[(k >> 2) * (MD_TILE * 4) + (k & 3)];
-        if (info.y) vertex_patchy_visit<true>(P, pos, quat, xi, qi, j, fx, fy, fz, pe, tx, ty, tz);
+        if (info.x >> 30) vertex_patchy_visit<true>(P, pos, quat, xi, qi, j, fx, fy, fz, pe, tx, ty, tz);
         else vertex_patchy_visit<false>(P, pos, quat, xi, qi, j, fx, fy, fz, pe, tx, ty, tz);
     }
     force[i] = make_float4(fx, fy, fz, 0.5f * pe);

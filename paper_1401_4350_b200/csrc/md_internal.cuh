@@ -34,12 +34,13 @@ struct DevParams {
     double rv2d, rc2d;                 // (rcut+skin)^2 and rcut^2 formed in double (S:O0, S:Q5)
     double cscale_x, cscale_y, cscale_z;   // cells per unit length, n_k / L_k
     int ncx, ncy, ncz, ncell;
-    float rc2, rc2_lo, rc2_hi;         // fp32 cutoff and the fp64-recheck band (S:H10)
+    float rc2, band_abs;               // fp32 cutoff and the half-width of the fp64-recheck band |d2 - rc2| (S:H10)
     float half_skin2;                  // (skin/2)^2
     // pair potential
     int kind;
     float eps, sig2, mass, inv_mass;
     float c48, c24, c4, vshift;        // 48 eps, 24 eps, 4 eps, V_c
+    float lj_a, lj_b, lj_c, lj_d;      // 48 eps sigma^12, 24 eps sigma^6, 4 eps sigma^12, 4 eps sigma^6
     // WCA core of the patchy potential
     float core_rc2, core_vshift;
     // FENE
@@ -67,7 +68,7 @@ struct DevBuffers {
     float4* pos_ref;       // [N]
     int* nl_count;         // [Npad]
     int* nl_full;          // [ntiles*32*cap] tile-transposed full list
-    int2* tile_info;       // [ntiles] (kmax, needs_image)
+    int2* tile_info;       // [ntiles] (kmax | needs_image << 30, kmin over the tile's live lanes)
     int* half_count;       // [N]
     unsigned int* edge_off;// [N+1]
     int2* edges;           // [ecap]
