@@ -32,7 +32,8 @@ import numpy as np
 
 METRIC = "pair interactions/s (Verlet pairs E per force evaluation / time), VERTEX vs EDGE, LJ N=2^20"
 UNIT = "pair interactions/s"
-EDGE_VARIANTS = ["red", "red_v4", "warp", "segmented"]
+EDGE_VARIANTS = ["red", "red_v4", "warp", "segmented", "warp_smem"]
+VERTEX_VARIANTS = ["smem", "l2"]
 
 
 def workload(name: str):
@@ -190,7 +191,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2a", choices=["C2a", "C2b"])
     ap.add_argument("--strategy", default="vertex", choices=["vertex", "edge"])
-    ap.add_argument("--scatter", default="warp", choices=EDGE_VARIANTS)
+    ap.add_argument("--scatter", default=None, choices=EDGE_VARIANTS + VERTEX_VARIANTS,
+                    help="EDGE scatter variant (default warp_smem) or VERTEX gather variant (default smem)")
     ap.add_argument("--order", default="hilbert", choices=["none", "cell", "hilbert"])
     ap.add_argument("--melt-steps", type=int, default=300)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -198,6 +200,10 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.scatter is None:
+        args.scatter = "smem" if args.strategy == "vertex" else "warp_smem"
+    if args.order == "none" and args.scatter in ("smem", "warp_smem"):
+        args.scatter = "l2" if args.strategy == "vertex" else "warp"
 
     import torch
     if not torch.cuda.is_available():
@@ -256,16 +262,23 @@ def main():
     stf = s.stats()
     Ef = stf["n_edges"]
     fe = {}
-    t_v = time_calls(torch, lambda: s.forces("vertex"), 20)
-    fe["vertex"] = {"us": t_v, "pairs_per_s": Ef / (t_v * 1e-6)}
+    for gv in VERTEX_VARIANTS:
+        if gv == "smem" and args.order == "none":
+            continue
+        t = time_calls(torch, lambda: s.forces("vertex", gv), 20)
+        fe[f"vertex_{gv}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
     for sc in EDGE_VARIANTS:
+        if sc == "warp_smem" and args.order == "none":
+            continue
         t = time_calls(torch, lambda: s.forces("edge", sc), 10 if sc != "red" else 5)
         fe[f"edge_{sc}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
+    best_vertex = min((k for k in fe if k.startswith("vertex")), key=lambda k: fe[k]["us"])
+    t_v = fe[best_vertex]["us"]
     clocks = sampler.stop()
     best_edge = min((k for k in fe if k.startswith("edge")), key=lambda k: fe[k]["us"])
     peak, peak_src = measured_peaks()
     dom = args.strategy
-    t_dom = t_v if dom == "vertex" else fe[f"edge_{args.scatter}"]["us"]
+    t_dom = fe[f"{dom}_{args.scatter}"]["us"]
     abytes = algorithmic_bytes(dom, Ef, N)
     achieved = abytes / (t_dom * 1e-6) / 1e9
     traffic = None
@@ -275,7 +288,9 @@ def main():
             traffic = json.loads(tf.read_text()).get(f"{args.workload}_{dom}")
         except Exception:
             traffic = None
-    roofline = {"bound": "hbm", "kernel": "k_vertex_lj" if dom == "vertex" else "k_edge_*", "achieved": achieved,
+    kname = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp_smem": "k_edge_staged", "warp": "k_edge_warp",
+             "red": "k_edge_red", "red_v4": "k_edge_red", "segmented": "k_edge_store+k_edge_segsum"}[args.scatter]
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "algorithmic_bytes_per_launch": abytes, "us_per_launch": t_dom, "peak_source": peak_src}
 
@@ -314,14 +329,14 @@ def main():
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{args.workload}: BASELINE.json configs[1], LJ fluid N=2^20 rho=0.8 rc={w.rcut} skin=0.3, "
                                f"fcc+jitter melted by {args.melt_steps} untimed steps",
-                   "N": N, "E": int(E_run), "strategy": args.strategy,
-                   "scatter": args.scatter if args.strategy == "edge" else None, "order": args.order,
+                   "N": N, "E": int(E_run), "strategy": args.strategy, "variant": args.scatter, "order": args.order,
                    "step": "md_integrate(1): kick, drift, skin check, device-side rebuild when triggered, forces, kick; "
                            "one md_energy per K steps",
                    "l2": "inputs larger than L2 (list 0.3 GB streamed per evaluation; no flush needed)",
                    "rebuilds_in_timed_region": st1["n_rebuilds"] - stw["n_rebuilds"],
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "force_eval": fe, "edge_vs_vertex": fe["vertex"]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
+        "force_eval": fe, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
+        "best_vertex": best_vertex,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "energy_total": sum(e_tot),
     }

@@ -4,8 +4,8 @@ Thin Python binding over the C ABI of include/md_b200.h (libmd_b200.so, hand-wri
 PyTorch is used for device memory and streams only; there is no CPU or PyTorch fallback: importing
 `MDSystem` without the built library raises.
 """
-from .binding import (MDSystem, MDError, load_library, STRATEGY, SCATTER, ORDER, POT_KIND, library_path,
+from .binding import (MDSystem, MDError, load_library, STRATEGY, SCATTER, GATHER, ORDER, POT_KIND, library_path,
                       EXPORTED_SYMBOLS)
 
-__all__ = ["MDSystem", "MDError", "load_library", "STRATEGY", "SCATTER", "ORDER", "POT_KIND", "library_path",
+__all__ = ["MDSystem", "MDError", "load_library", "STRATEGY", "SCATTER", "GATHER", "ORDER", "POT_KIND", "library_path",
            "EXPORTED_SYMBOLS"]

@@ -11,7 +11,8 @@ _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libmd_b200.so"
 
 STRATEGY = {"vertex": 0, "edge": 1}
-SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3}
+SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3, "warp_smem": 4}
+GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
 POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2}
 STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPACITY", -4: "MD_ERR_CUDA",
@@ -122,8 +123,11 @@ def load_library() -> C.CDLL:
     return L
 
 
-def _code(x) -> int:
-    return x if isinstance(x, int) else (STRATEGY.get(x, None) if x in STRATEGY else SCATTER[x])
+def variant_code(strategy: str, variant) -> int:
+    """Third argument of md_forces / md_integrate / md_step_host: md_gather for VERTEX, md_scatter for EDGE."""
+    if strategy == "vertex":
+        return GATHER.get(variant, 0)      # anything that is not a gather name means "auto"
+    return SCATTER[variant]
 
 
 class MDSystem:
@@ -224,10 +228,11 @@ class MDSystem:
         self._check(self.lib.md_build_verlet(self.h))
 
     def forces(self, strategy="vertex", scatter="red_v4"):
-        self._check(self.lib.md_forces(self.h, STRATEGY[strategy], SCATTER[scatter]))
+        self._check(self.lib.md_forces(self.h, STRATEGY[strategy], variant_code(strategy, scatter)))
 
     def integrate(self, dt, nsteps, strategy="vertex", scatter="red_v4"):
-        self._check(self.lib.md_integrate(self.h, float(dt), int(nsteps), STRATEGY[strategy], SCATTER[scatter]))
+        self._check(self.lib.md_integrate(self.h, float(dt), int(nsteps), STRATEGY[strategy],
+                                            variant_code(strategy, scatter)))
 
     def energy(self):
         u, kt, kr = C.c_double(0), C.c_double(0), C.c_double(0)
@@ -258,7 +263,7 @@ class MDSystem:
         """End-to-end call on HOST (pinned or pageable) torch/numpy float32 [N,4] buffers, updated in place."""
         ptr = lambda a: None if a is None else C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
         self._check(self.lib.md_step_host(self.h, ptr(pos), ptr(vel), ptr(force), ptr(quat), ptr(angmom), ptr(torque),
-                                          float(dt), int(nsteps), STRATEGY[strategy], SCATTER[scatter]))
+                                          float(dt), int(nsteps), STRATEGY[strategy], variant_code(strategy, scatter)))
 
     def launch_count(self) -> int:
         return int(self.lib.md_launch_count(self.h))

@@ -9,7 +9,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libmd_b200.so"
-SOURCES = ["md_api.cu", "md_build.cu", "md_forces.cu", "md_integrate.cu"]
+SOURCES = ["md_api.cu", "md_build.cu", "md_forces.cu", "md_staged.cu", "md_integrate.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"]
 
@@ -25,7 +25,7 @@ def needs_build() -> bool:
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime
-    deps = [CSRC / f for f in SOURCES] + [CSRC / "md_internal.cuh", ROOT / "include" / "md_b200.h"]
+    deps = [CSRC / f for f in SOURCES] + [CSRC / "md_internal.cuh", CSRC / "md_pair.cuh", ROOT / "include" / "md_b200.h"]
     return any(d.stat().st_mtime > t for d in deps)
 
 

@@ -17,6 +17,7 @@ struct Geometry {
     int64_t ncell;
     int cap, ntiles;
     size_t ecap;
+    int rcap, nblk, stage_cap, slice;   // staged path
 };
 
 // S:Q8: n_k = max(1, floor(L_k / (r_v (1 + 1e-5)))) cells per axis, width >= r_v
@@ -35,6 +36,19 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
     g->ntiles = (int)((N + MD_TILE - 1) / MD_TILE);
     if ((int64_t)g->ntiles * MD_TILE * g->cap >= (1ll << 31)) return false;
     g->ecap = (size_t)N * g->cap / 2 + 64;
+    // staged path: rows of 16-bit local indices in chunks of 4*slice entries; smem capacity of the build kernel
+    g->rcap = (g->cap + 31) / 32 * 32;
+    g->slice = max_neigh >= 64 ? 8 : 4;
+    g->nblk = (int)((N + MD_TB - 1) / MD_TB);
+    {
+        const double ppc = (double)N / (double)g->ncell;                 // particles per cell
+        const double own = std::min<double>(MD_TB, MD_TB / std::max(ppc, 1e-9));   // cells per block
+        const double side = cbrt(own) + 2.0;                               // stencil union of a compact blob, x1.5 for ragged shapes
+        double m = 2.0 * (1.5 * side * side * side * ppc) + 256.0;
+        m = std::min<double>(m, (double)N + 64.0);
+        m = std::min<double>(m, 11000.0);                                  // 16 B each: <= 176 KB of the 227 KB
+        g->stage_cap = ((int)m + 63) / 64 * 64;
+    }
     return true;
 }
 
@@ -79,6 +93,12 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.e_part = (double*)take(8 * 3 * 2048);
     b.e_out = (double*)take(8 * 4);
     b.stage4 = (float4*)take(16 * Npad);
+    b.cell_lin = (int*)take(4 * (size_t)g.ncell);
+    b.rows = (unsigned short*)take(2 * Npad * (size_t)g.rcap);
+    b.row_count = (int*)take(4 * Npad);
+    b.lo_count = (int*)take(4 * Npad);
+    b.blk = (BlkInfo*)take(sizeof(BlkInfo) * (size_t)g.nblk);
+    b.seg = (int2*)take(8 * (size_t)g.nblk * MD_SEGMAX);
     if (B) *B = b;
     return off;
 }
@@ -158,6 +178,15 @@ md_status check_cuda(md_system* s, const char* where) {
     return MD_OK;
 }
 
+// cell_rank[linear cell] = storage rank and its inverse cell_lin[rank] = linear cell
+void upload_cell_rank(md_system* s, const std::vector<int>& rank) {
+    std::vector<int> inv(rank.size());
+    for (size_t c = 0; c < rank.size(); ++c) inv[(size_t)rank[c]] = (int)c;
+    cudaMemcpyAsync(s->B.cell_rank, rank.data(), 4 * rank.size(), cudaMemcpyHostToDevice, s->stream);
+    cudaMemcpyAsync(s->B.cell_lin, inv.data(), 4 * inv.size(), cudaMemcpyHostToDevice, s->stream);
+    cudaStreamSynchronize(s->stream);   // host temporaries
+}
+
 // slot s holds original id s (state arrays given in original id order)
 void reset_ids(md_system* s) {
     std::vector<int> iden((size_t)s->N);
@@ -181,6 +210,20 @@ md_status sync_and_check(md_system* s, const char* where) {
         snprintf(s->errmsg, sizeof(s->errmsg), "neighbour capacity exceeded: a particle has %d Verlet neighbours, max_neigh = %d", c.max_seen, s->P.cap);
         s->lists_valid = false;
         return MD_ERR_CAPACITY;
+    }
+    if (c.err & MD_DEVERR_STAGE) {
+        snprintf(s->errmsg, sizeof(s->errmsg), "staged neighbourhood capacity exceeded: a block needs %d staged particles / %d segments "
+                 "(build capacity %d, launch capacity %d, segment capacity %d); rebuild with md_build_cells + md_build_verlet",
+                 c.max_stage, c.max_seg, s->P.stage_cap, s->stage_launch, MD_SEGMAX);
+        s->lists_valid = s->staged_valid = false;
+        return MD_ERR_CAPACITY;
+    }
+    if (s->order != MD_ORDER_NONE && c.max_stage > 0) {
+        // size the staged force launches from the largest neighbourhood seen, with 25 % head room for the
+        // device-side rebuilds that happen before the next synchronising call
+        int want = (int)(c.max_stage * 1.25) + 64;
+        want = (want + 63) / 64 * 64;
+        s->stage_launch = want;
     }
     if (c.err & MD_DEVERR_FENE) {
         snprintf(s->errmsg, sizeof(s->errmsg), "FENE bond length reached R0");
@@ -236,6 +279,11 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.rc2 = (float)P.rc2d;
     P.band_abs = (float)(P.rc2d * 1e-6);   // S:H10 band; the fp32 d2 is accurate to ~3e-7 relative
     P.half_skin2 = (float)(0.25 * skin * skin);
+    P.rv2 = (float)P.rv2d;
+    P.band_rv = (float)(P.rv2d * 1e-6);    // S:Q6 band of the list predicate
+    P.nblk = g.nblk; P.slice = g.slice; P.stage_cap = g.stage_cap; P.rcap = g.rcap;
+    P.skinf = (float)skin;
+    s->stage_launch = g.stage_cap;
     P.kind = pot->kind;
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
     P.sigma = pot->sigma;
@@ -280,8 +328,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
         reset_ids(s);
         std::vector<int> rank;
         make_cell_rank(g.nc, MD_ORDER_NONE, rank);
-        cudaMemcpyAsync(s->B.cell_rank, rank.data(), 4 * rank.size(), cudaMemcpyHostToDevice, s->stream);
-        cudaStreamSynchronize(s->stream);
+        upload_cell_rank(s, rank);
     }
     if (check_cuda(s, "md_create") != MD_OK) { free(s); return MD_ERR_CUDA; }
     *out = s;
@@ -301,7 +348,7 @@ md_status md_bind_state(md_system* s, void* pos, void* vel, void* force, void* q
     s->angmom = s->rigid ? (float4*)angmom : nullptr;
     s->torque = s->rigid ? (float4*)torque : nullptr;
     s->bound = true;
-    s->cells_valid = s->lists_valid = s->forces_valid = s->seg_valid = false;
+    s->cells_valid = s->lists_valid = s->forces_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
     reset_ids(s);   // the arrays are taken to be in original id order
     return check_cuda(s, "md_bind_state");
 }
@@ -314,9 +361,8 @@ md_status md_set_order(md_system* s, int32_t order) {
     std::vector<int> rank;
     int nc[3] = { s->P.ncx, s->P.ncy, s->P.ncz };
     make_cell_rank(nc, order, rank);
-    cudaMemcpyAsync(s->B.cell_rank, rank.data(), 4 * rank.size(), cudaMemcpyHostToDevice, s->stream);
-    cudaStreamSynchronize(s->stream);   // rank is a host temporary
-    s->cells_valid = s->lists_valid = s->seg_valid = false;
+    upload_cell_rank(s, rank);
+    s->cells_valid = s->lists_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
     return check_cuda(s, "md_set_order");
 }
 
@@ -326,7 +372,7 @@ md_status md_build_cells(md_system* s) {
     if (!s->bound) return fail(s, MD_ERR_STATE, "md_build_cells: no state bound");
     md_launch_build_cells(s, false);
     s->cells_valid = true;
-    s->lists_valid = s->seg_valid = false;
+    s->lists_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
     return check_cuda(s, "md_build_cells");
 }
 
@@ -334,17 +380,57 @@ md_status md_build_verlet(md_system* s) {
     if (!s) return MD_ERR_INVALID;
     if (s->sticky) return (md_status)s->sticky;
     if (!s->bound || !s->cells_valid) return fail(s, MD_ERR_STATE, "md_build_verlet: call md_build_cells first");
-    md_launch_build_verlet(s, false);
-    md_launch_build_end(s, false);
-    s->lists_valid = true;
-    s->seg_valid = false;
+    s->staged_valid = s->legacy_valid = s->seg_valid = false;
+    if (s->order != MD_ORDER_NONE) {
+        // cell-sorted storage: rows of block-local indices (md_staged.cu); the explicit global-slot lists of the
+        // L2-gather variants are derived lazily from the same cells and the build-time positions (ensure_explicit)
+        md_launch_build_staged(s, false);
+        md_launch_build_end(s, false);
+        s->lists_valid = true;
+        md_status st = sync_and_check(s, "md_build_verlet");   // reads the largest staged neighbourhood: sizes the launches
+        if (st != MD_OK) { s->lists_valid = false; return st; }
+        s->staged_valid = true;
+    } else {
+        md_launch_build_verlet(s, false, s->pos);
+        md_launch_build_end(s, false);
+        s->lists_valid = true;
+        s->legacy_valid = true;
+    }
     s->cells_valid = false;   // cells describe the positions at build time only
     return check_cuda(s, "md_build_verlet");
 }
 
+// The explicit lists (tile-transposed full list + (i, j) edge list) for the current build.  The cell arrays still
+// describe the build-time positions kept in pos_ref (no md_build_cells since), so the lists can be made on demand.
+static void ensure_explicit(md_system* s) {
+    if (s->legacy_valid) return;
+    md_launch_build_verlet(s, false, s->B.pos_ref);
+    s->legacy_valid = true;
+    s->seg_valid = false;
+}
+
+// which list representation a (strategy, variant) pair runs on
+static bool wants_staged(const md_system* s, int32_t strategy, int32_t variant) {
+    if (s->order == MD_ORDER_NONE) return false;
+    if (strategy == MD_VERTEX) return variant != MD_GATHER_L2;
+    return variant == MD_SCATTER_WARP_SMEM;
+}
+
 static md_status check_strategy(md_system* s, int32_t strategy, int32_t scatter) {
     if (strategy != MD_VERTEX && strategy != MD_EDGE) return fail(s, MD_ERR_INVALID, "unknown strategy");
-    if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_SEGMENTED)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
+    if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_WARP_SMEM)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
+    if (strategy == MD_VERTEX && (scatter < MD_GATHER_AUTO || scatter > MD_GATHER_SMEM)) return fail(s, MD_ERR_INVALID, "unknown gather variant");
+    if (s->order == MD_ORDER_NONE && ((strategy == MD_VERTEX && scatter == MD_GATHER_SMEM) || (strategy == MD_EDGE && scatter == MD_SCATTER_WARP_SMEM)))
+        return fail(s, MD_ERR_STATE, "the shared-memory staged variants need cell-sorted storage: md_set_order(MD_ORDER_CELL or MD_ORDER_HILBERT)");
+    return MD_OK;
+}
+
+static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatter) {
+    if (wants_staged(s, strategy, scatter)) {
+        if (!md_launch_forces_staged(s, strategy, scatter)) return fail(s, MD_ERR_CAPACITY, "staged neighbourhood does not fit in shared memory");
+    } else {
+        md_launch_forces(s, strategy, scatter);
+    }
     return MD_OK;
 }
 
@@ -354,11 +440,16 @@ md_status md_forces(md_system* s, int32_t strategy, int32_t scatter) {
     if (!s->bound || !s->lists_valid) return fail(s, MD_ERR_STATE, "md_forces: lists are not built (md_build_cells, md_build_verlet)");
     md_status st = check_strategy(s, strategy, scatter);
     if (st != MD_OK) return st;
-    if (strategy == MD_EDGE && scatter == MD_SCATTER_SEGMENTED && !s->seg_valid) {
-        md_launch_seg_index(s, false);
-        s->seg_valid = true;
+    if (wants_staged(s, strategy, scatter)) {
+        if (!s->staged_valid) return fail(s, MD_ERR_STATE, "md_forces: staged lists are not valid, call md_build_cells + md_build_verlet");
+    } else {
+        ensure_explicit(s);
+        if (strategy == MD_EDGE && scatter == MD_SCATTER_SEGMENTED && !s->seg_valid) {
+            md_launch_seg_index(s, false);
+            s->seg_valid = true;
+        }
     }
-    md_launch_forces(s, strategy, scatter);
+    if ((st = launch_forces_any(s, strategy, scatter)) != MD_OK) return st;
     s->forces_valid = true;
     return check_cuda(s, "md_forces");
 }
@@ -370,19 +461,28 @@ md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy
     if (!(dt > 0) || nsteps < 0) return fail(s, MD_ERR_INVALID, "md_integrate: dt > 0 and nsteps >= 0 required");
     md_status st = check_strategy(s, strategy, scatter);
     if (st != MD_OK) return st;
+    const bool staged = wants_staged(s, strategy, scatter);
     const bool seg = strategy == MD_EDGE && scatter == MD_SCATTER_SEGMENTED;
+    if (staged && !s->staged_valid) return fail(s, MD_ERR_STATE, "md_integrate: staged lists are not valid, call md_build_cells + md_build_verlet");
+    if (!staged) ensure_explicit(s);
     if (seg && !s->seg_valid) { md_launch_seg_index(s, false); s->seg_valid = true; }
     const float fdt = (float)dt;
     for (int64_t k = 0; k < nsteps; ++k) {
         md_launch_kick_drift(s, fdt);            // sets the device rebuild flag (S:A5)
         md_launch_build_cells(s, true);          // gated on the flag: no host synchronisation (S:H6)
-        md_launch_build_verlet(s, true);
+        if (staged) md_launch_build_staged(s, true);
+        else md_launch_build_verlet(s, true, s->pos);
         if (seg) md_launch_seg_index(s, true);
         md_launch_build_end(s, true);
-        md_launch_forces(s, strategy, scatter);
+        if ((st = launch_forces_any(s, strategy, scatter)) != MD_OK) return st;
         md_launch_kick(s, fdt);
     }
-    if (!seg) s->seg_valid = false;   // a device-side rebuild may have happened without the index
+    if (nsteps > 0) {
+        // a device-side rebuild may have replaced the lists of the representation in use; the other one is stale
+        if (staged) { s->legacy_valid = false; s->seg_valid = false; }
+        else { s->staged_valid = false; if (!seg) s->seg_valid = false; }
+        s->cells_valid = false;
+    }
     return check_cuda(s, "md_integrate");
 }
 
@@ -426,6 +526,11 @@ md_status md_get_pairs(md_system* s, int32_t* pairs_host, int64_t capacity, int6
     if (!s || !n) return MD_ERR_INVALID;
     if (s->sticky) return (md_status)s->sticky;
     if (!s->lists_valid) return fail(s, MD_ERR_STATE, "md_get_pairs: lists are not built");
+    if (s->staged_valid && !s->legacy_valid) {   // export what the staged kernels use: rows -> explicit (i, j) pairs
+        md_launch_edge_offsets(s, false);
+        md_launch_edges_from_rows(s);
+        s->seg_valid = false;                     // the edge array now follows the row order, not the explicit build
+    }
     DevCtrl c;
     cudaMemcpyAsync(&c, s->B.ctrl, sizeof(c), cudaMemcpyDeviceToHost, s->stream);
     md_status st = sync_and_check(s, "md_get_pairs");

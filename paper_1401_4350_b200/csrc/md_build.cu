@@ -334,17 +334,21 @@ __global__ void k_build_end(DevBuffers B, int gated) {
     B.ctrl->rebuild = 0;
 }
 
-void md_launch_build_verlet(md_system* s, bool gated) {
+void md_launch_build_verlet(md_system* s, bool gated, const float4* pos_src) {
     const DevParams& P = s->P;
     int g = gated ? 1 : 0;
     k_build_begin<<<1, 1, 0, s->stream>>>(s->B, g);
     int nb = cdiv((int64_t)P.ntiles * MD_TILE, 128);
-    if (s->order != MD_ORDER_NONE) k_build_verlet<true><<<nb, 128, 0, s->stream>>>(P, s->B, g, s->pos);
-    else k_build_verlet<false><<<nb, 128, 0, s->stream>>>(P, s->B, g, s->pos);
+    if (s->order != MD_ORDER_NONE) k_build_verlet<true><<<nb, 128, 0, s->stream>>>(P, s->B, g, pos_src);
+    else k_build_verlet<false><<<nb, 128, 0, s->stream>>>(P, s->B, g, pos_src);
     s->launches += 2;
     launch_scan(s, gated, (const unsigned int*)s->B.half_count, s->B.edge_off, P.N, &s->B.ctrl->n_edges);
-    k_fill_edges<<<cdiv(P.N, 128), 128, 0, s->stream>>>(P, s->B, g, s->pos);
+    k_fill_edges<<<cdiv(P.N, 128), 128, 0, s->stream>>>(P, s->B, g, pos_src);
     s->launches += 1;
+}
+
+void md_launch_edge_offsets(md_system* s, bool gated) {
+    launch_scan(s, gated, (const unsigned int*)s->B.half_count, s->B.edge_off, s->P.N, nullptr);
 }
 
 void md_launch_build_end(md_system* s, bool gated) {

@@ -11,154 +11,7 @@
 
 static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
-// ------------------------------------------------------------------------------------------------
-// small device helpers
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ float rcp_approx(float x) {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ float rsqrt_approx(float x) {
-    float r;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ float ex2_approx(float x) {
-    float r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ void red_add_v4(float4* addr, float a, float b, float c, float d) {
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
-}
-__device__ __forceinline__ void red_add_f32(float* addr, float a) {
-    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
-}
-__device__ __forceinline__ float4 ldg4(const float4* p) { return __ldg(p); }
-
-// S:H9 robust fp32 minimum image: subtract L from the larger coordinate before differencing (both inner
-// subtractions are exact), used only by warps that hold a pair crossing a periodic face.
-__device__ __forceinline__ float min_image(float xj, float xi, float L, float hL) {
-    float t = xj - xi;
-    if (t > hL) t = (xj - L) - xi;
-    else if (t < -hL) t = xj - (xi - L);
-    return t;
-}
-
-// S:O0 / S:Q5 predicate in fp64, fixed operation order, no FMA contraction.
-__device__ __noinline__ bool inside_fp64(float4 xi, float4 xj, double Lx, double Ly, double Lz, double thr2) {
-    double dx = (double)xj.x - (double)xi.x;
-    if (dx > 0.5 * Lx) dx -= Lx; else if (dx < -0.5 * Lx) dx += Lx;
-    double dy = (double)xj.y - (double)xi.y;
-    if (dy > 0.5 * Ly) dy -= Ly; else if (dy < -0.5 * Ly) dy += Ly;
-    double dz = (double)xj.z - (double)xi.z;
-    if (dz > 0.5 * Lz) dz -= Lz; else if (dz < -0.5 * Lz) dz += Lz;
-    double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-    return d2 < thr2;
-}
-
-// in-cutoff decision: fp32 away from the threshold, fp64 inside the band
-__device__ __forceinline__ bool in_cutoff(const DevParams& P, float d2, float4 xi, float4 xj) {
-    const float t = d2 - P.rc2;
-    bool in = t < 0.0f;
-    if (fabsf(t) < P.band_abs) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rc2d);
-    return in;
-}
-
-// ------------------------------------------------------------------------------------------------
-// pair functions.  d = r_j - r_i (minimum image).  They return the force ON j:  F_j = g*d (+ ...),
-// F_i = -F_j, and the pair energy V; the callers split V in halves (S:O1).
-// ------------------------------------------------------------------------------------------------
-// O1 Eq.(1), cut + energy shift P:99;  O2 WCA is the same with rc = 2^(1/6) sigma, V_c = -eps.
-__device__ __forceinline__ void lj_pair(const DevParams& P, float d2, float& g, float& V) {
-    float inv = rcp_approx(d2);
-    float inv3 = inv * inv * inv;
-    g = inv * inv3 * fmaf(P.lj_a, inv3, -P.lj_b);            // 24 eps s6 (2 s6 - 1) / d2, s6 = sigma^6 / d2^3
-    V = fmaf(inv3, fmaf(P.lj_c, inv3, -P.lj_d), -P.vshift);   // 4 eps s6 (s6 - 1) - V_c
-}
-
-struct Rot { float m[3][3]; };
-__device__ __forceinline__ Rot quat_to_rot(float4 q) {   // q = (w,x,y,z) stored as (.x,.y,.z,.w) = (w,x,y,z)
-    float w = q.x, x = q.y, y = q.z, z = q.w;
-    Rot R;
-    R.m[0][0] = 1.f - 2.f * (y * y + z * z); R.m[0][1] = 2.f * (x * y - w * z);       R.m[0][2] = 2.f * (x * z + w * y);
-    R.m[1][0] = 2.f * (x * y + w * z);       R.m[1][1] = 1.f - 2.f * (x * x + z * z); R.m[1][2] = 2.f * (y * z - w * x);
-    R.m[2][0] = 2.f * (x * z - w * y);       R.m[2][1] = 2.f * (y * z + w * x);       R.m[2][2] = 1.f - 2.f * (x * x + y * y);
-    return R;
-}
-
-// angular factor of one particle (S:O4, factorised form): with v = R^T * dir (dir = +u for i, -u for j)
-//   A = sum_a exp((b_a.v - 1)/w^2),   S = (1/w^2) R sum_a e_a b_a
-__device__ __forceinline__ void patch_factor(const DevParams& P, float4 q, float ux, float uy, float uz,
-                                             float& A, float& Sx, float& Sy, float& Sz) {
-    Rot R = quat_to_rot(q);
-    float vx = R.m[0][0] * ux + R.m[1][0] * uy + R.m[2][0] * uz;
-    float vy = R.m[0][1] * ux + R.m[1][1] * uy + R.m[2][1] * uz;
-    float vz = R.m[0][2] * ux + R.m[1][2] * uy + R.m[2][2] * uz;
-    const float k = P.inv_w2 * 1.4426950408889634f;   // exp(x) = 2^(x log2 e)
-    float a = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
-    for (int p = 0; p < P.n_patches; ++p) {
-        float c = P.pdir[p][0] * vx + P.pdir[p][1] * vy + P.pdir[p][2] * vz;
-        float e = ex2_approx((c - 1.0f) * k);
-        a += e;
-        bx = fmaf(e, P.pdir[p][0], bx); by = fmaf(e, P.pdir[p][1], by); bz = fmaf(e, P.pdir[p][2], bz);
-    }
-    A = a;
-    Sx = P.inv_w2 * (R.m[0][0] * bx + R.m[0][1] * by + R.m[0][2] * bz);
-    Sy = P.inv_w2 * (R.m[1][0] * bx + R.m[1][1] * by + R.m[1][2] * bz);
-    Sz = P.inv_w2 * (R.m[2][0] * bx + R.m[2][1] * by + R.m[2][2] * bz);
-}
-
-// O4 (B:10): WCA core + patch term.  Outputs force on j (fx,fy,fz), V, torque on i, torque on j.
-template <bool NEED_TJ>
-__device__ __forceinline__ void patchy_pair(const DevParams& P, float dx, float dy, float dz, float d2, float4 qi, float4 qj,
-                                            float& fx, float& fy, float& fz, float& V,
-                                            float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
-    float rinv = rsqrt_approx(d2);
-    float r = d2 * rinv;
-    float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
-    float Ai, Six, Siy, Siz, Aj, Sjx, Sjy, Sjz;
-    patch_factor(P, qi, ux, uy, uz, Ai, Six, Siy, Siz);
-    patch_factor(P, qj, -ux, -uy, -uz, Aj, Sjx, Sjy, Sjz);
-    float dr = r - P.sigma;
-    float G = ex2_approx(-dr * dr * P.inv_2sr2 * 1.4426950408889634f);
-    float dG = -dr * P.inv_sr2 * G;
-    float eG = P.eps_patch * G;
-    V = -eG * Ai * Aj;
-    // dA_i/dr_vec = (S_i - (S_i.u)u)/r ; dA_j/dr_vec = -(S_j - (S_j.u)u)/r
-    float siu = Six * ux + Siy * uy + Siz * uz;
-    float sju = Sjx * ux + Sjy * uy + Sjz * uz;
-    float ci = eG * Aj * rinv, cj = eG * Ai * rinv;
-    float rad = P.eps_patch * dG * Ai * Aj;
-    // dV/dr_vec = -[ rad*u + ci*(S_i - siu u) - cj*(S_j - sju u) ] ; F_j = -dV/dr_vec
-    fx = rad * ux + ci * (Six - siu * ux) - cj * (Sjx - sju * ux);
-    fy = rad * uy + ci * (Siy - siu * uy) - cj * (Sjy - sju * uy);
-    fz = rad * uz + ci * (Siz - siu * uz) - cj * (Sjz - sju * uz);
-    // tau_i = eps_p G A_j (S_i x u)
-    float ti = eG * Aj;
-    tix = ti * (Siy * uz - Siz * uy); tiy = ti * (Siz * ux - Six * uz); tiz = ti * (Six * uy - Siy * ux);
-    if (NEED_TJ) {   // tau_j = eps_p G A_i (S_j x (-u))
-        float tj = -eG * Ai;
-        tjx = tj * (Sjy * uz - Sjz * uy); tjy = tj * (Sjz * ux - Sjx * uz); tjz = tj * (Sjx * uy - Sjy * ux);
-    }
-    if (d2 < P.core_rc2) {   // WCA core (force continuous at its cut: plain fp32 test)
-        float inv = rinv * rinv;
-        float s2 = P.sig2 * inv, s6 = s2 * s2 * s2;
-        float g = inv * s6 * fmaf(P.c48, s6, -P.c24);
-        V += fmaf(s6, fmaf(P.c4, s6, -P.c4), -P.core_vshift);
-        fx = fmaf(g, dx, fx); fy = fmaf(g, dy, fy); fz = fmaf(g, dz, fz);
-    }
-}
-
-// O3 FENE (B:9): U = -1/2 K R0^2 ln(1 - d2/R0^2); force on j = -K d / (1 - d2/R0^2)
-__device__ __forceinline__ bool fene_pair(const DevParams& P, float d2, float& g, float& V) {
-    float q = 1.0f - d2 * P.fene_invR02;
-    if (!(q > 0.0f)) { g = 0.f; V = 0.f; return false; }
-    g = -P.fene_K / q;
-    V = -0.5f * P.fene_K * P.fene_R02 * __logf(q);
-    return true;
-}
+#include "md_pair.cuh"
 
 // FENE partners of slot i (ids id-1 and id+1 inside its chain) -> accumulates into (f, pe)
 __device__ __forceinline__ void fene_vertex(const DevParams& P, const DevBuffers& B, const float4* __restrict__ pos,

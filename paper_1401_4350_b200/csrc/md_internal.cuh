@@ -12,6 +12,17 @@
 // Device error bits latched in DevCtrl::err
 #define MD_DEVERR_CAPACITY 1
 #define MD_DEVERR_FENE 2
+#define MD_DEVERR_STAGE 4     // a block's staged neighbourhood / segment table exceeds its capacity
+
+// ---- shared-memory staged path (md_staged.cu) ----
+#define MD_TB 128             // particles per block (consecutive slots of the cell-sorted storage)
+#define MD_NCAND 4096         // candidate cells per block before sort + unique (27 x non-empty own cells <= 27 x MD_TB)
+#define MD_UMAX 2048          // distinct cells in a block's neighbourhood
+#define MD_SEGMAX 1024        // contiguous slot segments per block
+// BlkInfo flags
+#define MD_BLK_WRAP 1         // some listed pair of the block crosses a periodic face
+#define MD_BLK_SHIFT_OK 2     // ... and the shift-down transform of the staged coordinates reproduces every minimum image
+#define MD_BLK_AXIS_SHIFT 4   // bits 2..4: axes (x, y, z) the transform applies to
 
 // Device-resident control block (first bytes of the workspace).
 struct DevCtrl {
@@ -23,7 +34,17 @@ struct DevCtrl {
     int n_rebuilds;              // builds triggered by the skin criterion inside md_integrate
     int pad0;
     unsigned int scan_total;     // scratch for the scan kernels
-    int pad[7];
+    int max_stage;               // largest staged neighbourhood (particles) over the blocks at the last staged build
+    int max_seg;                 // largest segment count
+    int pad[5];
+};
+
+// per-block header of the staged path
+struct BlkInfo {
+    int nseg;        // contiguous slot segments to stage
+    int M;           // staged particles (the dummy entry sits at local index M)
+    int own_base;    // local index of the block's first own particle
+    int flags;       // MD_BLK_*
 };
 
 // Parameter block passed by value to every kernel.
@@ -36,6 +57,9 @@ struct DevParams {
     int ncx, ncy, ncz, ncell;
     float rc2, band_abs;               // fp32 cutoff and the half-width of the fp64-recheck band |d2 - rc2| (S:H10)
     float half_skin2;                  // (skin/2)^2
+    float rv2, band_rv;                // fp32 list radius^2 and its fp64-recheck band (S:Q6)
+    int nblk, slice, stage_cap, rcap;  // staged path: blocks of MD_TB slots, lanes per particle, smem capacity (particles), row stride
+    float skinf;
     // pair potential
     int kind;
     float eps, sig2, mass, inv_mass;
@@ -81,6 +105,13 @@ struct DevBuffers {
     double* e_part;        // [e_blocks*3]
     double* e_out;         // [3]
     float4* stage4;        // [N] staging for md_step_host un-permute
+    // staged path
+    int* cell_lin;         // [ncell] storage rank -> linear cell index (inverse of cell_rank)
+    unsigned short* rows;  // [Npad*cap] per-particle Verlet rows of block-local indices, slice-transposed chunks
+    int* row_count;        // [Npad] |L_i|
+    int* lo_count;         // [Npad] neighbours with slot < i (the EDGE half list is the suffix of the row)
+    BlkInfo* blk;          // [nblk]
+    int2* seg;             // [nblk*MD_SEGMAX] (first slot, first local index)
 };
 
 struct md_system {
@@ -95,6 +126,8 @@ struct md_system {
     bool rigid;
     float4 *pos, *vel, *force, *quat, *angmom, *torque;
     bool bound, cells_valid, lists_valid, forces_valid, seg_valid;
+    bool staged_valid, legacy_valid;   // which list representations describe the current build
+    int stage_launch;        // staged-particle capacity the force kernels are launched with (from the last synchronised build)
     int64_t launches;
     int sticky;              // sticky md_status (CUDA errors)
     char errmsg[512];
@@ -105,7 +138,8 @@ struct md_system {
 
 // ---- kernel launch entry points (defined in the .cu files) ----
 void md_launch_build_cells(md_system* s, bool gated);
-void md_launch_build_verlet(md_system* s, bool gated);
+void md_launch_build_verlet(md_system* s, bool gated, const float4* pos_src);   // explicit (global-slot) lists
+void md_launch_edge_offsets(md_system* s, bool gated);   // edge_off = exclusive scan of half_count
 void md_launch_seg_index(md_system* s, bool gated);
 void md_launch_build_end(md_system* s, bool gated);
 void md_launch_forces(md_system* s, int strategy, int scatter);
@@ -113,5 +147,10 @@ void md_launch_kick_drift(md_system* s, float dt);
 void md_launch_kick(md_system* s, float dt);
 void md_launch_energy(md_system* s);
 void md_launch_unpermute(md_system* s, const float4* src, float4* dst);   // dst[ids[s]] = src[s]
+// staged path (md_staged.cu)
+void md_launch_build_staged(md_system* s, bool gated);
+void md_launch_edges_from_rows(md_system* s);     // explicit (i, j) edge list from the staged rows (export / legacy EDGE variants)
+bool md_launch_forces_staged(md_system* s, int strategy, int scatter);
+size_t md_staged_smem_bytes(const md_system* s, int stage_entries, bool edge);
 
 #define MD_ERRBUF(s, ...) snprintf((s)->errmsg, sizeof((s)->errmsg), __VA_ARGS__)

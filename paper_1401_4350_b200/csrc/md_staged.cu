@@ -1,0 +1,856 @@
+// md_staged.cu -- the shared-memory staged path.
+//
+// Storage is cell-sorted (MD_ORDER_CELL / MD_ORDER_HILBERT), so the particles of a cell are one
+// contiguous slot range.  A block owns MD_TB consecutive slots; the union of the 27-cell stencils (P:53
+// "standard cell algorithm") of its cells is a short list of contiguous slot SEGMENTS.  Both the Verlet-list
+// build and the force kernels first copy those segments into shared memory -- the force kernels with 1-D bulk
+// TMA copies (cp.async.bulk + mbarrier) -- and then address neighbours by a 16-bit block-LOCAL index:
+//   * the Verlet row of particle i (S:A4) holds |L_i| local indices sorted by slot; entries with slot < i come
+//     first, so the EDGE half list (i < j) is the suffix of the same row;
+//   * VERTEX and EDGE run one SLICE of 4 or 8 lanes per particle: consecutive lanes read
+//     consecutive sorted neighbours, i.e. mostly consecutive float4 in shared memory (few bank conflicts),
+//     instead of one 128-byte L1 line per lane from global memory (profiles/r01a_first_path.md).
+// The pair arithmetic, the fp64 recheck band (S:H10) and all tolerances are those of md_forces.cu.
+#include <stdio.h>
+#include "md_pair.cuh"
+
+#define GATE(B, gated) if ((gated) && (B).ctrl->rebuild == 0) return
+
+static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ------------------------------------------------------------------------------------------------
+// PTX wrappers: mbarrier + 1-D bulk TMA copy global -> shared
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, void* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// position of sorted entry k inside a row: chunks of 4*S entries, lane l of the slice owns 4 consecutive u16
+// (one 64-bit load) holding the entries of 4 successive iterations
+__device__ __forceinline__ int row_pos(int k, int S) {
+    const int c4 = 4 * S, r = k % c4;
+    return (k - r) + (r % S) * 4 + r / S;
+}
+
+#define DUMMY_COORD 1.0e15f   // the padding entry of every staged neighbourhood: d2 ~ 3e30, never inside a cutoff
+
+// ------------------------------------------------------------------------------------------------
+// block scan over TB threads (exclusive), total in *tot
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int blk_excl_scan(int v, int* tot, int* sh /* >= 33 ints */) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) sh[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        int s = lane < nw ? sh[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += y;
+        }
+        if (lane < nw) sh[lane] = s;
+    }
+    __syncthreads();
+    const int base = w ? sh[w - 1] : 0;
+    *tot = sh[nw - 1];
+    __syncthreads();
+    return base + x - v;
+}
+
+__device__ __forceinline__ int pack_coord(int cx, int cy, int cz) { return cx | (cy << 10) | (cz << 20); }
+
+// ------------------------------------------------------------------------------------------------
+// S:A4 staged Verlet build.  One block per MD_TB slots, one thread per particle.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
+                                                        int ncand_cap, int umax) {
+    GATE(B, gated);
+    extern __shared__ __align__(16) unsigned char smraw[];
+    float4* spos = reinterpret_cast<float4*>(smraw);                 // [stage_cap]
+    int* cand = reinterpret_cast<int*>(spos + P.stage_cap);          // [ncand_cap]
+    int* urank = cand + ncand_cap;                                   // [umax]
+    int* ubase = urank + umax;                                       // [umax + 1]
+    int* ucoord = ubase + umax + 1;                                  // [umax]
+    int* own_rank = ucoord + umax;                                   // [MD_TB]
+    __shared__ int sh_scan[33];
+    __shared__ int s_flags, s_err, s_own_base;
+
+    const int b = blockIdx.x, tid = threadIdx.x;
+    const int i0 = b * MD_TB, i1 = min(P.N, i0 + MD_TB);
+    const int i = i0 + tid;
+    const bool live = i < i1;
+    if (tid == 0) { s_flags = 0; s_err = 0; s_own_base = 0; }
+
+    // 1. the block's non-empty cells (storage ranks, ascending), compacted
+    const int myrank = live ? B.cell_of[i] : -1;
+    const int head = live && (tid == 0 || B.cell_of[i - 1] != myrank) ? 1 : 0;
+    int nownc;
+    const int oc = blk_excl_scan(head, &nownc, sh_scan);
+    if (head) own_rank[oc] = myrank;
+    __syncthreads();
+
+    // 2. candidate cells: the 27-cell stencil of every own cell (S:Q8; duplicates removed below)
+    const int n = 27 * nownc;
+    int n2 = 32;
+    while (n2 < n) n2 <<= 1;
+    if (n2 > ncand_cap) {   // cannot happen for n <= 27*MD_TB = 3456 <= MD_NCAND unless the launch was sized smaller
+        if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
+        if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
+        return;
+    }
+    for (int t = tid; t < n2; t += MD_TB) {
+        int v = 0x7fffffff;
+        if (t < n) {
+            const int lin = B.cell_lin[own_rank[t / 27]];
+            const int s = t % 27;
+            const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
+            int ax = cx + s / 9 - 1, ay = cy + (s / 3) % 3 - 1, az = cz + s % 3 - 1;
+            int wrapped = 0;
+            if (ax < 0) { ax += P.ncx; wrapped = 1; } else if (ax >= P.ncx) { ax -= P.ncx; wrapped = 1; }
+            if (ay < 0) { ay += P.ncy; wrapped = 1; } else if (ay >= P.ncy) { ay -= P.ncy; wrapped = 1; }
+            if (az < 0) { az += P.ncz; wrapped = 1; } else if (az >= P.ncz) { az -= P.ncz; wrapped = 1; }
+            // fewer than 3 cells on an axis: the wrap lands on a cell of the axis again; duplicates vanish in the unique step
+            if (wrapped) atomicOr(&s_flags, MD_BLK_WRAP);
+            const int r = B.cell_rank[(ax * P.ncy + ay) * P.ncz + az];
+            v = (B.cell_start[r + 1] > B.cell_start[r]) ? r : 0x7fffffff;   // empty cells contribute nothing
+        }
+        cand[t] = v;
+    }
+    __syncthreads();
+
+    // 3. bitonic sort of the candidate ranks
+    for (int k = 2; k <= n2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = tid; t < n2; t += MD_TB) {
+                const int x = t ^ j;
+                if (x > t) {
+                    const int a = cand[t], c = cand[x];
+                    const bool asc = (t & k) == 0;
+                    if ((a > c) == asc) { cand[t] = c; cand[x] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // 4. unique -> urank[0..U)
+    int U = 0;
+    for (int base = 0; base < n2; base += MD_TB) {
+        const int t = base + tid;
+        const int v = t < n2 ? cand[t] : 0x7fffffff;
+        const int f = (v != 0x7fffffff && (t == 0 || cand[t - 1] != v)) ? 1 : 0;
+        int tot;
+        const int p = blk_excl_scan(f, &tot, sh_scan);
+        if (f && U + p < umax) urank[U + p] = v;
+        U += tot;
+    }
+    if (U > umax) {
+        if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
+        if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
+        return;
+    }
+    __syncthreads();
+
+    // 5. local base of every distinct cell (exclusive scan of the cell populations), packed cell coordinates
+    int M = 0;
+    for (int base = 0; base < U; base += MD_TB) {
+        const int u = base + tid;
+        int c = 0;
+        if (u < U) {
+            const int r = urank[u];
+            c = B.cell_start[r + 1] - B.cell_start[r];
+            const int lin = B.cell_lin[r];
+            ucoord[u] = pack_coord(lin / (P.ncz * P.ncy), (lin / P.ncz) % P.ncy, lin % P.ncz);
+        }
+        int tot;
+        const int p = blk_excl_scan(c, &tot, sh_scan);
+        if (u < U) ubase[u] = M + p;
+        M += tot;
+    }
+    if (tid == 0) ubase[U] = M;
+    if (M + 1 > P.stage_cap) {
+        if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); atomicMax(&B.ctrl->max_stage, M + 1); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
+        if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
+        return;
+    }
+    __syncthreads();
+
+    // 6. contiguous slot segments -> global segment table (first slot, first local index)
+    int nseg = 0;
+    for (int base = 0; base < U; base += MD_TB) {
+        const int u = base + tid;
+        int f = 0;
+        if (u < U) f = (u == 0 || B.cell_start[urank[u - 1] + 1] != B.cell_start[urank[u]]) ? 1 : 0;
+        int tot;
+        const int p = blk_excl_scan(f, &tot, sh_scan);
+        if (f && nseg + p < MD_SEGMAX) B.seg[(size_t)b * MD_SEGMAX + nseg + p] = make_int2(B.cell_start[urank[u]], ubase[u]);
+        nseg += tot;
+    }
+    if (nseg > MD_SEGMAX) {
+        if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
+        if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
+        return;
+    }
+
+    // 7. stage the neighbourhood (plain coalesced copies, one warp per cell) and locate the block's own particles
+    for (int u = tid >> 5; u < U; u += MD_TB / 32) {
+        const int s0 = B.cell_start[urank[u]], l0 = ubase[u], len = ubase[u + 1] - l0;
+        for (int k = tid & 31; k < len; k += 32) spos[l0 + k] = pos[s0 + k];
+    }
+    if (tid == 0) {
+        const int r0 = own_rank[0];
+        int lo = 0, hi = U - 1;
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (urank[mid] < r0) lo = mid + 1; else hi = mid; }
+        s_own_base = ubase[lo] + (i0 - B.cell_start[r0]);
+    }
+    __syncthreads();
+    const int own_base = s_own_base;
+    const bool maywrap = (s_flags & MD_BLK_WRAP) != 0 || P.ncx < 3 || P.ncy < 3 || P.ncz < 3;
+    __syncthreads();
+    if (tid == 0) s_flags = 0;   // from here on: bit 0 = a listed pair wraps, bits 2..4 = axes, bit 5 = shift transform fails
+    __syncthreads();
+
+    // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6), rows sorted by slot
+    int cnt = 0, lo_cnt = 0, flags = 0;
+    if (live) {
+        const int me = own_base + tid;
+        const float4 xi = spos[me];
+        const int S = P.slice;
+        unsigned short* __restrict__ row = B.rows + (size_t)i * P.rcap;
+        const int lin = B.cell_lin[myrank];
+        const int cx = lin / (P.ncz * P.ncy), cy = (lin / P.ncz) % P.ncy, cz = lin % P.ncz;
+        const float hLx = P.hLx, hLy = P.hLy, hLz = P.hLz;
+        for (int u = 0; u < U; ++u) {
+            const int pc = ucoord[u];
+            int dx = abs((pc & 1023) - cx), dy = abs(((pc >> 10) & 1023) - cy), dz = abs((pc >> 20) - cz);
+            const bool mx = dx <= 1 || dx == P.ncx - 1, my = dy <= 1 || dy == P.ncy - 1, mz = dz <= 1 || dz == P.ncz - 1;
+            if (!(mx && my && mz)) continue;
+            const int t1 = ubase[u + 1];
+            for (int t = ubase[u]; t < t1; ++t) {
+                if (t == me) continue;
+                const float4 xj = spos[t];
+                float ddx, ddy, ddz;
+                if (maywrap) {
+                    ddx = min_image(xj.x, xi.x, P.Lx, hLx); ddy = min_image(xj.y, xi.y, P.Ly, hLy); ddz = min_image(xj.z, xi.z, P.Lz, hLz);
+                } else {
+                    ddx = xj.x - xi.x; ddy = xj.y - xi.y; ddz = xj.z - xi.z;
+                }
+                const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
+                const float tt = d2 - P.rv2;
+                bool in = tt < 0.0f;
+                if (fabsf(tt) < P.band_rv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
+                if (in) {
+                    if (cnt < P.cap) row[row_pos(cnt, S)] = (unsigned short)t;
+                    ++cnt;
+                    lo_cnt += (t < me);
+                    if (maywrap) {
+                        // which axes wrap, and does the shift-down transform T(x) = x > L/2 ? x - L : x reproduce the image?
+                        const float rx = xj.x - xi.x, ry = xj.y - xi.y, rz = xj.z - xi.z;
+                        if (fabsf(rx) > hLx) flags |= 1 | (MD_BLK_AXIS_SHIFT << 0);
+                        if (fabsf(ry) > hLy) flags |= 1 | (MD_BLK_AXIS_SHIFT << 1);
+                        if (fabsf(rz) > hLz) flags |= 1 | (MD_BLK_AXIS_SHIFT << 2);
+                        const float tx = (xj.x > hLx ? xj.x - P.Lx : xj.x) - (xi.x > hLx ? xi.x - P.Lx : xi.x);
+                        const float ty = (xj.y > hLy ? xj.y - P.Ly : xj.y) - (xi.y > hLy ? xi.y - P.Ly : xi.y);
+                        const float tz = (xj.z > hLz ? xj.z - P.Lz : xj.z) - (xi.z > hLz ? xi.z - P.Lz : xi.z);
+                        if ((fabsf(rx) > hLx && tx != ddx) || (fabsf(ry) > hLy && ty != ddy) || (fabsf(rz) > hLz && tz != ddz)) flags |= 32;
+                        // an axis that is shifted must also keep its unwrapped pairs intact
+                        // ... and stay valid while the particles move by up to skin/2 before the next build
+                        const float sk = P.skinf;
+                        if ((fabsf(rx) <= hLx && tx != ddx) || fabsf(xj.x - hLx) <= sk || fabsf(xi.x - hLx) <= sk) flags |= 64 << 0;
+                        if ((fabsf(ry) <= hLy && ty != ddy) || fabsf(xj.y - hLy) <= sk || fabsf(xi.y - hLy) <= sk) flags |= 64 << 1;
+                        if ((fabsf(rz) <= hLz && tz != ddz) || fabsf(xj.z - hLz) <= sk || fabsf(xi.z - hLz) <= sk) flags |= 64 << 2;
+                    }
+                }
+            }
+        }
+        if (cnt > P.cap) atomicOr(&B.ctrl->err, MD_DEVERR_CAPACITY);
+        const int c2 = min(cnt, P.cap);
+        for (int k = c2; k < ((c2 + S - 1) / S) * S; ++k) row[row_pos(k, S)] = (unsigned short)M;   // dummy padding
+        B.row_count[i] = c2;
+        B.lo_count[i] = cnt > P.cap ? 0 : lo_cnt;
+        B.half_count[i] = cnt > P.cap ? 0 : cnt - lo_cnt;
+        B.pos_ref[i] = xi;
+    }
+    if (flags) atomicOr(&s_flags, flags);
+    // 9. block totals
+    int tot_full, tot_half;
+    blk_excl_scan(min(cnt, P.cap), &tot_full, sh_scan);
+    blk_excl_scan(cnt > P.cap ? 0 : cnt - lo_cnt, &tot_half, sh_scan);
+    const int seen = __reduce_max_sync(0xffffffffu, cnt);
+    if ((tid & 31) == 0) atomicMax(&B.ctrl->max_seen, seen);
+    __syncthreads();
+    if (tid == 0) {
+        const int f = s_flags;
+        int out = 0;
+        if (f & 1) {
+            out = MD_BLK_WRAP | (f & (7 * MD_BLK_AXIS_SHIFT));
+            // the transform is usable if no wrapped pair disagrees and no SHIFTED axis breaks an unwrapped pair
+            const int shifted = (f >> 2) & 7, broken = (f >> 6) & 7;
+            if (!(f & 32) && !(shifted & broken)) out |= MD_BLK_SHIFT_OK;
+        }
+        B.blk[b] = BlkInfo{ nseg, M, own_base, out };
+        atomicAdd(&B.ctrl->n_full, (unsigned long long)tot_full);
+        atomicAdd(&B.ctrl->n_edges, (unsigned int)tot_half);
+        atomicMax(&B.ctrl->max_stage, M + 1);
+        atomicMax(&B.ctrl->max_seg, nseg);
+    }
+}
+
+__global__ void k_staged_begin(DevBuffers B, int gated) {
+    GATE(B, gated);
+    B.ctrl->max_seen = 0;
+    B.ctrl->n_full = 0ull;
+    B.ctrl->n_edges = 0u;
+    B.ctrl->max_stage = 0;
+    B.ctrl->max_seg = 0;
+}
+
+static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, size_t* smem) {
+    const DevParams& P = s->P;
+    const double ppc = (double)P.N / (double)P.ncell;
+    double own = (double)MD_TB / (ppc > 1e-9 ? ppc : 1e-9);
+    if (own > MD_TB) own = MD_TB;
+    int nc = 64;
+    while (nc < 27 * (2 * own + 4) && nc < MD_NCAND) nc <<= 1;
+    if (nc > MD_NCAND) nc = MD_NCAND;
+    int um = nc < MD_UMAX ? nc : MD_UMAX;
+    *ncand_cap = nc;
+    *umax = um;
+    *smem = 16 * (size_t)P.stage_cap + 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 16;
+}
+
+void md_launch_build_staged(md_system* s, bool gated) {
+    const DevParams& P = s->P;
+    const int g = gated ? 1 : 0;
+    int nc, um;
+    size_t smem;
+    staged_build_sizes(s, &nc, &um, &smem);
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncSetAttribute(k_build_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+        attr_done = true;
+    }
+    k_staged_begin<<<1, 1, 0, s->stream>>>(s->B, g);
+    k_build_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um);
+    s->launches += 2;
+}
+
+// ------------------------------------------------------------------------------------------------
+// explicit (i, j) edge list from the staged rows: i < j slots, sorted by i, bit 31 of j = periodic image flag.
+// Used by md_get_pairs (list parity export).  Needs edge_off = exclusive scan of half_count.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(MD_TB) k_edges_from_rows(DevParams P, DevBuffers B, const float4* __restrict__ pos) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    int* sslot = reinterpret_cast<int*>(smraw);   // [M]
+    const int b = blockIdx.x, tid = threadIdx.x;
+    const BlkInfo bi = B.blk[b];
+    const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
+    for (int sg = tid >> 5; sg < bi.nseg; sg += MD_TB / 32) {
+        const int2 s0 = seg[sg];
+        const int len = (sg + 1 < bi.nseg ? seg[sg + 1].y : bi.M) - s0.y;
+        for (int k = tid & 31; k < len; k += 32) sslot[s0.y + k] = s0.x + k;
+    }
+    __syncthreads();
+    const int i = b * MD_TB + tid;
+    if (i >= P.N) return;
+    const int cnt = B.row_count[i], lo = B.lo_count[i], S = P.slice;
+    const unsigned short* __restrict__ row = B.rows + (size_t)i * P.rcap;
+    const float4 xi = pos[i];
+    unsigned int o = B.edge_off[i];
+    for (int k = lo; k < cnt; ++k) {
+        const int j = sslot[row[row_pos(k, S)]];
+        const float4 xj = pos[j];
+        const int w = (fabsf(xj.x - xi.x) > P.hLx) | (fabsf(xj.y - xi.y) > P.hLy) | (fabsf(xj.z - xi.z) > P.hLz);
+        B.edges[o++] = make_int2(i, j | (w << 31));
+    }
+}
+
+void md_launch_edges_from_rows(md_system* s) {
+    const DevParams& P = s->P;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncSetAttribute(k_edges_from_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+        attr_done = true;
+    }
+    k_edges_from_rows<<<P.nblk, MD_TB, 4 * (size_t)P.stage_cap, s->stream>>>(P, s->B, s->pos);
+    s->launches += 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// staging prologue of the force kernels: bulk TMA copies of the block's segments into shared memory
+// ------------------------------------------------------------------------------------------------
+struct Stage {
+    float4* spos;    // [M + 1]  (entry M = dummy)
+    float4* squat;   // [M + 1]  rigid bodies only
+    int* sslot;      // [M]      EDGE only: local index -> slot
+};
+
+template <bool QUAT, bool SLOT>
+__device__ __forceinline__ Stage stage_block(const DevParams& P, const DevBuffers& B, const BlkInfo bi, int b, int stage_entries,
+                                             const float4* __restrict__ pos, const float4* __restrict__ quat, unsigned char* smraw) {
+    Stage st;
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smraw);
+    st.spos = reinterpret_cast<float4*>(smraw + 16);
+    st.squat = QUAT ? st.spos + stage_entries : nullptr;
+    st.sslot = SLOT ? reinterpret_cast<int*>(st.spos + (QUAT ? 2 : 1) * (size_t)stage_entries) : nullptr;
+    const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
+    const int tid = threadIdx.x;
+    if (tid < 32) {
+        if (tid == 0) {
+            mbar_init(bar, 1);
+            mbar_expect_tx(bar, (unsigned)bi.M * 16u * (QUAT ? 2u : 1u));
+        }
+        __syncwarp();
+        for (int sg = tid; sg < bi.nseg; sg += 32) {
+            const int2 s0 = seg[sg];
+            const int len = (sg + 1 < bi.nseg ? seg[sg + 1].y : bi.M) - s0.y;
+            bulk_g2s(st.spos + s0.y, pos + s0.x, (unsigned)len * 16u, bar);
+            if (QUAT) bulk_g2s(st.squat + s0.y, quat + s0.x, (unsigned)len * 16u, bar);
+        }
+    } else if (SLOT) {
+        for (int sg = (tid >> 5) - 1; sg < bi.nseg; sg += (blockDim.x >> 5) - 1) {
+            const int2 s0 = seg[sg];
+            const int len = (sg + 1 < bi.nseg ? seg[sg + 1].y : bi.M) - s0.y;
+            for (int k = tid & 31; k < len; k += 32) st.sslot[s0.y + k] = s0.x + k;
+        }
+    }
+    if (tid == 32) {
+        st.spos[bi.M] = make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
+        if (QUAT) st.squat[bi.M] = make_float4(1.f, 0.f, 0.f, 0.f);
+    }
+    __syncthreads();          // barrier initialised, slot map and dummy written
+    mbar_wait(bar, 0);        // all segments have landed
+    // periodic blocks: shift the upper half of the box down by L on the wrapped axes (exact in fp32: Sterbenz),
+    // after which plain differences ARE the minimum images (verified pair by pair at build time)
+    if ((bi.flags & MD_BLK_WRAP) && (bi.flags & MD_BLK_SHIFT_OK)) {
+        const bool sx = bi.flags & (MD_BLK_AXIS_SHIFT << 0), sy = bi.flags & (MD_BLK_AXIS_SHIFT << 1), sz = bi.flags & (MD_BLK_AXIS_SHIFT << 2);
+        for (int t = tid; t < bi.M; t += blockDim.x) {
+            float4 x = st.spos[t];
+            if (sx && x.x > P.hLx) x.x -= P.Lx;
+            if (sy && x.y > P.hLy) x.y -= P.Ly;
+            if (sz && x.z > P.hLz) x.z -= P.Lz;
+            st.spos[t] = x;
+        }
+        __syncthreads();
+    }
+    return st;
+}
+
+// slice-wide sums (S a power of two <= 32; all 32 lanes participate)
+template <int S>
+__device__ __forceinline__ float slice_sum(float v) {
+#pragma unroll
+    for (int o = S / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+template <int S>
+__device__ __forceinline__ int slice_sum_i(int v) {
+#pragma unroll
+    for (int o = S / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+template <int S>
+__device__ __forceinline__ float slice_min(float v) {
+#pragma unroll
+    for (int o = S / 2; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// VERTEX, LJ / WCA (+ FENE bonds), staged (S:A6)
+// ------------------------------------------------------------------------------------------------
+struct LJAccS { float fx, fy, fz, pe, band; int nin; };
+
+template <bool IMG>
+__device__ __forceinline__ void lj_visit_s(const DevParams& P, float4 xi, float4 xj, LJAccS& a) {
+    float dx, dy, dz;
+    if (IMG) {
+        dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+    } else {
+        dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+    }
+    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float t = d2 - P.rc2;
+    const bool in = t < 0.0f;
+    a.band = fminf(a.band, fabsf(t));
+    const float inv = rcp_approx(d2);
+    float inv3 = inv * inv * inv;
+    inv3 = in ? inv3 : 0.0f;
+    const float g = inv * inv3 * fmaf(P.lj_a, inv3, -P.lj_b);     // 24 eps s6 (2 s6 - 1) / d2
+    a.fx = fmaf(-g, dx, a.fx); a.fy = fmaf(-g, dy, a.fy); a.fz = fmaf(-g, dz, a.fz);
+    a.pe = fmaf(inv3, fmaf(P.lj_c, inv3, -P.lj_d), a.pe);        // 4 eps s6 (s6 - 1); the shift is nin * V_c
+    a.nin += in ? 1 : 0;
+}
+
+// rare path: a visit of this particle fell inside the fp64-recheck band -> one lane redoes the particle with the
+// S:O0 / S:Q5 decision for every banded pair
+__device__ __noinline__ void lj_careful_s(const float4* spos, const unsigned short* __restrict__ row, int cnt, int S, float4 xi,
+                                          float Lx, float Ly, float Lz, float rc2, float band_abs, float lj_a, float lj_b,
+                                          float lj_c, float lj_d, float vshift, double dLx, double dLy, double dLz, double rc2d,
+                                          float4* out) {
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f;
+    int nin = 0;
+    for (int k = 0; k < cnt; ++k) {
+        const float4 xj = spos[row[row_pos(k, S)]];
+        const float dx = min_image(xj.x, xi.x, Lx, 0.5f * Lx);
+        const float dy = min_image(xj.y, xi.y, Ly, 0.5f * Ly);
+        const float dz = min_image(xj.z, xi.z, Lz, 0.5f * Lz);
+        const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        const float t = d2 - rc2;
+        bool in = t < 0.0f;
+        if (fabsf(t) < band_abs) in = inside_fp64(xi, xj, dLx, dLy, dLz, rc2d);
+        const float inv = rcp_approx(d2);
+        float inv3 = inv * inv * inv;
+        inv3 = in ? inv3 : 0.0f;
+        const float g = inv * inv3 * fmaf(lj_a, inv3, -lj_b);
+        fx = fmaf(-g, dx, fx); fy = fmaf(-g, dy, fy); fz = fmaf(-g, dz, fz);
+        pe = fmaf(inv3, fmaf(lj_c, inv3, -lj_d), pe);
+        nin += in ? 1 : 0;
+    }
+    *out = make_float4(fx, fy, fz, fmaf(-(float)nin, vshift, pe));
+}
+
+// FENE partners of slot i (ids id-1 and id+1 inside its chain), global gathers through slot_of_id
+__device__ __forceinline__ void fene_vertex_s(const DevParams& P, const DevBuffers& B, const float4* __restrict__ pos, int i,
+                                              float& fx, float& fy, float& fz, float& pe) {
+    const float4 xi = pos[i];
+    const int id = B.ids[i];
+    const int m = id % P.chain_len;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const int pid = s == 0 ? id - 1 : id + 1;
+        const bool ok = s == 0 ? (m != 0) : (m != P.chain_len - 1 && pid < P.N);
+        if (!ok) continue;
+        const float4 xj = pos[B.slot_of_id[pid]];
+        const float dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
+        const float dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
+        const float dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+        const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        float g, V;
+        if (!fene_pair(P, d2, g, V)) atomicOr(&B.ctrl->err, MD_DEVERR_FENE);
+        fx -= g * dx; fy -= g * dy; fz -= g * dz;
+        pe += V;
+    }
+}
+
+template <int S, bool IMG>
+__device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
+                                               const float4* __restrict__ pos, float4* __restrict__ force, bool bonds) {
+    const int tid = threadIdx.x, l = tid & (S - 1);
+    const int nslices = blockDim.x / S, sid = tid / S;
+    const int i0 = b * MD_TB, nown = min(P.N - i0, MD_TB);
+    for (int p0 = 0; p0 < nown; p0 += nslices) {          // warp-uniform
+        const int p = p0 + sid;
+        const bool act = p < nown;
+        const int i = i0 + p;
+        const int cnt = act ? B.row_count[i] : 0;
+        const float4 xi = st.spos[bi.own_base + (act ? p : 0)];
+        const uint2* __restrict__ row = reinterpret_cast<const uint2*>(B.rows + (size_t)(act ? i : i0) * P.rcap) + l;
+        const int iters = (cnt + S - 1) / S;
+        LJAccS a = { 0.f, 0.f, 0.f, 0.f, 3.0e38f, 0 };
+        int it = 0;
+        uint2 pk = iters > 0 ? __ldg(row) : make_uint2(0u, 0u);
+        for (; it + 4 <= iters; it += 4) {
+            const uint2 cur = pk;
+            if (it + 4 < iters) pk = __ldg(row + (it / 4 + 1) * S);
+            const float4 x0 = st.spos[cur.x & 0xffffu], x1 = st.spos[cur.x >> 16], x2 = st.spos[cur.y & 0xffffu], x3 = st.spos[cur.y >> 16];
+            lj_visit_s<IMG>(P, xi, x0, a);
+            lj_visit_s<IMG>(P, xi, x1, a);
+            lj_visit_s<IMG>(P, xi, x2, a);
+            lj_visit_s<IMG>(P, xi, x3, a);
+        }
+        if (it < iters) {                                  // 1..3 remaining iterations of the last chunk
+            const int rem = iters - it;
+            lj_visit_s<IMG>(P, xi, st.spos[pk.x & 0xffffu], a);
+            if (rem > 1) lj_visit_s<IMG>(P, xi, st.spos[pk.x >> 16], a);
+            if (rem > 2) lj_visit_s<IMG>(P, xi, st.spos[pk.y & 0xffffu], a);
+        }
+        __syncwarp();
+        a.fx = slice_sum<S>(a.fx); a.fy = slice_sum<S>(a.fy); a.fz = slice_sum<S>(a.fz); a.pe = slice_sum<S>(a.pe);
+        a.nin = slice_sum_i<S>(a.nin); a.band = slice_min<S>(a.band);
+        if (act && l == 0) {
+            if (a.band < P.band_abs) {
+                lj_careful_s(st.spos, B.rows + (size_t)i * P.rcap, cnt, S, xi, P.Lx, P.Ly, P.Lz, P.rc2, P.band_abs, P.lj_a, P.lj_b,
+                             P.lj_c, P.lj_d, P.vshift, P.dLx, P.dLy, P.dLz, P.rc2d, force + i);
+                const float4 r = force[i];
+                a.fx = r.x; a.fy = r.y; a.fz = r.z; a.pe = r.w; a.nin = 0;
+            }
+            float pe = 0.5f * fmaf(-(float)a.nin, P.vshift, a.pe);
+            if (bonds) {
+                float bpe = 0.f;
+                fene_vertex_s(P, B, pos, i, a.fx, a.fy, a.fz, bpe);
+                pe += 0.5f * bpe;
+            }
+            force[i] = make_float4(a.fx, a.fy, a.fz, pe);
+        }
+    }
+}
+
+template <int S>
+__global__ void __launch_bounds__(256) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
+                                                          float4* __restrict__ force) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const int b = blockIdx.x;
+    const BlkInfo bi = B.blk[b];
+    if (bi.M <= 0 || bi.M + 1 > stage_entries) {   // build failed for this block / launch sized too small: latch, never guess
+        if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
+        return;
+    }
+    const Stage st = stage_block<false, false>(P, B, bi, b, stage_entries, pos, nullptr, smraw);
+    const bool bonds = P.kind == MD_POT_FENE_WCA;
+    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_lj_rows<S, true>(P, B, bi, st, b, pos, force, bonds);
+    else vertex_lj_rows<S, false>(P, B, bi, st, b, pos, force, bonds);
+}
+
+// ------------------------------------------------------------------------------------------------
+// VERTEX, patchy rigid bodies, staged
+// ------------------------------------------------------------------------------------------------
+template <int S, bool IMG>
+__device__ __forceinline__ void vertex_patchy_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
+                                                   float4* __restrict__ force, float4* __restrict__ torque) {
+    const int tid = threadIdx.x, l = tid & (S - 1);
+    const int nslices = blockDim.x / S, sid = tid / S;
+    const int i0 = b * MD_TB, nown = min(P.N - i0, MD_TB);
+    for (int p0 = 0; p0 < nown; p0 += nslices) {
+        const int p = p0 + sid;
+        const bool act = p < nown;
+        const int i = i0 + p;
+        const int cnt = act ? B.row_count[i] : 0;
+        const int me = bi.own_base + (act ? p : 0);
+        const float4 xi = st.spos[me], qi = st.squat[me];
+        const unsigned short* __restrict__ row = B.rows + (size_t)(act ? i : i0) * P.rcap;
+        float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
+        for (int k = l; k < cnt; k += S) {
+            const int t = row[row_pos(k, S)];
+            const float4 xj = st.spos[t];
+            float dx, dy, dz;
+            if (IMG) {
+                dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+            } else {
+                dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+            }
+            const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            if (in_cutoff(P, d2, xi, xj)) {
+                const float4 qj = st.squat[t];
+                float gx, gy, gz, V, a, bb, c, u, v, w;
+                patchy_pair<false>(P, dx, dy, dz, d2, qi, qj, gx, gy, gz, V, a, bb, c, u, v, w);
+                fx -= gx; fy -= gy; fz -= gz;
+                tx += a; ty += bb; tz += c;
+                pe += V;
+            }
+        }
+        __syncwarp();
+        fx = slice_sum<S>(fx); fy = slice_sum<S>(fy); fz = slice_sum<S>(fz); pe = slice_sum<S>(pe);
+        tx = slice_sum<S>(tx); ty = slice_sum<S>(ty); tz = slice_sum<S>(tz);
+        if (act && l == 0) {
+            force[i] = make_float4(fx, fy, fz, 0.5f * pe);
+            torque[i] = make_float4(tx, ty, tz, 0.f);
+        }
+    }
+}
+
+template <int S>
+__global__ void __launch_bounds__(256) k_vertex_patchy_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
+                                                              const float4* __restrict__ quat, float4* __restrict__ force,
+                                                              float4* __restrict__ torque) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const int b = blockIdx.x;
+    const BlkInfo bi = B.blk[b];
+    if (bi.M <= 0 || bi.M + 1 > stage_entries) {
+        if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
+        return;
+    }
+    const Stage st = stage_block<true, false>(P, B, bi, b, stage_entries, pos, quat, smraw);
+    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_patchy_rows<S, true>(P, B, bi, st, b, force, torque);
+    else vertex_patchy_rows<S, false>(P, B, bi, st, b, force, torque);
+}
+
+// ------------------------------------------------------------------------------------------------
+// EDGE, staged (S:A7): one lane per unordered pair of the half list (the row suffix, slot j > i); the owning
+// particle's side is summed over the slice in registers (warp-aggregated scatter, B:5), the partner's side is
+// scattered with red.global.add.v4.f32, only for pairs inside the cutoff.
+// ------------------------------------------------------------------------------------------------
+template <int S, int KIND, bool IMG>
+__device__ __forceinline__ void edge_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
+                                          float4* force, float4* torque) {
+    const int tid = threadIdx.x, l = tid & (S - 1);
+    const int nslices = blockDim.x / S, sid = tid / S;
+    const int i0 = b * MD_TB, nown = min(P.N - i0, MD_TB);
+    for (int p0 = 0; p0 < nown; p0 += nslices) {
+        const int p = p0 + sid;
+        const bool act = p < nown;
+        const int i = i0 + p;
+        const int cnt = act ? B.row_count[i] : 0, lo = act ? B.lo_count[i] : 0;
+        const int me = bi.own_base + (act ? p : 0);
+        const float4 xi = st.spos[me];
+        float4 qi = make_float4(1.f, 0.f, 0.f, 0.f);
+        if (KIND == MD_POT_PATCHY) qi = st.squat[me];
+        const unsigned short* __restrict__ row = B.rows + (size_t)(act ? i : i0) * P.rcap;
+        float ax = 0.f, ay = 0.f, az = 0.f, ape = 0.f, atx = 0.f, aty = 0.f, atz = 0.f;
+        for (int k = lo + l; k < cnt; k += S) {
+            const int t = row[row_pos(k, S)];
+            const float4 xj = st.spos[t];
+            float dx, dy, dz;
+            if (IMG) {
+                dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+            } else {
+                dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+            }
+            const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            if (!in_cutoff(P, d2, xi, xj)) continue;        // no memory traffic for zero-force pairs
+            const int j = st.sslot[t];
+            float fx, fy, fz, V;
+            if (KIND == MD_POT_PATCHY) {
+                const float4 qj = st.squat[t];
+                float tix, tiy, tiz, tjx, tjy, tjz;
+                patchy_pair<true>(P, dx, dy, dz, d2, qi, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
+                atx += tix; aty += tiy; atz += tiz;
+                red_add_v4(torque + j, tjx, tjy, tjz, 0.f);
+            } else {
+                float g;
+                lj_pair(P, d2, g, V);
+                fx = g * dx; fy = g * dy; fz = g * dz;
+            }
+            const float hV = 0.5f * V;
+            ax -= fx; ay -= fy; az -= fz; ape += hV;
+            red_add_v4(force + j, fx, fy, fz, hV);
+        }
+        __syncwarp();
+        ax = slice_sum<S>(ax); ay = slice_sum<S>(ay); az = slice_sum<S>(az); ape = slice_sum<S>(ape);
+        if (KIND == MD_POT_PATCHY) { atx = slice_sum<S>(atx); aty = slice_sum<S>(aty); atz = slice_sum<S>(atz); }
+        if (act && l == 0 && cnt > lo) {   // one reduction per owning particle
+            red_add_v4(force + i, ax, ay, az, ape);
+            if (KIND == MD_POT_PATCHY) red_add_v4(torque + i, atx, aty, atz, 0.f);
+        }
+    }
+}
+
+template <int S, int KIND>
+__global__ void __launch_bounds__(256) k_edge_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
+                                                     const float4* __restrict__ quat, float4* force, float4* torque) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const int b = blockIdx.x;
+    const BlkInfo bi = B.blk[b];
+    if (bi.M <= 0 || bi.M + 1 > stage_entries) {
+        if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
+        return;
+    }
+    const Stage st = stage_block<KIND == MD_POT_PATCHY, true>(P, B, bi, b, stage_entries, pos, quat, smraw);
+    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) edge_rows<S, KIND, true>(P, B, bi, st, b, force, torque);
+    else edge_rows<S, KIND, false>(P, B, bi, st, b, force, torque);
+}
+
+__global__ void k_zero4_s(DevParams P, float4* a, float4* b) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < P.N) {
+        a[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (b) b[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+// S:A8 bonded pass for EDGE (C3): one thread per static bond (id, id+1), FENE only, scatter with red.v4
+__global__ void k_edge_bonds_s(DevParams P, DevBuffers B, const float4* __restrict__ pos, float4* force) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= P.N - 1 || (id % P.chain_len) == P.chain_len - 1) return;
+    const int i = B.slot_of_id[id], j = B.slot_of_id[id + 1];
+    const float4 xi = pos[i], xj = pos[j];
+    const float dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
+    const float dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
+    const float dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    float g, V;
+    if (!fene_pair(P, d2, g, V)) atomicOr(&B.ctrl->err, MD_DEVERR_FENE);
+    red_add_v4(force + i, -g * dx, -g * dy, -g * dz, 0.5f * V);
+    red_add_v4(force + j, g * dx, g * dy, g * dz, 0.5f * V);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-side dispatch
+// ------------------------------------------------------------------------------------------------
+size_t md_staged_smem_bytes(const md_system* s, int stage_entries, bool edge) {
+    size_t b = 16 + 16 * (size_t)stage_entries * (s->rigid ? 2 : 1);
+    if (edge) b += 4 * (size_t)stage_entries;
+    return b;
+}
+
+template <typename K>
+static void allow_big_smem(K kernel) {
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+}
+
+static void staged_attrs_once() {
+    static bool done = false;
+    if (done) return;
+    done = true;
+    allow_big_smem(k_vertex_lj_staged<4>);
+    allow_big_smem(k_vertex_lj_staged<8>);
+    allow_big_smem(k_vertex_patchy_staged<4>);
+    allow_big_smem(k_vertex_patchy_staged<8>);
+    allow_big_smem(k_edge_staged<4, MD_POT_LJ>);
+    allow_big_smem(k_edge_staged<8, MD_POT_LJ>);
+    allow_big_smem(k_edge_staged<4, MD_POT_PATCHY>);
+    allow_big_smem(k_edge_staged<8, MD_POT_PATCHY>);
+}
+
+// returns false if the staged path cannot serve this request (caller falls back to the explicit-list kernels)
+bool md_launch_forces_staged(md_system* s, int strategy, int scatter) {
+    const DevParams& P = s->P;
+    staged_attrs_once();
+    const int se = s->stage_launch;
+    const bool edge = strategy == MD_EDGE;
+    const size_t smem = md_staged_smem_bytes(s, se, edge);
+    if (smem > 224 * 1024) return false;
+    const int S = P.slice;
+    if (!edge) {
+        if (P.kind == MD_POT_PATCHY) {
+            if (S == 8) k_vertex_patchy_staged<8><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
+            else k_vertex_patchy_staged<4><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
+        } else {
+            if (S == 8) k_vertex_lj_staged<8><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+            else k_vertex_lj_staged<4><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+        }
+        s->launches += 1;
+        return true;
+    }
+    (void)scatter;
+    const int nbN = cdiv(P.N, 256);
+    float4* tq = P.kind == MD_POT_PATCHY ? s->torque : nullptr;
+    k_zero4_s<<<nbN, 256, 0, s->stream>>>(P, s->force, tq);
+    if (P.kind == MD_POT_PATCHY) {
+        if (S == 8) k_edge_staged<8, MD_POT_PATCHY><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, tq);
+        else k_edge_staged<4, MD_POT_PATCHY><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, tq);
+    } else {
+        if (S == 8) k_edge_staged<8, MD_POT_LJ><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, nullptr, s->force, tq);
+        else k_edge_staged<4, MD_POT_LJ><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, nullptr, s->force, tq);
+    }
+    s->launches += 2;
+    if (P.kind == MD_POT_FENE_WCA) {
+        k_edge_bonds_s<<<nbN, 256, 0, s->stream>>>(P, s->B, s->pos, s->force);
+        s->launches += 1;
+    }
+    return true;
+}

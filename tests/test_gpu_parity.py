@@ -8,7 +8,14 @@ import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = [("vertex", "red_v4"), ("edge", "red"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented")]
+# (strategy, variant): VERTEX gather alternatives {l2, smem}, EDGE scatter alternatives {red, red_v4, warp, segmented,
+# warp_smem}; the shared-memory staged variants need cell-sorted storage (order != none)
+VARIANTS = [("vertex", "l2"), ("edge", "red"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented")]
+STAGED = [("vertex", "smem"), ("edge", "warp_smem")]
+
+
+def variants(order):
+    return (STAGED + VARIANTS) if order != "none" else VARIANTS
 FTOL_REL, FTOL_ABS, ETOL = 1e-4, 1e-6, 1e-5
 
 
@@ -74,12 +81,14 @@ def test_step0_parity(MD, oracle, case, order):
     o = oracle.forces(w.pos, w.box, dict(w.potential), quat=w.quat)
     assert o["bad"] == 0
     results = {}
-    for strat, sc in VARIANTS:
+    for strat, sc in variants(order):
         s.forces(strat, sc)
         results[(strat, sc)] = assert_forces(s, o, w.quat is not None)
+    # the explicit global-slot lists (built on demand for the L2-gather variants) hold the same pair set
+    assert_pairs(s, oracle, w.pos, w.box, w.rcut, w.skin)
     # P11: the strategies agree with each other within twice the oracle tolerance
     fmax = np.abs(o["F"]).max()
-    ref = results[("vertex", "red_v4")]
+    ref = results[("vertex", "l2")]
     for k, F in results.items():
         assert np.abs(F[:, :3] - ref[:, :3]).max() <= 2 * (FTOL_REL * fmax + FTOL_ABS)
     # P7: Newton's third law survives fp32 accumulation
@@ -107,7 +116,7 @@ def test_vertex_and_segmented_are_bitwise_reproducible(MD):
     for rep in range(2):
         s = MD.from_workload(w, order="cell")
         s.build_cells(); s.build_verlet()
-        for strat, sc in [("vertex", "red_v4"), ("edge", "segmented")]:
+        for strat, sc in [("vertex", "l2"), ("vertex", "smem"), ("edge", "segmented")]:
             s.forces(strat, sc)
             F = s.in_id_order(s.force)
             if rep:
@@ -153,7 +162,8 @@ def test_error_paths(MD):
     s.close()
 
 
-@pytest.mark.parametrize("strat,sc", [("vertex", "red_v4"), ("edge", "warp"), ("edge", "segmented")])
+@pytest.mark.parametrize("strat,sc", [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp_smem"), ("edge", "warp"),
+                                      ("edge", "segmented")])
 def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
     """C1 (BASELINE.json configs[0]): 100 velocity-Verlet steps at dt = 0.002; fp32 GPU state against the fp64
     oracle trajectory from the same fp32 input.  SURVEY 8(d): the two stay within the force tolerance for 100 steps."""
@@ -178,9 +188,10 @@ def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
 
 
 @pytest.mark.parametrize("case,steps,strat,sc", [
-    ("lj", 300, "vertex", "red_v4"), ("lj", 300, "edge", "red_v4"),
-    ("polymer", 200, "vertex", "red_v4"), ("polymer", 200, "edge", "warp"),
-    ("patchy", 300, "vertex", "red_v4"), ("patchy", 300, "edge", "segmented")])
+    ("lj", 300, "vertex", "smem"), ("lj", 300, "vertex", "l2"), ("lj", 300, "edge", "red_v4"), ("lj", 300, "edge", "warp_smem"),
+    ("polymer", 200, "vertex", "smem"), ("polymer", 200, "edge", "warp"), ("polymer", 200, "edge", "warp_smem"),
+    ("patchy", 300, "vertex", "smem"), ("patchy", 300, "vertex", "l2"), ("patchy", 300, "edge", "segmented"),
+    ("patchy", 300, "edge", "warp_smem")])
 def test_snapshot_parity_after_device_side_rebuilds(MD, oracle, case, steps, strat, sc):
     """Run md_integrate long enough for several skin-triggered rebuilds, then compare the forces the path holds
     (computed from lists rebuilt on the device) with the oracle's plain definition on the SAME positions, and the
