@@ -32,7 +32,7 @@ import numpy as np
 
 METRIC = "pair interactions/s (Verlet pairs E per force evaluation / time), VERTEX vs EDGE, LJ N=2^20"
 UNIT = "pair interactions/s"
-EDGE_VARIANTS = ["red", "red_v4", "warp", "segmented", "warp_smem"]
+EDGE_VARIANTS = ["red", "red_v4", "warp", "segmented"]
 VERTEX_VARIANTS = ["smem", "l2"]
 
 
@@ -192,7 +192,7 @@ def main():
     ap.add_argument("--workload", default="C2a", choices=["C2a", "C2b"])
     ap.add_argument("--strategy", default="vertex", choices=["vertex", "edge"])
     ap.add_argument("--scatter", default=None, choices=EDGE_VARIANTS + VERTEX_VARIANTS,
-                    help="EDGE scatter variant (default warp_smem) or VERTEX gather variant (default smem)")
+                    help="EDGE scatter variant (default warp) or VERTEX gather variant (default smem)")
     ap.add_argument("--order", default="hilbert", choices=["none", "cell", "hilbert"])
     ap.add_argument("--melt-steps", type=int, default=300)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -201,9 +201,9 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
     if args.scatter is None:
-        args.scatter = "smem" if args.strategy == "vertex" else "warp_smem"
-    if args.order == "none" and args.scatter in ("smem", "warp_smem"):
-        args.scatter = "l2" if args.strategy == "vertex" else "warp"
+        args.scatter = "smem" if args.strategy == "vertex" else "warp"
+    if args.order == "none" and args.scatter == "smem":
+        args.scatter = "l2"
 
     import torch
     if not torch.cuda.is_available():
@@ -268,8 +268,6 @@ def main():
         t = time_calls(torch, lambda: s.forces("vertex", gv), 20)
         fe[f"vertex_{gv}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
     for sc in EDGE_VARIANTS:
-        if sc == "warp_smem" and args.order == "none":
-            continue
         t = time_calls(torch, lambda: s.forces("edge", sc), 10 if sc != "red" else 5)
         fe[f"edge_{sc}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
     best_vertex = min((k for k in fe if k.startswith("vertex")), key=lambda k: fe[k]["us"])
@@ -288,7 +286,7 @@ def main():
             traffic = json.loads(tf.read_text()).get(f"{args.workload}_{dom}")
         except Exception:
             traffic = None
-    kname = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp_smem": "k_edge_staged", "warp": "k_edge_warp",
+    kname = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp": "k_edge_warp",
              "red": "k_edge_red", "red_v4": "k_edge_red", "segmented": "k_edge_store+k_edge_segsum"}[args.scatter]
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,

@@ -63,16 +63,15 @@ typedef enum {
     MD_SCATTER_RED = 0,      /* red.global.add.f32, one per component                           */
     MD_SCATTER_RED_V4 = 1,   /* red.global.add.v4.f32, one per particle and output array        */
     MD_SCATTER_WARP = 2,     /* runs of equal owner i combined by warp shuffles, then one red.v4 */
-    MD_SCATTER_SEGMENTED = 3,/* per-edge store + atomic-free segmented reduction         */
-    MD_SCATTER_WARP_SMEM = 4 /* as WARP, neighbours read from the block's shared-memory staged neighbourhood
-                                instead of L2-resident gathers (needs MD_ORDER_CELL / MD_ORDER_HILBERT)   */
+    MD_SCATTER_SEGMENTED = 3 /* per-edge store + atomic-free segmented reduction         */
 } md_scatter;
 /* VERTEX gather alternatives (B:5 "neighbour positions staged through shared memory or L2-resident gathers"):
  * passed as the third argument of md_forces / md_integrate / md_step_host when strategy == MD_VERTEX. */
 typedef enum {
     MD_GATHER_AUTO = 0, /* SMEM when the storage is cell-sorted (an order is set), else L2 */
     MD_GATHER_L2 = 1,   /* one thread per particle, neighbour positions gathered from L1/L2 by global slot */
-    MD_GATHER_SMEM = 2  /* one 4- or 8-lane slice per particle, neighbourhood staged in shared memory by bulk TMA copies */
+    MD_GATHER_SMEM = 2  /* one thread per particle, the block's neighbourhood staged in shared memory by bulk TMA copies,
+                           16-bit block-local list entries ordered at build time for conflict-free 128-bit gathers */
 } md_gather;
 typedef enum { MD_ORDER_NONE = 0, MD_ORDER_CELL = 1, MD_ORDER_HILBERT = 2 } md_order;
 

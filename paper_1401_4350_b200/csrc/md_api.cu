@@ -17,7 +17,7 @@ struct Geometry {
     int64_t ncell;
     int cap, ntiles;
     size_t ecap;
-    int rcap, nblk, stage_cap, slice;   // staged path
+    int rcap, nblk, stage_cap;   // staged path
 };
 
 // S:Q8: n_k = max(1, floor(L_k / (r_v (1 + 1e-5)))) cells per axis, width >= r_v
@@ -36,9 +36,8 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
     g->ntiles = (int)((N + MD_TILE - 1) / MD_TILE);
     if ((int64_t)g->ntiles * MD_TILE * g->cap >= (1ll << 31)) return false;
     g->ecap = (size_t)N * g->cap / 2 + 64;
-    // staged path: rows of 16-bit local indices in chunks of 4*slice entries; smem capacity of the build kernel
+    // staged path: rows of 16-bit local indices in chunks of 4 entries; smem capacity of the build kernel
     g->rcap = (g->cap + 31) / 32 * 32;
-    g->slice = max_neigh >= 64 ? 8 : 4;
     g->nblk = (int)((N + MD_TB - 1) / MD_TB);
     {
         const double ppc = (double)N / (double)g->ncell;                 // particles per cell
@@ -46,7 +45,12 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
         const double side = cbrt(own) + 2.0;                               // stencil union of a compact blob, x1.5 for ragged shapes
         double m = 2.0 * (1.5 * side * side * side * ppc) + 256.0;
         m = std::min<double>(m, (double)N + 64.0);
-        m = std::min<double>(m, 11000.0);                                  // 16 B each: <= 176 KB of the 227 KB
+        // shared memory of the build kernel: positions (16 B each) + candidate/unique cell tables (md_staged.cu) <= 224 KB
+        int nc = 64;
+        while (nc < 27 * (2 * own + 4) && nc < MD_NCAND) nc <<= 1;
+        const int um = nc < MD_UMAX ? nc : MD_UMAX;
+        const double tables = 4.0 * (nc + 3.0 * um + 1 + MD_TB) + 32.0 * MD_TB + 16 + 1024;
+        m = std::min<double>(m, floor((224.0 * 1024 - tables) / 16.0) - 64.0);
         g->stage_cap = ((int)m + 63) / 64 * 64;
     }
     return true;
@@ -94,7 +98,8 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.e_out = (double*)take(8 * 4);
     b.stage4 = (float4*)take(16 * Npad);
     b.cell_lin = (int*)take(4 * (size_t)g.ncell);
-    b.rows = (unsigned short*)take(2 * Npad * (size_t)g.rcap);
+    b.rows = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);
+    b.rows_tmp = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);
     b.row_count = (int*)take(4 * Npad);
     b.lo_count = (int*)take(4 * Npad);
     b.blk = (BlkInfo*)take(sizeof(BlkInfo) * (size_t)g.nblk);
@@ -221,7 +226,7 @@ md_status sync_and_check(md_system* s, const char* where) {
     if (s->order != MD_ORDER_NONE && c.max_stage > 0) {
         // size the staged force launches from the largest neighbourhood seen, with 25 % head room for the
         // device-side rebuilds that happen before the next synchronising call
-        int want = (int)(c.max_stage * 1.25) + 64;
+        int want = (int)(c.max_stage * 1.15) + 64;
         want = (want + 63) / 64 * 64;
         s->stage_launch = want;
     }
@@ -281,7 +286,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.half_skin2 = (float)(0.25 * skin * skin);
     P.rv2 = (float)P.rv2d;
     P.band_rv = (float)(P.rv2d * 1e-6);    // S:Q6 band of the list predicate
-    P.nblk = g.nblk; P.slice = g.slice; P.stage_cap = g.stage_cap; P.rcap = g.rcap;
+    P.nblk = g.nblk; P.stage_cap = g.stage_cap; P.rcap = g.rcap; P.row_shift = g.stage_cap <= 4096 ? 4 : 0;
     P.skinf = (float)skin;
     s->stage_launch = g.stage_cap;
     P.kind = pot->kind;
@@ -299,6 +304,8 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
         bool shift = pot->shift_energy != 0 || pot->kind == MD_POT_FENE_WCA;   // WCA is always shifted (B:9)
         P.vshift = (pot->kind == MD_POT_PATCHY || !shift) ? 0.0f : (float)vc;
     }
+    P.k_nrc2 = make_float2(-P.rc2, -P.rc2); P.k_na = make_float2(-P.lj_a, -P.lj_a); P.k_b = make_float2(P.lj_b, P.lj_b);
+    P.k_c = make_float2(P.lj_c, P.lj_c); P.k_nd = make_float2(-P.lj_d, -P.lj_d); P.k_nvs = make_float2(-P.vshift, -P.vshift);
     if (rigid) {
         double rc = pot->rcut_core;
         double s2 = (double)pot->sigma * pot->sigma / (rc * rc), s6 = s2 * s2 * s2;
@@ -412,22 +419,21 @@ static void ensure_explicit(md_system* s) {
 // which list representation a (strategy, variant) pair runs on
 static bool wants_staged(const md_system* s, int32_t strategy, int32_t variant) {
     if (s->order == MD_ORDER_NONE) return false;
-    if (strategy == MD_VERTEX) return variant != MD_GATHER_L2;
-    return variant == MD_SCATTER_WARP_SMEM;
+    return strategy == MD_VERTEX && variant != MD_GATHER_L2;
 }
 
 static md_status check_strategy(md_system* s, int32_t strategy, int32_t scatter) {
     if (strategy != MD_VERTEX && strategy != MD_EDGE) return fail(s, MD_ERR_INVALID, "unknown strategy");
-    if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_WARP_SMEM)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
+    if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_SEGMENTED)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
     if (strategy == MD_VERTEX && (scatter < MD_GATHER_AUTO || scatter > MD_GATHER_SMEM)) return fail(s, MD_ERR_INVALID, "unknown gather variant");
-    if (s->order == MD_ORDER_NONE && ((strategy == MD_VERTEX && scatter == MD_GATHER_SMEM) || (strategy == MD_EDGE && scatter == MD_SCATTER_WARP_SMEM)))
-        return fail(s, MD_ERR_STATE, "the shared-memory staged variants need cell-sorted storage: md_set_order(MD_ORDER_CELL or MD_ORDER_HILBERT)");
+    if (s->order == MD_ORDER_NONE && strategy == MD_VERTEX && scatter == MD_GATHER_SMEM)
+        return fail(s, MD_ERR_STATE, "the shared-memory staged variant needs cell-sorted storage: md_set_order(MD_ORDER_CELL or MD_ORDER_HILBERT)");
     return MD_OK;
 }
 
 static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatter) {
     if (wants_staged(s, strategy, scatter)) {
-        if (!md_launch_forces_staged(s, strategy, scatter)) return fail(s, MD_ERR_CAPACITY, "staged neighbourhood does not fit in shared memory");
+        if (!md_launch_forces_staged(s)) return fail(s, MD_ERR_CAPACITY, "staged neighbourhood does not fit in shared memory");
     } else {
         md_launch_forces(s, strategy, scatter);
     }

@@ -15,9 +15,9 @@
 #define MD_DEVERR_STAGE 4     // a block's staged neighbourhood / segment table exceeds its capacity
 
 // ---- shared-memory staged path (md_staged.cu) ----
-#define MD_TB 128             // particles per block (consecutive slots of the cell-sorted storage)
-#define MD_NCAND 4096         // candidate cells per block before sort + unique (27 x non-empty own cells <= 27 x MD_TB)
-#define MD_UMAX 2048          // distinct cells in a block's neighbourhood
+#define MD_TB 256             // particles per block (consecutive slots of the cell-sorted storage)
+#define MD_NCAND 8192         // candidate cells per block before sort + unique (27 x non-empty own cells <= 27 x MD_TB)
+#define MD_UMAX 4096          // distinct cells in a block's neighbourhood
 #define MD_SEGMAX 1024        // contiguous slot segments per block
 // BlkInfo flags
 #define MD_BLK_WRAP 1         // some listed pair of the block crosses a periodic face
@@ -58,13 +58,15 @@ struct DevParams {
     float rc2, band_abs;               // fp32 cutoff and the half-width of the fp64-recheck band |d2 - rc2| (S:H10)
     float half_skin2;                  // (skin/2)^2
     float rv2, band_rv;                // fp32 list radius^2 and its fp64-recheck band (S:Q6)
-    int nblk, slice, stage_cap, rcap;  // staged path: blocks of MD_TB slots, lanes per particle, smem capacity (particles), row stride
+    int nblk, stage_cap, rcap, row_shift;   // staged path: blocks of MD_TB slots, smem capacity (particles), row capacity (entries),
+                                            // row entries = local index << row_shift (4 = byte offset of the float4, when stage_cap <= 4096)
     float skinf;
     // pair potential
     int kind;
     float eps, sig2, mass, inv_mass;
     float c48, c24, c4, vshift;        // 48 eps, 24 eps, 4 eps, V_c
     float lj_a, lj_b, lj_c, lj_d;      // 48 eps sigma^12, 24 eps sigma^6, 4 eps sigma^12, 4 eps sigma^6
+    float2 k_nrc2, k_na, k_b, k_c, k_nd, k_nvs;   // duplicated constants of the packed (f32x2) LJ visit: -rc2, -lj_a, lj_b, lj_c, -lj_d, -vshift
     // WCA core of the patchy potential
     float core_rc2, core_vshift;
     // FENE
@@ -107,9 +109,10 @@ struct DevBuffers {
     float4* stage4;        // [N] staging for md_step_host un-permute
     // staged path
     int* cell_lin;         // [ncell] storage rank -> linear cell index (inverse of cell_rank)
-    unsigned short* rows;  // [Npad*cap] per-particle Verlet rows of block-local indices, slice-transposed chunks
+    unsigned short* rows;  // [nblk][rcap/4][MD_TB] x 4 u16: Verlet rows of block-local indices, block-transposed chunks of 4
+    unsigned short* rows_tmp; // [nblk*MD_TB*rcap] build scratch: rows in scan order
     int* row_count;        // [Npad] |L_i|
-    int* lo_count;         // [Npad] neighbours with slot < i (the EDGE half list is the suffix of the row)
+    int* lo_count;         // [Npad] neighbours with slot < i
     BlkInfo* blk;          // [nblk]
     int2* seg;             // [nblk*MD_SEGMAX] (first slot, first local index)
 };
@@ -150,7 +153,7 @@ void md_launch_unpermute(md_system* s, const float4* src, float4* dst);   // dst
 // staged path (md_staged.cu)
 void md_launch_build_staged(md_system* s, bool gated);
 void md_launch_edges_from_rows(md_system* s);     // explicit (i, j) edge list from the staged rows (export / legacy EDGE variants)
-bool md_launch_forces_staged(md_system* s, int strategy, int scatter);
-size_t md_staged_smem_bytes(const md_system* s, int stage_entries, bool edge);
+bool md_launch_forces_staged(md_system* s);             // VERTEX on the staged rows
+size_t md_staged_smem_bytes(const md_system* s, int stage_entries);
 
 #define MD_ERRBUF(s, ...) snprintf((s)->errmsg, sizeof((s)->errmsg), __VA_ARGS__)

@@ -43,13 +43,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
                  ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-// position of sorted entry k inside a row: chunks of 4*S entries, lane l of the slice owns 4 consecutive u16
-// (one 64-bit load) holding the entries of 4 successive iterations
-__device__ __forceinline__ int row_pos(int k, int S) {
-    const int c4 = 4 * S, r = k % c4;
-    return (k - r) + (r % S) * 4 + r / S;
-}
-
 #define DUMMY_COORD 1.0e15f   // the padding entry of every staged neighbourhood: d2 ~ 3e30, never inside a cutoff
 
 // ------------------------------------------------------------------------------------------------
@@ -117,7 +110,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     const int n = 27 * nownc;
     int n2 = 32;
     while (n2 < n) n2 <<= 1;
-    if (n2 > ncand_cap) {   // cannot happen for n <= 27*MD_TB = 3456 <= MD_NCAND unless the launch was sized smaller
+    if (n2 > ncand_cap) {   // cannot happen for n <= 27*MD_TB <= MD_NCAND unless the launch was sized smaller
         if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
         if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
         return;
@@ -234,13 +227,19 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     if (tid == 0) s_flags = 0;   // from here on: bit 0 = a listed pair wraps, bits 2..4 = axes, bit 5 = shift transform fails
     __syncthreads();
 
-    // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6), rows sorted by slot
+    // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6).  Pass A writes the
+    //    neighbours in scan order (ascending local index = ascending slot) to a thread-private scratch row and counts
+    //    them per shared-memory bank column (local index mod 8: one float4 = one of the 8 16-byte columns of a wavefront).
+    unsigned short* s_rem = reinterpret_cast<unsigned short*>(own_rank + MD_TB);   // [8][MD_TB] entries left per column
+    unsigned short* s_cur = s_rem + 8 * MD_TB;                                        // [8][MD_TB] scan cursor per column
     int cnt = 0, lo_cnt = 0, flags = 0;
+    float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
+    unsigned short* __restrict__ tmp = B.rows_tmp + (size_t)(live ? i : i0) * P.rcap;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) { s_rem[c * MD_TB + tid] = 0; s_cur[c * MD_TB + tid] = 0; }
     if (live) {
         const int me = own_base + tid;
-        const float4 xi = spos[me];
-        const int S = P.slice;
-        unsigned short* __restrict__ row = B.rows + (size_t)i * P.rcap;
+        xi = spos[me];
         const int lin = B.cell_lin[myrank];
         const int cx = lin / (P.ncz * P.ncy), cy = (lin / P.ncz) % P.ncy, cz = lin % P.ncz;
         const float hLx = P.hLx, hLy = P.hLy, hLz = P.hLz;
@@ -264,7 +263,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                 bool in = tt < 0.0f;
                 if (fabsf(tt) < P.band_rv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
                 if (in) {
-                    if (cnt < P.cap) row[row_pos(cnt, S)] = (unsigned short)t;
+                    if (cnt < P.cap) { tmp[cnt] = (unsigned short)t; s_rem[(t & 7) * MD_TB + tid] += 1; }
                     ++cnt;
                     lo_cnt += (t < me);
                     if (maywrap) {
@@ -288,12 +287,45 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
             }
         }
         if (cnt > P.cap) atomicOr(&B.ctrl->err, MD_DEVERR_CAPACITY);
+    }
+    // 8b. Pass B: emit the row in the order the force kernels read it.  Thread tid (lane p of its quarter-warp) reads
+    //     entry k at the same time as the 7 other lanes of the quarter read theirs; a 128-bit shared-memory gather is
+    //     conflict-free when the 8 lanes hit 8 different columns, so lane p takes, at step k, a neighbour of column
+    //     (k + p) mod 8 while it has one (else of its fullest column).  Row layout: block-transposed chunks of four
+    //     16-bit local indices, rows[((b * nchunk) + k/4) * MD_TB + tid] -> one coalesced 64-bit load per 4 visits.
+    {
         const int c2 = min(cnt, P.cap);
-        for (int k = c2; k < ((c2 + S - 1) / S) * S; ++k) row[row_pos(k, S)] = (unsigned short)M;   // dummy padding
-        B.row_count[i] = c2;
-        B.lo_count[i] = cnt > P.cap ? 0 : lo_cnt;
-        B.half_count[i] = cnt > P.cap ? 0 : cnt - lo_cnt;
-        B.pos_ref[i] = xi;
+        const int nchunk = P.rcap >> 2;
+        uint2* __restrict__ rowb = reinterpret_cast<uint2*>(B.rows) + (size_t)b * nchunk * MD_TB + tid;
+        unsigned int w[4] = { 0u, 0u, 0u, 0u };
+        const unsigned int dummy = (unsigned int)M << P.row_shift;
+        for (int k0 = 0; k0 < c2; k0 += 4) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int k = k0 + q;
+                unsigned int t = dummy;
+                if (k < c2) {
+                    int c = (k + tid) & 7;
+                    if (s_rem[c * MD_TB + tid] == 0) {
+                        int bv = 0;
+                        for (int cc = 0; cc < 8; ++cc) { const int v = s_rem[cc * MD_TB + tid]; if (v > bv) { bv = v; c = cc; } }
+                    }
+                    int pos = s_cur[c * MD_TB + tid];
+                    while ((tmp[pos] & 7) != c) ++pos;
+                    t = (unsigned int)tmp[pos] << P.row_shift;
+                    s_cur[c * MD_TB + tid] = (unsigned short)(pos + 1);
+                    s_rem[c * MD_TB + tid] -= 1;
+                }
+                w[q] = t;
+            }
+            rowb[(size_t)(k0 >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+        }
+        if (live) {
+            B.row_count[i] = c2;
+            B.lo_count[i] = cnt > P.cap ? 0 : lo_cnt;
+            B.half_count[i] = cnt > P.cap ? 0 : cnt - lo_cnt;
+            B.pos_ref[i] = xi;
+        }
     }
     if (flags) atomicOr(&s_flags, flags);
     // 9. block totals
@@ -340,7 +372,7 @@ static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, si
     int um = nc < MD_UMAX ? nc : MD_UMAX;
     *ncand_cap = nc;
     *umax = um;
-    *smem = 16 * (size_t)P.stage_cap + 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 16;
+    *smem = 16 * (size_t)P.stage_cap + 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 2 * 2 * 8 * MD_TB + 16;
 }
 
 void md_launch_build_staged(md_system* s, bool gated) {
@@ -361,8 +393,15 @@ void md_launch_build_staged(md_system* s, bool gated) {
 
 // ------------------------------------------------------------------------------------------------
 // explicit (i, j) edge list from the staged rows: i < j slots, sorted by i, bit 31 of j = periodic image flag.
-// Used by md_get_pairs (list parity export).  Needs edge_off = exclusive scan of half_count.
+// Used by md_get_pairs (list parity export).  Needs edge_off = exclusive scan of half_count.  Local indices
+// ascend with the slot, so the half list (i < j) of particle i is { t in row : t > own local index }.
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned int row_entry(const uint2* __restrict__ rowb, int k, int shift) {
+    const uint2 pk = rowb[(size_t)(k >> 2) * MD_TB];
+    const unsigned int w = (k & 2) ? pk.y : pk.x;
+    return ((k & 1) ? (w >> 16) : (w & 0xffffu)) >> shift;   // local index
+}
+
 __global__ void __launch_bounds__(MD_TB) k_edges_from_rows(DevParams P, DevBuffers B, const float4* __restrict__ pos) {
     extern __shared__ __align__(16) unsigned char smraw[];
     int* sslot = reinterpret_cast<int*>(smraw);   // [M]
@@ -377,12 +416,14 @@ __global__ void __launch_bounds__(MD_TB) k_edges_from_rows(DevParams P, DevBuffe
     __syncthreads();
     const int i = b * MD_TB + tid;
     if (i >= P.N) return;
-    const int cnt = B.row_count[i], lo = B.lo_count[i], S = P.slice;
-    const unsigned short* __restrict__ row = B.rows + (size_t)i * P.rcap;
+    const int cnt = B.row_count[i], me = bi.own_base + tid;
+    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + tid;
     const float4 xi = pos[i];
     unsigned int o = B.edge_off[i];
-    for (int k = lo; k < cnt; ++k) {
-        const int j = sslot[row[row_pos(k, S)]];
+    for (int k = 0; k < cnt; ++k) {
+        const int t = (int)row_entry(rowb, k, P.row_shift);
+        if (t <= me) continue;
+        const int j = sslot[t];
         const float4 xj = pos[j];
         const int w = (fabsf(xj.x - xi.x) > P.hLx) | (fabsf(xj.y - xi.y) > P.hLy) | (fabsf(xj.z - xi.z) > P.hLz);
         B.edges[o++] = make_int2(i, j | (w << 31));
@@ -406,17 +447,15 @@ void md_launch_edges_from_rows(md_system* s) {
 struct Stage {
     float4* spos;    // [M + 1]  (entry M = dummy)
     float4* squat;   // [M + 1]  rigid bodies only
-    int* sslot;      // [M]      EDGE only: local index -> slot
 };
 
-template <bool QUAT, bool SLOT>
+template <bool QUAT>
 __device__ __forceinline__ Stage stage_block(const DevParams& P, const DevBuffers& B, const BlkInfo bi, int b, int stage_entries,
                                              const float4* __restrict__ pos, const float4* __restrict__ quat, unsigned char* smraw) {
     Stage st;
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(smraw);
     st.spos = reinterpret_cast<float4*>(smraw + 16);
     st.squat = QUAT ? st.spos + stage_entries : nullptr;
-    st.sslot = SLOT ? reinterpret_cast<int*>(st.spos + (QUAT ? 2 : 1) * (size_t)stage_entries) : nullptr;
     const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
     const int tid = threadIdx.x;
     if (tid < 32) {
@@ -431,18 +470,12 @@ __device__ __forceinline__ Stage stage_block(const DevParams& P, const DevBuffer
             bulk_g2s(st.spos + s0.y, pos + s0.x, (unsigned)len * 16u, bar);
             if (QUAT) bulk_g2s(st.squat + s0.y, quat + s0.x, (unsigned)len * 16u, bar);
         }
-    } else if (SLOT) {
-        for (int sg = (tid >> 5) - 1; sg < bi.nseg; sg += (blockDim.x >> 5) - 1) {
-            const int2 s0 = seg[sg];
-            const int len = (sg + 1 < bi.nseg ? seg[sg + 1].y : bi.M) - s0.y;
-            for (int k = tid & 31; k < len; k += 32) st.sslot[s0.y + k] = s0.x + k;
-        }
     }
     if (tid == 32) {
         st.spos[bi.M] = make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
         if (QUAT) st.squat[bi.M] = make_float4(1.f, 0.f, 0.f, 0.f);
     }
-    __syncthreads();          // barrier initialised, slot map and dummy written
+    __syncthreads();          // barrier initialised, dummy written
     mbar_wait(bar, 0);        // all segments have landed
     // periodic blocks: shift the upper half of the box down by L on the wrapped axes (exact in fp32: Sterbenz),
     // after which plain differences ARE the minimum images (verified pair by pair at build time)
@@ -460,62 +493,61 @@ __device__ __forceinline__ Stage stage_block(const DevParams& P, const DevBuffer
     return st;
 }
 
-// slice-wide sums (S a power of two <= 32; all 32 lanes participate)
-template <int S>
-__device__ __forceinline__ float slice_sum(float v) {
-#pragma unroll
-    for (int o = S / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-template <int S>
-__device__ __forceinline__ int slice_sum_i(int v) {
-#pragma unroll
-    for (int o = S / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-template <int S>
-__device__ __forceinline__ float slice_min(float v) {
-#pragma unroll
-    for (int o = S / 2; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
+// ------------------------------------------------------------------------------------------------
+// VERTEX, LJ / WCA (+ FENE bonds), staged (S:A6): one thread per particle loops over its row; neighbour
+// positions come from the block's shared-memory neighbourhood by 128-bit gathers whose bank columns were
+// de-conflicted at build time (k_build_staged pass B).  No atomics, every pair computed twice.
+// ------------------------------------------------------------------------------------------------
+struct LJAccS { float fx, fy, fz, band; float2 pe; };
+
+// staged position of a row entry: entries hold (local index << SH); SH == 4 makes the entry the byte offset
+template <int SH>
+__device__ __forceinline__ float4 staged_pos(const float4* sp, unsigned int e) {
+    if (SH == 4) return *reinterpret_cast<const float4*>(reinterpret_cast<const char*>(sp) + e);
+    return sp[e];
 }
 
-// ------------------------------------------------------------------------------------------------
-// VERTEX, LJ / WCA (+ FENE bonds), staged (S:A6)
-// ------------------------------------------------------------------------------------------------
-struct LJAccS { float fx, fy, fz, pe, band; int nin; };
-
+// Two visits (a, b) at once.  Distances and the force accumulation are scalar fp32; the chain in between --
+// cutoff mask, 1/d2, s6, force and energy polynomials -- runs on both visits with packed f32x2 instructions
+// (FADD2 / FMUL2 / FFMA2: half the issue slots).  The cutoff enters as a 0/1 mask m (no branch, no select):
+// s = m / d2, so force and energy of an outside pair are exactly zero; the energy shift is -m V_c.
+// `band` tracks min |d2 - rc^2| for the fp64 recheck (S:H10).
 template <bool IMG>
-__device__ __forceinline__ void lj_visit_s(const DevParams& P, float4 xi, float4 xj, LJAccS& a) {
-    float dx, dy, dz;
+__device__ __forceinline__ void lj_visit2_s(const DevParams& P, float4 xi, float4 xa, float4 xb, LJAccS& a) {
+    float dxa, dya, dza, dxb, dyb, dzb;
     if (IMG) {
-        dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+        dxa = min_image(xa.x, xi.x, P.Lx, P.hLx); dya = min_image(xa.y, xi.y, P.Ly, P.hLy); dza = min_image(xa.z, xi.z, P.Lz, P.hLz);
+        dxb = min_image(xb.x, xi.x, P.Lx, P.hLx); dyb = min_image(xb.y, xi.y, P.Ly, P.hLy); dzb = min_image(xb.z, xi.z, P.Lz, P.hLz);
     } else {
-        dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+        dxa = xa.x - xi.x; dya = xa.y - xi.y; dza = xa.z - xi.z;
+        dxb = xb.x - xi.x; dyb = xb.y - xi.y; dzb = xb.z - xi.z;
     }
-    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const float t = d2 - P.rc2;
-    const bool in = t < 0.0f;
-    a.band = fminf(a.band, fabsf(t));
-    const float inv = rcp_approx(d2);
-    float inv3 = inv * inv * inv;
-    inv3 = in ? inv3 : 0.0f;
-    const float g = inv * inv3 * fmaf(P.lj_a, inv3, -P.lj_b);     // 24 eps s6 (2 s6 - 1) / d2
-    a.fx = fmaf(-g, dx, a.fx); a.fy = fmaf(-g, dy, a.fy); a.fz = fmaf(-g, dz, a.fz);
-    a.pe = fmaf(inv3, fmaf(P.lj_c, inv3, -P.lj_d), a.pe);        // 4 eps s6 (s6 - 1); the shift is nin * V_c
-    a.nin += in ? 1 : 0;
+    const float2 d2 = make_float2(fmaf(dza, dza, fmaf(dya, dya, dxa * dxa)), fmaf(dzb, dzb, fmaf(dyb, dyb, dxb * dxb)));
+    const float2 t = __fadd2_rn(d2, P.k_nrc2);
+    const float2 m = make_float2(t.x < 0.0f ? 1.0f : 0.0f, t.y < 0.0f ? 1.0f : 0.0f);
+    a.band = fminf(fminf(a.band, fabsf(t.x)), fabsf(t.y));
+    const float2 inv = make_float2(rcp_approx(d2.x), rcp_approx(d2.y));
+    const float2 s = __fmul2_rn(inv, m);                       // m / d2
+    const float2 s2 = __fmul2_rn(s, s);
+    const float2 u = __fmul2_rn(s2, s);                        // m / d2^3  (sigma^-6 s6)
+    const float2 w = __fmul2_rn(s2, s2);                       // m / d2^4
+    const float2 ng = __fmul2_rn(w, __ffma2_rn(P.k_na, u, P.k_b));   // -24 eps s6 (2 s6 - 1) / d2
+    a.fx = fmaf(ng.x, dxa, a.fx); a.fy = fmaf(ng.x, dya, a.fy); a.fz = fmaf(ng.x, dza, a.fz);
+    a.fx = fmaf(ng.y, dxb, a.fx); a.fy = fmaf(ng.y, dyb, a.fy); a.fz = fmaf(ng.y, dzb, a.fz);
+    a.pe = __ffma2_rn(u, __ffma2_rn(P.k_c, u, P.k_nd), a.pe);  // 4 eps s6 (s6 - 1)
+    a.pe = __ffma2_rn(m, P.k_nvs, a.pe);                       // - V_c
 }
 
-// rare path: a visit of this particle fell inside the fp64-recheck band -> one lane redoes the particle with the
+// rare path: a visit of this particle fell inside the fp64-recheck band -> redo the particle with the
 // S:O0 / S:Q5 decision for every banded pair
-__device__ __noinline__ void lj_careful_s(const float4* spos, const unsigned short* __restrict__ row, int cnt, int S, float4 xi,
+__device__ __noinline__ void lj_careful_s(const float4* spos, const uint2* __restrict__ rowb, int cnt, int shift, float4 xi,
                                           float Lx, float Ly, float Lz, float rc2, float band_abs, float lj_a, float lj_b,
                                           float lj_c, float lj_d, float vshift, double dLx, double dLy, double dLz, double rc2d,
                                           float4* out) {
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f;
     int nin = 0;
     for (int k = 0; k < cnt; ++k) {
-        const float4 xj = spos[row[row_pos(k, S)]];
+        const float4 xj = spos[row_entry(rowb, k, shift)];
         const float dx = min_image(xj.x, xi.x, Lx, 0.5f * Lx);
         const float dy = min_image(xj.y, xi.y, Ly, 0.5f * Ly);
         const float dz = min_image(xj.z, xi.z, Lz, 0.5f * Lz);
@@ -557,62 +589,48 @@ __device__ __forceinline__ void fene_vertex_s(const DevParams& P, const DevBuffe
     }
 }
 
-template <int S, bool IMG>
+template <bool IMG, int SH>
 __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
                                                const float4* __restrict__ pos, float4* __restrict__ force, bool bonds) {
-    const int tid = threadIdx.x, l = tid & (S - 1);
-    const int nslices = blockDim.x / S, sid = tid / S;
-    const int i0 = b * MD_TB, nown = min(P.N - i0, MD_TB);
-    for (int p0 = 0; p0 < nown; p0 += nslices) {          // warp-uniform
-        const int p = p0 + sid;
-        const bool act = p < nown;
-        const int i = i0 + p;
-        const int cnt = act ? B.row_count[i] : 0;
-        const float4 xi = st.spos[bi.own_base + (act ? p : 0)];
-        const uint2* __restrict__ row = reinterpret_cast<const uint2*>(B.rows + (size_t)(act ? i : i0) * P.rcap) + l;
-        const int iters = (cnt + S - 1) / S;
-        LJAccS a = { 0.f, 0.f, 0.f, 0.f, 3.0e38f, 0 };
-        int it = 0;
-        uint2 pk = iters > 0 ? __ldg(row) : make_uint2(0u, 0u);
-        for (; it + 4 <= iters; it += 4) {
-            const uint2 cur = pk;
-            if (it + 4 < iters) pk = __ldg(row + (it / 4 + 1) * S);
-            const float4 x0 = st.spos[cur.x & 0xffffu], x1 = st.spos[cur.x >> 16], x2 = st.spos[cur.y & 0xffffu], x3 = st.spos[cur.y >> 16];
-            lj_visit_s<IMG>(P, xi, x0, a);
-            lj_visit_s<IMG>(P, xi, x1, a);
-            lj_visit_s<IMG>(P, xi, x2, a);
-            lj_visit_s<IMG>(P, xi, x3, a);
-        }
-        if (it < iters) {                                  // 1..3 remaining iterations of the last chunk
-            const int rem = iters - it;
-            lj_visit_s<IMG>(P, xi, st.spos[pk.x & 0xffffu], a);
-            if (rem > 1) lj_visit_s<IMG>(P, xi, st.spos[pk.x >> 16], a);
-            if (rem > 2) lj_visit_s<IMG>(P, xi, st.spos[pk.y & 0xffffu], a);
-        }
-        __syncwarp();
-        a.fx = slice_sum<S>(a.fx); a.fy = slice_sum<S>(a.fy); a.fz = slice_sum<S>(a.fz); a.pe = slice_sum<S>(a.pe);
-        a.nin = slice_sum_i<S>(a.nin); a.band = slice_min<S>(a.band);
-        if (act && l == 0) {
-            if (a.band < P.band_abs) {
-                lj_careful_s(st.spos, B.rows + (size_t)i * P.rcap, cnt, S, xi, P.Lx, P.Ly, P.Lz, P.rc2, P.band_abs, P.lj_a, P.lj_b,
-                             P.lj_c, P.lj_d, P.vshift, P.dLx, P.dLy, P.dLz, P.rc2d, force + i);
-                const float4 r = force[i];
-                a.fx = r.x; a.fy = r.y; a.fz = r.z; a.pe = r.w; a.nin = 0;
-            }
-            float pe = 0.5f * fmaf(-(float)a.nin, P.vshift, a.pe);
-            if (bonds) {
-                float bpe = 0.f;
-                fene_vertex_s(P, B, pos, i, a.fx, a.fy, a.fz, bpe);
-                pe += 0.5f * bpe;
-            }
-            force[i] = make_float4(a.fx, a.fy, a.fz, pe);
-        }
+    const int tid = threadIdx.x;
+    const int i = b * MD_TB + tid;
+    if (i >= P.N) return;
+    const int cnt = B.row_count[i];
+    const float4 xi = st.spos[bi.own_base + tid];
+    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + tid;
+    const float4* sp = st.spos;
+    const int nch = (cnt + 3) >> 2;                        // the last chunk is padded with the dummy entry
+    LJAccS a = { 0.f, 0.f, 0.f, 3.0e38f, make_float2(0.f, 0.f) };
+    // row chunks are prefetched two ahead (HBM latency is ~2 chunks of arithmetic at this occupancy)
+    uint2 pk = nch > 0 ? __ldg(rowb) : make_uint2(0u, 0u);
+    uint2 pk2 = nch > 1 ? __ldg(rowb + MD_TB) : make_uint2(0u, 0u);
+    for (int c = 0; c < nch; ++c) {
+        const uint2 cur = pk;
+        pk = pk2;
+        if (c + 2 < nch) pk2 = __ldg(rowb + (size_t)(c + 2) * MD_TB);
+        const float4 x0 = staged_pos<SH>(sp, cur.x & 0xffffu), x1 = staged_pos<SH>(sp, cur.x >> 16);
+        const float4 x2 = staged_pos<SH>(sp, cur.y & 0xffffu), x3 = staged_pos<SH>(sp, cur.y >> 16);
+        lj_visit2_s<IMG>(P, xi, x0, x1, a);
+        lj_visit2_s<IMG>(P, xi, x2, x3, a);
     }
+    float pe2 = a.pe.x + a.pe.y;
+    if (a.band < P.band_abs) {
+        lj_careful_s(st.spos, rowb, cnt, SH, xi, P.Lx, P.Ly, P.Lz, P.rc2, P.band_abs, P.lj_a, P.lj_b,
+                     P.lj_c, P.lj_d, P.vshift, P.dLx, P.dLy, P.dLz, P.rc2d, force + i);
+        const float4 r = force[i];
+        a.fx = r.x; a.fy = r.y; a.fz = r.z; pe2 = r.w;
+    }
+    float pe = 0.5f * pe2;
+    if (bonds) {
+        float bpe = 0.f;
+        fene_vertex_s(P, B, pos, i, a.fx, a.fy, a.fz, bpe);
+        pe += 0.5f * bpe;
+    }
+    force[i] = make_float4(a.fx, a.fy, a.fz, pe);
 }
 
-template <int S>
-__global__ void __launch_bounds__(256) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
-                                                          float4* __restrict__ force) {
+__global__ void __launch_bounds__(MD_TB) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
+                                                            float4* __restrict__ force) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int b = blockIdx.x;
     const BlkInfo bi = B.blk[b];
@@ -620,63 +638,69 @@ __global__ void __launch_bounds__(256) k_vertex_lj_staged(DevParams P, DevBuffer
         if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
         return;
     }
-    const Stage st = stage_block<false, false>(P, B, bi, b, stage_entries, pos, nullptr, smraw);
+    const Stage st = stage_block<false>(P, B, bi, b, stage_entries, pos, nullptr, smraw);
     const bool bonds = P.kind == MD_POT_FENE_WCA;
-    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_lj_rows<S, true>(P, B, bi, st, b, pos, force, bonds);
-    else vertex_lj_rows<S, false>(P, B, bi, st, b, pos, force, bonds);
+    const bool img = (bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK);
+    if (P.row_shift == 4) {
+        if (img) vertex_lj_rows<true, 4>(P, B, bi, st, b, pos, force, bonds);
+        else vertex_lj_rows<false, 4>(P, B, bi, st, b, pos, force, bonds);
+    } else {
+        if (img) vertex_lj_rows<true, 0>(P, B, bi, st, b, pos, force, bonds);
+        else vertex_lj_rows<false, 0>(P, B, bi, st, b, pos, force, bonds);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
-// VERTEX, patchy rigid bodies, staged
+// VERTEX, patchy rigid bodies, staged: positions and quaternions of the neighbourhood in shared memory
 // ------------------------------------------------------------------------------------------------
-template <int S, bool IMG>
+template <bool IMG>
+__device__ __forceinline__ void patchy_visit_s(const DevParams& P, const Stage& st, float4 xi, float4 qi, unsigned int t,
+                                               float& fx, float& fy, float& fz, float& pe, float& tx, float& ty, float& tz) {
+    const float4 xj = st.spos[t];
+    float dx, dy, dz;
+    if (IMG) {
+        dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+    } else {
+        dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+    }
+    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (in_cutoff(P, d2, xi, xj)) {
+        const float4 qj = st.squat[t];
+        float gx, gy, gz, V, a, bb, c, u, v, w;
+        patchy_pair<false>(P, dx, dy, dz, d2, qi, qj, gx, gy, gz, V, a, bb, c, u, v, w);
+        fx -= gx; fy -= gy; fz -= gz;
+        tx += a; ty += bb; tz += c;
+        pe += V;
+    }
+}
+
+template <bool IMG>
 __device__ __forceinline__ void vertex_patchy_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
                                                    float4* __restrict__ force, float4* __restrict__ torque) {
-    const int tid = threadIdx.x, l = tid & (S - 1);
-    const int nslices = blockDim.x / S, sid = tid / S;
-    const int i0 = b * MD_TB, nown = min(P.N - i0, MD_TB);
-    for (int p0 = 0; p0 < nown; p0 += nslices) {
-        const int p = p0 + sid;
-        const bool act = p < nown;
-        const int i = i0 + p;
-        const int cnt = act ? B.row_count[i] : 0;
-        const int me = bi.own_base + (act ? p : 0);
-        const float4 xi = st.spos[me], qi = st.squat[me];
-        const unsigned short* __restrict__ row = B.rows + (size_t)(act ? i : i0) * P.rcap;
-        float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
-        for (int k = l; k < cnt; k += S) {
-            const int t = row[row_pos(k, S)];
-            const float4 xj = st.spos[t];
-            float dx, dy, dz;
-            if (IMG) {
-                dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
-            } else {
-                dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
-            }
-            const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (in_cutoff(P, d2, xi, xj)) {
-                const float4 qj = st.squat[t];
-                float gx, gy, gz, V, a, bb, c, u, v, w;
-                patchy_pair<false>(P, dx, dy, dz, d2, qi, qj, gx, gy, gz, V, a, bb, c, u, v, w);
-                fx -= gx; fy -= gy; fz -= gz;
-                tx += a; ty += bb; tz += c;
-                pe += V;
-            }
-        }
-        __syncwarp();
-        fx = slice_sum<S>(fx); fy = slice_sum<S>(fy); fz = slice_sum<S>(fz); pe = slice_sum<S>(pe);
-        tx = slice_sum<S>(tx); ty = slice_sum<S>(ty); tz = slice_sum<S>(tz);
-        if (act && l == 0) {
-            force[i] = make_float4(fx, fy, fz, 0.5f * pe);
-            torque[i] = make_float4(tx, ty, tz, 0.f);
-        }
+    const int tid = threadIdx.x;
+    const int i = b * MD_TB + tid;
+    if (i >= P.N) return;
+    const int cnt = B.row_count[i];
+    const int me = bi.own_base + tid;
+    const float4 xi = st.spos[me], qi = st.squat[me];
+    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + tid;
+    const int nch = (cnt + 3) >> 2;
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
+    const int sh = P.row_shift;
+    for (int c = 0; c < nch; ++c) {
+        const uint2 cur = __ldg(rowb + (size_t)c * MD_TB);     // padding entries = dummy (far away -> outside the cutoff)
+        patchy_visit_s<IMG>(P, st, xi, qi, (cur.x & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG>(P, st, xi, qi, (cur.x >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG>(P, st, xi, qi, (cur.y & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG>(P, st, xi, qi, (cur.y >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
     }
+    force[i] = make_float4(fx, fy, fz, 0.5f * pe);
+    torque[i] = make_float4(tx, ty, tz, 0.f);
 }
 
-template <int S>
-__global__ void __launch_bounds__(256) k_vertex_patchy_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
-                                                              const float4* __restrict__ quat, float4* __restrict__ force,
-                                                              float4* __restrict__ torque) {
+__global__ void __launch_bounds__(MD_TB) k_vertex_patchy_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
+                                                                const float4* __restrict__ quat, float4* __restrict__ force,
+                                                                float4* __restrict__ torque) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int b = blockIdx.x;
     const BlkInfo bi = B.blk[b];
@@ -684,173 +708,35 @@ __global__ void __launch_bounds__(256) k_vertex_patchy_staged(DevParams P, DevBu
         if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
         return;
     }
-    const Stage st = stage_block<true, false>(P, B, bi, b, stage_entries, pos, quat, smraw);
-    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_patchy_rows<S, true>(P, B, bi, st, b, force, torque);
-    else vertex_patchy_rows<S, false>(P, B, bi, st, b, force, torque);
-}
-
-// ------------------------------------------------------------------------------------------------
-// EDGE, staged (S:A7): one lane per unordered pair of the half list (the row suffix, slot j > i); the owning
-// particle's side is summed over the slice in registers (warp-aggregated scatter, B:5), the partner's side is
-// scattered with red.global.add.v4.f32, only for pairs inside the cutoff.
-// ------------------------------------------------------------------------------------------------
-template <int S, int KIND, bool IMG>
-__device__ __forceinline__ void edge_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
-                                          float4* force, float4* torque) {
-    const int tid = threadIdx.x, l = tid & (S - 1);
-    const int nslices = blockDim.x / S, sid = tid / S;
-    const int i0 = b * MD_TB, nown = min(P.N - i0, MD_TB);
-    for (int p0 = 0; p0 < nown; p0 += nslices) {
-        const int p = p0 + sid;
-        const bool act = p < nown;
-        const int i = i0 + p;
-        const int cnt = act ? B.row_count[i] : 0, lo = act ? B.lo_count[i] : 0;
-        const int me = bi.own_base + (act ? p : 0);
-        const float4 xi = st.spos[me];
-        float4 qi = make_float4(1.f, 0.f, 0.f, 0.f);
-        if (KIND == MD_POT_PATCHY) qi = st.squat[me];
-        const unsigned short* __restrict__ row = B.rows + (size_t)(act ? i : i0) * P.rcap;
-        float ax = 0.f, ay = 0.f, az = 0.f, ape = 0.f, atx = 0.f, aty = 0.f, atz = 0.f;
-        for (int k = lo + l; k < cnt; k += S) {
-            const int t = row[row_pos(k, S)];
-            const float4 xj = st.spos[t];
-            float dx, dy, dz;
-            if (IMG) {
-                dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
-            } else {
-                dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
-            }
-            const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (!in_cutoff(P, d2, xi, xj)) continue;        // no memory traffic for zero-force pairs
-            const int j = st.sslot[t];
-            float fx, fy, fz, V;
-            if (KIND == MD_POT_PATCHY) {
-                const float4 qj = st.squat[t];
-                float tix, tiy, tiz, tjx, tjy, tjz;
-                patchy_pair<true>(P, dx, dy, dz, d2, qi, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
-                atx += tix; aty += tiy; atz += tiz;
-                red_add_v4(torque + j, tjx, tjy, tjz, 0.f);
-            } else {
-                float g;
-                lj_pair(P, d2, g, V);
-                fx = g * dx; fy = g * dy; fz = g * dz;
-            }
-            const float hV = 0.5f * V;
-            ax -= fx; ay -= fy; az -= fz; ape += hV;
-            red_add_v4(force + j, fx, fy, fz, hV);
-        }
-        __syncwarp();
-        ax = slice_sum<S>(ax); ay = slice_sum<S>(ay); az = slice_sum<S>(az); ape = slice_sum<S>(ape);
-        if (KIND == MD_POT_PATCHY) { atx = slice_sum<S>(atx); aty = slice_sum<S>(aty); atz = slice_sum<S>(atz); }
-        if (act && l == 0 && cnt > lo) {   // one reduction per owning particle
-            red_add_v4(force + i, ax, ay, az, ape);
-            if (KIND == MD_POT_PATCHY) red_add_v4(torque + i, atx, aty, atz, 0.f);
-        }
-    }
-}
-
-template <int S, int KIND>
-__global__ void __launch_bounds__(256) k_edge_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
-                                                     const float4* __restrict__ quat, float4* force, float4* torque) {
-    extern __shared__ __align__(16) unsigned char smraw[];
-    const int b = blockIdx.x;
-    const BlkInfo bi = B.blk[b];
-    if (bi.M <= 0 || bi.M + 1 > stage_entries) {
-        if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
-        return;
-    }
-    const Stage st = stage_block<KIND == MD_POT_PATCHY, true>(P, B, bi, b, stage_entries, pos, quat, smraw);
-    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) edge_rows<S, KIND, true>(P, B, bi, st, b, force, torque);
-    else edge_rows<S, KIND, false>(P, B, bi, st, b, force, torque);
-}
-
-__global__ void k_zero4_s(DevParams P, float4* a, float4* b) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < P.N) {
-        a[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (b) b[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-}
-
-// S:A8 bonded pass for EDGE (C3): one thread per static bond (id, id+1), FENE only, scatter with red.v4
-__global__ void k_edge_bonds_s(DevParams P, DevBuffers B, const float4* __restrict__ pos, float4* force) {
-    const int id = blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= P.N - 1 || (id % P.chain_len) == P.chain_len - 1) return;
-    const int i = B.slot_of_id[id], j = B.slot_of_id[id + 1];
-    const float4 xi = pos[i], xj = pos[j];
-    const float dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
-    const float dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
-    const float dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
-    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    float g, V;
-    if (!fene_pair(P, d2, g, V)) atomicOr(&B.ctrl->err, MD_DEVERR_FENE);
-    red_add_v4(force + i, -g * dx, -g * dy, -g * dz, 0.5f * V);
-    red_add_v4(force + j, g * dx, g * dy, g * dz, 0.5f * V);
+    const Stage st = stage_block<true>(P, B, bi, b, stage_entries, pos, quat, smraw);
+    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_patchy_rows<true>(P, B, bi, st, b, force, torque);
+    else vertex_patchy_rows<false>(P, B, bi, st, b, force, torque);
 }
 
 // ------------------------------------------------------------------------------------------------
 // host-side dispatch
 // ------------------------------------------------------------------------------------------------
-size_t md_staged_smem_bytes(const md_system* s, int stage_entries, bool edge) {
-    size_t b = 16 + 16 * (size_t)stage_entries * (s->rigid ? 2 : 1);
-    if (edge) b += 4 * (size_t)stage_entries;
-    return b;
-}
-
-template <typename K>
-static void allow_big_smem(K kernel) {
-    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+size_t md_staged_smem_bytes(const md_system* s, int stage_entries) {
+    return 16 + 16 * (size_t)stage_entries * (s->rigid ? 2 : 1);
 }
 
 static void staged_attrs_once() {
     static bool done = false;
     if (done) return;
     done = true;
-    allow_big_smem(k_vertex_lj_staged<4>);
-    allow_big_smem(k_vertex_lj_staged<8>);
-    allow_big_smem(k_vertex_patchy_staged<4>);
-    allow_big_smem(k_vertex_patchy_staged<8>);
-    allow_big_smem(k_edge_staged<4, MD_POT_LJ>);
-    allow_big_smem(k_edge_staged<8, MD_POT_LJ>);
-    allow_big_smem(k_edge_staged<4, MD_POT_PATCHY>);
-    allow_big_smem(k_edge_staged<8, MD_POT_PATCHY>);
+    cudaFuncSetAttribute(k_vertex_lj_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaFuncSetAttribute(k_vertex_patchy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
 }
 
-// returns false if the staged path cannot serve this request (caller falls back to the explicit-list kernels)
-bool md_launch_forces_staged(md_system* s, int strategy, int scatter) {
+// VERTEX on the staged rows.  Returns false if the neighbourhood does not fit in shared memory.
+bool md_launch_forces_staged(md_system* s) {
     const DevParams& P = s->P;
     staged_attrs_once();
     const int se = s->stage_launch;
-    const bool edge = strategy == MD_EDGE;
-    const size_t smem = md_staged_smem_bytes(s, se, edge);
+    const size_t smem = md_staged_smem_bytes(s, se);
     if (smem > 224 * 1024) return false;
-    const int S = P.slice;
-    if (!edge) {
-        if (P.kind == MD_POT_PATCHY) {
-            if (S == 8) k_vertex_patchy_staged<8><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
-            else k_vertex_patchy_staged<4><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
-        } else {
-            if (S == 8) k_vertex_lj_staged<8><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
-            else k_vertex_lj_staged<4><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
-        }
-        s->launches += 1;
-        return true;
-    }
-    (void)scatter;
-    const int nbN = cdiv(P.N, 256);
-    float4* tq = P.kind == MD_POT_PATCHY ? s->torque : nullptr;
-    k_zero4_s<<<nbN, 256, 0, s->stream>>>(P, s->force, tq);
-    if (P.kind == MD_POT_PATCHY) {
-        if (S == 8) k_edge_staged<8, MD_POT_PATCHY><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, tq);
-        else k_edge_staged<4, MD_POT_PATCHY><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, tq);
-    } else {
-        if (S == 8) k_edge_staged<8, MD_POT_LJ><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, nullptr, s->force, tq);
-        else k_edge_staged<4, MD_POT_LJ><<<P.nblk, 256, smem, s->stream>>>(P, s->B, se, s->pos, nullptr, s->force, tq);
-    }
-    s->launches += 2;
-    if (P.kind == MD_POT_FENE_WCA) {
-        k_edge_bonds_s<<<nbN, 256, 0, s->stream>>>(P, s->B, s->pos, s->force);
-        s->launches += 1;
-    }
+    if (P.kind == MD_POT_PATCHY) k_vertex_patchy_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
+    else k_vertex_lj_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+    s->launches += 1;
     return true;
 }

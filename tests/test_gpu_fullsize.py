@@ -21,7 +21,7 @@ def test_c2_full_size_parity(oracle):
     o = oracle.forces(w.pos, w.box, dict(w.potential))
     fmax = np.abs(o["F"]).max()
     tol = 1e-4 * fmax + 1e-6
-    for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp_smem"), ("edge", "red_v4"), ("edge", "warp"),
+    for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "red_v4"), ("edge", "warp"),
                       ("edge", "segmented")]:
         s.forces(strat, sc)
         F = s.in_id_order(s.force)
@@ -46,7 +46,7 @@ def test_c2b_many_neighbours(oracle):
     s.build_cells(); s.build_verlet()
     st = s.stats()
     o = oracle.forces(w.pos, w.box, dict(w.potential))
-    for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp_smem"), ("edge", "warp")]:
+    for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp")]:
         s.forces(strat, sc)
         F = s.in_id_order(s.force)
         assert np.abs(F[:, :3] - o["F"]).max() <= 1e-4 * np.abs(o["F"]).max() + 1e-6

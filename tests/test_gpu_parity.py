@@ -8,10 +8,10 @@ import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-# (strategy, variant): VERTEX gather alternatives {l2, smem}, EDGE scatter alternatives {red, red_v4, warp, segmented,
-# warp_smem}; the shared-memory staged variants need cell-sorted storage (order != none)
+# (strategy, variant): VERTEX gather alternatives {l2, smem}, EDGE scatter alternatives {red, red_v4, warp, segmented};
+# the shared-memory staged VERTEX variant needs cell-sorted storage (order != none)
 VARIANTS = [("vertex", "l2"), ("edge", "red"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented")]
-STAGED = [("vertex", "smem"), ("edge", "warp_smem")]
+STAGED = [("vertex", "smem")]
 
 
 def variants(order):
@@ -162,7 +162,7 @@ def test_error_paths(MD):
     s.close()
 
 
-@pytest.mark.parametrize("strat,sc", [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp_smem"), ("edge", "warp"),
+@pytest.mark.parametrize("strat,sc", [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp"),
                                       ("edge", "segmented")])
 def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
     """C1 (BASELINE.json configs[0]): 100 velocity-Verlet steps at dt = 0.002; fp32 GPU state against the fp64
@@ -188,10 +188,10 @@ def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
 
 
 @pytest.mark.parametrize("case,steps,strat,sc", [
-    ("lj", 300, "vertex", "smem"), ("lj", 300, "vertex", "l2"), ("lj", 300, "edge", "red_v4"), ("lj", 300, "edge", "warp_smem"),
-    ("polymer", 200, "vertex", "smem"), ("polymer", 200, "edge", "warp"), ("polymer", 200, "edge", "warp_smem"),
+    ("lj", 300, "vertex", "smem"), ("lj", 300, "vertex", "l2"), ("lj", 300, "edge", "red_v4"), 
+    ("polymer", 200, "vertex", "smem"), ("polymer", 200, "edge", "warp"), 
     ("patchy", 300, "vertex", "smem"), ("patchy", 300, "vertex", "l2"), ("patchy", 300, "edge", "segmented"),
-    ("patchy", 300, "edge", "warp_smem")])
+    ])
 def test_snapshot_parity_after_device_side_rebuilds(MD, oracle, case, steps, strat, sc):
     """Run md_integrate long enough for several skin-triggered rebuilds, then compare the forces the path holds
     (computed from lists rebuilt on the device) with the oracle's plain definition on the SAME positions, and the
