@@ -77,7 +77,7 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.ids = (int*)take(4 * Npad);
     b.ids_tmp = (int*)take(4 * Npad);
     b.slot_of_id = (int*)take(4 * Npad);
-    b.tmp4 = (float4*)take(16 * Npad);
+    b.tmp4 = (float4*)take(16 * Npad * (rigid ? 6 : 3));   // permutation scratch, one plane per state array
     b.pos_ref = (float4*)take(16 * Npad);
     b.nl_count = (int*)take(4 * Npad);
     b.nl_full = (int*)take(4 * Npad * g.cap);
@@ -99,7 +99,7 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.stage4 = (float4*)take(16 * Npad);
     b.cell_lin = (int*)take(4 * (size_t)g.ncell);
     b.rows = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);
-    b.rows_tmp = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);
+    b.rows_tmp = (unsigned short*)take(2 * 2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);   // scan order + sorted by column
     b.row_count = (int*)take(4 * Npad);
     b.lo_count = (int*)take(4 * Npad);
     b.blk = (BlkInfo*)take(sizeof(BlkInfo) * (size_t)g.nblk);
@@ -286,7 +286,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.half_skin2 = (float)(0.25 * skin * skin);
     P.rv2 = (float)P.rv2d;
     P.band_rv = (float)(P.rv2d * 1e-6);    // S:Q6 band of the list predicate
-    P.nblk = g.nblk; P.stage_cap = g.stage_cap; P.rcap = g.rcap; P.row_shift = g.stage_cap <= 4096 ? 4 : 0;
+    P.nblk = g.nblk; P.stage_cap = g.stage_cap; P.rcap = g.rcap; P.pad1 = 0;
     P.skinf = (float)skin;
     s->stage_launch = g.stage_cap;
     P.kind = pot->kind;

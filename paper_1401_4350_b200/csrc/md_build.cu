@@ -168,29 +168,24 @@ __global__ void k_cell_rank_sort(DevParams P, DevBuffers B, int gated) {
 // ------------------------------------------------------------------------------------------------
 // S:A3 physical reordering: new slot s takes the particle of old slot items[s]
 // ------------------------------------------------------------------------------------------------
-__global__ void k_gather4(DevParams P, DevBuffers B, int gated, float4* dst, const float4* src) {
-    GATE(B, gated);
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < P.N) dst[i] = src[B.items[i]];
-}
-__global__ void k_copy4(DevParams P, DevBuffers B, int gated, float4* dst, const float4* src) {
-    GATE(B, gated);
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < P.N) dst[i] = src[i];
-}
-__global__ void k_gather_ids(DevParams P, DevBuffers B, int gated) {
+struct StateArrays { float4* a[6]; int n; };
+
+// all bound state arrays, ids and cell indices in one pass: plane k of tmp4 takes array k in the new order
+__global__ void k_gather_state(DevParams P, DevBuffers B, int gated, StateArrays S, size_t plane) {
     GATE(B, gated);
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.N) return;
-    int o = B.items[i];
+    const int o = B.items[i];
+    for (int k = 0; k < S.n; ++k) B.tmp4[k * plane + i] = S.a[k][o];
     B.ids_tmp[i] = B.ids[o];
     B.items_tmp[i] = B.cell_of[o];
 }
-__global__ void k_commit_ids(DevParams P, DevBuffers B, int gated) {
+__global__ void k_commit_state(DevParams P, DevBuffers B, int gated, StateArrays S, size_t plane) {
     GATE(B, gated);
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.N) return;
-    int id = B.ids_tmp[i];
+    for (int k = 0; k < S.n; ++k) S.a[k][i] = B.tmp4[k * plane + i];
+    const int id = B.ids_tmp[i];
     B.ids[i] = id;
     B.slot_of_id[id] = i;
     B.cell_of[i] = B.items_tmp[i];
@@ -210,14 +205,12 @@ void md_launch_build_cells(md_system* s, bool gated) {
     s->launches += 2;
     if (s->order != MD_ORDER_NONE) {
         float4* arrs[6] = { s->pos, s->vel, s->force, s->quat, s->angmom, s->torque };
-        for (int a = 0; a < 6; ++a) {
-            if (!arrs[a]) continue;
-            k_gather4<<<nbN, 256, 0, s->stream>>>(P, s->B, g, s->B.tmp4, arrs[a]);
-            k_copy4<<<nbN, 256, 0, s->stream>>>(P, s->B, g, arrs[a], s->B.tmp4);
-            s->launches += 2;
-        }
-        k_gather_ids<<<nbN, 256, 0, s->stream>>>(P, s->B, g);
-        k_commit_ids<<<nbN, 256, 0, s->stream>>>(P, s->B, g);
+        StateArrays S;
+        S.n = 0;
+        for (int a = 0; a < 6; ++a) if (arrs[a]) S.a[S.n++] = arrs[a];
+        const size_t plane = (size_t)P.ntiles * MD_TILE;
+        k_gather_state<<<nbN, 256, 0, s->stream>>>(P, s->B, g, S, plane);
+        k_commit_state<<<nbN, 256, 0, s->stream>>>(P, s->B, g, S, plane);
         s->launches += 2;
     }
 }

@@ -23,6 +23,7 @@
 #define MD_BLK_WRAP 1         // some listed pair of the block crosses a periodic face
 #define MD_BLK_SHIFT_OK 2     // ... and the shift-down transform of the staged coordinates reproduces every minimum image
 #define MD_BLK_AXIS_SHIFT 4   // bits 2..4: axes (x, y, z) the transform applies to
+#define MD_BLK_SH4 256         // row entries of the block are byte offsets (local index << 4): its neighbourhood has <= 4096 entries
 
 // Device-resident control block (first bytes of the workspace).
 struct DevCtrl {
@@ -58,8 +59,7 @@ struct DevParams {
     float rc2, band_abs;               // fp32 cutoff and the half-width of the fp64-recheck band |d2 - rc2| (S:H10)
     float half_skin2;                  // (skin/2)^2
     float rv2, band_rv;                // fp32 list radius^2 and its fp64-recheck band (S:Q6)
-    int nblk, stage_cap, rcap, row_shift;   // staged path: blocks of MD_TB slots, smem capacity (particles), row capacity (entries),
-                                            // row entries = local index << row_shift (4 = byte offset of the float4, when stage_cap <= 4096)
+    int nblk, stage_cap, rcap, pad1;   // staged path: blocks of MD_TB slots, smem capacity (particles), row capacity (entries)
     float skinf;
     // pair potential
     int kind;
@@ -90,7 +90,7 @@ struct DevBuffers {
     int* ids;              // [N] slot -> original id
     int* ids_tmp;          // [N]
     int* slot_of_id;       // [N]
-    float4* tmp4;          // [N] permutation scratch
+    float4* tmp4;          // [3 or 6][Npad] permutation scratch, one plane per bound state array
     float4* pos_ref;       // [N]
     int* nl_count;         // [Npad]
     int* nl_full;          // [ntiles*32*cap] tile-transposed full list
@@ -110,7 +110,7 @@ struct DevBuffers {
     // staged path
     int* cell_lin;         // [ncell] storage rank -> linear cell index (inverse of cell_rank)
     unsigned short* rows;  // [nblk][rcap/4][MD_TB] x 4 u16: Verlet rows of block-local indices, block-transposed chunks of 4
-    unsigned short* rows_tmp; // [nblk*MD_TB*rcap] build scratch: rows in scan order
+    unsigned short* rows_tmp; // [2][nblk][rcap][MD_TB] build scratch: rows in scan order, then sorted by bank column
     int* row_count;        // [Npad] |L_i|
     int* lo_count;         // [Npad] neighbours with slot < i
     BlkInfo* blk;          // [nblk]

@@ -102,8 +102,9 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     const int myrank = live ? B.cell_of[i] : -1;
     const int head = live && (tid == 0 || B.cell_of[i - 1] != myrank) ? 1 : 0;
     int nownc;
-    const int oc = blk_excl_scan(head, &nownc, sh_scan);
-    if (head) own_rank[oc] = myrank;
+    const int oc_ex = blk_excl_scan(head, &nownc, sh_scan);
+    if (head) own_rank[oc_ex] = myrank;
+    const int myoc = oc_ex + head - 1;       // ordinal of this thread's cell among the block's own cells
     __syncthreads();
 
     // 2. candidate cells: the 27-cell stencil of every own cell (S:Q8; duplicates removed below)
@@ -220,6 +221,31 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         while (lo < hi) { const int mid = (lo + hi) >> 1; if (urank[mid] < r0) lo = mid + 1; else hi = mid; }
         s_own_base = ubase[lo] + (i0 - B.cell_start[r0]);
     }
+    // 7b. stencil table (reuses cand[]): cand[oc * 27 + s] = index into urank of stencil cell s of own cell oc, or -1 for
+    //     an empty cell / a cell already listed for this own cell (axes with fewer than 3 cells, S:Q8)
+    {
+        const bool small_axis = P.ncx < 3 || P.ncy < 3 || P.ncz < 3;
+        auto stencil_rank = [&](int lin, int st) {
+            const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
+            int ax = cx + st / 9 - 1, ay = cy + (st / 3) % 3 - 1, az = cz + st % 3 - 1;
+            if (ax < 0) ax += P.ncx; else if (ax >= P.ncx) ax -= P.ncx;
+            if (ay < 0) ay += P.ncy; else if (ay >= P.ncy) ay -= P.ncy;
+            if (az < 0) az += P.ncz; else if (az >= P.ncz) az -= P.ncz;
+            return B.cell_rank[(ax * P.ncy + ay) * P.ncz + az];
+        };
+        __syncthreads();   // cand[] is no longer read by the unique pass
+        for (int t = tid; t < n; t += MD_TB) {
+            const int lin = B.cell_lin[own_rank[t / 27]];
+            const int st = t % 27;
+            const int r = stencil_rank(lin, st);
+            int lo = 0, hi = U - 1;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (urank[mid] < r) lo = mid + 1; else hi = mid; }
+            int u = (U > 0 && urank[lo] == r) ? lo : -1;
+            if (small_axis && u >= 0)
+                for (int s2 = 0; s2 < st; ++s2) if (stencil_rank(lin, s2) == r) { u = -1; break; }
+            cand[t] = u;
+        }
+    }
     __syncthreads();
     const int own_base = s_own_base;
     const bool maywrap = (s_flags & MD_BLK_WRAP) != 0 || P.ncx < 3 || P.ncy < 3 || P.ncz < 3;
@@ -234,20 +260,19 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     unsigned short* s_cur = s_rem + 8 * MD_TB;                                        // [8][MD_TB] scan cursor per column
     int cnt = 0, lo_cnt = 0, flags = 0;
     float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
-    unsigned short* __restrict__ tmp = B.rows_tmp + (size_t)(live ? i : i0) * P.rcap;
+    // scan-order scratch row, block-transposed (entry k of thread tid at k * MD_TB + tid): lanes of a warp sit at
+    // similar k, so both passes touch a few sectors per warp access instead of one per lane
+    unsigned short* __restrict__ tmp = B.rows_tmp + (size_t)b * P.rcap * MD_TB + tid;
 #pragma unroll
     for (int c = 0; c < 8; ++c) { s_rem[c * MD_TB + tid] = 0; s_cur[c * MD_TB + tid] = 0; }
     if (live) {
         const int me = own_base + tid;
         xi = spos[me];
-        const int lin = B.cell_lin[myrank];
-        const int cx = lin / (P.ncz * P.ncy), cy = (lin / P.ncz) % P.ncy, cz = lin % P.ncz;
         const float hLx = P.hLx, hLy = P.hLy, hLz = P.hLz;
-        for (int u = 0; u < U; ++u) {
-            const int pc = ucoord[u];
-            int dx = abs((pc & 1023) - cx), dy = abs(((pc >> 10) & 1023) - cy), dz = abs((pc >> 20) - cz);
-            const bool mx = dx <= 1 || dx == P.ncx - 1, my = dy <= 1 || dy == P.ncy - 1, mz = dz <= 1 || dz == P.ncz - 1;
-            if (!(mx && my && mz)) continue;
+        const int* __restrict__ mycells = cand + myoc * 27;
+        for (int sc = 0; sc < 27; ++sc) {
+            const int u = mycells[sc];
+            if (u < 0) continue;
             const int t1 = ubase[u + 1];
             for (int t = ubase[u]; t < t1; ++t) {
                 if (t == me) continue;
@@ -263,7 +288,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                 bool in = tt < 0.0f;
                 if (fabsf(tt) < P.band_rv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
                 if (in) {
-                    if (cnt < P.cap) { tmp[cnt] = (unsigned short)t; s_rem[(t & 7) * MD_TB + tid] += 1; }
+                    if (cnt < P.cap) { tmp[(size_t)cnt * MD_TB] = (unsigned short)t; s_rem[(t & 7) * MD_TB + tid] += 1; }
                     ++cnt;
                     lo_cnt += (t < me);
                     if (maywrap) {
@@ -298,7 +323,22 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         const int nchunk = P.rcap >> 2;
         uint2* __restrict__ rowb = reinterpret_cast<uint2*>(B.rows) + (size_t)b * nchunk * MD_TB + tid;
         unsigned int w[4] = { 0u, 0u, 0u, 0u };
-        const unsigned int dummy = (unsigned int)M << P.row_shift;
+        const int rsh = (M + 1 <= 4096) ? 4 : 0;   // MD_BLK_SH4: entries are byte offsets into the staged float4 array
+        const unsigned int dummy = (unsigned int)M << rsh;
+        // counting sort of the scratch row by column into a second scratch row: s_cur[c] ends as the END of column c
+        unsigned short* __restrict__ tmp2 = tmp + (size_t)P.nblk * P.rcap * MD_TB;
+        {
+            int acc = 0;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) { s_cur[c * MD_TB + tid] = (unsigned short)acc; acc += s_rem[c * MD_TB + tid]; }
+            for (int k = 0; k < c2; ++k) {
+                const unsigned short e = tmp[(size_t)k * MD_TB];
+                const int c = e & 7;
+                const int p = s_cur[c * MD_TB + tid];
+                s_cur[c * MD_TB + tid] = (unsigned short)(p + 1);
+                tmp2[(size_t)p * MD_TB] = e;
+            }
+        }
         for (int k0 = 0; k0 < c2; k0 += 4) {
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
@@ -310,11 +350,9 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                         int bv = 0;
                         for (int cc = 0; cc < 8; ++cc) { const int v = s_rem[cc * MD_TB + tid]; if (v > bv) { bv = v; c = cc; } }
                     }
-                    int pos = s_cur[c * MD_TB + tid];
-                    while ((tmp[pos] & 7) != c) ++pos;
-                    t = (unsigned int)tmp[pos] << P.row_shift;
-                    s_cur[c * MD_TB + tid] = (unsigned short)(pos + 1);
-                    s_rem[c * MD_TB + tid] -= 1;
+                    const int rem = s_rem[c * MD_TB + tid];
+                    t = (unsigned int)tmp2[(size_t)(s_cur[c * MD_TB + tid] - rem) * MD_TB] << rsh;   // next unused entry of column c
+                    s_rem[c * MD_TB + tid] = (unsigned short)(rem - 1);
                 }
                 w[q] = t;
             }
@@ -344,6 +382,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
             const int shifted = (f >> 2) & 7, broken = (f >> 6) & 7;
             if (!(f & 32) && !(shifted & broken)) out |= MD_BLK_SHIFT_OK;
         }
+        if (M + 1 <= 4096) out |= MD_BLK_SH4;
         B.blk[b] = BlkInfo{ nseg, M, own_base, out };
         atomicAdd(&B.ctrl->n_full, (unsigned long long)tot_full);
         atomicAdd(&B.ctrl->n_edges, (unsigned int)tot_half);
@@ -421,7 +460,7 @@ __global__ void __launch_bounds__(MD_TB) k_edges_from_rows(DevParams P, DevBuffe
     const float4 xi = pos[i];
     unsigned int o = B.edge_off[i];
     for (int k = 0; k < cnt; ++k) {
-        const int t = (int)row_entry(rowb, k, P.row_shift);
+        const int t = (int)row_entry(rowb, k, (bi.flags & MD_BLK_SH4) ? 4 : 0);
         if (t <= me) continue;
         const int j = sslot[t];
         const float4 xj = pos[j];
@@ -450,7 +489,7 @@ struct Stage {
 };
 
 template <bool QUAT>
-__device__ __forceinline__ Stage stage_block(const DevParams& P, const DevBuffers& B, const BlkInfo bi, int b, int stage_entries,
+__device__ __forceinline__ Stage stage_issue(const DevParams& P, const DevBuffers& B, const BlkInfo bi, int b, int stage_entries,
                                              const float4* __restrict__ pos, const float4* __restrict__ quat, unsigned char* smraw) {
     Stage st;
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(smraw);
@@ -476,7 +515,13 @@ __device__ __forceinline__ Stage stage_block(const DevParams& P, const DevBuffer
         if (QUAT) st.squat[bi.M] = make_float4(1.f, 0.f, 0.f, 0.f);
     }
     __syncthreads();          // barrier initialised, dummy written
-    mbar_wait(bar, 0);        // all segments have landed
+    return st;
+}
+
+// second half of the prologue: wait for the bulk copies, then the periodic shift transform
+__device__ __forceinline__ void stage_wait(const DevParams& P, const BlkInfo bi, const Stage& st, unsigned char* smraw) {
+    const int tid = threadIdx.x;
+    mbar_wait(smraw, 0);      // all segments have landed
     // periodic blocks: shift the upper half of the box down by L on the wrapped axes (exact in fp32: Sterbenz),
     // after which plain differences ARE the minimum images (verified pair by pair at build time)
     if ((bi.flags & MD_BLK_WRAP) && (bi.flags & MD_BLK_SHIFT_OK)) {
@@ -490,7 +535,6 @@ __device__ __forceinline__ Stage stage_block(const DevParams& P, const DevBuffer
         }
         __syncthreads();
     }
-    return st;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -590,28 +634,33 @@ __device__ __forceinline__ void fene_vertex_s(const DevParams& P, const DevBuffe
 }
 
 template <bool IMG, int SH>
-__device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
+__device__ __forceinline__ void lj_chunk_s(const DevParams& P, const float4* sp, float4 xi, uint2 cur, LJAccS& a) {
+    const float4 x0 = staged_pos<SH>(sp, cur.x & 0xffffu), x1 = staged_pos<SH>(sp, cur.x >> 16);
+    const float4 x2 = staged_pos<SH>(sp, cur.y & 0xffffu), x3 = staged_pos<SH>(sp, cur.y >> 16);
+    lj_visit2_s<IMG>(P, xi, x0, x1, a);
+    lj_visit2_s<IMG>(P, xi, x2, x3, a);
+}
+
+// cnt, pkA, pkB: |L_i| and the first two row chunks, loaded by the caller while the staging copies were in flight.
+// Chunks are consumed in pairs through two separate load instructions (two scoreboards), each re-issued two chunks
+// ahead of its use, so a chunk has ~2 chunks of arithmetic to arrive from HBM.
+template <bool IMG, int SH>
+__device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int i,
+                                               int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB,
                                                const float4* __restrict__ pos, float4* __restrict__ force, bool bonds) {
-    const int tid = threadIdx.x;
-    const int i = b * MD_TB + tid;
-    if (i >= P.N) return;
-    const int cnt = B.row_count[i];
-    const float4 xi = st.spos[bi.own_base + tid];
-    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + tid;
+    const float4 xi = st.spos[bi.own_base + threadIdx.x];
     const float4* sp = st.spos;
     const int nch = (cnt + 3) >> 2;                        // the last chunk is padded with the dummy entry
     LJAccS a = { 0.f, 0.f, 0.f, 3.0e38f, make_float2(0.f, 0.f) };
-    // row chunks are prefetched two ahead (HBM latency is ~2 chunks of arithmetic at this occupancy)
-    uint2 pk = nch > 0 ? __ldg(rowb) : make_uint2(0u, 0u);
-    uint2 pk2 = nch > 1 ? __ldg(rowb + MD_TB) : make_uint2(0u, 0u);
-    for (int c = 0; c < nch; ++c) {
-        const uint2 cur = pk;
-        pk = pk2;
-        if (c + 2 < nch) pk2 = __ldg(rowb + (size_t)(c + 2) * MD_TB);
-        const float4 x0 = staged_pos<SH>(sp, cur.x & 0xffffu), x1 = staged_pos<SH>(sp, cur.x >> 16);
-        const float4 x2 = staged_pos<SH>(sp, cur.y & 0xffffu), x3 = staged_pos<SH>(sp, cur.y >> 16);
-        lj_visit2_s<IMG>(P, xi, x0, x1, a);
-        lj_visit2_s<IMG>(P, xi, x2, x3, a);
+    for (int c = 0; c < nch; c += 2) {
+        const uint2 curA = pkA;
+        if (c + 2 < nch) pkA = __ldg(rowb + (size_t)(c + 2) * MD_TB);
+        lj_chunk_s<IMG, SH>(P, sp, xi, curA, a);
+        if (c + 1 < nch) {
+            const uint2 curB = pkB;
+            if (c + 3 < nch) pkB = __ldg(rowb + (size_t)(c + 3) * MD_TB);
+            lj_chunk_s<IMG, SH>(P, sp, xi, curB, a);
+        }
     }
     float pe2 = a.pe.x + a.pe.y;
     if (a.band < P.band_abs) {
@@ -638,15 +687,24 @@ __global__ void __launch_bounds__(MD_TB) k_vertex_lj_staged(DevParams P, DevBuff
         if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
         return;
     }
-    const Stage st = stage_block<false>(P, B, bi, b, stage_entries, pos, nullptr, smraw);
+    const Stage st = stage_issue<false>(P, B, bi, b, stage_entries, pos, nullptr, smraw);
+    // while the copies are in flight: |L_i| and the first two row chunks
+    const int i = b * MD_TB + threadIdx.x;
+    const bool live = i < P.N;
+    const int cnt = live ? B.row_count[i] : 0;
+    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + threadIdx.x;
+    const uint2 pkA = cnt > 0 ? __ldg(rowb) : make_uint2(0u, 0u);
+    const uint2 pkB = cnt > 4 ? __ldg(rowb + MD_TB) : make_uint2(0u, 0u);
+    stage_wait(P, bi, st, smraw);
+    if (!live) return;
     const bool bonds = P.kind == MD_POT_FENE_WCA;
     const bool img = (bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK);
-    if (P.row_shift == 4) {
-        if (img) vertex_lj_rows<true, 4>(P, B, bi, st, b, pos, force, bonds);
-        else vertex_lj_rows<false, 4>(P, B, bi, st, b, pos, force, bonds);
+    if (bi.flags & MD_BLK_SH4) {
+        if (img) vertex_lj_rows<true, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
+        else vertex_lj_rows<false, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
     } else {
-        if (img) vertex_lj_rows<true, 0>(P, B, bi, st, b, pos, force, bonds);
-        else vertex_lj_rows<false, 0>(P, B, bi, st, b, pos, force, bonds);
+        if (img) vertex_lj_rows<true, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
+        else vertex_lj_rows<false, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
     }
 }
 
@@ -686,7 +744,7 @@ __device__ __forceinline__ void vertex_patchy_rows(const DevParams& P, const Dev
     const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + tid;
     const int nch = (cnt + 3) >> 2;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
-    const int sh = P.row_shift;
+    const int sh = (bi.flags & MD_BLK_SH4) ? 4 : 0;
     for (int c = 0; c < nch; ++c) {
         const uint2 cur = __ldg(rowb + (size_t)c * MD_TB);     // padding entries = dummy (far away -> outside the cutoff)
         patchy_visit_s<IMG>(P, st, xi, qi, (cur.x & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
@@ -708,7 +766,8 @@ __global__ void __launch_bounds__(MD_TB) k_vertex_patchy_staged(DevParams P, Dev
         if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
         return;
     }
-    const Stage st = stage_block<true>(P, B, bi, b, stage_entries, pos, quat, smraw);
+    const Stage st = stage_issue<true>(P, B, bi, b, stage_entries, pos, quat, smraw);
+    stage_wait(P, bi, st, smraw);
     if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_patchy_rows<true>(P, B, bi, st, b, force, torque);
     else vertex_patchy_rows<false>(P, B, bi, st, b, force, torque);
 }
