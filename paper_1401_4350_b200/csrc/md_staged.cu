@@ -544,6 +544,14 @@ __device__ __forceinline__ void stage_wait(const DevParams& P, const BlkInfo bi,
 // ------------------------------------------------------------------------------------------------
 struct LJAccS { float fx, fy, fz, band; float2 pe; };
 
+// streamed row chunk: read once per evaluation, so it bypasses L1 allocation (the L1 left beside the staged
+// neighbourhoods is small) (no_allocate)
+__device__ __forceinline__ uint2 ld_row(const uint2* p) {
+    uint2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    return v;
+}
+
 // staged position of a row entry: entries hold (local index << SH); SH == 4 makes the entry the byte offset
 template <int SH>
 __device__ __forceinline__ float4 staged_pos(const float4* sp, unsigned int e) {
@@ -582,32 +590,37 @@ __device__ __forceinline__ void lj_visit2_s(const DevParams& P, float4 xi, float
     a.pe = __ffma2_rn(m, P.k_nvs, a.pe);                       // - V_c
 }
 
-// rare path: a visit of this particle fell inside the fp64-recheck band -> redo the particle with the
-// S:O0 / S:Q5 decision for every banded pair
-__device__ __noinline__ void lj_careful_s(const float4* spos, const uint2* __restrict__ rowb, int cnt, int shift, float4 xi,
-                                          float Lx, float Ly, float Lz, float rc2, float band_abs, float lj_a, float lj_b,
-                                          float lj_c, float lj_d, float vshift, double dLx, double dLy, double dLz, double rc2d,
-                                          float4* out) {
-    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f;
-    int nin = 0;
+// rare path (~1.6e-4 of the particles at rc = 2.5): a visit of this particle fell inside the fp64-recheck band.
+// Re-scan the row for the banded pairs only and, where the S:O0 / S:Q5 fp64 decision differs from the fp32 one the
+// fast loop took, add or remove that pair's contribution.  acc = (fx, fy, fz, pe) of the fast loop, corrected in place.
+template <bool IMG>
+__device__ __noinline__ void lj_fix_band_s(const float4* spos, const uint2* __restrict__ rowb, int cnt, int shift, float4 xi,
+                                           float Lx, float Ly, float Lz, float rc2, float band_abs, float lj_a, float lj_b,
+                                           float lj_c, float lj_d, float vshift, double dLx, double dLy, double dLz, double rc2d,
+                                           float4* acc) {
+    float4 a = *acc;
     for (int k = 0; k < cnt; ++k) {
         const float4 xj = spos[row_entry(rowb, k, shift)];
-        const float dx = min_image(xj.x, xi.x, Lx, 0.5f * Lx);
-        const float dy = min_image(xj.y, xi.y, Ly, 0.5f * Ly);
-        const float dz = min_image(xj.z, xi.z, Lz, 0.5f * Lz);
+        float dx, dy, dz;
+        if (IMG) {
+            dx = min_image(xj.x, xi.x, Lx, 0.5f * Lx); dy = min_image(xj.y, xi.y, Ly, 0.5f * Ly); dz = min_image(xj.z, xi.z, Lz, 0.5f * Lz);
+        } else {
+            dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
+        }
         const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
         const float t = d2 - rc2;
-        bool in = t < 0.0f;
-        if (fabsf(t) < band_abs) in = inside_fp64(xi, xj, dLx, dLy, dLz, rc2d);
+        if (!(fabsf(t) < band_abs)) continue;
+        const bool in32 = t < 0.0f;
+        const bool in64 = inside_fp64(xi, xj, dLx, dLy, dLz, rc2d);
+        if (in32 == in64) continue;
+        const float sgn = in64 ? 1.0f : -1.0f;
         const float inv = rcp_approx(d2);
-        float inv3 = inv * inv * inv;
-        inv3 = in ? inv3 : 0.0f;
-        const float g = inv * inv3 * fmaf(lj_a, inv3, -lj_b);
-        fx = fmaf(-g, dx, fx); fy = fmaf(-g, dy, fy); fz = fmaf(-g, dz, fz);
-        pe = fmaf(inv3, fmaf(lj_c, inv3, -lj_d), pe);
-        nin += in ? 1 : 0;
+        const float u = inv * inv * inv;
+        const float ng = sgn * (inv * u) * fmaf(-lj_a, u, lj_b);
+        a.x = fmaf(ng, dx, a.x); a.y = fmaf(ng, dy, a.y); a.z = fmaf(ng, dz, a.z);
+        a.w += sgn * (fmaf(u, fmaf(lj_c, u, -lj_d), -vshift));
     }
-    *out = make_float4(fx, fy, fz, fmaf(-(float)nin, vshift, pe));
+    *acc = a;
 }
 
 // FENE partners of slot i (ids id-1 and id+1 inside its chain), global gathers through slot_of_id
@@ -641,32 +654,41 @@ __device__ __forceinline__ void lj_chunk_s(const DevParams& P, const float4* sp,
     lj_visit2_s<IMG>(P, xi, x2, x3, a);
 }
 
-// cnt, pkA, pkB: |L_i| and the first two row chunks, loaded by the caller while the staging copies were in flight.
-// Chunks are consumed in pairs through two separate load instructions (two scoreboards), each re-issued two chunks
-// ahead of its use, so a chunk has ~2 chunks of arithmetic to arrive from HBM.
+// cnt, pk[0..3]: |L_i| and the first four row chunks, loaded by the caller while the staging copies were in flight.
+// The row streams from HBM (~1300 cycles under load); chunks are consumed four per iteration through four separate
+// load instructions, each re-issued four chunks (~350 instructions of arithmetic) ahead of its use.
 template <bool IMG, int SH>
 __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int i,
-                                               int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB,
+                                               int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB, uint2 pkC, uint2 pkD,
                                                const float4* __restrict__ pos, float4* __restrict__ force, bool bonds) {
     const float4 xi = st.spos[bi.own_base + threadIdx.x];
     const float4* sp = st.spos;
     const int nch = (cnt + 3) >> 2;                        // the last chunk is padded with the dummy entry
     LJAccS a = { 0.f, 0.f, 0.f, 3.0e38f, make_float2(0.f, 0.f) };
-    for (int c = 0; c < nch; c += 2) {
+    for (int c = 0; c < nch; c += 4) {
         const uint2 curA = pkA;
-        if (c + 2 < nch) pkA = __ldg(rowb + (size_t)(c + 2) * MD_TB);
+        if (c + 4 < nch) pkA = ld_row(rowb + (size_t)(c + 4) * MD_TB);
         lj_chunk_s<IMG, SH>(P, sp, xi, curA, a);
-        if (c + 1 < nch) {
-            const uint2 curB = pkB;
-            if (c + 3 < nch) pkB = __ldg(rowb + (size_t)(c + 3) * MD_TB);
-            lj_chunk_s<IMG, SH>(P, sp, xi, curB, a);
-        }
+        if (c + 1 >= nch) break;
+        const uint2 curB = pkB;
+        if (c + 5 < nch) pkB = ld_row(rowb + (size_t)(c + 5) * MD_TB);
+        lj_chunk_s<IMG, SH>(P, sp, xi, curB, a);
+        if (c + 2 >= nch) break;
+        const uint2 curC = pkC;
+        if (c + 6 < nch) pkC = ld_row(rowb + (size_t)(c + 6) * MD_TB);
+        lj_chunk_s<IMG, SH>(P, sp, xi, curC, a);
+        if (c + 3 >= nch) break;
+        const uint2 curD = pkD;
+        if (c + 7 < nch) pkD = ld_row(rowb + (size_t)(c + 7) * MD_TB);
+        lj_chunk_s<IMG, SH>(P, sp, xi, curD, a);
     }
     float pe2 = a.pe.x + a.pe.y;
     if (a.band < P.band_abs) {
-        lj_careful_s(st.spos, rowb, cnt, SH, xi, P.Lx, P.Ly, P.Lz, P.rc2, P.band_abs, P.lj_a, P.lj_b,
-                     P.lj_c, P.lj_d, P.vshift, P.dLx, P.dLy, P.dLz, P.rc2d, force + i);
-        const float4 r = force[i];
+        float4* scratch = force + i;           // own output slot as scratch (rewritten below)
+        *scratch = make_float4(a.fx, a.fy, a.fz, pe2);
+        lj_fix_band_s<IMG>(st.spos, rowb, cnt, SH, xi, P.Lx, P.Ly, P.Lz, P.rc2, P.band_abs, P.lj_a, P.lj_b,
+                           P.lj_c, P.lj_d, P.vshift, P.dLx, P.dLy, P.dLz, P.rc2d, scratch);
+        const float4 r = *scratch;
         a.fx = r.x; a.fy = r.y; a.fz = r.z; pe2 = r.w;
     }
     float pe = 0.5f * pe2;
@@ -678,7 +700,7 @@ __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuff
     force[i] = make_float4(a.fx, a.fy, a.fz, pe);
 }
 
-__global__ void __launch_bounds__(MD_TB) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
+__global__ void __launch_bounds__(MD_TB, 4) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
                                                             float4* __restrict__ force) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int b = blockIdx.x;
@@ -693,18 +715,20 @@ __global__ void __launch_bounds__(MD_TB) k_vertex_lj_staged(DevParams P, DevBuff
     const bool live = i < P.N;
     const int cnt = live ? B.row_count[i] : 0;
     const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + threadIdx.x;
-    const uint2 pkA = cnt > 0 ? __ldg(rowb) : make_uint2(0u, 0u);
-    const uint2 pkB = cnt > 4 ? __ldg(rowb + MD_TB) : make_uint2(0u, 0u);
+    const uint2 pkA = cnt > 0 ? ld_row(rowb) : make_uint2(0u, 0u);
+    const uint2 pkB = cnt > 4 ? ld_row(rowb + MD_TB) : make_uint2(0u, 0u);
+    const uint2 pkC = cnt > 8 ? ld_row(rowb + 2 * MD_TB) : make_uint2(0u, 0u);
+    const uint2 pkD = cnt > 12 ? ld_row(rowb + 3 * MD_TB) : make_uint2(0u, 0u);
     stage_wait(P, bi, st, smraw);
     if (!live) return;
     const bool bonds = P.kind == MD_POT_FENE_WCA;
     const bool img = (bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK);
     if (bi.flags & MD_BLK_SH4) {
-        if (img) vertex_lj_rows<true, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
-        else vertex_lj_rows<false, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
+        if (img) vertex_lj_rows<true, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
+        else vertex_lj_rows<false, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
     } else {
-        if (img) vertex_lj_rows<true, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
-        else vertex_lj_rows<false, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pos, force, bonds);
+        if (img) vertex_lj_rows<true, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
+        else vertex_lj_rows<false, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
     }
 }
 
