@@ -210,6 +210,26 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         return;
     }
 
+    // 6b. pack the segment length beside its first local index: seg.y = local << 16 | len (both < 65536), so the force
+    //     kernels can issue a segment's bulk copy from its own table entry alone
+    {
+        __syncthreads();
+        int2* sgt = B.seg + (size_t)b * MD_SEGMAX;
+        int ys[MD_SEGMAX / MD_TB], ln[MD_SEGMAX / MD_TB];
+#pragma unroll
+        for (int q = 0; q < MD_SEGMAX / MD_TB; ++q) {
+            const int sg = q * MD_TB + tid;
+            ys[q] = 0; ln[q] = 0;
+            if (sg < nseg) { ys[q] = sgt[sg].y; ln[q] = (sg + 1 < nseg ? sgt[sg + 1].y : M) - ys[q]; }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < MD_SEGMAX / MD_TB; ++q) {
+            const int sg = q * MD_TB + tid;
+            if (sg < nseg) sgt[sg].y = (ys[q] << 16) | ln[q];
+        }
+    }
+
     // 7. stage the neighbourhood (plain coalesced copies, one warp per cell) and locate the block's own particles
     for (int u = tid >> 5; u < U; u += MD_TB / 32) {
         const int s0 = B.cell_start[urank[u]], l0 = ubase[u], len = ubase[u + 1] - l0;
@@ -449,8 +469,8 @@ __global__ void __launch_bounds__(MD_TB) k_edges_from_rows(DevParams P, DevBuffe
     const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
     for (int sg = tid >> 5; sg < bi.nseg; sg += MD_TB / 32) {
         const int2 s0 = seg[sg];
-        const int len = (sg + 1 < bi.nseg ? seg[sg + 1].y : bi.M) - s0.y;
-        for (int k = tid & 31; k < len; k += 32) sslot[s0.y + k] = s0.x + k;
+        const int l0 = (int)((unsigned)s0.y >> 16), len = s0.y & 0xffff;
+        for (int k = tid & 31; k < len; k += 32) sslot[l0 + k] = s0.x + k;
     }
     __syncthreads();
     const int i = b * MD_TB + tid;
@@ -488,9 +508,24 @@ struct Stage {
     float4* squat;   // [M + 1]  rigid bodies only
 };
 
+// the first SEG_PRE table entries of each lane of warp 0, loaded at kernel entry together with the block header so
+// that the staging copies wait for ONE memory latency instead of two
+#define SEG_PRE 4
+struct SegPre { int2 e[SEG_PRE]; };
+__device__ __forceinline__ SegPre seg_preload(const DevBuffers& B, int b) {
+    SegPre sp;
+    const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
+    if (threadIdx.x < 32) {
+#pragma unroll
+        for (int q = 0; q < SEG_PRE; ++q) sp.e[q] = seg[threadIdx.x + 32 * q];   // always inside the table; entries >= nseg are ignored
+    }
+    return sp;
+}
+
 template <bool QUAT>
 __device__ __forceinline__ Stage stage_issue(const DevParams& P, const DevBuffers& B, const BlkInfo bi, int b, int stage_entries,
-                                             const float4* __restrict__ pos, const float4* __restrict__ quat, unsigned char* smraw) {
+                                             const SegPre& pre, const float4* __restrict__ pos, const float4* __restrict__ quat,
+                                             unsigned char* smraw) {
     Stage st;
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(smraw);
     st.spos = reinterpret_cast<float4*>(smraw + 16);
@@ -503,11 +538,20 @@ __device__ __forceinline__ Stage stage_issue(const DevParams& P, const DevBuffer
             mbar_expect_tx(bar, (unsigned)bi.M * 16u * (QUAT ? 2u : 1u));
         }
         __syncwarp();
-        for (int sg = tid; sg < bi.nseg; sg += 32) {
+#pragma unroll
+        for (int q = 0; q < SEG_PRE; ++q) {
+            const int2 s0 = pre.e[q];
+            if (tid + 32 * q < bi.nseg) {
+                const int l0 = (int)((unsigned)s0.y >> 16), len = s0.y & 0xffff;
+                bulk_g2s(st.spos + l0, pos + s0.x, (unsigned)len * 16u, bar);
+                if (QUAT) bulk_g2s(st.squat + l0, quat + s0.x, (unsigned)len * 16u, bar);
+            }
+        }
+        for (int sg = tid + 32 * SEG_PRE; sg < bi.nseg; sg += 32) {
             const int2 s0 = seg[sg];
-            const int len = (sg + 1 < bi.nseg ? seg[sg + 1].y : bi.M) - s0.y;
-            bulk_g2s(st.spos + s0.y, pos + s0.x, (unsigned)len * 16u, bar);
-            if (QUAT) bulk_g2s(st.squat + s0.y, quat + s0.x, (unsigned)len * 16u, bar);
+            const int l0 = (int)((unsigned)s0.y >> 16), len = s0.y & 0xffff;
+            bulk_g2s(st.spos + l0, pos + s0.x, (unsigned)len * 16u, bar);
+            if (QUAT) bulk_g2s(st.squat + l0, quat + s0.x, (unsigned)len * 16u, bar);
         }
     }
     if (tid == 32) {
@@ -704,21 +748,21 @@ __global__ void __launch_bounds__(MD_TB, 4) k_vertex_lj_staged(DevParams P, DevB
                                                             float4* __restrict__ force) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int b = blockIdx.x;
+    // everything the block needs from global memory before it can compute is requested at once: the block header, the
+    // head of its segment table, |L_i| and the first four row chunks (rows hold >= 8 chunks; chunks past |L_i| are
+    // loaded but never consumed)
+    const SegPre pre = seg_preload(B, b);
+    const int i = b * MD_TB + threadIdx.x;
+    const bool live = i < P.N;
+    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + threadIdx.x;
+    const uint2 pkA = ld_row(rowb), pkB = ld_row(rowb + MD_TB), pkC = ld_row(rowb + 2 * MD_TB), pkD = ld_row(rowb + 3 * MD_TB);
+    const int cnt = live ? B.row_count[i] : 0;
     const BlkInfo bi = B.blk[b];
     if (bi.M <= 0 || bi.M + 1 > stage_entries) {   // build failed for this block / launch sized too small: latch, never guess
         if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
         return;
     }
-    const Stage st = stage_issue<false>(P, B, bi, b, stage_entries, pos, nullptr, smraw);
-    // while the copies are in flight: |L_i| and the first two row chunks
-    const int i = b * MD_TB + threadIdx.x;
-    const bool live = i < P.N;
-    const int cnt = live ? B.row_count[i] : 0;
-    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + threadIdx.x;
-    const uint2 pkA = cnt > 0 ? ld_row(rowb) : make_uint2(0u, 0u);
-    const uint2 pkB = cnt > 4 ? ld_row(rowb + MD_TB) : make_uint2(0u, 0u);
-    const uint2 pkC = cnt > 8 ? ld_row(rowb + 2 * MD_TB) : make_uint2(0u, 0u);
-    const uint2 pkD = cnt > 12 ? ld_row(rowb + 3 * MD_TB) : make_uint2(0u, 0u);
+    const Stage st = stage_issue<false>(P, B, bi, b, stage_entries, pre, pos, nullptr, smraw);
     stage_wait(P, bi, st, smraw);
     if (!live) return;
     const bool bonds = P.kind == MD_POT_FENE_WCA;
@@ -790,7 +834,8 @@ __global__ void __launch_bounds__(MD_TB) k_vertex_patchy_staged(DevParams P, Dev
         if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
         return;
     }
-    const Stage st = stage_issue<true>(P, B, bi, b, stage_entries, pos, quat, smraw);
+    const SegPre pre = seg_preload(B, b);
+    const Stage st = stage_issue<true>(P, B, bi, b, stage_entries, pre, pos, quat, smraw);
     stage_wait(P, bi, st, smraw);
     if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_patchy_rows<true>(P, B, bi, st, b, force, torque);
     else vertex_patchy_rows<false>(P, B, bi, st, b, force, torque);
