@@ -168,6 +168,10 @@ void make_cell_rank(const int nc[3], int order, std::vector<int>& rank) {
     for (int64_t r = 0; r < ncell; ++r) rank[(size_t)keys[(size_t)r].second] = (int)r;
 }
 
+void drop_step_graph(md_system* s) {
+    if (s->step_exec) { cudaGraphExecDestroy(s->step_exec); s->step_exec = nullptr; }
+}
+
 md_status fail(md_system* s, md_status code, const char* msg) {
     if (s) snprintf(s->errmsg, sizeof(s->errmsg), "%s", msg);
     return code;
@@ -356,6 +360,7 @@ md_status md_bind_state(md_system* s, void* pos, void* vel, void* force, void* q
     s->torque = s->rigid ? (float4*)torque : nullptr;
     s->bound = true;
     s->cells_valid = s->lists_valid = s->forces_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
+    drop_step_graph(s);   // the step graph bakes the state pointers in
     reset_ids(s);   // the arrays are taken to be in original id order
     return check_cuda(s, "md_bind_state");
 }
@@ -365,6 +370,7 @@ md_status md_set_order(md_system* s, int32_t order) {
     if (s->sticky) return (md_status)s->sticky;
     if (order < MD_ORDER_NONE || order > MD_ORDER_HILBERT) return fail(s, MD_ERR_INVALID, "md_set_order: unknown order");
     s->order = order;
+    drop_step_graph(s);
     std::vector<int> rank;
     int nc[3] = { s->P.ncx, s->P.ncy, s->P.ncz };
     make_cell_rank(nc, order, rank);
@@ -440,6 +446,80 @@ static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatt
     return MD_OK;
 }
 
+// One step of md_integrate captured as a graph.  The rebuild chain (cells, reordering, Verlet rows, bookkeeping) sits
+// in the body of a conditional IF node: when the skin flag is clear it costs nothing, where the plain-launch path pays
+// a dozen gated no-op kernels per step.  Returns false (and leaves no graph) if any graph call fails.
+#define GCHK(call) do { if (ok) { cudaError_t e_ = (call); if (e_ != cudaSuccess) { ok = false; \
+    snprintf(s->errmsg, sizeof(s->errmsg), "step graph: %s -> %s", #call, cudaGetErrorString(e_)); \
+    if (getenv("MD_B200_DEBUG")) fprintf(stderr, "%s\n", s->errmsg); } } } while (0)
+static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t scatter, bool staged, bool seg) {
+    drop_step_graph(s);
+    // capture happens on two internal streams (the caller's stream may be the legacy default stream, which cannot be
+    // captured); the instantiated graph is launched on the caller's stream
+    if (!s->aux_stream && cudaStreamCreateWithFlags(&s->aux_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
+    if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
+    const int64_t launches0 = s->launches;
+    cudaStream_t user_stream = s->stream;
+    cudaStream_t main_stream = s->cap_stream;
+    s->stream = main_stream;
+    cudaGraph_t graph = nullptr;
+    bool ok = true;
+    GCHK(cudaStreamBeginCapture(main_stream, cudaStreamCaptureModeRelaxed));
+    if (!ok) { cudaGetLastError(); s->stream = user_stream; return false; }
+    cudaStreamCaptureStatus st;
+    cudaGraph_t cg = nullptr;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t ndeps = 0;
+    cudaGraphConditionalHandle handle = 0;
+    GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
+    GCHK(cudaGraphConditionalHandleCreate(&handle, cg, 0, cudaGraphCondAssignDefault));
+    if (ok) {
+        md_launch_kick_drift(s, fdt);            // sets the device rebuild flag (S:A5)
+        md_launch_set_cond(s, handle);
+        GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
+    }
+    cudaGraphNode_t cond_node = nullptr;
+    if (ok) {
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = handle;
+        np.conditional.type = cudaGraphCondTypeIf;
+        np.conditional.size = 1;
+        GCHK(cudaGraphAddNode(&cond_node, cg, deps, ndeps, &np));
+        if (ok) {
+            cudaGraph_t body = np.conditional.phGraph_out[0];
+            GCHK(cudaStreamBeginCaptureToGraph(s->aux_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+            if (ok) {
+                s->stream = s->aux_stream;
+                md_launch_build_cells(s, true);
+                if (staged) md_launch_build_staged(s, true);
+                else md_launch_build_verlet(s, true, s->pos);
+                if (seg) md_launch_seg_index(s, true);
+                md_launch_build_end(s, true);
+                s->stream = main_stream;
+                cudaGraph_t tmp = nullptr;
+                GCHK(cudaStreamEndCapture(s->aux_stream, &tmp));
+            }
+        }
+        GCHK(cudaStreamUpdateCaptureDependencies(main_stream, &cond_node, 1, cudaStreamSetCaptureDependencies));
+    }
+    const int64_t before_tail = s->launches;
+    if (ok) {
+        ok = launch_forces_any(s, strategy, scatter) == MD_OK;
+        md_launch_kick(s, fdt);
+    }
+    const int tail_nodes = (int)(s->launches - before_tail);
+    { cudaError_t e_ = cudaStreamEndCapture(main_stream, &graph); if (e_ != cudaSuccess) { if (ok && getenv("MD_B200_DEBUG")) fprintf(stderr, "step graph: end capture -> %s\n", cudaGetErrorString(e_)); ok = false; } }
+    s->launches = launches0;
+    s->stream = user_stream;
+    GCHK(cudaGraphInstantiate(&s->step_exec, graph, 0));
+    if (graph) cudaGraphDestroy(graph);
+    if (!ok) { cudaGetLastError(); drop_step_graph(s); return false; }
+    s->step_strategy = strategy; s->step_variant = scatter; s->step_dt = fdt; s->step_stage = s->stage_launch;
+    s->step_nodes = 2 + tail_nodes;   // kernels outside the conditional body
+    return true;
+}
+
 md_status md_forces(md_system* s, int32_t strategy, int32_t scatter) {
     if (!s) return MD_ERR_INVALID;
     if (s->sticky) return (md_status)s->sticky;
@@ -473,7 +553,20 @@ md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy
     if (!staged) ensure_explicit(s);
     if (seg && !s->seg_valid) { md_launch_seg_index(s, false); s->seg_valid = true; }
     const float fdt = (float)dt;
-    for (int64_t k = 0; k < nsteps; ++k) {
+    int64_t k0 = 0;
+    if (!s->graphs_off && nsteps > 0) {
+        if (!s->step_exec || s->step_strategy != strategy || s->step_variant != scatter || s->step_dt != fdt ||
+            s->step_stage != s->stage_launch) {
+            if (!build_step_graph(s, fdt, strategy, scatter, staged, seg)) s->graphs_off = true;
+        }
+        if (s->step_exec) {
+            for (; k0 < nsteps; ++k0) {
+                if (cudaGraphLaunch(s->step_exec, s->stream) != cudaSuccess) break;
+                s->launches += s->step_nodes;
+            }
+        }
+    }
+    for (int64_t k = k0; k < nsteps; ++k) {
         md_launch_kick_drift(s, fdt);            // sets the device rebuild flag (S:A5)
         md_launch_build_cells(s, true);          // gated on the flag: no host synchronisation (S:H6)
         if (staged) md_launch_build_staged(s, true);
@@ -598,6 +691,9 @@ const char* md_last_error(const md_system* s) { return s ? s->errmsg : "null han
 
 void md_destroy(md_system* s) {
     if (!s) return;
+    drop_step_graph(s);
+    if (s->aux_stream) cudaStreamDestroy(s->aux_stream);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     free(s);
 }
 

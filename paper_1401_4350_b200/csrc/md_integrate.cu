@@ -65,6 +65,14 @@ __global__ void __launch_bounds__(256) k_kick(DevParams P, float dt, float4* __r
     }
 }
 
+// drives the IF node of the step graph: run the rebuild body iff the skin criterion tripped (S:A5)
+__global__ void k_set_cond(cudaGraphConditionalHandle h, DevBuffers B) { cudaGraphSetConditional(h, B.ctrl->rebuild != 0 ? 1u : 0u); }
+
+void md_launch_set_cond(md_system* s, unsigned long long cond_handle) {
+    k_set_cond<<<1, 1, 0, s->stream>>>((cudaGraphConditionalHandle)cond_handle, s->B);
+    s->launches += 1;
+}
+
 void md_launch_kick_drift(md_system* s, float dt) {
     int nb = cdiv(s->P.N, 256);
     if (s->rigid) k_kick_drift<true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);

@@ -137,6 +137,13 @@ struct md_system {
     void* workspace;
     size_t workspace_bytes;
     int* h_cell_rank;        // host copy (built at create)
+    // one velocity-Verlet step as an executable CUDA graph: kick+drift, rebuild inside a conditional IF node that the
+    // device-side skin flag drives, forces, kick (md_api.cu build_step_graph)
+    cudaGraphExec_t step_exec;
+    cudaStream_t cap_stream, aux_stream; // internal capture streams: main sequence, conditional body
+    int step_strategy, step_variant, step_stage, step_nodes;
+    float step_dt;
+    bool graphs_off;                     // graph construction failed once: plain launches from then on
 };
 
 // ---- kernel launch entry points (defined in the .cu files) ----
@@ -149,6 +156,7 @@ void md_launch_forces(md_system* s, int strategy, int scatter);
 void md_launch_kick_drift(md_system* s, float dt);
 void md_launch_kick(md_system* s, float dt);
 void md_launch_energy(md_system* s);
+void md_launch_set_cond(md_system* s, unsigned long long cond_handle);   // conditional value = rebuild flag
 void md_launch_unpermute(md_system* s, const float4* src, float4* dst);   // dst[ids[s]] = src[s]
 // staged path (md_staged.cu)
 void md_launch_build_staged(md_system* s, bool gated);
