@@ -292,6 +292,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.band_rv = (float)(P.rv2d * 1e-6);    // S:Q6 band of the list predicate
     P.nblk = g.nblk; P.stage_cap = g.stage_cap; P.rcap = g.rcap; P.pad1 = 0;
     P.skinf = (float)skin;
+    P.shift_margin = (float)(rv + skin);
     s->stage_launch = g.stage_cap;
     P.kind = pot->kind;
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;

@@ -61,6 +61,7 @@ struct DevParams {
     float rv2, band_rv;                // fp32 list radius^2 and its fp64-recheck band (S:Q6)
     int nblk, stage_cap, rcap, pad1;   // staged path: blocks of MD_TB slots, smem capacity (particles), row capacity (entries)
     float skinf;
+    float shift_margin;                // r_v + skin: see k_build_staged step 7c
     // pair potential
     int kind;
     float eps, sig2, mass, inv_mass;

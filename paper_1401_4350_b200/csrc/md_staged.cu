@@ -123,12 +123,12 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
             const int s = t % 27;
             const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
             int ax = cx + s / 9 - 1, ay = cy + (s / 3) % 3 - 1, az = cz + s % 3 - 1;
-            int wrapped = 0;
-            if (ax < 0) { ax += P.ncx; wrapped = 1; } else if (ax >= P.ncx) { ax -= P.ncx; wrapped = 1; }
-            if (ay < 0) { ay += P.ncy; wrapped = 1; } else if (ay >= P.ncy) { ay -= P.ncy; wrapped = 1; }
-            if (az < 0) { az += P.ncz; wrapped = 1; } else if (az >= P.ncz) { az -= P.ncz; wrapped = 1; }
+            int wrapped = 0;   // bit a: the stencil crosses the periodic face of axis a
+            if (ax < 0) { ax += P.ncx; wrapped |= 1; } else if (ax >= P.ncx) { ax -= P.ncx; wrapped |= 1; }
+            if (ay < 0) { ay += P.ncy; wrapped |= 2; } else if (ay >= P.ncy) { ay -= P.ncy; wrapped |= 2; }
+            if (az < 0) { az += P.ncz; wrapped |= 4; } else if (az >= P.ncz) { az -= P.ncz; wrapped |= 4; }
             // fewer than 3 cells on an axis: the wrap lands on a cell of the axis again; duplicates vanish in the unique step
-            if (wrapped) atomicOr(&s_flags, MD_BLK_WRAP);
+            if (wrapped) atomicOr(&s_flags, wrapped);
             const int r = B.cell_rank[(ax * P.ncy + ay) * P.ncz + az];
             v = (B.cell_start[r + 1] > B.cell_start[r]) ? r : 0x7fffffff;   // empty cells contribute nothing
         }
@@ -268,9 +268,39 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     }
     __syncthreads();
     const int own_base = s_own_base;
-    const bool maywrap = (s_flags & MD_BLK_WRAP) != 0 || P.ncx < 3 || P.ncy < 3 || P.ncz < 3;
+    // 7c. periodic blocks.  wrap_axes = axes on which the neighbourhood crosses a periodic face.  The shift-down transform
+    //     T(x) = x > L/2 ? x - L : x (exact in fp32, Sterbenz) turns every minimum image of a listed pair into a plain
+    //     difference provided no pair straddles L/2 unwrapped, now or before the next rebuild: guaranteed when no staged
+    //     coordinate of a wrapped axis lies within r_v + skin of L/2 (always true unless the box is a few cells wide).
+    //     Then the staged copy is transformed and the scan below needs no minimum image; else the block is flagged for
+    //     the minimum-image variants of the scan and of the force kernels.
+    const int wrap_axes = s_flags & 7;
     __syncthreads();
-    if (tid == 0) s_flags = 0;   // from here on: bit 0 = a listed pair wraps, bits 2..4 = axes, bit 5 = shift transform fails
+    if (tid == 0) s_flags = 0;   // from here on: bit a = axis a violates the margin criterion
+    __syncthreads();
+    if (wrap_axes) {
+        int bad = 0;
+        for (int t = tid; t < M; t += MD_TB) {
+            const float4 x = spos[t];
+            if ((wrap_axes & 1) && fabsf(x.x - P.hLx) <= P.shift_margin) bad |= 1;
+            if ((wrap_axes & 2) && fabsf(x.y - P.hLy) <= P.shift_margin) bad |= 2;
+            if ((wrap_axes & 4) && fabsf(x.z - P.hLz) <= P.shift_margin) bad |= 4;
+        }
+        if (bad) atomicOr(&s_flags, bad);
+    }
+    __syncthreads();
+    const bool small_box = P.ncx < 3 || P.ncy < 3 || P.ncz < 3;
+    const bool shift_ok = wrap_axes != 0 && (s_flags & 7) == 0 && !small_box;
+    const bool maywrap = (wrap_axes != 0 && !shift_ok) || small_box;
+    if (shift_ok) {
+        for (int t = tid; t < M; t += MD_TB) {
+            float4 x = spos[t];
+            if ((wrap_axes & 1) && x.x > P.hLx) x.x -= P.Lx;
+            if ((wrap_axes & 2) && x.y > P.hLy) x.y -= P.Ly;
+            if ((wrap_axes & 4) && x.z > P.hLz) x.z -= P.Lz;
+            spos[t] = x;
+        }
+    }
     __syncthreads();
 
     // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6).  Pass A writes the
@@ -278,7 +308,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     //    them per shared-memory bank column (local index mod 8: one float4 = one of the 8 16-byte columns of a wavefront).
     unsigned short* s_rem = reinterpret_cast<unsigned short*>(own_rank + MD_TB);   // [8][MD_TB] entries left per column
     unsigned short* s_cur = s_rem + 8 * MD_TB;                                        // [8][MD_TB] scan cursor per column
-    int cnt = 0, lo_cnt = 0, flags = 0;
+    int cnt = 0, lo_cnt = 0;
     float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
     // scan-order scratch row, block-transposed (entry k of thread tid at k * MD_TB + tid): lanes of a warp sit at
     // similar k, so both passes touch a few sectors per warp access instead of one per lane
@@ -290,6 +320,30 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         xi = spos[me];
         const float hLx = P.hLx, hLy = P.hLy, hLz = P.hLz;
         const int* __restrict__ mycells = cand + myoc * 27;
+        if (!maywrap) {
+            // interior blocks (the common case): no minimum image, no wrap bookkeeping; the listed-pair branch is
+            // reduced to a predicated store so that the 32 lanes of a warp stay converged over the candidate loop
+            const float rv2 = P.rv2, bandv = P.band_rv;
+            const int cap = P.cap;
+            for (int sc = 0; sc < 27; ++sc) {
+                const int u = mycells[sc];
+                if (u < 0) continue;
+                const int t1 = ubase[u + 1];
+#pragma unroll 4
+                for (int t = ubase[u]; t < t1; ++t) {
+                    const float4 xj = spos[t];
+                    const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
+                    const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
+                    const float tt = d2 - rv2;
+                    bool in = tt < 0.0f;
+                    if (fabsf(tt) < bandv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
+                    in = in && (t != me);
+                    if (in && cnt < cap) tmp[(size_t)cnt * MD_TB] = (unsigned short)t;
+                    cnt += in ? 1 : 0;
+                    lo_cnt += (in && t < me) ? 1 : 0;
+                }
+            }
+        } else
         for (int sc = 0; sc < 27; ++sc) {
             const int u = mycells[sc];
             if (u < 0) continue;
@@ -308,26 +362,9 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                 bool in = tt < 0.0f;
                 if (fabsf(tt) < P.band_rv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
                 if (in) {
-                    if (cnt < P.cap) { tmp[(size_t)cnt * MD_TB] = (unsigned short)t; s_rem[(t & 7) * MD_TB + tid] += 1; }
+                    if (cnt < P.cap) tmp[(size_t)cnt * MD_TB] = (unsigned short)t;
                     ++cnt;
                     lo_cnt += (t < me);
-                    if (maywrap) {
-                        // which axes wrap, and does the shift-down transform T(x) = x > L/2 ? x - L : x reproduce the image?
-                        const float rx = xj.x - xi.x, ry = xj.y - xi.y, rz = xj.z - xi.z;
-                        if (fabsf(rx) > hLx) flags |= 1 | (MD_BLK_AXIS_SHIFT << 0);
-                        if (fabsf(ry) > hLy) flags |= 1 | (MD_BLK_AXIS_SHIFT << 1);
-                        if (fabsf(rz) > hLz) flags |= 1 | (MD_BLK_AXIS_SHIFT << 2);
-                        const float tx = (xj.x > hLx ? xj.x - P.Lx : xj.x) - (xi.x > hLx ? xi.x - P.Lx : xi.x);
-                        const float ty = (xj.y > hLy ? xj.y - P.Ly : xj.y) - (xi.y > hLy ? xi.y - P.Ly : xi.y);
-                        const float tz = (xj.z > hLz ? xj.z - P.Lz : xj.z) - (xi.z > hLz ? xi.z - P.Lz : xi.z);
-                        if ((fabsf(rx) > hLx && tx != ddx) || (fabsf(ry) > hLy && ty != ddy) || (fabsf(rz) > hLz && tz != ddz)) flags |= 32;
-                        // an axis that is shifted must also keep its unwrapped pairs intact
-                        // ... and stay valid while the particles move by up to skin/2 before the next build
-                        const float sk = P.skinf;
-                        if ((fabsf(rx) <= hLx && tx != ddx) || fabsf(xj.x - hLx) <= sk || fabsf(xi.x - hLx) <= sk) flags |= 64 << 0;
-                        if ((fabsf(ry) <= hLy && ty != ddy) || fabsf(xj.y - hLy) <= sk || fabsf(xi.y - hLy) <= sk) flags |= 64 << 1;
-                        if ((fabsf(rz) <= hLz && tz != ddz) || fabsf(xj.z - hLz) <= sk || fabsf(xi.z - hLz) <= sk) flags |= 64 << 2;
-                    }
                 }
             }
         }
@@ -348,6 +385,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         // counting sort of the scratch row by column into a second scratch row: s_cur[c] ends as the END of column c
         unsigned short* __restrict__ tmp2 = tmp + (size_t)P.nblk * P.rcap * MD_TB;
         {
+            for (int k = 0; k < c2; ++k) s_rem[(tmp[(size_t)k * MD_TB] & 7) * MD_TB + tid] += 1;   // entries per column
             int acc = 0;
 #pragma unroll
             for (int c = 0; c < 8; ++c) { s_cur[c * MD_TB + tid] = (unsigned short)acc; acc += s_rem[c * MD_TB + tid]; }
@@ -382,10 +420,9 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
             B.row_count[i] = c2;
             B.lo_count[i] = cnt > P.cap ? 0 : lo_cnt;
             B.half_count[i] = cnt > P.cap ? 0 : cnt - lo_cnt;
-            B.pos_ref[i] = xi;
+            B.pos_ref[i] = pos[i];      // the skin reference is the untransformed position
         }
     }
-    if (flags) atomicOr(&s_flags, flags);
     // 9. block totals
     int tot_full, tot_half;
     blk_excl_scan(min(cnt, P.cap), &tot_full, sh_scan);
@@ -394,13 +431,10 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     if ((tid & 31) == 0) atomicMax(&B.ctrl->max_seen, seen);
     __syncthreads();
     if (tid == 0) {
-        const int f = s_flags;
         int out = 0;
-        if (f & 1) {
-            out = MD_BLK_WRAP | (f & (7 * MD_BLK_AXIS_SHIFT));
-            // the transform is usable if no wrapped pair disagrees and no SHIFTED axis breaks an unwrapped pair
-            const int shifted = (f >> 2) & 7, broken = (f >> 6) & 7;
-            if (!(f & 32) && !(shifted & broken)) out |= MD_BLK_SHIFT_OK;
+        if (wrap_axes || small_box) {
+            out = MD_BLK_WRAP | (wrap_axes * MD_BLK_AXIS_SHIFT);
+            if (shift_ok) out |= MD_BLK_SHIFT_OK;
         }
         if (M + 1 <= 4096) out |= MD_BLK_SH4;
         B.blk[b] = BlkInfo{ nseg, M, own_base, out };
