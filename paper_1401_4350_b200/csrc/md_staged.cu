@@ -620,7 +620,7 @@ __device__ __forceinline__ void stage_wait(const DevParams& P, const BlkInfo bi,
 // positions come from the block's shared-memory neighbourhood by 128-bit gathers whose bank columns were
 // de-conflicted at build time (k_build_staged pass B).  No atomics, every pair computed twice.
 // ------------------------------------------------------------------------------------------------
-struct LJAccS { float fx, fy, fz, band; float2 pe; };
+struct LJAccS { float fx, fy, fz, band; float2 pe, nin; };
 
 // streamed row chunk: read once per evaluation, so it bypasses L1 allocation (the L1 left beside the staged
 // neighbourhoods is small) (no_allocate)
@@ -631,10 +631,13 @@ __device__ __forceinline__ uint2 ld_row(const uint2* p) {
 }
 
 // staged position of a row entry: entries hold (local index << SH); SH == 4 makes the entry the byte offset
+// sp32 = 32-bit shared-window address of the staged array, computed once per thread
 template <int SH>
-__device__ __forceinline__ float4 staged_pos(const float4* sp, unsigned int e) {
-    if (SH == 4) return *reinterpret_cast<const float4*>(reinterpret_cast<const char*>(sp) + e);
-    return sp[e];
+__device__ __forceinline__ float4 staged_pos(unsigned int sp32, unsigned int e) {
+    float4 v;
+    const unsigned int a = sp32 + (SH == 4 ? e : (e << 4));
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
 }
 
 // Two visits (a, b) at once.  Distances and the force accumulation are scalar fp32; the chain in between --
@@ -724,43 +727,83 @@ __device__ __forceinline__ void fene_vertex_s(const DevParams& P, const DevBuffe
     }
 }
 
-template <bool IMG, int SH>
-__device__ __forceinline__ void lj_chunk_s(const DevParams& P, const float4* sp, float4 xi, uint2 cur, LJAccS& a) {
-    const float4 x0 = staged_pos<SH>(sp, cur.x & 0xffffu), x1 = staged_pos<SH>(sp, cur.x >> 16);
-    const float4 x2 = staged_pos<SH>(sp, cur.y & 0xffffu), x3 = staged_pos<SH>(sp, cur.y >> 16);
-    lj_visit2_s<IMG>(P, xi, x0, x1, a);
-    lj_visit2_s<IMG>(P, xi, x2, x3, a);
+// The same two visits in reduced units for sigma == 1 (every BASELINE config): with s = m / d2 the sums
+//   A = sum (s^4 - 2 s^7) d,  pe = sum (s^6 - s^3),  nin = sum m
+// need no potential constants inside the loop (F_i = 24 eps A, V = 4 eps pe - V_c nin are applied once per particle),
+// which removes the per-chunk constant reloads and eight registers.  a.pe holds sum (s^6 - s^3), a.nin the count.
+template <bool IMG>
+__device__ __forceinline__ void lj_visit2_unit_s(const DevParams& P, float4 xi, float4 xa, float4 xb, LJAccS& a) {
+    float dxa, dya, dza, dxb, dyb, dzb;
+    if (IMG) {
+        dxa = min_image(xa.x, xi.x, P.Lx, P.hLx); dya = min_image(xa.y, xi.y, P.Ly, P.hLy); dza = min_image(xa.z, xi.z, P.Lz, P.hLz);
+        dxb = min_image(xb.x, xi.x, P.Lx, P.hLx); dyb = min_image(xb.y, xi.y, P.Ly, P.hLy); dzb = min_image(xb.z, xi.z, P.Lz, P.hLz);
+    } else {
+        dxa = xa.x - xi.x; dya = xa.y - xi.y; dza = xa.z - xi.z;
+        dxb = xb.x - xi.x; dyb = xb.y - xi.y; dzb = xb.z - xi.z;
+    }
+    const float2 d2 = make_float2(fmaf(dza, dza, fmaf(dya, dya, dxa * dxa)), fmaf(dzb, dzb, fmaf(dyb, dyb, dxb * dxb)));
+    const float2 t = __fadd2_rn(d2, P.k_nrc2);
+    const float2 m = make_float2(t.x < 0.0f ? 1.0f : 0.0f, t.y < 0.0f ? 1.0f : 0.0f);
+    a.band = fminf(fminf(a.band, fabsf(t.x)), fabsf(t.y));
+    const float2 inv = make_float2(rcp_approx(d2.x), rcp_approx(d2.y));
+    const float2 s = __fmul2_rn(inv, m);
+    const float2 s2 = __fmul2_rn(s, s);
+    const float2 z3 = __fmul2_rn(s2, s);
+    const float2 z4 = __fmul2_rn(s2, s2);
+    const float2 z7 = __fmul2_rn(z4, z3);
+    const float2 ng = __ffma2_rn(z7, make_float2(-2.0f, -2.0f), z4);
+    a.fx = fmaf(ng.x, dxa, a.fx); a.fy = fmaf(ng.x, dya, a.fy); a.fz = fmaf(ng.x, dza, a.fz);
+    a.fx = fmaf(ng.y, dxb, a.fx); a.fy = fmaf(ng.y, dyb, a.fy); a.fz = fmaf(ng.y, dzb, a.fz);
+    a.pe = __fadd2_rn(a.pe, __ffma2_rn(z3, z3, make_float2(-z3.x, -z3.y)));
+    a.nin = __fadd2_rn(a.nin, m);
+}
+
+template <bool IMG, int SH, bool UNIT>
+__device__ __forceinline__ void lj_chunk_s(const DevParams& P, unsigned int sp32, float4 xi, uint2 cur, LJAccS& a) {
+    const float4 x0 = staged_pos<SH>(sp32, cur.x & 0xffffu), x1 = staged_pos<SH>(sp32, cur.x >> 16);
+    const float4 x2 = staged_pos<SH>(sp32, cur.y & 0xffffu), x3 = staged_pos<SH>(sp32, cur.y >> 16);
+    if (UNIT) {
+        lj_visit2_unit_s<IMG>(P, xi, x0, x1, a);
+        lj_visit2_unit_s<IMG>(P, xi, x2, x3, a);
+    } else {
+        lj_visit2_s<IMG>(P, xi, x0, x1, a);
+        lj_visit2_s<IMG>(P, xi, x2, x3, a);
+    }
 }
 
 // cnt, pk[0..3]: |L_i| and the first four row chunks, loaded by the caller while the staging copies were in flight.
 // The row streams from HBM (~1300 cycles under load); chunks are consumed four per iteration through four separate
 // load instructions, each re-issued four chunks (~350 instructions of arithmetic) ahead of its use.
-template <bool IMG, int SH>
+template <bool IMG, int SH, bool UNIT>
 __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int i,
                                                int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB, uint2 pkC, uint2 pkD,
                                                const float4* __restrict__ pos, float4* __restrict__ force, bool bonds) {
     const float4 xi = st.spos[bi.own_base + threadIdx.x];
-    const float4* sp = st.spos;
+    const unsigned int sp = smem_u32(st.spos);
     const int nch = (cnt + 3) >> 2;                        // the last chunk is padded with the dummy entry
-    LJAccS a = { 0.f, 0.f, 0.f, 3.0e38f, make_float2(0.f, 0.f) };
+    LJAccS a = { 0.f, 0.f, 0.f, 3.0e38f, make_float2(0.f, 0.f), make_float2(0.f, 0.f) };
     for (int c = 0; c < nch; c += 4) {
         const uint2 curA = pkA;
         if (c + 4 < nch) pkA = ld_row(rowb + (size_t)(c + 4) * MD_TB);
-        lj_chunk_s<IMG, SH>(P, sp, xi, curA, a);
+        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curA, a);
         if (c + 1 >= nch) break;
         const uint2 curB = pkB;
         if (c + 5 < nch) pkB = ld_row(rowb + (size_t)(c + 5) * MD_TB);
-        lj_chunk_s<IMG, SH>(P, sp, xi, curB, a);
+        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curB, a);
         if (c + 2 >= nch) break;
         const uint2 curC = pkC;
         if (c + 6 < nch) pkC = ld_row(rowb + (size_t)(c + 6) * MD_TB);
-        lj_chunk_s<IMG, SH>(P, sp, xi, curC, a);
+        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curC, a);
         if (c + 3 >= nch) break;
         const uint2 curD = pkD;
         if (c + 7 < nch) pkD = ld_row(rowb + (size_t)(c + 7) * MD_TB);
-        lj_chunk_s<IMG, SH>(P, sp, xi, curD, a);
+        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curD, a);
     }
     float pe2 = a.pe.x + a.pe.y;
+    if (UNIT) {   // back from reduced units: F = 24 eps A, V = 4 eps sum (s^6 - s^3) - V_c nin
+        a.fx *= P.c24; a.fy *= P.c24; a.fz *= P.c24;
+        pe2 = fmaf(P.c4, pe2, -P.vshift * (a.nin.x + a.nin.y));
+    }
     if (a.band < P.band_abs) {
         float4* scratch = force + i;           // own output slot as scratch (rewritten below)
         *scratch = make_float4(a.fx, a.fy, a.fz, pe2);
@@ -801,13 +844,16 @@ __global__ void __launch_bounds__(MD_TB, 4) k_vertex_lj_staged(DevParams P, DevB
     if (!live) return;
     const bool bonds = P.kind == MD_POT_FENE_WCA;
     const bool img = (bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK);
+    const bool unit = P.sig2 == 1.0f;
+#define LJ_ROWS(IMG_, SH_, UNIT_) vertex_lj_rows<IMG_, SH_, UNIT_>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds)
     if (bi.flags & MD_BLK_SH4) {
-        if (img) vertex_lj_rows<true, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
-        else vertex_lj_rows<false, 4>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
+        if (unit) { if (img) LJ_ROWS(true, 4, true); else LJ_ROWS(false, 4, true); }
+        else { if (img) LJ_ROWS(true, 4, false); else LJ_ROWS(false, 4, false); }
     } else {
-        if (img) vertex_lj_rows<true, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
-        else vertex_lj_rows<false, 0>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds);
+        if (unit) { if (img) LJ_ROWS(true, 0, true); else LJ_ROWS(false, 0, true); }
+        else { if (img) LJ_ROWS(true, 0, false); else LJ_ROWS(false, 0, false); }
     }
+#undef LJ_ROWS
 }
 
 // ------------------------------------------------------------------------------------------------
