@@ -542,17 +542,16 @@ struct Stage {
     float4* squat;   // [M + 1]  rigid bodies only
 };
 
-// the first SEG_PRE table entries of each lane of warp 0, loaded at kernel entry together with the block header so
-// that the staging copies wait for ONE memory latency instead of two
-#define SEG_PRE 4
-struct SegPre { int2 e[SEG_PRE]; };
+// Segment copies are issued by ALL warps: a bulk copy takes uniform operands, so the lanes of a warp issue theirs one
+// after the other; spreading the ~100 segments of a block over its 8 warps (segment l*8+w to lane l of warp w) cuts
+// the issue chain from ~100 to ~13 copies.  Each thread's first table entry is loaded at kernel entry together with
+// the block header, so the staging copies wait for ONE memory latency.
+struct SegPre { int2 e; int sg; };
 __device__ __forceinline__ SegPre seg_preload(const DevBuffers& B, int b) {
     SegPre sp;
-    const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
-    if (threadIdx.x < 32) {
-#pragma unroll
-        for (int q = 0; q < SEG_PRE; ++q) sp.e[q] = seg[threadIdx.x + 32 * q];   // always inside the table; entries >= nseg are ignored
-    }
+    const int nw = blockDim.x >> 5;
+    sp.sg = (threadIdx.x & 31) * nw + (threadIdx.x >> 5);
+    sp.e = B.seg[(size_t)b * MD_SEGMAX + sp.sg];   // always inside the table; entries >= nseg are ignored
     return sp;
 }
 
@@ -566,33 +565,26 @@ __device__ __forceinline__ Stage stage_issue(const DevParams& P, const DevBuffer
     st.squat = QUAT ? st.spos + stage_entries : nullptr;
     const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
     const int tid = threadIdx.x;
-    if (tid < 32) {
-        if (tid == 0) {
-            mbar_init(bar, 1);
-            mbar_expect_tx(bar, (unsigned)bi.M * 16u * (QUAT ? 2u : 1u));
-        }
-        __syncwarp();
-#pragma unroll
-        for (int q = 0; q < SEG_PRE; ++q) {
-            const int2 s0 = pre.e[q];
-            if (tid + 32 * q < bi.nseg) {
-                const int l0 = (int)((unsigned)s0.y >> 16), len = s0.y & 0xffff;
-                bulk_g2s(st.spos + l0, pos + s0.x, (unsigned)len * 16u, bar);
-                if (QUAT) bulk_g2s(st.squat + l0, quat + s0.x, (unsigned)len * 16u, bar);
-            }
-        }
-        for (int sg = tid + 32 * SEG_PRE; sg < bi.nseg; sg += 32) {
-            const int2 s0 = seg[sg];
-            const int l0 = (int)((unsigned)s0.y >> 16), len = s0.y & 0xffff;
-            bulk_g2s(st.spos + l0, pos + s0.x, (unsigned)len * 16u, bar);
-            if (QUAT) bulk_g2s(st.squat + l0, quat + s0.x, (unsigned)len * 16u, bar);
-        }
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_expect_tx(bar, (unsigned)bi.M * 16u * (QUAT ? 2u : 1u));
     }
     if (tid == 32) {
         st.spos[bi.M] = make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
         if (QUAT) st.squat[bi.M] = make_float4(1.f, 0.f, 0.f, 0.f);
     }
-    __syncthreads();          // barrier initialised, dummy written
+    __syncthreads();          // barrier initialised and armed before any copy is issued; dummy entry written
+    if (pre.sg < bi.nseg) {
+        const int l0 = (int)((unsigned)pre.e.y >> 16), len = pre.e.y & 0xffff;
+        bulk_g2s(st.spos + l0, pos + pre.e.x, (unsigned)len * 16u, bar);
+        if (QUAT) bulk_g2s(st.squat + l0, quat + pre.e.x, (unsigned)len * 16u, bar);
+    }
+    for (int sg = pre.sg + (int)blockDim.x; sg < bi.nseg; sg += blockDim.x) {
+        const int2 s0 = seg[sg];
+        const int l0 = (int)((unsigned)s0.y >> 16), len = s0.y & 0xffff;
+        bulk_g2s(st.spos + l0, pos + s0.x, (unsigned)len * 16u, bar);
+        if (QUAT) bulk_g2s(st.squat + l0, quat + s0.x, (unsigned)len * 16u, bar);
+    }
     return st;
 }
 
