@@ -279,15 +279,16 @@ def main():
     t_dom = fe[f"{dom}_{args.scatter}"]["us"]
     abytes = algorithmic_bytes(dom, Ef, N)
     achieved = abytes / (t_dom * 1e-6) / 1e9
+    knames = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp": "k_edge_warp", "red": "k_edge_red", "red_v4": "k_edge_red",
+              "segmented": "k_edge_store+k_edge_segsum"}
     traffic = None
-    tf = ROOT / "profiles" / "roofline_traffic.json"
+    tf = ROOT / "profiles" / "roofline_traffic.csv"     # dram bytes per launch from the committed ncu --set full capture
     if tf.exists():
-        try:
-            traffic = json.loads(tf.read_text()).get(f"{args.workload}_{dom}")
-        except Exception:
-            traffic = None
-    kname = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp": "k_edge_warp",
-             "red": "k_edge_red", "red_v4": "k_edge_red", "segmented": "k_edge_store+k_edge_segsum"}[args.scatter]
+        for ln in tf.read_text().splitlines()[1:]:
+            f = ln.split(",")
+            if len(f) >= 4 and f[0] == args.workload and f[1] == dom and f[2] == knames[args.scatter]:
+                traffic = float(f[3])
+    kname = knames[args.scatter]
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "algorithmic_bytes_per_launch": abytes, "us_per_launch": t_dom, "peak_source": peak_src}

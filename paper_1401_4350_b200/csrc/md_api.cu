@@ -555,6 +555,7 @@ md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy
     if (seg && !s->seg_valid) { md_launch_seg_index(s, false); s->seg_valid = true; }
     const float fdt = (float)dt;
     int64_t k0 = 0;
+    if (!s->graphs_off && getenv("MD_B200_NO_GRAPH")) s->graphs_off = true;   // plain launches (profilers list every kernel)
     if (!s->graphs_off && nsteps > 0) {
         if (!s->step_exec || s->step_strategy != strategy || s->step_variant != scatter || s->step_dt != fdt ||
             s->step_stage != s->stage_launch) {
