@@ -323,26 +323,47 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         if (!maywrap) {
             // interior blocks (the common case): no minimum image, no wrap bookkeeping; the listed-pair branch is
             // reduced to a predicated store so that the 32 lanes of a warp stay converged over the candidate loop
+            //  The fp64 band decision (S:Q6) is kept out of the loop: the loop tracks min |d2 - r_v^2| and the rare thread
+            //  with a banded candidate (~1e-4) repeats its scan with the fp64 predicate.  lo_cnt is counted in pass B.
             const float rv2 = P.rv2, bandv = P.band_rv;
             const int cap = P.cap;
+            float bandmin = 3.0e38f;
             for (int sc = 0; sc < 27; ++sc) {
                 const int u = mycells[sc];
                 if (u < 0) continue;
                 const int t1 = ubase[u + 1];
+                const int self = sc == 13 ? me : -1;      // stencil entry 13 is the own cell
 #pragma unroll 4
                 for (int t = ubase[u]; t < t1; ++t) {
                     const float4 xj = spos[t];
                     const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
                     const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
                     const float tt = d2 - rv2;
-                    bool in = tt < 0.0f;
-                    if (fabsf(tt) < bandv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
-                    in = in && (t != me);
+                    bandmin = fminf(bandmin, fabsf(tt));
+                    const bool in = tt < 0.0f && t != self;
                     if (in && cnt < cap) tmp[(size_t)cnt * MD_TB] = (unsigned short)t;
                     cnt += in ? 1 : 0;
-                    lo_cnt += (in && t < me) ? 1 : 0;
                 }
             }
+            if (bandmin < bandv) {      // rare: repeat with the fp64 decision for banded candidates
+                cnt = 0;
+                for (int sc = 0; sc < 27; ++sc) {
+                    const int u = mycells[sc];
+                    if (u < 0) continue;
+                    const int t1 = ubase[u + 1];
+                    for (int t = ubase[u]; t < t1; ++t) {
+                        if (t == me) continue;
+                        const float4 xj = spos[t];
+                        const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
+                        const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
+                        const float tt = d2 - rv2;
+                        bool in = tt < 0.0f;
+                        if (fabsf(tt) < bandv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
+                        if (in) { if (cnt < cap) tmp[(size_t)cnt * MD_TB] = (unsigned short)t; ++cnt; }
+                    }
+                }
+            }
+            lo_cnt = -1;                // counted from the scratch row in pass B
         } else
         for (int sc = 0; sc < 27; ++sc) {
             const int u = mycells[sc];
@@ -385,23 +406,41 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         // counting sort of the scratch row by column into a second scratch row: s_cur[c] ends as the END of column c
         unsigned short* __restrict__ tmp2 = tmp + (size_t)P.nblk * P.rcap * MD_TB;
         {
-            for (int k = 0; k < c2; ++k) s_rem[(tmp[(size_t)k * MD_TB] & 7) * MD_TB + tid] += 1;   // entries per column
+            const int me_l = own_base + tid;
+            int lo_b = 0;
+            for (int k = 0; k < c2; k += 8) {            // entries per column (loads first: eight in flight)
+                unsigned short e[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) e[q] = k + q < c2 ? tmp[(size_t)(k + q) * MD_TB] : (unsigned short)0xffff;
+#pragma unroll
+                for (int q = 0; q < 8; ++q)
+                    if (k + q < c2) { s_rem[(e[q] & 7) * MD_TB + tid] += 1; lo_b += e[q] < me_l; }
+            }
+            if (lo_cnt < 0) lo_cnt = lo_b;
             int acc = 0;
 #pragma unroll
             for (int c = 0; c < 8; ++c) { s_cur[c * MD_TB + tid] = (unsigned short)acc; acc += s_rem[c * MD_TB + tid]; }
-            for (int k = 0; k < c2; ++k) {
-                const unsigned short e = tmp[(size_t)k * MD_TB];
-                const int c = e & 7;
-                const int p = s_cur[c * MD_TB + tid];
-                s_cur[c * MD_TB + tid] = (unsigned short)(p + 1);
-                tmp2[(size_t)p * MD_TB] = e;
+            for (int k = 0; k < c2; k += 8) {
+                unsigned short e[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) e[q] = k + q < c2 ? tmp[(size_t)(k + q) * MD_TB] : (unsigned short)0xffff;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    if (k + q < c2) {
+                        const int c = e[q] & 7;
+                        const int p = s_cur[c * MD_TB + tid];
+                        s_cur[c * MD_TB + tid] = (unsigned short)(p + 1);
+                        tmp2[(size_t)p * MD_TB] = e[q];
+                    }
+                }
             }
         }
         for (int k0 = 0; k0 < c2; k0 += 4) {
+            int src[4];                                   // scratch positions of the four entries (-1 = padding)
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int k = k0 + q;
-                unsigned int t = dummy;
+                src[q] = -1;
                 if (k < c2) {
                     int c = (k + tid) & 7;
                     if (s_rem[c * MD_TB + tid] == 0) {
@@ -409,11 +448,12 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                         for (int cc = 0; cc < 8; ++cc) { const int v = s_rem[cc * MD_TB + tid]; if (v > bv) { bv = v; c = cc; } }
                     }
                     const int rem = s_rem[c * MD_TB + tid];
-                    t = (unsigned int)tmp2[(size_t)(s_cur[c * MD_TB + tid] - rem) * MD_TB] << rsh;   // next unused entry of column c
+                    src[q] = s_cur[c * MD_TB + tid] - rem;    // next unused entry of column c
                     s_rem[c * MD_TB + tid] = (unsigned short)(rem - 1);
                 }
-                w[q] = t;
             }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) w[q] = src[q] >= 0 ? ((unsigned int)tmp2[(size_t)src[q] * MD_TB] << rsh) : dummy;
             rowb[(size_t)(k0 >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
         }
         if (live) {
