@@ -39,20 +39,8 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
     // staged path: rows of 16-bit local indices in chunks of 4 entries; smem capacity of the build kernel
     g->rcap = (g->cap + 31) / 32 * 32;
     g->nblk = (int)((N + MD_TB - 1) / MD_TB);
-    {
-        const double ppc = (double)N / (double)g->ncell;                 // particles per cell
-        const double own = std::min<double>(MD_TB, MD_TB / std::max(ppc, 1e-9));   // cells per block
-        const double side = cbrt(own) + 2.0;                               // stencil union of a compact blob, x1.5 for ragged shapes
-        double m = 2.0 * (1.5 * side * side * side * ppc) + 256.0;
-        m = std::min<double>(m, (double)N + 64.0);
-        // shared memory of the build kernel: positions (16 B each) + candidate/unique cell tables (md_staged.cu) <= 224 KB
-        int nc = 64;
-        while (nc < 27 * (2 * own + 4) && nc < MD_NCAND) nc <<= 1;
-        const int um = nc < MD_UMAX ? nc : MD_UMAX;
-        const double tables = 4.0 * (nc + 3.0 * um + 1 + MD_TB) + 32.0 * MD_TB + 16 + 1024;
-        m = std::min<double>(m, floor((224.0 * 1024 - tables) / 16.0) - 64.0);
-        g->stage_cap = ((int)m + 63) / 64 * 64;
-    }
+    // largest neighbourhood (entries) a force kernel can stage: 16 B (+16 B quaternion) each in <= 224 KB of shared memory
+    g->stage_cap = 0;   // set by the caller (depends on the potential)
     return true;
 }
 
@@ -290,10 +278,11 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.half_skin2 = (float)(0.25 * skin * skin);
     P.rv2 = (float)P.rv2d;
     P.band_rv = (float)(P.rv2d * 1e-6);    // S:Q6 band of the list predicate
-    P.nblk = g.nblk; P.stage_cap = g.stage_cap; P.rcap = g.rcap; P.pad1 = 0;
+    P.nblk = g.nblk; P.rcap = g.rcap; P.pad1 = 0;
+    P.stage_cap = (int)((224 * 1024 - 16) / (rigid ? 32 : 16)) - 1;
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);
-    s->stage_launch = g.stage_cap;
+    s->stage_launch = P.stage_cap;
     P.kind = pot->kind;
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
     P.sigma = pot->sigma;

@@ -83,12 +83,13 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                                                         int ncand_cap, int umax) {
     GATE(B, gated);
     extern __shared__ __align__(16) unsigned char smraw[];
-    float4* spos = reinterpret_cast<float4*>(smraw);                 // [stage_cap]
-    int* cand = reinterpret_cast<int*>(spos + P.stage_cap);          // [ncand_cap]
+    // The build reads candidate positions straight from global memory (all lanes of a warp read the same candidate: one
+    // sector, L1-resident), so its shared memory holds only the cell tables and four blocks fit on an SM.
+    int* cand = reinterpret_cast<int*>(smraw);                       // [ncand_cap]
     int* urank = cand + ncand_cap;                                   // [umax]
     int* ubase = urank + umax;                                       // [umax + 1]
-    int* ucoord = ubase + umax + 1;                                  // [umax]
-    int* own_rank = ucoord + umax;                                   // [MD_TB]
+    int* ustart = ubase + umax + 1;                                  // [umax] first slot of the cell
+    int* own_rank = ustart + umax;                                   // [MD_TB]
     __shared__ int sh_scan[33];
     __shared__ int s_flags, s_err, s_own_base;
 
@@ -176,9 +177,9 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         int c = 0;
         if (u < U) {
             const int r = urank[u];
-            c = B.cell_start[r + 1] - B.cell_start[r];
-            const int lin = B.cell_lin[r];
-            ucoord[u] = pack_coord(lin / (P.ncz * P.ncy), (lin / P.ncz) % P.ncy, lin % P.ncz);
+            const int s0 = B.cell_start[r];
+            c = B.cell_start[r + 1] - s0;
+            ustart[u] = s0;
         }
         int tot;
         const int p = blk_excl_scan(c, &tot, sh_scan);
@@ -230,11 +231,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         }
     }
 
-    // 7. stage the neighbourhood (plain coalesced copies, one warp per cell) and locate the block's own particles
-    for (int u = tid >> 5; u < U; u += MD_TB / 32) {
-        const int s0 = B.cell_start[urank[u]], l0 = ubase[u], len = ubase[u + 1] - l0;
-        for (int k = tid & 31; k < len; k += 32) spos[l0 + k] = pos[s0 + k];
-    }
+    // 7. locate the block's own particles in the local index space
     if (tid == 0) {
         const int r0 = own_rank[0];
         int lo = 0, hi = U - 1;
@@ -280,11 +277,14 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     __syncthreads();
     if (wrap_axes) {
         int bad = 0;
-        for (int t = tid; t < M; t += MD_TB) {
-            const float4 x = spos[t];
-            if ((wrap_axes & 1) && fabsf(x.x - P.hLx) <= P.shift_margin) bad |= 1;
-            if ((wrap_axes & 2) && fabsf(x.y - P.hLy) <= P.shift_margin) bad |= 2;
-            if ((wrap_axes & 4) && fabsf(x.z - P.hLz) <= P.shift_margin) bad |= 4;
+        for (int u = tid >> 5; u < U; u += MD_TB / 32) {
+            const int s0 = ustart[u], len = ubase[u + 1] - ubase[u];
+            for (int k = tid & 31; k < len; k += 32) {
+                const float4 x = pos[s0 + k];
+                if ((wrap_axes & 1) && fabsf(x.x - P.hLx) <= P.shift_margin) bad |= 1;
+                if ((wrap_axes & 2) && fabsf(x.y - P.hLy) <= P.shift_margin) bad |= 2;
+                if ((wrap_axes & 4) && fabsf(x.z - P.hLz) <= P.shift_margin) bad |= 4;
+            }
         }
         if (bad) atomicOr(&s_flags, bad);
     }
@@ -292,16 +292,18 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     const bool small_box = P.ncx < 3 || P.ncy < 3 || P.ncz < 3;
     const bool shift_ok = wrap_axes != 0 && (s_flags & 7) == 0 && !small_box;
     const bool maywrap = (wrap_axes != 0 && !shift_ok) || small_box;
-    if (shift_ok) {
-        for (int t = tid; t < M; t += MD_TB) {
-            float4 x = spos[t];
-            if ((wrap_axes & 1) && x.x > P.hLx) x.x -= P.Lx;
-            if ((wrap_axes & 2) && x.y > P.hLy) x.y -= P.Ly;
-            if ((wrap_axes & 4) && x.z > P.hLz) x.z -= P.Lz;
-            spos[t] = x;
+    // the transform is applied on the fly to the coordinates this kernel reads (and to the staged copy in the force kernels)
+    const float tLx = (shift_ok && (wrap_axes & 1)) ? P.Lx : 0.0f, tLy = (shift_ok && (wrap_axes & 2)) ? P.Ly : 0.0f,
+                tLz = (shift_ok && (wrap_axes & 4)) ? P.Lz : 0.0f;
+    auto load_pos = [&](int slot) {
+        float4 x = __ldg(pos + slot);
+        if (shift_ok) {
+            if (x.x > P.hLx) x.x -= tLx;
+            if (x.y > P.hLy) x.y -= tLy;
+            if (x.z > P.hLz) x.z -= tLz;
         }
-    }
-    __syncthreads();
+        return x;
+    };
 
     // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6).  Pass A writes the
     //    neighbours in scan order (ascending local index = ascending slot) to a thread-private scratch row and counts
@@ -317,7 +319,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     for (int c = 0; c < 8; ++c) { s_rem[c * MD_TB + tid] = 0; s_cur[c * MD_TB + tid] = 0; }
     if (live) {
         const int me = own_base + tid;
-        xi = spos[me];
+        xi = load_pos(i);
         const float hLx = P.hLx, hLy = P.hLy, hLz = P.hLz;
         const int* __restrict__ mycells = cand + myoc * 27;
         if (!maywrap) {
@@ -333,9 +335,10 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                 if (u < 0) continue;
                 const int t1 = ubase[u + 1];
                 const int self = sc == 13 ? me : -1;      // stencil entry 13 is the own cell
+                const int sdelta = ustart[u] - ubase[u];  // slot = local index + sdelta inside this cell
 #pragma unroll 4
                 for (int t = ubase[u]; t < t1; ++t) {
-                    const float4 xj = spos[t];
+                    const float4 xj = load_pos(t + sdelta);
                     const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
                     const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
                     const float tt = d2 - rv2;
@@ -351,9 +354,10 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
                     const int u = mycells[sc];
                     if (u < 0) continue;
                     const int t1 = ubase[u + 1];
+                    const int sdelta = ustart[u] - ubase[u];
                     for (int t = ubase[u]; t < t1; ++t) {
                         if (t == me) continue;
-                        const float4 xj = spos[t];
+                        const float4 xj = load_pos(t + sdelta);
                         const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
                         const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
                         const float tt = d2 - rv2;
@@ -369,9 +373,10 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
             const int u = mycells[sc];
             if (u < 0) continue;
             const int t1 = ubase[u + 1];
+            const int sdelta = ustart[u] - ubase[u];
             for (int t = ubase[u]; t < t1; ++t) {
                 if (t == me) continue;
-                const float4 xj = spos[t];
+                const float4 xj = __ldg(pos + t + sdelta);
                 float ddx, ddy, ddz;
                 if (maywrap) {
                     ddx = min_image(xj.x, xi.x, P.Lx, hLx); ddy = min_image(xj.y, xi.y, P.Ly, hLy); ddz = min_image(xj.z, xi.z, P.Lz, hLz);
@@ -505,7 +510,7 @@ static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, si
     int um = nc < MD_UMAX ? nc : MD_UMAX;
     *ncand_cap = nc;
     *umax = um;
-    *smem = 16 * (size_t)P.stage_cap + 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 2 * 2 * 8 * MD_TB + 16;
+    *smem = 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 2 * 2 * 8 * MD_TB + 16;
 }
 
 void md_launch_build_staged(md_system* s, bool gated) {
