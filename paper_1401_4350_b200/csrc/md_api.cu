@@ -158,6 +158,7 @@ void make_cell_rank(const int nc[3], int order, std::vector<int>& rank) {
 
 void drop_step_graph(md_system* s) {
     if (s->step_exec) { cudaGraphExecDestroy(s->step_exec); s->step_exec = nullptr; }
+    if (s->multi_exec) { cudaGraphExecDestroy(s->multi_exec); s->multi_exec = nullptr; }
 }
 
 md_status fail(md_system* s, md_status code, const char* msg) {
@@ -442,8 +443,8 @@ static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatt
 #define GCHK(call) do { if (ok) { cudaError_t e_ = (call); if (e_ != cudaSuccess) { ok = false; \
     snprintf(s->errmsg, sizeof(s->errmsg), "step graph: %s -> %s", #call, cudaGetErrorString(e_)); \
     if (getenv("MD_B200_DEBUG")) fprintf(stderr, "%s\n", s->errmsg); } } } while (0)
-static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t scatter, bool staged, bool seg) {
-    drop_step_graph(s);
+static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t scatter, bool staged, bool seg, int reps,
+                             cudaGraphExec_t* exec_out) {
     // capture happens on two internal streams (the caller's stream may be the legacy default stream, which cannot be
     // captured); the instantiated graph is launched on the caller's stream
     if (!s->aux_stream && cudaStreamCreateWithFlags(&s->aux_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
@@ -460,6 +461,8 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     cudaGraph_t cg = nullptr;
     const cudaGraphNode_t* deps = nullptr;
     size_t ndeps = 0;
+    int tail_nodes = 0;
+    for (int rep_i = 0; rep_i < reps && ok; ++rep_i) {   // `reps` consecutive steps in one graph, one IF node each
     cudaGraphConditionalHandle handle = 0;
     GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
     GCHK(cudaGraphConditionalHandleCreate(&handle, cg, 0, cudaGraphCondAssignDefault));
@@ -498,11 +501,12 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
         ok = launch_forces_any(s, strategy, scatter) == MD_OK;
         md_launch_kick(s, fdt);
     }
-    const int tail_nodes = (int)(s->launches - before_tail);
+    tail_nodes = (int)(s->launches - before_tail);
+    }
     { cudaError_t e_ = cudaStreamEndCapture(main_stream, &graph); if (e_ != cudaSuccess) { if (ok && getenv("MD_B200_DEBUG")) fprintf(stderr, "step graph: end capture -> %s\n", cudaGetErrorString(e_)); ok = false; } }
     s->launches = launches0;
     s->stream = user_stream;
-    GCHK(cudaGraphInstantiate(&s->step_exec, graph, 0));
+    GCHK(cudaGraphInstantiate(exec_out, graph, 0));
     if (graph) cudaGraphDestroy(graph);
     if (!ok) { cudaGetLastError(); drop_step_graph(s); return false; }
     s->step_strategy = strategy; s->step_variant = scatter; s->step_dt = fdt; s->step_stage = s->stage_launch;
@@ -548,12 +552,16 @@ md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy
     if (!s->graphs_off && nsteps > 0) {
         if (!s->step_exec || s->step_strategy != strategy || s->step_variant != scatter || s->step_dt != fdt ||
             s->step_stage != s->stage_launch) {
-            if (!build_step_graph(s, fdt, strategy, scatter, staged, seg)) s->graphs_off = true;
+            drop_step_graph(s);
+            if (!build_step_graph(s, fdt, strategy, scatter, staged, seg, 1, &s->step_exec) ||
+                !build_step_graph(s, fdt, strategy, scatter, staged, seg, MD_GRAPH_STEPS, &s->multi_exec)) s->graphs_off = true;
         }
-        if (s->step_exec) {
-            for (; k0 < nsteps; ++k0) {
-                if (cudaGraphLaunch(s->step_exec, s->stream) != cudaSuccess) break;
-                s->launches += s->step_nodes;
+        if (s->step_exec && s->multi_exec) {
+            while (k0 < nsteps) {      // MD_GRAPH_STEPS steps per launch while they fit, single steps for the rest
+                const bool multi = nsteps - k0 >= MD_GRAPH_STEPS;
+                if (cudaGraphLaunch(multi ? s->multi_exec : s->step_exec, s->stream) != cudaSuccess) break;
+                k0 += multi ? MD_GRAPH_STEPS : 1;
+                s->launches += (int64_t)s->step_nodes * (multi ? MD_GRAPH_STEPS : 1);
             }
         }
     }

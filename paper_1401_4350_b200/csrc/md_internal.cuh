@@ -8,6 +8,7 @@
 
 #define MD_TILE 32            // particles per list tile (one warp)
 #define MD_MAX_PATCH 8
+#define MD_GRAPH_STEPS 8        // steps per launch of the multi-step graph of md_integrate
 
 // Device error bits latched in DevCtrl::err
 #define MD_DEVERR_CAPACITY 1
@@ -140,7 +141,7 @@ struct md_system {
     int* h_cell_rank;        // host copy (built at create)
     // one velocity-Verlet step as an executable CUDA graph: kick+drift, rebuild inside a conditional IF node that the
     // device-side skin flag drives, forces, kick (md_api.cu build_step_graph)
-    cudaGraphExec_t step_exec;
+    cudaGraphExec_t step_exec, multi_exec;   // one step / MD_GRAPH_STEPS steps per launch
     cudaStream_t cap_stream, aux_stream; // internal capture streams: main sequence, conditional body
     int step_strategy, step_variant, step_stage, step_nodes;
     float step_dt;
