@@ -76,6 +76,31 @@ __device__ __forceinline__ int blk_excl_scan(int v, int* tot, int* sh /* >= 33 i
 
 __device__ __forceinline__ int pack_coord(int cx, int cy, int cz) { return cx | (cy << 10) | (cz << 20); }
 
+// Candidate scan of one stencil cell for interior / shift-transformed blocks: all lanes of a warp walk the same cell, so
+// the loop is kept branch-free: a predicated store at the thread's write offset, which advances (by one scratch row)
+// when the candidate is inside r_v (sign bit of d2 - r_v^2), clamped at the overflow row cap + 1.
+template <bool SHIFT, bool SELF>
+__device__ __forceinline__ void scan_cell_fast(const float4* __restrict__ cellpos, int n, int t0, int me, float4 xi, float rv2,
+                                               float hLx, float hLy, float hLz, float tLx, float tLy, float tLz,
+                                               unsigned short* tmp_blk, unsigned int& off, unsigned int offmax, float& bandmin) {
+#pragma unroll 8
+    for (int k = 0; k < n; ++k) {
+        float4 xj = __ldg(cellpos + k);
+        if (SHIFT) {
+            if (xj.x > hLx) xj.x -= tLx;
+            if (xj.y > hLy) xj.y -= tLy;
+            if (xj.z > hLz) xj.z -= tLz;
+        }
+        const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
+        const float tt = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)) - rv2;
+        bandmin = fminf(bandmin, fabsf(tt));
+        int m = __float_as_int(tt) >> 31;                  // -1 inside r_v, 0 outside
+        if (SELF) m = (t0 + k == me) ? 0 : m;
+        if (m) *reinterpret_cast<unsigned short*>(reinterpret_cast<char*>(tmp_blk) + off) = (unsigned short)(t0 + k);
+        off = min(off + ((unsigned int)m & (2u * MD_TB)), offmax);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // S:A4 staged Verlet build.  One block per MD_TB slots, one thread per particle.
 // ------------------------------------------------------------------------------------------------
@@ -314,7 +339,9 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
     float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
     // scan-order scratch row, block-transposed (entry k of thread tid at k * MD_TB + tid): lanes of a warp sit at
     // similar k, so both passes touch a few sectors per warp access instead of one per lane
-    unsigned short* __restrict__ tmp = B.rows_tmp + (size_t)b * P.rcap * MD_TB + tid;
+    const size_t tstride = (size_t)(P.rcap + 2) * MD_TB;        // scratch rows per block (cap + 2: overflow row)
+    unsigned short* tmp_blk = B.rows_tmp + (size_t)b * tstride;
+    unsigned short* tmp = tmp_blk + tid;
 #pragma unroll
     for (int c = 0; c < 8; ++c) { s_rem[c * MD_TB + tid] = 0; s_cur[c * MD_TB + tid] = 0; }
     if (live) {
@@ -330,24 +357,22 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
             const float rv2 = P.rv2, bandv = P.band_rv;
             const int cap = P.cap;
             float bandmin = 3.0e38f;
+            unsigned int off = 2u * tid;
+            const unsigned int offmax = (unsigned int)(cap + 1) * (2u * MD_TB) + 2u * tid;
             for (int sc = 0; sc < 27; ++sc) {
                 const int u = mycells[sc];
                 if (u < 0) continue;
-                const int t1 = ubase[u + 1];
-                const int self = sc == 13 ? me : -1;      // stencil entry 13 is the own cell
-                const int sdelta = ustart[u] - ubase[u];  // slot = local index + sdelta inside this cell
-#pragma unroll 4
-                for (int t = ubase[u]; t < t1; ++t) {
-                    const float4 xj = load_pos(t + sdelta);
-                    const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
-                    const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
-                    const float tt = d2 - rv2;
-                    bandmin = fminf(bandmin, fabsf(tt));
-                    const bool in = tt < 0.0f && t != self;
-                    if (in && cnt < cap) tmp[(size_t)cnt * MD_TB] = (unsigned short)t;
-                    cnt += in ? 1 : 0;
+                const int t0 = ubase[u], n = ubase[u + 1] - t0;
+                const float4* cellpos = pos + ustart[u];
+                if (sc == 13) {                           // stencil entry 13 is the own cell: exclude the particle itself
+                    if (shift_ok) scan_cell_fast<true, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
+                    else scan_cell_fast<false, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
+                } else {
+                    if (shift_ok) scan_cell_fast<true, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
+                    else scan_cell_fast<false, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
                 }
             }
+            cnt = (int)((off - 2u * tid) / (2u * MD_TB));   // cap + 1 = overflow
             if (bandmin < bandv) {      // rare: repeat with the fp64 decision for banded candidates
                 cnt = 0;
                 for (int sc = 0; sc < 27; ++sc) {
@@ -409,7 +434,7 @@ __global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers 
         const int rsh = (M + 1 <= 4096) ? 4 : 0;   // MD_BLK_SH4: entries are byte offsets into the staged float4 array
         const unsigned int dummy = (unsigned int)M << rsh;
         // counting sort of the scratch row by column into a second scratch row: s_cur[c] ends as the END of column c
-        unsigned short* __restrict__ tmp2 = tmp + (size_t)P.nblk * P.rcap * MD_TB;
+        unsigned short* __restrict__ tmp2 = tmp + (size_t)P.nblk * tstride;
         {
             const int me_l = own_base + tid;
             int lo_b = 0;
