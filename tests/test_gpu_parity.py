@@ -125,6 +125,27 @@ def test_vertex_and_segmented_are_bitwise_reproducible(MD):
         s.close()
 
 
+def test_step_graph_equals_plain_launches(MD, monkeypatch):
+    """md_integrate replays a CUDA graph (rebuild inside a conditional node, 8 steps per launch); with
+    MD_B200_NO_GRAPH=1 it launches the same kernels one by one.  VERTEX is deterministic, so both give the same bits,
+    the same number of device-side rebuilds, and 37 steps exercise the multi-step graph and the single-step tail."""
+    w = W.lj_fluid(2 ** 14)
+    out = []
+    for no_graph in (False, True):
+        if no_graph:
+            monkeypatch.setenv("MD_B200_NO_GRAPH", "1")
+        s = MD.from_workload(w, order="hilbert")
+        s.build_cells(); s.build_verlet(); s.forces("vertex", "smem")
+        l0 = s.launch_count()
+        s.integrate(w.dt, 37, "vertex", "smem")
+        per_step = (s.launch_count() - l0) / 37
+        out.append((s.in_id_order(s.pos), s.in_id_order(s.vel), s.stats()["n_rebuilds"], per_step))
+        s.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert out[0][2] == out[1][2] and out[0][2] >= 1
+    assert out[0][3] == 4 and out[1][3] > 4        # graph: kick+drift, condition, forces, kick
+
+
 def test_error_paths(MD):
     from paper_1401_4350_b200 import MDError
     w = W.config("C1")
