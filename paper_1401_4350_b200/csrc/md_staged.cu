@@ -12,6 +12,7 @@
 //     instead of one 128-byte L1 line per lane from global memory (profiles/r01a_first_path.md).
 // The pair arithmetic, the fp64 recheck band (S:H10) and all tolerances are those of md_forces.cu.
 #include <stdio.h>
+#include <stdlib.h>
 #include "md_pair.cuh"
 
 #define GATE(B, gated) if ((gated) && (B).ctrl->rebuild == 0) return
@@ -547,6 +548,8 @@ void md_launch_build_staged(md_system* s, bool gated) {
     static bool attr_done = false;
     if (!attr_done) {
         cudaFuncSetAttribute(k_build_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+        // candidates are read through L1: leave it as large as the four resident blocks allow
+        cudaFuncSetAttribute(k_build_staged, cudaFuncAttributePreferredSharedMemoryCarveout, 50);   // measured: 25 -> 1.96 ms, 50 -> 1.65, 75 -> 1.82, 100 -> 2.02
         attr_done = true;
     }
     k_staged_begin<<<1, 1, 0, s->stream>>>(s->B, g);
