@@ -105,7 +105,7 @@ __device__ __forceinline__ void scan_cell_fast(const float4* __restrict__ cellpo
 // ------------------------------------------------------------------------------------------------
 // S:A4 staged Verlet build.  One block per MD_TB slots, one thread per particle.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(MD_TB) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
+__global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
                                                         int ncand_cap, int umax) {
     GATE(B, gated);
     extern __shared__ __align__(16) unsigned char smraw[];
