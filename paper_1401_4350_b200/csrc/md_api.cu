@@ -444,7 +444,7 @@ static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatt
     snprintf(s->errmsg, sizeof(s->errmsg), "step graph: %s -> %s", #call, cudaGetErrorString(e_)); \
     if (getenv("MD_B200_DEBUG")) fprintf(stderr, "%s\n", s->errmsg); } } } while (0)
 static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t scatter, bool staged, bool seg, int reps,
-                             cudaGraphExec_t* exec_out) {
+                             cudaGraphExec_t* exec_out, int* nodes_out) {
     // capture happens on two internal streams (the caller's stream may be the legacy default stream, which cannot be
     // captured); the instantiated graph is launched on the caller's stream
     if (!s->aux_stream && cudaStreamCreateWithFlags(&s->aux_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
@@ -461,13 +461,13 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     cudaGraph_t cg = nullptr;
     const cudaGraphNode_t* deps = nullptr;
     size_t ndeps = 0;
-    int tail_nodes = 0;
+    int tail_nodes = 0, main_nodes = 0;
     for (int rep_i = 0; rep_i < reps && ok; ++rep_i) {   // `reps` consecutive steps in one graph, one IF node each
     cudaGraphConditionalHandle handle = 0;
     GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
     GCHK(cudaGraphConditionalHandleCreate(&handle, cg, 0, cudaGraphCondAssignDefault));
     if (ok) {
-        md_launch_kick_drift(s, fdt);            // sets the device rebuild flag (S:A5)
+        md_launch_kick_drift(s, fdt, rep_i > 0);   // sets the device rebuild flag (S:A5); carries the previous step's closing kick
         md_launch_set_cond(s, handle);
         GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
     }
@@ -499,9 +499,10 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     const int64_t before_tail = s->launches;
     if (ok) {
         ok = launch_forces_any(s, strategy, scatter) == MD_OK;
-        md_launch_kick(s, fdt);
+        if (rep_i == reps - 1) md_launch_kick(s, fdt);   // inner steps: fused into the next kick+drift
     }
     tail_nodes = (int)(s->launches - before_tail);
+    main_nodes += 2 + tail_nodes;   // kernels outside the conditional body
     }
     { cudaError_t e_ = cudaStreamEndCapture(main_stream, &graph); if (e_ != cudaSuccess) { if (ok && getenv("MD_B200_DEBUG")) fprintf(stderr, "step graph: end capture -> %s\n", cudaGetErrorString(e_)); ok = false; } }
     s->launches = launches0;
@@ -510,7 +511,7 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     if (graph) cudaGraphDestroy(graph);
     if (!ok) { cudaGetLastError(); drop_step_graph(s); return false; }
     s->step_strategy = strategy; s->step_variant = scatter; s->step_dt = fdt; s->step_stage = s->stage_launch;
-    s->step_nodes = 2 + tail_nodes;   // kernels outside the conditional body
+    *nodes_out = main_nodes;
     return true;
 }
 
@@ -553,20 +554,20 @@ md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy
         if (!s->step_exec || s->step_strategy != strategy || s->step_variant != scatter || s->step_dt != fdt ||
             s->step_stage != s->stage_launch) {
             drop_step_graph(s);
-            if (!build_step_graph(s, fdt, strategy, scatter, staged, seg, 1, &s->step_exec) ||
-                !build_step_graph(s, fdt, strategy, scatter, staged, seg, MD_GRAPH_STEPS, &s->multi_exec)) s->graphs_off = true;
+            if (!build_step_graph(s, fdt, strategy, scatter, staged, seg, 1, &s->step_exec, &s->step_nodes) ||
+                !build_step_graph(s, fdt, strategy, scatter, staged, seg, MD_GRAPH_STEPS, &s->multi_exec, &s->multi_nodes)) s->graphs_off = true;
         }
         if (s->step_exec && s->multi_exec) {
             while (k0 < nsteps) {      // MD_GRAPH_STEPS steps per launch while they fit, single steps for the rest
                 const bool multi = nsteps - k0 >= MD_GRAPH_STEPS;
                 if (cudaGraphLaunch(multi ? s->multi_exec : s->step_exec, s->stream) != cudaSuccess) break;
                 k0 += multi ? MD_GRAPH_STEPS : 1;
-                s->launches += (int64_t)s->step_nodes * (multi ? MD_GRAPH_STEPS : 1);
+                s->launches += multi ? s->multi_nodes : s->step_nodes;
             }
         }
     }
     for (int64_t k = k0; k < nsteps; ++k) {
-        md_launch_kick_drift(s, fdt);            // sets the device rebuild flag (S:A5)
+        md_launch_kick_drift(s, fdt, false);     // sets the device rebuild flag (S:A5)
         md_launch_build_cells(s, true);          // gated on the flag: no host synchronisation (S:H6)
         if (staged) md_launch_build_staged(s, true);
         else md_launch_build_verlet(s, true, s->pos);

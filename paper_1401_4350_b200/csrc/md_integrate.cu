@@ -5,8 +5,10 @@
 
 static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
-// first half: v += dt/2 F/m ; [L += dt/2 tau ; q <- dq (x) q] ; x += dt v ; skin check
-template <bool RIGID>
+// first half: v += dt/2 F/m ; [L += dt/2 tau ; q <- dq (x) q] ; x += dt v ; skin check.
+// PRE: the closing half kick of the previous step is applied first, in this kernel (same two roundings as k_kick
+// followed by this kernel: inside a multi-step graph the separate k_kick launch and its pass over vel/force are saved).
+template <bool RIGID, bool PRE>
 __global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, float dt, float4* __restrict__ pos, float4* __restrict__ vel,
                                                     const float4* __restrict__ force, float4* __restrict__ quat,
                                                     float4* __restrict__ angmom, const float4* __restrict__ torque) {
@@ -15,6 +17,7 @@ __global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, f
     if (i < P.N) {
         const float hk = 0.5f * dt * P.inv_mass;
         float4 v = vel[i], f = force[i], x = pos[i];
+        if (PRE) { v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z); }
         v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z);
         x.x = fmaf(dt, v.x, x.x); x.y = fmaf(dt, v.y, x.y); x.z = fmaf(dt, v.z, x.z);
         vel[i] = v;
@@ -22,6 +25,7 @@ __global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, f
         if (RIGID) {
             float4 L = angmom[i], t = torque[i], q = quat[i];
             const float hd = 0.5f * dt;
+            if (PRE) { L.x = fmaf(hd, t.x, L.x); L.y = fmaf(hd, t.y, L.y); L.z = fmaf(hd, t.z, L.z); }
             L.x = fmaf(hd, t.x, L.x); L.y = fmaf(hd, t.y, L.y); L.z = fmaf(hd, t.z, L.z);
             angmom[i] = L;
             float wx = L.x * P.inv_inertia, wy = L.y * P.inv_inertia, wz = L.z * P.inv_inertia;
@@ -73,10 +77,15 @@ void md_launch_set_cond(md_system* s, unsigned long long cond_handle) {
     s->launches += 1;
 }
 
-void md_launch_kick_drift(md_system* s, float dt) {
+void md_launch_kick_drift(md_system* s, float dt, bool pre) {
     int nb = cdiv(s->P.N, 256);
-    if (s->rigid) k_kick_drift<true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
-    else k_kick_drift<false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
+    if (s->rigid) {
+        if (pre) k_kick_drift<true, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
+        else k_kick_drift<true, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
+    } else {
+        if (pre) k_kick_drift<false, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
+        else k_kick_drift<false, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
+    }
     s->launches += 1;
 }
 

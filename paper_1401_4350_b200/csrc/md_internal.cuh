@@ -143,7 +143,7 @@ struct md_system {
     // device-side skin flag drives, forces, kick (md_api.cu build_step_graph)
     cudaGraphExec_t step_exec, multi_exec;   // one step / MD_GRAPH_STEPS steps per launch
     cudaStream_t cap_stream, aux_stream; // internal capture streams: main sequence, conditional body
-    int step_strategy, step_variant, step_stage, step_nodes;
+    int step_strategy, step_variant, step_stage, step_nodes, multi_nodes;   // *_nodes: kernels per launch outside the IF body
     float step_dt;
     bool graphs_off;                     // graph construction failed once: plain launches from then on
 };
@@ -155,7 +155,7 @@ void md_launch_edge_offsets(md_system* s, bool gated);   // edge_off = exclusive
 void md_launch_seg_index(md_system* s, bool gated);
 void md_launch_build_end(md_system* s, bool gated);
 void md_launch_forces(md_system* s, int strategy, int scatter);
-void md_launch_kick_drift(md_system* s, float dt);
+void md_launch_kick_drift(md_system* s, float dt, bool pre);   // pre: also the previous step's closing half kick
 void md_launch_kick(md_system* s, float dt);
 void md_launch_energy(md_system* s);
 void md_launch_set_cond(md_system* s, unsigned long long cond_handle);   // conditional value = rebuild flag
