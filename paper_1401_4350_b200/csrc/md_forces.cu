@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(128, 8) k_vertex_lj(DevParams P, DevBuffers B,
 
 template <bool IMG>
 __device__ __forceinline__ void vertex_patchy_visit(const DevParams& P, const float4* __restrict__ pos, const float4* __restrict__ quat,
-                                                    float4 xi, float4 qi, int j, float& fx, float& fy, float& fz, float& pe,
+                                                    float4 xi, const Rot& Ri, int j, float& fx, float& fy, float& fz, float& pe,
                                                     float& tx, float& ty, float& tz) {
     float4 xj = ldg4(pos + j);
     float dx, dy, dz;
@@ -170,7 +170,8 @@ __device__ __forceinline__ void vertex_patchy_visit(const DevParams& P, const fl
     if (in_cutoff(P, d2, xi, xj)) {
         float4 qj = ldg4(quat + j);
         float gx, gy, gz, V, a, b, c, u, v, w;
-        patchy_pair<false>(P, dx, dy, dz, d2, qi, qj, gx, gy, gz, V, a, b, c, u, v, w);
+        if (P.n_patches == 4) patchy_pair<false, 4>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, b, c, u, v, w);
+        else patchy_pair<false, 0>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, b, c, u, v, w);
         fx -= gx; fy -= gy; fz -= gz;
         tx += a; ty += b; tz += c;
         pe += V;
@@ -188,10 +189,11 @@ __global__ void __launch_bounds__(128) k_vertex_patchy(DevParams P, DevBuffers B
     const float4 xi = pos[i], qi = quat[i];
     const int* __restrict__ row = B.nl_full + ((size_t)tile * P.capg * MD_TILE + lane) * 4;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
+    const Rot Ri = quat_to_rot(qi);     // once per particle
     for (int k = 0; k < cnt; ++k) {
         int j = row[(k >> 2) * (MD_TILE * 4) + (k & 3)];
-        if (info.x >> 30) vertex_patchy_visit<true>(P, pos, quat, xi, qi, j, fx, fy, fz, pe, tx, ty, tz);
-        else vertex_patchy_visit<false>(P, pos, quat, xi, qi, j, fx, fy, fz, pe, tx, ty, tz);
+        if (info.x >> 30) vertex_patchy_visit<true>(P, pos, quat, xi, Ri, j, fx, fy, fz, pe, tx, ty, tz);
+        else vertex_patchy_visit<false>(P, pos, quat, xi, Ri, j, fx, fy, fz, pe, tx, ty, tz);
     }
     force[i] = make_float4(fx, fy, fz, 0.5f * pe);
     torque[i] = make_float4(tx, ty, tz, 0.f);
@@ -225,7 +227,9 @@ __device__ __forceinline__ bool edge_eval(const DevParams& P, const float4* __re
     if (!in_cutoff(P, d2, xi, xj)) return false;
     if (KIND == MD_POT_PATCHY) {
         float4 qi = ldg4(quat + i), qj = ldg4(quat + j);
-        patchy_pair<true>(P, dx, dy, dz, d2, qi, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
+        const Rot Ri = quat_to_rot(qi);
+        if (P.n_patches == 4) patchy_pair<true, 4>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
+        else patchy_pair<true, 0>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
     } else {
         float g;
         lj_pair(P, d2, g, V);

@@ -83,15 +83,18 @@ __device__ __forceinline__ Rot quat_to_rot(float4 q) {   // q = (w,x,y,z) stored
 
 // angular factor of one particle (S:O4, factorised form): with v = R^T * dir (dir = +u for i, -u for j)
 //   A = sum_a exp((b_a.v - 1)/w^2),   S = (1/w^2) R sum_a e_a b_a
-__device__ __forceinline__ void patch_factor(const DevParams& P, float4 q, float ux, float uy, float uz,
+// NP = number of patches known at compile time (4: the tetrahedral model of config 4, fully unrolled), 0 = P.n_patches
+template <int NP>
+__device__ __forceinline__ void patch_factor(const DevParams& P, const Rot& R, float ux, float uy, float uz,
                                              float& A, float& Sx, float& Sy, float& Sz) {
-    Rot R = quat_to_rot(q);
     float vx = R.m[0][0] * ux + R.m[1][0] * uy + R.m[2][0] * uz;
     float vy = R.m[0][1] * ux + R.m[1][1] * uy + R.m[2][1] * uz;
     float vz = R.m[0][2] * ux + R.m[1][2] * uy + R.m[2][2] * uz;
     const float k = P.inv_w2 * 1.4426950408889634f;   // exp(x) = 2^(x log2 e)
     float a = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
-    for (int p = 0; p < P.n_patches; ++p) {
+    const int np = NP > 0 ? NP : P.n_patches;
+#pragma unroll
+    for (int p = 0; p < np; ++p) {
         float c = P.pdir[p][0] * vx + P.pdir[p][1] * vy + P.pdir[p][2] * vz;
         float e = ex2_approx((c - 1.0f) * k);
         a += e;
@@ -104,16 +107,18 @@ __device__ __forceinline__ void patch_factor(const DevParams& P, float4 q, float
 }
 
 // O4 (B:10): WCA core + patch term.  Outputs force on j (fx,fy,fz), V, torque on i, torque on j.
-template <bool NEED_TJ>
-__device__ __forceinline__ void patchy_pair(const DevParams& P, float dx, float dy, float dz, float d2, float4 qi, float4 qj,
+// Ri = rotation matrix of particle i (callers that keep i fixed over a loop compute it once).
+template <bool NEED_TJ, int NP>
+__device__ __forceinline__ void patchy_pair(const DevParams& P, float dx, float dy, float dz, float d2, const Rot& Ri, float4 qj,
                                             float& fx, float& fy, float& fz, float& V,
                                             float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
     float rinv = rsqrt_approx(d2);
     float r = d2 * rinv;
     float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
     float Ai, Six, Siy, Siz, Aj, Sjx, Sjy, Sjz;
-    patch_factor(P, qi, ux, uy, uz, Ai, Six, Siy, Siz);
-    patch_factor(P, qj, -ux, -uy, -uz, Aj, Sjx, Sjy, Sjz);
+    const Rot Rj = quat_to_rot(qj);
+    patch_factor<NP>(P, Ri, ux, uy, uz, Ai, Six, Siy, Siz);
+    patch_factor<NP>(P, Rj, -ux, -uy, -uz, Aj, Sjx, Sjy, Sjz);
     float dr = r - P.sigma;
     float G = ex2_approx(-dr * dr * P.inv_2sr2 * 1.4426950408889634f);
     float dG = -dr * P.inv_sr2 * G;

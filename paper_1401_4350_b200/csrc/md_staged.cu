@@ -925,7 +925,7 @@ __global__ void __launch_bounds__(MD_TB, 4) k_vertex_lj_staged(DevParams P, DevB
 // VERTEX, patchy rigid bodies, staged: positions and quaternions of the neighbourhood in shared memory
 // ------------------------------------------------------------------------------------------------
 template <bool IMG>
-__device__ __forceinline__ void patchy_visit_s(const DevParams& P, const Stage& st, float4 xi, float4 qi, unsigned int t,
+__device__ __forceinline__ void patchy_visit_s(const DevParams& P, const Stage& st, float4 xi, const Rot& Ri, unsigned int t,
                                                float& fx, float& fy, float& fz, float& pe, float& tx, float& ty, float& tz) {
     const float4 xj = st.spos[t];
     float dx, dy, dz;
@@ -938,7 +938,8 @@ __device__ __forceinline__ void patchy_visit_s(const DevParams& P, const Stage& 
     if (in_cutoff(P, d2, xi, xj)) {
         const float4 qj = st.squat[t];
         float gx, gy, gz, V, a, bb, c, u, v, w;
-        patchy_pair<false>(P, dx, dy, dz, d2, qi, qj, gx, gy, gz, V, a, bb, c, u, v, w);
+        if (P.n_patches == 4) patchy_pair<false, 4>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, bb, c, u, v, w);
+        else patchy_pair<false, 0>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, bb, c, u, v, w);
         fx -= gx; fy -= gy; fz -= gz;
         tx += a; ty += bb; tz += c;
         pe += V;
@@ -958,12 +959,13 @@ __device__ __forceinline__ void vertex_patchy_rows(const DevParams& P, const Dev
     const int nch = (cnt + 3) >> 2;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
     const int sh = (bi.flags & MD_BLK_SH4) ? 4 : 0;
+    const Rot Ri = quat_to_rot(qi);     // once per particle
     for (int c = 0; c < nch; ++c) {
         const uint2 cur = __ldg(rowb + (size_t)c * MD_TB);     // padding entries = dummy (far away -> outside the cutoff)
-        patchy_visit_s<IMG>(P, st, xi, qi, (cur.x & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
-        patchy_visit_s<IMG>(P, st, xi, qi, (cur.x >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
-        patchy_visit_s<IMG>(P, st, xi, qi, (cur.y & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
-        patchy_visit_s<IMG>(P, st, xi, qi, (cur.y >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.x & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.x >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.y & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.y >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
     }
     force[i] = make_float4(fx, fy, fz, 0.5f * pe);
     torque[i] = make_float4(tx, ty, tz, 0.f);
