@@ -33,6 +33,13 @@ import numpy as np
 METRIC = "pair interactions/s (Verlet pairs E per force evaluation / time), VERTEX vs EDGE, LJ N=2^20"
 UNIT = "pair interactions/s"
 EDGE_VARIANTS = ["red", "red_v4", "warp", "segmented"]
+WORKLOAD_TEXT = {
+    "C1": "BASELINE.json configs[0], LJ fluid N=2048 rho=0.8 rc=2.5 skin=0.3, fcc+jitter",
+    "C2a": "BASELINE.json configs[1], LJ fluid N=2^20 rho=0.8 rc=2.5 skin=0.3, fcc+jitter",
+    "C2b": "BASELINE.json configs[1] many-neighbour variant, LJ fluid N=2^20 rho=0.8 rc=4.0 skin=0.3, fcc+jitter",
+    "C3": "BASELINE.json configs[2], bead-spring melt 4096 x 64, rho=0.85, FENE + WCA, skin=0.3, seeded walks + push-off",
+    "C4": "BASELINE.json configs[3], patchy rigid bodies N=2^18 rho=0.5, WCA core + 4 tetrahedral patches, rc=1.5 skin=0.3",
+}
 VERTEX_VARIANTS = ["smem", "l2"]
 
 
@@ -49,11 +56,13 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def algorithmic_bytes(strategy: str, E: int, N: int) -> float:
-    """VERTEX 4(2E) + 4N + 16N + 16N; EDGE 8E + 16N + 2*16N (LJ: pos in, force out)."""
+def algorithmic_bytes(strategy: str, E: int, N: int, rigid: bool = False) -> float:
+    """VERTEX 4(2E) + 4N + S_in N + S_out N; EDGE 8E + S_in N + 2 S_out N, with S_in = 16 (pos) [+16 quat]
+    and S_out = 16 (force) [+16 torque]."""
+    s_in = s_out = 32.0 if rigid else 16.0
     if strategy == "vertex":
-        return 4.0 * 2 * E + 4.0 * N + 16.0 * N + 16.0 * N
-    return 8.0 * E + 16.0 * N + 2 * 16.0 * N
+        return 4.0 * 2 * E + 4.0 * N + s_in * N + s_out * N
+    return 8.0 * E + s_in * N + 2 * s_out * N
 
 
 class ClockSampler:
@@ -189,7 +198,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2a", choices=["C2a", "C2b"])
+    ap.add_argument("--workload", default="C2a", choices=["C1", "C2a", "C2b", "C3", "C4"],
+                    help="BASELINE.json config; the headline metric is quoted on C2a (default)")
     ap.add_argument("--strategy", default="vertex", choices=["vertex", "edge"])
     ap.add_argument("--scatter", default=None, choices=EDGE_VARIANTS + VERTEX_VARIANTS,
                     help="EDGE scatter variant (default warp) or VERTEX gather variant (default smem)")
@@ -277,7 +287,8 @@ def main():
     peak, peak_src = measured_peaks()
     dom = args.strategy
     t_dom = fe[f"{dom}_{args.scatter}"]["us"]
-    abytes = algorithmic_bytes(dom, Ef, N)
+    rigid = w.quat is not None
+    abytes = algorithmic_bytes(dom, Ef, N, rigid)
     achieved = abytes / (t_dom * 1e-6) / 1e9
     knames = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp": "k_edge_warp", "red": "k_edge_red", "red_v4": "k_edge_red",
               "segmented": "k_edge_store+k_edge_segsum"}
@@ -299,18 +310,24 @@ def main():
         pos_h = torch.from_numpy(s.in_id_order(s.pos)).pin_memory()
         vel_h = torch.from_numpy(s.in_id_order(s.vel)).pin_memory()
         f_h = torch.zeros_like(pos_h).pin_memory()
+        rb = {}
+        if rigid:                                 # rigid bodies: quaternions and angular momenta in, torques out as well
+            rb = {"quat": torch.from_numpy(s.in_id_order(s.quat)).pin_memory(),
+                  "angmom": torch.from_numpy(s.in_id_order(s.angmom)).pin_memory(),
+                  "torque": torch.zeros_like(pos_h).pin_memory()}
         ne = max(1, args.e2e_steps)
-        s.step_host(pos_h, vel_h, f_h, w.dt, 1, args.strategy, args.scatter)     # warm
+        s.step_host(pos_h, vel_h, f_h, w.dt, 1, args.strategy, args.scatter, **rb)     # warm
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
         for _ in range(ne):
-            s.step_host(pos_h, vel_h, f_h, w.dt, 1, args.strategy, args.scatter)
+            s.step_host(pos_h, vel_h, f_h, w.dt, 1, args.strategy, args.scatter, **rb)
         t_e = (time.perf_counter() - t0) / ne
         Ee = s.stats()["n_edges"]
         pe_all, te_max = aggregate(dist, torch, float(Ee), t_e * 1e3, dev)
-        e2e = {"value": pe_all / (te_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 2 * 16 * N,
-               "d2h_bytes_per_step": 3 * 16 * N, "ms_per_step": te_max,
-               "what": "md_step_host: H2D pos+vel, cell+Verlet build, forces, 1 velocity-Verlet step, D2H pos+vel+force"}
+        e2e = {"value": pe_all / (te_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": (4 if rigid else 2) * 16 * N,
+               "d2h_bytes_per_step": (6 if rigid else 3) * 16 * N, "ms_per_step": te_max,
+               "what": "md_step_host: H2D pos+vel(+quat+angmom), cell+Verlet build, forces, 1 velocity-Verlet step, "
+                       "D2H pos+vel+force(+quat+angmom+torque)"}
 
     if rank != 0:
         s.close()
@@ -319,19 +336,21 @@ def main():
         return
 
     cpu = None
-    if not args.no_cpu_baseline and world == 1:
+    if not args.no_cpu_baseline and world == 1 and args.workload in ("C2a", "C2b"):
         cpu, _ = cpu_baseline(w)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: BASELINE.json configs[1], LJ fluid N=2^20 rho=0.8 rc={w.rcut} skin=0.3, "
-                               f"fcc+jitter melted by {args.melt_steps} untimed steps",
+        "config": {"workload": f"{args.workload}: {WORKLOAD_TEXT[args.workload]}, relaxed by {args.melt_steps} untimed steps",
                    "N": N, "E": int(E_run), "strategy": args.strategy, "variant": args.scatter, "order": args.order,
                    "step": "md_integrate(1): kick, drift, skin check, device-side rebuild when triggered, forces, kick; "
                            "one md_energy per K steps",
-                   "l2": "inputs larger than L2 (list 0.3 GB streamed per evaluation; no flush needed)",
+                   "l2": (f"inputs larger than L2 (neighbour rows {4.0 * Ef / 1e6:.0f} MB streamed per evaluation; no flush needed)"
+                          if 4.0 * Ef > 126e6 else
+                          f"working set ({4.0 * Ef / 1e6:.0f} MB of neighbour rows) fits in the 126 MB L2: steady-state L2-resident "
+                          "timing without a flush -- a secondary workload, the headline is C2a"),
                    "rebuilds_in_timed_region": st1["n_rebuilds"] - stw["n_rebuilds"],
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "force_eval": fe, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
