@@ -134,56 +134,48 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     const int myoc = oc_ex + head - 1;       // ordinal of this thread's cell among the block's own cells
     __syncthreads();
 
-    // 2. candidate cells: the 27-cell stencil of every own cell (S:Q8; duplicates removed below)
+    // 2. candidate cells: the 27-cell stencil of every own cell (S:Q8)
     const int n = 27 * nownc;
-    int n2 = 32;
-    while (n2 < n) n2 <<= 1;
-    if (n2 > ncand_cap) {   // cannot happen for n <= 27*MD_TB <= MD_NCAND unless the launch was sized smaller
+    if (n >= ncand_cap) {   // the hash set below needs a free slot: cannot happen for n <= 27*MD_TB < MD_NCAND unless sized smaller   // cannot happen for n <= 27*MD_TB <= MD_NCAND unless the launch was sized smaller
         if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
         if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
         return;
     }
-    for (int t = tid; t < n2; t += MD_TB) {
-        int v = 0x7fffffff;
-        if (t < n) {
-            const int lin = B.cell_lin[own_rank[t / 27]];
-            const int s = t % 27;
-            const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
-            int ax = cx + s / 9 - 1, ay = cy + (s / 3) % 3 - 1, az = cz + s % 3 - 1;
-            int wrapped = 0;   // bit a: the stencil crosses the periodic face of axis a
-            if (ax < 0) { ax += P.ncx; wrapped |= 1; } else if (ax >= P.ncx) { ax -= P.ncx; wrapped |= 1; }
-            if (ay < 0) { ay += P.ncy; wrapped |= 2; } else if (ay >= P.ncy) { ay -= P.ncy; wrapped |= 2; }
-            if (az < 0) { az += P.ncz; wrapped |= 4; } else if (az >= P.ncz) { az -= P.ncz; wrapped |= 4; }
-            // fewer than 3 cells on an axis: the wrap lands on a cell of the axis again; duplicates vanish in the unique step
-            if (wrapped) atomicOr(&s_flags, wrapped);
-            const int r = B.cell_rank[(ax * P.ncy + ay) * P.ncz + az];
-            v = (B.cell_start[r + 1] > B.cell_start[r]) ? r : 0x7fffffff;   // empty cells contribute nothing
+    // the candidates go through a shared-memory hash set (cand[], open addressing, native 32-bit CAS): neighbouring own
+    // cells share most of their stencils, so only the DISTINCT cells (a few hundred) are compacted and sorted, not the
+    // 27 x own-cells candidates (thousands at 2-3 particles per cell)
+    const int hmask = ncand_cap - 1;                  // ncand_cap is a power of two > n
+    for (int t = tid; t < ncand_cap; t += MD_TB) cand[t] = 0x7fffffff;
+    __syncthreads();
+    for (int t = tid; t < n; t += MD_TB) {
+        const int lin = B.cell_lin[own_rank[t / 27]];
+        const int s = t % 27;
+        const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
+        int ax = cx + s / 9 - 1, ay = cy + (s / 3) % 3 - 1, az = cz + s % 3 - 1;
+        int wrapped = 0;   // bit a: the stencil crosses the periodic face of axis a
+        if (ax < 0) { ax += P.ncx; wrapped |= 1; } else if (ax >= P.ncx) { ax -= P.ncx; wrapped |= 1; }
+        if (ay < 0) { ay += P.ncy; wrapped |= 2; } else if (ay >= P.ncy) { ay -= P.ncy; wrapped |= 2; }
+        if (az < 0) { az += P.ncz; wrapped |= 4; } else if (az >= P.ncz) { az -= P.ncz; wrapped |= 4; }
+        // fewer than 3 cells on an axis: the wrap lands on a cell of the axis again; the set removes the duplicates
+        if (wrapped) atomicOr(&s_flags, wrapped);
+        const int r = B.cell_rank[(ax * P.ncy + ay) * P.ncz + az];
+        if (B.cell_start[r + 1] > B.cell_start[r]) {      // empty cells contribute nothing
+            unsigned int h = ((unsigned int)r * 2654435761u) >> 7;
+            for (;;) {
+                h &= hmask;
+                const int old = atomicCAS(&cand[h], 0x7fffffff, r);
+                if (old == 0x7fffffff || old == r) break;
+                ++h;
+            }
         }
-        cand[t] = v;
     }
     __syncthreads();
 
-    // 3. bitonic sort of the candidate ranks
-    for (int k = 2; k <= n2; k <<= 1) {
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int t = tid; t < n2; t += MD_TB) {
-                const int x = t ^ j;
-                if (x > t) {
-                    const int a = cand[t], c = cand[x];
-                    const bool asc = (t & k) == 0;
-                    if ((a > c) == asc) { cand[t] = c; cand[x] = a; }
-                }
-            }
-            __syncthreads();
-        }
-    }
-
-    // 4. unique -> urank[0..U)
+    // 3. compact the distinct ranks -> urank[0..U)
     int U = 0;
-    for (int base = 0; base < n2; base += MD_TB) {
-        const int t = base + tid;
-        const int v = t < n2 ? cand[t] : 0x7fffffff;
-        const int f = (v != 0x7fffffff && (t == 0 || cand[t - 1] != v)) ? 1 : 0;
+    for (int base = 0; base < ncand_cap; base += MD_TB) {
+        const int v = cand[base + tid];
+        const int f = v != 0x7fffffff ? 1 : 0;
         int tot;
         const int p = blk_excl_scan(f, &tot, sh_scan);
         if (f && U + p < umax) urank[U + p] = v;
@@ -194,7 +186,24 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
         if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
         return;
     }
+    // 4. bitonic sort of the distinct ranks (ascending rank = ascending slot)
+    int U2 = 32;
+    while (U2 < U) U2 <<= 1;                          // U2 <= umax (a power of two)
+    for (int t = U + tid; t < U2; t += MD_TB) urank[t] = 0x7fffffff;
     __syncthreads();
+    for (int k = 2; k <= U2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = tid; t < U2; t += MD_TB) {
+                const int x = t ^ j;
+                if (x > t) {
+                    const int a = urank[t], c = urank[x];
+                    const bool asc = (t & k) == 0;
+                    if ((a > c) == asc) { urank[t] = c; urank[x] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    }
 
     // 5. local base of every distinct cell (exclusive scan of the cell populations), packed cell coordinates
     int M = 0;
