@@ -848,35 +848,55 @@ __device__ __forceinline__ void lj_chunk_s(const DevParams& P, unsigned int sp32
 // cnt, pk[0..3]: |L_i| and the first four row chunks, loaded by the caller while the staging copies were in flight.
 // The row streams from HBM (~1300 cycles under load); chunks are consumed four per iteration through four separate
 // load instructions, each re-issued four chunks (~350 instructions of arithmetic) ahead of its use.
-template <bool IMG, int SH, bool UNIT>
+// NS = threads per particle (1, or 2 when the staged neighbourhood is so large that only one or two 256-particle blocks
+// fit on an SM: the block then runs 512 threads, thread h * 256 + p takes the row chunks c = h mod 2 of particle p and the
+// two partial sums meet in shared memory -- twice the warps for the same shared memory).  xch = exchange buffer (NS == 2).
+template <bool IMG, int SH, bool UNIT, int NS>
 __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int i,
-                                               int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB, uint2 pkC, uint2 pkD,
-                                               const float4* __restrict__ pos, float4* __restrict__ force, bool bonds) {
-    const float4 xi = st.spos[bi.own_base + threadIdx.x];
+                                               bool live, int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB, uint2 pkC,
+                                               uint2 pkD, float* xch, const float4* __restrict__ pos, float4* __restrict__ force,
+                                               bool bonds) {
+    const int tp = threadIdx.x % MD_TB, h = threadIdx.x / MD_TB;
+    const float4 xi = st.spos[bi.own_base + (live ? tp : 0)];
     const unsigned int sp = smem_u32(st.spos);
-    const int nch = (cnt + 3) >> 2;                        // the last chunk is padded with the dummy entry
+    const int nall = (cnt + 3) >> 2;                       // the last chunk is padded with the dummy entry
+    const int nch = (nall - h + NS - 1) / NS;              // chunks h, h + NS, ... of the row
+    const uint2* __restrict__ rowh = rowb + (size_t)h * MD_TB;
+    const size_t cs = (size_t)NS * MD_TB;                  // stride between this thread's chunks
     LJAccS a = { 0.f, 0.f, 0.f, 3.0e38f, make_float2(0.f, 0.f), make_float2(0.f, 0.f) };
     for (int c = 0; c < nch; c += 4) {
         const uint2 curA = pkA;
-        if (c + 4 < nch) pkA = ld_row(rowb + (size_t)(c + 4) * MD_TB);
+        if (c + 4 < nch) pkA = ld_row(rowh + (size_t)(c + 4) * cs);
         lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curA, a);
         if (c + 1 >= nch) break;
         const uint2 curB = pkB;
-        if (c + 5 < nch) pkB = ld_row(rowb + (size_t)(c + 5) * MD_TB);
+        if (c + 5 < nch) pkB = ld_row(rowh + (size_t)(c + 5) * cs);
         lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curB, a);
         if (c + 2 >= nch) break;
         const uint2 curC = pkC;
-        if (c + 6 < nch) pkC = ld_row(rowb + (size_t)(c + 6) * MD_TB);
+        if (c + 6 < nch) pkC = ld_row(rowh + (size_t)(c + 6) * cs);
         lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curC, a);
         if (c + 3 >= nch) break;
         const uint2 curD = pkD;
-        if (c + 7 < nch) pkD = ld_row(rowb + (size_t)(c + 7) * MD_TB);
+        if (c + 7 < nch) pkD = ld_row(rowh + (size_t)(c + 7) * cs);
         lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curD, a);
     }
     float pe2 = a.pe.x + a.pe.y;
+    float nin = a.nin.x + a.nin.y;
+    if (NS == 2) {                                         // second half hands its partial sums to the first
+        if (h == 1) {
+            xch[tp] = a.fx; xch[MD_TB + tp] = a.fy; xch[2 * MD_TB + tp] = a.fz; xch[3 * MD_TB + tp] = pe2;
+            xch[4 * MD_TB + tp] = nin; xch[5 * MD_TB + tp] = a.band;
+        }
+        __syncthreads();
+        if (h == 1) return;
+        a.fx += xch[tp]; a.fy += xch[MD_TB + tp]; a.fz += xch[2 * MD_TB + tp]; pe2 += xch[3 * MD_TB + tp];
+        nin += xch[4 * MD_TB + tp]; a.band = fminf(a.band, xch[5 * MD_TB + tp]);
+    }
+    if (!live) return;
     if (UNIT) {   // back from reduced units: F = 24 eps A, V = 4 eps sum (s^6 - s^3) - V_c nin
         a.fx *= P.c24; a.fy *= P.c24; a.fz *= P.c24;
-        pe2 = fmaf(P.c4, pe2, -P.vshift * (a.nin.x + a.nin.y));
+        pe2 = fmaf(P.c4, pe2, -P.vshift * nin);
     }
     if (a.band < P.band_abs) {
         float4* scratch = force + i;           // own output slot as scratch (rewritten below)
@@ -895,18 +915,22 @@ __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuff
     force[i] = make_float4(a.fx, a.fy, a.fz, pe);
 }
 
-__global__ void __launch_bounds__(MD_TB, 4) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
-                                                            float4* __restrict__ force) {
+template <int NS>
+__global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : 2) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries,
+                                                                                  const float4* __restrict__ pos,
+                                                                                  float4* __restrict__ force) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int b = blockIdx.x;
+    const int tp = threadIdx.x % MD_TB, h = threadIdx.x / MD_TB;
     // everything the block needs from global memory before it can compute is requested at once: the block header, the
-    // head of its segment table, |L_i| and the first four row chunks (rows hold >= 8 chunks; chunks past |L_i| are
-    // loaded but never consumed)
+    // head of its segment table, |L_i| and the first four row chunks of this thread (rows hold >= 8 chunks; chunks past
+    // |L_i| are loaded but never consumed)
     const SegPre pre = seg_preload(B, b);
-    const int i = b * MD_TB + threadIdx.x;
+    const int i = b * MD_TB + tp;
     const bool live = i < P.N;
-    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + threadIdx.x;
-    const uint2 pkA = ld_row(rowb), pkB = ld_row(rowb + MD_TB), pkC = ld_row(rowb + 2 * MD_TB), pkD = ld_row(rowb + 3 * MD_TB);
+    const uint2* __restrict__ rowb = reinterpret_cast<const uint2*>(B.rows) + (size_t)b * (P.rcap >> 2) * MD_TB + tp;
+    const uint2* __restrict__ rowh = rowb + (size_t)h * MD_TB;
+    const uint2 pkA = ld_row(rowh), pkB = ld_row(rowh + NS * MD_TB), pkC = ld_row(rowh + 2 * NS * MD_TB), pkD = ld_row(rowh + 3 * NS * MD_TB);
     const int cnt = live ? B.row_count[i] : 0;
     const BlkInfo bi = B.blk[b];
     if (bi.M <= 0 || bi.M + 1 > stage_entries) {   // build failed for this block / launch sized too small: latch, never guess
@@ -914,12 +938,13 @@ __global__ void __launch_bounds__(MD_TB, 4) k_vertex_lj_staged(DevParams P, DevB
         return;
     }
     const Stage st = stage_issue<false>(P, B, bi, b, stage_entries, pre, pos, nullptr, smraw);
+    float* xch = reinterpret_cast<float*>(st.spos + stage_entries);     // [6][MD_TB] floats, NS == 2 only
     stage_wait(P, bi, st, smraw);
-    if (!live) return;
+    if (NS == 1 && !live) return;
     const bool bonds = P.kind == MD_POT_FENE_WCA;
     const bool img = (bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK);
     const bool unit = P.sig2 == 1.0f;
-#define LJ_ROWS(IMG_, SH_, UNIT_) vertex_lj_rows<IMG_, SH_, UNIT_>(P, B, bi, st, i, cnt, rowb, pkA, pkB, pkC, pkD, pos, force, bonds)
+#define LJ_ROWS(IMG_, SH_, UNIT_) vertex_lj_rows<IMG_, SH_, UNIT_, NS>(P, B, bi, st, i, live, cnt, rowb, pkA, pkB, pkC, pkD, xch, pos, force, bonds)
     if (bi.flags & MD_BLK_SH4) {
         if (unit) { if (img) LJ_ROWS(true, 4, true); else LJ_ROWS(false, 4, true); }
         else { if (img) LJ_ROWS(true, 4, false); else LJ_ROWS(false, 4, false); }
@@ -1008,7 +1033,8 @@ static void staged_attrs_once() {
     static bool done = false;
     if (done) return;
     done = true;
-    cudaFuncSetAttribute(k_vertex_lj_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
     cudaFuncSetAttribute(k_vertex_patchy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
 }
 
@@ -1020,7 +1046,9 @@ bool md_launch_forces_staged(md_system* s) {
     const size_t smem = md_staged_smem_bytes(s, se);
     if (smem > 224 * 1024) return false;
     if (P.kind == MD_POT_PATCHY) k_vertex_patchy_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
-    else k_vertex_lj_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+    else if (smem > 75 * 1024 && smem + 24 * MD_TB <= 224 * 1024)   // <= 2 blocks per SM: two threads per particle
+        k_vertex_lj_staged<2><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
+    else k_vertex_lj_staged<1><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
     s->launches += 1;
     return true;
 }
