@@ -50,5 +50,16 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+def build_microbench() -> Path:
+    """Stand-alone micro-benchmark of the non-HBM ceilings (csrc/microbench.cu -> microbench, not part of the library)."""
+    exe = PKG / "microbench"
+    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-o", str(exe), str(CSRC / "microbench.cu")]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        print(r.stdout, r.stderr)
+        raise RuntimeError("nvcc failed on microbench.cu")
+    return exe
+
+
 if __name__ == "__main__":
     print(build(force=True, verbose=True))
