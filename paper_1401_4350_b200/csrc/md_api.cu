@@ -17,7 +17,7 @@ struct Geometry {
     int64_t ncell;
     int cap, ntiles;
     size_t ecap;
-    int rcap, nblk, stage_cap;   // staged path
+    int rcap, nblk, stage_cap, mask_words;   // staged path
 };
 
 // S:Q8: n_k = max(1, floor(L_k / (r_v (1 + 1e-5)))) cells per axis, width >= r_v
@@ -41,6 +41,11 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
     g->nblk = (int)((N + MD_TB - 1) / MD_TB);
     // largest neighbourhood (entries) a force kernel can stage: 16 B (+16 B quaternion) each in <= 224 KB of shared memory
     g->stage_cap = 0;   // set by the caller (depends on the potential)
+    {   // candidate masks of the staged build: room for twice the mean cell population plus 24
+        const double ppc = (double)N / (double)g->ncell;
+        g->mask_words = (int)((2.0 * ppc + 24.0 + 31.0) / 32.0);
+        if (g->mask_words < 1) g->mask_words = 1;
+    }
     return true;
 }
 
@@ -87,7 +92,8 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.stage4 = (float4*)take(16 * Npad);
     b.cell_lin = (int*)take(4 * (size_t)g.ncell);
     b.rows = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);
-    b.rows_tmp = (unsigned short*)take(2 * 2 * (size_t)g.nblk * MD_TB * (size_t)(g.rcap + 2));   // scan order + sorted by column
+    b.rows_tmp = (unsigned short*)take(2 * 2 * (size_t)g.nblk * MD_TB * (size_t)(g.rcap + 2));
+    b.cmask = (unsigned int*)take(4 * (size_t)g.nblk * 27 * (size_t)g.mask_words * MD_TB);   // scan order + sorted by column
     b.row_count = (int*)take(4 * Npad);
     b.lo_count = (int*)take(4 * Npad);
     b.blk = (BlkInfo*)take(sizeof(BlkInfo) * (size_t)g.nblk);
@@ -279,7 +285,8 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.half_skin2 = (float)(0.25 * skin * skin);
     P.rv2 = (float)P.rv2d;
     P.band_rv = (float)(P.rv2d * 1e-6);    // S:Q6 band of the list predicate
-    P.nblk = g.nblk; P.rcap = g.rcap; P.pad1 = 0;
+    P.nblk = g.nblk; P.rcap = g.rcap; P.mask_words = g.mask_words;
+    P.use_masks = ((double)N / (double)g.ncell >= 8.0) ? 1 : 0;   // measured: masks win at 17.7 particles per cell, lists at 2.5-3
     P.stage_cap = (int)((224 * 1024 - 16) / (rigid ? 32 : 16)) - 1;
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);

@@ -60,7 +60,8 @@ struct DevParams {
     float rc2, band_abs;               // fp32 cutoff and the half-width of the fp64-recheck band |d2 - rc2| (S:H10)
     float half_skin2;                  // (skin/2)^2
     float rv2, band_rv;                // fp32 list radius^2 and its fp64-recheck band (S:Q6)
-    int nblk, stage_cap, rcap, pad1;   // staged path: blocks of MD_TB slots, smem capacity (particles), row capacity (entries)
+    int nblk, stage_cap, rcap, mask_words;   // mask_words: 32-bit candidate-mask words per stencil cell (build scratch)
+    int use_masks;                     // staged build: candidate masks (1) or index lists (0, few particles per cell)
     float skinf;
     float shift_margin;                // r_v + skin: see k_build_staged step 7c
     // pair potential
@@ -112,7 +113,8 @@ struct DevBuffers {
     // staged path
     int* cell_lin;         // [ncell] storage rank -> linear cell index (inverse of cell_rank)
     unsigned short* rows;  // [nblk][rcap/4][MD_TB] x 4 u16: Verlet rows of block-local indices, block-transposed chunks of 4
-    unsigned short* rows_tmp; // [2][nblk][rcap][MD_TB] build scratch: rows in scan order, then sorted by bank column
+    unsigned short* rows_tmp; // [2][nblk][rcap + 2][MD_TB] build scratch: neighbours sorted by bank column; list form: scan order
+    unsigned int* cmask;      // [nblk][27 * mask_words][MD_TB] build scratch: per stencil cell, bitmask of the candidates inside r_v
     int* row_count;        // [Npad] |L_i|
     int* lo_count;         // [Npad] neighbours with slot < i
     BlkInfo* blk;          // [nblk]

@@ -78,6 +78,41 @@ __device__ __forceinline__ int blk_excl_scan(int v, int* tot, int* sh /* >= 33 i
 __device__ __forceinline__ int pack_coord(int cx, int cy, int cz) { return cx | (cy << 10) | (cz << 20); }
 
 // Candidate scan of one stencil cell for interior / shift-transformed blocks: all lanes of a warp walk the same cell, so
+// the loop is branch-free.  The result is a BITMASK per 32 candidates (bit k = candidate k of the cell is inside r_v,
+// from the sign bit of d2 - r_v^2), written with one coalesced 32-bit store per word -- a list of indices would be ~70
+// scattered 16-bit stores per thread.  mrow = word 0 of this cell for this thread (words are MD_TB apart).
+// self = index of the particle itself in this cell, or -1.  Returns the number of neighbours found.
+template <bool SHIFT>
+__device__ __forceinline__ int scan_cell_mask(const float4* __restrict__ cellpos, int n, int self, float4 xi, float rv2,
+                                              float hLx, float hLy, float hLz, float tLx, float tLy, float tLz,
+                                              unsigned int* mrow, float& bandmin) {
+    int found = 0;
+    for (int k0 = 0; k0 < n; k0 += 32) {
+        const int kn = min(32, n - k0);
+        unsigned int mask = 0u, bit = 1u;
+#pragma unroll 8
+        for (int k = 0; k < kn; ++k) {
+            float4 xj = __ldg(cellpos + k0 + k);
+            if (SHIFT) {
+                if (xj.x > hLx) xj.x -= tLx;
+                if (xj.y > hLy) xj.y -= tLy;
+                if (xj.z > hLz) xj.z -= tLz;
+            }
+            const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
+            const float tt = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)) - rv2;
+            bandmin = fminf(bandmin, fabsf(tt));
+            mask |= (unsigned int)(__float_as_int(tt) >> 31) & bit;      // sign bit: inside r_v
+            bit <<= 1;
+        }
+        if ((unsigned int)(self - k0) < 32u) mask &= ~(1u << (self - k0));
+        mrow[(size_t)(k0 >> 5) * MD_TB] = mask;
+        found += __popc(mask);
+    }
+    return found;
+}
+
+// LIST form of the candidate scan, used when cells hold few particles (mask_words == 0: at 2-3 particles per cell 27
+// mostly empty mask words per thread cost more than ~10 index stores).  All lanes of a warp walk the same cell, so
 // the loop is kept branch-free: a predicated store at the thread's write offset, which advances (by one scratch row)
 // when the candidate is inside r_v (sign bit of d2 - r_v^2), clamped at the overflow row cap + 1.
 template <bool SHIFT, bool SELF>
@@ -100,6 +135,32 @@ __device__ __forceinline__ void scan_cell_fast(const float4* __restrict__ cellpo
         if (m) *reinterpret_cast<unsigned short*>(reinterpret_cast<char*>(tmp_blk) + off) = (unsigned short)(t0 + k);
         off = min(off + ((unsigned int)m & (2u * MD_TB)), offmax);
     }
+}
+
+// The same scan with every decision taken carefully: minimum image (blocks whose neighbourhood crosses a periodic face
+// without a valid shift transform) and the fp64 predicate inside the band (S:Q6).  Rare path.
+__device__ __noinline__ int scan_cell_slow(const float4* __restrict__ cellpos, int n, int self, float4 xi,
+                                           float Lx, float Ly, float Lz, float rv2, float bandv, double dLx, double dLy,
+                                           double dLz, double rv2d, unsigned int* mrow) {
+    int found = 0;
+    for (int k0 = 0; k0 < n; k0 += 32) {
+        const int kn = min(32, n - k0);
+        unsigned int mask = 0u;
+        for (int k = 0; k < kn; ++k) {
+            if (k0 + k == self) continue;
+            const float4 xj = __ldg(cellpos + k0 + k);
+            // raw (untransformed) coordinates of both particles: the robust minimum image is right for every pair
+            const float ddx = min_image(xj.x, xi.x, Lx, 0.5f * Lx), ddy = min_image(xj.y, xi.y, Ly, 0.5f * Ly),
+                        ddz = min_image(xj.z, xi.z, Lz, 0.5f * Lz);
+            const float tt = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)) - rv2;
+            bool in = tt < 0.0f;
+            if (fabsf(tt) < bandv) in = inside_fp64(xi, xj, dLx, dLy, dLz, rv2d);
+            if (in) mask |= 1u << k;
+        }
+        mrow[(size_t)(k0 >> 5) * MD_TB] = mask;
+        found += __popc(mask);
+    }
+    return found;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -340,35 +401,29 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
         return x;
     };
 
-    // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6).  Pass A writes the
-    //    neighbours in scan order (ascending local index = ascending slot) to a thread-private scratch row and counts
-    //    them per shared-memory bank column (local index mod 8: one float4 = one of the 8 16-byte columns of a wavefront).
+    // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6).  Pass A leaves, per
+    //    stencil cell, a bitmask of the candidates inside r_v (scan_cell_mask); pass B turns the masks into the row.
     unsigned short* s_rem = reinterpret_cast<unsigned short*>(own_rank + MD_TB);   // [8][MD_TB] entries left per column
-    unsigned short* s_cur = s_rem + 8 * MD_TB;                                        // [8][MD_TB] scan cursor per column
+    unsigned short* s_cur = s_rem + 8 * MD_TB;                                        // [8][MD_TB] cursor per column
     int cnt = 0, lo_cnt = 0;
-    float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
-    // scan-order scratch row, block-transposed (entry k of thread tid at k * MD_TB + tid): lanes of a warp sit at
-    // similar k, so both passes touch a few sectors per warp access instead of one per lane
-    const size_t tstride = (size_t)(P.rcap + 2) * MD_TB;        // scratch rows per block (cap + 2: overflow row)
-    unsigned short* tmp_blk = B.rows_tmp + (size_t)b * tstride;
+    const int W = P.mask_words;                                   // 32-bit mask words per stencil cell
+    const bool use_masks = P.use_masks != 0;                      // else: list form (few particles per cell)
+    unsigned int* cm = B.cmask + (size_t)b * 27 * W * MD_TB + tid;   // word (cell sc, w) at cm[(sc * W + w) * MD_TB]
+    unsigned short* tmp_blk = B.rows_tmp + ((size_t)P.nblk + b) * (P.rcap + 2) * MD_TB;   // list form: neighbours in scan order
     unsigned short* tmp = tmp_blk + tid;
+    const int* __restrict__ mycells = cand + max(myoc, 0) * 27;
+    const int me = own_base + tid;
 #pragma unroll
     for (int c = 0; c < 8; ++c) { s_rem[c * MD_TB + tid] = 0; s_cur[c * MD_TB + tid] = 0; }
     if (live) {
-        const int me = own_base + tid;
-        xi = load_pos(i);
+        const float4 xi_raw = __ldg(pos + i);
+        const float4 xi = load_pos(i);
         const float hLx = P.hLx, hLy = P.hLy, hLz = P.hLz;
-        const int* __restrict__ mycells = cand + myoc * 27;
-        if (!maywrap) {
-            // interior blocks (the common case): no minimum image, no wrap bookkeeping; the listed-pair branch is
-            // reduced to a predicated store so that the 32 lanes of a warp stay converged over the candidate loop
-            //  The fp64 band decision (S:Q6) is kept out of the loop: the loop tracks min |d2 - r_v^2| and the rare thread
-            //  with a banded candidate (~1e-4) repeats its scan with the fp64 predicate.  lo_cnt is counted in pass B.
-            const float rv2 = P.rv2, bandv = P.band_rv;
-            const int cap = P.cap;
-            float bandmin = 3.0e38f;
+        float bandmin = maywrap ? 0.0f : 3.0e38f;                 // maywrap blocks go straight to the careful scan
+        if (!maywrap && !use_masks) {
+            const float rv2 = P.rv2;
             unsigned int off = 2u * tid;
-            const unsigned int offmax = (unsigned int)(cap + 1) * (2u * MD_TB) + 2u * tid;
+            const unsigned int offmax = (unsigned int)(P.cap + 1) * (2u * MD_TB) + 2u * tid;
             for (int sc = 0; sc < 27; ++sc) {
                 const int u = mycells[sc];
                 if (u < 0) continue;
@@ -383,97 +438,99 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
                 }
             }
             cnt = (int)((off - 2u * tid) / (2u * MD_TB));   // cap + 1 = overflow
-            if (bandmin < bandv) {      // rare: repeat with the fp64 decision for banded candidates
-                cnt = 0;
+        } else if (!maywrap) {
+            const float rv2 = P.rv2;
+            for (int sc = 0; sc < 27; ++sc) {
+                const int u = mycells[sc];
+                if (u < 0) continue;
+                const int t0 = ubase[u];
+                int n = ubase[u + 1] - t0;
+                if (n > 32 * W) { n = 32 * W; atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); }   // cell fuller than the mask capacity
+                const int self = sc == 13 ? me - t0 : -1;        // stencil entry 13 is the own cell
+                const float4* cellpos = pos + ustart[u];
+                if (shift_ok) cnt += scan_cell_mask<true>(cellpos, n, self, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, cm + (size_t)sc * W * MD_TB, bandmin);
+                else cnt += scan_cell_mask<false>(cellpos, n, self, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, cm + (size_t)sc * W * MD_TB, bandmin);
+            }
+        }
+        if (bandmin < P.band_rv) {      // rare: a banded candidate (or a block that needs the minimum image)
+            cnt = 0;
+            for (int sc = 0; sc < 27; ++sc) {
+                const int u = mycells[sc];
+                if (u < 0) continue;
+                const int t0 = ubase[u];
+                int n = ubase[u + 1] - t0;
+                if (n > 32 * W) { n = 32 * W; atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); }
+                const int self = (me >= t0 && me < t0 + n) ? me - t0 : -1;   // (small boxes: the own cell may sit elsewhere in the stencil)
+                cnt += scan_cell_slow(pos + ustart[u], n, self, xi_raw, P.Lx, P.Ly, P.Lz, P.rv2, P.band_rv, P.dLx, P.dLy, P.dLz,
+                                      P.rv2d, cm + (size_t)sc * W * MD_TB);
+            }
+            if (!use_masks) {           // list form: expand the careful masks into the scan-order list
+                int k = 0;
                 for (int sc = 0; sc < 27; ++sc) {
                     const int u = mycells[sc];
                     if (u < 0) continue;
-                    const int t1 = ubase[u + 1];
-                    const int sdelta = ustart[u] - ubase[u];
-                    for (int t = ubase[u]; t < t1; ++t) {
-                        if (t == me) continue;
-                        const float4 xj = load_pos(t + sdelta);
-                        const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
-                        const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
-                        const float tt = d2 - rv2;
-                        bool in = tt < 0.0f;
-                        if (fabsf(tt) < bandv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
-                        if (in) { if (cnt < cap) tmp[(size_t)cnt * MD_TB] = (unsigned short)t; ++cnt; }
+                    const int t0 = ubase[u];
+                    const int nw = min(W, (ubase[u + 1] - t0 + 31) >> 5);
+                    for (int w = 0; w < nw; ++w) {
+                        unsigned int m = cm[(size_t)(sc * W + w) * MD_TB];
+                        while (m) {
+                            const int bit = __ffs(m) - 1;
+                            m &= m - 1;
+                            if (k < P.cap) tmp[(size_t)k * MD_TB] = (unsigned short)(t0 + 32 * w + bit);
+                            ++k;
+                        }
                     }
-                }
-            }
-            lo_cnt = -1;                // counted from the scratch row in pass B
-        } else
-        for (int sc = 0; sc < 27; ++sc) {
-            const int u = mycells[sc];
-            if (u < 0) continue;
-            const int t1 = ubase[u + 1];
-            const int sdelta = ustart[u] - ubase[u];
-            for (int t = ubase[u]; t < t1; ++t) {
-                if (t == me) continue;
-                const float4 xj = __ldg(pos + t + sdelta);
-                float ddx, ddy, ddz;
-                if (maywrap) {
-                    ddx = min_image(xj.x, xi.x, P.Lx, hLx); ddy = min_image(xj.y, xi.y, P.Ly, hLy); ddz = min_image(xj.z, xi.z, P.Lz, hLz);
-                } else {
-                    ddx = xj.x - xi.x; ddy = xj.y - xi.y; ddz = xj.z - xi.z;
-                }
-                const float d2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
-                const float tt = d2 - P.rv2;
-                bool in = tt < 0.0f;
-                if (fabsf(tt) < P.band_rv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
-                if (in) {
-                    if (cnt < P.cap) tmp[(size_t)cnt * MD_TB] = (unsigned short)t;
-                    ++cnt;
-                    lo_cnt += (t < me);
                 }
             }
         }
         if (cnt > P.cap) atomicOr(&B.ctrl->err, MD_DEVERR_CAPACITY);
     }
+    // every set bit of the thread's masks = one neighbour (local index t), visited cell by cell in ascending t
+    auto for_each_neighbour = [&](auto&& f) {
+        if (!use_masks) {
+            const int c2l = min(cnt, P.cap);
+            for (int k = 0; k < c2l; ++k) f((int)tmp[(size_t)k * MD_TB]);
+            return;
+        }
+        for (int sc = 0; sc < 27; ++sc) {
+            const int u = mycells[sc];
+            if (u < 0) continue;
+            const int t0 = ubase[u];
+            const int nw = min(W, (ubase[u + 1] - t0 + 31) >> 5);
+            for (int w = 0; w < nw; ++w) {
+                unsigned int m = cm[(size_t)(sc * W + w) * MD_TB];
+                const int tb = t0 + 32 * w;
+                while (m) { const int bit = __ffs(m) - 1; m &= m - 1; f(tb + bit); }
+            }
+        }
+    };
     // 8b. Pass B: emit the row in the order the force kernels read it.  Thread tid (lane p of its quarter-warp) reads
     //     entry k at the same time as the 7 other lanes of the quarter read theirs; a 128-bit shared-memory gather is
     //     conflict-free when the 8 lanes hit 8 different columns, so lane p takes, at step k, a neighbour of column
     //     (k + p) mod 8 while it has one (else of its fullest column).  Row layout: block-transposed chunks of four
     //     16-bit local indices, rows[((b * nchunk) + k/4) * MD_TB + tid] -> one coalesced 64-bit load per 4 visits.
     {
-        const int c2 = min(cnt, P.cap);
+        const int c2 = (live && cnt <= P.cap) ? cnt : 0;
         const int nchunk = P.rcap >> 2;
         uint2* __restrict__ rowb = reinterpret_cast<uint2*>(B.rows) + (size_t)b * nchunk * MD_TB + tid;
         unsigned int w[4] = { 0u, 0u, 0u, 0u };
         const int rsh = (M + 1 <= 4096) ? 4 : 0;   // MD_BLK_SH4: entries are byte offsets into the staged float4 array
         const unsigned int dummy = (unsigned int)M << rsh;
-        // counting sort of the scratch row by column into a second scratch row: s_cur[c] ends as the END of column c
-        unsigned short* __restrict__ tmp2 = tmp + (size_t)P.nblk * tstride;
-        {
-            const int me_l = own_base + tid;
+        // counting sort of the neighbours by column into a scratch row: s_cur[c] ends as the END of column c
+        unsigned short* __restrict__ tmp2 = B.rows_tmp + (size_t)b * (P.rcap + 2) * MD_TB + tid;
+        if (c2 > 0) {
             int lo_b = 0;
-            for (int k = 0; k < c2; k += 8) {            // entries per column (loads first: eight in flight)
-                unsigned short e[8];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) e[q] = k + q < c2 ? tmp[(size_t)(k + q) * MD_TB] : (unsigned short)0xffff;
-#pragma unroll
-                for (int q = 0; q < 8; ++q)
-                    if (k + q < c2) { s_rem[(e[q] & 7) * MD_TB + tid] += 1; lo_b += e[q] < me_l; }
-            }
-            if (lo_cnt < 0) lo_cnt = lo_b;
+            for_each_neighbour([&](int t) { s_rem[(t & 7) * MD_TB + tid] += 1; lo_b += t < me; });
+            lo_cnt = lo_b;
             int acc = 0;
 #pragma unroll
             for (int c = 0; c < 8; ++c) { s_cur[c * MD_TB + tid] = (unsigned short)acc; acc += s_rem[c * MD_TB + tid]; }
-            for (int k = 0; k < c2; k += 8) {
-                unsigned short e[8];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) e[q] = k + q < c2 ? tmp[(size_t)(k + q) * MD_TB] : (unsigned short)0xffff;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    if (k + q < c2) {
-                        const int c = e[q] & 7;
-                        const int p = s_cur[c * MD_TB + tid];
-                        s_cur[c * MD_TB + tid] = (unsigned short)(p + 1);
-                        tmp2[(size_t)p * MD_TB] = e[q];
-                    }
-                }
-            }
+            for_each_neighbour([&](int t) {
+                const int c = t & 7;
+                const int p = s_cur[c * MD_TB + tid];
+                s_cur[c * MD_TB + tid] = (unsigned short)(p + 1);
+                tmp2[(size_t)p * MD_TB] = (unsigned short)t;
+            });
         }
         for (int k0 = 0; k0 < c2; k0 += 4) {
             int src[4];                                   // scratch positions of the four entries (-1 = padding)
