@@ -92,7 +92,7 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.stage4 = (float4*)take(16 * Npad);
     b.cell_lin = (int*)take(4 * (size_t)g.ncell);
     b.rows = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);
-    b.rows_tmp = (unsigned short*)take(2 * 2 * (size_t)g.nblk * MD_TB * (size_t)(g.rcap + 2));
+    b.rows_tmp = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)(8 * ((g.rcap + 2) / 2) + g.rcap + 2));   // 8 column buckets + list form
     b.cmask = (unsigned int*)take(4 * (size_t)g.nblk * 27 * (size_t)g.mask_words * MD_TB);   // scan order + sorted by column
     b.row_count = (int*)take(4 * Npad);
     b.lo_count = (int*)take(4 * Npad);

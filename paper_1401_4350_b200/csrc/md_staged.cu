@@ -409,7 +409,8 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     const int W = P.mask_words;                                   // 32-bit mask words per stencil cell
     const bool use_masks = P.use_masks != 0;                      // else: list form (few particles per cell)
     unsigned int* cm = B.cmask + (size_t)b * 27 * W * MD_TB + tid;   // word (cell sc, w) at cm[(sc * W + w) * MD_TB]
-    unsigned short* tmp_blk = B.rows_tmp + ((size_t)P.nblk + b) * (P.rcap + 2) * MD_TB;   // list form: neighbours in scan order
+    const int cap8 = (P.rcap + 2) >> 1;                             // capacity of one column bucket of pass B
+    unsigned short* tmp_blk = B.rows_tmp + ((size_t)P.nblk * 8 * cap8 + (size_t)b * (P.rcap + 2)) * MD_TB;   // list form: neighbours in scan order
     unsigned short* tmp = tmp_blk + tid;
     const int* __restrict__ mycells = cand + max(myoc, 0) * 27;
     const int me = own_base + tid;
@@ -516,21 +517,27 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
         unsigned int w[4] = { 0u, 0u, 0u, 0u };
         const int rsh = (M + 1 <= 4096) ? 4 : 0;   // MD_BLK_SH4: entries are byte offsets into the staged float4 array
         const unsigned int dummy = (unsigned int)M << rsh;
-        // counting sort of the neighbours by column into a scratch row: s_cur[c] ends as the END of column c
-        unsigned short* __restrict__ tmp2 = B.rows_tmp + (size_t)b * (P.rcap + 2) * MD_TB + tid;
+        // one decoding sweep drops every neighbour into the bucket of its column (8 buckets of cap8 entries: a column with
+        // more than half a row's capacity is reported as a capacity error); s_cur[c] ends as the population of column c
+        unsigned short* __restrict__ tmp2 = B.rows_tmp + (size_t)b * 8 * cap8 * MD_TB + tid;
         if (c2 > 0) {
             int lo_b = 0;
-            for_each_neighbour([&](int t) { s_rem[(t & 7) * MD_TB + tid] += 1; lo_b += t < me; });
-            lo_cnt = lo_b;
-            int acc = 0;
-#pragma unroll
-            for (int c = 0; c < 8; ++c) { s_cur[c * MD_TB + tid] = (unsigned short)acc; acc += s_rem[c * MD_TB + tid]; }
+            bool over = false;
             for_each_neighbour([&](int t) {
                 const int c = t & 7;
                 const int p = s_cur[c * MD_TB + tid];
                 s_cur[c * MD_TB + tid] = (unsigned short)(p + 1);
-                tmp2[(size_t)p * MD_TB] = (unsigned short)t;
+                if (p < cap8) tmp2[(size_t)(c * cap8 + p) * MD_TB] = (unsigned short)t; else over = true;
+                lo_b += t < me;
             });
+            lo_cnt = lo_b;
+            if (over) atomicOr(&B.ctrl->err, MD_DEVERR_CAPACITY);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const int pop = min((int)s_cur[c * MD_TB + tid], cap8);
+                s_cur[c * MD_TB + tid] = (unsigned short)(c * cap8 + pop);      // END of column c in the scratch
+                s_rem[c * MD_TB + tid] = (unsigned short)pop;
+            }
         }
         for (int k0 = 0; k0 < c2; k0 += 4) {
             int src[4];                                   // scratch positions of the four entries (-1 = padding)
