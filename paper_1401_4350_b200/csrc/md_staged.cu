@@ -166,6 +166,7 @@ __device__ __noinline__ int scan_cell_slow(const float4* __restrict__ cellpos, i
 // ------------------------------------------------------------------------------------------------
 // S:A4 staged Verlet build.  One block per MD_TB slots, one thread per particle.
 // ------------------------------------------------------------------------------------------------
+template <bool MASKS>
 __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
                                                         int ncand_cap, int umax) {
     GATE(B, gated);
@@ -407,7 +408,7 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     unsigned short* s_cur = s_rem + 8 * MD_TB;                                        // [8][MD_TB] cursor per column
     int cnt = 0, lo_cnt = 0;
     const int W = P.mask_words;                                   // 32-bit mask words per stencil cell
-    const bool use_masks = P.use_masks != 0;                      // else: list form (few particles per cell)
+    constexpr bool use_masks = MASKS;                             // else: list form (few particles per cell)
     unsigned int* cm = B.cmask + (size_t)b * 27 * W * MD_TB + tid;   // word (cell sc, w) at cm[(sc * W + w) * MD_TB]
     const int cap8 = (P.rcap + 2) >> 1;                             // capacity of one column bucket of pass B
     unsigned short* tmp_blk = B.rows_tmp + ((size_t)P.nblk * 8 * cap8 + (size_t)b * (P.rcap + 2)) * MD_TB;   // list form: neighbours in scan order
@@ -620,13 +621,16 @@ void md_launch_build_staged(md_system* s, bool gated) {
     staged_build_sizes(s, &nc, &um, &smem);
     static bool attr_done = false;
     if (!attr_done) {
-        cudaFuncSetAttribute(k_build_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+        cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+        cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
         // candidates are read through L1: leave it as large as the four resident blocks allow
-        cudaFuncSetAttribute(k_build_staged, cudaFuncAttributePreferredSharedMemoryCarveout, 50);   // measured: 25 -> 1.96 ms, 50 -> 1.65, 75 -> 1.82, 100 -> 2.02
+        cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 50);
+        cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 50);   // measured: 25 -> 1.96 ms, 50 -> 1.65, 75 -> 1.82, 100 -> 2.02
         attr_done = true;
     }
     k_staged_begin<<<1, 1, 0, s->stream>>>(s->B, g);
-    k_build_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um);
+    if (P.use_masks) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um);
+    else k_build_staged<false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um);
     s->launches += 2;
 }
 
