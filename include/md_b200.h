@@ -104,8 +104,8 @@ md_status md_workspace_bytes(int64_t N, const double box[3], double rcut, double
  * rcut + skin, Verlet lists of radius r_v).  box, pot: host.  workspace: DEVICE pointer, 256-byte
  * aligned, workspace_bytes >= md_workspace_bytes(...), owned by the caller and borrowed until
  * md_destroy.  cuda_stream: a cudaStream_t (may be NULL for the legacy default stream).
- * max_neigh: capacity of every L_i (rounded up to a multiple of 4).
- * MD_ERR_INVALID if N <= 0, N*max_neigh >= 2^31, box[k] < 2 (rcut + 2 skin), bad potential. */
+ * max_neigh: capacity of every L_i (rounded up to a multiple of 4), at most 480.
+ * MD_ERR_INVALID if N <= 0, max_neigh > 480, N*max_neigh >= 2^31, box[k] < 2 (rcut + 2 skin), bad potential. */
 md_status md_create(md_system** out, int64_t N, const double box[3], double rcut, double skin,
                     const md_potential* pot, int32_t max_neigh, void* workspace, size_t workspace_bytes,
                     void* cuda_stream);

@@ -32,6 +32,7 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
         g->ncell *= g->nc[k];
     }
     if (g->ncell > (1ll << 30)) return false;
+    if (max_neigh > 480) return false;            // the staged build keeps column populations in 8-bit fields (md_staged.cu pass B)
     g->cap = (max_neigh + 3) / 4 * 4;
     g->ntiles = (int)((N + MD_TILE - 1) / MD_TILE);
     if ((int64_t)g->ntiles * MD_TILE * g->cap >= (1ll << 31)) return false;

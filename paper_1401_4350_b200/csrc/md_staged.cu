@@ -404,8 +404,6 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
 
     // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6).  Pass A leaves, per
     //    stencil cell, a bitmask of the candidates inside r_v (scan_cell_mask); pass B turns the masks into the row.
-    unsigned short* s_rem = reinterpret_cast<unsigned short*>(own_rank + MD_TB);   // [8][MD_TB] entries left per column
-    unsigned short* s_cur = s_rem + 8 * MD_TB;                                        // [8][MD_TB] cursor per column
     int cnt = 0, lo_cnt = 0;
     const int W = P.mask_words;                                   // 32-bit mask words per stencil cell
     constexpr bool use_masks = MASKS;                             // else: list form (few particles per cell)
@@ -415,8 +413,6 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     unsigned short* tmp = tmp_blk + tid;
     const int* __restrict__ mycells = cand + max(myoc, 0) * 27;
     const int me = own_base + tid;
-#pragma unroll
-    for (int c = 0; c < 8; ++c) { s_rem[c * MD_TB + tid] = 0; s_cur[c * MD_TB + tid] = 0; }
     if (live) {
         const float4 xi_raw = __ldg(pos + i);
         const float4 xi = load_pos(i);
@@ -519,42 +515,39 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
         const int rsh = (M + 1 <= 4096) ? 4 : 0;   // MD_BLK_SH4: entries are byte offsets into the staged float4 array
         const unsigned int dummy = (unsigned int)M << rsh;
         // one decoding sweep drops every neighbour into the bucket of its column (8 buckets of cap8 entries: a column with
-        // more than half a row's capacity is reported as a capacity error); s_cur[c] ends as the population of column c
+        // more than half a row's capacity is reported as a capacity error)
         unsigned short* __restrict__ tmp2 = B.rows_tmp + (size_t)b * 8 * cap8 * MD_TB + tid;
+        // the eight column populations live in one 64-bit register, 8 bits each (a column holds <= cap8 <= 255 entries)
+        unsigned long long pops = 0ull, rem8 = 0ull;
+        int c2e = c2;                                      // entries to emit (0 after a bucket overflow)
         if (c2 > 0) {
             int lo_b = 0;
             bool over = false;
             for_each_neighbour([&](int t) {
-                const int c = t & 7;
-                const int p = s_cur[c * MD_TB + tid];
-                s_cur[c * MD_TB + tid] = (unsigned short)(p + 1);
-                if (p < cap8) tmp2[(size_t)(c * cap8 + p) * MD_TB] = (unsigned short)t; else over = true;
+                const int c = t & 7, sh8 = c * 8;
+                const int p = (int)((pops >> sh8) & 255ull);
+                if (p < cap8) { tmp2[(size_t)(c * cap8 + p) * MD_TB] = (unsigned short)t; pops += 1ull << sh8; } else over = true;
                 lo_b += t < me;
             });
             lo_cnt = lo_b;
-            if (over) atomicOr(&B.ctrl->err, MD_DEVERR_CAPACITY);
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const int pop = min((int)s_cur[c * MD_TB + tid], cap8);
-                s_cur[c * MD_TB + tid] = (unsigned short)(c * cap8 + pop);      // END of column c in the scratch
-                s_rem[c * MD_TB + tid] = (unsigned short)pop;
-            }
+            if (over) { atomicOr(&B.ctrl->err, MD_DEVERR_CAPACITY); c2e = 0; }
+            rem8 = pops;
         }
-        for (int k0 = 0; k0 < c2; k0 += 4) {
+        for (int k0 = 0; k0 < c2e; k0 += 4) {
             int src[4];                                   // scratch positions of the four entries (-1 = padding)
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int k = k0 + q;
                 src[q] = -1;
-                if (k < c2) {
+                if (k < c2e) {
                     int c = (k + tid) & 7;
-                    if (s_rem[c * MD_TB + tid] == 0) {
-                        int bv = 0;
-                        for (int cc = 0; cc < 8; ++cc) { const int v = s_rem[cc * MD_TB + tid]; if (v > bv) { bv = v; c = cc; } }
+                    int r = (int)((rem8 >> (8 * c)) & 255ull);
+                    if (r == 0) {                          // preferred column exhausted: take the fullest one
+#pragma unroll
+                        for (int cc = 0; cc < 8; ++cc) { const int v = (int)((rem8 >> (8 * cc)) & 255ull); if (v > r) { r = v; c = cc; } }
                     }
-                    const int rem = s_rem[c * MD_TB + tid];
-                    src[q] = s_cur[c * MD_TB + tid] - rem;    // next unused entry of column c
-                    s_rem[c * MD_TB + tid] = (unsigned short)(rem - 1);
+                    src[q] = c * cap8 + (int)((pops >> (8 * c)) & 255ull) - r;    // next unused entry of column c
+                    rem8 -= 1ull << (8 * c);
                 }
             }
 #pragma unroll
@@ -610,7 +603,7 @@ static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, si
     int um = nc < MD_UMAX ? nc : MD_UMAX;
     *ncand_cap = nc;
     *umax = um;
-    *smem = 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 2 * 2 * 8 * MD_TB + 16;
+    *smem = 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 16;
 }
 
 void md_launch_build_staged(md_system* s, bool gated) {
