@@ -61,6 +61,8 @@ def test_workspace_bytes_and_validation(lib):
     assert _ws(lib, 2048, [5.0] * 3, 2.5, 0.3, pot, 116)[0] == -1           # box < 2 (rcut + 2 skin)
     assert _ws(lib, 2048, [13.68] * 3, -1.0, 0.3, pot, 116)[0] == -1
     assert _ws(lib, 2 ** 22, [200.0] * 3, 2.5, 0.3, pot, 1024)[0] == -1     # N * max_neigh >= 2^31
+    assert _ws(lib, 2048, [13.68] * 3, 2.5, 0.3, pot, 480)[0] == 0
+    assert _ws(lib, 2048, [13.68] * 3, 2.5, 0.3, pot, 481)[0] == -1          # max_neigh > 480 (md_b200.h)
     bad = dict(W.patchy_potential())
     bad["patch_dir"] = bad["patch_dir"] * 1.1                               # non-unit patch vectors
     assert _ws(lib, 2048, [20.0] * 3, 1.5, 0.3, bad, 40)[0] == -1

@@ -267,3 +267,13 @@ def test_step_host_end_to_end(MD, oracle):
     o10 = oracle.integrate(w.pos, w.vel, w.box, dict(w.potential), w.skin, w.dt, 10)
     assert np.abs(force.numpy()[:, :3] - o10["F"]).max() <= FTOL_REL * np.abs(o10["F"]).max() + FTOL_ABS
     s.close()
+
+
+def test_crossover_sweep_runs(capsys, monkeypatch):
+    """The configs[4] sweep script: one small cell of the grid, every variant, a table on stdout."""
+    import sys
+    from paper_1401_4350_b200 import crossover
+    monkeypatch.setattr(sys, "argv", ["crossover", "--min-log2n", "12", "--max-log2n", "12", "--evals", "2", "--rcuts", "2.5"])
+    crossover.main()
+    out = capsys.readouterr().out
+    assert "| lj | 2^12 | 2.5 |" in out and "| patchy | 2^12 | 1.5 |" in out
