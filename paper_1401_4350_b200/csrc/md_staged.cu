@@ -179,13 +179,13 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     int* ustart = ubase + umax + 1;                                  // [umax] first slot of the cell
     int* own_rank = ustart + umax;                                   // [MD_TB]
     __shared__ int sh_scan[33];
-    __shared__ int s_flags, s_err, s_own_base;
+    __shared__ int s_flags, s_err, s_own_base, s_U;
 
     const int b = blockIdx.x, tid = threadIdx.x;
     const int i0 = b * MD_TB, i1 = min(P.N, i0 + MD_TB);
     const int i = i0 + tid;
     const bool live = i < i1;
-    if (tid == 0) { s_flags = 0; s_err = 0; s_own_base = 0; }
+    if (tid == 0) { s_flags = 0; s_err = 0; s_own_base = 0; s_U = 0; }
 
     // 1. the block's non-empty cells (storage ranks, ascending), compacted
     const int myrank = live ? B.cell_of[i] : -1;
@@ -226,23 +226,20 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
             for (;;) {
                 h &= hmask;
                 const int old = atomicCAS(&cand[h], 0x7fffffff, r);
-                if (old == 0x7fffffff || old == r) break;
+                if (old == 0x7fffffff) {                  // first sighting of this cell: append it to the distinct list
+                    const int idx = atomicAdd(&s_U, 1);
+                    if (idx < umax) urank[idx] = r;
+                    break;
+                }
+                if (old == r) break;
                 ++h;
             }
         }
     }
     __syncthreads();
 
-    // 3. compact the distinct ranks -> urank[0..U)
-    int U = 0;
-    for (int base = 0; base < ncand_cap; base += MD_TB) {
-        const int v = cand[base + tid];
-        const int f = v != 0x7fffffff ? 1 : 0;
-        int tot;
-        const int p = blk_excl_scan(f, &tot, sh_scan);
-        if (f && U + p < umax) urank[U + p] = v;
-        U += tot;
-    }
+    // 3. the distinct ranks were appended to urank[0..U) as they entered the set (arbitrary order, sorted next)
+    const int U = s_U;
     if (U > umax) {
         if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
         if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
