@@ -288,6 +288,11 @@ def main():
     for sc in EDGE_VARIANTS:
         t = time_calls(torch, lambda: s.forces("edge", sc), 10 if sc != "red" else 5)
         fe[f"edge_{sc}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
+    # S:8(f1): VERTEX with Newton's third law, m private force copies per particle (reported beside, not ranked)
+    n3 = {}
+    for m in (1, 4, 12):
+        t = time_calls(torch, lambda: s.forces("vertex_n3", m), 10)
+        n3[f"m{m}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
     best_vertex = min((k for k in fe if k.startswith("vertex")), key=lambda k: fe[k]["us"])
     t_v = fe[best_vertex]["us"]
     clocks = sampler.stop()
@@ -361,7 +366,7 @@ def main():
                           "timing without a flush -- a secondary workload, the headline is C2a"),
                    "rebuilds_in_timed_region": st1["n_rebuilds"] - stw["n_rebuilds"],
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "force_eval": fe, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
+        "force_eval": fe, "vertex_n3_eval": n3, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
         "best_vertex": best_vertex,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "energy_total": sum(e_tot),

@@ -32,8 +32,8 @@
  *                text is available from md_last_error().  Device-detected conditions (neighbour
  *                capacity overflow, FENE bond >= R0) are latched in a device flag and reported by
  *                the next synchronising call.  No partial results are defined after a failure.
- *   Determinism  VERTEX and MD_SCATTER_SEGMENTED are run-to-run bitwise reproducible; the
- *                atomic scatter variants are not.
+ *   Determinism  MD_VERTEX and MD_SCATTER_SEGMENTED are run-to-run bitwise reproducible; the
+ *                atomic scatter variants and MD_VERTEX_N3 are not.
  */
 #ifndef MD_B200_H
 #define MD_B200_H
@@ -57,8 +57,16 @@ typedef enum {
 } md_status;
 
 typedef enum { MD_POT_LJ = 0, MD_POT_FENE_WCA = 1, MD_POT_PATCHY = 2 } md_pot_kind;
-typedef enum { MD_VERTEX = 0, MD_EDGE = 1 } md_strategy;
-/* EDGE scatter alternatives (B:5, S:A7); ignored for MD_VERTEX. */
+typedef enum {
+    MD_VERTEX = 0,   /* one thread per particle, every pair evaluated twice, no atomics                        */
+    MD_EDGE = 1,     /* one thread per pair of the Verlet list, scatter to both particles                      */
+    MD_VERTEX_N3 = 2 /* one thread per particle over its HALF list (j-side of every pair), Newton's third law:
+                        own sum in registers, -f added atomically into one of m private force copies per particle,
+                        copies combined afterwards.  Third argument of md_forces / md_integrate = m (1..64, 0 = 12;
+                        P:71 "insensitive ... as long as m > 10"); MD_ERR_INVALID if m * N exceeds the edge capacity
+                        N * max_neigh / 2 (the copies live in the workspace's per-edge scratch).                    */
+} md_strategy;
+/* EDGE scatter alternatives (B:5, S:A7); third argument of md_forces / md_integrate / md_step_host when strategy == MD_EDGE. */
 typedef enum {
     MD_SCATTER_RED = 0,      /* red.global.add.f32, one per component                           */
     MD_SCATTER_RED_V4 = 1,   /* red.global.add.v4.f32, one per particle and output array        */

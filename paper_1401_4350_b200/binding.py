@@ -10,7 +10,7 @@ import numpy as np
 _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libmd_b200.so"
 
-STRATEGY = {"vertex": 0, "edge": 1}
+STRATEGY = {"vertex": 0, "edge": 1, "vertex_n3": 2}
 SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3}
 GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
@@ -124,9 +124,12 @@ def load_library() -> C.CDLL:
 
 
 def variant_code(strategy: str, variant) -> int:
-    """Third argument of md_forces / md_integrate / md_step_host: md_gather for VERTEX, md_scatter for EDGE."""
+    """Third argument of md_forces / md_integrate / md_step_host: md_gather for VERTEX, md_scatter for EDGE, the number
+    of force copies m for VERTEX_N3 (an int; anything else means the default)."""
     if strategy == "vertex":
         return GATHER.get(variant, 0)      # anything that is not a gather name means "auto"
+    if strategy == "vertex_n3":
+        return int(variant) if isinstance(variant, int) else 0
     return SCATTER[variant]
 
 

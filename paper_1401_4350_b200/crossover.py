@@ -50,6 +50,7 @@ def run_cell(torch, MDSystem, w, kind, evals, melt):
     for v in EDGE:
         n = max(2, evals // 4) if v == "red" else evals
         out[f"edge_{v}"] = time_calls(torch, lambda: s.forces("edge", v), n)
+    out["vertex_n3_m12"] = time_calls(torch, lambda: s.forces("vertex_n3", 12), evals)   # P:71, beside the two contenders
     s.close()
     bv = min(VERTEX, key=lambda v: out[f"vertex_{v}"])
     be = min(EDGE, key=lambda v: out[f"edge_{v}"])
@@ -86,7 +87,7 @@ def main():
         print(json.dumps(r), file=sys.stderr, flush=True)
         rows.append(r)
 
-    cols = [f"vertex_{v}" for v in VERTEX] + [f"edge_{v}" for v in EDGE]
+    cols = [f"vertex_{v}" for v in VERTEX] + [f"edge_{v}" for v in EDGE] + ["vertex_n3_m12"]
     print("| potential | N | r_c | entries/particle | E | " + " | ".join(c + " us" for c in cols) +
           " | t_VERTEX / t_EDGE (best of each) | x |")
     print("|" + "---|" * (7 + len(cols)))

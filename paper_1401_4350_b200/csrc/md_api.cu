@@ -428,7 +428,13 @@ static bool wants_staged(const md_system* s, int32_t strategy, int32_t variant) 
 }
 
 static md_status check_strategy(md_system* s, int32_t strategy, int32_t scatter) {
-    if (strategy != MD_VERTEX && strategy != MD_EDGE) return fail(s, MD_ERR_INVALID, "unknown strategy");
+    if (strategy != MD_VERTEX && strategy != MD_EDGE && strategy != MD_VERTEX_N3) return fail(s, MD_ERR_INVALID, "unknown strategy");
+    if (strategy == MD_VERTEX_N3) {
+        const int64_t m = scatter == 0 ? 12 : scatter;
+        if (scatter < 0 || m > 64) return fail(s, MD_ERR_INVALID, "MD_VERTEX_N3: the number of force copies m must be 1..64 (0 = 12)");
+        if ((size_t)(m * s->N) > s->ecap) return fail(s, MD_ERR_INVALID, "MD_VERTEX_N3: m * N exceeds the edge capacity N * max_neigh / 2");
+        return MD_OK;
+    }
     if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_SEGMENTED)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
     if (strategy == MD_VERTEX && (scatter < MD_GATHER_AUTO || scatter > MD_GATHER_SMEM)) return fail(s, MD_ERR_INVALID, "unknown gather variant");
     if (s->order == MD_ORDER_NONE && strategy == MD_VERTEX && scatter == MD_GATHER_SMEM)

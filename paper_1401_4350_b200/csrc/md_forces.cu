@@ -379,6 +379,78 @@ __global__ void k_edge_bonds(DevParams P, DevBuffers B, const float4* __restrict
 }
 
 // ------------------------------------------------------------------------------------------------
+// VERTEX with Newton's third law and m private force copies per particle (S:8(f1))
+// ------------------------------------------------------------------------------------------------
+// One thread per particle i over its half row (the edges (i, j) sorted by i): own side in registers and one plain
+// store, -f (and the j-side torque) added with red.v4 into copy (i mod m) of particle j (DESIGN Q20: the paper does
+// not say how a writer picks its copy).  Pairs outside the cutoff issue no atomics.
+template <int KIND>
+__global__ void __launch_bounds__(128) k_vertex_n3(DevParams P, DevBuffers B, const float4* __restrict__ pos,
+                                                   const float4* __restrict__ quat, float4* __restrict__ force,
+                                                   float4* __restrict__ torque, float4* fcopy, float4* tcopy, int m) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const size_t plane = (size_t)(i % m) * (size_t)P.N;
+    float4* fc = fcopy + plane;
+    float4* tc = KIND == MD_POT_PATCHY ? tcopy + plane : nullptr;
+    const unsigned int e0 = B.edge_off[i], e1 = B.edge_off[i + 1];
+    float ax = 0.f, ay = 0.f, az = 0.f, ape = 0.f, atx = 0.f, aty = 0.f, atz = 0.f;
+    for (unsigned int e = e0; e < e1; ++e) {
+        const int jw = B.edges[e].y;
+        float fx, fy, fz, V, tix = 0.f, tiy = 0.f, tiz = 0.f, tjx = 0.f, tjy = 0.f, tjz = 0.f;
+        if (!edge_eval<KIND>(P, pos, quat, i, jw, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz)) continue;
+        const int j = jw & 0x7fffffff;
+        const float hV = 0.5f * V;
+        ax -= fx; ay -= fy; az -= fz; ape += hV;
+        red_add_v4(fc + j, fx, fy, fz, hV);
+        if (KIND == MD_POT_PATCHY) {
+            atx += tix; aty += tiy; atz += tiz;
+            red_add_v4(tc + j, tjx, tjy, tjz, 0.f);
+        }
+    }
+    force[i] = make_float4(ax, ay, az, ape);
+    if (KIND == MD_POT_PATCHY) torque[i] = make_float4(atx, aty, atz, 0.f);
+}
+
+// "then the vectors are combined to obtain the total force acting on each particle": copies added in index order
+__global__ void __launch_bounds__(256) k_n3_combine(DevParams P, float4* __restrict__ force, float4* __restrict__ torque,
+                                                    const float4* __restrict__ fcopy, const float4* __restrict__ tcopy, int m) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    float4 f = force[i];
+    for (int c = 0; c < m; ++c) {
+        const float4 g = fcopy[(size_t)c * P.N + i];
+        f.x += g.x; f.y += g.y; f.z += g.z; f.w += g.w;
+    }
+    force[i] = f;
+    if (torque) {
+        float4 t = torque[i];
+        for (int c = 0; c < m; ++c) {
+            const float4 g = tcopy[(size_t)c * P.N + i];
+            t.x += g.x; t.y += g.y; t.z += g.z;
+        }
+        torque[i] = t;
+    }
+}
+
+template <int KIND>
+static void launch_vertex_n3(md_system* s, int m) {
+    const DevParams& P = s->P;
+    float4* tq = KIND == MD_POT_PATCHY ? s->torque : nullptr;
+    float4* fcopy = s->B.edge_f;                                   // the per-edge scratch of the segmented variant
+    float4* tcopy = KIND == MD_POT_PATCHY ? s->B.edge_tj : nullptr;
+    cudaMemsetAsync(fcopy, 0, 16 * (size_t)m * P.N, s->stream);
+    if (tcopy) cudaMemsetAsync(tcopy, 0, 16 * (size_t)m * P.N, s->stream);
+    k_vertex_n3<KIND><<<cdiv(P.N, 128), 128, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq, fcopy, tcopy, m);
+    k_n3_combine<<<cdiv(P.N, 256), 256, 0, s->stream>>>(P, s->force, tq, fcopy, tcopy, m);
+    s->launches += 2;
+    if (P.kind == MD_POT_FENE_WCA) {
+        k_edge_bonds<<<cdiv(P.N, 256), 256, 0, s->stream>>>(P, s->B, s->pos, s->force);
+        s->launches += 1;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // host-side dispatch
 // ------------------------------------------------------------------------------------------------
 template <int KIND>
@@ -413,6 +485,10 @@ void md_launch_forces(md_system* s, int strategy, int scatter) {
         else if (P.kind == MD_POT_FENE_WCA) k_vertex_lj<true><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->force);
         else k_vertex_lj<false><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->force);
         s->launches += 1;
+    } else if (strategy == MD_VERTEX_N3) {
+        const int m = scatter == 0 ? 12 : scatter;
+        if (P.kind == MD_POT_PATCHY) launch_vertex_n3<MD_POT_PATCHY>(s, m);
+        else launch_vertex_n3<MD_POT_LJ>(s, m);
     } else {
         if (P.kind == MD_POT_PATCHY) launch_edge<MD_POT_PATCHY>(s, scatter);
         else launch_edge<MD_POT_LJ>(s, scatter);

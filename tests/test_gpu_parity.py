@@ -10,7 +10,9 @@ pytestmark = pytest.mark.gpu
 
 # (strategy, variant): VERTEX gather alternatives {l2, smem}, EDGE scatter alternatives {red, red_v4, warp, segmented};
 # the shared-memory staged VERTEX variant needs cell-sorted storage (order != none)
-VARIANTS = [("vertex", "l2"), ("edge", "red"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented")]
+# VERTEX with Newton's third law (S:8(f1)): the variant is m, the number of private force copies per particle
+VARIANTS = [("vertex", "l2"), ("edge", "red"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented"),
+            ("vertex_n3", 1), ("vertex_n3", 12)]
 STAGED = [("vertex", "smem")]
 
 
@@ -81,7 +83,13 @@ def test_step0_parity(MD, oracle, case, order):
     o = oracle.forces(w.pos, w.box, dict(w.potential), quat=w.quat)
     assert o["bad"] == 0
     results = {}
+    from paper_1401_4350_b200 import MDError
     for strat, sc in variants(order):
+        if strat == "vertex_n3" and sc * w.N > w.N * ((s.max_neigh + 3) // 4 * 4) // 2 + 64:
+            with pytest.raises(MDError) as e:    # the m copies do not fit in the per-edge scratch: an error, not a clamp
+                s.forces(strat, sc)
+            assert e.value.code == -1
+            continue
         s.forces(strat, sc)
         results[(strat, sc)] = assert_forces(s, o, w.quat is not None)
     # the explicit global-slot lists (built on demand for the L2-gather variants) hold the same pair set
@@ -165,6 +173,9 @@ def test_error_paths(MD):
         s.lib.md_forces(s.h, 7, 0) and None
         s._check(s.lib.md_forces(s.h, 7, 0))    # unknown strategy
     assert e.value.code == -1
+    with pytest.raises(MDError) as e:
+        s._check(s.lib.md_forces(s.h, 2, 65))   # VERTEX_N3: m out of range
+    assert e.value.code == -1
     s.close()
     # capacity overflow is an error, never a silent truncation
     s = MD.from_workload(w, max_neigh=40)
@@ -185,7 +196,7 @@ def test_error_paths(MD):
 
 
 @pytest.mark.parametrize("strat,sc", [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp"),
-                                      ("edge", "segmented")])
+                                      ("edge", "segmented"), ("vertex_n3", 12)])
 def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
     """C1 (BASELINE.json configs[0]): 100 velocity-Verlet steps at dt = 0.002; fp32 GPU state against the fp64
     oracle trajectory from the same fp32 input.  SURVEY 8(d): the two stay within the force tolerance for 100 steps."""
@@ -213,6 +224,7 @@ def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
     ("lj", 300, "vertex", "smem"), ("lj", 300, "vertex", "l2"), ("lj", 300, "edge", "red_v4"), 
     ("polymer", 200, "vertex", "smem"), ("polymer", 200, "edge", "warp"), 
     ("patchy", 300, "vertex", "smem"), ("patchy", 300, "vertex", "l2"), ("patchy", 300, "edge", "segmented"),
+    ("lj", 300, "vertex_n3", 12), ("polymer", 200, "vertex_n3", 4), ("patchy", 300, "vertex_n3", 12),
     ])
 def test_snapshot_parity_after_device_side_rebuilds(MD, oracle, case, steps, strat, sc):
     """Run md_integrate long enough for several skin-triggered rebuilds, then compare the forces the path holds
