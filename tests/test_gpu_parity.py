@@ -288,4 +288,4 @@ def test_crossover_sweep_runs(capsys, monkeypatch):
     monkeypatch.setattr(sys, "argv", ["crossover", "--min-log2n", "12", "--max-log2n", "12", "--evals", "2", "--rcuts", "2.5"])
     crossover.main()
     out = capsys.readouterr().out
-    assert "| lj | 2^12 | 2.5 |" in out and "| patchy | 2^12 | 1.5 |" in out
+    assert "| lj | 2^12 | 0.8 | 2.5 |" in out and "| patchy | 2^12 | 0.5 | 1.5 |" in out
