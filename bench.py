@@ -296,6 +296,20 @@ def main():
     best_vertex = min((k for k in fe if k.startswith("vertex")), key=lambda k: fe[k]["us"])
     t_v = fe[best_vertex]["us"]
     clocks = sampler.stop()
+    # S:8(f3): the same K steps in mixed precision (fp64 integration of the state, fp32 forces), reported beside
+    s.set_precision("mixed")
+    s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
+    s.integrate(w.dt, Wm, args.strategy, args.scatter)
+    torch.cuda.synchronize(dev)
+    am, bm = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    am.record()
+    s.integrate(w.dt, K, args.strategy, args.scatter)
+    s.energy()
+    bm.record()
+    torch.cuda.synchronize(dev)
+    ms_mixed = am.elapsed_time(bm) / K
+    mixed = {"ms_per_step": ms_mixed, "cost_vs_fp32": ms_mixed / (ms_total / K), "paper": "10-40 % on C2070/K10/K20 (P:59)"}
+    s.set_precision("f32")
     best_edge = min((k for k in fe if k.startswith("edge")), key=lambda k: fe[k]["us"])
     peak, peak_src = measured_peaks()
     dom = args.strategy
@@ -366,7 +380,7 @@ def main():
                           "timing without a flush -- a secondary workload, the headline is C2a"),
                    "rebuilds_in_timed_region": st1["n_rebuilds"] - stw["n_rebuilds"],
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "force_eval": fe, "vertex_n3_eval": n3, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
+        "force_eval": fe, "vertex_n3_eval": n3, "mixed_precision": mixed, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
         "best_vertex": best_vertex,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "energy_total": sum(e_tot),

@@ -82,6 +82,10 @@ typedef enum {
                            16-bit block-local list entries ordered at build time for conflict-free 128-bit gathers */
 } md_gather;
 typedef enum { MD_ORDER_NONE = 0, MD_ORDER_CELL = 1, MD_ORDER_HILBERT = 2 } md_order;
+/* P:59 (S:8(f3)): MD_PREC_F32 = fp32 state and integration (B:7, the default); MD_PREC_MIXED = the paper's production
+ * mode, "mixed precision": positions, velocities (and angular momenta, quaternions) integrated in fp64, forces and
+ * torques computed in fp32 from the rounded positions. */
+typedef enum { MD_PREC_F32 = 0, MD_PREC_MIXED = 1 } md_precision;
 
 /* Pair potential and rigid-body parameters.
  *   MD_POT_LJ        Eq. (1), cut at rcut and energy-shifted by V(rcut) if shift_energy.
@@ -125,6 +129,18 @@ md_status md_bind_state(md_system*, void* pos, void* vel, void* force, void* qua
 
 /* Storage order applied at every list build ("sorted along a Hilbert curve"). Default NONE. */
 md_status md_set_order(md_system*, int32_t order);
+
+/* precision of md_integrate's state (default MD_PREC_F32).  In MD_PREC_MIXED the library keeps fp64 copies of
+ * the integrated arrays in its workspace: they are taken from the bound fp32 arrays by the first md_build_cells /
+ * md_integrate / md_step_host after md_bind_state or md_set_precision, advanced by md_integrate, wrapped and
+ * reordered with the fp32 arrays, and the fp32 arrays are rewritten from them (round to nearest) at every step, so
+ * every other call sees the same interface.  State written into the fp32 arrays behind the library's back is not
+ * seen until the next md_bind_state.  MD_ERR_INVALID for an unknown value. */
+md_status md_set_precision(md_system*, int32_t precision);
+
+/* The fp64 state of MD_PREC_MIXED in ORIGINAL id order: pos_host, vel_host = HOST double[3 N] (x, y, z per particle),
+ * either may be NULL.  Synchronises.  MD_ERR_STATE unless the precision is MD_PREC_MIXED and the copies exist. */
+md_status md_get_state_double(md_system*, double* pos_host, double* vel_host);
 
 /* S:A2/A3 ("cell filling ... one-particle-per-thread"): wrap positions into [0, box), bin into
  * cells, counting sort; with an order set, permute all bound state arrays into cell / Hilbert order. */

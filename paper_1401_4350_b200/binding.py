@@ -14,12 +14,14 @@ STRATEGY = {"vertex": 0, "edge": 1, "vertex_n3": 2}
 SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3}
 GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
+PRECISION = {"f32": 0, "mixed": 1}
 POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2}
 STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPACITY", -4: "MD_ERR_CUDA",
           -5: "MD_ERR_NUMERIC"}
 
 # every symbol include/md_b200.h declares (checked by tests/test_abi.py against the header and the .so)
-EXPORTED_SYMBOLS = ["md_workspace_bytes", "md_create", "md_bind_state", "md_set_order", "md_build_cells",
+EXPORTED_SYMBOLS = ["md_workspace_bytes", "md_create", "md_bind_state", "md_set_order", "md_set_precision",
+                    "md_get_state_double", "md_build_cells",
                     "md_build_verlet", "md_forces", "md_integrate", "md_energy", "md_stats", "md_get_pairs",
                     "md_get_ids", "md_step_host", "md_launch_count", "md_last_error", "md_destroy"]
 
@@ -96,6 +98,10 @@ def load_library() -> C.CDLL:
     L.md_bind_state.argtypes = [vp] * 7
     L.md_set_order.restype = C.c_int
     L.md_set_order.argtypes = [vp, C.c_int32]
+    L.md_set_precision.restype = C.c_int
+    L.md_set_precision.argtypes = [vp, C.c_int32]
+    L.md_get_state_double.restype = C.c_int
+    L.md_get_state_double.argtypes = [vp, vp, vp]
     for name in ("md_build_cells", "md_build_verlet"):
         getattr(L, name).restype = C.c_int
         getattr(L, name).argtypes = [vp]
@@ -223,6 +229,15 @@ class MDSystem:
     # ---- the C ABI, same names ----
     def set_order(self, order):
         self._check(self.lib.md_set_order(self.h, ORDER[order] if isinstance(order, str) else int(order)))
+
+    def set_precision(self, precision):
+        self._check(self.lib.md_set_precision(self.h, PRECISION[precision] if isinstance(precision, str) else int(precision)))
+
+    def state_f64(self):
+        """(pos, vel) of MD_PREC_MIXED as float64 [N,3] arrays in original id order."""
+        pos, vel = np.empty((self.N, 3), dtype=np.float64), np.empty((self.N, 3), dtype=np.float64)
+        self._check(self.lib.md_get_state_double(self.h, C.c_void_p(pos.ctypes.data), C.c_void_p(vel.ctypes.data)))
+        return pos, vel
 
     def build_cells(self):
         self._check(self.lib.md_build_cells(self.h))

@@ -71,7 +71,8 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.ids = (int*)take(4 * Npad);
     b.ids_tmp = (int*)take(4 * Npad);
     b.slot_of_id = (int*)take(4 * Npad);
-    b.tmp4 = (float4*)take(16 * Npad * (rigid ? 6 : 3));   // permutation scratch, one plane per state array
+    b.tmp4 = (float4*)take(16 * Npad * (rigid ? 14 : 7));   // permutation scratch, one plane per state array and fp64 half
+    for (int k = 0; k < (rigid ? 8 : 4); ++k) b.shadow[k] = (float4*)take(16 * Npad);
     b.pos_ref = (float4*)take(16 * Npad);
     b.nl_count = (int*)take(4 * Npad);
     b.nl_full = (int*)take(4 * Npad * g.cap);
@@ -358,6 +359,7 @@ md_status md_bind_state(md_system* s, void* pos, void* vel, void* force, void* q
     s->angmom = s->rigid ? (float4*)angmom : nullptr;
     s->torque = s->rigid ? (float4*)torque : nullptr;
     s->bound = true;
+    s->shadow_valid = false;
     s->cells_valid = s->lists_valid = s->forces_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
     drop_step_graph(s);   // the step graph bakes the state pointers in
     reset_ids(s);   // the arrays are taken to be in original id order
@@ -378,10 +380,57 @@ md_status md_set_order(md_system* s, int32_t order) {
     return check_cuda(s, "md_set_order");
 }
 
+// mixed precision: the fp64 copies are taken from the bound fp32 arrays the first time they are needed after a bind
+static void ensure_shadows(md_system* s) {
+    if (s->precision != MD_PREC_MIXED || s->shadow_valid) return;
+    md_launch_shadow_init(s);
+    s->shadow_valid = true;
+}
+
+md_status md_set_precision(md_system* s, int32_t precision) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (precision != MD_PREC_F32 && precision != MD_PREC_MIXED) return fail(s, MD_ERR_INVALID, "md_set_precision: unknown precision");
+    if (precision != s->precision) {
+        s->precision = precision;
+        s->shadow_valid = false;
+        drop_step_graph(s);   // the step graph bakes the integration kernels in
+    }
+    return MD_OK;
+}
+
+md_status md_get_state_double(md_system* s, double* pos_host, double* vel_host) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (s->precision != MD_PREC_MIXED || !s->bound || !s->shadow_valid)
+        return fail(s, MD_ERR_STATE, "md_get_state_double: needs MD_PREC_MIXED and a bound state that md_build_cells or md_integrate has seen");
+    const size_t n = (size_t)s->N;
+    std::vector<double> plane(2 * n);
+    std::vector<int> ids(n);
+    cudaMemcpyAsync(ids.data(), s->B.ids, 4 * n, cudaMemcpyDeviceToHost, s->stream);
+    md_status st = sync_and_check(s, "md_get_state_double");
+    if (st != MD_OK) return st;
+    double* outs[2] = { pos_host, vel_host };
+    for (int a = 0; a < 2; ++a) {
+        if (!outs[a]) continue;
+        for (int h = 0; h < 2; ++h) {   // plane 2a: (x, y), plane 2a+1: (z, -)
+            cudaMemcpyAsync(plane.data(), s->B.shadow[2 * a + h], 16 * n, cudaMemcpyDeviceToHost, s->stream);
+            if ((st = sync_and_check(s, "md_get_state_double")) != MD_OK) return st;
+            for (size_t i = 0; i < n; ++i) {
+                double* o = outs[a] + 3 * (size_t)ids[i];
+                if (h == 0) { o[0] = plane[2 * i]; o[1] = plane[2 * i + 1]; }
+                else o[2] = plane[2 * i];
+            }
+        }
+    }
+    return MD_OK;
+}
+
 md_status md_build_cells(md_system* s) {
     if (!s) return MD_ERR_INVALID;
     if (s->sticky) return (md_status)s->sticky;
     if (!s->bound) return fail(s, MD_ERR_STATE, "md_build_cells: no state bound");
+    ensure_shadows(s);
     md_launch_build_cells(s, false);
     s->cells_valid = true;
     s->lists_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
@@ -524,7 +573,7 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     GCHK(cudaGraphInstantiate(exec_out, graph, 0));
     if (graph) cudaGraphDestroy(graph);
     if (!ok) { cudaGetLastError(); drop_step_graph(s); return false; }
-    s->step_strategy = strategy; s->step_variant = scatter; s->step_dt = fdt; s->step_stage = s->stage_launch;
+    s->step_strategy = strategy; s->step_variant = scatter; s->step_dt = fdt; s->step_dt_d = s->dt_d; s->step_stage = s->stage_launch;
     *nodes_out = main_nodes;
     return true;
 }
@@ -562,11 +611,13 @@ md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy
     if (!staged) ensure_explicit(s);
     if (seg && !s->seg_valid) { md_launch_seg_index(s, false); s->seg_valid = true; }
     const float fdt = (float)dt;
+    s->dt_d = dt;
+    ensure_shadows(s);
     int64_t k0 = 0;
     if (!s->graphs_off && getenv("MD_B200_NO_GRAPH")) s->graphs_off = true;   // plain launches (profilers list every kernel)
     if (!s->graphs_off && nsteps > 0) {
         if (!s->step_exec || s->step_strategy != strategy || s->step_variant != scatter || s->step_dt != fdt ||
-            s->step_stage != s->stage_launch) {
+            s->step_dt_d != dt || s->step_stage != s->stage_launch) {
             drop_step_graph(s);
             if (!build_step_graph(s, fdt, strategy, scatter, staged, seg, 1, &s->step_exec, &s->step_nodes) ||
                 !build_step_graph(s, fdt, strategy, scatter, staged, seg, MD_GRAPH_STEPS, &s->multi_exec, &s->multi_nodes)) s->graphs_off = true;
@@ -675,6 +726,7 @@ md_status md_step_host(md_system* s, void* pos_host, void* vel_host, void* force
     if (st != MD_OK) return st;
     const size_t bytes = 16 * (size_t)s->N;
     reset_ids(s);   // host buffers are in ORIGINAL id order
+    s->shadow_valid = false;
     cudaMemcpyAsync(s->pos, pos_host, bytes, cudaMemcpyHostToDevice, s->stream);
     cudaMemcpyAsync(s->vel, vel_host, bytes, cudaMemcpyHostToDevice, s->stream);
     if (s->rigid) {

@@ -146,6 +146,37 @@ __global__ void k_wrap_bin(DevParams P, DevBuffers B, int gated, float4* pos) {
     B.ids_tmp[i] = atomicAdd(&B.cell_count[c], 1);   // arrival index inside the cell (order fixed below)
 }
 
+// mixed precision: the fp64 position is wrapped, the fp32 position is its rounding, kept inside [0, L)
+__device__ __forceinline__ double wrap1d(double x, double L) {
+    if (x >= 0.0 && x < L) return x;
+    double w = x - L * floor(x / L);
+    if (!(w >= 0.0) || w >= L) w = 0.0;
+    return w;
+}
+__device__ __forceinline__ float round_inside(double x, float L) {
+    float f = (float)x;
+    return f < L ? f : nextafterf(L, 0.0f);   // a double just below L may round up to L
+}
+__global__ void k_wrap_bin_mixed(DevParams P, DevBuffers B, int gated, float4* pos) {
+    GATE(B, gated);
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    double2* pxy = reinterpret_cast<double2*>(B.shadow[0]);
+    double2* pz = reinterpret_cast<double2*>(B.shadow[1]);
+    double2 xy = pxy[i], z_ = pz[i];
+    xy.x = wrap1d(xy.x, P.dLx); xy.y = wrap1d(xy.y, P.dLy); z_.x = wrap1d(z_.x, P.dLz);
+    pxy[i] = xy; pz[i] = z_;
+    float4 x = pos[i];
+    x.x = round_inside(xy.x, P.Lx); x.y = round_inside(xy.y, P.Ly); x.z = round_inside(z_.x, P.Lz);
+    pos[i] = x;
+    int cx = cell_coord(x.x, P.cscale_x, P.ncx);
+    int cy = cell_coord(x.y, P.cscale_y, P.ncy);
+    int cz = cell_coord(x.z, P.cscale_z, P.ncz);
+    int c = B.cell_rank[(cx * P.ncy + cy) * P.ncz + cz];
+    B.cell_of[i] = c;
+    B.ids_tmp[i] = atomicAdd(&B.cell_count[c], 1);
+}
+
 __global__ void k_cell_scatter(DevParams P, DevBuffers B, int gated) {
     GATE(B, gated);
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -168,7 +199,7 @@ __global__ void k_cell_rank_sort(DevParams P, DevBuffers B, int gated) {
 // ------------------------------------------------------------------------------------------------
 // S:A3 physical reordering: new slot s takes the particle of old slot items[s]
 // ------------------------------------------------------------------------------------------------
-struct StateArrays { float4* a[6]; int n; };
+struct StateArrays { float4* a[14]; int n; };   // six fp32 arrays + up to eight fp64 half planes (mixed precision)
 
 // all bound state arrays, ids and cell indices in one pass: plane k of tmp4 takes array k in the new order
 __global__ void k_gather_state(DevParams P, DevBuffers B, int gated, StateArrays S, size_t plane) {
@@ -197,7 +228,9 @@ void md_launch_build_cells(md_system* s, bool gated) {
     int g = gated ? 1 : 0;
     int nbN = cdiv(P.N, 256);
     k_zero_counts<<<cdiv(P.ncell + 1, 256), 256, 0, s->stream>>>(P, s->B, g);
-    k_wrap_bin<<<nbN, 256, 0, s->stream>>>(P, s->B, g, s->pos);
+    const bool mixed = s->precision == MD_PREC_MIXED && s->shadow_valid;
+    if (mixed) k_wrap_bin_mixed<<<nbN, 256, 0, s->stream>>>(P, s->B, g, s->pos);
+    else k_wrap_bin<<<nbN, 256, 0, s->stream>>>(P, s->B, g, s->pos);
     s->launches += 2;
     launch_scan(s, gated, (const unsigned int*)s->B.cell_count, (unsigned int*)s->B.cell_start, P.ncell, nullptr);
     k_cell_scatter<<<nbN, 256, 0, s->stream>>>(P, s->B, g);
@@ -208,6 +241,7 @@ void md_launch_build_cells(md_system* s, bool gated) {
         StateArrays S;
         S.n = 0;
         for (int a = 0; a < 6; ++a) if (arrs[a]) S.a[S.n++] = arrs[a];
+        if (mixed) for (int k = 0; k < (s->rigid ? 8 : 4); ++k) S.a[S.n++] = s->B.shadow[k];
         const size_t plane = (size_t)P.ntiles * MD_TILE;
         k_gather_state<<<nbN, 256, 0, s->stream>>>(P, s->B, g, S, plane);
         k_commit_state<<<nbN, 256, 0, s->stream>>>(P, s->B, g, S, plane);

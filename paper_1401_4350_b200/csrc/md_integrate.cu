@@ -69,6 +69,120 @@ __global__ void __launch_bounds__(256) k_kick(DevParams P, float dt, float4* __r
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Mixed precision (S:8(f3)): the same two kernels on the fp64 copies of the state; forces and torques stay
+// fp32, the fp32 arrays are rewritten (round to nearest) for the force kernels, the skin check and the caller.
+// ------------------------------------------------------------------------------------------------
+template <bool RIGID, bool PRE>
+__global__ void __launch_bounds__(256) k_kick_drift_mixed(DevParams P, DevBuffers B, double dt, float4* pos, float4* vel,
+                                                          const float4* __restrict__ force, float4* quat, float4* angmom,
+                                                          const float4* __restrict__ torque) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i < P.N) {
+        double2* pxy = reinterpret_cast<double2*>(B.shadow[0]); double2* pz = reinterpret_cast<double2*>(B.shadow[1]);
+        double2* vxy = reinterpret_cast<double2*>(B.shadow[2]); double2* vz = reinterpret_cast<double2*>(B.shadow[3]);
+        const double hk = 0.5 * dt / (double)P.mass;
+        const float4 f = force[i];
+        double2 xa = pxy[i], xb = pz[i], va = vxy[i], vb = vz[i];
+        if (PRE) { va.x = fma(hk, (double)f.x, va.x); va.y = fma(hk, (double)f.y, va.y); vb.x = fma(hk, (double)f.z, vb.x); }
+        va.x = fma(hk, (double)f.x, va.x); va.y = fma(hk, (double)f.y, va.y); vb.x = fma(hk, (double)f.z, vb.x);
+        xa.x = fma(dt, va.x, xa.x); xa.y = fma(dt, va.y, xa.y); xb.x = fma(dt, vb.x, xb.x);
+        pxy[i] = xa; pz[i] = xb; vxy[i] = va; vz[i] = vb;
+        float4 x = pos[i], v = vel[i];
+        x.x = (float)xa.x; x.y = (float)xa.y; x.z = (float)xb.x;
+        v.x = (float)va.x; v.y = (float)va.y; v.z = (float)vb.x;
+        pos[i] = x; vel[i] = v;
+        if (RIGID) {
+            double2* lxy = reinterpret_cast<double2*>(B.shadow[4]); double2* lz = reinterpret_cast<double2*>(B.shadow[5]);
+            double2* qa = reinterpret_cast<double2*>(B.shadow[6]); double2* qb = reinterpret_cast<double2*>(B.shadow[7]);
+            const float4 t = torque[i];
+            const double hd = 0.5 * dt;
+            double2 La = lxy[i], Lb = lz[i];
+            if (PRE) { La.x = fma(hd, (double)t.x, La.x); La.y = fma(hd, (double)t.y, La.y); Lb.x = fma(hd, (double)t.z, Lb.x); }
+            La.x = fma(hd, (double)t.x, La.x); La.y = fma(hd, (double)t.y, La.y); Lb.x = fma(hd, (double)t.z, Lb.x);
+            lxy[i] = La; lz[i] = Lb;
+            float4 L = angmom[i];
+            L.x = (float)La.x; L.y = (float)La.y; L.z = (float)Lb.x;
+            angmom[i] = L;
+            const double inv_I = (double)P.inv_inertia;
+            const double wx = La.x * inv_I, wy = La.y * inv_I, wz = Lb.x * inv_I;
+            const double wn = sqrt(wx * wx + wy * wy + wz * wz);
+            if (wn > 0.0) {   // S:O7, as k_kick_drift
+                double sn, c;
+                sincos(0.5 * wn * dt, &sn, &c);
+                sn /= wn;
+                const double a0 = c, a1 = sn * wx, a2 = sn * wy, a3 = sn * wz;
+                const double2 q01 = qa[i], q23 = qb[i];
+                const double q0 = q01.x, q1 = q01.y, q2 = q23.x, q3 = q23.y;
+                double r0 = a0 * q0 - a1 * q1 - a2 * q2 - a3 * q3;
+                double r1 = a0 * q1 + a1 * q0 + a2 * q3 - a3 * q2;
+                double r2 = a0 * q2 - a1 * q3 + a2 * q0 + a3 * q1;
+                double r3 = a0 * q3 + a1 * q2 - a2 * q1 + a3 * q0;
+                const double nrm = 1.0 / sqrt(r0 * r0 + r1 * r1 + r2 * r2 + r3 * r3);
+                r0 *= nrm; r1 *= nrm; r2 *= nrm; r3 *= nrm;
+                qa[i] = make_double2(r0, r1); qb[i] = make_double2(r2, r3);
+                quat[i] = make_float4((float)r0, (float)r1, (float)r2, (float)r3);
+            }
+        }
+        const float4 r = B.pos_ref[i];
+        const float dx = x.x - r.x, dy = x.y - r.y, dz = x.z - r.z;
+        moved = (dx * dx + dy * dy + dz * dz) > P.half_skin2;   // S:Q4, on the fp32 positions the lists were built from
+    }
+    if (__any_sync(0xffffffffu, moved) && (threadIdx.x & 31) == 0) B.ctrl->rebuild = 1;
+}
+
+template <bool RIGID>
+__global__ void __launch_bounds__(256) k_kick_mixed(DevParams P, DevBuffers B, double dt, float4* vel, const float4* __restrict__ force,
+                                                    float4* angmom, const float4* __restrict__ torque) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    double2* vxy = reinterpret_cast<double2*>(B.shadow[2]); double2* vz = reinterpret_cast<double2*>(B.shadow[3]);
+    const double hk = 0.5 * dt / (double)P.mass;
+    const float4 f = force[i];
+    double2 va = vxy[i], vb = vz[i];
+    va.x = fma(hk, (double)f.x, va.x); va.y = fma(hk, (double)f.y, va.y); vb.x = fma(hk, (double)f.z, vb.x);
+    vxy[i] = va; vz[i] = vb;
+    float4 v = vel[i];
+    v.x = (float)va.x; v.y = (float)va.y; v.z = (float)vb.x;
+    vel[i] = v;
+    if (RIGID) {
+        double2* lxy = reinterpret_cast<double2*>(B.shadow[4]); double2* lz = reinterpret_cast<double2*>(B.shadow[5]);
+        const float4 t = torque[i];
+        const double hd = 0.5 * dt;
+        double2 La = lxy[i], Lb = lz[i];
+        La.x = fma(hd, (double)t.x, La.x); La.y = fma(hd, (double)t.y, La.y); Lb.x = fma(hd, (double)t.z, Lb.x);
+        lxy[i] = La; lz[i] = Lb;
+        float4 L = angmom[i];
+        L.x = (float)La.x; L.y = (float)La.y; L.z = (float)Lb.x;
+        angmom[i] = L;
+    }
+}
+
+// fp64 copies <- the bound fp32 arrays (exact)
+__global__ void __launch_bounds__(256) k_shadow_init(DevParams P, DevBuffers B, const float4* __restrict__ pos, const float4* __restrict__ vel,
+                                                     const float4* __restrict__ quat, const float4* __restrict__ angmom) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const float4 x = pos[i], v = vel[i];
+    reinterpret_cast<double2*>(B.shadow[0])[i] = make_double2((double)x.x, (double)x.y);
+    reinterpret_cast<double2*>(B.shadow[1])[i] = make_double2((double)x.z, 0.0);
+    reinterpret_cast<double2*>(B.shadow[2])[i] = make_double2((double)v.x, (double)v.y);
+    reinterpret_cast<double2*>(B.shadow[3])[i] = make_double2((double)v.z, 0.0);
+    if (quat) {
+        const float4 q = quat[i], L = angmom[i];
+        reinterpret_cast<double2*>(B.shadow[4])[i] = make_double2((double)L.x, (double)L.y);
+        reinterpret_cast<double2*>(B.shadow[5])[i] = make_double2((double)L.z, 0.0);
+        reinterpret_cast<double2*>(B.shadow[6])[i] = make_double2((double)q.x, (double)q.y);
+        reinterpret_cast<double2*>(B.shadow[7])[i] = make_double2((double)q.z, (double)q.w);
+    }
+}
+
+void md_launch_shadow_init(md_system* s) {
+    k_shadow_init<<<cdiv(s->P.N, 256), 256, 0, s->stream>>>(s->P, s->B, s->pos, s->vel, s->rigid ? s->quat : nullptr, s->rigid ? s->angmom : nullptr);
+    s->launches += 1;
+}
+
 // drives the IF node of the step graph: run the rebuild body iff the skin criterion tripped (S:A5)
 __global__ void k_set_cond(cudaGraphConditionalHandle h, DevBuffers B) { cudaGraphSetConditional(h, B.ctrl->rebuild != 0 ? 1u : 0u); }
 
@@ -79,6 +193,18 @@ void md_launch_set_cond(md_system* s, unsigned long long cond_handle) {
 
 void md_launch_kick_drift(md_system* s, float dt, bool pre) {
     int nb = cdiv(s->P.N, 256);
+    if (s->precision == MD_PREC_MIXED) {
+        const double d = s->dt_d;
+        if (s->rigid) {
+            if (pre) k_kick_drift_mixed<true, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, d, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
+            else k_kick_drift_mixed<true, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, d, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
+        } else {
+            if (pre) k_kick_drift_mixed<false, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, d, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
+            else k_kick_drift_mixed<false, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, d, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
+        }
+        s->launches += 1;
+        return;
+    }
     if (s->rigid) {
         if (pre) k_kick_drift<true, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
         else k_kick_drift<true, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
@@ -91,6 +217,12 @@ void md_launch_kick_drift(md_system* s, float dt, bool pre) {
 
 void md_launch_kick(md_system* s, float dt) {
     int nb = cdiv(s->P.N, 256);
+    if (s->precision == MD_PREC_MIXED) {
+        if (s->rigid) k_kick_mixed<true><<<nb, 256, 0, s->stream>>>(s->P, s->B, s->dt_d, s->vel, s->force, s->angmom, s->torque);
+        else k_kick_mixed<false><<<nb, 256, 0, s->stream>>>(s->P, s->B, s->dt_d, s->vel, s->force, nullptr, nullptr);
+        s->launches += 1;
+        return;
+    }
     if (s->rigid) k_kick<true><<<nb, 256, 0, s->stream>>>(s->P, dt, s->vel, s->force, s->angmom, s->torque);
     else k_kick<false><<<nb, 256, 0, s->stream>>>(s->P, dt, s->vel, s->force, nullptr, nullptr);
     s->launches += 1;

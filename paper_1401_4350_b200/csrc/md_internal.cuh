@@ -119,6 +119,10 @@ struct DevBuffers {
     int* lo_count;         // [Npad] neighbours with slot < i
     BlkInfo* blk;          // [nblk]
     int2* seg;             // [nblk*MD_SEGMAX] (first slot, first local index)
+    // mixed precision (S:8(f3)): fp64 copies of the integrated state, two 16-byte planes per array so that the
+    // reordering moves them like any other plane: [0] pos (x,y) [1] pos (z,-) [2] vel (x,y) [3] vel (z,-)
+    // [4] angmom (x,y) [5] angmom (z,-) [6] quat (w,x) [7] quat (y,z)
+    float4* shadow[8];     // each [Npad]; [4..7] only for rigid bodies
 };
 
 struct md_system {
@@ -147,6 +151,9 @@ struct md_system {
     cudaStream_t cap_stream, aux_stream; // internal capture streams: main sequence, conditional body
     int step_strategy, step_variant, step_stage, step_nodes, multi_nodes;   // *_nodes: kernels per launch outside the IF body
     float step_dt;
+    int precision;                       // md_precision
+    bool shadow_valid;                   // the fp64 copies describe the bound fp32 arrays
+    double dt_d, step_dt_d;              // time step of the running / captured md_integrate in fp64 (mixed precision)
     bool graphs_off;                     // graph construction failed once: plain launches from then on
 };
 
@@ -159,6 +166,7 @@ void md_launch_build_end(md_system* s, bool gated);
 void md_launch_forces(md_system* s, int strategy, int scatter);
 void md_launch_kick_drift(md_system* s, float dt, bool pre);   // pre: also the previous step's closing half kick
 void md_launch_kick(md_system* s, float dt);
+void md_launch_shadow_init(md_system* s);   // fp64 copies <- bound fp32 arrays
 void md_launch_energy(md_system* s);
 void md_launch_set_cond(md_system* s, unsigned long long cond_handle);   // conditional value = rebuild flag
 void md_launch_unpermute(md_system* s, const float4* src, float4* dst);   // dst[ids[s]] = src[s]

@@ -289,3 +289,104 @@ def test_crossover_sweep_runs(capsys, monkeypatch):
     crossover.main()
     out = capsys.readouterr().out
     assert "| lj | 2^12 | 0.8 | 2.5 |" in out and "| patchy | 2^12 | 0.5 | 1.5 |" in out
+
+
+# ---- mixed precision (S:8(f3)): fp64 integration of the state, fp32 forces ----
+def test_mixed_precision_free_flight_matches_fp64_oracle(MD, oracle):
+    """A dilute lattice (nearest neighbours beyond r_v, so every force is exactly zero) translating rigidly: the fp64
+    state must follow the fp64 oracle and the closed form x0 + n dt v to rounding through ~20 device-side rebuilds
+    (wrap in fp64, Hilbert reordering of the fp64 planes); the fp32 state of the default precision cannot."""
+    w = W.lj_fluid(256, rho=0.03, jitter=0.0)
+    w.vel[:, :3] = np.array([0.7, -0.3, 0.45], dtype=np.float32)
+    nsteps = 2000
+    o = oracle.integrate(w.pos, w.vel, w.box, dict(w.potential), w.skin, w.dt, nsteps)
+    assert np.abs(o["F"]).max() == 0.0
+    exact = w.pos[:, :3].astype(np.float64) + nsteps * w.dt * w.vel[:, :3].astype(np.float64)
+    err = {}
+    for prec in ("mixed", "f32"):
+        s = MD.from_workload(w, order="hilbert")
+        s.set_precision(prec)
+        s.build_cells(); s.build_verlet(); s.forces("vertex")
+        s.integrate(w.dt, nsteps, "vertex")
+        assert s.stats()["n_rebuilds"] >= 10
+        if prec == "mixed":
+            x, v = s.state_f64()
+            assert np.array_equal(v, w.vel[:, :3].astype(np.float64))
+            x32 = s.in_id_order(s.pos)[:, :3]
+            assert np.array_equal(x32, x.astype(np.float32))            # the fp32 arrays are the rounded fp64 state
+        else:
+            x = s.in_id_order(s.pos)[:, :3].astype(np.float64)
+        for name, ref in (("oracle", o["pos"][:, :3]), ("closed_form", exact)):
+            dx = x - ref
+            dx -= w.box * np.round(dx / w.box)
+            err[(prec, name)] = np.abs(dx).max()
+        s.close()
+    assert err[("mixed", "oracle")] < 1e-11 and err[("mixed", "closed_form")] < 1e-11
+    assert err[("f32", "closed_form")] > 1e-8                            # what the mode is for
+
+
+@pytest.mark.parametrize("strat,sc", [("vertex", "smem"), ("edge", "warp")])
+def test_mixed_precision_c1_trajectory(MD, oracle, strat, sc):
+    """C1, 100 steps: mixed precision stays within the tolerances of the fp32 trajectory test against the fp64 oracle."""
+    w = W.config("C1")
+    o = oracle.integrate(w.pos, w.vel, w.box, dict(w.potential), w.skin, w.dt, 100, every=100)
+    s = MD.from_workload(w, order="cell")
+    s.set_precision("mixed")
+    s.build_cells(); s.build_verlet(); s.forces(strat, sc)
+    s.integrate(w.dt, 100, strat, sc)
+    assert s.stats()["n_rebuilds"] >= 1
+    fmax = np.abs(o["F"]).max()
+    F = s.in_id_order(s.force)
+    assert np.abs(F[:, :3] - o["F"]).max() <= FTOL_REL * fmax + FTOL_ABS
+    x, v = s.state_f64()
+    dx = x - o["pos"][:, :3]
+    dx -= w.box * np.round(dx / w.box)
+    assert np.abs(dx).max() < 1e-4
+    assert np.abs(v - o["vel"][:, :3]).max() < 1e-3
+    e1 = s.energy()
+    assert abs(sum(e1) - o["energies"][-1].sum()) <= ETOL * abs(o["energies"][-1].sum())
+    s.close()
+
+
+def test_mixed_precision_rigid_bodies_after_rebuilds(MD, oracle):
+    """Patchy rigid bodies in mixed precision: after several device-side rebuilds the forces and torques the path holds
+    equal the oracle's on the same positions and orientations, and the quaternions are still unit."""
+    w = W.patchy_fluid(2 ** 12, T=1.0)
+    s = MD.from_workload(w, order="hilbert")
+    s.set_precision("mixed")
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    s.integrate(w.dt, 300, "vertex")
+    assert s.stats()["n_rebuilds"] >= 2
+    pos, quat = s.in_id_order(s.pos), s.in_id_order(s.quat)
+    assert np.abs(np.linalg.norm(quat.astype(np.float64), axis=1) - 1.0).max() < 1e-6
+    o = oracle.forces(pos, w.box, dict(w.potential), quat=quat)
+    assert_forces(s, o, True)
+    s.close()
+
+
+def test_mixed_precision_nve_drift_c1(MD):
+    """mixed precision 'improves stability': the C1 energy drift over 10^4 steps is bounded as in fp32."""
+    w = W.config("C1")
+    s = MD.from_workload(w, order="cell")
+    s.set_precision("mixed")
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    e0 = sum(s.energy())
+    worst = 0.0
+    for _ in range(20):
+        s.integrate(w.dt, 500, "vertex")
+        worst = max(worst, abs(sum(s.energy()) - e0) / abs(e0))
+    print("mixed-precision C1 drift over 1e4 steps:", worst)
+    assert worst <= 5e-5
+    s.close()
+
+
+def test_precision_errors(MD):
+    from paper_1401_4350_b200 import MDError
+    s = MD.from_workload(W.config("C1"))
+    with pytest.raises(MDError) as e:
+        s.set_precision(5)
+    assert e.value.code == -1
+    with pytest.raises(MDError) as e:
+        s.state_f64()                          # default precision: no fp64 state
+    assert e.value.code == -2
+    s.close()
