@@ -225,10 +225,25 @@ md_status sync_and_check(md_system* s, const char* where) {
         return MD_ERR_CAPACITY;
     }
     if (s->order != MD_ORDER_NONE && c.max_stage > 0) {
-        // size the staged force launches from the largest neighbourhood seen, with 25 % head room for the
-        // device-side rebuilds that happen before the next synchronising call
+        // size the staged force launches from the largest neighbourhood seen, with 15 % head room for the
+        // device-side rebuilds that happen before the next synchronising call; if that head room alone costs a
+        // resident block per SM, keep only as much of it as still fits the block count of a tight (4 %) fit
         int want = (int)(c.max_stage * 1.15) + 64;
         want = (want + 63) / 64 * 64;
+        const size_t per_entry = s->rigid ? 32 : 16, sm_bytes = 228 * 1024, xch = s->rigid ? 0 : 24 * MD_TB;
+        auto per_block = [&](int se) {
+            size_t b = 16 + per_entry * (size_t)se;
+            if (b > 75 * 1024) b += xch;
+            return b + 1024;
+        };
+        const int tight = ((int)(c.max_stage * 1.04) + 32 + 63) / 64 * 64;
+        const int nb_t = (int)std::min<size_t>(4, sm_bytes / per_block(tight)), nb_w = (int)std::min<size_t>(4, sm_bytes / per_block(want));
+        if (nb_t > nb_w) {
+            size_t budget = sm_bytes / nb_t - 1024 - 16;
+            if (budget > 75 * 1024 + xch) budget -= xch;
+            const int fit = (int)(budget / per_entry) / 64 * 64;
+            if (fit >= tight && fit < want) want = fit;
+        }
         s->stage_launch = want;
     }
     if (c.err & MD_DEVERR_FENE) {

@@ -906,7 +906,7 @@ __device__ __forceinline__ void lj_chunk_s(const DevParams& P, unsigned int sp32
 // cnt, pk[0..3]: |L_i| and the first four row chunks, loaded by the caller while the staging copies were in flight.
 // The row streams from HBM (~1300 cycles under load); chunks are consumed four per iteration through four separate
 // load instructions, each re-issued four chunks (~350 instructions of arithmetic) ahead of its use.
-// NS = threads per particle (1, or 2 when the staged neighbourhood is so large that only one or two 256-particle blocks
+// NS = threads per particle (1; 2 or 4 when the staged neighbourhood is so large that only one or two 256-particle blocks
 // fit on an SM: the block then runs 512 threads, thread h * 256 + p takes the row chunks c = h mod 2 of particle p and the
 // two partial sums meet in shared memory -- twice the warps for the same shared memory).  xch = exchange buffer (NS == 2).
 template <bool IMG, int SH, bool UNIT, int NS>
@@ -941,15 +941,20 @@ __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuff
     }
     float pe2 = a.pe.x + a.pe.y;
     float nin = a.nin.x + a.nin.y;
-    if (NS == 2) {                                         // second half hands its partial sums to the first
-        if (h == 1) {
-            xch[tp] = a.fx; xch[MD_TB + tp] = a.fy; xch[2 * MD_TB + tp] = a.fz; xch[3 * MD_TB + tp] = pe2;
-            xch[4 * MD_TB + tp] = nin; xch[5 * MD_TB + tp] = a.band;
+    if (NS > 1) {                                          // threads h > 0 hand their partial sums to thread h == 0
+        if (h > 0) {
+            float* x = xch + (size_t)(h - 1) * 6 * MD_TB;
+            x[tp] = a.fx; x[MD_TB + tp] = a.fy; x[2 * MD_TB + tp] = a.fz; x[3 * MD_TB + tp] = pe2;
+            x[4 * MD_TB + tp] = nin; x[5 * MD_TB + tp] = a.band;
         }
         __syncthreads();
-        if (h == 1) return;
-        a.fx += xch[tp]; a.fy += xch[MD_TB + tp]; a.fz += xch[2 * MD_TB + tp]; pe2 += xch[3 * MD_TB + tp];
-        nin += xch[4 * MD_TB + tp]; a.band = fminf(a.band, xch[5 * MD_TB + tp]);
+        if (h > 0) return;
+#pragma unroll
+        for (int k = 0; k < NS - 1; ++k) {                 // fixed order: run-to-run reproducible
+            const float* x = xch + (size_t)k * 6 * MD_TB;
+            a.fx += x[tp]; a.fy += x[MD_TB + tp]; a.fz += x[2 * MD_TB + tp]; pe2 += x[3 * MD_TB + tp];
+            nin += x[4 * MD_TB + tp]; a.band = fminf(a.band, x[5 * MD_TB + tp]);
+        }
     }
     if (!live) return;
     if (UNIT) {   // back from reduced units: F = 24 eps A, V = 4 eps sum (s^6 - s^3) - V_c nin
@@ -974,7 +979,7 @@ __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuff
 }
 
 template <int NS>
-__global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : 2) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries,
+__global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries,
                                                                                   const float4* __restrict__ pos,
                                                                                   float4* __restrict__ force) {
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -996,7 +1001,7 @@ __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : 2) k_vertex_lj_stage
         return;
     }
     const Stage st = stage_issue<false>(P, B, bi, b, stage_entries, pre, pos, nullptr, smraw);
-    float* xch = reinterpret_cast<float*>(st.spos + stage_entries);     // [6][MD_TB] floats, NS == 2 only
+    float* xch = reinterpret_cast<float*>(st.spos + stage_entries);     // [NS - 1][6][MD_TB] floats, NS > 1 only
     stage_wait(P, bi, st, smraw);
     if (NS == 1 && !live) return;
     const bool bonds = P.kind == MD_POT_FENE_WCA;
@@ -1093,6 +1098,13 @@ static void staged_attrs_once() {
     done = true;
     cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
     cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    // the neighbourhoods live in shared memory and the rows bypass L1: ask for the largest shared-memory carveout so that
+    // as many blocks as the sizing in sync_and_check counted on are resident
+    cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_patchy_staged, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_patchy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
 }
 
@@ -1104,6 +1116,9 @@ bool md_launch_forces_staged(md_system* s) {
     const size_t smem = md_staged_smem_bytes(s, se);
     if (smem > 224 * 1024) return false;
     if (P.kind == MD_POT_PATCHY) k_vertex_patchy_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
+    else if (2 * (smem + 24 * MD_TB + 1024) > 227 * 1024 && smem + 72 * MD_TB <= 224 * 1024 && P.rcap >= 64)
+        // one block per SM: four threads per particle (1024-thread blocks, 32 warps on the SM)
+        k_vertex_lj_staged<4><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
     else if (smem > 75 * 1024 && smem + 24 * MD_TB <= 224 * 1024)   // <= 2 blocks per SM: two threads per particle
         k_vertex_lj_staged<2><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
     else k_vertex_lj_staged<1><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
