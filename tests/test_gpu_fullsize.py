@@ -22,7 +22,7 @@ def test_c2_full_size_parity(oracle):
     fmax = np.abs(o["F"]).max()
     tol = 1e-4 * fmax + 1e-6
     for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "red_v4"), ("edge", "warp"),
-                      ("edge", "segmented")]:
+                      ("edge", "segmented"), ("vertex_n3", 12)]:
         s.forces(strat, sc)
         F = s.in_id_order(s.force)
         assert np.abs(F[:, :3] - o["F"]).max() <= tol, (strat, sc)
@@ -35,6 +35,49 @@ def test_c2_full_size_parity(oracle):
     o = oracle.forces(pos, w.box, dict(w.potential))
     F = s.in_id_order(s.force)
     assert np.abs(F[:, :3] - o["F"]).max() <= 1e-4 * np.abs(o["F"]).max() + 1e-6
+    # the same in mixed precision: fp64 state through the device-side rebuilds, fp32 forces on its rounding
+    s.set_precision("mixed")
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    s.integrate(w.dt, 100, "vertex")
+    x64, _ = s.state_f64()
+    pos = s.in_id_order(s.pos)
+    assert np.array_equal(pos[:, :3], x64.astype(np.float32))
+    o = oracle.forces(pos, w.box, dict(w.potential))
+    F = s.in_id_order(s.force)
+    assert np.abs(F[:, :3] - o["F"]).max() <= 1e-4 * np.abs(o["F"]).max() + 1e-6
+    s.close()
+
+
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_c3_c4_full_size_parity(oracle, name):
+    """configs[2] (polymer melt, 4096 x 64 beads) and configs[3] (patchy rigid bodies, N = 2^18) at full size, every
+    particle compared: lattice / walk start, then the state after device-side rebuilds."""
+    from paper_1401_4350_b200 import MDSystem
+    w = W.config(name)
+    rigid = w.quat is not None
+    s = MDSystem.from_workload(w, order="hilbert")
+    s.build_cells(); s.build_verlet()
+    assert s.stats()["n_edges"] == oracle.pair_count(w.pos, w.box, w.rcut, w.skin)
+    o = oracle.forces(w.pos, w.box, dict(w.potential), quat=w.quat)
+    variants = [("vertex", "smem"), ("vertex", "l2"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented"), ("vertex_n3", 4)]
+    for strat, sc in variants:
+        s.forces(strat, sc)
+        F = s.in_id_order(s.force)
+        assert np.abs(F[:, :3] - o["F"]).max() <= 1e-4 * np.abs(o["F"]).max() + 1e-6, (strat, sc)
+        if rigid:
+            T = s.in_id_order(s.torque)
+            assert np.abs(T[:, :3] - o["T"]).max() <= 1e-4 * np.abs(o["T"]).max() + 1e-6, (strat, sc)
+    s.forces("vertex")
+    s.integrate(w.dt, 200, "vertex")
+    assert s.stats()["n_rebuilds"] >= 1
+    pos = s.in_id_order(s.pos)
+    quat = s.in_id_order(s.quat) if rigid else None
+    o = oracle.forces(pos, w.box, dict(w.potential), quat=quat)
+    F = s.in_id_order(s.force)
+    assert np.abs(F[:, :3] - o["F"]).max() <= 1e-4 * np.abs(o["F"]).max() + 1e-6
+    if rigid:
+        T = s.in_id_order(s.torque)
+        assert np.abs(T[:, :3] - o["T"]).max() <= 1e-4 * np.abs(o["T"]).max() + 1e-6
     s.close()
 
 
