@@ -17,6 +17,13 @@
  *   O5  Energies U, K_trans, K_rot.
  *   O6  velocity-Verlet NVE (BASELINE.json north_star "md_integrate velocity-Verlet").
  *   O7  rigid-body velocity-Verlet for a spherical top (S:O7).
+ *   O8  the paper's own patchy model (S:8(f2)): Eq. (3) core (sigma/r)^200 plus Eq. (4) patch-patch terms
+ *       -eps exp[-1/2 (r^{ij}/0.12 sigma)^n] over the M x M patch pairs, r^{ij} the distance between patch i of
+ *       particle 1 and patch j of particle 2.  Eq. (4) is garbled in PAPER.md (no minus sign, n undefined) and
+ *       the patch positions are not stated: reading S:Q1 (n = 10, patches on the surface at 0.5 sigma, antipodal
+ *       for M = 2, r_c = 0.18 sigma cuts r^{ij}).  PARITY UNPINNED for that reading (the cited sources are not in
+ *       the container); the arithmetic of the reading itself is pinned (closed forms, finite differences,
+ *       Newton-3 invariants).
  * Forces/torques/energies are the PLAIN DEFINITION: a direct sum over all pairs with d2 < rcut^2
  * (both strategies evaluate exactly the pairs of the Verlet list that are inside r_c).
  * The oracle's own cell list only prunes pairs that cannot be inside the cutoff; `use_cells=0`
@@ -29,7 +36,7 @@
  *
  * Parity pins (tests/test_oracle_pins.py): closed forms P1-P4, fcc lattice sums P5, brute force P6/P8,
  * Newton-3 invariants P7, finite-difference force/torque vs energy, NVE drift P9, free rotor P10,
- * Fig. 1 thread counts P12.  No function here is "parity unpinned".
+ * Fig. 1 thread counts P12.  Only O8 (patch_point_pair) is "parity unpinned" (see O8 above).
  */
 #include <math.h>
 #include <stdint.h>
@@ -39,7 +46,7 @@
 #include <omp.h>
 #endif
 
-enum { ORC_LJ = 0, ORC_FENE_WCA = 1, ORC_PATCHY = 2 };
+enum { ORC_LJ = 0, ORC_FENE_WCA = 1, ORC_PATCHY = 2, ORC_PATCHY_PP = 3 };
 
 typedef struct {
     int kind;
@@ -53,6 +60,11 @@ typedef struct {
     double eps_patch, patch_sigma_r, patch_sigma_ang;
     double rcut_core;     /* PATCHY: WCA core cut 2^(1/6) sigma */
     double inertia;
+    /* ORC_PATCHY_PP (O8, the paper's own patchy model, Eqs. (2)-(4) P:103-113, reading S:Q1) */
+    double patch_radius;  /* distance of a patch from the centre of its particle (0.5 sigma, S:Q1)            */
+    double patch_exponent;/* n of Eq. (4) (10, S:Q1)                                                          */
+    double core_exponent; /* 200 of Eq. (3)                                                                   */
+    double rcut_patch;    /* cut on the patch-patch distance r^{ij} (0.18 sigma); rcut = 2 patch_radius + rcut_patch */
 } orc_pot;
 
 int orc_num_threads(void) {
@@ -309,6 +321,49 @@ static double patch_pair(double d2, const double* rvec, const double* qi, const 
     return V;
 }
 
+/* O8, Eqs. (2)-(4) P:103-113 under reading S:Q1.  p_a = patch_radius * R_i dir_a, d = r_vec + p_b - p_a is the
+ * vector from patch a of i to patch b of j, u = |d|; a patch pair contributes only if u < rcut_patch:
+ *   term = -eps_patch exp(-g),  g = 1/2 (u / w)^n,   d term / d d_vec = -term n g d / u^2
+ * The force on j's patch is -d term/d d_vec, on i's patch +d term/d d_vec; torques are p x F. */
+static double patch_point_pair(double d2, const double* rvec, const double* qi, const double* qj, const orc_pot* p,
+                               double* dVdr, double* tau_i, double* tau_j) {
+    double Ri[3][3], Rj[3][3];
+    quat_to_R(qi, Ri);
+    quat_to_R(qj, Rj);
+    /* Eq. (3): V_CM = eps (sigma/r)^m, dV/dr_vec = -m V r_vec / r^2 */
+    double V = p->epsilon * pow(p->sigma * p->sigma / d2, 0.5 * p->core_exponent);
+    for (int k = 0; k < 3; ++k) dVdr[k] = -p->core_exponent * V / d2 * rvec[k];
+    tau_i[0] = tau_i[1] = tau_i[2] = 0.0;
+    tau_j[0] = tau_j[1] = tau_j[2] = 0.0;
+    for (int a = 0; a < p->n_patches; ++a) {
+        double pa[3];
+        for (int k = 0; k < 3; ++k)
+            pa[k] = p->patch_radius * (Ri[k][0] * p->patch_dir[a][0] + Ri[k][1] * p->patch_dir[a][1] + Ri[k][2] * p->patch_dir[a][2]);
+        for (int b = 0; b < p->n_patches; ++b) {
+            double pb[3], d[3];
+            for (int k = 0; k < 3; ++k)
+                pb[k] = p->patch_radius * (Rj[k][0] * p->patch_dir[b][0] + Rj[k][1] * p->patch_dir[b][1] + Rj[k][2] * p->patch_dir[b][2]);
+            for (int k = 0; k < 3; ++k) d[k] = (rvec[k] + pb[k]) - pa[k];
+            double u2 = (d[0] * d[0] + d[1] * d[1]) + d[2] * d[2];
+            if (!(u2 < p->rcut_patch * p->rcut_patch)) continue;
+            double u = sqrt(u2);
+            double g = 0.5 * pow(u / p->patch_sigma_r, p->patch_exponent);
+            double term = -p->eps_patch * exp(-g);                       /* Eq. (4), one (i, j) patch pair */
+            V += term;
+            if (u2 > 0.0) {
+                double c = -term * p->patch_exponent * g / u2;           /* d term / d d_vec = c d */
+                double gd[3] = { c * d[0], c * d[1], c * d[2] }, x[3];
+                for (int k = 0; k < 3; ++k) dVdr[k] += gd[k];
+                cross3(pa, gd, x);                                       /* force on i's patch = +gd */
+                for (int k = 0; k < 3; ++k) tau_i[k] += x[k];
+                cross3(pb, gd, x);                                       /* force on j's patch = -gd */
+                for (int k = 0; k < 3; ++k) tau_j[k] -= x[k];
+            }
+        }
+    }
+    return V;
+}
+
 /* One ordered pair (i <- j): energy V of the pair, gradient dV/dr_vec, torque on i.  Returns 1 if the pair
  * is inside the interaction cutoff (S:Q5: the "force can be non-zero" test is d2 < rcut^2, strict). */
 static int pair_eval(const orc_pot* p, double d2, const double* rvec, const double* qi, const double* qj,
@@ -323,6 +378,8 @@ static int pair_eval(const orc_pot* p, double d2, const double* rvec, const doub
     } else if (p->kind == ORC_FENE_WCA) {
         /* O2: rcut = 2^(1/6) sigma, shift = +eps */
         *V = lj_pair(d2, rvec, p->epsilon, p->sigma, p->rcut, 1, dVdr);
+    } else if (p->kind == ORC_PATCHY_PP) {
+        *V = patch_point_pair(d2, rvec, qi, qj, p, dVdr, tau_i, tau_j);   /* truncated, not shifted */
     } else {
         double g[3], t1[3], t2[3];
         *V = patch_pair(d2, rvec, qi, qj, p, dVdr, tau_i, tau_j);   /* truncated, not shifted (S:Q15) */

@@ -16,7 +16,7 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "md_oracle.c"
 _LIB = _HERE / "libmd_oracle.so"
 
-KINDS = {"lj": 0, "fene_wca": 1, "patchy": 2}
+KINDS = {"lj": 0, "fene_wca": 1, "patchy": 2, "patchy_pp": 3}
 
 
 class OrcPot(C.Structure):
@@ -32,6 +32,8 @@ class OrcPot(C.Structure):
         ("eps_patch", C.c_double), ("patch_sigma_r", C.c_double), ("patch_sigma_ang", C.c_double),
         ("rcut_core", C.c_double),
         ("inertia", C.c_double),
+        ("patch_radius", C.c_double), ("patch_exponent", C.c_double), ("core_exponent", C.c_double),
+        ("rcut_patch", C.c_double),
     ]
 
 
@@ -56,6 +58,10 @@ def make_pot(d: dict) -> OrcPot:
     p.patch_sigma_ang = d.get("patch_sigma_ang", 0.3)
     p.rcut_core = d.get("rcut_core", 2.0 ** (1.0 / 6.0))
     p.inertia = d.get("inertia", 0.1)
+    p.patch_radius = d.get("patch_radius", 0.5)
+    p.patch_exponent = d.get("patch_exponent", 10.0)
+    p.core_exponent = d.get("core_exponent", 200.0)
+    p.rcut_patch = d.get("rcut_patch", 0.18)
     return p
 
 

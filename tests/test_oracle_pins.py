@@ -435,3 +435,91 @@ def test_p10_free_rotor(oracle):
         want = qmul(dq, q0[i])
         got = out["quat"][i]
         assert min(np.abs(got - want).max(), np.abs(got + want).max()) < 1e-9
+
+
+# ------------------------------------------------------------------ O8: the paper's own patchy model (S:8(f2), reading Q1)
+PP = W.patchy_pp_potential()
+
+
+def test_o8_patchy_pp_closed_forms(oracle):
+    """Eqs. (3)-(4) P:103-113 for two particles on the x axis whose patches 0 face each other: the patch-patch distance
+    is r - 1, so V = r^-200 - exp[-1/2 ((r - 1)/0.12)^10] and the force is its radial derivative; with the patch axes
+    perpendicular to the bond every patch pair is beyond 0.18 sigma and only the core of Eq. (3) is left."""
+    qi = quat_from_to([0, 0, 1], [1, 0, 0])
+    qj = quat_from_to([0, 0, 1], [-1, 0, 0])
+    for r in (1.0, 1.03, 1.12, 1.17):
+        u = r - 1.0
+        g = 0.5 * (u / 0.12) ** 10
+        V_ref = r ** -200.0 - math.exp(-g)
+        dVdr = -200.0 * r ** -201.0 + (math.exp(-g) * 10.0 * g / u if u > 0 else 0.0)
+        inside, V, Fj, ti, tj = oracle.pair(PP, [r, 0, 0], qi, qj)
+        assert inside
+        assert abs(V - V_ref) < 1e-12 * max(1.0, abs(V_ref))
+        assert abs(Fj[0] + dVdr) < 1e-9 * max(1.0, abs(dVdr)) and abs(Fj[1]) < 1e-12 and abs(Fj[2]) < 1e-12
+        assert np.abs(ti).max() < 1e-12 and np.abs(tj).max() < 1e-12          # central geometry: no torque
+    assert abs((1.12 ** -200.0 - math.exp(-0.5)) - oracle.pair(PP, [1.12, 0, 0], qi, qj)[1]) < 1e-12   # u = w: g = 1/2
+    for r in (0.99, 1.05):
+        inside, V, Fj, ti, tj = oracle.pair(PP, [r, 0, 0], ID, ID)            # patch axes along z, bond along x
+        assert abs(V - r ** -200.0) < 1e-12 * r ** -200.0 and abs(Fj[0] - 200.0 * r ** -201.0) < 1e-9 * r ** -201.0 * 200
+        assert np.abs(ti).max() == 0.0 and np.abs(tj).max() == 0.0
+    assert not oracle.pair(PP, [1.18, 0, 0], qi, qj)[0]                       # strict centre cutoff 2 * 0.5 + 0.18
+    # a patch pair just outside 0.18 sigma contributes nothing (truncated, P:117): tilt i's patch away
+    tilt = quat_from_to([0, 0, 1], [math.cos(0.5), math.sin(0.5), 0.0])
+    _, V, _, _, _ = oracle.pair(PP, [1.1, 0, 0], tilt, qj)
+    pa = 0.5 * np.array([math.cos(0.5), math.sin(0.5), 0.0])
+    d = np.array([1.1, 0, 0]) + np.array([-0.5, 0, 0]) - pa
+    assert np.linalg.norm(d) > 0.18 and abs(V - 1.1 ** -200.0) < 1e-15
+
+
+def test_o8_patchy_pp_finite_differences(oracle):
+    """Force and both torques of O8 against central differences of its energy on bonded, tilted geometries, and the pair
+    invariant tau_i + tau_j + r_vec x F_j = 0 (a wrong sign, a swapped patch or a dropped term fails one of them)."""
+    rng = np.random.default_rng(8)
+    worst, bonded = 0.0, 0
+    for _ in range(200):
+        d = rng.normal(size=3)
+        d /= np.linalg.norm(d)
+        r = rng.uniform(1.0, 1.15)
+        def facing(target, patch):
+            t = target + 0.12 * rng.normal(size=3)
+            t /= np.linalg.norm(t)
+            return quat_from_to(W.PP_DIRS[patch], t)
+        qi, qj = facing(d, rng.integers(2)), facing(-d, rng.integers(2))
+        _, V, Fj, ti, tj = oracle.pair(PP, r * d, qi, qj)
+        bonded += V < r ** -200.0 - 1e-3
+        Fd, tid, tjd = _fd_pair(oracle, PP, r * d, qi, qj, h=1e-7)
+        scale = max(1.0, np.abs(Fj).max(), np.abs(ti).max(), np.abs(tj).max())
+        worst = max(worst, np.abs(Fj - Fd).max() / scale, np.abs(ti - tid).max() / scale, np.abs(tj - tjd).max() / scale)
+        assert np.abs(ti + tj + np.cross(r * d, Fj)).max() < 1e-10 * scale
+    assert bonded > 60            # the sample does exercise the patch term
+    assert worst < 5e-6
+
+
+def test_o8_patchy_pp_system(oracle):
+    """Whole periodic system of bonded dimers: cells vs brute force, zero net force, F_i = -dU/dx_i, tau_i = -dU/d(rot_i)."""
+    w = W.dimer_gas(108, "patchy_pp")
+    f = oracle.forces(w.pos, w.box, w.potential, w.quat)
+    fb = oracle.forces(w.pos, w.box, w.potential, w.quat, use_cells=False)
+    assert np.array_equal(f["F"], fb["F"]) or np.abs(f["F"] - fb["F"]).max() < 1e-10 * np.abs(f["F"]).max()
+    assert f["n_in_cut"] == fb["n_in_cut"] and (f["pe"] < -0.05).sum() > 40
+    assert np.abs(f["F"].sum(0)).max() < 1e-10 * np.abs(f["F"]).max()
+    x = w.pos[:, :3].astype(np.float64)
+    q = w.quat.astype(np.float64)
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    fd = oracle.forces_d(x, w.box, w.potential, q)
+    h = 1e-7
+    bonded = np.nonzero(fd["pe"] < -0.05)[0]
+    for i in bonded[:4]:
+        for k in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, k] += h
+            xm[i, k] -= h
+            g = -(_total_U(oracle, xp, w.box, w.potential, q) - _total_U(oracle, xm, w.box, w.potential, q)) / (2 * h)
+            assert abs(g - fd["F"][i, k]) < 5e-6 * max(1.0, np.abs(fd["F"]).max())
+            ax = np.zeros(3)
+            ax[k] = 1
+            qp, qm = q.copy(), q.copy()
+            qp[i] = qmul(np.array([math.cos(h / 2), *(math.sin(h / 2) * ax)]), q[i])
+            qm[i] = qmul(np.array([math.cos(h / 2), *(-math.sin(h / 2) * ax)]), q[i])
+            t = -(_total_U(oracle, x, w.box, w.potential, qp) - _total_U(oracle, x, w.box, w.potential, qm)) / (2 * h)
+            assert abs(t - fd["T"][i, k]) < 5e-6 * max(1.0, np.abs(fd["T"]).max())

@@ -167,6 +167,17 @@ def patchy_potential() -> dict:
                 eps_patch=5.0, patch_sigma_r=0.1, patch_sigma_ang=0.3, inertia=0.1)
 
 
+PP_DIRS = np.array([[0.0, 0.0, 1.0], [0.0, 0.0, -1.0]])
+
+
+def patchy_pp_potential() -> dict:
+    """The paper's own patchy model under reading Q1: (sigma/r)^200 core, M = 2 antipodal
+    patches at 0.5 sigma from the centre, -eps exp[-1/2 (r_pp / 0.12 sigma)^10] between patches closer than 0.18 sigma."""
+    return dict(kind="patchy_pp", epsilon=1.0, sigma=1.0, mass=1.0, shift_energy=0, rcut=1.18, rcut_core=1.18,
+                n_patches=2, patch_dir=PP_DIRS.copy(), eps_patch=1.0, patch_sigma_r=0.12, patch_sigma_ang=1.0,
+                inertia=0.1, patch_radius=0.5, patch_exponent=10.0, core_exponent=200.0, rcut_patch=0.18)
+
+
 def patchy_fluid(N: int = 2 ** 18, rho: float = 0.5, T: float = 0.15, skin: float = 0.3,
                  jitter: float = 0.05, seed: int = BASE_SEED + 4, dt: float = 0.002) -> Workload:
     pot = patchy_potential()
@@ -291,6 +302,8 @@ def dimer_gas(n_dimers: int = 4096, kind: str = "lj", seed: int = BASE_SEED + 6,
         pot["chain_len"] = 2
     elif kind == "patchy":
         pot, lo, hi = patchy_potential(), 0.90, 1.05 * 1.5
+    elif kind == "patchy_pp":
+        pot, lo, hi = patchy_pp_potential(), 1.00, 1.14      # contact to just past the 0.18 sigma patch range
     else:
         raise ValueError(kind)
     sep = lo + (hi - lo) * uniform01(seed, 1, n_dimers)
@@ -300,7 +313,7 @@ def dimer_gas(n_dimers: int = 4096, kind: str = "lj", seed: int = BASE_SEED + 6,
     x[1::2] = centres + 0.5 * sep[:, None] * dirs
     N = 2 * n_dimers
     quat = angmom = None
-    if kind == "patchy":
+    if kind in ("patchy", "patchy_pp"):
         q = normal(seed, 3, 4 * N).reshape(N, 4)
         q /= np.linalg.norm(q, axis=1, keepdims=True)
         # second half of the dimers: rotate each partner so that its patch 0 points within 30 deg
@@ -310,11 +323,11 @@ def dimer_gas(n_dimers: int = 4096, kind: str = "lj", seed: int = BASE_SEED + 6,
         tgt[0::2] = dirs
         tgt[1::2] = -dirs
         tilt = _unit_vectors(seed, 5, N)
-        ang = uniform01(seed, 6, N) * (math.pi / 6.0)
+        ang = uniform01(seed, 6, N) * (math.pi / 6.0 if kind == "patchy" else math.pi / 18.0)
         perp = tilt - (tilt * tgt).sum(1, keepdims=True) * tgt
         perp /= np.maximum(np.linalg.norm(perp, axis=1, keepdims=True), 1e-12)
         want = np.cos(ang)[:, None] * tgt + np.sin(ang)[:, None] * perp   # desired space-frame patch 0
-        b0 = TETRA[0]
+        b0 = TETRA[0] if kind == "patchy" else PP_DIRS[0]
         # shortest-arc quaternion taking b0 -> want
         c = np.cross(np.broadcast_to(b0, want.shape), want)
         w = 1.0 + (want * b0).sum(1)
