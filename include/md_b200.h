@@ -56,7 +56,7 @@ typedef enum {
     MD_ERR_NUMERIC = -5   /* FENE bond length >= R0                                          */
 } md_status;
 
-typedef enum { MD_POT_LJ = 0, MD_POT_FENE_WCA = 1, MD_POT_PATCHY = 2 } md_pot_kind;
+typedef enum { MD_POT_LJ = 0, MD_POT_FENE_WCA = 1, MD_POT_PATCHY = 2, MD_POT_PATCHY_PP = 3 } md_pot_kind;
 typedef enum {
     MD_VERTEX = 0,   /* one thread per particle, every pair evaluated twice, no atomics                        */
     MD_EDGE = 1,     /* one thread per pair of the Verlet list, scatter to both particles                      */
@@ -94,7 +94,13 @@ typedef enum { MD_PREC_F32 = 0, MD_PREC_MIXED = 1 } md_precision;
  *                    chain_len consecutive ids.
  *   MD_POT_PATCHY    B:10: WCA core cut at rcut_core plus n_patches x n_patches patch terms
  *                    -eps_patch exp(-(r-sigma)^2/(2 patch_sigma_r^2)) exp(-(1-cos th_i)/patch_sigma_ang^2)
- *                    exp(-(1-cos th_j)/patch_sigma_ang^2), truncated (not shifted) at rcut. */
+ *                    exp(-(1-cos th_j)/patch_sigma_ang^2), truncated (not shifted) at rcut.
+ *   MD_POT_PATCHY_PP the paper's own patchy model, Eqs. (2)-(4) P:103-113 (S:8(f2), reading S:Q1 -- Eq. (4) is garbled in
+ *                    the source, parity unpinned): V = epsilon (sigma/r)^core_exponent - eps_patch sum_a sum_b
+ *                    exp[-1/2 (r_ab / patch_sigma_r)^patch_exponent], r_ab = distance between patch a of i and patch b of
+ *                    j, patches at patch_radius * patch_dir from the centres, only patch pairs with r_ab < rcut_patch
+ *                    (P:117), truncated not shifted.  Both exponents even integers <= 400; rcut >= 2 patch_radius +
+ *                    rcut_patch; rcut_core and patch_sigma_ang are ignored but must be valid (> 0, rcut_core <= rcut). */
 typedef struct {
     int32_t kind; /* md_pot_kind */
     float epsilon, sigma, mass;
@@ -106,6 +112,7 @@ typedef struct {
     float eps_patch, patch_sigma_r, patch_sigma_ang;
     float rcut_core;
     float inertia; /* scalar moment of inertia of the spherical top (S:O7) */
+    float patch_radius, patch_exponent, core_exponent, rcut_patch; /* MD_POT_PATCHY_PP only */
 } md_potential;
 
 /* Bytes of device workspace md_create needs for these parameters.  host pointers. */

@@ -15,7 +15,7 @@ SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3}
 GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
 PRECISION = {"f32": 0, "mixed": 1}
-POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2}
+POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2, "patchy_pp": 3}
 STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPACITY", -4: "MD_ERR_CUDA",
           -5: "MD_ERR_NUMERIC"}
 
@@ -44,6 +44,8 @@ class MDPotential(C.Structure):
         ("eps_patch", C.c_float), ("patch_sigma_r", C.c_float), ("patch_sigma_ang", C.c_float),
         ("rcut_core", C.c_float),
         ("inertia", C.c_float),
+        ("patch_radius", C.c_float), ("patch_exponent", C.c_float), ("core_exponent", C.c_float),
+        ("rcut_patch", C.c_float),
     ]
 
 
@@ -67,6 +69,10 @@ def make_potential(d: dict) -> MDPotential:
     p.patch_sigma_ang = d.get("patch_sigma_ang", 0.3)
     p.rcut_core = d.get("rcut_core", 2.0 ** (1.0 / 6.0))
     p.inertia = d.get("inertia", 0.1)
+    p.patch_radius = d.get("patch_radius", 0.5)
+    p.patch_exponent = d.get("patch_exponent", 10.0)
+    p.core_exponent = d.get("core_exponent", 200.0)
+    p.rcut_patch = d.get("rcut_patch", 0.18)
     return p
 
 
@@ -156,7 +162,7 @@ class MDSystem:
         self.box = np.ascontiguousarray(box, dtype=np.float64)
         self.rcut, self.skin = float(rcut), float(skin)
         self.pot = make_potential(potential)
-        self.rigid = potential["kind"] == "patchy"
+        self.rigid = potential["kind"] in ("patchy", "patchy_pp")
         self.max_neigh = int(max_neigh)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         nbytes = C.c_size_t(0)

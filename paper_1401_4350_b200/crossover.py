@@ -23,7 +23,8 @@ if str(ROOT) not in sys.path:
 
 VERTEX = ["smem", "l2"]
 EDGE = ["red", "red_v4", "warp", "segmented"]
-FLOPS_PER_PAIR = {"lj": 39.0, "patchy": 235.0}          # SURVEY 8(d) algorithmic work table
+FLOPS_PER_PAIR = {"lj": 39.0, "patchy": 235.0,          # SURVEY 8(d) algorithmic work table
+                  "patchy_pp": 260.0}                   # the paper's own model: core + 4 patch pairs (this build's count)
 
 
 def time_calls(torch, fn, n):
@@ -94,13 +95,18 @@ def main():
             r = run_cell(torch, MDSystem, w, "patchy", args.evals, args.melt_steps, rho or 0.5)
             print(json.dumps(r), file=sys.stderr, flush=True)
             rows.append(r)
+        # the paper's own patchy model (S:8(f2), reading Q1; "mostly zero" interactions): bonded dimers on a lattice
+        w = W.dimer_gas(N // 2, "patchy_pp", spacing=2.6)
+        r = run_cell(torch, MDSystem, w, "patchy_pp", args.evals, 0, 2.0 / 2.6 ** 3)
+        print(json.dumps(r), file=sys.stderr, flush=True)
+        rows.append(r)
 
     cols = [f"vertex_{v}" for v in VERTEX] + [f"edge_{v}" for v in EDGE] + ["vertex_n3"]
     print("| potential | N | rho | r_c | entries/particle | E | " + " | ".join(c + " us" for c in cols) +
           " | t_VERTEX / t_EDGE (best of each) | x |")
     print("|" + "---|" * (8 + len(cols)))
     for r in rows:
-        print(f"| {r['kind']} | 2^{r['N'].bit_length() - 1} | {r['rho']} | {r['rcut']} | {r['entries_per_particle']:.1f} | {r['E']} | " +
+        print(f"| {r['kind']} | 2^{r['N'].bit_length() - 1} | {r['rho']:.3g} | {r['rcut']} | {r['entries_per_particle']:.1f} | {r['E']} | " +
               " | ".join(f"{r[c]:.1f}" for c in cols) +
               f" | {r['t_vertex_over_t_edge']:.2f} ({r['best_vertex']} / {r['best_edge']}) | {r['x']:.0f} |")
 

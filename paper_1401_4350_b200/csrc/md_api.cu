@@ -106,10 +106,16 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
 
 bool check_pot(const md_potential* p, double rcut) {
     if (!p) return false;
-    if (p->kind < MD_POT_LJ || p->kind > MD_POT_PATCHY) return false;
+    if (p->kind < MD_POT_LJ || p->kind > MD_POT_PATCHY_PP) return false;
     if (!(p->epsilon > 0) || !(p->sigma > 0) || !(p->mass > 0)) return false;
     if (p->kind == MD_POT_FENE_WCA && (p->chain_len < 1 || !(p->fene_K > 0) || !(p->fene_R0 > 0))) return false;
-    if (p->kind == MD_POT_PATCHY) {
+    if (p->kind == MD_POT_PATCHY_PP) {
+        const double ne = p->patch_exponent, ce = p->core_exponent;
+        if (!(p->patch_radius > 0) || !(p->rcut_patch > 0)) return false;
+        if (!(ne >= 2 && ne <= 400 && ne == 2 * floor(ne / 2)) || !(ce >= 2 && ce <= 400 && ce == 2 * floor(ce / 2))) return false;
+        if (rcut < (2.0 * p->patch_radius + p->rcut_patch) * (1.0 - 1e-6)) return false;   // a patch pair in range would be missed
+    }
+    if (p->kind == MD_POT_PATCHY || p->kind == MD_POT_PATCHY_PP) {
         if (p->n_patches < 1 || p->n_patches > MD_MAX_PATCH) return false;
         if (!(p->inertia > 0) || !(p->patch_sigma_r > 0) || !(p->patch_sigma_ang > 0) || !(p->rcut_core > 0)) return false;
         if (p->rcut_core > rcut) return false;
@@ -261,7 +267,7 @@ md_status md_workspace_bytes(int64_t N, const double box[3], double rcut, double
                              int32_t max_neigh, size_t* bytes) {
     Geometry g;
     if (!bytes || !box || !check_pot(pot, rcut) || !make_geometry(N, box, rcut, skin, max_neigh, &g)) return MD_ERR_INVALID;
-    *bytes = carve(nullptr, N, g, pot->kind == MD_POT_PATCHY, nullptr);
+    *bytes = carve(nullptr, N, g, pot->kind == MD_POT_PATCHY || pot->kind == MD_POT_PATCHY_PP, nullptr);
     return MD_OK;
 }
 
@@ -271,7 +277,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     *out = nullptr;
     Geometry g;
     if (!box || !check_pot(pot, rcut) || !make_geometry(N, box, rcut, skin, max_neigh, &g)) return MD_ERR_INVALID;
-    const bool rigid = pot->kind == MD_POT_PATCHY;
+    const bool rigid = pot->kind == MD_POT_PATCHY || pot->kind == MD_POT_PATCHY_PP;
     size_t need = carve(nullptr, N, g, rigid, nullptr);
     if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return MD_ERR_INVALID;
 
@@ -308,7 +314,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);
     s->stage_launch = P.stage_cap;
-    P.kind = pot->kind;
+    P.kind = rigid ? MD_POT_PATCHY : pot->kind;   // both rigid-body models run on the same kernels (P.pp_model tells them apart)
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
     P.sigma = pot->sigma;
     P.c48 = 48.0f * pot->epsilon; P.c24 = 24.0f * pot->epsilon; P.c4 = 4.0f * pot->epsilon;
@@ -321,7 +327,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
         double s2 = (double)pot->sigma * pot->sigma / (rcut * rcut), s6 = s2 * s2 * s2;
         double vc = 4.0 * pot->epsilon * s6 * (s6 - 1.0);
         bool shift = pot->shift_energy != 0 || pot->kind == MD_POT_FENE_WCA;   // WCA is always shifted (B:9)
-        P.vshift = (pot->kind == MD_POT_PATCHY || !shift) ? 0.0f : (float)vc;
+        P.vshift = (rigid || !shift) ? 0.0f : (float)vc;
     }
     P.k_nrc2 = make_float2(-P.rc2, -P.rc2); P.k_na = make_float2(-P.lj_a, -P.lj_a); P.k_b = make_float2(P.lj_b, P.lj_b);
     P.k_c = make_float2(P.lj_c, P.lj_c); P.k_nd = make_float2(-P.lj_d, -P.lj_d); P.k_nvs = make_float2(-P.vshift, -P.vshift);
@@ -338,6 +344,14 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
         P.inv_2sr2 = 0.5f * P.inv_sr2;
         P.inv_w2 = 1.0f / (pot->patch_sigma_ang * pot->patch_sigma_ang);
         P.inv_inertia = 1.0f / pot->inertia;
+        P.pp_model = pot->kind == MD_POT_PATCHY_PP ? 1 : 0;
+        if (P.pp_model) {
+            P.pp_core_half = (int)(pot->core_exponent / 2); P.pp_half_n = (int)(pot->patch_exponent / 2);
+            P.pp_core_n = pot->core_exponent; P.pp_n = pot->patch_exponent;
+            P.pp_radius = pot->patch_radius;
+            P.pp_inv_w2 = 1.0f / (pot->patch_sigma_r * pot->patch_sigma_r);
+            P.pp_rc2 = pot->rcut_patch * pot->rcut_patch;
+        }
     }
     if (pot->kind == MD_POT_FENE_WCA) {
         P.fene_K = pot->fene_K;

@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(128, 8) k_vertex_lj(DevParams P, DevBuffers B,
     force[i] = make_float4(a.fx, a.fy, a.fz, pe);
 }
 
-template <bool IMG>
+template <bool IMG, bool PP>
 __device__ __forceinline__ void vertex_patchy_visit(const DevParams& P, const float4* __restrict__ pos, const float4* __restrict__ quat,
                                                     float4 xi, const Rot& Ri, int j, float& fx, float& fy, float& fz, float& pe,
                                                     float& tx, float& ty, float& tz) {
@@ -170,14 +170,14 @@ __device__ __forceinline__ void vertex_patchy_visit(const DevParams& P, const fl
     if (in_cutoff(P, d2, xi, xj)) {
         float4 qj = ldg4(quat + j);
         float gx, gy, gz, V, a, b, c, u, v, w;
-        if (P.n_patches == 4) patchy_pair<false, 4>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, b, c, u, v, w);
-        else patchy_pair<false, 0>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, b, c, u, v, w);
+        rigid_pair<false, PP>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, b, c, u, v, w);
         fx -= gx; fy -= gy; fz -= gz;
         tx += a; ty += b; tz += c;
         pe += V;
     }
 }
 
+template <bool PP>
 __global__ void __launch_bounds__(128) k_vertex_patchy(DevParams P, DevBuffers B, const float4* __restrict__ pos,
                                                        const float4* __restrict__ quat, float4* __restrict__ force,
                                                        float4* __restrict__ torque) {
@@ -192,8 +192,8 @@ __global__ void __launch_bounds__(128) k_vertex_patchy(DevParams P, DevBuffers B
     const Rot Ri = quat_to_rot(qi);     // once per particle
     for (int k = 0; k < cnt; ++k) {
         int j = row[(k >> 2) * (MD_TILE * 4) + (k & 3)];
-        if (info.x >> 30) vertex_patchy_visit<true>(P, pos, quat, xi, Ri, j, fx, fy, fz, pe, tx, ty, tz);
-        else vertex_patchy_visit<false>(P, pos, quat, xi, Ri, j, fx, fy, fz, pe, tx, ty, tz);
+        if (info.x >> 30) vertex_patchy_visit<true, PP>(P, pos, quat, xi, Ri, j, fx, fy, fz, pe, tx, ty, tz);
+        else vertex_patchy_visit<false, PP>(P, pos, quat, xi, Ri, j, fx, fy, fz, pe, tx, ty, tz);
     }
     force[i] = make_float4(fx, fy, fz, 0.5f * pe);
     torque[i] = make_float4(tx, ty, tz, 0.f);
@@ -225,11 +225,10 @@ __device__ __forceinline__ bool edge_eval(const DevParams& P, const float4* __re
     }
     float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     if (!in_cutoff(P, d2, xi, xj)) return false;
-    if (KIND == MD_POT_PATCHY) {
+    if (md_is_rigid(KIND)) {
         float4 qi = ldg4(quat + i), qj = ldg4(quat + j);
         const Rot Ri = quat_to_rot(qi);
-        if (P.n_patches == 4) patchy_pair<true, 4>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
-        else patchy_pair<true, 0>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
+        rigid_pair<true, KIND == MD_POT_PATCHY_PP>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
     } else {
         float g;
         lj_pair(P, d2, g, V);
@@ -253,7 +252,7 @@ __global__ void __launch_bounds__(256) k_edge_red(DevParams P, DevBuffers B, con
         if (V4) {
             red_add_v4(force + ij.x, -fx, -fy, -fz, hV);
             red_add_v4(force + j, fx, fy, fz, hV);
-            if (KIND == MD_POT_PATCHY) {
+            if (md_is_rigid(KIND)) {
                 red_add_v4(torque + ij.x, tix, tiy, tiz, 0.f);
                 red_add_v4(torque + j, tjx, tjy, tjz, 0.f);
             }
@@ -262,7 +261,7 @@ __global__ void __launch_bounds__(256) k_edge_red(DevParams P, DevBuffers B, con
             float* fj = reinterpret_cast<float*>(force + j);
             red_add_f32(fi + 0, -fx); red_add_f32(fi + 1, -fy); red_add_f32(fi + 2, -fz); red_add_f32(fi + 3, hV);
             red_add_f32(fj + 0, fx);  red_add_f32(fj + 1, fy);  red_add_f32(fj + 2, fz);  red_add_f32(fj + 3, hV);
-            if (KIND == MD_POT_PATCHY) {
+            if (md_is_rigid(KIND)) {
                 float* ti = reinterpret_cast<float*>(torque + ij.x);
                 float* tj = reinterpret_cast<float*>(torque + j);
                 red_add_f32(ti + 0, tix); red_add_f32(ti + 1, tiy); red_add_f32(ti + 2, tiz);
@@ -297,7 +296,7 @@ __global__ void __launch_bounds__(256) k_edge_warp(DevParams P, DevBuffers B, co
             const float hV = 0.5f * V;
             ax -= fx; ay -= fy; az -= fz; ape += hV;
             red_add_v4(force + j, fx, fy, fz, hV);
-            if (KIND == MD_POT_PATCHY) {
+            if (md_is_rigid(KIND)) {
                 atx += tix; aty += tiy; atz += tiz;
                 red_add_v4(torque + j, tjx, tjy, tjz, 0.f);
             }
@@ -309,7 +308,7 @@ __global__ void __launch_bounds__(256) k_edge_warp(DevParams P, DevBuffers B, co
             ay += __shfl_xor_sync(0xffffffffu, ay, o);
             az += __shfl_xor_sync(0xffffffffu, az, o);
             ape += __shfl_xor_sync(0xffffffffu, ape, o);
-            if (KIND == MD_POT_PATCHY) {
+            if (md_is_rigid(KIND)) {
                 atx += __shfl_xor_sync(0xffffffffu, atx, o);
                 aty += __shfl_xor_sync(0xffffffffu, aty, o);
                 atz += __shfl_xor_sync(0xffffffffu, atz, o);
@@ -317,7 +316,7 @@ __global__ void __launch_bounds__(256) k_edge_warp(DevParams P, DevBuffers B, co
         }
         if (sl == 0 && e1 > e0) {   // one reduction per owning particle
             red_add_v4(force + i, ax, ay, az, ape);
-            if (KIND == MD_POT_PATCHY) red_add_v4(torque + i, atx, aty, atz, 0.f);
+            if (md_is_rigid(KIND)) red_add_v4(torque + i, atx, aty, atz, 0.f);
         }
     }
 }
@@ -335,7 +334,7 @@ __global__ void __launch_bounds__(256) k_edge_store(DevParams P, DevBuffers B, c
             fx = fy = fz = V = 0.f; tix = tiy = tiz = tjx = tjy = tjz = 0.f;
         }
         B.edge_f[e] = make_float4(fx, fy, fz, V);
-        if (KIND == MD_POT_PATCHY) {
+        if (md_is_rigid(KIND)) {
             B.edge_ti[e] = make_float4(tix, tiy, tiz, 0.f);
             B.edge_tj[e] = make_float4(tjx, tjy, tjz, 0.f);
         }
@@ -350,16 +349,16 @@ __global__ void __launch_bounds__(128) k_edge_segsum(DevParams P, DevBuffers B, 
     for (unsigned int e = B.edge_off[p]; e < B.edge_off[p + 1]; ++e) {   // p is the first member: F_i = -F_j
         float4 f = B.edge_f[e];
         fx -= f.x; fy -= f.y; fz -= f.z; pe += f.w;
-        if (KIND == MD_POT_PATCHY) { float4 t = B.edge_ti[e]; tx += t.x; ty += t.y; tz += t.z; }
+        if (md_is_rigid(KIND)) { float4 t = B.edge_ti[e]; tx += t.x; ty += t.y; tz += t.z; }
     }
     for (unsigned int t = B.in_off[p]; t < B.in_off[p + 1]; ++t) {       // p is the second member
         unsigned int e = B.in_edge[t];
         float4 f = B.edge_f[e];
         fx += f.x; fy += f.y; fz += f.z; pe += f.w;
-        if (KIND == MD_POT_PATCHY) { float4 q = B.edge_tj[e]; tx += q.x; ty += q.y; tz += q.z; }
+        if (md_is_rigid(KIND)) { float4 q = B.edge_tj[e]; tx += q.x; ty += q.y; tz += q.z; }
     }
     force[p] = make_float4(fx, fy, fz, 0.5f * pe);
-    if (KIND == MD_POT_PATCHY) torque[p] = make_float4(tx, ty, tz, 0.f);
+    if (md_is_rigid(KIND)) torque[p] = make_float4(tx, ty, tz, 0.f);
 }
 
 // S:A8 bonded pass for EDGE (C3): one thread per static bond (id, id+1), FENE only, scatter with red.v4
@@ -392,7 +391,7 @@ __global__ void __launch_bounds__(128) k_vertex_n3(DevParams P, DevBuffers B, co
     if (i >= P.N) return;
     const size_t plane = (size_t)(i % m) * (size_t)P.N;
     float4* fc = fcopy + plane;
-    float4* tc = KIND == MD_POT_PATCHY ? tcopy + plane : nullptr;
+    float4* tc = md_is_rigid(KIND) ? tcopy + plane : nullptr;
     const unsigned int e0 = B.edge_off[i], e1 = B.edge_off[i + 1];
     float ax = 0.f, ay = 0.f, az = 0.f, ape = 0.f, atx = 0.f, aty = 0.f, atz = 0.f;
     for (unsigned int e = e0; e < e1; ++e) {
@@ -403,13 +402,13 @@ __global__ void __launch_bounds__(128) k_vertex_n3(DevParams P, DevBuffers B, co
         const float hV = 0.5f * V;
         ax -= fx; ay -= fy; az -= fz; ape += hV;
         red_add_v4(fc + j, fx, fy, fz, hV);
-        if (KIND == MD_POT_PATCHY) {
+        if (md_is_rigid(KIND)) {
             atx += tix; aty += tiy; atz += tiz;
             red_add_v4(tc + j, tjx, tjy, tjz, 0.f);
         }
     }
     force[i] = make_float4(ax, ay, az, ape);
-    if (KIND == MD_POT_PATCHY) torque[i] = make_float4(atx, aty, atz, 0.f);
+    if (md_is_rigid(KIND)) torque[i] = make_float4(atx, aty, atz, 0.f);
 }
 
 // "then the vectors are combined to obtain the total force acting on each particle": copies added in index order
@@ -436,9 +435,9 @@ __global__ void __launch_bounds__(256) k_n3_combine(DevParams P, float4* __restr
 template <int KIND>
 static void launch_vertex_n3(md_system* s, int m) {
     const DevParams& P = s->P;
-    float4* tq = KIND == MD_POT_PATCHY ? s->torque : nullptr;
+    float4* tq = md_is_rigid(KIND) ? s->torque : nullptr;
     float4* fcopy = s->B.edge_f;                                   // the per-edge scratch of the segmented variant
-    float4* tcopy = KIND == MD_POT_PATCHY ? s->B.edge_tj : nullptr;
+    float4* tcopy = md_is_rigid(KIND) ? s->B.edge_tj : nullptr;
     cudaMemsetAsync(fcopy, 0, 16 * (size_t)m * P.N, s->stream);
     if (tcopy) cudaMemsetAsync(tcopy, 0, 16 * (size_t)m * P.N, s->stream);
     k_vertex_n3<KIND><<<cdiv(P.N, 128), 128, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq, fcopy, tcopy, m);
@@ -458,7 +457,7 @@ static void launch_edge(md_system* s, int scatter) {
     const DevParams& P = s->P;
     const int nbN = cdiv(P.N, 256);
     const int persistent = 148 * 8;   // 8 CTAs of 256 threads per SM, grid-stride over the device-resident edge count
-    float4* tq = KIND == MD_POT_PATCHY ? s->torque : nullptr;
+    float4* tq = md_is_rigid(KIND) ? s->torque : nullptr;
     if (scatter == MD_SCATTER_SEGMENTED) {
         k_edge_store<KIND><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat);
         k_edge_segsum<KIND><<<cdiv(P.N, 128), 128, 0, s->stream>>>(P, s->B, s->force, tq);
@@ -481,16 +480,19 @@ void md_launch_forces(md_system* s, int strategy, int scatter) {
     const DevParams& P = s->P;
     if (strategy == MD_VERTEX) {
         int nb = cdiv((int64_t)P.ntiles * MD_TILE, 128);
-        if (P.kind == MD_POT_PATCHY) k_vertex_patchy<<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, s->torque);
+        if (P.kind == MD_POT_PATCHY && P.pp_model) k_vertex_patchy<true><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, s->torque);
+        else if (P.kind == MD_POT_PATCHY) k_vertex_patchy<false><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, s->torque);
         else if (P.kind == MD_POT_FENE_WCA) k_vertex_lj<true><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->force);
         else k_vertex_lj<false><<<nb, 128, 0, s->stream>>>(P, s->B, s->pos, s->force);
         s->launches += 1;
     } else if (strategy == MD_VERTEX_N3) {
         const int m = scatter == 0 ? 12 : scatter;
-        if (P.kind == MD_POT_PATCHY) launch_vertex_n3<MD_POT_PATCHY>(s, m);
+        if (P.kind == MD_POT_PATCHY && P.pp_model) launch_vertex_n3<MD_POT_PATCHY_PP>(s, m);
+        else if (P.kind == MD_POT_PATCHY) launch_vertex_n3<MD_POT_PATCHY>(s, m);
         else launch_vertex_n3<MD_POT_LJ>(s, m);
     } else {
-        if (P.kind == MD_POT_PATCHY) launch_edge<MD_POT_PATCHY>(s, scatter);
+        if (P.kind == MD_POT_PATCHY && P.pp_model) launch_edge<MD_POT_PATCHY_PP>(s, scatter);
+        else if (P.kind == MD_POT_PATCHY) launch_edge<MD_POT_PATCHY>(s, scatter);
         else launch_edge<MD_POT_LJ>(s, scatter);
     }
 }

@@ -79,6 +79,9 @@ struct DevParams {
     int n_patches;
     float pdir[MD_MAX_PATCH][3];
     float eps_patch, inv_2sr2, inv_sr2, inv_w2, sigma, inv_inertia;
+    // MD_POT_PATCHY_PP (the paper's own patchy model, S:8(f2)): runs on the rigid-body kernels with kind == MD_POT_PATCHY
+    int pp_model, pp_core_half, pp_half_n;   // flag; core_exponent / 2; patch_exponent / 2
+    float pp_radius, pp_inv_w2, pp_rc2, pp_core_n, pp_n;
 };
 
 // All device pointers carved from the caller's workspace.

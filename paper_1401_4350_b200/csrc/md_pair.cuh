@@ -106,6 +106,57 @@ __device__ __forceinline__ void patch_factor(const DevParams& P, const Rot& R, f
     Sz = P.inv_w2 * (R.m[2][0] * bx + R.m[2][1] * by + R.m[2][2] * bz);
 }
 
+// x^n for a small runtime integer n >= 1 by squaring (the paper's exponents: 100 = 200/2 and 5 = 10/2)
+__device__ __forceinline__ float ipow(float x, int n) {
+    float r = 1.0f;
+    while (n) {
+        if (n & 1) r *= x;
+        x *= x;
+        n >>= 1;
+    }
+    return r;
+}
+
+// The paper's own patchy model, Eqs. (2)-(4) P:103-113 under reading S:Q1 (S:8(f2)): core eps (sigma/r)^m plus, for every
+// patch pair (a of i, b of j) closer than rcut_patch, -eps_p exp[-1/2 (r_ab / w)^n] with r_ab the patch-patch distance,
+// patches at pp_radius * R dir from the centres.  With e = d + p_b - p_a, u2 = |e|^2, g = 1/2 (u2 / w^2)^(n/2):
+//   term = -eps_p exp(-g),  d term / d e = c e,  c = -term n g / u2;  F_j = -sum c e,  tau_i = sum p_a x (c e),  tau_j = -sum p_b x (c e)
+template <bool NEED_TJ>
+__device__ __forceinline__ void patchy_pp_pair(const DevParams& P, float dx, float dy, float dz, float d2, const Rot& Ri, float4 qj,
+                                               float& fx, float& fy, float& fz, float& V,
+                                               float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
+    const Rot Rj = quat_to_rot(qj);
+    const float inv = 1.0f / d2;
+    V = P.eps * ipow(P.sig2 * inv, P.pp_core_half);          // Eq. (3)
+    const float gc = P.pp_core_n * V * inv;                   // F_j = -dV/dr_vec = m V r_vec / r^2
+    fx = gc * dx; fy = gc * dy; fz = gc * dz;
+    tix = tiy = tiz = 0.f;
+    tjx = tjy = tjz = 0.f;
+    for (int a = 0; a < P.n_patches; ++a) {
+        const float pax = P.pp_radius * (Ri.m[0][0] * P.pdir[a][0] + Ri.m[0][1] * P.pdir[a][1] + Ri.m[0][2] * P.pdir[a][2]);
+        const float pay = P.pp_radius * (Ri.m[1][0] * P.pdir[a][0] + Ri.m[1][1] * P.pdir[a][1] + Ri.m[1][2] * P.pdir[a][2]);
+        const float paz = P.pp_radius * (Ri.m[2][0] * P.pdir[a][0] + Ri.m[2][1] * P.pdir[a][1] + Ri.m[2][2] * P.pdir[a][2]);
+        for (int b = 0; b < P.n_patches; ++b) {
+            const float pbx = P.pp_radius * (Rj.m[0][0] * P.pdir[b][0] + Rj.m[0][1] * P.pdir[b][1] + Rj.m[0][2] * P.pdir[b][2]);
+            const float pby = P.pp_radius * (Rj.m[1][0] * P.pdir[b][0] + Rj.m[1][1] * P.pdir[b][1] + Rj.m[1][2] * P.pdir[b][2]);
+            const float pbz = P.pp_radius * (Rj.m[2][0] * P.pdir[b][0] + Rj.m[2][1] * P.pdir[b][1] + Rj.m[2][2] * P.pdir[b][2]);
+            const float ex = (dx + pbx) - pax, ey = (dy + pby) - pay, ez = (dz + pbz) - paz;
+            const float u2 = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
+            if (!(u2 < P.pp_rc2)) continue;                   // only patch pairs closer than 0.18 sigma
+            const float g = 0.5f * ipow(u2 * P.pp_inv_w2, P.pp_half_n);
+            const float term = -P.eps_patch * ex2_approx(-g * 1.4426950408889634f);   // Eq. (4), one patch pair
+            V += term;
+            if (u2 > 0.0f) {
+                const float c = -term * P.pp_n * g / u2;
+                const float gx = c * ex, gy = c * ey, gz = c * ez;
+                fx -= gx; fy -= gy; fz -= gz;
+                tix += pay * gz - paz * gy; tiy += paz * gx - pax * gz; tiz += pax * gy - pay * gx;
+                if (NEED_TJ) { tjx -= pby * gz - pbz * gy; tjy -= pbz * gx - pbx * gz; tjz -= pbx * gy - pby * gx; }
+            }
+        }
+    }
+}
+
 // O4 (B:10): WCA core + patch term.  Outputs force on j (fx,fy,fz), V, torque on i, torque on j.
 // Ri = rotation matrix of particle i (callers that keep i fixed over a loop compute it once).
 template <bool NEED_TJ, int NP>
@@ -147,6 +198,17 @@ __device__ __forceinline__ void patchy_pair(const DevParams& P, float dx, float 
         V += fmaf(s6, fmaf(P.c4, s6, -P.c4), -P.core_vshift);
         fx = fmaf(g, dx, fx); fy = fmaf(g, dy, fy); fz = fmaf(g, dz, fz);
     }
+}
+
+// the rigid-body pair function a kernel instance is compiled for: PP = the paper's own model (S:8(f2)), else config 4's
+__host__ __device__ constexpr bool md_is_rigid(int kind) { return kind == MD_POT_PATCHY || kind == MD_POT_PATCHY_PP; }
+template <bool NEED_TJ, bool PP>
+__device__ __forceinline__ void rigid_pair(const DevParams& P, float dx, float dy, float dz, float d2, const Rot& Ri, float4 qj,
+                                           float& fx, float& fy, float& fz, float& V,
+                                           float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
+    if (PP) patchy_pp_pair<NEED_TJ>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
+    else if (P.n_patches == 4) patchy_pair<NEED_TJ, 4>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
+    else patchy_pair<NEED_TJ, 0>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
 }
 
 // O3 FENE (B:9): U = -1/2 K R0^2 ln(1 - d2/R0^2); force on j = -K d / (1 - d2/R0^2)

@@ -1021,7 +1021,7 @@ __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k
 // ------------------------------------------------------------------------------------------------
 // VERTEX, patchy rigid bodies, staged: positions and quaternions of the neighbourhood in shared memory
 // ------------------------------------------------------------------------------------------------
-template <bool IMG>
+template <bool IMG, bool PP>
 __device__ __forceinline__ void patchy_visit_s(const DevParams& P, const Stage& st, float4 xi, const Rot& Ri, unsigned int t,
                                                float& fx, float& fy, float& fz, float& pe, float& tx, float& ty, float& tz) {
     const float4 xj = st.spos[t];
@@ -1035,15 +1035,14 @@ __device__ __forceinline__ void patchy_visit_s(const DevParams& P, const Stage& 
     if (in_cutoff(P, d2, xi, xj)) {
         const float4 qj = st.squat[t];
         float gx, gy, gz, V, a, bb, c, u, v, w;
-        if (P.n_patches == 4) patchy_pair<false, 4>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, bb, c, u, v, w);
-        else patchy_pair<false, 0>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, bb, c, u, v, w);
+        rigid_pair<false, PP>(P, dx, dy, dz, d2, Ri, qj, gx, gy, gz, V, a, bb, c, u, v, w);
         fx -= gx; fy -= gy; fz -= gz;
         tx += a; ty += bb; tz += c;
         pe += V;
     }
 }
 
-template <bool IMG>
+template <bool IMG, bool PP>
 __device__ __forceinline__ void vertex_patchy_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int b,
                                                    float4* __restrict__ force, float4* __restrict__ torque) {
     const int tid = threadIdx.x;
@@ -1059,15 +1058,16 @@ __device__ __forceinline__ void vertex_patchy_rows(const DevParams& P, const Dev
     const Rot Ri = quat_to_rot(qi);     // once per particle
     for (int c = 0; c < nch; ++c) {
         const uint2 cur = __ldg(rowb + (size_t)c * MD_TB);     // padding entries = dummy (far away -> outside the cutoff)
-        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.x & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
-        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.x >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
-        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.y & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
-        patchy_visit_s<IMG>(P, st, xi, Ri, (cur.y >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG, PP>(P, st, xi, Ri, (cur.x & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG, PP>(P, st, xi, Ri, (cur.x >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG, PP>(P, st, xi, Ri, (cur.y & 0xffffu) >> sh, fx, fy, fz, pe, tx, ty, tz);
+        patchy_visit_s<IMG, PP>(P, st, xi, Ri, (cur.y >> 16) >> sh, fx, fy, fz, pe, tx, ty, tz);
     }
     force[i] = make_float4(fx, fy, fz, 0.5f * pe);
     torque[i] = make_float4(tx, ty, tz, 0.f);
 }
 
+template <bool PP>
 __global__ void __launch_bounds__(MD_TB) k_vertex_patchy_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
                                                                 const float4* __restrict__ quat, float4* __restrict__ force,
                                                                 float4* __restrict__ torque) {
@@ -1081,8 +1081,8 @@ __global__ void __launch_bounds__(MD_TB) k_vertex_patchy_staged(DevParams P, Dev
     const SegPre pre = seg_preload(B, b);
     const Stage st = stage_issue<true>(P, B, bi, b, stage_entries, pre, pos, quat, smraw);
     stage_wait(P, bi, st, smraw);
-    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_patchy_rows<true>(P, B, bi, st, b, force, torque);
-    else vertex_patchy_rows<false>(P, B, bi, st, b, force, torque);
+    if ((bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK)) vertex_patchy_rows<true, PP>(P, B, bi, st, b, force, torque);
+    else vertex_patchy_rows<false, PP>(P, B, bi, st, b, force, torque);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1104,8 +1104,10 @@ static void staged_attrs_once() {
     cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    cudaFuncSetAttribute(k_vertex_patchy_staged, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    cudaFuncSetAttribute(k_vertex_patchy_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaFuncSetAttribute(k_vertex_patchy_staged<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_patchy_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_patchy_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaFuncSetAttribute(k_vertex_patchy_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
 }
 
 // VERTEX on the staged rows.  Returns false if the neighbourhood does not fit in shared memory.
@@ -1115,7 +1117,8 @@ bool md_launch_forces_staged(md_system* s) {
     const int se = s->stage_launch;
     const size_t smem = md_staged_smem_bytes(s, se);
     if (smem > 224 * 1024) return false;
-    if (P.kind == MD_POT_PATCHY) k_vertex_patchy_staged<<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
+    if (P.kind == MD_POT_PATCHY && P.pp_model) k_vertex_patchy_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
+    else if (P.kind == MD_POT_PATCHY) k_vertex_patchy_staged<false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
     else if (2 * (smem + 24 * MD_TB + 1024) > 227 * 1024 && smem + 72 * MD_TB <= 224 * 1024 && P.rcap >= 64)
         // one block per SM: four threads per particle (1024-thread blocks, 32 warps on the SM)
         k_vertex_lj_staged<4><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);

@@ -67,6 +67,7 @@ CASES = {
     "dimers_lj_ragged_N": lambda: W.dimer_gas(1001, "lj"),
     "dimers_fene": lambda: W.dimer_gas(4096, "fene_wca"),
     "dimers_patchy": lambda: W.dimer_gas(4096, "patchy"),
+    "dimers_patchy_pp_paper_model": lambda: W.dimer_gas(4096, "patchy_pp"),   # S:8(f2), Eqs. (2)-(4) under reading Q1
     "polymer_64x64": lambda: W.polymer_melt(64, 64),
     "patchy4096": lambda: W.patchy_fluid(2 ** 12),
     "tiny_16": lambda: W.dimer_gas(8, "lj"),
@@ -288,7 +289,7 @@ def test_crossover_sweep_runs(capsys, monkeypatch):
     monkeypatch.setattr(sys, "argv", ["crossover", "--min-log2n", "12", "--max-log2n", "12", "--evals", "2", "--rcuts", "2.5"])
     crossover.main()
     out = capsys.readouterr().out
-    assert "| lj | 2^12 | 0.8 | 2.5 |" in out and "| patchy | 2^12 | 0.5 | 1.5 |" in out
+    assert "| lj | 2^12 | 0.8 | 2.5 |" in out and "| patchy | 2^12 | 0.5 | 1.5 |" in out and "| patchy_pp | 2^12 |" in out
 
 
 # ---- mixed precision (S:8(f3)): fp64 integration of the state, fp32 forces ----
@@ -390,3 +391,26 @@ def test_precision_errors(MD):
         s.state_f64()                          # default precision: no fp64 state
     assert e.value.code == -2
     s.close()
+
+
+def test_patchy_pp_short_trajectory(MD, oracle):
+    """The paper's own patchy model (S:8(f2)): bonded dimers released from rest, 100 rigid-body steps.  With a
+    (sigma/r)^200 core a force follows a position error 200-fold, so the forces are compared on the positions and
+    orientations the GPU holds (plain definition), the trajectory itself through positions and the conserved energy."""
+    w = W.dimer_gas(512, "patchy_pp")
+    o = oracle.integrate(w.pos, w.vel, w.box, dict(w.potential), w.skin, w.dt, 100, every=100, quat=w.quat, angmom=w.angmom)
+    for strat, sc in (("vertex", "smem"), ("vertex", "l2"), ("edge", "red_v4"), ("edge", "segmented"), ("vertex_n3", 4)):
+        s = MD.from_workload(w, order="hilbert")
+        s.build_cells(); s.build_verlet(); s.forces(strat, sc)
+        e0 = sum(s.energy())
+        s.integrate(w.dt, 100, strat, sc)
+        pos, quat = s.in_id_order(s.pos), s.in_id_order(s.quat)
+        snap = oracle.forces(pos, w.box, dict(w.potential), quat=quat)
+        assert_forces(s, snap, True)
+        dx = pos[:, :3].astype(np.float64) - o["pos"][:, :3]
+        dx -= w.box * np.round(dx / w.box)
+        assert np.abs(dx).max() < 1e-4
+        e1 = sum(s.energy())                                  # U on these positions was compared inside assert_forces
+        assert abs(e1 - e0) <= 2e-3 * abs(e0)                 # conserved along the stiff trajectory (dt = 0.002)
+        assert abs(o["energies"][-1].sum() - o["e0"].sum()) <= 2e-3 * abs(o["e0"].sum())
+        s.close()
