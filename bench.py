@@ -245,7 +245,9 @@ def main():
     s = MDSystem.from_workload(w, device=str(dev), order=args.order)
     s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
     if args.melt_steps > 0:                       # untimed setup: melt the lattice (paper: thermalised states)
-        s.integrate(w.dt, args.melt_steps, args.strategy, args.scatter)
+        for k in range(0, args.melt_steps, 100):  # md_stats between chunks lets the staged launch capacity follow the melt
+            s.integrate(w.dt, min(100, args.melt_steps - k), args.strategy, args.scatter)
+            s.stats()
     s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
     st0 = s.stats()
     E, N = st0["n_edges"], w.N

@@ -43,8 +43,10 @@ def time_calls(torch, fn, n):
 def run_cell(torch, MDSystem, w, kind, evals, melt, rho):
     s = MDSystem.from_workload(w, device="cuda:0", order="hilbert")
     s.build_cells(); s.build_verlet(); s.forces("vertex", "smem")
+    for k in range(0, melt, 100):                          # md_stats between chunks: the staged launch capacity follows
+        s.integrate(w.dt, min(100, melt - k), "vertex", "smem")   # the neighbourhoods while the lattice melts
+        s.stats()
     if melt > 0:
-        s.integrate(w.dt, melt, "vertex", "smem")
         s.build_cells(); s.build_verlet()
     st = s.stats()
     E, nfull = st["n_edges"], st["n_full_entries"]

@@ -234,8 +234,10 @@ md_status sync_and_check(md_system* s, const char* where) {
         // size the staged force launches from the largest neighbourhood seen, with 15 % head room for the
         // device-side rebuilds that happen before the next synchronising call; if that head room alone costs a
         // resident block per SM, keep only as much of it as still fits the block count of a tight (4 %) fit
-        int want = (int)(c.max_stage * 1.15) + 64;
+        // (30 % for systems of fewer blocks than SMs: their maximum fluctuates more and occupancy does not matter there)
+        int want = (int)(c.max_stage * (s->P.nblk >= 148 ? 1.15 : 1.30)) + 64;
         want = (want + 63) / 64 * 64;
+        want = std::min(want, ((int)s->N + 1 + 63) / 64 * 64);   // a neighbourhood never holds more than the whole system
         const size_t per_entry = s->rigid ? 32 : 16, sm_bytes = 228 * 1024, xch = s->rigid ? 0 : 24 * MD_TB;
         auto per_block = [&](int se) {
             size_t b = 16 + per_entry * (size_t)se;
@@ -244,7 +246,15 @@ md_status sync_and_check(md_system* s, const char* where) {
         };
         const int tight = ((int)(c.max_stage * 1.04) + 32 + 63) / 64 * 64;
         const int nb_t = (int)std::min<size_t>(4, sm_bytes / per_block(tight)), nb_w = (int)std::min<size_t>(4, sm_bytes / per_block(want));
-        if (nb_t > nb_w) {
+        // only where it matters and where the maximum over blocks is statistically stable: at least one block per SM
+        if (nb_t == nb_w && nb_w >= 1 && nb_w <= 4 && s->P.nblk >= 148) {
+            // head room that costs nothing: up to 30 % if the same number of blocks stays resident
+            size_t budget = sm_bytes / nb_w - 1024 - 16;
+            if (budget > 75 * 1024 + xch) budget -= xch;
+            const int fit = (int)(budget / per_entry) / 64 * 64;
+            const int roomy = ((int)(c.max_stage * 1.30) + 64 + 63) / 64 * 64;
+            if (fit > want && per_block(std::min(fit, roomy)) * nb_w <= sm_bytes) want = std::min(fit, roomy);
+        } else if (nb_t > nb_w && s->P.nblk >= 148) {
             size_t budget = sm_bytes / nb_t - 1024 - 16;
             if (budget > 75 * 1024 + xch) budget -= xch;
             const int fit = (int)(budget / per_entry) / 64 * 64;
