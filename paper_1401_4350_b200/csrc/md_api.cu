@@ -230,6 +230,7 @@ md_status sync_and_check(md_system* s, const char* where) {
         s->lists_valid = s->staged_valid = false;
         return MD_ERR_CAPACITY;
     }
+    s->n_edges_host = (long long)c.n_edges;
     if (s->order != MD_ORDER_NONE && c.max_stage > 0) {
         // size the staged force launches from the largest neighbourhood seen, with 15 % head room for the
         // device-side rebuilds that happen before the next synchronising call; if that head room alone costs a

@@ -274,8 +274,9 @@ __global__ void __launch_bounds__(256) k_edge_red(DevParams P, DevBuffers B, con
 // (c) warp-aggregated by the owning particle: SLICE lanes walk the half row of particle i (edges sorted by
 // i), keep the i-side sum in registers, combine it with __shfl_xor and issue ONE red per particle and array;
 // the j side is scattered with red.v4.
-#define EDGE_SLICE 8
-template <int KIND>
+// EDGE_SLICE lanes per owner: 8 for long half rows (LJ at r_c >= 2.5), 4 or 2 for the short rows of the polymer and patchy
+// configs (an 8-lane slice on a 6-entry half row leaves most lanes idle)
+template <int KIND, int EDGE_SLICE>
 __global__ void __launch_bounds__(256) k_edge_warp(DevParams P, DevBuffers B, const float4* __restrict__ pos,
                                                    const float4* __restrict__ quat, float4* force, float4* torque) {
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -467,7 +468,12 @@ static void launch_edge(md_system* s, int scatter) {
         s->launches += 1;
         if (scatter == MD_SCATTER_RED) k_edge_red<KIND, false><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
         else if (scatter == MD_SCATTER_RED_V4) k_edge_red<KIND, true><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
-        else k_edge_warp<KIND><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+        else {
+            const double half_row = (double)s->n_edges_host / (double)P.N;   // E / N at the last synchronised build (0 if unknown)
+            if (half_row > 0 && half_row < 8.0) k_edge_warp<KIND, 2><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+            else if (half_row > 0 && half_row < 14.0) k_edge_warp<KIND, 4><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+            else k_edge_warp<KIND, 8><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+        }
         s->launches += 1;
     }
     if (P.kind == MD_POT_FENE_WCA) {
