@@ -168,9 +168,10 @@ md_status md_forces(md_system*, int32_t strategy, int32_t scatter);
  * device without host synchronisation, forces, half kick.  Requires valid forces on entry. */
 md_status md_integrate(md_system*, double dt, int64_t nsteps, int32_t strategy, int32_t scatter);
 /* Note on capacity: the shared-memory staged VERTEX variant is launched with room for the largest block neighbourhood
- * seen at the last synchronising call plus 15-30 %.  While the structure of the system changes (a lattice melting),
- * call md_stats every ~100 steps so that this capacity follows; an overflow is reported as MD_ERR_CAPACITY, never
- * computed wrongly in silence. */
+ * seen at the last synchronising call plus 15-30 %.  A block whose neighbourhood outgrows that room in a device-side
+ * rebuild (a lattice melting) is still computed, from global memory through its segment table (slower, same pairs and
+ * decisions); calling md_stats every ~100 steps while the structure changes lets the capacity follow.  Only a
+ * neighbourhood beyond the BUILD capacity (a quarter of a million staged bytes per block) is an error, MD_ERR_CAPACITY. */
 
 /* S:A9: U = sum_i pe_i, K_t = 1/2 m sum |v|^2, K_r = sum |L|^2 / (2 I), accumulated in fp64.
  * Host output pointers.  Synchronises; reports latched device errors. */

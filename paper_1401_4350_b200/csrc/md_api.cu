@@ -224,9 +224,8 @@ md_status sync_and_check(md_system* s, const char* where) {
         return MD_ERR_CAPACITY;
     }
     if (c.err & MD_DEVERR_STAGE) {
-        snprintf(s->errmsg, sizeof(s->errmsg), "staged neighbourhood capacity exceeded: a block needs %d staged particles / %d segments "
-                 "(build capacity %d, launch capacity %d, segment capacity %d); rebuild with md_build_cells + md_build_verlet",
-                 c.max_stage, c.max_seg, s->P.stage_cap, s->stage_launch, MD_SEGMAX);
+        snprintf(s->errmsg, sizeof(s->errmsg), "staged build capacity exceeded: a block needs %d staged particles / %d segments "
+                 "(build capacity %d, segment capacity %d)", c.max_stage, c.max_seg, s->P.stage_cap, MD_SEGMAX);
         s->lists_valid = s->staged_valid = false;
         return MD_ERR_CAPACITY;
     }
@@ -325,6 +324,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);
     s->stage_launch = P.stage_cap;
+    s->stage_limit = getenv("MD_B200_STAGE_LIMIT") ? atoi(getenv("MD_B200_STAGE_LIMIT")) : 0;
     P.kind = rigid ? MD_POT_PATCHY : pot->kind;   // both rigid-body models run on the same kernels (P.pp_model tells them apart)
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
     P.sigma = pot->sigma;

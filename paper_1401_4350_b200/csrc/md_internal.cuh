@@ -141,6 +141,7 @@ struct md_system {
     float4 *pos, *vel, *force, *quat, *angmom, *torque;
     bool bound, cells_valid, lists_valid, forces_valid, seg_valid;
     bool staged_valid, legacy_valid;   // which list representations describe the current build
+    int stage_limit;         // MD_B200_STAGE_LIMIT: cap on the staged launch capacity (0 = none; tests of the unstaged path)
     long long n_edges_host;  // E at the last synchronising call (0 before the first): picks the EDGE slice width
     int stage_launch;        // staged-particle capacity the force kernels are launched with (from the last synchronised build)
     int64_t launches;

@@ -13,6 +13,7 @@
 // The pair arithmetic, the fp64 recheck band (S:H10) and all tolerances are those of md_forces.cu.
 #include <stdio.h>
 #include <stdlib.h>
+#include <algorithm>
 #include "md_pair.cuh"
 
 #define GATE(B, gated) if ((gated) && (B).ctrl->rebuild == 0) return
@@ -978,6 +979,63 @@ __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuff
     force[i] = make_float4(a.fx, a.fy, a.fz, pe);
 }
 
+// Blocks whose neighbourhood does not fit the launch (it grew past the head room since the last synchronising call)
+// are not failed: they take this slow path, which reads the same rows but fetches each neighbour from global memory --
+// local index -> slot through the block's segment table (sorted by local base: binary search), raw positions, minimum
+// image.  Same pair set, same decisions (fp64 band), so the result stays within the parity tolerance.
+__device__ __forceinline__ int staged_slot_of_local(const int2* __restrict__ seg, int nseg, int t) {
+    int lo = 0, hi = nseg - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if ((int)((unsigned)seg[mid].y >> 16) <= t) lo = mid; else hi = mid - 1;
+    }
+    const int2 sg = seg[lo];
+    return sg.x + (t - (int)((unsigned)sg.y >> 16));
+}
+
+template <bool RIGID, bool PP>
+__device__ __forceinline__ void vertex_rows_unstaged(const DevParams& P, const DevBuffers& B, const BlkInfo bi, int b,
+                                                  const float4* __restrict__ pos, const float4* __restrict__ quat,
+                                                  float4* __restrict__ force, float4* __restrict__ torque) {
+    if (threadIdx.x >= MD_TB) return;
+    const int i = b * MD_TB + threadIdx.x;
+    if (i >= P.N) return;
+    const int cnt = B.row_count[i];
+    const int sh = (bi.flags & MD_BLK_SH4) ? 4 : 0;
+    const int2* __restrict__ seg = B.seg + (size_t)b * MD_SEGMAX;
+    const unsigned short* __restrict__ row = B.rows + ((size_t)b * (P.rcap >> 2) * MD_TB + threadIdx.x) * 4;
+    const float4 xi = pos[i];
+    Rot Ri;
+    if (RIGID) Ri = quat_to_rot(quat[i]);
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, tx = 0.f, ty = 0.f, tz = 0.f;
+    for (int k = 0; k < cnt; ++k) {
+        const int t = (int)row[(size_t)(k >> 2) * MD_TB * 4 + (k & 3)] >> sh;
+        const int j = staged_slot_of_local(seg, bi.nseg, t);
+        const float4 xj = pos[j];
+        const float dx = min_image(xj.x, xi.x, P.Lx, P.hLx), dy = min_image(xj.y, xi.y, P.Ly, P.hLy), dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+        const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        if (!in_cutoff(P, d2, xi, xj)) continue;
+        if (RIGID) {
+            float gx, gy, gz, V, a, bb, c, u, v, w;
+            rigid_pair<false, PP>(P, dx, dy, dz, d2, Ri, quat[j], gx, gy, gz, V, a, bb, c, u, v, w);
+            fx -= gx; fy -= gy; fz -= gz; pe += V;
+            tx += a; ty += bb; tz += c;
+        } else {
+            float g, V;
+            lj_pair(P, d2, g, V);
+            fx = fmaf(-g, dx, fx); fy = fmaf(-g, dy, fy); fz = fmaf(-g, dz, fz); pe += V;
+        }
+    }
+    pe *= 0.5f;
+    if (!RIGID && P.kind == MD_POT_FENE_WCA) {
+        float bpe = 0.f;
+        fene_vertex_s(P, B, pos, i, fx, fy, fz, bpe);
+        pe += 0.5f * bpe;
+    }
+    force[i] = make_float4(fx, fy, fz, pe);
+    if (RIGID) torque[i] = make_float4(tx, ty, tz, 0.f);
+}
+
 template <int NS>
 __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries,
                                                                                   const float4* __restrict__ pos,
@@ -996,8 +1054,9 @@ __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k
     const uint2 pkA = ld_row(rowh), pkB = ld_row(rowh + NS * MD_TB), pkC = ld_row(rowh + 2 * NS * MD_TB), pkD = ld_row(rowh + 3 * NS * MD_TB);
     const int cnt = live ? B.row_count[i] : 0;
     const BlkInfo bi = B.blk[b];
-    if (bi.M <= 0 || bi.M + 1 > stage_entries) {   // build failed for this block / launch sized too small: latch, never guess
-        if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
+    if (bi.M <= 0) return;                         // the build failed for this block and latched the error: never guess
+    if (bi.M + 1 > stage_entries) {                // launch sized too small for this block: slow path from global memory
+        vertex_rows_unstaged<false, false>(P, B, bi, b, pos, nullptr, force, nullptr);
         return;
     }
     const Stage st = stage_issue<false>(P, B, bi, b, stage_entries, pre, pos, nullptr, smraw);
@@ -1068,14 +1127,15 @@ __device__ __forceinline__ void vertex_patchy_rows(const DevParams& P, const Dev
 }
 
 template <bool PP>
-__global__ void __launch_bounds__(MD_TB) k_vertex_patchy_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
+__global__ void __launch_bounds__(MD_TB, 4) k_vertex_patchy_staged(DevParams P, DevBuffers B, int stage_entries, const float4* __restrict__ pos,
                                                                 const float4* __restrict__ quat, float4* __restrict__ force,
                                                                 float4* __restrict__ torque) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int b = blockIdx.x;
     const BlkInfo bi = B.blk[b];
-    if (bi.M <= 0 || bi.M + 1 > stage_entries) {
-        if (threadIdx.x == 0 && bi.M + 1 > stage_entries) atomicOr(&B.ctrl->err, MD_DEVERR_STAGE);
+    if (bi.M <= 0) return;
+    if (bi.M + 1 > stage_entries) {                // as in k_vertex_lj_staged
+        vertex_rows_unstaged<true, PP>(P, B, bi, b, pos, quat, force, torque);
         return;
     }
     const SegPre pre = seg_preload(B, b);
@@ -1114,7 +1174,8 @@ static void staged_attrs_once() {
 bool md_launch_forces_staged(md_system* s) {
     const DevParams& P = s->P;
     staged_attrs_once();
-    const int se = s->stage_launch;
+    int se = s->stage_launch;
+    if (s->stage_limit > 0) se = std::min(se, s->stage_limit);   // MD_B200_STAGE_LIMIT (tests): force blocks onto the unstaged path
     const size_t smem = md_staged_smem_bytes(s, se);
     if (smem > 224 * 1024) return false;
     if (P.kind == MD_POT_PATCHY && P.pp_model) k_vertex_patchy_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);

@@ -414,3 +414,22 @@ def test_patchy_pp_short_trajectory(MD, oracle):
         assert abs(e1 - e0) <= 2e-3 * abs(e0)                 # conserved along the stiff trajectory (dt = 0.002)
         assert abs(o["energies"][-1].sum() - o["e0"].sum()) <= 2e-3 * abs(o["e0"].sum())
         s.close()
+
+
+@pytest.mark.parametrize("case", ["lj", "polymer", "patchy", "patchy_pp"])
+def test_blocks_over_the_launch_capacity_take_the_unstaged_path(MD, oracle, case, monkeypatch):
+    """A block whose neighbourhood outgrew the staged launch capacity is computed from global memory through its
+    segment table instead of failing the run: force every block onto that path (MD_B200_STAGE_LIMIT) and compare with
+    the oracle."""
+    monkeypatch.setenv("MD_B200_STAGE_LIMIT", "64")
+    w = {"lj": lambda: W.lj_fluid(2 ** 13), "polymer": lambda: W.polymer_melt(64, 64),
+         "patchy": lambda: W.patchy_fluid(2 ** 12, rho=0.9, jitter=0.1), "patchy_pp": lambda: W.dimer_gas(2048, "patchy_pp")}[case]()
+    s = MD.from_workload(w, order="hilbert")
+    s.build_cells(); s.build_verlet(); s.forces("vertex", "smem")
+    o = oracle.forces(w.pos, w.box, dict(w.potential), quat=w.quat)
+    assert_forces(s, o, w.quat is not None)
+    s.integrate(w.dt, 20, "vertex", "smem")
+    pos = s.in_id_order(s.pos)
+    quat = s.in_id_order(s.quat) if w.quat is not None else None
+    assert_forces(s, oracle.forces(pos, w.box, dict(w.potential), quat=quat), quat is not None)
+    s.close()
