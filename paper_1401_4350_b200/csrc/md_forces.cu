@@ -211,21 +211,28 @@ __global__ void k_zero4(DevParams P, float4* a, float4* b) {
 }
 
 // evaluate one edge: returns true if inside the cutoff; F_j = (fx,fy,fz), V full pair energy
-template <int KIND>
-__device__ __forceinline__ bool edge_eval(const DevParams& P, const float4* __restrict__ pos, const float4* __restrict__ quat,
-                                          int i, int jw, float& fx, float& fy, float& fz, float& V,
-                                          float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
+// first half of an edge: separation and the cutoff decision (cheap: two position loads, ~25 instructions)
+__device__ __forceinline__ bool edge_test(const DevParams& P, const float4* __restrict__ pos, int i, int jw,
+                                          float& dx, float& dy, float& dz, float& d2) {
     const int j = jw & 0x7fffffff;
     float4 xi = ldg4(pos + i), xj = ldg4(pos + j);
-    float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
+    dx = xj.x - xi.x; dy = xj.y - xi.y; dz = xj.z - xi.z;
     if (jw < 0) {   // the pair crosses a periodic face (flag set at build time)
         dx = min_image(xj.x, xi.x, P.Lx, P.hLx);
         dy = min_image(xj.y, xi.y, P.Ly, P.hLy);
         dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
     }
-    float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    if (!in_cutoff(P, d2, xi, xj)) return false;
+    d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    return in_cutoff(P, d2, xi, xj);
+}
+
+// second half: the pair function of an edge inside the cutoff.  F_j = (fx,fy,fz), V full pair energy
+template <int KIND>
+__device__ __forceinline__ void edge_force(const DevParams& P, const float4* __restrict__ quat, int i, int jw,
+                                           float dx, float dy, float dz, float d2, float& fx, float& fy, float& fz, float& V,
+                                           float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
     if (md_is_rigid(KIND)) {
+        const int j = jw & 0x7fffffff;
         float4 qi = ldg4(quat + i), qj = ldg4(quat + j);
         const Rot Ri = quat_to_rot(qi);
         rigid_pair<true, KIND == MD_POT_PATCHY_PP>(P, dx, dy, dz, d2, Ri, qj, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
@@ -234,6 +241,16 @@ __device__ __forceinline__ bool edge_eval(const DevParams& P, const float4* __re
         lj_pair(P, d2, g, V);
         fx = g * dx; fy = g * dy; fz = g * dz;
     }
+}
+
+// evaluate one edge: returns true if inside the cutoff
+template <int KIND>
+__device__ __forceinline__ bool edge_eval(const DevParams& P, const float4* __restrict__ pos, const float4* __restrict__ quat,
+                                          int i, int jw, float& fx, float& fy, float& fz, float& V,
+                                          float& tix, float& tiy, float& tiz, float& tjx, float& tjy, float& tjz) {
+    float dx, dy, dz, d2;
+    if (!edge_test(P, pos, i, jw, dx, dy, dz, d2)) return false;
+    edge_force<KIND>(P, quat, i, jw, dx, dy, dz, d2, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
     return true;
 }
 
@@ -243,10 +260,22 @@ __global__ void __launch_bounds__(256) k_edge_red(DevParams P, DevBuffers B, con
                                                   const float4* __restrict__ quat, float4* force, float4* torque) {
     const unsigned int E = B.ctrl->n_edges;
     const unsigned int stride = gridDim.x * blockDim.x;
-    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < E; e += stride) {
-        int2 ij = B.edges[e];
+    unsigned int e = blockIdx.x * blockDim.x + threadIdx.x;
+    for (;;) {
+        // every lane scans forward to its next edge inside the cutoff (the others cost a distance test and nothing
+        // else), so that the lanes of a warp enter the pair function together: for the rigid bodies, where that function is
+        // ~250 instructions and half of the listed pairs are outside r_c, this is what the time goes into
+        int2 ij;
+        float dx, dy, dz, d2;
+        bool have = false;
+        while (e < E) {
+            ij = B.edges[e];
+            e += stride;
+            if (edge_test(P, pos, ij.x, ij.y, dx, dy, dz, d2)) { have = true; break; }
+        }
+        if (!have) break;
         float fx, fy, fz, V, tix = 0.f, tiy = 0.f, tiz = 0.f, tjx = 0.f, tjy = 0.f, tjz = 0.f;
-        if (!edge_eval<KIND>(P, pos, quat, ij.x, ij.y, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz)) continue;
+        edge_force<KIND>(P, quat, ij.x, ij.y, dx, dy, dz, d2, fx, fy, fz, V, tix, tiy, tiz, tjx, tjy, tjz);
         const int j = ij.y & 0x7fffffff;
         const float hV = 0.5f * V;
         if (V4) {
