@@ -169,13 +169,13 @@ __device__ __noinline__ int scan_cell_slow(const float4* __restrict__ cellpos, i
 // ------------------------------------------------------------------------------------------------
 template <bool MASKS>
 __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
-                                                        int ncand_cap, int umax) {
+                                                        int ncand_cap, int umax, int tbl_cap) {
     GATE(B, gated);
     extern __shared__ __align__(16) unsigned char smraw[];
     // The build reads candidate positions straight from global memory (all lanes of a warp read the same candidate: one
     // sector, L1-resident), so its shared memory holds only the cell tables and four blocks fit on an SM.
     int* cand = reinterpret_cast<int*>(smraw);                       // [ncand_cap]
-    int* urank = cand + ncand_cap;                                   // [umax]
+    int* urank = cand + (tbl_cap >> 1);                              // [umax]  (cand[]: max(hash set, stencil table) = tbl_cap / 2 ints)
     int* ubase = urank + umax;                                       // [umax + 1]
     int* ustart = ubase + umax + 1;                                  // [umax] first slot of the cell
     int* own_rank = ustart + umax;                                   // [MD_TB]
@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
 
     // 2. candidate cells: the 27-cell stencil of every own cell (S:Q8)
     const int n = 27 * nownc;
-    if (n >= ncand_cap) {   // the hash set below needs a free slot: cannot happen for n <= 27*MD_TB < MD_NCAND unless sized smaller   // cannot happen for n <= 27*MD_TB <= MD_NCAND unless the launch was sized smaller
+    if (n > tbl_cap) {      // the stencil table (27 16-bit entries per own cell, in the storage of the hash set) was sized smaller
         if (tid == 0) { atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); B.blk[b] = BlkInfo{ 0, 0, 0, 0 }; }
         if (live) { B.row_count[i] = 0; B.lo_count[i] = 0; B.half_count[i] = 0; B.pos_ref[i] = pos[i]; }
         return;
@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     // the candidates go through a shared-memory hash set (cand[], open addressing, native 32-bit CAS): neighbouring own
     // cells share most of their stencils, so only the DISTINCT cells (a few hundred) are compacted and sorted, not the
     // 27 x own-cells candidates (thousands at 2-3 particles per cell)
-    const int hmask = ncand_cap - 1;                  // ncand_cap is a power of two > n
+    const int hmask = ncand_cap - 1;                  // ncand_cap is a power of two >= 2 umax (or > 27 x own cells)
     for (int t = tid; t < ncand_cap; t += MD_TB) cand[t] = 0x7fffffff;
     __syncthreads();
     for (int t = tid; t < n; t += MD_TB) {
@@ -224,7 +224,8 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
         const int r = B.cell_rank[(ax * P.ncy + ay) * P.ncz + az];
         if (B.cell_start[r + 1] > B.cell_start[r]) {      // empty cells contribute nothing
             unsigned int h = ((unsigned int)r * 2654435761u) >> 7;
-            for (;;) {
+            for (int probes = 0;; ++probes) {
+                if (probes > hmask) { atomicAdd(&s_U, umax + 1); break; }   // set full: more distinct cells than it was sized for
                 h &= hmask;
                 const int old = atomicCAS(&cand[h], 0x7fffffff, r);
                 if (old == 0x7fffffff) {                  // first sighting of this cell: append it to the distinct list
@@ -355,7 +356,7 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
             int u = (U > 0 && urank[lo] == r) ? lo : -1;
             if (small_axis && u >= 0)
                 for (int s2 = 0; s2 < st; ++s2) if (stencil_rank(lin, s2) == r) { u = -1; break; }
-            cand[t] = u;
+            reinterpret_cast<short*>(cand)[t] = (short)u;   // u < umax <= 4096
         }
     }
     __syncthreads();
@@ -409,7 +410,7 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     const int cap8 = (P.rcap + 2) >> 1;                             // capacity of one column bucket of pass B
     unsigned short* tmp_blk = B.rows_tmp + ((size_t)P.nblk * 8 * cap8 + (size_t)b * (P.rcap + 2)) * MD_TB;   // list form: neighbours in scan order
     unsigned short* tmp = tmp_blk + tid;
-    const int* __restrict__ mycells = cand + max(myoc, 0) * 27;
+    const short* __restrict__ mycells = reinterpret_cast<const short*>(cand) + max(myoc, 0) * 27;
     const int me = own_base + tid;
     if (live) {
         const float4 xi_raw = __ldg(pos + i);
@@ -590,7 +591,7 @@ __global__ void k_staged_begin(DevBuffers B, int gated) {
     B.ctrl->max_seg = 0;
 }
 
-static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, size_t* smem) {
+static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, int* tbl_cap, size_t* smem) {
     const DevParams& P = s->P;
     const double ppc = (double)P.N / (double)P.ncell;
     double own = (double)MD_TB / (ppc > 1e-9 ? ppc : 1e-9);
@@ -599,29 +600,50 @@ static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, si
     while (nc < 27 * (2 * own + 4) && nc < MD_NCAND) nc <<= 1;
     if (nc > MD_NCAND) nc = MD_NCAND;
     int um = nc < MD_UMAX ? nc : MD_UMAX;
+    int region = nc;                                  // ints shared by the hash set and, after it, the stencil table
+    if (4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) > 40 * 1024) {
+        // sparse cells (2-3 particles per cell): ~100 own cells per block.  The set holds DISTINCT cells only, about
+        // (own^(1/3) + 2)^3 of them for a compact block: size it (4x that, load <= 1/2) instead of 27 x own cells, and
+        // keep the table at its hard bound of 27 x MD_TB 16-bit entries -- 42 KB instead of 83 KB per block at 2.5
+        // particles per cell, five resident blocks instead of one.
+        const double side = cbrt(own) + 2.0;
+        int want = 256;
+        while (want < 4.0 * side * side * side && want < MD_UMAX) want <<= 1;
+        um = want < um ? want : um;
+        nc = 2 * um;
+        region = nc > (27 * MD_TB + 1) / 2 ? nc : (27 * MD_TB + 1) / 2;
+    }
     *ncand_cap = nc;
     *umax = um;
-    *smem = 4 * ((size_t)nc + 3 * (size_t)um + 1 + MD_TB) + 16;
+    *tbl_cap = 2 * region;
+    *smem = 4 * ((size_t)region + 3 * (size_t)um + 1 + MD_TB) + 16;
 }
 
 void md_launch_build_staged(md_system* s, bool gated) {
     const DevParams& P = s->P;
     const int g = gated ? 1 : 0;
-    int nc, um;
+    int nc, um, tc;
     size_t smem;
-    staged_build_sizes(s, &nc, &um, &smem);
+    staged_build_sizes(s, &nc, &um, &tc, &smem);
     static bool attr_done = false;
+    static int carve_now = -1;
     if (!attr_done) {
         cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
         cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-        // candidates are read through L1: leave it as large as the four resident blocks allow
-        cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 50);
-        cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 50);   // measured: 25 -> 1.96 ms, 50 -> 1.65, 75 -> 1.82, 100 -> 2.02
         attr_done = true;
     }
+    // candidates are read through L1: with the small tables of dense cells leave it as large as the resident blocks allow
+    // (measured at C2a: carveout 25 -> 1.96 ms, 50 -> 1.65, 75 -> 1.82, 100 -> 2.02); the 42 KB tables of sparse cells need
+    // the shared memory itself (five resident blocks instead of two)
+    const int carve = smem > 30 * 1024 ? (int)cudaSharedmemCarveoutMaxShared : 50;
+    if (carve != carve_now) {
+        cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+        cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+        carve_now = carve;
+    }
     k_staged_begin<<<1, 1, 0, s->stream>>>(s->B, g);
-    if (P.use_masks) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um);
-    else k_build_staged<false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um);
+    if (P.use_masks) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
+    else k_build_staged<false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
     s->launches += 2;
 }
 
