@@ -24,6 +24,9 @@
  *       for M = 2, r_c = 0.18 sigma cuts r^{ij}).  PARITY UNPINNED for that reading (the cited sources are not in
  *       the container); the arithmetic of the reading itself is pinned (closed forms, finite differences,
  *       Newton-3 invariants).
+ *   O9  the NVT thermostat of P:53 (Ref. 27, not in the container): reading DESIGN.md QT, an Andersen-type
+ *       velocity refresh driven by Philox4x32-10.  PARITY UNPINNED with respect to Ref. 27; the reading's
+ *       arithmetic is pinned (see O9 below).
  * Forces/torques/energies are the PLAIN DEFINITION: a direct sum over all pairs with d2 < rcut^2
  * (both strategies evaluate exactly the pairs of the Verlet list that are inside r_c).
  * The oracle's own cell list only prunes pairs that cannot be inside the cutoff; `use_cells=0`
@@ -36,7 +39,8 @@
  *
  * Parity pins (tests/test_oracle_pins.py): closed forms P1-P4, fcc lattice sums P5, brute force P6/P8,
  * Newton-3 invariants P7, finite-difference force/torque vs energy, NVE drift P9, free rotor P10,
- * Fig. 1 thread counts P12.  Only O8 (patch_point_pair) is "parity unpinned" (see O8 above).
+ * Fig. 1 thread counts P12.  Only O8 (patch_point_pair) and O9 (thermostat) are "parity unpinned"
+ * (see O8 above, O9 below).
  */
 #include <math.h>
 #include <stdint.h>
@@ -571,4 +575,74 @@ int orc_integrate_d(int64_t N, double* pos, double* vel, double* quat, double* a
     free(ref);
     if (n_rebuilds) *n_rebuilds = rebuilds;
     return bad;
+}
+
+/* =====================================================================================
+ * O9: the NVT thermostat the paper names but does not describe ("Brownian dynamics simulations in
+ * the NVT ensemble, with the thermostat described in Ref. 27"; S:8(f3), item 12 of S:2).  Ref. 27 is not in
+ * the container: reading DESIGN.md QT -- an Andersen-type velocity refresh: after every n_newt-th
+ * velocity-Verlet step each particle, independently and with probability p_t, has its velocity replaced by
+ * a Maxwell-Boltzmann draw at temperature T (each component Gaussian of variance k_B T / m); a rigid body,
+ * with probability p_r, likewise its angular momentum (variance k_B T I).  PARITY UNPINNED with respect to
+ * Ref. 27; the arithmetic of the reading is pinned (Philox known answers, moments and a KS test of the draws,
+ * refreshed fraction, p = 0 and p = 1, relaxation of an LJ fluid to the target temperature).
+ *
+ * Random numbers: the counter-based generator Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11); both
+ * sides implement it, nothing is shared.  key = (seed low word, seed high word); counter =
+ * (particle id, call index, stream, block): stream 0 = translation, 1 = rotation; block 0 word 0 decides
+ * (refresh iff word0 < floor(p 2^32), compared in 64 bits so that p = 1 always refreshes); block 1 words
+ * 0..3 give u_k = (word_k + 0.5) 2^-32 and, by Box-Muller in fp64,
+ *   g0 = sqrt(-2 ln u0) cos(2 pi u1), g1 = sqrt(-2 ln u0) sin(2 pi u1), g2 = sqrt(-2 ln u2) cos(2 pi u3).
+ * ===================================================================================== */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* one stream of one particle: returns 1 and the three Gaussians if the particle is refreshed */
+static int thermostat_draw(uint32_t id, uint32_t call, uint32_t stream, uint64_t seed, double p, double g[3]) {
+    const uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
+    uint32_t c[4] = { id, call, stream, 0u }, w[4];
+    double thr_d = floor(p * 4294967296.0);
+    uint64_t thr = thr_d <= 0.0 ? 0u : (thr_d >= 4294967296.0 ? 4294967296ull : (uint64_t)thr_d);
+    orc_philox4x32_10(c, key, w);
+    if (!((uint64_t)w[0] < thr)) return 0;
+    c[3] = 1u;
+    orc_philox4x32_10(c, key, w);
+    const double two_pi = 6.283185307179586476925286766559;
+    double u0 = ((double)w[0] + 0.5) / 4294967296.0, u1 = ((double)w[1] + 0.5) / 4294967296.0;
+    double u2 = ((double)w[2] + 0.5) / 4294967296.0, u3 = ((double)w[3] + 0.5) / 4294967296.0;
+    double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
+    g[0] = r0 * cos(two_pi * u1);
+    g[1] = r0 * sin(two_pi * u1);
+    g[2] = r1 * cos(two_pi * u3);
+    return 1;
+}
+
+/* one application of the thermostat to fp64 state in id order; returns the number of refreshed velocities
+ * (n_rot: refreshed angular momenta).  angmom may be NULL. */
+int64_t orc_thermostat_d(int64_t N, double* vel, double* angmom, double mass, double inertia, double T,
+                         double p_t, double p_r, uint64_t seed, uint32_t call, int64_t* n_rot) {
+    int64_t nt = 0, nr = 0;
+    const double sv = sqrt(T / mass), sl = sqrt(T * inertia);
+    for (int64_t i = 0; i < N; ++i) {
+        double g[3];
+        if (thermostat_draw((uint32_t)i, call, 0u, seed, p_t, g)) {
+            for (int k = 0; k < 3; ++k) vel[3 * i + k] = sv * g[k];
+            ++nt;
+        }
+        if (angmom && thermostat_draw((uint32_t)i, call, 1u, seed, p_r, g)) {
+            for (int k = 0; k < 3; ++k) angmom[3 * i + k] = sl * g[k];
+            ++nr;
+        }
+    }
+    if (n_rot) *n_rot = nr;
+    return nt;
 }

@@ -111,6 +111,12 @@ class Oracle:
         L.orc_integrate_d.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, _dp, C.POINTER(OrcPot), C.c_double, C.c_double,
                                       C.c_int64, C.c_int64, _dp, _dp, _dp, _dp, _lp]
         L.orc_set_threads.argtypes = [C.c_int]
+        _up = C.POINTER(C.c_uint32)
+        L.orc_philox4x32_10.restype = None
+        L.orc_philox4x32_10.argtypes = [_up, _up, _up]
+        L.orc_thermostat_d.restype = C.c_int64
+        L.orc_thermostat_d.argtypes = [C.c_int64, _dp, _dp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                       C.c_uint64, C.c_uint32, _lp]
 
     @property
     def threads(self) -> int:
@@ -218,6 +224,46 @@ class Oracle:
                                        _d(F), _d(T), _d(pe), _d(en), C.byref(nreb))
         return dict(pos=x, vel=v, quat=q, angmom=L, F=F, T=T, pe=pe, e0=np.array(e0), energies=en[:nrec],
                     rebuilds=int(nreb.value), bad=int(bad | f0["bad"]))
+
+    # ---- O9: thermostat (reading DESIGN.md QT of P:53; parity unpinned w.r.t. the paper's Ref. 27)
+    def philox(self, ctr, key):
+        """Philox4x32-10 block: ctr 4 x uint32, key 2 x uint32 -> 4 x uint32."""
+        c = np.ascontiguousarray(ctr, dtype=np.uint32)
+        k = np.ascontiguousarray(key, dtype=np.uint32)
+        out = np.zeros(4, dtype=np.uint32)
+        up = C.POINTER(C.c_uint32)
+        self.lib.orc_philox4x32_10(c.ctypes.data_as(up), k.ctypes.data_as(up), out.ctypes.data_as(up))
+        return out
+
+    def thermostat(self, vel_d, pot, T, p_t, seed, call, angmom_d=None, p_r=0.0):
+        """One application on fp64 copies (id order). Returns (vel, angmom, n_refreshed_trans, n_refreshed_rot)."""
+        op = pot if isinstance(pot, OrcPot) else make_pot(pot)
+        v = np.ascontiguousarray(np.asarray(vel_d)[:, :3], dtype=np.float64).copy()
+        L = np.ascontiguousarray(np.asarray(angmom_d)[:, :3], dtype=np.float64).copy() if angmom_d is not None else None
+        nr = C.c_int64(0)
+        nt = self.lib.orc_thermostat_d(v.shape[0], _d(v), _d(L), op.mass, op.inertia, float(T), float(p_t), float(p_r),
+                                       int(seed), int(call), C.byref(nr))
+        return v, L, int(nt), int(nr.value)
+
+    def integrate_nvt(self, pos, vel, box, pot, skin, dt, nsteps, T, n_newt, p_t, seed, quat=None, angmom=None,
+                      p_r=0.0, every=0):
+        """O6/O7 with O9 applied after every n_newt-th step (call index = steps done / n_newt, counted from this
+        call). Returns the dict of integrate() plus 'temps': kinetic temperature 2 K_t / (3 N) after each chunk."""
+        op = pot if isinstance(pot, OrcPot) else make_pot(pot)
+        x, v, q, L = pos, vel, quat, angmom
+        done, temps, reb, out = 0, [], 0, None
+        while done < nsteps:
+            chunk = min(n_newt - done % n_newt, nsteps - done)
+            out = self.integrate(x, v, box, op, skin, dt, chunk, quat=q, angmom=L)
+            x, v, q, L = out["pos"], out["vel"], out["quat"], out["angmom"]
+            reb += out["rebuilds"]
+            done += chunk
+            if done % n_newt == 0:
+                v, L, _, _ = self.thermostat(v, op, T, p_t, seed, done // n_newt, angmom_d=L, p_r=p_r)
+            temps.append(op.mass * float((v * v).sum()) / (3.0 * v.shape[0]))
+        out = dict(out)
+        out.update(vel=v, angmom=L, rebuilds=reb, temps=np.array(temps))
+        return out
 
 
 if __name__ == "__main__":

@@ -523,3 +523,69 @@ def test_o8_patchy_pp_system(oracle):
             qm[i] = qmul(np.array([math.cos(h / 2), *(-math.sin(h / 2) * ax)]), q[i])
             t = -(_total_U(oracle, x, w.box, w.potential, qp) - _total_U(oracle, x, w.box, w.potential, qm)) / (2 * h)
             assert abs(t - fd["T"][i, k]) < 5e-6 * max(1.0, np.abs(fd["T"]).max())
+
+
+# ------------------------------------------------------------------ O9: thermostat (reading QT of P:53)
+def test_o9_philox_known_answers(oracle):
+    from conftest import GOLDEN
+    rows = [ln.split() for ln in (GOLDEN / "philox4x32_10_kat.txt").read_text().splitlines()
+            if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        assert [int(x) for x in oracle.philox(v[0:4], v[4:6])] == v[6:10]
+
+
+def test_o9_p0_is_identity_p1_refreshes_everything(oracle):
+    rng = np.random.default_rng(5)
+    v = rng.normal(size=(1000, 3))
+    L = rng.normal(size=(1000, 3))
+    v0, L0, nt, nr = oracle.thermostat(v, PATCHY, 0.15, 0.0, 7, 1, angmom_d=L, p_r=0.0)
+    assert nt == 0 and nr == 0 and np.array_equal(v0, v) and np.array_equal(L0, L)
+    v1, L1, nt, nr = oracle.thermostat(v, PATCHY, 0.15, 1.0, 7, 1, angmom_d=L, p_r=1.0)
+    assert nt == 1000 and nr == 1000
+    assert not np.any(v1 == v) and not np.any(L1 == L)
+    # the draw does not depend on the state it replaces, only on (id, call, seed)
+    v2, L2, _, _ = oracle.thermostat(np.zeros_like(v), PATCHY, 0.15, 1.0, 7, 1, angmom_d=np.zeros_like(L), p_r=1.0)
+    assert np.array_equal(v1, v2) and np.array_equal(L1, L2)
+    v3, _, _, _ = oracle.thermostat(v, PATCHY, 0.15, 1.0, 7, 2, angmom_d=L, p_r=1.0)
+    v4, _, _, _ = oracle.thermostat(v, PATCHY, 0.15, 1.0, 8, 1, angmom_d=L, p_r=1.0)
+    assert not np.any(v3 == v1) and not np.any(v4 == v1)
+
+
+def test_o9_maxwell_boltzmann_moments_and_ks(oracle):
+    from scipy import stats
+    N, T, mass, inertia = 200000, 1.7, 2.0, 0.1
+    pot = dict(PATCHY, mass=mass, inertia=inertia)
+    v, L, nt, nr = oracle.thermostat(np.zeros((N, 3)), pot, T, 1.0, 2024, 3, angmom_d=np.zeros((N, 3)), p_r=1.0)
+    for a, var in ((v, T / mass), (L, T * inertia)):
+        for k in range(3):
+            x = a[:, k]
+            assert abs(x.mean()) < 5.0 * math.sqrt(var / N)                 # 5 sigma of the sample mean
+            assert abs(x.var() / var - 1.0) < 5.0 * math.sqrt(2.0 / N)      # 5 sigma of the sample variance
+            assert abs(stats.kurtosis(x)) < 5.0 * math.sqrt(24.0 / N)
+            assert stats.kstest(x / math.sqrt(var), "norm").pvalue > 1e-4
+        c = np.corrcoef(a.T)
+        assert np.abs(c - np.eye(3)).max() < 5.0 / math.sqrt(N)            # components independent
+    assert np.abs(np.corrcoef(v[:, 0], L[:, 0])[0, 1]) < 5.0 / math.sqrt(N)  # streams independent
+    # equipartition: 1/2 m <v^2> = 3/2 T, <L^2>/(2 I) = 3/2 T
+    assert abs(0.5 * mass * (v * v).sum() / N / (1.5 * T) - 1.0) < 0.01
+    assert abs((L * L).sum() / (2.0 * inertia) / N / (1.5 * T) - 1.0) < 0.01
+
+
+def test_o9_refreshed_fraction_is_binomial(oracle):
+    N = 200000
+    for p in (0.02, 0.3, 0.75):
+        v, _, nt, _ = oracle.thermostat(np.zeros((N, 3)), LJ25, 1.0, p, 99, 1)
+        assert abs(nt - p * N) < 5.0 * math.sqrt(N * p * (1.0 - p))
+        assert nt == int(np.count_nonzero(np.any(v != 0.0, axis=1)))
+
+
+def test_o9_lj_fluid_relaxes_to_the_target_temperature(oracle):
+    """A hot LJ fluid (T = 2) under the thermostat at T = 1 ends at kinetic temperature 1 (NVT)."""
+    w = W.lj_fluid(500, T=2.0)
+    out = oracle.integrate_nvt(w.pos, w.vel, w.box, w.potential, w.skin, w.dt, 1200, T=1.0, n_newt=10, p_t=0.2, seed=11)
+    temps = out["temps"]
+    assert temps[0] > 1.3
+    assert abs(temps[-40:].mean() - 1.0) < 0.06
+    assert out["bad"] == 0
