@@ -145,6 +145,20 @@ md_status md_set_order(md_system*, int32_t order);
  * seen until the next md_bind_state.  MD_ERR_INVALID for an unknown value. */
 md_status md_set_precision(md_system*, int32_t precision);
 
+/* P:53 "Brownian dynamics simulations in the NVT ensemble, with the thermostat described in Ref. 27" -- Ref. 27 is not
+ * in the container; reading DESIGN.md QT: an Andersen-type velocity refresh.  One application: each particle,
+ * independently and with probability p_trans, gets a velocity drawn from the Maxwell-Boltzmann distribution at
+ * temperature T (components Gaussian, variance T / mass); with kind == MD_POT_PATCHY each body, with probability
+ * p_rot, likewise an angular momentum of variance T * inertia.  Draws come from Philox4x32-10 keyed by `seed`, counter
+ * (ORIGINAL particle id, `call`, stream, block): the result depends on neither the storage order nor the launch
+ * shape.  Positions and forces are untouched (forces stay valid); in MD_PREC_MIXED the fp64 copies are refreshed too.
+ * md_thermostat applies it once (asynchronous, on the stream).  md_set_thermostat makes md_integrate (and
+ * md_step_host) apply it after every n_newt-th step counted from this call, with call = steps / n_newt;
+ * n_newt = 0 switches it off (the default: NVE, B:5).  MD_ERR_INVALID for T <= 0, a probability outside [0, 1] or
+ * n_newt < 0; MD_ERR_STATE without a bound state. */
+md_status md_set_thermostat(md_system*, double T, int64_t n_newt, double p_trans, double p_rot, uint64_t seed);
+md_status md_thermostat(md_system*, double T, double p_trans, double p_rot, uint64_t seed, uint32_t call);
+
 /* The fp64 state of MD_PREC_MIXED in ORIGINAL id order: pos_host, vel_host = HOST double[3 N] (x, y, z per particle),
  * either may be NULL.  Synchronises.  MD_ERR_STATE unless the precision is MD_PREC_MIXED and the copies exist. */
 md_status md_get_state_double(md_system*, double* pos_host, double* vel_host);

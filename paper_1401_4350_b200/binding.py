@@ -21,7 +21,7 @@ STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPA
 
 # every symbol include/md_b200.h declares (checked by tests/test_abi.py against the header and the .so)
 EXPORTED_SYMBOLS = ["md_workspace_bytes", "md_create", "md_bind_state", "md_set_order", "md_set_precision",
-                    "md_get_state_double", "md_build_cells",
+                    "md_get_state_double", "md_set_thermostat", "md_thermostat", "md_build_cells",
                     "md_build_verlet", "md_forces", "md_integrate", "md_energy", "md_stats", "md_get_pairs",
                     "md_get_ids", "md_step_host", "md_launch_count", "md_last_error", "md_destroy"]
 
@@ -106,6 +106,10 @@ def load_library() -> C.CDLL:
     L.md_set_order.argtypes = [vp, C.c_int32]
     L.md_set_precision.restype = C.c_int
     L.md_set_precision.argtypes = [vp, C.c_int32]
+    L.md_set_thermostat.restype = C.c_int
+    L.md_set_thermostat.argtypes = [vp, C.c_double, C.c_int64, C.c_double, C.c_double, C.c_uint64]
+    L.md_thermostat.restype = C.c_int
+    L.md_thermostat.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint32]
     L.md_get_state_double.restype = C.c_int
     L.md_get_state_double.argtypes = [vp, vp, vp]
     for name in ("md_build_cells", "md_build_verlet"):
@@ -238,6 +242,14 @@ class MDSystem:
 
     def set_precision(self, precision):
         self._check(self.lib.md_set_precision(self.h, PRECISION[precision] if isinstance(precision, str) else int(precision)))
+
+    def set_thermostat(self, T, n_newt, p_trans, p_rot=0.0, seed=0):
+        """md_integrate applies the thermostat of reading QT after every n_newt-th step; n_newt = 0: off."""
+        self._check(self.lib.md_set_thermostat(self.h, float(T), int(n_newt), float(p_trans), float(p_rot), int(seed)))
+
+    def thermostat(self, T, p_trans, p_rot=0.0, seed=0, call=0):
+        """One application of the thermostat (asynchronous)."""
+        self._check(self.lib.md_thermostat(self.h, float(T), float(p_trans), float(p_rot), int(seed), int(call)))
 
     def state_f64(self):
         """(pos, vel) of MD_PREC_MIXED as float64 [N,3] arrays in original id order."""

@@ -638,7 +638,47 @@ md_status md_forces(md_system* s, int32_t strategy, int32_t scatter) {
     return check_cuda(s, "md_forces");
 }
 
+md_status md_set_thermostat(md_system* s, double T, int64_t n_newt, double p_trans, double p_rot, uint64_t seed) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (n_newt < 0 || (n_newt > 0 && (!(T > 0) || !(p_trans >= 0 && p_trans <= 1) || !(p_rot >= 0 && p_rot <= 1))))
+        return fail(s, MD_ERR_INVALID, "md_set_thermostat: n_newt >= 0, T > 0 and probabilities in [0, 1] required");
+    s->thermo_n = n_newt; s->thermo_steps = 0;
+    s->thermo_T = T; s->thermo_pt = p_trans; s->thermo_pr = p_rot; s->thermo_seed = seed;
+    return MD_OK;
+}
+
+md_status md_thermostat(md_system* s, double T, double p_trans, double p_rot, uint64_t seed, uint32_t call) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (!s->bound) return fail(s, MD_ERR_STATE, "md_thermostat: no state bound");
+    if (!(T > 0) || !(p_trans >= 0 && p_trans <= 1) || !(p_rot >= 0 && p_rot <= 1))
+        return fail(s, MD_ERR_INVALID, "md_thermostat: T > 0 and probabilities in [0, 1] required");
+    ensure_shadows(s);
+    md_launch_thermostat(s, T, p_trans, p_rot, seed, call);
+    return check_cuda(s, "md_thermostat");
+}
+
+static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t strategy, int32_t scatter);
+
+// NVE velocity-Verlet (B:5), with the thermostat of reading QT after every thermo_n-th step when it is set
 md_status md_integrate(md_system* s, double dt, int64_t nsteps, int32_t strategy, int32_t scatter) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->thermo_n <= 0 || nsteps <= 0) return integrate_nve(s, dt, nsteps, strategy, scatter);
+    int64_t done = 0;
+    while (done < nsteps) {
+        const int64_t to_next = s->thermo_n - s->thermo_steps % s->thermo_n;
+        const int64_t chunk = to_next < nsteps - done ? to_next : nsteps - done;
+        md_status st = integrate_nve(s, dt, chunk, strategy, scatter);
+        if (st != MD_OK) return st;
+        s->thermo_steps += chunk; done += chunk;
+        if (s->thermo_steps % s->thermo_n == 0)
+            md_launch_thermostat(s, s->thermo_T, s->thermo_pt, s->thermo_pr, s->thermo_seed, (unsigned int)(s->thermo_steps / s->thermo_n));
+    }
+    return check_cuda(s, "md_integrate");
+}
+
+static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t strategy, int32_t scatter) {
     if (!s) return MD_ERR_INVALID;
     if (s->sticky) return (md_status)s->sticky;
     if (!s->bound || !s->lists_valid || !s->forces_valid) return fail(s, MD_ERR_STATE, "md_integrate: needs built lists and valid forces on entry");

@@ -229,6 +229,93 @@ void md_launch_kick(md_system* s, float dt) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// S:8(f3), "the thermostat described in Ref. 27" -- reading DESIGN.md QT: Andersen-type velocity refresh.
+// One thread per slot; the random stream belongs to the ORIGINAL id (B.ids), so the result does not depend on the
+// storage order.  Philox4x32-10, key = seed words, counter = (id, application index, stream, block): block 0 word 0
+// decides by an integer comparison, block 1 gives three Gaussians by Box-Muller in fp64 (p N particles every n_newt
+// steps: fp64 here costs nothing, and the draw is then exact to the fp32 rounding of the stored velocity).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned int h0 = __umulhi(0xD2511F53u, c.x), l0 = 0xD2511F53u * c.x;
+        const unsigned int h1 = __umulhi(0xCD9E8D57u, c.z), l1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(h1 ^ c.y ^ k.x, l1, h0 ^ c.w ^ k.y, l0);
+        k.x += 0x9E3779B9u; k.y += 0xBB67AE85u;
+    }
+    return c;
+}
+
+__device__ __forceinline__ bool thermostat_draw(unsigned int id, unsigned int call, unsigned int stream, uint2 key,
+                                                unsigned long long thr, double g[3]) {
+    uint4 w = philox4x32_10(make_uint4(id, call, stream, 0u), key);
+    if (!((unsigned long long)w.x < thr)) return false;
+    w = philox4x32_10(make_uint4(id, call, stream, 1u), key);
+    const double sc = 1.0 / 4294967296.0;
+    const double u0 = ((double)w.x + 0.5) * sc, u1 = ((double)w.y + 0.5) * sc;
+    const double u2 = ((double)w.z + 0.5) * sc, u3 = ((double)w.w + 0.5) * sc;
+    const double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
+    double sn, cs, sn2, cs2;
+    sincospi(2.0 * u1, &sn, &cs);
+    sincospi(2.0 * u3, &sn2, &cs2);
+    g[0] = r0 * cs; g[1] = r0 * sn; g[2] = r1 * cs2;
+    return true;
+}
+
+template <bool RIGID, bool MIXED>
+__global__ void __launch_bounds__(256) k_thermostat(DevParams P, DevBuffers B, float4* __restrict__ vel, float4* __restrict__ angmom,
+                                                    double sv, double sl, unsigned long long thr_t, unsigned long long thr_r,
+                                                    uint2 key, unsigned int call) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.N) return;
+    const unsigned int id = (unsigned int)B.ids[i];
+    double g[3];
+    if (thermostat_draw(id, call, 0u, key, thr_t, g)) {
+        const double vx = sv * g[0], vy = sv * g[1], vz = sv * g[2];
+        float4 v = vel[i];
+        v.x = (float)vx; v.y = (float)vy; v.z = (float)vz;
+        vel[i] = v;
+        if (MIXED) {
+            reinterpret_cast<double2*>(B.shadow[2])[i] = make_double2(vx, vy);
+            reinterpret_cast<double2*>(B.shadow[3])[i] = make_double2(vz, 0.0);
+        }
+    }
+    if (RIGID) {
+        if (thermostat_draw(id, call, 1u, key, thr_r, g)) {
+            const double lx = sl * g[0], ly = sl * g[1], lz = sl * g[2];
+            float4 L = angmom[i];
+            L.x = (float)lx; L.y = (float)ly; L.z = (float)lz;
+            angmom[i] = L;
+            if (MIXED) {
+                reinterpret_cast<double2*>(B.shadow[4])[i] = make_double2(lx, ly);
+                reinterpret_cast<double2*>(B.shadow[5])[i] = make_double2(lz, 0.0);
+            }
+        }
+    }
+}
+
+static unsigned long long thermostat_threshold(double p) {
+    const double t = floor(p * 4294967296.0);
+    return t <= 0.0 ? 0ull : (t >= 4294967296.0 ? 4294967296ull : (unsigned long long)t);
+}
+
+void md_launch_thermostat(md_system* s, double T, double p_t, double p_r, unsigned long long seed, unsigned int call) {
+    const int nb = cdiv(s->P.N, 256);
+    const double sv = sqrt(T / (double)s->pot.mass), sl = s->rigid ? sqrt(T * (double)s->pot.inertia) : 0.0;
+    const unsigned long long tt = thermostat_threshold(p_t), tr = thermostat_threshold(p_r);
+    const uint2 key = make_uint2((unsigned int)(seed & 0xffffffffull), (unsigned int)(seed >> 32));
+    const bool mixed = s->precision == MD_PREC_MIXED;
+    if (s->rigid) {
+        if (mixed) k_thermostat<true, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, s->vel, s->angmom, sv, sl, tt, tr, key, call);
+        else k_thermostat<true, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, s->vel, s->angmom, sv, sl, tt, tr, key, call);
+    } else {
+        if (mixed) k_thermostat<false, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, s->vel, nullptr, sv, sl, tt, tr, key, call);
+        else k_thermostat<false, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, s->vel, nullptr, sv, sl, tt, tr, key, call);
+    }
+    s->launches += 1;
+}
+
+// ------------------------------------------------------------------------------------------------
 // S:A9 energies: fp32 per-particle terms accumulated in fp64, two deterministic stages
 // ------------------------------------------------------------------------------------------------
 #define E_THREADS 256

@@ -160,6 +160,10 @@ struct md_system {
     bool shadow_valid;                   // the fp64 copies describe the bound fp32 arrays
     double dt_d, step_dt_d;              // time step of the running / captured md_integrate in fp64 (mixed precision)
     bool graphs_off;                     // graph construction failed once: plain launches from then on
+    // thermostat (reading QT of P:53): applied by md_integrate after every thermo_n-th step since md_set_thermostat
+    int64_t thermo_n, thermo_steps;      // 0 = off; steps integrated since md_set_thermostat
+    double thermo_T, thermo_pt, thermo_pr;
+    unsigned long long thermo_seed;
 };
 
 // ---- kernel launch entry points (defined in the .cu files) ----
@@ -171,6 +175,7 @@ void md_launch_build_end(md_system* s, bool gated);
 void md_launch_forces(md_system* s, int strategy, int scatter);
 void md_launch_kick_drift(md_system* s, float dt, bool pre);   // pre: also the previous step's closing half kick
 void md_launch_kick(md_system* s, float dt);
+void md_launch_thermostat(md_system* s, double T, double p_t, double p_r, unsigned long long seed, unsigned int call);   // reading QT
 void md_launch_shadow_init(md_system* s);   // fp64 copies <- bound fp32 arrays
 void md_launch_energy(md_system* s);
 void md_launch_set_cond(md_system* s, unsigned long long cond_handle);   // conditional value = rebuild flag

@@ -433,3 +433,108 @@ def test_blocks_over_the_launch_capacity_take_the_unstaged_path(MD, oracle, case
     quat = s.in_id_order(s.quat) if w.quat is not None else None
     assert_forces(s, oracle.forces(pos, w.box, dict(w.potential), quat=quat), quat is not None)
     s.close()
+
+
+# ---- thermostat (S:8(f3); reading DESIGN.md QT, oracle O9) ----
+@pytest.mark.parametrize("order", ["none", "hilbert"])
+@pytest.mark.parametrize("prec", ["f32", "mixed"])
+def test_thermostat_one_application_matches_oracle(MD, oracle, order, prec):
+    """One application on rigid bodies over several blocks and a ragged tail: the SET of refreshed particles is the
+    oracle's exactly (integer decision), untouched entries keep their bits, refreshed ones are the oracle's fp64 draws
+    rounded to fp32 (fp64 copies: to 1e-13); independent of the storage order."""
+    w = W.patchy_fluid(2 ** 12, T=0.15)
+    T, pt, pr, seed, call = 0.4, 0.3, 0.6, (7 << 32) + 12345, 9
+    s = MD.from_workload(w, order=order)
+    s.set_precision(prec)
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    v_in, L_in = s.in_id_order(s.vel).copy(), s.in_id_order(s.angmom).copy()
+    F_in = s.in_id_order(s.force).copy()
+    ov, oL, nt, nr = oracle.thermostat(v_in[:, :3].astype(np.float64), dict(w.potential), T, pt, seed, call,
+                                       angmom_d=L_in[:, :3].astype(np.float64), p_r=pr)
+    s.thermostat(T, pt, pr, seed, call)
+    v, L = s.in_id_order(s.vel), s.in_id_order(s.angmom)
+    for got, before, ref, n in ((v, v_in, ov, nt), (L, L_in, oL, nr)):
+        changed_ref = np.any(ref != before[:, :3].astype(np.float64), axis=1)
+        changed = np.any(got[:, :3] != before[:, :3], axis=1)
+        assert changed_ref.sum() == n and 0 < n < w.N
+        assert np.array_equal(changed, changed_ref)
+        assert np.array_equal(got[~changed], before[~changed])               # bits untouched, w component included
+        assert np.array_equal(got[:, 3], before[:, 3])
+        assert np.abs(got[:, :3] - ref).max() <= 2e-7 * np.abs(ref).max()
+    assert np.array_equal(s.in_id_order(s.force), F_in)                       # forces untouched and still valid
+    if prec == "mixed":
+        _, v64 = s.state_f64()
+        assert np.abs(v64 - ov).max() <= 1e-13
+        assert np.array_equal(v64.astype(np.float32), v[:, :3])
+    K = s.energy()[1]
+    assert abs(K - 0.5 * (ov * ov).sum()) <= 1e-5 * K
+    s.close()
+
+
+def test_thermostat_p0_p1_and_small_sizes(MD, oracle):
+    """p = 0 is the identity, p = 1 refreshes everything; N below one block, one block and a ragged tail."""
+    for N in (32, 256, 500):
+        w = W.lj_fluid(N, rho=0.03)
+        s = MD.from_workload(w)
+        v_in = s.in_id_order(s.vel).copy()
+        s.thermostat(1.0, 0.0, 0.0, 3, 1)
+        assert np.array_equal(s.in_id_order(s.vel), v_in)
+        s.thermostat(1.3, 1.0, 0.0, 3, 1)
+        ov, _, nt, _ = oracle.thermostat(v_in[:, :3], dict(w.potential), 1.3, 1.0, 3, 1)
+        assert nt == w.N
+        assert np.abs(s.in_id_order(s.vel)[:, :3] - ov).max() <= 2e-7 * np.abs(ov).max()
+        s.close()
+
+
+@pytest.mark.parametrize("strat,sc", [("vertex", "smem"), ("edge", "warp")])
+def test_thermostat_nvt_trajectory_c1(MD, oracle, strat, sc):
+    """C1, 60 steps with a refresh every 20 (three applications, one inside an 8-step graph chunk boundary): same
+    tolerances as the NVE trajectory test, and the refreshed velocities of the LAST application are the oracle's."""
+    w = W.config("C1")
+    T, n_newt, pt, seed = 0.8, 20, 0.25, 424242
+    o = oracle.integrate_nvt(w.pos, w.vel, w.box, dict(w.potential), w.skin, w.dt, 60, T=T, n_newt=n_newt, p_t=pt, seed=seed)
+    s = MD.from_workload(w, order="hilbert")
+    s.build_cells(); s.build_verlet(); s.forces(strat, sc)
+    s.set_thermostat(T, n_newt, pt, 0.0, seed)
+    s.integrate(w.dt, 33, strat, sc)            # split across calls: the step count carries over
+    s.integrate(w.dt, 27, strat, sc)
+    fmax = np.abs(o["F"]).max()
+    F = s.in_id_order(s.force)
+    assert np.abs(F[:, :3] - o["F"]).max() <= FTOL_REL * fmax + FTOL_ABS
+    x = s.in_id_order(s.pos)[:, :3].astype(np.float64)
+    dx = x - o["pos"][:, :3]
+    dx -= w.box * np.round(dx / w.box)
+    assert np.abs(dx).max() < 1e-4
+    v = s.in_id_order(s.vel)[:, :3]
+    assert np.abs(v - o["vel"][:, :3]).max() < 1e-3
+    # the particles refreshed by application 3 (after step 60) carry exactly the oracle's draw
+    ov3, _, n3, _ = oracle.thermostat(np.zeros((w.N, 3)), dict(w.potential), T, pt, seed, 3)
+    hit = np.any(ov3 != 0.0, axis=1)
+    assert n3 == hit.sum() > 0
+    assert np.abs(v[hit] - ov3[hit]).max() <= 2e-7 * np.abs(ov3).max()
+    s.set_thermostat(T, 0, 0.0, 0.0, 0)         # off again: NVE
+    e0 = sum(s.energy())
+    s.integrate(w.dt, 40, strat, sc)
+    assert abs(sum(s.energy()) - e0) <= 5e-5 * abs(e0)
+    s.close()
+
+
+def test_thermostat_relaxes_a_hot_fluid_and_errors(MD):
+    from paper_1401_4350_b200 import MDError
+    w = W.lj_fluid(2 ** 14, T=2.0)
+    s = MD.from_workload(w, order="hilbert")
+    with pytest.raises(MDError) as e:
+        s.set_thermostat(-1.0, 10, 0.1)
+    assert e.value.code == -1
+    with pytest.raises(MDError) as e:
+        s.thermostat(1.0, 1.5)
+    assert e.value.code == -1
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    s.set_thermostat(1.0, 10, 0.2, 0.0, 11)
+    s.integrate(w.dt, 1200, "vertex")
+    temps = []
+    for _ in range(10):
+        s.integrate(w.dt, 20, "vertex")
+        temps.append(2.0 * s.energy()[1] / (3.0 * w.N))
+    assert abs(np.mean(temps) - 1.0) < 0.04
+    s.close()
