@@ -41,6 +41,7 @@ WORKLOAD_TEXT = {
     "C4": "BASELINE.json configs[3], patchy rigid bodies N=2^18 rho=0.5, WCA core + 4 tetrahedral patches, rc=1.5 skin=0.3",
 }
 VERTEX_VARIANTS = ["smem", "l2"]
+NVT_N_NEWT, NVT_P = 20, 0.1     # thermostat leg (reading QT of P:53): refresh every 20 steps, 10 % of the particles
 
 
 def workload(name: str):
@@ -312,6 +313,23 @@ def main():
     ms_mixed = am.elapsed_time(bm) / K
     mixed = {"ms_per_step": ms_mixed, "cost_vs_fp32": ms_mixed / (ms_total / K), "paper": "10-40 % on C2070/K10/K20 (P:59)"}
     s.set_precision("f32")
+    # S:8(f3): the same K steps under the thermostat of reading QT (NVT), reported beside; the target temperature
+    # is the kinetic temperature the system has now, so the thermostat holds the state point instead of moving it
+    s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
+    T_now = 2.0 * s.energy()[1] / (3.0 * N)
+    s.set_thermostat(T_now, NVT_N_NEWT, NVT_P, NVT_P if w.quat is not None else 0.0, 20140117)
+    s.integrate(w.dt, Wm, args.strategy, args.scatter)
+    torch.cuda.synchronize(dev)
+    an, bn = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    an.record()
+    s.integrate(w.dt, K, args.strategy, args.scatter)
+    k_nvt = s.energy()[1]
+    bn.record()
+    torch.cuda.synchronize(dev)
+    ms_nvt = an.elapsed_time(bn) / K
+    s.set_thermostat(T_now, 0, 0.0, 0.0, 0)
+    nvt = {"ms_per_step": ms_nvt, "cost_vs_nve": ms_nvt / (ms_total / K), "T_target": T_now, "T_after": 2.0 * k_nvt / (3.0 * N),
+           "n_newt": NVT_N_NEWT, "p": NVT_P, "paper": "'does not significantly affect performances' (P:53)"}
     best_edge = min((k for k in fe if k.startswith("edge")), key=lambda k: fe[k]["us"])
     peak, peak_src = measured_peaks()
     dom = args.strategy
@@ -382,7 +400,7 @@ def main():
                           "timing without a flush -- a secondary workload, the headline is C2a"),
                    "rebuilds_in_timed_region": st1["n_rebuilds"] - stw["n_rebuilds"],
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "force_eval": fe, "vertex_n3_eval": n3, "mixed_precision": mixed, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
+        "force_eval": fe, "vertex_n3_eval": n3, "mixed_precision": mixed, "thermostat": nvt, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
         "best_vertex": best_vertex,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "energy_total": sum(e_tot),
