@@ -66,6 +66,21 @@ def algorithmic_bytes(strategy: str, E: int, N: int, rigid: bool = False) -> flo
     return 8.0 * E + s_in * N + 2 * s_out * N
 
 
+def fp32_peak_tflops() -> float:
+    """148 SMs x 128 FP32 lanes x 2 flops (FMA) x SM max clock (MEASURED_PEAKS.json, else 1965 MHz)."""
+    p = ROOT / "MEASURED_PEAKS.json"
+    mhz = float(json.loads(p.read_text()).get("sm_max_mhz", 1965.0)) if p.exists() else 1965.0
+    return 148 * 128 * 2 * mhz * 1e6 / 1e12
+
+
+def algorithmic_flops(strategy: str, E: int, rigid: bool, rcut: float, rv: float) -> float:
+    """DESIGN.md 6 / SURVEY 8(d): LJ ~21 flops per visit + 18 inside the cutoff (in-cutoff share of a uniform fluid,
+    (rc/rv)^3); patchy rigid bodies ~215 flops per visit.  VERTEX visits every pair twice, EDGE once."""
+    visits = 2.0 * E if strategy == "vertex" else 1.0 * E
+    per = 215.0 if rigid else 21.0 + 18.0 * (rcut / rv) ** 3
+    return visits * per
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -347,9 +362,22 @@ def main():
             if len(f) >= 4 and f[0] == args.workload and f[1] == dom and f[2] == knames[args.scatter]:
                 traffic = float(f[3])
     kname = knames[args.scatter]
-    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
-                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
-                "algorithmic_bytes_per_launch": abytes, "us_per_launch": t_dom, "peak_source": peak_src}
+    if rigid:
+        kname = kname.replace("_lj", "_patchy")
+    # B:5: the roofline is the SLOWER of the algorithmic bytes at HBM bandwidth and the FP32 flops at peak
+    aflops = algorithmic_flops(dom, Ef, rigid, w.rcut, w.rcut + w.skin)
+    fpeak = fp32_peak_tflops()
+    t_hbm, t_alu = abytes / (peak * 1e9) * 1e6, aflops / (fpeak * 1e12) * 1e6
+    if t_alu > t_hbm:
+        ach = aflops / (t_dom * 1e-6) / 1e12
+        roofline = {"bound": "alu", "kernel": kname, "achieved": ach, "peak": fpeak, "unit": "TFLOP/s", "frac": ach / fpeak,
+                    "traffic": traffic, "algorithmic_flops_per_launch": aflops, "us_per_launch": t_dom,
+                    "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x SM max clock (DESIGN.md 6)"}
+    else:
+        roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
+                    "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                    "algorithmic_bytes_per_launch": abytes, "us_per_launch": t_dom, "peak_source": peak_src}
+    roofline["t_bound_us"] = {"hbm": t_hbm, "fp32": t_alu}
 
     # ---- end to end through the C ABI with HOST buffers (md_step_host): H2D state, build, forces, 1 step, D2H ----
     e2e = None
