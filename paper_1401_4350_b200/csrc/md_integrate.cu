@@ -246,11 +246,12 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
     return c;
 }
 
-__device__ __forceinline__ bool thermostat_draw(unsigned int id, unsigned int call, unsigned int stream, uint2 key,
-                                                unsigned long long thr, double g[3]) {
-    uint4 w = philox4x32_10(make_uint4(id, call, stream, 0u), key);
-    if (!((unsigned long long)w.x < thr)) return false;
-    w = philox4x32_10(make_uint4(id, call, stream, 1u), key);
+__device__ __forceinline__ bool thermostat_decide(unsigned int id, unsigned int call, unsigned int stream, uint2 key, unsigned long long thr) {
+    return (unsigned long long)philox4x32_10(make_uint4(id, call, stream, 0u), key).x < thr;
+}
+
+__device__ __forceinline__ void thermostat_gauss(unsigned int id, unsigned int call, unsigned int stream, uint2 key, double g[3]) {
+    const uint4 w = philox4x32_10(make_uint4(id, call, stream, 1u), key);
     const double sc = 1.0 / 4294967296.0;
     const double u0 = ((double)w.x + 0.5) * sc, u1 = ((double)w.y + 0.5) * sc;
     const double u2 = ((double)w.z + 0.5) * sc, u3 = ((double)w.w + 0.5) * sc;
@@ -259,37 +260,41 @@ __device__ __forceinline__ bool thermostat_draw(unsigned int id, unsigned int ca
     sincospi(2.0 * u1, &sn, &cs);
     sincospi(2.0 * u3, &sn2, &cs2);
     g[0] = r0 * cs; g[1] = r0 * sn; g[2] = r1 * cs2;
-    return true;
 }
 
+// Two phases per block: every thread takes the integer decisions of its slot (Philox block 0) and appends the
+// refreshed (slot, stream) to a shared-memory list; then the list is worked off with full warps, so the fp64
+// Box-Muller runs on ~p x 256 lanes instead of dragging every warp through it for its few refreshed lanes.
 template <bool RIGID, bool MIXED>
 __global__ void __launch_bounds__(256) k_thermostat(DevParams P, DevBuffers B, float4* __restrict__ vel, float4* __restrict__ angmom,
                                                     double sv, double sl, unsigned long long thr_t, unsigned long long thr_r,
                                                     uint2 key, unsigned int call) {
+    __shared__ unsigned int todo[2 * 256];   // slot | stream << 31
+    __shared__ int ntodo;
+    if (threadIdx.x == 0) ntodo = 0;
+    __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.N) return;
-    const unsigned int id = (unsigned int)B.ids[i];
-    double g[3];
-    if (thermostat_draw(id, call, 0u, key, thr_t, g)) {
-        const double vx = sv * g[0], vy = sv * g[1], vz = sv * g[2];
-        float4 v = vel[i];
-        v.x = (float)vx; v.y = (float)vy; v.z = (float)vz;
-        vel[i] = v;
-        if (MIXED) {
-            reinterpret_cast<double2*>(B.shadow[2])[i] = make_double2(vx, vy);
-            reinterpret_cast<double2*>(B.shadow[3])[i] = make_double2(vz, 0.0);
-        }
+    if (i < P.N) {
+        const unsigned int id = (unsigned int)B.ids[i];
+        if (thermostat_decide(id, call, 0u, key, thr_t)) todo[atomicAdd(&ntodo, 1)] = (unsigned int)i;
+        if (RIGID && thermostat_decide(id, call, 1u, key, thr_r)) todo[atomicAdd(&ntodo, 1)] = (unsigned int)i | 0x80000000u;
     }
-    if (RIGID) {
-        if (thermostat_draw(id, call, 1u, key, thr_r, g)) {
-            const double lx = sl * g[0], ly = sl * g[1], lz = sl * g[2];
-            float4 L = angmom[i];
-            L.x = (float)lx; L.y = (float)ly; L.z = (float)lz;
-            angmom[i] = L;
-            if (MIXED) {
-                reinterpret_cast<double2*>(B.shadow[4])[i] = make_double2(lx, ly);
-                reinterpret_cast<double2*>(B.shadow[5])[i] = make_double2(lz, 0.0);
-            }
+    __syncthreads();
+    const int n = ntodo;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) {
+        const unsigned int e = todo[k], stream = e >> 31;
+        const int slot = (int)(e & 0x7fffffffu);
+        double g[3];
+        thermostat_gauss((unsigned int)B.ids[slot], call, stream, key, g);
+        const double sc = stream ? sl : sv;
+        const double a = sc * g[0], b = sc * g[1], c = sc * g[2];
+        float4* arr = stream ? angmom : vel;
+        float4 v = arr[slot];
+        v.x = (float)a; v.y = (float)b; v.z = (float)c;
+        arr[slot] = v;
+        if (MIXED) {
+            reinterpret_cast<double2*>(B.shadow[stream ? 4 : 2])[slot] = make_double2(a, b);
+            reinterpret_cast<double2*>(B.shadow[stream ? 5 : 3])[slot] = make_double2(c, 0.0);
         }
     }
 }
