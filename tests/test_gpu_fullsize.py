@@ -97,3 +97,38 @@ def test_c2b_many_neighbours(oracle):
     # density and cutoff is done at N = 2^14 in test_step0_parity)
     assert st["n_edges"] == oracle.pair_count(w.pos, w.box, w.rcut, w.skin)
     s.close()
+
+
+@pytest.mark.parametrize("name,prec", [("C2a", "f32"), ("C4", "mixed")])
+def test_thermostat_full_size(oracle, name, prec):
+    """The thermostat (reading QT) at full size in bench.py's configuration (Hilbert-ordered storage, so the
+    id-keyed streams are read through a non-trivial permutation); O9 is O(N): every particle is compared."""
+    from paper_1401_4350_b200 import MDSystem
+    w = W.config(name)
+    rigid = w.quat is not None
+    s = MDSystem.from_workload(w, order="hilbert")
+    s.set_precision(prec)
+    s.build_cells(); s.build_verlet(); s.forces("vertex")
+    assert not np.array_equal(s.get_ids(), np.arange(w.N))
+    v0 = s.in_id_order(s.vel).copy()
+    L0 = s.in_id_order(s.angmom).copy() if rigid else None
+    T, pt, pr, seed, call = 0.7, 0.1, 0.1 if rigid else 0.0, (1 << 63) + 5, 4000000000
+    s.thermostat(T, pt, pr, seed, call)
+    ov, oL, nt, nr = oracle.thermostat(v0[:, :3].astype(np.float64), dict(w.potential), T, pt, seed, call,
+                                       angmom_d=L0[:, :3].astype(np.float64) if rigid else None, p_r=pr)
+    v1 = s.in_id_order(s.vel)
+    hit = np.any(ov != v0[:, :3], axis=1)
+    assert hit.sum() == nt and abs(nt - pt * w.N) < 5.0 * np.sqrt(w.N * pt * (1 - pt))
+    assert np.array_equal(np.any(v1[:, :3] != v0[:, :3], axis=1), hit)
+    assert np.array_equal(v1[~hit], v0[~hit])
+    assert np.abs(v1[:, :3] - ov).max() <= 2e-7 * np.abs(ov).max()
+    if rigid:
+        L1 = s.in_id_order(s.angmom)
+        hitr = np.any(oL != L0[:, :3], axis=1)
+        assert hitr.sum() == nr > 0
+        assert np.array_equal(np.any(L1[:, :3] != L0[:, :3], axis=1), hitr)
+        assert np.abs(L1[:, :3] - oL).max() <= 2e-7 * np.abs(oL).max()
+    if prec == "mixed":
+        _, v64 = s.state_f64()
+        assert np.abs(v64 - ov).max() <= 1e-13
+    s.close()
