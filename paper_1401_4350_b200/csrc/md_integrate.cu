@@ -265,31 +265,42 @@ __device__ __forceinline__ void thermostat_gauss(unsigned int id, unsigned int c
 // Two phases per block: every thread takes the integer decisions of its slot (Philox block 0) and appends the
 // refreshed (slot, stream) to a shared-memory list; then the list is worked off with full warps, so the fp64
 // Box-Muller runs on ~p x 256 lanes instead of dragging every warp through it for its few refreshed lanes.
+#define THERMO_ITEMS 4     // slots per thread: 1024 decisions per block amortise the two barriers and fill the second phase
 template <bool RIGID, bool MIXED>
 __global__ void __launch_bounds__(256) k_thermostat(DevParams P, DevBuffers B, float4* __restrict__ vel, float4* __restrict__ angmom,
                                                     double sv, double sl, unsigned long long thr_t, unsigned long long thr_r,
                                                     uint2 key, unsigned int call) {
-    __shared__ unsigned int todo[2 * 256];   // slot | stream << 31
+    __shared__ unsigned int todo[2 * 256 * THERMO_ITEMS];      // slot | stream << 31
+    __shared__ unsigned int todo_id[2 * 256 * THERMO_ITEMS];   // original id of that slot
     __shared__ int ntodo;
     if (threadIdx.x == 0) ntodo = 0;
     __syncthreads();
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < P.N) {
-        const unsigned int id = (unsigned int)B.ids[i];
-        if (thermostat_decide(id, call, 0u, key, thr_t)) todo[atomicAdd(&ntodo, 1)] = (unsigned int)i;
-        if (RIGID && thermostat_decide(id, call, 1u, key, thr_r)) todo[atomicAdd(&ntodo, 1)] = (unsigned int)i | 0x80000000u;
+#pragma unroll
+    for (int k = 0; k < THERMO_ITEMS; ++k) {
+        const int i = (blockIdx.x * THERMO_ITEMS + k) * 256 + threadIdx.x;
+        if (i < P.N) {
+            const unsigned int id = (unsigned int)B.ids[i];
+            if (thermostat_decide(id, call, 0u, key, thr_t)) {
+                const int q = atomicAdd(&ntodo, 1);
+                todo[q] = (unsigned int)i; todo_id[q] = id;
+            }
+            if (RIGID && thermostat_decide(id, call, 1u, key, thr_r)) {
+                const int q = atomicAdd(&ntodo, 1);
+                todo[q] = (unsigned int)i | 0x80000000u; todo_id[q] = id;
+            }
+        }
     }
     __syncthreads();
     const int n = ntodo;
     for (int k = threadIdx.x; k < n; k += blockDim.x) {
         const unsigned int e = todo[k], stream = e >> 31;
         const int slot = (int)(e & 0x7fffffffu);
+        float4* arr = stream ? angmom : vel;
+        float4 v = arr[slot];                  // keeps the w component; requested before the fp64 chain
         double g[3];
-        thermostat_gauss((unsigned int)B.ids[slot], call, stream, key, g);
+        thermostat_gauss(todo_id[k], call, stream, key, g);
         const double sc = stream ? sl : sv;
         const double a = sc * g[0], b = sc * g[1], c = sc * g[2];
-        float4* arr = stream ? angmom : vel;
-        float4 v = arr[slot];
         v.x = (float)a; v.y = (float)b; v.z = (float)c;
         arr[slot] = v;
         if (MIXED) {
@@ -305,7 +316,7 @@ static unsigned long long thermostat_threshold(double p) {
 }
 
 void md_launch_thermostat(md_system* s, double T, double p_t, double p_r, unsigned long long seed, unsigned int call) {
-    const int nb = cdiv(s->P.N, 256);
+    const int nb = cdiv(s->P.N, 256 * THERMO_ITEMS);
     const double sv = sqrt(T / (double)s->pot.mass), sl = s->rigid ? sqrt(T * (double)s->pot.inertia) : 0.0;
     const unsigned long long tt = thermostat_threshold(p_t), tr = thermostat_threshold(p_r);
     const uint2 key = make_uint2((unsigned int)(seed & 0xffffffffull), (unsigned int)(seed >> 32));
