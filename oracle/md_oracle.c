@@ -27,6 +27,10 @@
  *   O9  the NVT thermostat of P:53 (Ref. 27, not in the container): reading DESIGN.md QT, an Andersen-type
  *       velocity refresh driven by Philox4x32-10.  PARITY UNPINNED with respect to Ref. 27; the reading's
  *       arithmetic is pinned (see O9 below).
+ *   O10 the same sums as O1-O5 accumulated the way a CPU MD code does it: ONE thread walks the half Verlet list
+ *       (i < j) once and applies Newton's third law to both members ("single CPU core").  It exists only
+ *       as the single-core timing baseline of S:8(d); pinned against the plain definition (brute force), the fcc
+ *       lattice sums and sum F = 0.
  * Forces/torques/energies are the PLAIN DEFINITION: a direct sum over all pairs with d2 < rcut^2
  * (both strategies evaluate exactly the pairs of the Verlet list that are inside r_c).
  * The oracle's own cell list only prunes pairs that cannot be inside the cutoff; `use_cells=0`
@@ -464,6 +468,56 @@ int orc_forces(int64_t N, const float* pos3, const float* quat4, const double* b
     double* pos = to_double(pos3, 3 * N);
     double* quat = quat4 ? to_double(quat4, 4 * N) : NULL;
     int rc = orc_forces_d(N, pos, quat, box, p, use_cells, F, T, pe, n_in_cut);
+    free(pos);
+    free(quat);
+    return rc;
+}
+
+/* O10 (S:8(d) "single-threaded over its own half pair list with Newton's third law (the classic CPU inner loop)",
+ * P:41): pairs = the half Verlet list O0 (i < j, npairs rows of two ids).  Every listed pair is evaluated
+ * once; F_i += dV/dr_vec, F_j -= dV/dr_vec, half the pair energy to each, torques to each.  Bonds (O3) are walked
+ * once per bond (i, i+1).  Single-threaded by construction.  Same return value as orc_forces_d. */
+int orc_forces_half_d(int64_t N, const double* pos, const double* quat, const double* box, const orc_pot* p,
+                      const int32_t* pairs, int64_t npairs, double* F, double* T, double* pe, int64_t* n_in_cut) {
+    static const double qid[4] = { 1.0, 0.0, 0.0, 0.0 };
+    int64_t in_cut = 0;
+    int bad = 0;
+    memset(F, 0, sizeof(double) * 3 * (size_t)N);
+    if (T) memset(T, 0, sizeof(double) * 3 * (size_t)N);
+    memset(pe, 0, sizeof(double) * (size_t)N);
+    for (int64_t e = 0; e < npairs; ++e) {
+        const int64_t i = pairs[2 * e], j = pairs[2 * e + 1];
+        double rvec[3], V, dVdr[3], ti[3], tj[3];
+        const double d2 = dist2(pos + 3 * i, pos + 3 * j, box, rvec);
+        const double* qi = quat ? quat + 4 * i : qid;
+        const double* qj = quat ? quat + 4 * j : qid;
+        if (!pair_eval(p, d2, rvec, qi, qj, &V, dVdr, ti, tj)) continue;
+        ++in_cut;
+        for (int k = 0; k < 3; ++k) { F[3 * i + k] += dVdr[k]; F[3 * j + k] -= dVdr[k]; }   /* F_i = +dV/dr_vec = -F_j */
+        if (T) for (int k = 0; k < 3; ++k) { T[3 * i + k] += ti[k]; T[3 * j + k] += tj[k]; }
+        pe[i] += 0.5 * V; pe[j] += 0.5 * V;
+    }
+    if (p->kind == ORC_FENE_WCA) {
+        for (int64_t i = 0; i + 1 < N; ++i) {
+            if ((i + 1) % p->chain_len == 0) continue;
+            double rvec[3], dVdr[3];
+            const double d2 = dist2(pos + 3 * i, pos + 3 * (i + 1), box, rvec);
+            int b = 0;
+            const double V = fene_pair(d2, rvec, p->fene_K, p->fene_R0, dVdr, &b);
+            bad |= b;
+            for (int k = 0; k < 3; ++k) { F[3 * i + k] += dVdr[k]; F[3 * (i + 1) + k] -= dVdr[k]; }
+            pe[i] += 0.5 * V; pe[i + 1] += 0.5 * V;
+        }
+    }
+    if (n_in_cut) *n_in_cut = in_cut;
+    return bad;
+}
+
+int orc_forces_half(int64_t N, const float* pos3, const float* quat4, const double* box, const orc_pot* p,
+                    const int32_t* pairs, int64_t npairs, double* F, double* T, double* pe, int64_t* n_in_cut) {
+    double* pos = to_double(pos3, 3 * N);
+    double* quat = quat4 ? to_double(quat4, 4 * N) : NULL;
+    int rc = orc_forces_half_d(N, pos, quat, box, p, pairs, npairs, F, T, pe, n_in_cut);
     free(pos);
     free(quat);
     return rc;

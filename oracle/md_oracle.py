@@ -99,6 +99,8 @@ class Oracle:
         L.orc_pair_set.argtypes = [C.c_int64, _fp, _dp, C.c_double, C.c_double, C.c_int, _ip, C.c_int64]
         L.orc_forces.restype = C.c_int
         L.orc_forces.argtypes = [C.c_int64, _fp, _fp, _dp, C.POINTER(OrcPot), C.c_int, _dp, _dp, _dp, _lp]
+        L.orc_forces_half.restype = C.c_int
+        L.orc_forces_half.argtypes = [C.c_int64, _fp, _fp, _dp, C.POINTER(OrcPot), _ip, C.c_int64, _dp, _dp, _dp, _lp]
         L.orc_forces_d.restype = C.c_int
         L.orc_forces_d.argtypes = [C.c_int64, _dp, _dp, _dp, C.POINTER(OrcPot), C.c_int, _dp, _dp, _dp, _lp]
         L.orc_pair.restype = C.c_int
@@ -159,6 +161,23 @@ class Oracle:
         nin = C.c_int64(0)
         bad = self.lib.orc_forces(N, _f(p3), _f(q4), _d(box), C.byref(op), int(use_cells), _d(F), _d(T), _d(pe),
                                   C.byref(nin))
+        return dict(F=F, T=T, pe=pe, n_in_cut=int(nin.value), bad=int(bad))
+
+    def forces_half(self, pos, box, pot, pairs, quat=None):
+        """O10: the same sums by ONE thread over the half Verlet list `pairs` (int32 [E,2], i<j) with Newton's third
+        law (S:8(d) single-core baseline).  Same return dict as forces()."""
+        p3 = self._pos3(pos)
+        N = p3.shape[0]
+        box = np.ascontiguousarray(box, dtype=np.float64)
+        op = pot if isinstance(pot, OrcPot) else make_pot(pot)
+        q4 = np.ascontiguousarray(quat, dtype=np.float32) if quat is not None else None
+        pr = np.ascontiguousarray(pairs, dtype=np.int32)
+        F = np.zeros((N, 3))
+        T = np.zeros((N, 3)) if quat is not None else None
+        pe = np.zeros(N)
+        nin = C.c_int64(0)
+        bad = self.lib.orc_forces_half(N, _f(p3), _f(q4), _d(box), C.byref(op), pr.ctypes.data_as(_ip), pr.shape[0],
+                                       _d(F), _d(T), _d(pe), C.byref(nin))
         return dict(F=F, T=T, pe=pe, n_in_cut=int(nin.value), bad=int(bad))
 
     def forces_d(self, pos_d, box, pot, quat_d=None, use_cells=True):

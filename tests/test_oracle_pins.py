@@ -345,6 +345,42 @@ def test_p8_forces_brute_vs_cells(oracle, gen):
         assert np.abs(a["T"] - b["T"]).max() < 1e-12 * max(1.0, np.abs(b["T"]).max())
 
 
+# ------------------------------------------------------------------ O10: the single-core half-list loop (S:8(d))
+@pytest.mark.parametrize("gen", ["lj", "poly", "patchy"])
+def test_o10_half_list_loop_equals_the_plain_definition(oracle, gen):
+    """O10 walks the half Verlet list once with Newton's third law; the pins are the O(N^2) plain definition (no cells,
+    no list), exact momentum conservation of a pairwise antisymmetric sum, and the fcc lattice sum (closed form)."""
+    if gen == "lj":
+        w = W.lj_fluid(2048, 2.5)
+    elif gen == "poly":
+        w = W.polymer_melt(32, 64, relax_iters=20)
+    else:
+        w = W.patchy_fluid(2048, rho=0.9, jitter=0.1)
+    pairs = oracle.pair_set(w.pos, w.box, w.rcut, w.skin)
+    h = oracle.forces_half(w.pos, w.box, w.potential, pairs, quat=w.quat)
+    b = oracle.forces(w.pos, w.box, w.potential, w.quat, use_cells=False)
+    s = max(1.0, np.abs(b["F"]).max())
+    assert np.abs(h["F"] - b["F"]).max() < 1e-11 * s
+    assert np.abs(h["pe"] - b["pe"]).max() < 1e-11 * max(1.0, np.abs(b["pe"]).max())
+    assert h["n_in_cut"] == b["n_in_cut"] and h["bad"] == 0
+    if w.quat is not None:
+        assert np.abs(h["T"] - b["T"]).max() < 1e-11 * max(1.0, np.abs(b["T"]).max())
+    assert np.abs(h["F"].sum(axis=0)).max() < 1e-9 * s                  # +f and -f of every pair are the same number
+    # a dropped pair, a pair taken twice or a wrong sign changes these:
+    half = oracle.forces_half(w.pos, w.box, w.potential, pairs[::2], quat=w.quat)
+    assert np.abs(half["F"] - b["F"]).max() > 1e-3 * s
+
+
+def test_o10_fcc_lattice_sum(oracle):
+    rc, n_rc, n_rv, u_ref = [r for r in read_table("fcc_lattice_sums.txt") if r[0] == 2.5][0]
+    w = W.lj_fluid(4 * 8 ** 3, rc, jitter=0.0)
+    pairs = oracle.pair_set(w.pos, w.box, rc, 0.3)
+    h = oracle.forces_half(w.pos, w.box, w.potential, pairs)
+    assert abs(h["pe"].sum() / w.N - u_ref) < 2e-6                       # fp32-rounded lattice against the closed form
+    assert 2 * h["n_in_cut"] == w.N * int(n_rc)
+    assert np.abs(h["F"]).max() < 1e-4
+
+
 # ------------------------------------------------------------------ P7: Newton's third law (P:41)
 @pytest.mark.parametrize("gen", ["lj", "poly", "patchy"])
 def test_p7_newton3_invariants(oracle, gen):
