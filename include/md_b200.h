@@ -26,12 +26,17 @@
  *                other than MD_ORDER_NONE is set, md_build_cells() PERMUTES them in place: slot s
  *                then holds the particle whose original id is ids[s] (md_get_ids).
  *   Stream       every call enqueues on the CUDA stream given to md_create and returns without
- *                synchronising, except md_energy, md_stats, md_get_pairs, md_get_ids,
- *                md_step_host (they synchronise that stream).
+ *                synchronising, except md_energy, md_stats, md_stats_ex, md_get_pairs, md_get_ids,
+ *                md_get_state_double, md_step_host, md_probe, and md_build_verlet when a storage order is set
+ *                (it reads the size of the largest staged neighbourhood back); they synchronise that stream.
  *   Errors       every function returns an md_status (0 = success, negative = failure); the
  *                text is available from md_last_error().  Device-detected conditions (neighbour
- *                capacity overflow, FENE bond >= R0) are latched in a device flag and reported by
- *                the next synchronising call.  No partial results are defined after a failure.
+ *                capacity overflow, FENE bond >= R0) are latched in a device flag, reported ONCE by
+ *                the next synchronising call and cleared by it: after md_bind_state / a rebuild with valid
+ *                data the handle works again.  Only MD_ERR_CUDA is sticky.  No partial results are defined
+ *                after a failure.
+ *   Box          box[k] must be exactly representable in fp32 ((double)(float)box[k] == box[k]): the fp32
+ *                minimum image and the fp64 list / cutoff predicates (S:O0) then use the same box (S:Q7).
  *   Determinism  MD_VERTEX and MD_SCATTER_SEGMENTED are run-to-run bitwise reproducible; the
  *                atomic scatter variants and MD_VERTEX_N3 are not.
  */
@@ -115,6 +120,43 @@ typedef struct {
     float patch_radius, patch_exponent, core_exponent, rcut_patch; /* MD_POT_PATCHY_PP only */
 } md_potential;
 
+/* Behaviour switches of a handle (no environment variables are read by the library, S:8(b)). */
+typedef enum {
+    MD_OPT_STAGE_LIMIT = 0, /* cap (staged particles, 0 = none) on the launch capacity of the shared-memory staged VERTEX
+                               kernels: blocks with a larger neighbourhood take the unstaged path (tests of that path) */
+    MD_OPT_NO_GRAPH = 1,    /* != 0: md_integrate launches its kernels one by one instead of replaying CUDA graphs
+                               (profilers then list every kernel); same results bit for bit                          */
+    MD_OPT_DEBUG = 2        /* != 0: step-graph construction failures are printed on stderr                         */
+} md_option;
+
+/* md_probe kinds: machine ceilings other than HBM bandwidth that bound the force kernels (S:8(d)). */
+typedef enum {
+    MD_PROBE_FFMA = 0,              /* fp32 FFMA issue rate          -> TFLOP/s                                    */
+    MD_PROBE_FFMA2 = 1,             /* packed f32x2 FFMA2 issue rate -> TFLOP/s                                    */
+    MD_PROBE_MUFU = 2,              /* MUFU.EX2 rate                 -> Tops/s                                     */
+    MD_PROBE_RED_V4_SCATTER = 3,    /* red.global.add.v4.f32 to hashed particles     -> G lane-operations/s       */
+    MD_PROBE_RED_F32_SCATTER = 4,   /* red.global.add.f32 to hashed components       -> G lane-operations/s       */
+    MD_PROBE_RED_V4_COALESCED = 5,  /* red.global.add.v4.f32, consecutive lanes -> consecutive particles           */
+    MD_PROBE_RED_F32_COALESCED = 6
+} md_probe_kind;
+
+/* Extended counters of md_stats_ex (host struct, filled up to `bytes`). */
+typedef struct {
+    int64_t n_edges;            /* E = 1/2 sum |L_i| at the last build                                         */
+    int64_t n_full_entries;     /* sum |L_i|                                                                          */
+    int64_t n_rebuilds;         /* skin-triggered device-side rebuilds inside md_integrate so far                      */
+    int64_t n_in_cutoff;        /* E_in: pairs of the current list with d2 < rcut^2 at the current positions (S:Q16),
+                                   counted by a kernel of its own with the fp64 predicate of S:Q5                      */
+    int32_t max_neigh_seen;     /* max |L_i| at the last build                                                         */
+    int32_t max_stage;          /* largest staged neighbourhood (particles) of a 256-particle block at the last build  */
+    int32_t stage_launch;       /* staged-particle capacity the staged VERTEX kernels are launched with               */
+    int32_t threads_per_particle; /* 1, 2 or 4: which instantiation of the staged LJ VERTEX kernel that capacity selects
+                                   (0: the staged path is not in use)                                                  */
+    int32_t cluster_size;       /* owners per cluster of MD_SCATTER_CLUSTER (0 until that list is built)              */
+    int32_t pad0;
+    int64_t n_cluster_units;    /* (cluster, j) units of MD_SCATTER_CLUSTER = L2 reductions of its j side at most      */
+} md_stats_ex_t;
+
 /* Bytes of device workspace md_create needs for these parameters.  host pointers. */
 md_status md_workspace_bytes(int64_t N, const double box[3], double rcut, double skin,
                              const md_potential* pot, int32_t max_neigh, size_t* bytes);
@@ -124,7 +166,8 @@ md_status md_workspace_bytes(int64_t N, const double box[3], double rcut, double
  * aligned, workspace_bytes >= md_workspace_bytes(...), owned by the caller and borrowed until
  * md_destroy.  cuda_stream: a cudaStream_t (may be NULL for the legacy default stream).
  * max_neigh: capacity of every L_i (rounded up to a multiple of 4), at most 480.
- * MD_ERR_INVALID if N <= 0, max_neigh > 480, N*max_neigh >= 2^31, box[k] < 2 (rcut + 2 skin), bad potential. */
+ * MD_ERR_INVALID if N <= 0, max_neigh > 480, N*max_neigh >= 2^31, box[k] < 2 (rcut + 2 skin), box[k] not exactly
+ * representable in fp32, bad potential. */
 md_status md_create(md_system** out, int64_t N, const double box[3], double rcut, double skin,
                     const md_potential* pot, int32_t max_neigh, void* workspace, size_t workspace_bytes,
                     void* cuda_stream);
@@ -194,6 +237,18 @@ md_status md_energy(md_system*, double* e_pot, double* e_kin_trans, double* e_ki
 /* Counters (host pointers, any may be NULL).  n_edges = E = 1/2 sum |L_i|. Synchronises. */
 md_status md_stats(md_system*, int64_t* n_edges, int64_t* n_full_entries, int32_t* max_neigh_seen,
                    int64_t* n_rebuilds);
+
+/* md_stats plus the counters above; `bytes` = sizeof(md_stats_ex_t) of the caller.  Needs built lists for n_in_cutoff
+ * (else that field is -1).  Synchronises. */
+md_status md_stats_ex(md_system*, md_stats_ex_t* out, size_t bytes);
+
+/* Set a behaviour switch (md_option).  MD_ERR_INVALID for an unknown option or a negative value. */
+md_status md_set_option(md_system*, int32_t option, int64_t value);
+
+/* Measure one machine ceiling (md_probe_kind) on the handle's device and stream; *value (host) in the unit listed with
+ * the kind.  Uses the permutation scratch of the workspace: lists, cells and forces stay valid, a state reordering in
+ * flight does not exist (the call synchronises before and after).  ~10 ms. */
+md_status md_probe(md_system*, int32_t kind, double* value);
 
 /* Copy the half list to the HOST as pairs of ORIGINAL ids (lo, hi), unsorted. pairs_host has room for
  * `capacity` pairs (2 int32 each); *n receives the pair count (even if > capacity). Synchronises. */

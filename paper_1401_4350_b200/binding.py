@@ -15,6 +15,9 @@ SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3}
 GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
 PRECISION = {"f32": 0, "mixed": 1}
+OPTION = {"stage_limit": 0, "no_graph": 1, "debug": 2}
+PROBE = {"ffma": 0, "ffma2": 1, "mufu": 2, "red_v4_scatter": 3, "red_f32_scatter": 4, "red_v4_coalesced": 5,
+         "red_f32_coalesced": 6}
 POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2, "patchy_pp": 3}
 STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPACITY", -4: "MD_ERR_CUDA",
           -5: "MD_ERR_NUMERIC"}
@@ -22,8 +25,9 @@ STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPA
 # every symbol include/md_b200.h declares (checked by tests/test_abi.py against the header and the .so)
 EXPORTED_SYMBOLS = ["md_workspace_bytes", "md_create", "md_bind_state", "md_set_order", "md_set_precision",
                     "md_get_state_double", "md_set_thermostat", "md_thermostat", "md_build_cells",
-                    "md_build_verlet", "md_forces", "md_integrate", "md_energy", "md_stats", "md_get_pairs",
-                    "md_get_ids", "md_step_host", "md_launch_count", "md_last_error", "md_destroy"]
+                    "md_build_verlet", "md_forces", "md_integrate", "md_energy", "md_stats", "md_stats_ex",
+                    "md_set_option", "md_probe", "md_get_pairs", "md_get_ids", "md_step_host", "md_launch_count",
+                    "md_last_error", "md_destroy"]
 
 
 class MDError(RuntimeError):
@@ -47,6 +51,13 @@ class MDPotential(C.Structure):
         ("patch_radius", C.c_float), ("patch_exponent", C.c_float), ("core_exponent", C.c_float),
         ("rcut_patch", C.c_float),
     ]
+
+
+class MDStatsEx(C.Structure):
+    _fields_ = [("n_edges", C.c_int64), ("n_full_entries", C.c_int64), ("n_rebuilds", C.c_int64),
+                ("n_in_cutoff", C.c_int64), ("max_neigh_seen", C.c_int32), ("max_stage", C.c_int32),
+                ("stage_launch", C.c_int32), ("threads_per_particle", C.c_int32), ("cluster_size", C.c_int32),
+                ("pad0", C.c_int32), ("n_cluster_units", C.c_int64)]
 
 
 def make_potential(d: dict) -> MDPotential:
@@ -123,6 +134,12 @@ def load_library() -> C.CDLL:
     L.md_energy.argtypes = [vp, dp3, dp3, dp3]
     L.md_stats.restype = C.c_int
     L.md_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
+    L.md_stats_ex.restype = C.c_int
+    L.md_stats_ex.argtypes = [vp, C.POINTER(MDStatsEx), C.c_size_t]
+    L.md_set_option.restype = C.c_int
+    L.md_set_option.argtypes = [vp, C.c_int32, C.c_int64]
+    L.md_probe.restype = C.c_int
+    L.md_probe.argtypes = [vp, C.c_int32, dp3]
     L.md_get_pairs.restype = C.c_int
     L.md_get_pairs.argtypes = [vp, C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int64)]
     L.md_get_ids.restype = C.c_int
@@ -280,6 +297,20 @@ class MDSystem:
         mx = C.c_int32(0)
         self._check(self.lib.md_stats(self.h, C.byref(ne), C.byref(nf), C.byref(mx), C.byref(nr)))
         return dict(n_edges=ne.value, n_full_entries=nf.value, max_neigh_seen=mx.value, n_rebuilds=nr.value)
+
+    def stats_ex(self):
+        r = MDStatsEx()
+        self._check(self.lib.md_stats_ex(self.h, C.byref(r), C.sizeof(r)))
+        return {k: getattr(r, k) for k, _ in MDStatsEx._fields_ if k != "pad0"}
+
+    def set_option(self, option, value):
+        self._check(self.lib.md_set_option(self.h, OPTION[option] if isinstance(option, str) else int(option), int(value)))
+
+    def probe(self, kind) -> float:
+        """One machine ceiling measured on this device (md_probe_kind): TFLOP/s, Tops/s or G lane-operations/s."""
+        v = C.c_double(0)
+        self._check(self.lib.md_probe(self.h, PROBE[kind] if isinstance(kind, str) else int(kind), C.byref(v)))
+        return v.value
 
     def get_pairs(self) -> np.ndarray:
         """Half list as ORIGINAL-id pairs (lo, hi), int32 [E,2], unsorted."""

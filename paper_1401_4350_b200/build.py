@@ -9,7 +9,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libmd_b200.so"
-SOURCES = ["md_api.cu", "md_build.cu", "md_forces.cu", "md_staged.cu", "md_integrate.cu"]
+SOURCES = ["md_api.cu", "md_build.cu", "md_forces.cu", "md_staged.cu", "md_integrate.cu", "md_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"]
 
@@ -25,40 +25,36 @@ def needs_build() -> bool:
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime
-    deps = [CSRC / f for f in SOURCES] + [CSRC / "md_internal.cuh", CSRC / "md_pair.cuh", ROOT / "include" / "md_b200.h"]
+    deps = [CSRC / f for f in SOURCES] + sorted(CSRC.glob("*.cuh")) + [ROOT / "include" / "md_b200.h"]
     return any(d.stat().st_mtime > t for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
-    objs = []
-    for src in SOURCES:
+    from concurrent.futures import ThreadPoolExecutor
+
+    def compile_one(src):
         obj = CSRC / (src[:-3] + ".o")
         cmd = [_nvcc(), *NVCC_FLAGS, "-I", str(ROOT / "include"), "-I", str(CSRC), "-c", str(CSRC / src), "-o", str(obj)]
         r = subprocess.run(cmd, capture_output=True, text=True)
+        return src, str(obj), r
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as ex:
+        results = list(ex.map(compile_one, SOURCES))
+    objs = []
+    for src, obj, r in results:
         if verbose or r.returncode != 0:
             print(r.stdout, r.stderr)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed on {src}")
-        objs.append(str(obj))
+        objs.append(obj)
     cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(LIB), *objs]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         print(r.stdout, r.stderr)
         raise RuntimeError("nvcc link failed")
     return LIB
-
-
-def build_microbench() -> Path:
-    """Stand-alone micro-benchmark of the non-HBM ceilings (csrc/microbench.cu -> microbench, not part of the library)."""
-    exe = PKG / "microbench"
-    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-o", str(exe), str(CSRC / "microbench.cu")]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        print(r.stdout, r.stderr)
-        raise RuntimeError("nvcc failed on microbench.cu")
-    return exe
 
 
 if __name__ == "__main__":

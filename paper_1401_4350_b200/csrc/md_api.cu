@@ -27,6 +27,7 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
     g->ncell = 1;
     for (int k = 0; k < 3; ++k) {
         if (!(box[k] > 0) || box[k] < 2.0 * (rcut + 2.0 * skin)) return false;
+        if ((double)(float)box[k] != box[k]) return false;   // S:Q7: fp32 minimum image and fp64 predicates share one box
         int n = (int)floor(box[k] / (rv * (1.0 + 1e-5)));
         g->nc[k] = n < 1 ? 1 : n;
         g->ncell *= g->nc[k];
@@ -91,7 +92,6 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.scan_blk = (unsigned int*)take(4 * nscan);
     b.e_part = (double*)take(8 * 3 * 2048);
     b.e_out = (double*)take(8 * 4);
-    b.stage4 = (float4*)take(16 * Npad);
     b.cell_lin = (int*)take(4 * (size_t)g.ncell);
     b.rows = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)g.rcap);
     b.rows_tmp = (unsigned short*)take(2 * (size_t)g.nblk * MD_TB * (size_t)(8 * ((g.rcap + 2) / 2) + g.rcap + 2));   // 8 column buckets + list form
@@ -199,14 +199,8 @@ void upload_cell_rank(md_system* s, const std::vector<int>& rank) {
     cudaStreamSynchronize(s->stream);   // host temporaries
 }
 
-// slot s holds original id s (state arrays given in original id order)
-void reset_ids(md_system* s) {
-    std::vector<int> iden((size_t)s->N);
-    for (int64_t i = 0; i < s->N; ++i) iden[(size_t)i] = (int)i;
-    cudaMemcpyAsync(s->B.ids, iden.data(), 4 * (size_t)s->N, cudaMemcpyHostToDevice, s->stream);
-    cudaMemcpyAsync(s->B.slot_of_id, iden.data(), 4 * (size_t)s->N, cudaMemcpyHostToDevice, s->stream);
-    cudaStreamSynchronize(s->stream);   // iden is a host temporary
-}
+// slot s holds original id s (state arrays given in original id order): a kernel, no host temporaries, no synchronisation
+void reset_ids(md_system* s) { md_launch_iota_ids(s); }
 
 // synchronise and surface latched device errors
 md_status sync_and_check(md_system* s, const char* where) {
@@ -218,15 +212,22 @@ md_status sync_and_check(md_system* s, const char* where) {
         s->sticky = MD_ERR_CUDA;
         return MD_ERR_CUDA;
     }
+    if (c.err) {
+        // latched device conditions are reported once and cleared (the header documents only MD_ERR_CUDA as sticky):
+        // after md_bind_state / a rebuild with valid data the handle works again
+        cudaMemsetAsync(&s->B.ctrl->err, 0, sizeof(int), s->stream);
+    }
     if (c.err & MD_DEVERR_CAPACITY) {
         snprintf(s->errmsg, sizeof(s->errmsg), "neighbour capacity exceeded: a particle has %d Verlet neighbours, max_neigh = %d", c.max_seen, s->P.cap);
-        s->lists_valid = false;
+        s->lists_valid = s->staged_valid = s->legacy_valid = s->cluster_valid = false;
+        s->forces_valid = false;
         return MD_ERR_CAPACITY;
     }
     if (c.err & MD_DEVERR_STAGE) {
         snprintf(s->errmsg, sizeof(s->errmsg), "staged build capacity exceeded: a block needs %d staged particles / %d segments "
                  "(build capacity %d, segment capacity %d)", c.max_stage, c.max_seg, s->P.stage_cap, MD_SEGMAX);
         s->lists_valid = s->staged_valid = false;
+        s->forces_valid = false;
         return MD_ERR_CAPACITY;
     }
     s->n_edges_host = (long long)c.n_edges;
@@ -235,10 +236,11 @@ md_status sync_and_check(md_system* s, const char* where) {
         // device-side rebuilds that happen before the next synchronising call; if that head room alone costs a
         // resident block per SM, keep only as much of it as still fits the block count of a tight (4 %) fit
         // (30 % for systems of fewer blocks than SMs: their maximum fluctuates more and occupancy does not matter there)
-        int want = (int)(c.max_stage * (s->P.nblk >= 148 ? 1.15 : 1.30)) + 64;
+        const int sms = s->sm_count;
+        int want = (int)(c.max_stage * (s->P.nblk >= sms ? 1.15 : 1.30)) + 64;
         want = (want + 63) / 64 * 64;
         want = std::min(want, ((int)s->N + 1 + 63) / 64 * 64);   // a neighbourhood never holds more than the whole system
-        const size_t per_entry = s->rigid ? 32 : 16, sm_bytes = 228 * 1024, xch = s->rigid ? 0 : 24 * MD_TB;
+        const size_t per_entry = s->rigid ? 32 : 16, sm_bytes = s->smem_per_sm, xch = s->rigid ? 0 : 24 * MD_TB;
         auto per_block = [&](int se) {
             size_t b = 16 + per_entry * (size_t)se;
             if (b > 75 * 1024) b += xch;
@@ -247,14 +249,14 @@ md_status sync_and_check(md_system* s, const char* where) {
         const int tight = ((int)(c.max_stage * 1.04) + 32 + 63) / 64 * 64;
         const int nb_t = (int)std::min<size_t>(4, sm_bytes / per_block(tight)), nb_w = (int)std::min<size_t>(4, sm_bytes / per_block(want));
         // only where it matters and where the maximum over blocks is statistically stable: at least one block per SM
-        if (nb_t == nb_w && nb_w >= 1 && nb_w <= 4 && s->P.nblk >= 148) {
+        if (nb_t == nb_w && nb_w >= 1 && nb_w <= 4 && s->P.nblk >= sms) {
             // head room that costs nothing: up to 30 % if the same number of blocks stays resident
             size_t budget = sm_bytes / nb_w - 1024 - 16;
             if (budget > 75 * 1024 + xch) budget -= xch;
             const int fit = (int)(budget / per_entry) / 64 * 64;
             const int roomy = ((int)(c.max_stage * 1.30) + 64 + 63) / 64 * 64;
             if (fit > want && per_block(std::min(fit, roomy)) * nb_w <= sm_bytes) want = std::min(fit, roomy);
-        } else if (nb_t > nb_w && s->P.nblk >= 148) {
+        } else if (nb_t > nb_w && s->P.nblk >= sms) {
             size_t budget = sm_bytes / nb_t - 1024 - 16;
             if (budget > 75 * 1024 + xch) budget -= xch;
             const int fit = (int)(budget / per_entry) / 64 * 64;
@@ -264,6 +266,7 @@ md_status sync_and_check(md_system* s, const char* where) {
     }
     if (c.err & MD_DEVERR_FENE) {
         snprintf(s->errmsg, sizeof(s->errmsg), "FENE bond length reached R0");
+        s->forces_valid = false;
         return MD_ERR_NUMERIC;
     }
     return MD_OK;
@@ -324,7 +327,18 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);
     s->stage_launch = P.stage_cap;
-    s->stage_limit = getenv("MD_B200_STAGE_LIMIT") ? atoi(getenv("MD_B200_STAGE_LIMIT")) : 0;
+    s->stage_limit = 0;
+    {   // the device the handle lives on: SM count and shared-memory sizes come from its properties, not from literals
+        cudaDeviceProp prop;
+        if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) { cudaGetLastError(); free(s); return MD_ERR_CUDA; }
+        s->sm_count = prop.multiProcessorCount;
+        s->smem_per_sm = prop.sharedMemPerMultiprocessor;
+        s->smem_optin = std::min<size_t>(prop.sharedMemPerBlockOptin, 224 * 1024);   // the workspace was sized for <= 224 KB per block
+        if (s->smem_optin < 96 * 1024) { free(s); return MD_ERR_INVALID; }            // not a device this library was written for
+        P.stage_cap = (int)((s->smem_optin - 16) / (rigid ? 32 : 16)) - 1;
+        s->stage_launch = P.stage_cap;
+        md_staged_configure(s);
+    }
     P.kind = rigid ? MD_POT_PATCHY : pot->kind;   // both rigid-body models run on the same kernels (P.pp_model tells them apart)
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
     P.sigma = pot->sigma;
@@ -545,7 +559,7 @@ static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatt
 // a dozen gated no-op kernels per step.  Returns false (and leaves no graph) if any graph call fails.
 #define GCHK(call) do { if (ok) { cudaError_t e_ = (call); if (e_ != cudaSuccess) { ok = false; \
     snprintf(s->errmsg, sizeof(s->errmsg), "step graph: %s -> %s", #call, cudaGetErrorString(e_)); \
-    if (getenv("MD_B200_DEBUG")) fprintf(stderr, "%s\n", s->errmsg); } } } while (0)
+    if (s->debug) fprintf(stderr, "%s\n", s->errmsg); } } } while (0)
 static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t scatter, bool staged, bool seg, int reps,
                              cudaGraphExec_t* exec_out, int* nodes_out) {
     // capture happens on two internal streams (the caller's stream may be the legacy default stream, which cannot be
@@ -565,6 +579,7 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     const cudaGraphNode_t* deps = nullptr;
     size_t ndeps = 0;
     int tail_nodes = 0, main_nodes = 0;
+    bool aux_open = false;
     for (int rep_i = 0; rep_i < reps && ok; ++rep_i) {   // `reps` consecutive steps in one graph, one IF node each
     cudaGraphConditionalHandle handle = 0;
     GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
@@ -586,6 +601,7 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
             cudaGraph_t body = np.conditional.phGraph_out[0];
             GCHK(cudaStreamBeginCaptureToGraph(s->aux_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
             if (ok) {
+                aux_open = true;
                 s->stream = s->aux_stream;
                 md_launch_build_cells(s, true);
                 if (staged) md_launch_build_staged(s, true);
@@ -594,7 +610,9 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
                 md_launch_build_end(s, true);
                 s->stream = main_stream;
                 cudaGraph_t tmp = nullptr;
-                GCHK(cudaStreamEndCapture(s->aux_stream, &tmp));
+                aux_open = false;       // ended here whatever the outcome
+                { cudaError_t e_ = cudaStreamEndCapture(s->aux_stream, &tmp); if (e_ != cudaSuccess && ok) { ok = false;
+                    snprintf(s->errmsg, sizeof(s->errmsg), "step graph: end of body capture -> %s", cudaGetErrorString(e_)); } }
             }
         }
         GCHK(cudaStreamUpdateCaptureDependencies(main_stream, &cond_node, 1, cudaStreamSetCaptureDependencies));
@@ -607,7 +625,12 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     tail_nodes = (int)(s->launches - before_tail);
     main_nodes += 2 + tail_nodes;   // kernels outside the conditional body
     }
-    { cudaError_t e_ = cudaStreamEndCapture(main_stream, &graph); if (e_ != cudaSuccess) { if (ok && getenv("MD_B200_DEBUG")) fprintf(stderr, "step graph: end capture -> %s\n", cudaGetErrorString(e_)); ok = false; } }
+    if (aux_open) {   // a failure while the body capture was open: close it, or aux_stream stays in capture mode for good
+        cudaGraph_t tmp = nullptr;
+        cudaStreamEndCapture(s->aux_stream, &tmp);
+        aux_open = false;
+    }
+    { cudaError_t e_ = cudaStreamEndCapture(main_stream, &graph); if (e_ != cudaSuccess) { if (ok && s->debug) fprintf(stderr, "step graph: end capture -> %s\n", cudaGetErrorString(e_)); ok = false; } }
     s->launches = launches0;
     s->stream = user_stream;
     GCHK(cudaGraphInstantiate(exec_out, graph, 0));
@@ -694,8 +717,7 @@ static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t 
     s->dt_d = dt;
     ensure_shadows(s);
     int64_t k0 = 0;
-    if (!s->graphs_off && getenv("MD_B200_NO_GRAPH")) s->graphs_off = true;   // plain launches (profilers list every kernel)
-    if (!s->graphs_off && nsteps > 0) {
+    if (!s->graphs_off && !s->no_graph && nsteps > 0) {   // MD_OPT_NO_GRAPH: plain launches (profilers list every kernel)
         if (!s->step_exec || s->step_strategy != strategy || s->step_variant != scatter || s->step_dt != fdt ||
             s->step_dt_d != dt || s->step_stage != s->stage_launch) {
             drop_step_graph(s);
@@ -756,6 +778,57 @@ md_status md_stats(md_system* s, int64_t* n_edges, int64_t* n_full_entries, int3
     if (max_neigh_seen) *max_neigh_seen = c.max_seen;
     if (n_rebuilds) *n_rebuilds = c.n_rebuilds;
     return st;
+}
+
+md_status md_stats_ex(md_system* s, md_stats_ex_t* out, size_t bytes) {
+    if (!s || !out || bytes == 0) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    const bool have_lists = s->bound && s->lists_valid;
+    if (have_lists) {
+        ensure_explicit(s);
+        md_launch_count_in_cutoff(s);
+    }
+    DevCtrl c;
+    cudaMemcpyAsync(&c, s->B.ctrl, sizeof(c), cudaMemcpyDeviceToHost, s->stream);
+    md_status st = sync_and_check(s, "md_stats_ex");
+    md_stats_ex_t r;
+    memset(&r, 0, sizeof(r));
+    r.n_edges = c.n_edges; r.n_full_entries = (int64_t)c.n_full; r.n_rebuilds = c.n_rebuilds;
+    r.n_in_cutoff = have_lists ? (int64_t)c.n_in : -1;
+    r.max_neigh_seen = c.max_seen; r.max_stage = c.max_stage; r.stage_launch = s->stage_launch;
+    r.threads_per_particle = s->staged_valid ? md_staged_threads_per_particle(s) : 0;
+    r.cluster_size = s->cluster_valid ? MD_CLUSTER : 0;
+    r.n_cluster_units = s->cluster_valid ? (int64_t)c.n_units : 0;
+    memcpy(out, &r, bytes < sizeof(r) ? bytes : sizeof(r));
+    return st;
+}
+
+md_status md_set_option(md_system* s, int32_t option, int64_t value) {
+    if (!s) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (value < 0) return fail(s, MD_ERR_INVALID, "md_set_option: negative value");
+    switch (option) {
+    case MD_OPT_STAGE_LIMIT:
+        s->stage_limit = (int)std::min<int64_t>(value, 1 << 30);
+        drop_step_graph(s);            // the step graph bakes the launch capacity in
+        return MD_OK;
+    case MD_OPT_NO_GRAPH: s->no_graph = value != 0; return MD_OK;
+    case MD_OPT_DEBUG: s->debug = value != 0; return MD_OK;
+    default: return fail(s, MD_ERR_INVALID, "md_set_option: unknown option");
+    }
+}
+
+md_status md_probe(md_system* s, int32_t kind, double* value) {
+    if (!s || !value) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    if (kind < MD_PROBE_FFMA || kind > MD_PROBE_RED_F32_COALESCED) return fail(s, MD_ERR_INVALID, "md_probe: unknown kind");
+    cudaStreamSynchronize(s->stream);
+    if (!md_run_probe(s, kind, value)) {
+        md_status st = check_cuda(s, "md_probe");
+        return st != MD_OK ? st : fail(s, MD_ERR_INVALID, "md_probe: the system is too small to hold the probe's scratch");
+    }
+    s->launches += 4;
+    return check_cuda(s, "md_probe");
 }
 
 md_status md_get_ids(md_system* s, int32_t* ids_host) {
@@ -819,13 +892,16 @@ md_status md_step_host(md_system* s, void* pos_host, void* vel_host, void* force
     if (nsteps > 0 && (st = md_integrate(s, dt, nsteps, strategy, scatter)) != MD_OK) return st;
     struct { float4* dev; void* host; } outs[6] = { { s->pos, pos_host }, { s->vel, vel_host }, { s->force, force_host },
                                                     { s->quat, quat_host }, { s->angmom, angmom_host }, { s->torque, torque_host } };
+    // back to ORIGINAL id order: every array goes through its own plane of the permutation scratch, so the un-permute
+    // kernels and the device->host copies queue back to back with no dependency between arrays
+    const size_t plane = (size_t)s->P.ntiles * MD_TILE;
     for (int k = 0; k < 6; ++k) {
         if (!outs[k].dev || !outs[k].host) continue;
         if (s->order == MD_ORDER_NONE) {
             cudaMemcpyAsync(outs[k].host, outs[k].dev, bytes, cudaMemcpyDeviceToHost, s->stream);
         } else {
-            md_launch_unpermute(s, outs[k].dev, s->B.stage4);
-            cudaMemcpyAsync(outs[k].host, s->B.stage4, bytes, cudaMemcpyDeviceToHost, s->stream);
+            md_launch_unpermute(s, outs[k].dev, s->B.tmp4 + (size_t)k * plane);
+            cudaMemcpyAsync(outs[k].host, s->B.tmp4 + (size_t)k * plane, bytes, cudaMemcpyDeviceToHost, s->stream);
         }
     }
     return sync_and_check(s, "md_step_host");

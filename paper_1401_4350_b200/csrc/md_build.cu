@@ -421,6 +421,16 @@ void md_launch_seg_index(md_system* s, bool gated) {
     s->launches += 1;
 }
 
+// slot s holds original id s
+__global__ void k_iota_ids(DevParams P, DevBuffers B) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < P.N) { B.ids[i] = i; B.slot_of_id[i] = i; }
+}
+void md_launch_iota_ids(md_system* s) {
+    k_iota_ids<<<cdiv(s->P.N, 256), 256, 0, s->stream>>>(s->P, s->B);
+    s->launches += 1;
+}
+
 // dst[ids[s]] = src[s]  (slot order -> original id order)
 __global__ void k_unpermute(DevParams P, DevBuffers B, const float4* src, float4* dst) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;

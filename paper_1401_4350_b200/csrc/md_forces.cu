@@ -479,6 +479,27 @@ static void launch_vertex_n3(md_system* s, int m) {
     }
 }
 
+// E_in (S:Q16): pairs of the explicit edge list inside the cutoff at the current positions, by the decision every force
+// kernel takes (fp32 away from the threshold, the fp64 predicate of S:Q5 inside the band) -> ctrl->n_in
+__global__ void __launch_bounds__(256) k_count_in_cutoff(DevParams P, DevBuffers B, const float4* __restrict__ pos) {
+    const unsigned int E = B.ctrl->n_edges;
+    const unsigned int stride = gridDim.x * blockDim.x;
+    unsigned int n = 0;
+    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < E; e += stride) {
+        const int2 ij = B.edges[e];
+        float dx, dy, dz, d2;
+        n += edge_test(P, pos, ij.x, ij.y, dx, dy, dz, d2) ? 1u : 0u;
+    }
+    n = __reduce_add_sync(0xffffffffu, n);
+    if ((threadIdx.x & 31) == 0 && n) atomicAdd(&B.ctrl->n_in, (unsigned long long)n);
+}
+
+void md_launch_count_in_cutoff(md_system* s) {
+    cudaMemsetAsync(&s->B.ctrl->n_in, 0, sizeof(unsigned long long), s->stream);
+    k_count_in_cutoff<<<s->sm_count * 8, 256, 0, s->stream>>>(s->P, s->B, s->pos);
+    s->launches += 1;
+}
+
 // ------------------------------------------------------------------------------------------------
 // host-side dispatch
 // ------------------------------------------------------------------------------------------------
@@ -486,7 +507,7 @@ template <int KIND>
 static void launch_edge(md_system* s, int scatter) {
     const DevParams& P = s->P;
     const int nbN = cdiv(P.N, 256);
-    const int persistent = 148 * 8;   // 8 CTAs of 256 threads per SM, grid-stride over the device-resident edge count
+    const int persistent = s->sm_count * 8;   // 8 CTAs of 256 threads per SM, grid-stride over the device-resident edge count
     float4* tq = md_is_rigid(KIND) ? s->torque : nullptr;
     if (scatter == MD_SCATTER_SEGMENTED) {
         k_edge_store<KIND><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat);

@@ -335,7 +335,7 @@ void md_launch_thermostat(md_system* s, double T, double p_t, double p_r, unsign
 // S:A9 energies: fp32 per-particle terms accumulated in fp64, two deterministic stages
 // ------------------------------------------------------------------------------------------------
 #define E_THREADS 256
-#define E_BLOCKS 1184   // 148 SMs x 8
+#define E_BLOCKS 2048   // capacity of the partial-sum table (md_api.cu carve: e_part); the launch uses 8 blocks per SM
 
 __device__ __forceinline__ double block_sum(double v, double* sh) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -388,6 +388,7 @@ __global__ void __launch_bounds__(E_THREADS) k_energy_final(DevParams P, DevBuff
 
 void md_launch_energy(md_system* s) {
     int nb = cdiv(s->P.N, E_THREADS);
+    if (nb > s->sm_count * 8) nb = s->sm_count * 8;
     if (nb > E_BLOCKS) nb = E_BLOCKS;
     k_energy_partial<<<nb, E_THREADS, 0, s->stream>>>(s->P, s->B, s->vel, s->force, s->rigid ? s->angmom : nullptr);
     k_energy_final<<<1, E_THREADS, 0, s->stream>>>(s->P, s->B, nb);

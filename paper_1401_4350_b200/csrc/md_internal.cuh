@@ -9,6 +9,7 @@
 #define MD_TILE 32            // particles per list tile (one warp)
 #define MD_MAX_PATCH 8
 #define MD_GRAPH_STEPS 8        // steps per launch of the multi-step graph of md_integrate
+#define MD_CLUSTER 16           // owners per cluster of MD_SCATTER_CLUSTER (one 16-bit mask per (cluster, j) unit)
 
 // Device error bits latched in DevCtrl::err
 #define MD_DEVERR_CAPACITY 1
@@ -38,7 +39,9 @@ struct DevCtrl {
     unsigned int scan_total;     // scratch for the scan kernels
     int max_stage;               // largest staged neighbourhood (particles) over the blocks at the last staged build
     int max_seg;                 // largest segment count
-    int pad[5];
+    int pad1;
+    unsigned long long n_in;     // E_in: listed pairs inside the cutoff at the current positions (md_stats_ex)
+    unsigned long long n_units;  // (cluster, j) units of the cluster list (MD_SCATTER_CLUSTER)
 };
 
 // per-block header of the staged path
@@ -112,7 +115,6 @@ struct DevBuffers {
     unsigned int* scan_blk;// [scan blocks]
     double* e_part;        // [e_blocks*3]
     double* e_out;         // [3]
-    float4* stage4;        // [N] staging for md_step_host un-permute
     // staged path
     int* cell_lin;         // [ncell] storage rank -> linear cell index (inverse of cell_rank)
     unsigned short* rows;  // [nblk][rcap/4][MD_TB] x 4 u16: Verlet rows of block-local indices, block-transposed chunks of 4
@@ -141,7 +143,12 @@ struct md_system {
     float4 *pos, *vel, *force, *quat, *angmom, *torque;
     bool bound, cells_valid, lists_valid, forces_valid, seg_valid;
     bool staged_valid, legacy_valid;   // which list representations describe the current build
-    int stage_limit;         // MD_B200_STAGE_LIMIT: cap on the staged launch capacity (0 = none; tests of the unstaged path)
+    bool cluster_valid;                // the (cluster, j) unit list of MD_SCATTER_CLUSTER describes the current build
+    int stage_limit;         // MD_OPT_STAGE_LIMIT: cap on the staged launch capacity (0 = none; tests of the unstaged path)
+    bool no_graph, debug;    // MD_OPT_NO_GRAPH, MD_OPT_DEBUG
+    int device, sm_count;    // the device the handle was created on and its SM count (cudaDeviceProp)
+    size_t smem_optin, smem_per_sm;   // largest opt-in dynamic shared memory per block / shared memory per SM of that device
+    int build_carve;         // shared-memory carveout k_build_staged was last configured with on this device (-1 = none)
     long long n_edges_host;  // E at the last synchronising call (0 before the first): picks the EDGE slice width
     int stage_launch;        // staged-particle capacity the force kernels are launched with (from the last synchronised build)
     int64_t launches;
@@ -180,6 +187,11 @@ void md_launch_shadow_init(md_system* s);   // fp64 copies <- bound fp32 arrays
 void md_launch_energy(md_system* s);
 void md_launch_set_cond(md_system* s, unsigned long long cond_handle);   // conditional value = rebuild flag
 void md_launch_unpermute(md_system* s, const float4* src, float4* dst);   // dst[ids[s]] = src[s]
+void md_launch_iota_ids(md_system* s);                                    // ids[s] = slot_of_id[s] = s
+void md_launch_count_in_cutoff(md_system* s);                             // ctrl->n_in from the explicit edge list
+void md_staged_configure(md_system* s);                                   // per-device kernel attributes of md_staged.cu
+int md_staged_threads_per_particle(const md_system* s);                   // NS the staged LJ launch would use (0: rigid)
+bool md_run_probe(md_system* s, int kind, double* value);                 // md_probe.cu
 // staged path (md_staged.cu)
 void md_launch_build_staged(md_system* s, bool gated);
 void md_launch_edges_from_rows(md_system* s);     // explicit (i, j) edge list from the staged rows (export / legacy EDGE variants)

@@ -625,21 +625,14 @@ void md_launch_build_staged(md_system* s, bool gated) {
     int nc, um, tc;
     size_t smem;
     staged_build_sizes(s, &nc, &um, &tc, &smem);
-    static bool attr_done = false;
-    static int carve_now = -1;
-    if (!attr_done) {
-        cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-        cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-        attr_done = true;
-    }
     // candidates are read through L1: with the small tables of dense cells leave it as large as the resident blocks allow
     // (measured at C2a: carveout 25 -> 1.96 ms, 50 -> 1.65, 75 -> 1.82, 100 -> 2.02); the 42 KB tables of sparse cells need
     // the shared memory itself (five resident blocks instead of two)
     const int carve = smem > 30 * 1024 ? (int)cudaSharedmemCarveoutMaxShared : 50;
-    if (carve != carve_now) {
+    if (carve != s->build_carve) {      // per handle = per device (function attributes are per device)
         cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
         cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
-        carve_now = carve;
+        s->build_carve = carve;
     }
     k_staged_begin<<<1, 1, 0, s->stream>>>(s->B, g);
     if (P.use_masks) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
@@ -688,11 +681,6 @@ __global__ void __launch_bounds__(MD_TB) k_edges_from_rows(DevParams P, DevBuffe
 
 void md_launch_edges_from_rows(md_system* s) {
     const DevParams& P = s->P;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaFuncSetAttribute(k_edges_from_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-        attr_done = true;
-    }
     k_edges_from_rows<<<P.nblk, MD_TB, 4 * (size_t)P.stage_cap, s->stream>>>(P, s->B, s->pos);
     s->launches += 1;
 }
@@ -1174,13 +1162,16 @@ size_t md_staged_smem_bytes(const md_system* s, int stage_entries) {
     return 16 + 16 * (size_t)stage_entries * (s->rigid ? 2 : 1);
 }
 
-static void staged_attrs_once() {
-    static bool done = false;
-    if (done) return;
-    done = true;
-    cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-    cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-    cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+// Function attributes are per DEVICE: set for the handle's device at md_create (a second handle on another GPU of the
+// same process gets its own opt-in), never behind a process-wide flag.
+void md_staged_configure(md_system* s) {
+    const int optin = (int)s->smem_optin;
+    cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_edges_from_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     // the neighbourhoods live in shared memory and the rows bypass L1: ask for the largest shared-memory carveout so that
     // as many blocks as the sizing in sync_and_check counted on are resident
     cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -1188,26 +1179,46 @@ static void staged_attrs_once() {
     cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_patchy_staged<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_patchy_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    cudaFuncSetAttribute(k_vertex_patchy_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-    cudaFuncSetAttribute(k_vertex_patchy_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    cudaFuncSetAttribute(k_vertex_patchy_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_patchy_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    s->build_carve = -1;
+}
+
+// which instantiation of k_vertex_lj_staged a launch capacity of `smem` bytes selects: threads per particle
+static int staged_lj_ns(const md_system* s, size_t smem) {
+    const size_t optin = s->smem_optin, per_sm = s->smem_per_sm;
+    if (2 * (smem + 24 * MD_TB + 1024) > per_sm - 1024 && smem + 72 * MD_TB <= optin && s->P.rcap >= 64) return 4;   // one block per SM
+    if (smem > 75 * 1024 && smem + 24 * MD_TB <= optin) return 2;                                                      // <= 2 blocks per SM
+    return 1;
+}
+
+static int staged_launch_entries(const md_system* s) {
+    int se = s->stage_launch;
+    if (s->stage_limit > 0) se = std::min(se, s->stage_limit);   // MD_OPT_STAGE_LIMIT (tests): force blocks onto the unstaged path
+    return se;
+}
+
+int md_staged_threads_per_particle(const md_system* s) {
+    if (s->rigid || s->order == MD_ORDER_NONE) return 0;
+    return staged_lj_ns(s, md_staged_smem_bytes(s, staged_launch_entries(s)));
 }
 
 // VERTEX on the staged rows.  Returns false if the neighbourhood does not fit in shared memory.
 bool md_launch_forces_staged(md_system* s) {
     const DevParams& P = s->P;
-    staged_attrs_once();
-    int se = s->stage_launch;
-    if (s->stage_limit > 0) se = std::min(se, s->stage_limit);   // MD_B200_STAGE_LIMIT (tests): force blocks onto the unstaged path
+    const int se = staged_launch_entries(s);
     const size_t smem = md_staged_smem_bytes(s, se);
-    if (smem > 224 * 1024) return false;
+    if (smem > s->smem_optin) return false;
     if (P.kind == MD_POT_PATCHY && P.pp_model) k_vertex_patchy_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
     else if (P.kind == MD_POT_PATCHY) k_vertex_patchy_staged<false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->quat, s->force, s->torque);
-    else if (2 * (smem + 24 * MD_TB + 1024) > 227 * 1024 && smem + 72 * MD_TB <= 224 * 1024 && P.rcap >= 64)
-        // one block per SM: four threads per particle (1024-thread blocks, 32 warps on the SM)
-        k_vertex_lj_staged<4><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
-    else if (smem > 75 * 1024 && smem + 24 * MD_TB <= 224 * 1024)   // <= 2 blocks per SM: two threads per particle
-        k_vertex_lj_staged<2><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
-    else k_vertex_lj_staged<1><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+    else {
+        const int ns = staged_lj_ns(s, smem);
+        if (ns == 4)        // one block per SM: four threads per particle (1024-thread blocks, 32 warps on the SM)
+            k_vertex_lj_staged<4><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
+        else if (ns == 2)   // <= 2 blocks per SM: two threads per particle
+            k_vertex_lj_staged<2><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
+        else k_vertex_lj_staged<1><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+    }
     s->launches += 1;
     return true;
 }

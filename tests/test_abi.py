@@ -42,10 +42,12 @@ def test_no_torch_types_in_header():
     assert 'extern "C"' in sigs
 
 
-def _ws(lib, N, box, rcut, skin, pot, max_neigh):
+def _ws(lib, N, box, rcut, skin, pot, max_neigh, f32_box=True):
     from paper_1401_4350_b200.binding import make_potential
     p = make_potential(pot)
     b = np.ascontiguousarray(box, dtype=np.float64)
+    if f32_box:
+        b = b.astype(np.float32).astype(np.float64)      # S:Q7: boxes exactly representable in fp32
     n = C.c_size_t(0)
     rc = lib.md_workspace_bytes(N, b.ctypes.data_as(C.POINTER(C.c_double)), rcut, skin, C.byref(p), max_neigh, C.byref(n))
     return rc, n.value
@@ -63,6 +65,9 @@ def test_workspace_bytes_and_validation(lib):
     assert _ws(lib, 2 ** 22, [200.0] * 3, 2.5, 0.3, pot, 1024)[0] == -1     # N * max_neigh >= 2^31
     assert _ws(lib, 2048, [13.68] * 3, 2.5, 0.3, pot, 480)[0] == 0
     assert _ws(lib, 2048, [13.68] * 3, 2.5, 0.3, pot, 481)[0] == -1          # max_neigh > 480 (md_b200.h)
+    # a box that fp32 cannot hold would give the fp32 minimum image and the fp64 predicates different boxes
+    assert _ws(lib, 2048, [13.68] * 3, 2.5, 0.3, pot, 116, f32_box=False)[0] == -1
+    assert _ws(lib, 2048, [13.5, 14.25, 16.0], 2.5, 0.3, pot, 116, f32_box=False)[0] == 0
     bad = dict(W.patchy_potential())
     bad["patch_dir"] = bad["patch_dir"] * 1.1                               # non-unit patch vectors
     assert _ws(lib, 2048, [20.0] * 3, 1.5, 0.3, bad, 40)[0] == -1
@@ -73,7 +78,7 @@ def test_workspace_bytes_and_validation(lib):
 def test_create_rejects_bad_workspace_without_gpu(lib):
     from paper_1401_4350_b200.binding import make_potential
     p = make_potential(W.lj_potential(2.5))
-    b = np.array([13.68] * 3)
+    b = np.array([13.68] * 3).astype(np.float32).astype(np.float64)
     h = C.c_void_p(None)
     rc = lib.md_create(C.byref(h), 2048, b.ctypes.data_as(C.POINTER(C.c_double)), 2.5, 0.3, C.byref(p), 116,
                        None, 0, None)
