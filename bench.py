@@ -2,13 +2,15 @@
 """bench.py -- pair interactions/s and us per force evaluation, VERTEX vs EDGE (BASELINE.json `metric`).
 
 Workload (N = 1 GPU): BASELINE.json configs[1], Lennard-Jones fluid, N = 2^20, rho = 0.8, r_c = 2.5, skin 0.3
-(`--workload C2b` for the r_c = 4.0 many-neighbour variant), seeded fcc + jitter, melted by an untimed
-md_integrate run so that the timed state is the load-imbalanced fluid.
+(`--workload C2b` for the r_c = 4.0 many-neighbour variant, C1 / C3 / C4 for the other configs, C5 for the strategy
+crossover sweep of configs[4]), seeded fcc + jitter, melted by an untimed md_integrate run so that the timed state
+is the load-imbalanced fluid.
 
 A timed "step" is one pass of the whole hot path: one md_integrate step (half kick, drift, skin check, device-side
 cell + Verlet rebuild when the skin criterion fires, force evaluation, half kick); one md_energy closes the K
-steps inside the timed region.  `value` = E (unordered Verlet pairs) x K / time.  The dominant kernel (the
-force kernel) is timed alone with CUDA events for `force_eval` and `roofline`.
+steps inside the timed region.  `value` = E (unordered Verlet pairs) x K / time.  The same K steps are timed
+for the other strategy too (`whole_step`).  The force kernels are timed alone with CUDA events, 5 repeats of >= 20
+back-to-back calls, median and min (P:135, S:8(d)), for `force_eval` and `roofline`.
 
 Multi-GPU: the path runs on one GPU (north_star) -> replicas only: every rank runs an independent system, no
 data-path collective; value = pairs processed by all ranks / max-over-ranks time ("scaling": "weak").
@@ -30,9 +32,14 @@ if str(ROOT) not in sys.path:
 
 import numpy as np
 
-METRIC = "pair interactions/s (Verlet pairs E per force evaluation / time), VERTEX vs EDGE, LJ N=2^20"
 UNIT = "pair interactions/s"
-EDGE_VARIANTS = ["red", "red_v4", "warp", "segmented"]
+def _edge_variants():
+    from paper_1401_4350_b200.binding import SCATTER
+    return [v for v in ("red", "red_v4", "warp", "segmented", "cluster") if v in SCATTER]
+
+
+EDGE_VARIANTS = _edge_variants()
+VERTEX_VARIANTS = ["smem", "l2"]
 WORKLOAD_TEXT = {
     "C1": "BASELINE.json configs[0], LJ fluid N=2048 rho=0.8 rc=2.5 skin=0.3, fcc+jitter",
     "C2a": "BASELINE.json configs[1], LJ fluid N=2^20 rho=0.8 rc=2.5 skin=0.3, fcc+jitter",
@@ -40,8 +47,15 @@ WORKLOAD_TEXT = {
     "C3": "BASELINE.json configs[2], bead-spring melt 4096 x 64, rho=0.85, FENE + WCA, skin=0.3, seeded walks + push-off",
     "C4": "BASELINE.json configs[3], patchy rigid bodies N=2^18 rho=0.5, WCA core + 4 tetrahedral patches, rc=1.5 skin=0.3",
 }
-VERTEX_VARIANTS = ["smem", "l2"]
+METRIC_TEXT = {
+    "C1": "LJ N=2048", "C2a": "LJ N=2^20", "C2b": "LJ N=2^20 rc=4.0", "C3": "bead-spring melt N=2^18",
+    "C4": "patchy rigid bodies N=2^18", "C5": "strategy crossover sweep",
+}
 NVT_N_NEWT, NVT_P = 20, 0.1     # thermostat leg (reading QT of P:53): refresh every 20 steps, 10 % of the particles
+
+
+def metric_text(workload: str) -> str:
+    return f"pair interactions/s (Verlet pairs E per force evaluation / time), VERTEX vs EDGE, {METRIC_TEXT[workload]}"
 
 
 def workload(name: str):
@@ -66,19 +80,31 @@ def algorithmic_bytes(strategy: str, E: int, N: int, rigid: bool = False) -> flo
     return 8.0 * E + s_in * N + 2 * s_out * N
 
 
-def fp32_peak_tflops() -> float:
+def layout_bytes(strategy: str, variant: str, E: int, N: int, rigid: bool, units: int = 0) -> float:
+    """Minimum bytes of the layout the kernel actually streams: the staged VERTEX rows hold 16-bit entries
+    (2 B per visit), the cluster EDGE list one 8-byte unit per (cluster, j); everything else as algorithmic_bytes."""
+    s_in = s_out = 32.0 if rigid else 16.0
+    if strategy == "vertex" and variant == "smem":
+        return 2.0 * 2 * E + 4.0 * N + s_in * N + s_out * N
+    if strategy == "edge" and variant == "cluster":
+        return 8.0 * units + s_in * N + 2 * s_out * N
+    return algorithmic_bytes(strategy, E, N, rigid)
+
+
+def fp32_nominal_tflops() -> float:
     """148 SMs x 128 FP32 lanes x 2 flops (FMA) x SM max clock (MEASURED_PEAKS.json, else 1965 MHz)."""
     p = ROOT / "MEASURED_PEAKS.json"
     mhz = float(json.loads(p.read_text()).get("sm_max_mhz", 1965.0)) if p.exists() else 1965.0
     return 148 * 128 * 2 * mhz * 1e6 / 1e12
 
 
-def algorithmic_flops(strategy: str, E: int, rigid: bool, rcut: float, rv: float) -> float:
-    """DESIGN.md 6 / SURVEY 8(d): LJ ~21 flops per visit + 18 inside the cutoff (in-cutoff share of a uniform fluid,
-    (rc/rv)^3); patchy rigid bodies ~215 flops per visit.  VERTEX visits every pair twice, EDGE once."""
-    visits = 2.0 * E if strategy == "vertex" else 1.0 * E
-    per = 215.0 if rigid else 21.0 + 18.0 * (rcut / rv) ** 3
-    return visits * per
+def algorithmic_flops(strategy: str, E: int, E_in: int, rigid: bool) -> float:
+    """LJ 21 flops per visit + 18 inside the cutoff (21 + 21 per EDGE pair); patchy rigid bodies 21 per
+    visit + 194 inside the cutoff for VERTEX (215 per in-cutoff visit), 21 + 214 per EDGE pair (235 in-cutoff).
+    VERTEX visits every pair twice, EDGE once.  E_in = listed pairs inside r_c (md_stats_ex, a device counter)."""
+    if strategy == "vertex":
+        return 2.0 * (21.0 * E + (194.0 if rigid else 18.0) * E_in)
+    return 21.0 * E + (214.0 if rigid else 21.0) * E_in
 
 
 class ClockSampler:
@@ -127,79 +153,129 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def time_calls(torch, fn, n, warm=3):
-    """Average device time of fn() in microseconds (CUDA events on the current stream = the library's stream)."""
+def time_calls(torch, fn, n=20, warm=5, repeats=5):
+    """S:8(d) timing protocol: CUDA events on the current stream (= the library's stream) around n back-to-back calls,
+    `warm` warm-up calls, `repeats` repeats (the paper's count).  Returns (median, min) in microseconds per call."""
     for _ in range(warm):
         fn()
     torch.cuda.synchronize()
+    ts = []
+    for _ in range(repeats):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b) * 1e3 / n)
+    return statistics.median(ts), min(ts)
+
+
+def time_steps(torch, s, w, K, Wm, strategy, variant, dev, dist=None):
+    """K whole-path steps + one md_energy, device-resident state; returns (ms_total, E_run, launches, rebuilds, energies)."""
+    s.build_cells(); s.build_verlet(); s.forces(strategy, variant)
+    E0 = s.stats()["n_edges"]
+    s.integrate(w.dt, Wm, strategy, variant)
+    stw = s.stats()
+    torch.cuda.synchronize(dev)
+    if dist is not None:
+        dist.barrier()
+    l0 = s.launch_count()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record()
-    for _ in range(n):
-        fn()
+    s.integrate(w.dt, K, strategy, variant)
+    e_tot = s.energy()                            # A9, synchronises: result read back by the host
     b.record()
-    torch.cuda.synchronize()
-    return a.elapsed_time(b) * 1e3 / n
+    torch.cuda.synchronize(dev)
+    if dist is not None:
+        dist.barrier()
+    ms_total = a.elapsed_time(b)
+    launches = s.launch_count() - l0
+    st1 = s.stats()
+    return ms_total, 0.5 * (E0 + st1["n_edges"]), launches, st1["n_rebuilds"] - stw["n_rebuilds"], e_tot
 
 
-def cpu_baseline(w, seconds_hint=20.0):
-    """The fp64 oracle, as it stands, timed on this box's host cores on a bounded sample of the workload:
-    the same generator at N = 2^17 (same density, cutoff, skin -> same per-particle structure)."""
+def oracle_inputs(s, w):
+    """The state the GPU holds, in original id order, as the oracle's input (identical input, S:8(d))."""
+    pos = s.in_id_order(s.pos)
+    quat = s.in_id_order(s.quat) if w.quat is not None else None
+    return pos, quat
+
+
+def cpu_baseline(w, pos, quat, E_gpu):
+    """S:8(d) / P:91: the fp64 oracle, as it stands, on this box's host cores on the IDENTICAL input (the positions the
+    GPU timed): (i) one thread over the half Verlet list with Newton's third law (O10), (ii) OpenMP over all cores with
+    the plain per-particle definition (O1-O5).  Systems whose list exceeds 60 M pairs are sampled at N = 2^18 of the
+    same generator (stated in `sample`)."""
     import workloads as W
     from oracle import Oracle
     orc = Oracle()
-    n_s = min(w.N, 2 ** 17)
-    ws = W.lj_fluid(n_s, rcut=w.rcut, skin=w.skin, seed=W.BASE_SEED + 2)
-    E_s = orc.pair_count(ws.pos, ws.box, ws.rcut, ws.skin)      # untimed: only to count the pairs credited
-    orc.forces(ws.pos, ws.box, dict(ws.potential))               # warm (page in, thread pool)
+    sample = f"the bench input itself (N={w.N}, positions copied from the GPU after the melt)"
+    box, pot = w.box, dict(w.potential)
+    if E_gpu > 60e6:
+        ws = W.lj_fluid(2 ** 18, rcut=w.rcut, skin=w.skin, seed=W.BASE_SEED + 2)
+        pos, quat, box, pot = ws.pos, None, ws.box, dict(ws.potential)
+        sample = f"lj_fluid N=2^18 rc={w.rcut} of the same generator (the full list has {E_gpu / 1e6:.0f} M pairs)"
+    t0 = time.perf_counter()
+    pairs = orc.pair_set(pos, box, w.rcut, w.skin)           # the oracle's own half list (timed separately)
+    t_list = time.perf_counter() - t0
+    E_s = int(pairs.shape[0])
+    orc.forces(pos, box, pot, quat=quat)                     # warm (page in, thread pool)
     reps, t0 = 0, time.perf_counter()
     while True:
-        orc.forces(ws.pos, ws.box, dict(ws.potential))
+        orc.forces(pos, box, pot, quat=quat)
         reps += 1
         dt = time.perf_counter() - t0
-        if dt > 0.5 * seconds_hint or reps >= 20:
+        if dt > 8.0 or reps >= 10:
             break
-    t = dt / reps
-    # the same oracle on ONE host core (the paper's "single CPU core" framing, P:91), two evaluations
-    nthreads = orc.threads
-    orc.set_threads(1)
-    t1 = time.perf_counter()
-    for _ in range(2):
-        orc.forces(ws.pos, ws.box, dict(ws.potential))
-    t1 = (time.perf_counter() - t1) / 2
-    orc.set_threads(nthreads)
-    return {"value": E_s / t, "unit": UNIT, "cores": nthreads, "kind": "oracle", "single_core_value": E_s / t1,
-            "sample": f"oracle.forces (fp64 plain definition, OpenMP) on lj_fluid N={n_s} rc={w.rcut} (same generator, "
-                      f"density and cutoffs as the bench workload), {reps} evaluations, E_sample={E_s}",
-            "us_per_eval": t * 1e6}, orc
+    t_omp = dt / reps
+    t0 = time.perf_counter()
+    orc.forces_half(pos, box, pot, pairs, quat=quat)
+    t_one = time.perf_counter() - t0
+    return {"value": E_s / t_omp, "unit": UNIT, "cores": orc.threads, "kind": "oracle",
+            "sample": f"{sample}; oracle.forces (fp64 plain definition, OpenMP full lists), {reps} evaluations, E={E_s}",
+            "us_per_eval": t_omp * 1e6,
+            "single_core_half_list": {"value": E_s / t_one, "us_per_eval": t_one * 1e6, "cores": 1,
+                                      "what": "oracle.forces_half (O10): one thread, half Verlet list, Newton's third law"},
+            "list_build_s": t_list}
 
 
 def run_reference(args):
-    """--impl reference: the oracle on host cores, same metric / config; each step = one force evaluation on the
-    bounded sample."""
+    """--impl reference: the oracle on host cores on OUR arm's config -- the same workload at full size, melted by the
+    same number of untimed steps (with the oracle's own integrator), W warm-up and K timed velocity-Verlet steps of
+    oracle.integrate (O6/O7: force evaluation by the plain definition, OpenMP).  value = E x K / time like our arm."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import workloads as W
     from oracle import Oracle
     orc = Oracle()
-    wname = args.workload
-    rcut = 4.0 if wname == "C2b" else 2.5
-    n_s = 2 ** 17
-    ws = W.lj_fluid(n_s, rcut=rcut, seed=W.BASE_SEED + 2)
-    E_s = orc.pair_count(ws.pos, ws.box, ws.rcut, ws.skin)
-    steps, warm = max(1, min(args.steps, 20)), max(1, min(args.warmup, 3))
-    for _ in range(warm):
-        orc.forces(ws.pos, ws.box, dict(ws.potential))
+    wname = args.workload if args.workload != "C5" else "C2a"
+    w = workload(wname)
+    pot = dict(w.potential)
+    K, Wm = max(1, args.steps), max(0, args.warmup)
+    pos, vel, quat, angmom = w.pos, w.vel, w.quat, w.angmom
+    t_melt = time.perf_counter()
+    for n in (args.melt_steps, Wm):                       # untimed: melt, then warm-up steps
+        if n > 0:
+            o = orc.integrate(pos, vel, w.box, pot, w.skin, w.dt, n, quat=quat, angmom=angmom)
+            pos, vel = o["pos"], o["vel"]
+            if quat is not None:
+                quat, angmom = o["quat"], o["angmom"]
+    t_melt = time.perf_counter() - t_melt
+    pos32 = np.zeros((w.N, 4), dtype=np.float32)
+    pos32[:, :3] = np.mod(pos[:, :3], w.box)
+    E = orc.pair_count(pos32, w.box, w.rcut, w.skin)
     t0 = time.perf_counter()
-    for _ in range(steps):
-        orc.forces(ws.pos, ws.box, dict(ws.potential))
-    t = (time.perf_counter() - t0) / steps
-    val = E_s / t
-    sample = f"oracle.forces on lj_fluid N={n_s} rc={rcut} (bounded sample of {wname}), E_sample={E_s}"
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-            "warmup": warm, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{wname}: LJ fluid rho=0.8 rc={rcut} skin=0.3, oracle sample N={n_s}"},
+    orc.integrate(pos, vel, w.box, pot, w.skin, w.dt, K, quat=quat, angmom=angmom)
+    t = (time.perf_counter() - t0) / K
+    val = E / t
+    sample = (f"oracle.integrate (fp64 plain-definition forces, OpenMP) on the full workload N={w.N}, melted by "
+              f"{args.melt_steps} + {Wm} untimed oracle steps ({t_melt:.0f} s), E={E}")
+    line = {"impl": "reference", "metric": metric_text(args.workload), "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": K, "warmup": Wm, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{wname}: {WORKLOAD_TEXT[wname]}, relaxed by {args.melt_steps} untimed steps",
+                       "N": w.N, "E": int(E)},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -216,28 +292,71 @@ def aggregate(dist, torch, pairs_local: float, ms_local: float, device):
     return float(t.item()), float(m.item())
 
 
+def roofline_for(strategy, variant, t_us, Ef, E_in, N, rigid, units, probes, workload_name):
+    """B:5: the roofline is the SLOWER of the algorithmic bytes at the measured HBM bandwidth and the algorithmic FP32
+    flops at peak.  The FP32 peak is the nominal one (conservative for `frac`); the measured FFMA / FFMA2 issue rates of
+    this run (md_probe) are recorded beside it."""
+    peak, peak_src = measured_peaks()
+    abytes = algorithmic_bytes(strategy, Ef, N, rigid)
+    aflops = algorithmic_flops(strategy, Ef, E_in, rigid)
+    fpeak = fp32_nominal_tflops()
+    t_hbm, t_alu = abytes / (peak * 1e9) * 1e6, aflops / (fpeak * 1e12) * 1e6
+    knames = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp": "k_edge_warp", "red": "k_edge_red",
+              "red_v4": "k_edge_red", "segmented": "k_edge_store+k_edge_segsum", "cluster": "k_edge_cluster"}
+    kname = knames[variant]
+    if rigid:
+        kname = kname.replace("_lj", "_patchy")
+    traffic = None
+    tf = ROOT / "profiles" / "roofline_traffic.csv"     # dram bytes per launch from the committed ncu --set full captures
+    if tf.exists():
+        for ln in tf.read_text().splitlines()[1:]:
+            f = ln.split(",")
+            if len(f) >= 4 and f[0] == workload_name and f[1] == strategy and f[2] == kname:
+                traffic = float(f[3])
+    if t_alu > t_hbm:
+        ach = aflops / (t_us * 1e-6) / 1e12
+        r = {"bound": "alu", "kernel": kname, "achieved": ach, "peak": fpeak, "unit": "TFLOP/s", "frac": ach / fpeak,
+             "traffic": traffic, "algorithmic_flops_per_launch": aflops, "us_per_launch": t_us,
+             "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x SM max clock (DESIGN.md 6); measured issue rates in fp32_measured"}
+    else:
+        ach = abytes / (t_us * 1e-6) / 1e9
+        r = {"bound": "hbm", "kernel": kname, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+             "traffic": traffic, "algorithmic_bytes_per_launch": abytes, "us_per_launch": t_us, "peak_source": peak_src}
+    r["t_bound_us"] = {"hbm": t_hbm, "fp32": t_alu}
+    r["E_in"] = int(E_in)
+    lb = layout_bytes(strategy, variant, Ef, N, rigid, units)
+    r["vs_layout_bytes"] = {"bytes_per_launch": lb, "frac": lb / (t_us * 1e-6) / 1e9 / peak,
+                            "note": "fraction of the HBM peak against the bytes of the layout the kernel streams (16-bit "
+                                    "staged rows / 8-byte cluster units); `frac` above is against SURVEY 8(d)'s algorithmic bytes"}
+    if traffic:
+        r["dram_frac_measured"] = traffic / (t_us * 1e-6) / 1e9 / peak
+    if probes:
+        r["fp32_measured"] = probes
+    return r
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2a", choices=["C1", "C2a", "C2b", "C3", "C4"],
-                    help="BASELINE.json config; the headline metric is quoted on C2a (default)")
+    ap.add_argument("--workload", default="C2a", choices=["C1", "C2a", "C2b", "C3", "C4", "C5"],
+                    help="BASELINE.json config; the headline metric is quoted on C2a (default); C5 = crossover sweep")
     ap.add_argument("--strategy", default="vertex", choices=["vertex", "edge"])
     ap.add_argument("--scatter", default=None, choices=EDGE_VARIANTS + VERTEX_VARIANTS,
-                    help="EDGE scatter variant (default warp) or VERTEX gather variant (default smem)")
+                    help="EDGE scatter variant (default: the fastest measured) or VERTEX gather variant (default smem)")
     ap.add_argument("--order", default="hilbert", choices=["none", "cell", "hilbert"])
     ap.add_argument("--melt-steps", type=int, default=300)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--c5-max-log2n", type=int, default=20, help="C5: largest N of the sweep (configs[4] goes to 22)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
-    if args.scatter is None:
-        args.scatter = "smem" if args.strategy == "vertex" else "warp"
-    if args.order == "none" and args.scatter == "smem":
-        args.scatter = "l2"
+    if args.workload == "C5":
+        import crossover
+        return crossover.bench_mode(args)
 
     import torch
     if not torch.cuda.is_available():
@@ -258,81 +377,77 @@ def main():
     K, Wm = args.steps, max(3, args.warmup)
 
     w = workload(args.workload)
+    N = w.N
+    rigid = w.quat is not None
     s = MDSystem.from_workload(w, device=str(dev), order=args.order)
-    s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
+    vgather = "smem" if args.order != "none" else "l2"
+    s.build_cells(); s.build_verlet(); s.forces("vertex", vgather)
     if args.melt_steps > 0:                       # untimed setup: melt the lattice (paper: thermalised states)
         for k in range(0, args.melt_steps, 100):  # md_stats between chunks lets the staged launch capacity follow the melt
-            s.integrate(w.dt, min(100, args.melt_steps - k), args.strategy, args.scatter)
+            s.integrate(w.dt, min(100, args.melt_steps - k), "vertex", vgather)
             s.stats()
-    s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
-    st0 = s.stats()
-    E, N = st0["n_edges"], w.N
 
-    # ---- whole-path steps: K x md_integrate(1 step) + one md_energy, device-resident state ----
-    s.integrate(w.dt, Wm, args.strategy, args.scatter)
-    stw = s.stats()
-    torch.cuda.synchronize(dev)
-    if dist is not None:
-        dist.barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    l0 = s.launch_count()
-    torch.cuda.synchronize(dev)
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record()
-    s.integrate(w.dt, K, args.strategy, args.scatter)
-    e_tot = s.energy()                            # A9, synchronises: result read back by the host
-    b.record()
-    torch.cuda.synchronize(dev)
-    if dist is not None:
-        dist.barrier()
-    ms_total = a.elapsed_time(b)
-    launches = s.launch_count() - l0
-    st1 = s.stats()
-    E_run = 0.5 * (E + st1["n_edges"])
-    pairs_all, ms_max = aggregate(dist, torch, E_run * K, ms_total, dev)
-    value = pairs_all / (ms_max * 1e-3)
-
-    # ---- dominant kernel alone: force evaluation, VERTEX and every EDGE variant (lists fixed, state in HBM) ----
+    # ---- force evaluation alone, VERTEX and every EDGE variant (lists fixed, state in HBM), S:8(d) protocol ----
     s.build_cells(); s.build_verlet()
     stf = s.stats()
     Ef = stf["n_edges"]
+    sampler = ClockSampler(local)
+    sampler.start()
     fe = {}
     for gv in VERTEX_VARIANTS:
         if gv == "smem" and args.order == "none":
             continue
-        t = time_calls(torch, lambda: s.forces("vertex", gv), 20)
-        fe[f"vertex_{gv}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
+        med, mn = time_calls(torch, lambda: s.forces("vertex", gv), 20)
+        fe[f"vertex_{gv}"] = {"us": med, "us_min": mn, "pairs_per_s": Ef / (med * 1e-6)}
     for sc in EDGE_VARIANTS:
-        t = time_calls(torch, lambda: s.forces("edge", sc), 10 if sc != "red" else 5)
-        fe[f"edge_{sc}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
+        med, mn = time_calls(torch, lambda: s.forces("edge", sc), 20 if sc != "red" else 5, warm=3)
+        fe[f"edge_{sc}"] = {"us": med, "us_min": mn, "pairs_per_s": Ef / (med * 1e-6)}
     # S:8(f1): VERTEX with Newton's third law, m private force copies per particle (reported beside, not ranked)
     n3 = {}
     for m in (1, 4, 12):
-        t = time_calls(torch, lambda: s.forces("vertex_n3", m), 10)
-        n3[f"m{m}"] = {"us": t, "pairs_per_s": Ef / (t * 1e-6)}
+        if m * N > N * ((s.max_neigh + 3) // 4 * 4) // 2 + 64:
+            continue
+        med, mn = time_calls(torch, lambda: s.forces("vertex_n3", m), 10, warm=2, repeats=3)
+        n3[f"m{m}"] = {"us": med, "us_min": mn, "pairs_per_s": Ef / (med * 1e-6)}
     best_vertex = min((k for k in fe if k.startswith("vertex")), key=lambda k: fe[k]["us"])
-    t_v = fe[best_vertex]["us"]
+    best_edge = min((k for k in fe if k.startswith("edge")), key=lambda k: fe[k]["us"])
+    sx = s.stats_ex()                              # E_in by a device counter (S:Q16), NS of the staged launch
+    E_in, units = sx["n_in_cutoff"], sx["n_cluster_units"]
+    probes = {"ffma_tflops": s.probe("ffma"), "ffma2_tflops": s.probe("ffma2"), "mufu_tops": s.probe("mufu"),
+              "red_v4_scatter_gops": s.probe("red_v4_scatter"), "red_v4_coalesced_gops": s.probe("red_v4_coalesced"),
+              "nominal_tflops": fp32_nominal_tflops()}
+    if args.scatter is None:
+        args.scatter = (vgather if args.strategy == "vertex" else best_edge[len("edge_"):])
+    if args.order == "none" and args.scatter == "smem":
+        args.scatter = "l2"
+    other = ("edge", best_edge[len("edge_"):]) if args.strategy == "vertex" else ("vertex", vgather)
+    rooflines = {}
+    for strat, var in ((args.strategy, args.scatter), other):
+        rooflines[f"{strat}_{var}"] = roofline_for(strat, var, fe[f"{strat}_{var}"]["us"], Ef, E_in, N, rigid, units,
+                                                   probes, args.workload)
+    roofline = rooflines[f"{args.strategy}_{args.scatter}"]
+    roofline["threads_per_particle"] = sx["threads_per_particle"]
+
+    # ---- whole-path steps: K x md_integrate(1 step) + one md_energy, device-resident state; both strategies ----
+    ms_total, E_run, launches, rebuilds, e_tot = time_steps(torch, s, w, K, Wm, args.strategy, args.scatter, dev, dist)
+    pairs_all, ms_max = aggregate(dist, torch, E_run * K, ms_total, dev)
+    value = pairs_all / (ms_max * 1e-3)
+    ms_o, E_o, _, reb_o, _ = time_steps(torch, s, w, K, Wm, other[0], other[1], dev)
+    whole = {f"{args.strategy}_{args.scatter}": {"ms_per_step": ms_total / K, "pairs_per_s": E_run * K / (ms_total * 1e-3),
+                                                  "rebuilds": rebuilds},
+             f"{other[0]}_{other[1]}": {"ms_per_step": ms_o / K, "pairs_per_s": E_o * K / (ms_o * 1e-3), "rebuilds": reb_o}}
     clocks = sampler.stop()
+
     # S:8(f3): the same K steps in mixed precision (fp64 integration of the state, fp32 forces), reported beside
     s.set_precision("mixed")
-    s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
-    s.integrate(w.dt, Wm, args.strategy, args.scatter)
-    torch.cuda.synchronize(dev)
-    am, bm = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    am.record()
-    s.integrate(w.dt, K, args.strategy, args.scatter)
-    s.energy()
-    bm.record()
-    torch.cuda.synchronize(dev)
-    ms_mixed = am.elapsed_time(bm) / K
+    ms_mixed = time_steps(torch, s, w, K, Wm, args.strategy, args.scatter, dev)[0] / K
     mixed = {"ms_per_step": ms_mixed, "cost_vs_fp32": ms_mixed / (ms_total / K), "paper": "10-40 % on C2070/K10/K20 (P:59)"}
     s.set_precision("f32")
     # S:8(f3): the same K steps under the thermostat of reading QT (NVT), reported beside; the target temperature
     # is the kinetic temperature the system has now, so the thermostat holds the state point instead of moving it
     s.build_cells(); s.build_verlet(); s.forces(args.strategy, args.scatter)
     T_now = 2.0 * s.energy()[1] / (3.0 * N)
-    s.set_thermostat(T_now, NVT_N_NEWT, NVT_P, NVT_P if w.quat is not None else 0.0, 20140117)
+    s.set_thermostat(T_now, NVT_N_NEWT, NVT_P, NVT_P if rigid else 0.0, 20140117)
     s.integrate(w.dt, Wm, args.strategy, args.scatter)
     torch.cuda.synchronize(dev)
     an, bn = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -345,49 +460,17 @@ def main():
     s.set_thermostat(T_now, 0, 0.0, 0.0, 0)
     nvt = {"ms_per_step": ms_nvt, "cost_vs_nve": ms_nvt / (ms_total / K), "T_target": T_now, "T_after": 2.0 * k_nvt / (3.0 * N),
            "n_newt": NVT_N_NEWT, "p": NVT_P, "paper": "'does not significantly affect performances' (P:53)"}
-    best_edge = min((k for k in fe if k.startswith("edge")), key=lambda k: fe[k]["us"])
-    peak, peak_src = measured_peaks()
-    dom = args.strategy
-    t_dom = fe[f"{dom}_{args.scatter}"]["us"]
-    rigid = w.quat is not None
-    abytes = algorithmic_bytes(dom, Ef, N, rigid)
-    achieved = abytes / (t_dom * 1e-6) / 1e9
-    knames = {"smem": "k_vertex_lj_staged", "l2": "k_vertex_lj", "warp": "k_edge_warp", "red": "k_edge_red", "red_v4": "k_edge_red",
-              "segmented": "k_edge_store+k_edge_segsum"}
-    traffic = None
-    tf = ROOT / "profiles" / "roofline_traffic.csv"     # dram bytes per launch from the committed ncu --set full capture
-    if tf.exists():
-        for ln in tf.read_text().splitlines()[1:]:
-            f = ln.split(",")
-            if len(f) >= 4 and f[0] == args.workload and f[1] == dom and f[2] == knames[args.scatter]:
-                traffic = float(f[3])
-    kname = knames[args.scatter]
-    if rigid:
-        kname = kname.replace("_lj", "_patchy")
-    # B:5: the roofline is the SLOWER of the algorithmic bytes at HBM bandwidth and the FP32 flops at peak
-    aflops = algorithmic_flops(dom, Ef, rigid, w.rcut, w.rcut + w.skin)
-    fpeak = fp32_peak_tflops()
-    t_hbm, t_alu = abytes / (peak * 1e9) * 1e6, aflops / (fpeak * 1e12) * 1e6
-    if t_alu > t_hbm:
-        ach = aflops / (t_dom * 1e-6) / 1e12
-        roofline = {"bound": "alu", "kernel": kname, "achieved": ach, "peak": fpeak, "unit": "TFLOP/s", "frac": ach / fpeak,
-                    "traffic": traffic, "algorithmic_flops_per_launch": aflops, "us_per_launch": t_dom,
-                    "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x SM max clock (DESIGN.md 6)"}
-    else:
-        roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved,
-                    "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
-                    "algorithmic_bytes_per_launch": abytes, "us_per_launch": t_dom, "peak_source": peak_src}
-    roofline["t_bound_us"] = {"hbm": t_hbm, "fp32": t_alu}
 
     # ---- end to end through the C ABI with HOST buffers (md_step_host): H2D state, build, forces, 1 step, D2H ----
+    pos_id, quat_id = oracle_inputs(s, w)         # the state the CPU baseline gets: identical input (S:8(d))
     e2e = None
     if rank == 0 or world > 1:
-        pos_h = torch.from_numpy(s.in_id_order(s.pos)).pin_memory()
+        pos_h = torch.from_numpy(pos_id.copy()).pin_memory()
         vel_h = torch.from_numpy(s.in_id_order(s.vel)).pin_memory()
         f_h = torch.zeros_like(pos_h).pin_memory()
         rb = {}
         if rigid:                                 # rigid bodies: quaternions and angular momenta in, torques out as well
-            rb = {"quat": torch.from_numpy(s.in_id_order(s.quat)).pin_memory(),
+            rb = {"quat": torch.from_numpy(quat_id.copy()).pin_memory(),
                   "angmom": torch.from_numpy(s.in_id_order(s.angmom)).pin_memory(),
                   "torque": torch.zeros_like(pos_h).pin_memory()}
         ne = max(1, args.e2e_steps)
@@ -411,11 +494,11 @@ def main():
         return
 
     cpu = None
-    if not args.no_cpu_baseline and world == 1 and args.workload in ("C2a", "C2b"):
-        cpu, _ = cpu_baseline(w)
+    if not args.no_cpu_baseline and world == 1:
+        cpu = cpu_baseline(w, pos_id, quat_id, Ef)
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "metric": metric_text(args.workload), "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{args.workload}: {WORKLOAD_TEXT[args.workload]}, relaxed by {args.melt_steps} untimed steps",
@@ -426,11 +509,13 @@ def main():
                           if 4.0 * Ef > 126e6 else
                           f"working set ({4.0 * Ef / 1e6:.0f} MB of neighbour rows) fits in the 126 MB L2: steady-state L2-resident "
                           "timing without a flush -- a secondary workload, the headline is C2a"),
-                   "rebuilds_in_timed_region": st1["n_rebuilds"] - stw["n_rebuilds"],
+                   "timing": "force_eval: CUDA events, 5 warm-up calls, 5 repeats of 20 back-to-back calls, median (us) and min (us_min)",
+                   "rebuilds_in_timed_region": rebuilds,
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "force_eval": fe, "vertex_n3_eval": n3, "mixed_precision": mixed, "thermostat": nvt, "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge,
-        "best_vertex": best_vertex,
-        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "force_eval": fe, "whole_step": whole, "vertex_n3_eval": n3, "mixed_precision": mixed, "thermostat": nvt,
+        "edge_vs_vertex": fe[best_vertex]["us"] / fe[best_edge]["us"], "best_edge": best_edge, "best_vertex": best_vertex,
+        "roofline": roofline, "roofline_other_strategy": rooflines[f"{other[0]}_{other[1]}"],
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "energy_total": sum(e_tot),
     }
     print(json.dumps(line))

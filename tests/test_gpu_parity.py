@@ -303,11 +303,12 @@ def test_step_host_end_to_end(MD, oracle):
 def test_crossover_sweep_runs(capsys, monkeypatch):
     """The configs[4] sweep script: one small cell of the grid, every variant, a table on stdout."""
     import sys
-    from paper_1401_4350_b200 import crossover
-    monkeypatch.setattr(sys, "argv", ["crossover", "--min-log2n", "12", "--max-log2n", "12", "--evals", "2", "--rcuts", "2.5"])
+    import crossover
+    monkeypatch.setattr(sys, "argv", ["crossover", "--min-log2n", "12", "--max-log2n", "12", "--evals", "2", "--rcuts", "2.5",
+                                      "--orders", "none,hilbert"])
     crossover.main()
     out = capsys.readouterr().out
-    assert "| lj | 2^12 | 0.8 | 2.5 |" in out and "| patchy | 2^12 | 0.5 | 1.5 |" in out and "| patchy_pp | 2^12 |" in out
+    assert "| lj | 2^12 | 0.8 | 2.5 | hilbert |" in out and "| patchy | 2^12 | 0.5 | 1.5 | none |" in out and "| patchy_pp | 2^12 |" in out
 
 
 # ---- mixed precision (S:8(f3), P:59): fp64 integration of the state, fp32 forces ----
