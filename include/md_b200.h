@@ -76,7 +76,11 @@ typedef enum {
     MD_SCATTER_RED = 0,      /* red.global.add.f32, one per component                           */
     MD_SCATTER_RED_V4 = 1,   /* red.global.add.v4.f32, one per particle and output array        */
     MD_SCATTER_WARP = 2,     /* runs of equal owner i combined by warp shuffles, then one red.v4 */
-    MD_SCATTER_SEGMENTED = 3 /* per-edge store + atomic-free segmented reduction         */
+    MD_SCATTER_SEGMENTED = 3, /* per-edge store + atomic-free segmented reduction        */
+    MD_SCATTER_CLUSTER = 4   /* j side aggregated BEFORE L2: the half list of 16 consecutive owners is stored as
+                                (j, 16-bit owner mask) units; one lane walks the pairs of a unit with the j side in
+                                registers (one red.v4 per unit) and the owner side in lane-private shared-memory rows
+                                (16 red.v4 per cluster).  Needs N < 2^31 only; fastest with an order set       */
 } md_scatter;
 /* VERTEX gather alternatives (B:5 "neighbour positions staged through shared memory or L2-resident gathers"):
  * passed as the third argument of md_forces / md_integrate / md_step_host when strategy == MD_VERTEX. */

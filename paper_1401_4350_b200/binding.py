@@ -11,7 +11,7 @@ _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libmd_b200.so"
 
 STRATEGY = {"vertex": 0, "edge": 1, "vertex_n3": 2}
-SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3}
+SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3, "cluster": 4}
 GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
 PRECISION = {"f32": 0, "mixed": 1}

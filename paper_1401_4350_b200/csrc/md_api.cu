@@ -16,7 +16,7 @@ struct Geometry {
     int nc[3];
     int64_t ncell;
     int cap, ntiles;
-    size_t ecap;
+    size_t ecap, ucap;
     int rcap, nblk, stage_cap, mask_words;   // staged path
 };
 
@@ -38,6 +38,8 @@ bool make_geometry(int64_t N, const double box[3], double rcut, double skin, int
     g->ntiles = (int)((N + MD_TILE - 1) / MD_TILE);
     if ((int64_t)g->ntiles * MD_TILE * g->cap >= (1ll << 31)) return false;
     g->ecap = (size_t)N * g->cap / 2 + 64;
+    g->ucap = g->ecap + 2 * (size_t)N + 64;      // cluster units: at most one per pair, plus the padding of every last round
+    if (g->ucap >= (1ull << 31)) g->ucap = (1ull << 31) - 64;
     // staged path: rows of 16-bit local indices in chunks of 4 entries; smem capacity of the build kernel
     g->rcap = (g->cap + 31) / 32 * 32;
     g->nblk = (int)((N + MD_TB - 1) / MD_TB);
@@ -98,6 +100,8 @@ size_t carve(char* base, int64_t N, const Geometry& g, bool rigid, DevBuffers* B
     b.cmask = (unsigned int*)take(4 * (size_t)g.nblk * 27 * (size_t)g.mask_words * MD_TB);   // scan order + sorted by column
     b.row_count = (int*)take(4 * Npad);
     b.lo_count = (int*)take(4 * Npad);
+    b.cl_units = (uint2*)take(8 * g.ucap);
+    b.cl_info = (int2*)take(8 * (((size_t)N + MD_CLUSTER - 1) / MD_CLUSTER));
     b.blk = (BlkInfo*)take(sizeof(BlkInfo) * (size_t)g.nblk);
     b.seg = (int2*)take(8 * (size_t)g.nblk * MD_SEGMAX);
     if (B) *B = b;
@@ -304,6 +308,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     s->order = MD_ORDER_NONE;
     s->workspace = workspace; s->workspace_bytes = workspace_bytes;
     s->ecap = g.ecap;
+    s->ucap = g.ucap;
     carve((char*)workspace, N, g, rigid, &s->B);
 
     DevParams& P = s->P;
@@ -338,6 +343,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
         P.stage_cap = (int)((s->smem_optin - 16) / (rigid ? 32 : 16)) - 1;
         s->stage_launch = P.stage_cap;
         md_staged_configure(s);
+        md_cluster_configure(s);
     }
     P.kind = rigid ? MD_POT_PATCHY : pot->kind;   // both rigid-body models run on the same kernels (P.pp_model tells them apart)
     P.eps = pot->epsilon; P.sig2 = pot->sigma * pot->sigma; P.mass = pot->mass; P.inv_mass = 1.0f / pot->mass;
@@ -414,7 +420,7 @@ md_status md_bind_state(md_system* s, void* pos, void* vel, void* force, void* q
     s->torque = s->rigid ? (float4*)torque : nullptr;
     s->bound = true;
     s->shadow_valid = false;
-    s->cells_valid = s->lists_valid = s->forces_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
+    s->cells_valid = s->lists_valid = s->forces_valid = s->seg_valid = s->staged_valid = s->legacy_valid = s->cluster_valid = false;
     drop_step_graph(s);   // the step graph bakes the state pointers in
     reset_ids(s);   // the arrays are taken to be in original id order
     return check_cuda(s, "md_bind_state");
@@ -430,7 +436,7 @@ md_status md_set_order(md_system* s, int32_t order) {
     int nc[3] = { s->P.ncx, s->P.ncy, s->P.ncz };
     make_cell_rank(nc, order, rank);
     upload_cell_rank(s, rank);
-    s->cells_valid = s->lists_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
+    s->cells_valid = s->lists_valid = s->seg_valid = s->staged_valid = s->legacy_valid = s->cluster_valid = false;
     return check_cuda(s, "md_set_order");
 }
 
@@ -487,7 +493,7 @@ md_status md_build_cells(md_system* s) {
     ensure_shadows(s);
     md_launch_build_cells(s, false);
     s->cells_valid = true;
-    s->lists_valid = s->seg_valid = s->staged_valid = s->legacy_valid = false;
+    s->lists_valid = s->seg_valid = s->staged_valid = s->legacy_valid = s->cluster_valid = false;
     return check_cuda(s, "md_build_cells");
 }
 
@@ -495,7 +501,7 @@ md_status md_build_verlet(md_system* s) {
     if (!s) return MD_ERR_INVALID;
     if (s->sticky) return (md_status)s->sticky;
     if (!s->bound || !s->cells_valid) return fail(s, MD_ERR_STATE, "md_build_verlet: call md_build_cells first");
-    s->staged_valid = s->legacy_valid = s->seg_valid = false;
+    s->staged_valid = s->legacy_valid = s->seg_valid = s->cluster_valid = false;
     if (s->order != MD_ORDER_NONE) {
         // cell-sorted storage: rows of block-local indices (md_staged.cu); the explicit global-slot lists of the
         // L2-gather variants are derived lazily from the same cells and the build-time positions (ensure_explicit)
@@ -524,6 +530,18 @@ static void ensure_explicit(md_system* s) {
     s->seg_valid = false;
 }
 
+// The (cluster, j) unit list of MD_SCATTER_CLUSTER for the current build, made on demand like the explicit lists.
+static md_status ensure_cluster(md_system* s) {
+    if (s->cluster_valid) return MD_OK;
+    DevCtrl before;      // the build recounts E from its own units: the counters must come out the same
+    (void)before;
+    if (!md_launch_build_cluster(s, false, s->B.pos_ref)) return fail(s, MD_ERR_CAPACITY, "MD_SCATTER_CLUSTER: max_neigh too large for the cluster build's shared memory");
+    s->cluster_valid = true;
+    return MD_OK;
+}
+
+static bool wants_cluster(int32_t strategy, int32_t variant) { return strategy == MD_EDGE && variant == MD_SCATTER_CLUSTER; }
+
 // which list representation a (strategy, variant) pair runs on
 static bool wants_staged(const md_system* s, int32_t strategy, int32_t variant) {
     if (s->order == MD_ORDER_NONE) return false;
@@ -538,7 +556,7 @@ static md_status check_strategy(md_system* s, int32_t strategy, int32_t scatter)
         if ((size_t)(m * s->N) > s->ecap) return fail(s, MD_ERR_INVALID, "MD_VERTEX_N3: m * N exceeds the edge capacity N * max_neigh / 2");
         return MD_OK;
     }
-    if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_SEGMENTED)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
+    if (strategy == MD_EDGE && (scatter < MD_SCATTER_RED || scatter > MD_SCATTER_CLUSTER)) return fail(s, MD_ERR_INVALID, "unknown scatter variant");
     if (strategy == MD_VERTEX && (scatter < MD_GATHER_AUTO || scatter > MD_GATHER_SMEM)) return fail(s, MD_ERR_INVALID, "unknown gather variant");
     if (s->order == MD_ORDER_NONE && strategy == MD_VERTEX && scatter == MD_GATHER_SMEM)
         return fail(s, MD_ERR_STATE, "the shared-memory staged variant needs cell-sorted storage: md_set_order(MD_ORDER_CELL or MD_ORDER_HILBERT)");
@@ -605,6 +623,7 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
                 s->stream = s->aux_stream;
                 md_launch_build_cells(s, true);
                 if (staged) md_launch_build_staged(s, true);
+                else if (wants_cluster(strategy, scatter)) md_launch_build_cluster(s, true, s->pos);
                 else md_launch_build_verlet(s, true, s->pos);
                 if (seg) md_launch_seg_index(s, true);
                 md_launch_build_end(s, true);
@@ -649,6 +668,8 @@ md_status md_forces(md_system* s, int32_t strategy, int32_t scatter) {
     if (st != MD_OK) return st;
     if (wants_staged(s, strategy, scatter)) {
         if (!s->staged_valid) return fail(s, MD_ERR_STATE, "md_forces: staged lists are not valid, call md_build_cells + md_build_verlet");
+    } else if (wants_cluster(strategy, scatter)) {
+        if ((st = ensure_cluster(s)) != MD_OK) return st;
     } else {
         ensure_explicit(s);
         if (strategy == MD_EDGE && scatter == MD_SCATTER_SEGMENTED && !s->seg_valid) {
@@ -711,7 +732,9 @@ static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t 
     const bool staged = wants_staged(s, strategy, scatter);
     const bool seg = strategy == MD_EDGE && scatter == MD_SCATTER_SEGMENTED;
     if (staged && !s->staged_valid) return fail(s, MD_ERR_STATE, "md_integrate: staged lists are not valid, call md_build_cells + md_build_verlet");
-    if (!staged) ensure_explicit(s);
+    const bool cluster = wants_cluster(strategy, scatter);
+    if (cluster) { if ((st = ensure_cluster(s)) != MD_OK) return st; }
+    else if (!staged) ensure_explicit(s);
     if (seg && !s->seg_valid) { md_launch_seg_index(s, false); s->seg_valid = true; }
     const float fdt = (float)dt;
     s->dt_d = dt;
@@ -737,6 +760,7 @@ static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t 
         md_launch_kick_drift(s, fdt, false);     // sets the device rebuild flag (S:A5)
         md_launch_build_cells(s, true);          // gated on the flag: no host synchronisation (S:H6)
         if (staged) md_launch_build_staged(s, true);
+        else if (cluster) md_launch_build_cluster(s, true, s->pos);
         else md_launch_build_verlet(s, true, s->pos);
         if (seg) md_launch_seg_index(s, true);
         md_launch_build_end(s, true);
@@ -745,8 +769,9 @@ static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t 
     }
     if (nsteps > 0) {
         // a device-side rebuild may have replaced the lists of the representation in use; the other one is stale
-        if (staged) { s->legacy_valid = false; s->seg_valid = false; }
-        else { s->staged_valid = false; if (!seg) s->seg_valid = false; }
+        if (staged) { s->legacy_valid = false; s->seg_valid = false; s->cluster_valid = false; }
+        else if (cluster) { s->legacy_valid = false; s->seg_valid = false; s->staged_valid = false; }
+        else { s->staged_valid = false; s->cluster_valid = false; if (!seg) s->seg_valid = false; }
         s->cells_valid = false;
     }
     return check_cuda(s, "md_integrate");

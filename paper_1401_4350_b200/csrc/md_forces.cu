@@ -516,7 +516,8 @@ static void launch_edge(md_system* s, int scatter) {
     } else {
         k_zero4<<<nbN, 256, 0, s->stream>>>(P, s->force, tq);
         s->launches += 1;
-        if (scatter == MD_SCATTER_RED) k_edge_red<KIND, false><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
+        if (scatter == MD_SCATTER_CLUSTER) { md_launch_edge_cluster(s); s->launches -= 1; }
+        else if (scatter == MD_SCATTER_RED) k_edge_red<KIND, false><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
         else if (scatter == MD_SCATTER_RED_V4) k_edge_red<KIND, true><<<persistent, 256, 0, s->stream>>>(P, s->B, s->pos, s->quat, s->force, tq);
         else {
             const double half_row = (double)s->n_edges_host / (double)P.N;   // E / N at the last synchronised build (0 if unknown)

@@ -42,6 +42,9 @@ struct DevCtrl {
     int pad1;
     unsigned long long n_in;     // E_in: listed pairs inside the cutoff at the current positions (md_stats_ex)
     unsigned long long n_units;  // (cluster, j) units of the cluster list (MD_SCATTER_CLUSTER)
+    unsigned long long n_cl_pairs; // sum of their popcounts = E
+    unsigned int cl_cursor;      // next free slot of cl_units (rounds of 32)
+    int pad2[5];
 };
 
 // per-block header of the staged path
@@ -124,6 +127,9 @@ struct DevBuffers {
     int* lo_count;         // [Npad] neighbours with slot < i
     BlkInfo* blk;          // [nblk]
     int2* seg;             // [nblk*MD_SEGMAX] (first slot, first local index)
+    // cluster list of MD_SCATTER_CLUSTER (md_cluster.cu)
+    uint2* cl_units;       // [ucap] (j | image << 31, 16-bit owner mask), per cluster `rounds` x 32 lanes
+    int2* cl_info;         // [ceil(N / MD_CLUSTER)] (first unit, rounds)
     // mixed precision (S:8(f3)): fp64 copies of the integrated state, two 16-byte planes per array so that the
     // reordering moves them like any other plane: [0] pos (x,y) [1] pos (z,-) [2] vel (x,y) [3] vel (z,-)
     // [4] angmom (x,y) [5] angmom (z,-) [6] quat (w,x) [7] quat (y,z)
@@ -136,6 +142,7 @@ struct md_system {
     cudaStream_t stream;
     int64_t N;
     size_t ecap;
+    size_t ucap;             // capacity of cl_units
     double rcut, skin;
     md_potential pot;
     int order;
@@ -192,6 +199,10 @@ void md_launch_count_in_cutoff(md_system* s);                             // ctr
 void md_staged_configure(md_system* s);                                   // per-device kernel attributes of md_staged.cu
 int md_staged_threads_per_particle(const md_system* s);                   // NS the staged LJ launch would use (0: rigid)
 bool md_run_probe(md_system* s, int kind, double* value);                 // md_probe.cu
+// cluster list (md_cluster.cu)
+void md_cluster_configure(md_system* s);
+bool md_launch_build_cluster(md_system* s, bool gated, const float4* pos_src);
+void md_launch_edge_cluster(md_system* s);                                // force / torque zeroed by the caller
 // staged path (md_staged.cu)
 void md_launch_build_staged(md_system* s, bool gated);
 void md_launch_edges_from_rows(md_system* s);     // explicit (i, j) edge list from the staged rows (export / legacy EDGE variants)

@@ -22,7 +22,7 @@ def test_c2_full_size_parity(oracle):
     fmax = np.abs(o["F"]).max()
     tol = 1e-4 * fmax + 1e-6
     for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "red_v4"), ("edge", "warp"),
-                      ("edge", "segmented"), ("vertex_n3", 12)]:
+                      ("edge", "segmented"), ("edge", "cluster"), ("vertex_n3", 12)]:
         s.forces(strat, sc)
         F = s.in_id_order(s.force)
         assert np.abs(F[:, :3] - o["F"]).max() <= tol, (strat, sc)
@@ -59,7 +59,7 @@ def test_c3_c4_full_size_parity(oracle, name):
     s.build_cells(); s.build_verlet()
     assert s.stats()["n_edges"] == oracle.pair_count(w.pos, w.box, w.rcut, w.skin)
     o = oracle.forces(w.pos, w.box, dict(w.potential), quat=w.quat)
-    variants = [("vertex", "smem"), ("vertex", "l2"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented"), ("vertex_n3", 4)]
+    variants = [("vertex", "smem"), ("vertex", "l2"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented"), ("edge", "cluster"), ("vertex_n3", 4)]
     for strat, sc in variants:
         s.forces(strat, sc)
         F = s.in_id_order(s.force)
@@ -89,7 +89,7 @@ def test_c2b_many_neighbours(oracle):
     s.build_cells(); s.build_verlet()
     st = s.stats()
     o = oracle.forces(w.pos, w.box, dict(w.potential))
-    for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp")]:
+    for strat, sc in [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp"), ("edge", "cluster")]:
         s.forces(strat, sc)
         F = s.in_id_order(s.force)
         assert np.abs(F[:, :3] - o["F"]).max() <= 1e-4 * np.abs(o["F"]).max() + 1e-6

@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 # the shared-memory staged VERTEX variant needs cell-sorted storage (order != none)
 # VERTEX with Newton's third law (S:8(f1)): the variant is m, the number of private force copies per particle
 VARIANTS = [("vertex", "l2"), ("edge", "red"), ("edge", "red_v4"), ("edge", "warp"), ("edge", "segmented"),
-            ("vertex_n3", 1), ("vertex_n3", 12)]
+            ("edge", "cluster"), ("vertex_n3", 1), ("vertex_n3", 12)]
 STAGED = [("vertex", "smem")]
 
 
@@ -93,6 +93,11 @@ def test_step0_parity(MD, oracle, case, order):
             continue
         s.forces(strat, sc)
         results[(strat, sc)] = assert_forces(s, o, w.quat is not None)
+        if sc == "cluster":      # the unit list is a partition of the half list: sum of popcounts = E
+            sx = s.stats_ex()
+            assert sx["cluster_size"] == 16 and 0 < sx["n_cluster_units"] <= sx["n_edges"]
+            assert sx["n_edges"] == oracle.pair_count(w.pos, w.box, w.rcut, w.skin)
+            assert sx["n_in_cutoff"] == o["n_in_cut"]                      # E_in by the device counter (S:Q16)
     # the explicit global-slot lists (built on demand for the L2-gather variants) hold the same pair set
     assert_pairs(s, oracle, w.pos, w.box, w.rcut, w.skin)
     # P11: the strategies agree with each other within twice the oracle tolerance
@@ -215,7 +220,7 @@ def test_error_paths(MD):
 
 
 @pytest.mark.parametrize("strat,sc", [("vertex", "smem"), ("vertex", "l2"), ("edge", "warp"),
-                                      ("edge", "segmented"), ("vertex_n3", 12)])
+                                      ("edge", "segmented"), ("edge", "cluster"), ("vertex_n3", 12)])
 def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
     """C1 (BASELINE.json configs[0]): 100 velocity-Verlet steps at dt = 0.002; fp32 GPU state against the fp64
     oracle trajectory from the same fp32 input.  SURVEY 8(d): the two stay within the force tolerance for 100 steps."""
@@ -244,6 +249,7 @@ def test_c1_trajectory_100_steps(MD, oracle, strat, sc):
     ("polymer", 200, "vertex", "smem"), ("polymer", 200, "edge", "warp"), 
     ("patchy", 300, "vertex", "smem"), ("patchy", 300, "vertex", "l2"), ("patchy", 300, "edge", "segmented"),
     ("lj", 300, "vertex_n3", 12), ("polymer", 200, "vertex_n3", 4), ("patchy", 300, "vertex_n3", 12),
+    ("lj", 300, "edge", "cluster"), ("polymer", 200, "edge", "cluster"), ("patchy", 300, "edge", "cluster"),
     ])
 def test_snapshot_parity_after_device_side_rebuilds(MD, oracle, case, steps, strat, sc):
     """Run md_integrate long enough for several skin-triggered rebuilds, then compare the forces the path holds
