@@ -5,6 +5,7 @@ import numpy as np
 import pytest
 
 import workloads as W
+from conftest import record_margin
 
 pytestmark = pytest.mark.gpu
 
@@ -43,19 +44,24 @@ def assert_pairs(s, oracle, pos, box, rcut, skin):
     return ref.shape[0]
 
 
-def assert_forces(s, o, rigid):
+def assert_forces(s, o, rigid, label=("", "")):
     fmax = np.abs(o["F"]).max()
     F = s.in_id_order(s.force)
     tol = FTOL_REL * fmax + FTOL_ABS
-    assert np.abs(F[:, :3] - o["F"]).max() <= tol
+    err = np.abs(F[:, :3] - o["F"]).max()
+    record_margin(label[0], label[1], "F", err, tol)
+    assert err <= tol
     # per-particle energies feed md_energy: compare the total to 1e-5 relative
     U, Kt, Kr = s.energy()
     Uo = o["pe"].sum()
+    record_margin(label[0], label[1], "U", abs(U - Uo), ETOL * max(abs(Uo), abs(Uo) + Kt + Kr, 1e-30))
     assert abs(U - Uo) <= ETOL * max(abs(Uo), 1e-30) or abs(U - Uo) <= ETOL * (abs(Uo) + Kt + Kr)   # S:Q17
     if rigid:
         tmax = np.abs(o["T"]).max()
         T = s.in_id_order(s.torque)
-        assert np.abs(T[:, :3] - o["T"]).max() <= FTOL_REL * tmax + FTOL_ABS
+        terr = np.abs(T[:, :3] - o["T"]).max()
+        record_margin(label[0], label[1], "T", terr, FTOL_REL * tmax + FTOL_ABS)
+        assert terr <= FTOL_REL * tmax + FTOL_ABS
     return F
 
 
@@ -92,7 +98,7 @@ def test_step0_parity(MD, oracle, case, order):
             assert e.value.code == -1
             continue
         s.forces(strat, sc)
-        results[(strat, sc)] = assert_forces(s, o, w.quat is not None)
+        results[(strat, sc)] = assert_forces(s, o, w.quat is not None, (f"{case}/{order}", f"{strat}_{sc}"))
         if sc == "cluster":      # the unit list is a partition of the half list: sum of popcounts = E
             sx = s.stats_ex()
             assert sx["cluster_size"] == 16 and 0 < sx["n_cluster_units"] <= sx["n_edges"]
@@ -264,7 +270,7 @@ def test_snapshot_parity_after_device_side_rebuilds(MD, oracle, case, steps, str
     pos = s.in_id_order(s.pos)
     quat = s.in_id_order(s.quat) if w.quat is not None else None
     o = oracle.forces(pos, w.box, dict(w.potential), quat=quat)
-    assert_forces(s, o, quat is not None)
+    assert_forces(s, o, quat is not None, (f"{case} after {steps} steps", f"{strat}_{sc}"))
     s.build_cells(); s.build_verlet()
     pos2 = s.in_id_order(s.pos)                               # wrapped by the build
     assert_pairs(s, oracle, pos2, w.box, w.rcut, w.skin)
