@@ -130,7 +130,10 @@ typedef enum {
                                kernels: blocks with a larger neighbourhood take the unstaged path (tests of that path) */
     MD_OPT_NO_GRAPH = 1,    /* != 0: md_integrate launches its kernels one by one instead of replaying CUDA graphs
                                (profilers then list every kernel); same results bit for bit                          */
-    MD_OPT_DEBUG = 2        /* != 0: step-graph construction failures are printed on stderr                         */
+    MD_OPT_DEBUG = 2,       /* != 0: step-graph construction failures are printed on stderr                         */
+    MD_OPT_ROW_SCHEDULE = 3 /* staged Verlet rows: 1 (default) = entries ordered at build time by shared-memory bank column
+                               so that the 128-bit gathers of the force kernels are conflict-free; 0 = scan order (a
+                               cheaper build, more bank conflicts per force evaluation).  Invalidates the lists.      */
 } md_option;
 
 /* md_probe kinds: machine ceilings other than HBM bandwidth that bound the force kernels (S:8(d)). */

@@ -15,7 +15,7 @@ SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3, "cluster": 4}
 GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
 PRECISION = {"f32": 0, "mixed": 1}
-OPTION = {"stage_limit": 0, "no_graph": 1, "debug": 2}
+OPTION = {"stage_limit": 0, "no_graph": 1, "debug": 2, "row_schedule": 3}
 PROBE = {"ffma": 0, "ffma2": 1, "mufu": 2, "red_v4_scatter": 3, "red_f32_scatter": 4, "red_v4_coalesced": 5,
          "red_f32_coalesced": 6}
 POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2, "patchy_pp": 3}

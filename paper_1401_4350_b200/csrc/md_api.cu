@@ -327,7 +327,8 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.rv2 = (float)P.rv2d;
     P.band_rv = (float)(P.rv2d * 1e-6);    // S:Q6 band of the list predicate
     P.nblk = g.nblk; P.rcap = g.rcap; P.mask_words = g.mask_words;
-    P.use_masks = ((double)N / (double)g.ncell >= 8.0) ? 1 : 0;   // measured: masks win at 17.7 particles per cell, lists at 2.5-3
+    P.use_masks = ((double)N / (double)g.ncell >= 8.0) ? 1 : 0;
+    P.row_schedule = 1;   // measured: masks win at 17.7 particles per cell, lists at 2.5-3
     P.stage_cap = (int)((224 * 1024 - 16) / (rigid ? 32 : 16)) - 1;
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);
@@ -563,9 +564,10 @@ static md_status check_strategy(md_system* s, int32_t strategy, int32_t scatter)
     return MD_OK;
 }
 
-static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatter) {
+// energy = false: nobody can observe force.w of this evaluation (an inner step of a multi-step graph)
+static md_status launch_forces_any(md_system* s, int32_t strategy, int32_t scatter, bool energy = true) {
     if (wants_staged(s, strategy, scatter)) {
-        if (!md_launch_forces_staged(s)) return fail(s, MD_ERR_CAPACITY, "staged neighbourhood does not fit in shared memory");
+        if (!md_launch_forces_staged(s, energy)) return fail(s, MD_ERR_CAPACITY, "staged neighbourhood does not fit in shared memory");
     } else {
         md_launch_forces(s, strategy, scatter);
     }
@@ -638,7 +640,7 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     }
     const int64_t before_tail = s->launches;
     if (ok) {
-        ok = launch_forces_any(s, strategy, scatter) == MD_OK;
+        ok = launch_forces_any(s, strategy, scatter, rep_i == reps - 1) == MD_OK;   // md_energy sees the last step only
         if (rep_i == reps - 1) md_launch_kick(s, fdt);   // inner steps: fused into the next kick+drift
     }
     tail_nodes = (int)(s->launches - before_tail);
@@ -838,6 +840,11 @@ md_status md_set_option(md_system* s, int32_t option, int64_t value) {
         drop_step_graph(s);            // the step graph bakes the launch capacity in
         return MD_OK;
     case MD_OPT_NO_GRAPH: s->no_graph = value != 0; return MD_OK;
+    case MD_OPT_ROW_SCHEDULE:
+        s->P.row_schedule = value != 0 ? 1 : 0;
+        drop_step_graph(s);            // the graph bakes the parameter block in
+        s->lists_valid = s->staged_valid = s->legacy_valid = s->seg_valid = s->cluster_valid = false;
+        return MD_OK;
     case MD_OPT_DEBUG: s->debug = value != 0; return MD_OK;
     default: return fail(s, MD_ERR_INVALID, "md_set_option: unknown option");
     }

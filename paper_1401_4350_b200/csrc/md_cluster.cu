@@ -193,11 +193,11 @@ __global__ void __launch_bounds__(32 * CLB_WARPS) k_build_cluster(DevParams P, D
 
 template <int KIND>
 struct ClusterSmem {
-    float px[MD_CLUSTER], py[MD_CLUSTER], pz[MD_CLUSTER], pw[MD_CLUSTER];   // owner positions, one 64-byte row per coordinate:
+    float px[MD_CLUSTER + 4], py[MD_CLUSTER + 4], pz[MD_CLUSTER + 4], pw[MD_CLUSTER + 4];   // [MD_CLUSTER] = the dummy owner at 1e15   // owner positions, one 64-byte row per coordinate:
                                                                             // a lookup by a lane-varying owner index is three
                                                                             // conflict-free broadcast loads (one wavefront each)
     float4 qi[md_is_rigid(KIND) ? MD_CLUSTER : 1];
-    float4 acc[MD_CLUSTER * 32];
+    float4 acc[(MD_CLUSTER + 1) * 32];      // row MD_CLUSTER: the dummy owner (collects exact zeros)
     float4 tacc[md_is_rigid(KIND) ? MD_CLUSTER * 32 : 1];
 };
 
@@ -211,14 +211,15 @@ __global__ void __launch_bounds__(32 * CLF_WARPS) k_edge_cluster(DevParams P, De
     const int ncl = (P.N + MD_CLUSTER - 1) / MD_CLUSTER;
     const int nwarps = gridDim.x * CLF_WARPS;
     const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int k = 0; k < MD_CLUSTER; ++k) {
-        S.acc[k * 32 + lane] = zero4;
-        if (RIGID) S.tacc[k * 32 + lane] = zero4;
-    }
+    for (int k = 0; k <= MD_CLUSTER; ++k) S.acc[k * 32 + lane] = zero4;
+    if (RIGID) for (int k = 0; k < MD_CLUSTER; ++k) S.tacc[k * 32 + lane] = zero4;
+    if (lane < 4) { S.px[MD_CLUSTER + lane] = 1.0e15f; S.py[MD_CLUSTER + lane] = 1.0e15f; S.pz[MD_CLUSTER + lane] = 1.0e15f; }
     const uint2* __restrict__ units = B.cl_units;
     // potential constants of the LJ pair function pinned in registers (otherwise reloaded from the constant bank per pair)
-    float c_a = P.lj_a, c_b = P.lj_b, c_hc = 0.5f * P.lj_c, c_hd = 0.5f * P.lj_d, c_hvs = 0.5f * P.vshift, c_rc2 = P.rc2, c_band = P.band_abs;
-    asm volatile("" : "+f"(c_a), "+f"(c_b), "+f"(c_hc), "+f"(c_hd), "+f"(c_hvs), "+f"(c_rc2), "+f"(c_band));
+    const float c_band = P.band_abs;
+    const float2 c2_nrc2 = make_float2(-P.rc2, -P.rc2), c2_a = make_float2(P.lj_a, P.lj_a), c2_nb = make_float2(-P.lj_b, -P.lj_b),
+                 c2_hc = make_float2(0.5f * P.lj_c, 0.5f * P.lj_c), c2_nhd = make_float2(-0.5f * P.lj_d, -0.5f * P.lj_d),
+                 c2_nhvs = make_float2(-0.5f * P.vshift, -0.5f * P.vshift);
     for (int c = blockIdx.x * CLF_WARPS + w; c < ncl; c += nwarps) {
         const int i0 = c * MD_CLUSTER;
         const int2 info = B.cl_info[c];
@@ -250,16 +251,16 @@ __global__ void __launch_bounds__(32 * CLF_WARPS) k_edge_cluster(DevParams P, De
                 if (RIGID) qn = ldg4(quat + (un.x & 0x7fffffffu));
             }
             float fjx = 0.f, fjy = 0.f, fjz = 0.f, pej = 0.f, tjx = 0.f, tjy = 0.f, tjz = 0.f;
-            while (mask) {               // one lane-iteration per listed pair
-                const int k = __ffs(mask) - 1;
-                mask &= mask - 1u;
-                const float4 xi = make_float4(S.px[k], S.py[k], S.pz[k], 0.f);
-                float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
-                if (img) {
-                    dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
-                }
-                const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                if (RIGID) {
+            if (RIGID) {
+                while (mask) {           // one lane-iteration per listed pair
+                    const int k = 31 - __clz(mask);
+                    mask ^= 1u << k;
+                    const float4 xi = make_float4(S.px[k], S.py[k], S.pz[k], 0.f);
+                    float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
+                    if (img) {
+                        dx = min_image(xj.x, xi.x, P.Lx, P.hLx); dy = min_image(xj.y, xi.y, P.Ly, P.hLy); dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
+                    }
+                    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                     if (in_cutoff(P, d2, xi, xj)) {
                         const Rot Ri = quat_to_rot(S.qi[k]);
                         float fx, fy, fz, V, tix, tiy, tiz, ax, ay, az;
@@ -272,20 +273,43 @@ __global__ void __launch_bounds__(32 * CLF_WARPS) k_edge_cluster(DevParams P, De
                         tq.x += tix; tq.y += tiy; tq.z += tiz;
                         S.acc[k * 32 + lane] = a; S.tacc[k * 32 + lane] = tq;
                     }
-                } else {
-                    // the cutoff enters as a 0/1 factor m (no select, no branch but the rare fp64 band): s = m / d2, so force
-                    // and energy of an outside pair are exactly zero; constants pinned in registers above, energy halved
-                    const float tt = d2 - c_rc2;
-                    float m = tt < 0.0f ? 1.0f : 0.0f;
-                    if (fabsf(tt) < c_band) m = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rc2d) ? 1.0f : 0.0f;   // S:Q5 / S:H10
-                    const float s = rcp_approx(d2) * m;
-                    const float z3 = s * s * s;
-                    const float g = (s * z3) * fmaf(c_a, z3, -c_b);               // 24 eps s6 (2 s6 - 1) / d2
-                    const float hV = fmaf(m, -c_hvs, z3 * fmaf(c_hc, z3, -c_hd));  // (4 eps s6 (s6 - 1) - V_c) / 2
-                    fjx = fmaf(g, dx, fjx); fjy = fmaf(g, dy, fjy); fjz = fmaf(g, dz, fjz); pej += hV;
-                    float4 a = S.acc[k * 32 + lane];
-                    a.x = fmaf(-g, dx, a.x); a.y = fmaf(-g, dy, a.y); a.z = fmaf(-g, dz, a.z); a.w += hV;
-                    S.acc[k * 32 + lane] = a;
+                }
+            } else {
+                // LJ / WCA: TWO listed pairs of the unit per lane-iteration (owners ka, kb; kb = the dummy owner MD_CLUSTER, parked
+                // at 1e15, when the unit has an odd pair left): two independent dependency chains per lane, and the cutoff
+                // factor, 1/d2, s6 and the force / energy polynomials of both pairs in packed f32x2 instructions.  The
+                // cutoff enters as a 0/1 factor m (s = m / d2): force and energy of an outside pair are exactly zero.
+                while (mask) {
+                    const int ka = 31 - __clz(mask);
+                    mask ^= 1u << ka;
+                    int kb = 31 - __clz(mask);                       // -1 when the mask is empty now
+                    kb = kb < 0 ? MD_CLUSTER : kb;
+                    mask &= ~(1u << kb);
+                    const float4 xa = make_float4(S.px[ka], S.py[ka], S.pz[ka], 0.f), xb = make_float4(S.px[kb], S.py[kb], S.pz[kb], 0.f);
+                    float dxa = xj.x - xa.x, dya = xj.y - xa.y, dza = xj.z - xa.z;
+                    float dxb = xj.x - xb.x, dyb = xj.y - xb.y, dzb = xj.z - xb.z;
+                    if (img) {
+                        dxa = min_image(xj.x, xa.x, P.Lx, P.hLx); dya = min_image(xj.y, xa.y, P.Ly, P.hLy); dza = min_image(xj.z, xa.z, P.Lz, P.hLz);
+                        dxb = min_image(xj.x, xb.x, P.Lx, P.hLx); dyb = min_image(xj.y, xb.y, P.Ly, P.hLy); dzb = min_image(xj.z, xb.z, P.Lz, P.hLz);
+                    }
+                    const float2 d2 = make_float2(fmaf(dza, dza, fmaf(dya, dya, dxa * dxa)), fmaf(dzb, dzb, fmaf(dyb, dyb, dxb * dxb)));
+                    const float2 tt = __fadd2_rn(d2, c2_nrc2);
+                    float2 m = make_float2(tt.x < 0.0f ? 1.0f : 0.0f, tt.y < 0.0f ? 1.0f : 0.0f);
+                    if (fminf(fabsf(tt.x), fabsf(tt.y)) < c_band) {          // S:Q5 / S:H10: fp64 decision inside the band (rare)
+                        if (fabsf(tt.x) < c_band) m.x = inside_fp64(xa, xj, P.dLx, P.dLy, P.dLz, P.rc2d) ? 1.0f : 0.0f;
+                        if (fabsf(tt.y) < c_band) m.y = inside_fp64(xb, xj, P.dLx, P.dLy, P.dLz, P.rc2d) ? 1.0f : 0.0f;
+                    }
+                    const float2 s = __fmul2_rn(make_float2(rcp_approx(d2.x), rcp_approx(d2.y)), m);
+                    const float2 z3 = __fmul2_rn(__fmul2_rn(s, s), s);
+                    const float2 g = __fmul2_rn(__fmul2_rn(s, z3), __ffma2_rn(c2_a, z3, c2_nb));     // 24 eps s6 (2 s6 - 1) / d2
+                    const float2 hV = __ffma2_rn(m, c2_nhvs, __fmul2_rn(z3, __ffma2_rn(c2_hc, z3, c2_nhd)));   // (4 eps s6 (s6 - 1) - V_c) / 2
+                    fjx = fmaf(g.x, dxa, fjx); fjy = fmaf(g.x, dya, fjy); fjz = fmaf(g.x, dza, fjz);
+                    fjx = fmaf(g.y, dxb, fjx); fjy = fmaf(g.y, dyb, fjy); fjz = fmaf(g.y, dzb, fjz);
+                    pej += hV.x + hV.y;
+                    float4 a = S.acc[ka * 32 + lane], b = S.acc[kb * 32 + lane];
+                    a.x = fmaf(-g.x, dxa, a.x); a.y = fmaf(-g.x, dya, a.y); a.z = fmaf(-g.x, dza, a.z); a.w += hV.x;
+                    b.x = fmaf(-g.y, dxb, b.x); b.y = fmaf(-g.y, dyb, b.y); b.z = fmaf(-g.y, dzb, b.z); b.w += hV.y;
+                    S.acc[ka * 32 + lane] = a; S.acc[kb * 32 + lane] = b;
                 }
             }
             // a unit none of whose pairs is inside the cutoff contributes exact zeros and issues no reduction

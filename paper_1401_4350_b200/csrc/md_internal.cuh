@@ -68,6 +68,7 @@ struct DevParams {
     float rv2, band_rv;                // fp32 list radius^2 and its fp64-recheck band (S:Q6)
     int nblk, stage_cap, rcap, mask_words;   // mask_words: 32-bit candidate-mask words per stencil cell (build scratch)
     int use_masks;                     // staged build: candidate masks (1) or index lists (0, few particles per cell)
+    int row_schedule;                  // staged build: 1 = rows ordered by bank column (pass B buckets), 0 = scan order (MD_OPT_ROW_SCHEDULE)
     float skinf;
     float shift_margin;                // r_v + skin: see k_build_staged step 7c
     // pair potential
@@ -206,7 +207,7 @@ void md_launch_edge_cluster(md_system* s);                                // for
 // staged path (md_staged.cu)
 void md_launch_build_staged(md_system* s, bool gated);
 void md_launch_edges_from_rows(md_system* s);     // explicit (i, j) edge list from the staged rows (export / legacy EDGE variants)
-bool md_launch_forces_staged(md_system* s);             // VERTEX on the staged rows
+bool md_launch_forces_staged(md_system* s, bool energy);   // VERTEX on the staged rows; energy = false: force.w is not needed
 size_t md_staged_smem_bytes(const md_system* s, int stage_entries);
 
 #define MD_ERRBUF(s, ...) snprintf((s)->errmsg, sizeof((s)->errmsg), __VA_ARGS__)

@@ -112,6 +112,50 @@ __device__ __forceinline__ int scan_cell_mask(const float4* __restrict__ cellpos
     return found;
 }
 
+// Candidate scan of one stencil cell FUSED with the column bucketing of pass B (dense cells).  All lanes of a warp walk the
+// same cell, candidate by candidate, so the bank column of the candidate (local index & 7) is warp-uniform: the walk is
+// aligned to groups of eight local indices and unrolled by eight, which makes the column a compile-time constant of every
+// unrolled slot -- the eight column populations pc[] stay in registers with static indexing and a neighbour goes to its
+// bucket with one predicated 16-bit store.  No candidate masks are written or decoded (they were 226 MB of scratch traffic
+// and a decode loop that ran at 9 of 32 lanes, profiles/r01d_ncu.md).  tb = bucket 0, entry 0 of this thread (entries are
+// MD_TB apart, buckets cap8 entries apart); a bucket that outgrows cap8 keeps overwriting its last slot and is reported
+// by the caller (pc[u] > cap8).
+template <bool SHIFT, bool SELF>
+__device__ __forceinline__ void scan_cell_bucket(const float4* __restrict__ cellpos, int n, int t0, int me, float4 xi, float rv2,
+                                                 float hLx, float hLy, float hLz, float tLx, float tLy, float tLz,
+                                                 unsigned short* __restrict__ tb, int cap8, int (&pc)[8], float& bandmin) {
+    const int a = t0 & 7;
+    const float4* __restrict__ cp = cellpos - a;     // index kk = candidate + a: local index tb0 + kk has column kk & 7
+    const int tb0 = t0 - a, kend = n + a;
+    auto one = [&](int u, int kk) {
+        float4 xj = __ldg(cp + kk);
+        if (SHIFT) {
+            if (xj.x > hLx) xj.x -= tLx;
+            if (xj.y > hLy) xj.y -= tLy;
+            if (xj.z > hLz) xj.z -= tLz;
+        }
+        const float ddx = xj.x - xi.x, ddy = xj.y - xi.y, ddz = xj.z - xi.z;
+        const float tt = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)) - rv2;
+        bandmin = fminf(bandmin, fabsf(tt));
+        int m = __float_as_int(tt) >> 31;                    // -1 inside r_v, 0 outside
+        const int t = tb0 + kk;
+        if (SELF) m = (t == me) ? 0 : m;
+        const int p = min(pc[u], cap8 - 1);
+        if (m) tb[(size_t)(u * cap8 + p) * MD_TB] = (unsigned short)t;
+        pc[u] -= m;
+    };
+    for (int g = 0; g < kend; g += 8) {
+        if (g >= a && g + 8 <= kend) {                       // a full aligned group: no bounds checks
+#pragma unroll
+            for (int u = 0; u < 8; ++u) one(u, g + u);
+        } else {
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (g + u >= a && g + u < kend) one(u, g + u);
+        }
+    }
+}
+
 // LIST form of the candidate scan, used when cells hold few particles (mask_words == 0: at 2-3 particles per cell 27
 // mostly empty mask words per thread cost more than ~10 index stores).  All lanes of a warp walk the same cell, so
 // the loop is kept branch-free: a predicated store at the thread's write offset, which advances (by one scratch row)
@@ -168,7 +212,7 @@ __device__ __noinline__ int scan_cell_slow(const float4* __restrict__ cellpos, i
 // S:A4 staged Verlet build.  One block per MD_TB slots, one thread per particle.
 // ------------------------------------------------------------------------------------------------
 template <bool MASKS>
-__global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
+__global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
                                                         int ncand_cap, int umax, int tbl_cap) {
     GATE(B, gated);
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -404,6 +448,8 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
     // 8. L_i = { j != i : d2 < r_v^2 }, fp32 filter + fp64 decision inside the band (S:Q6).  Pass A leaves, per
     //    stencil cell, a bitmask of the candidates inside r_v (scan_cell_mask); pass B turns the masks into the row.
     int cnt = 0, lo_cnt = 0;
+    bool bucketed = false, bucket_over = false;                   // dense cells: the scan already filled the column buckets
+    unsigned long long pops_pre = 0ull;
     const int W = P.mask_words;                                   // 32-bit mask words per stencil cell
     constexpr bool use_masks = MASKS;                             // else: list form (few particles per cell)
     unsigned int* cm = B.cmask + (size_t)b * 27 * W * MD_TB + tid;   // word (cell sc, w) at cm[(sc * W + w) * MD_TB]
@@ -437,20 +483,34 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
             cnt = (int)((off - 2u * tid) / (2u * MD_TB));   // cap + 1 = overflow
         } else if (!maywrap) {
             const float rv2 = P.rv2;
+            unsigned short* __restrict__ tb = B.rows_tmp + (size_t)b * 8 * cap8 * MD_TB + tid;
+            int pc[8] = { 0, 0, 0, 0, 0, 0, 0, 0 };
             for (int sc = 0; sc < 27; ++sc) {
                 const int u = mycells[sc];
                 if (u < 0) continue;
                 const int t0 = ubase[u];
                 int n = ubase[u + 1] - t0;
-                if (n > 32 * W) { n = 32 * W; atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); }   // cell fuller than the mask capacity
-                const int self = sc == 13 ? me - t0 : -1;        // stencil entry 13 is the own cell
+                if (n > 32 * W) { n = 32 * W; atomicOr(&B.ctrl->err, MD_DEVERR_STAGE); }   // cell fuller than the mask capacity of the careful path
                 const float4* cellpos = pos + ustart[u];
-                if (shift_ok) cnt += scan_cell_mask<true>(cellpos, n, self, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, cm + (size_t)sc * W * MD_TB, bandmin);
-                else cnt += scan_cell_mask<false>(cellpos, n, self, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, cm + (size_t)sc * W * MD_TB, bandmin);
+                if (sc == 13) {                           // stencil entry 13 is the own cell: exclude the particle itself
+                    if (shift_ok) scan_cell_bucket<true, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tb, cap8, pc, bandmin);
+                    else scan_cell_bucket<false, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tb, cap8, pc, bandmin);
+                } else {
+                    if (shift_ok) scan_cell_bucket<true, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tb, cap8, pc, bandmin);
+                    else scan_cell_bucket<false, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tb, cap8, pc, bandmin);
+                }
+            }
+            bucketed = true;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                cnt += pc[c];
+                if (pc[c] > cap8 || pc[c] > 255) bucket_over = true;
+                pops_pre |= (unsigned long long)(pc[c] & 255) << (8 * c);
             }
         }
         if (bandmin < P.band_rv) {      // rare: a banded candidate (or a block that needs the minimum image)
             cnt = 0;
+            bucketed = false;           // the careful scan leaves masks: pass B decodes them (and overwrites the buckets)
             for (int sc = 0; sc < 27; ++sc) {
                 const int u = mycells[sc];
                 if (u < 0) continue;
@@ -519,7 +579,26 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
         // the eight column populations live in one 64-bit register, 8 bits each (a column holds <= cap8 <= 255 entries)
         unsigned long long pops = 0ull, rem8 = 0ull;
         int c2e = c2;                                      // entries to emit (0 after a bucket overflow)
-        if (c2 > 0) {
+        int lo_e = 0;                                      // neighbours with a lower slot, counted while emitting
+        if (c2 > 0 && !P.row_schedule && !use_masks) {
+            // scan order, no column scheduling: the list the candidate scan left in scratch goes straight into the row
+            for (int k0 = 0; k0 < c2; k0 += 4) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int k = k0 + q;
+                    const unsigned int tq = k < c2 ? (unsigned int)tmp[(size_t)k * MD_TB] : 0x7fffffffu;
+                    lo_e += (int)tq < me ? 1 : 0;
+                    w[q] = k < c2 ? (tq << rsh) : dummy;
+                }
+                rowb[(size_t)(k0 >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+            }
+            lo_cnt = lo_e;
+            c2e = 0;                                       // nothing left for the scheduled emission below
+        } else if (c2 > 0 && bucketed) {
+            pops = pops_pre;                               // buckets filled by scan_cell_bucket; lo_cnt is counted below
+            if (bucket_over) { atomicOr(&B.ctrl->err, MD_DEVERR_CAPACITY); c2e = 0; }
+            rem8 = pops;
+        } else if (c2 > 0) {
             int lo_b = 0;
             bool over = false;
             for_each_neighbour([&](int t) {
@@ -550,9 +629,14 @@ __global__ void __launch_bounds__(MD_TB, 5) k_build_staged(DevParams P, DevBuffe
                 }
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) w[q] = src[q] >= 0 ? ((unsigned int)tmp2[(size_t)src[q] * MD_TB] << rsh) : dummy;
+            for (int q = 0; q < 4; ++q) {
+                const unsigned int tq = src[q] >= 0 ? (unsigned int)tmp2[(size_t)src[q] * MD_TB] : 0x7fffffffu;
+                lo_e += (int)tq < me ? 1 : 0;              // local indices ascend with the slot: t < me <=> slot < i  (padding never counts)
+                w[q] = src[q] >= 0 ? (tq << rsh) : dummy;
+            }
             rowb[(size_t)(k0 >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
         }
+        if (bucketed && P.row_schedule) lo_cnt = lo_e;
         if (live) {
             B.row_count[i] = c2;
             B.lo_count[i] = cnt > P.cap ? 0 : lo_cnt;
@@ -635,7 +719,7 @@ void md_launch_build_staged(md_system* s, bool gated) {
         s->build_carve = carve;
     }
     k_staged_begin<<<1, 1, 0, s->stream>>>(s->B, g);
-    if (P.use_masks) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
+    if (P.use_masks && P.row_schedule) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
     else k_build_staged<false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
     s->launches += 2;
 }
@@ -874,7 +958,9 @@ __device__ __forceinline__ void fene_vertex_s(const DevParams& P, const DevBuffe
 //   A = sum (s^4 - 2 s^7) d,  pe = sum (s^6 - s^3),  nin = sum m
 // need no potential constants inside the loop (F_i = 24 eps A, V = 4 eps pe - V_c nin are applied once per particle),
 // which removes the per-chunk constant reloads and eight registers.  a.pe holds sum (s^6 - s^3), a.nin the count.
-template <bool IMG>
+// ENERGY = false: the per-particle energy is not needed (inner steps of a multi-step md_integrate graph: md_energy can only
+// observe the forces of the LAST step) -- the pe and nin sums are dropped, ~7 % of the loop's issue slots.
+template <bool IMG, bool ENERGY>
 __device__ __forceinline__ void lj_visit2_unit_s(const DevParams& P, float4 xi, float4 xa, float4 xb, LJAccS& a) {
     float dxa, dya, dza, dxb, dyb, dzb;
     if (IMG) {
@@ -897,17 +983,19 @@ __device__ __forceinline__ void lj_visit2_unit_s(const DevParams& P, float4 xi, 
     const float2 ng = __ffma2_rn(z7, make_float2(-2.0f, -2.0f), z4);
     a.fx = fmaf(ng.x, dxa, a.fx); a.fy = fmaf(ng.x, dya, a.fy); a.fz = fmaf(ng.x, dza, a.fz);
     a.fx = fmaf(ng.y, dxb, a.fx); a.fy = fmaf(ng.y, dyb, a.fy); a.fz = fmaf(ng.y, dzb, a.fz);
-    a.pe = __fadd2_rn(a.pe, __ffma2_rn(z3, z3, make_float2(-z3.x, -z3.y)));
-    a.nin = __fadd2_rn(a.nin, m);
+    if (ENERGY) {
+        a.pe = __fadd2_rn(a.pe, __ffma2_rn(z3, z3, make_float2(-z3.x, -z3.y)));
+        a.nin = __fadd2_rn(a.nin, m);
+    }
 }
 
-template <bool IMG, int SH, bool UNIT>
+template <bool IMG, int SH, bool UNIT, bool ENERGY>
 __device__ __forceinline__ void lj_chunk_s(const DevParams& P, unsigned int sp32, float4 xi, uint2 cur, LJAccS& a) {
     const float4 x0 = staged_pos<SH>(sp32, cur.x & 0xffffu), x1 = staged_pos<SH>(sp32, cur.x >> 16);
     const float4 x2 = staged_pos<SH>(sp32, cur.y & 0xffffu), x3 = staged_pos<SH>(sp32, cur.y >> 16);
     if (UNIT) {
-        lj_visit2_unit_s<IMG>(P, xi, x0, x1, a);
-        lj_visit2_unit_s<IMG>(P, xi, x2, x3, a);
+        lj_visit2_unit_s<IMG, ENERGY>(P, xi, x0, x1, a);
+        lj_visit2_unit_s<IMG, ENERGY>(P, xi, x2, x3, a);
     } else {
         lj_visit2_s<IMG>(P, xi, x0, x1, a);
         lj_visit2_s<IMG>(P, xi, x2, x3, a);
@@ -920,7 +1008,7 @@ __device__ __forceinline__ void lj_chunk_s(const DevParams& P, unsigned int sp32
 // NS = threads per particle (1; 2 or 4 when the staged neighbourhood is so large that only one or two 256-particle blocks
 // fit on an SM: the block then runs 512 threads, thread h * 256 + p takes the row chunks c = h mod 2 of particle p and the
 // two partial sums meet in shared memory -- twice the warps for the same shared memory).  xch = exchange buffer (NS == 2).
-template <bool IMG, int SH, bool UNIT, int NS>
+template <bool IMG, int SH, bool UNIT, int NS, bool ENERGY>
 __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int i,
                                                bool live, int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB, uint2 pkC,
                                                uint2 pkD, float* xch, const float4* __restrict__ pos, float4* __restrict__ force,
@@ -936,19 +1024,19 @@ __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuff
     for (int c = 0; c < nch; c += 4) {
         const uint2 curA = pkA;
         if (c + 4 < nch) pkA = ld_row(rowh + (size_t)(c + 4) * cs);
-        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curA, a);
+        lj_chunk_s<IMG, SH, UNIT, ENERGY>(P, sp, xi, curA, a);
         if (c + 1 >= nch) break;
         const uint2 curB = pkB;
         if (c + 5 < nch) pkB = ld_row(rowh + (size_t)(c + 5) * cs);
-        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curB, a);
+        lj_chunk_s<IMG, SH, UNIT, ENERGY>(P, sp, xi, curB, a);
         if (c + 2 >= nch) break;
         const uint2 curC = pkC;
         if (c + 6 < nch) pkC = ld_row(rowh + (size_t)(c + 6) * cs);
-        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curC, a);
+        lj_chunk_s<IMG, SH, UNIT, ENERGY>(P, sp, xi, curC, a);
         if (c + 3 >= nch) break;
         const uint2 curD = pkD;
         if (c + 7 < nch) pkD = ld_row(rowh + (size_t)(c + 7) * cs);
-        lj_chunk_s<IMG, SH, UNIT>(P, sp, xi, curD, a);
+        lj_chunk_s<IMG, SH, UNIT, ENERGY>(P, sp, xi, curD, a);
     }
     float pe2 = a.pe.x + a.pe.y;
     float nin = a.nin.x + a.nin.y;
@@ -1046,7 +1134,7 @@ __device__ __forceinline__ void vertex_rows_unstaged(const DevParams& P, const D
     if (RIGID) torque[i] = make_float4(tx, ty, tz, 0.f);
 }
 
-template <int NS>
+template <int NS, bool ENERGY>
 __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries,
                                                                                   const float4* __restrict__ pos,
                                                                                   float4* __restrict__ force) {
@@ -1076,13 +1164,14 @@ __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k
     const bool bonds = P.kind == MD_POT_FENE_WCA;
     const bool img = (bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK);
     const bool unit = P.sig2 == 1.0f;
-#define LJ_ROWS(IMG_, SH_, UNIT_) vertex_lj_rows<IMG_, SH_, UNIT_, NS>(P, B, bi, st, i, live, cnt, rowb, pkA, pkB, pkC, pkD, xch, pos, force, bonds)
+#define LJ_ROWS(IMG_, SH_, UNIT_, EN_) vertex_lj_rows<IMG_, SH_, UNIT_, NS, EN_>(P, B, bi, st, i, live, cnt, rowb, pkA, pkB, pkC, pkD, xch, pos, force, bonds)
+    // (the energy-free form exists for the reduced-unit loop only: sigma == 1 in every config)
     if (bi.flags & MD_BLK_SH4) {
-        if (unit) { if (img) LJ_ROWS(true, 4, true); else LJ_ROWS(false, 4, true); }
-        else { if (img) LJ_ROWS(true, 4, false); else LJ_ROWS(false, 4, false); }
+        if (unit) { if (img) LJ_ROWS(true, 4, true, ENERGY); else LJ_ROWS(false, 4, true, ENERGY); }
+        else { if (img) LJ_ROWS(true, 4, false, true); else LJ_ROWS(false, 4, false, true); }
     } else {
-        if (unit) { if (img) LJ_ROWS(true, 0, true); else LJ_ROWS(false, 0, true); }
-        else { if (img) LJ_ROWS(true, 0, false); else LJ_ROWS(false, 0, false); }
+        if (unit) { if (img) LJ_ROWS(true, 0, true, ENERGY); else LJ_ROWS(false, 0, true, ENERGY); }
+        else { if (img) LJ_ROWS(true, 0, false, true); else LJ_ROWS(false, 0, false, true); }
     }
 #undef LJ_ROWS
 }
@@ -1169,14 +1258,20 @@ void md_staged_configure(md_system* s) {
     cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     cudaFuncSetAttribute(k_build_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     cudaFuncSetAttribute(k_edges_from_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
-    cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
-    cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
-    cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    cudaFuncSetAttribute(k_vertex_lj_staged<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     // the neighbourhoods live in shared memory and the rows bypass L1: ask for the largest shared-memory carveout so that
     // as many blocks as the sizing in sync_and_check counted on are resident
-    cudaFuncSetAttribute(k_vertex_lj_staged<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    cudaFuncSetAttribute(k_vertex_lj_staged<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    cudaFuncSetAttribute(k_vertex_lj_staged<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<1, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<1, false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<2, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<2, false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<4, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(k_vertex_lj_staged<4, false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_patchy_staged<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_patchy_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     cudaFuncSetAttribute(k_vertex_patchy_staged<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
@@ -1204,7 +1299,7 @@ int md_staged_threads_per_particle(const md_system* s) {
 }
 
 // VERTEX on the staged rows.  Returns false if the neighbourhood does not fit in shared memory.
-bool md_launch_forces_staged(md_system* s) {
+bool md_launch_forces_staged(md_system* s, bool energy) {
     const DevParams& P = s->P;
     const int se = staged_launch_entries(s);
     const size_t smem = md_staged_smem_bytes(s, se);
@@ -1214,10 +1309,13 @@ bool md_launch_forces_staged(md_system* s) {
     else {
         const int ns = staged_lj_ns(s, smem);
         if (ns == 4)        // one block per SM: four threads per particle (1024-thread blocks, 32 warps on the SM)
-            k_vertex_lj_staged<4><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
+            { if (energy) k_vertex_lj_staged<4, true><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
+              else k_vertex_lj_staged<4, false><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force); }
         else if (ns == 2)   // <= 2 blocks per SM: two threads per particle
-            k_vertex_lj_staged<2><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
-        else k_vertex_lj_staged<1><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+            { if (energy) k_vertex_lj_staged<2, true><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
+              else k_vertex_lj_staged<2, false><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force); }
+        else if (energy) k_vertex_lj_staged<1, true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+        else k_vertex_lj_staged<1, false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
     }
     s->launches += 1;
     return true;
