@@ -335,6 +335,67 @@ def roofline_for(strategy, variant, t_us, Ef, E_in, N, rigid, units, probes, wor
     return r
 
 
+def run_dd(args):
+    """--dd: ONE system of the workload's size split into slabs over the ranks (space decomposition, P:37-39, S:8(e) /
+    S:8(f4); paper_1401_4350_b200/dd.py) instead of independent replicas -> "scaling": "strong".  A timed step = kick+drift,
+    halo refresh (NCCL point-to-point), all-reduce of the skin flags, rebuild with migration when it trips, forces, kick."""
+    import torch
+    from paper_1401_4350_b200.dd import DDSimulation, DistTransport, Domain, LocalTransport, SlabPlan
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    w = workload(args.workload)
+    plan = SlabPlan(w.box, world, w.rcut + w.skin)
+    variant = args.scatter or ("smem" if args.strategy == "vertex" else "warp")
+    d = Domain(rank, plan, w.N, w.rcut, w.skin, w.potential, w.max_neigh, device=str(dev), order=args.order,
+               strategy=args.strategy, variant=variant)
+    d.load_initial(w.pos, w.vel, w.quat, w.angmom)
+    sim = DDSimulation([d], DistTransport(plan, dist, dev) if world > 1 else LocalTransport(plan))
+    sim.rebuild()
+    K, Wm = args.steps, max(3, args.warmup)
+    sim.run(w.dt, args.melt_steps + Wm)
+    torch.cuda.synchronize(dev)
+    if dist is not None:
+        dist.barrier()
+    l0, r0 = d.sys.launch_count(), d.n_rebuilds
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    sim.run(w.dt, K)
+    e = sim.energy()
+    b.record()
+    torch.cuda.synchronize(dev)
+    if dist is not None:
+        dist.barrier()
+    ms = a.elapsed_time(b)
+    E_loc = float(d.sys.stats()["n_edges"])                  # pairs of the local list (cross-face pairs are in two lists)
+    n_loc = float(d.sys.N)
+    if dist is not None:
+        tt = torch.tensor([ms], dtype=torch.float64, device=dev); dist.all_reduce(tt, op=dist.ReduceOp.MAX); ms = float(tt.item())
+        ee = torch.tensor(list(e) + [E_loc, n_loc], dtype=torch.float64, device=dev); dist.all_reduce(ee); e = ee[:3].tolist(); E_loc = float(ee[3]); n_loc = float(ee[4])
+    if rank == 0:
+        # credit the global system's pairs once: E_global ~ pairs of all local lists x N / (owned + ghosts)
+        E = E_loc * w.N / n_loc
+        print(json.dumps({"metric": metric_text(args.workload), "value": E * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+                          "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                          "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": f"{args.workload}: {WORKLOAD_TEXT[args.workload]}, relaxed by {args.melt_steps} untimed steps",
+                                     "N": w.N, "E": int(E), "strategy": args.strategy, "variant": variant, "order": args.order,
+                                     "parallelism": f"slab space decomposition over {world} rank(s), halo r_v, ghosts {n_loc / w.N - 1.0:.3f} x N",
+                                     "rebuilds_in_timed_region": d.n_rebuilds - r0},
+                          "gpu_launches": int(d.sys.launch_count() - l0), "energy_total": sum(e), "e2e": None, "roofline": None,
+                          "cpu_baseline": None}))
+    sim.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -351,12 +412,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--c5-max-log2n", type=int, default=20, help="C5: largest N of the sweep (configs[4] goes to 22)")
+    ap.add_argument("--dd", action="store_true", help="slab space decomposition of ONE system over the ranks instead of replicas")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.workload == "C5":
         import crossover
         return crossover.bench_mode(args)
+    if args.dd:
+        return run_dd(args)
 
     import torch
     if not torch.cuda.is_available():

@@ -272,6 +272,53 @@ md_status md_step_host(md_system*, void* pos_host, void* vel_host, void* force_h
                        void* angmom_host, void* torque_host, double dt, int64_t nsteps, int32_t strategy,
                        int32_t scatter);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * Space decomposition ("space-decomposition: the domain ... partitioned into smaller subsets"; S:8(e), S:8(f4)).
+ * One handle per rank holds the particles the rank OWNS (original ids 0 .. n_active-1) followed by GHOST copies of the
+ * neighbouring ranks' particles within the halo width of its sub-domain (ids n_active .. N-1), all in GLOBAL coordinates
+ * and the GLOBAL periodic box, so cells, Verlet lists and both force strategies run unchanged; every pair that involves
+ * an owned particle is evaluated by the owner's rank (pairs across a face by both ranks: redundant arithmetic instead of
+ * a reverse force exchange), forces on ghosts are discarded.  Protocol of one step (paper_1401_4350_b200/dd.py):
+ *   md_half_step(KICK_DRIFT) -> halo refresh: md_gather_ids(send list) / send / recv / md_scatter_ids(ghost ids)
+ *   -> md_rebuild_flag on every rank, all-reduce(max) -> [migration + new halo + md_resize + md_bind_state + builds]
+ *   -> md_forces -> md_half_step(KICK).
+ * ------------------------------------------------------------------------------------------------------------------- */
+typedef enum { MD_ARRAY_POS = 0, MD_ARRAY_VEL = 1, MD_ARRAY_FORCE = 2, MD_ARRAY_QUAT = 3, MD_ARRAY_ANGMOM = 4, MD_ARRAY_TORQUE = 5 } md_array;
+typedef enum { MD_STEP_KICK_DRIFT = 0, MD_STEP_KICK = 1 } md_step_part;
+
+/* Change the particle count of the handle to n_new in [1, N at creation] (the workspace was carved for the creation N;
+ * cells and capacities keep the creation geometry).  Unbinds the state: md_bind_state arrays of the new length next.
+ * Resets n_active to n_new. */
+md_status md_resize(md_system*, int64_t n_new);
+
+/* Particles with ORIGINAL id >= n_active are ghosts: md_integrate / md_half_step neither kick nor drift them (the halo
+ * refresh moves them), md_energy leaves them out; forces and lists treat them like any particle.  Default: N (none).
+ * fp32 precision only (MD_ERR_STATE in MD_PREC_MIXED). */
+md_status md_set_active(md_system*, int64_t n_active);
+
+/* One half of a velocity-Verlet step (S:O6 / S:O7) on the owned particles, asynchronous:
+ *   MD_STEP_KICK_DRIFT  v += dt/2 F/m, x += dt v (rigid bodies: L, q likewise) and the skin check of S:Q4 on ALL particles,
+ *                       which latches the device-side rebuild flag; the forces are stale afterwards (call md_forces)
+ *   MD_STEP_KICK        v += dt/2 F/m with the forces of the new positions.
+ * MD_ERR_STATE without valid forces. */
+md_status md_half_step(md_system*, double dt, int32_t part);
+
+/* *flag (host) = 1 if the skin criterion has tripped since the last list build.  Synchronises. */
+md_status md_rebuild_flag(md_system*, int32_t* flag);
+
+/* dst_dev[k] = array[particle with original id ids_dev[k]] (ids_dev == NULL: id first_id + k), k < n; float4 each, DEVICE
+ * pointers; array = md_array.  Asynchronous.  md_scatter_ids is the inverse for the id range [first_id, first_id + n):
+ * array[particle first_id + k] = src_dev[k] (writing positions or quaternions invalidates the forces). */
+md_status md_gather_ids(md_system*, int32_t array, const int32_t* ids_dev, int64_t first_id, int64_t n, void* dst_dev);
+md_status md_scatter_ids(md_system*, int32_t array, int64_t first_id, int64_t n, const void* src_dev);
+
+/* Stable compaction (ascending index) of { i < n : lo <= pos_dev[i][axis] < hi } into idx_out_dev[capacity] (may be NULL to
+ * count only); *count_host receives the count (even if > capacity).  pos_dev: DEVICE float4[n]; the bounds are compared
+ * in fp32.  scratch_dev: DEVICE, >= 4 * (n / 1024 + 3) bytes, 4-byte aligned.  Independent of any handle.  Synchronises
+ * cuda_stream. */
+md_status md_dd_select(const void* pos_dev, int64_t n, int32_t axis, double lo, double hi, int32_t* idx_out_dev, int64_t capacity,
+                       int64_t* count_host, void* scratch_dev, size_t scratch_bytes, void* cuda_stream);
+
 /* Number of kernels this library has launched on behalf of the handle (for bench.py's gpu_launches). */
 int64_t md_launch_count(const md_system*);
 

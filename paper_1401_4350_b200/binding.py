@@ -15,6 +15,8 @@ SCATTER = {"red": 0, "red_v4": 1, "warp": 2, "segmented": 3, "cluster": 4}
 GATHER = {"auto": 0, "l2": 1, "smem": 2}
 ORDER = {"none": 0, "cell": 1, "hilbert": 2}
 PRECISION = {"f32": 0, "mixed": 1}
+ARRAY = {"pos": 0, "vel": 1, "force": 2, "quat": 3, "angmom": 4, "torque": 5}
+STEP_PART = {"kick_drift": 0, "kick": 1}
 OPTION = {"stage_limit": 0, "no_graph": 1, "debug": 2, "row_schedule": 3}
 PROBE = {"ffma": 0, "ffma2": 1, "mufu": 2, "red_v4_scatter": 3, "red_f32_scatter": 4, "red_v4_coalesced": 5,
          "red_f32_coalesced": 6}
@@ -26,7 +28,8 @@ STATUS = {0: "MD_OK", -1: "MD_ERR_INVALID", -2: "MD_ERR_STATE", -3: "MD_ERR_CAPA
 EXPORTED_SYMBOLS = ["md_workspace_bytes", "md_create", "md_bind_state", "md_set_order", "md_set_precision",
                     "md_get_state_double", "md_set_thermostat", "md_thermostat", "md_build_cells",
                     "md_build_verlet", "md_forces", "md_integrate", "md_energy", "md_stats", "md_stats_ex",
-                    "md_set_option", "md_probe", "md_get_pairs", "md_get_ids", "md_step_host", "md_launch_count",
+                    "md_set_option", "md_probe", "md_resize", "md_set_active", "md_half_step", "md_rebuild_flag",
+                    "md_gather_ids", "md_scatter_ids", "md_dd_select", "md_get_pairs", "md_get_ids", "md_step_host", "md_launch_count",
                     "md_last_error", "md_destroy"]
 
 
@@ -140,6 +143,21 @@ def load_library() -> C.CDLL:
     L.md_set_option.argtypes = [vp, C.c_int32, C.c_int64]
     L.md_probe.restype = C.c_int
     L.md_probe.argtypes = [vp, C.c_int32, dp3]
+    L.md_resize.restype = C.c_int
+    L.md_resize.argtypes = [vp, C.c_int64]
+    L.md_set_active.restype = C.c_int
+    L.md_set_active.argtypes = [vp, C.c_int64]
+    L.md_half_step.restype = C.c_int
+    L.md_half_step.argtypes = [vp, C.c_double, C.c_int32]
+    L.md_rebuild_flag.restype = C.c_int
+    L.md_rebuild_flag.argtypes = [vp, C.POINTER(C.c_int32)]
+    L.md_gather_ids.restype = C.c_int
+    L.md_gather_ids.argtypes = [vp, C.c_int32, vp, C.c_int64, C.c_int64, vp]
+    L.md_scatter_ids.restype = C.c_int
+    L.md_scatter_ids.argtypes = [vp, C.c_int32, C.c_int64, C.c_int64, vp]
+    L.md_dd_select.restype = C.c_int
+    L.md_dd_select.argtypes = [vp, C.c_int64, C.c_int32, C.c_double, C.c_double, vp, C.c_int64, C.POINTER(C.c_int64), vp,
+                               C.c_size_t, vp]
     L.md_get_pairs.restype = C.c_int
     L.md_get_pairs.argtypes = [vp, C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int64)]
     L.md_get_ids.restype = C.c_int
@@ -202,19 +220,28 @@ class MDSystem:
         if rc != 0:
             raise MDError(rc, "md_create failed (invalid geometry / parameters)")
         self.h = h
+        self.N_capacity = self.N
         z = lambda: torch.zeros((self.N, 4), dtype=torch.float32, device=self.device)
-        self.pos, self.vel, self.force = z(), z(), z()
-        self.quat = self.angmom = self.torque = None
+        self._full = {"pos": z(), "vel": z(), "force": z()}
         if self.rigid:
-            self.quat, self.angmom, self.torque = z(), z(), z()
-            self.quat[:, 0] = 1.0
-        self._check(self.lib.md_bind_state(self.h, *[C.c_void_p(t.data_ptr()) if t is not None else None for t in
-                                                    (self.pos, self.vel, self.force, self.quat, self.angmom,
-                                                     self.torque)]))
+            self._full.update({"quat": z(), "angmom": z(), "torque": z()})
+            self._full["quat"][:, 0] = 1.0
+        self._views_and_bind()
         if order != "none":
             self.set_order(order)
 
     # ---- plumbing ----
+    def _views_and_bind(self):
+        """State tensors = the first N rows of the capacity tensors (md_resize keeps the base pointers)."""
+        f = self._full
+        self.pos, self.vel, self.force = f["pos"][:self.N], f["vel"][:self.N], f["force"][:self.N]
+        self.quat = self.angmom = self.torque = None
+        if self.rigid:
+            self.quat, self.angmom, self.torque = f["quat"][:self.N], f["angmom"][:self.N], f["torque"][:self.N]
+        self._check(self.lib.md_bind_state(self.h, *[C.c_void_p(x.data_ptr()) if x is not None else None for x in
+                                                    (self.pos, self.vel, self.force, self.quat, self.angmom,
+                                                     self.torque)]))
+
     def _check(self, rc: int):
         if rc != 0:
             raise MDError(rc, self.lib.md_last_error(self.h).decode())
@@ -312,6 +339,39 @@ class MDSystem:
         self._check(self.lib.md_probe(self.h, PROBE[kind] if isinstance(kind, str) else int(kind), C.byref(v)))
         return v.value
 
+    # ---- space decomposition support (md_b200.h "Space decomposition"; paper_1401_4350_b200/dd.py drives it) ----
+    def resize(self, n: int):
+        """md_resize + rebind: the state tensors become the first n rows of the capacity tensors (contents kept)."""
+        self._check(self.lib.md_resize(self.h, int(n)))
+        self.N = int(n)
+        self._views_and_bind()
+
+    def set_active(self, n_active: int):
+        self._check(self.lib.md_set_active(self.h, int(n_active)))
+
+    def half_step(self, dt, part):
+        self._check(self.lib.md_half_step(self.h, float(dt), STEP_PART[part] if isinstance(part, str) else int(part)))
+
+    def rebuild_flag(self) -> int:
+        f = C.c_int32(0)
+        self._check(self.lib.md_rebuild_flag(self.h, C.byref(f)))
+        return int(f.value)
+
+    def gather_ids(self, array, ids=None, first_id=0, n=None):
+        """float32 [n,4] device tensor: array rows of the particles with ORIGINAL ids `ids` (int32 device tensor) or
+        first_id .. first_id + n - 1."""
+        t = self.torch
+        n = int(ids.shape[0]) if ids is not None else int(n)
+        out = t.empty((n, 4), dtype=t.float32, device=self.device)
+        self._check(self.lib.md_gather_ids(self.h, ARRAY[array], C.c_void_p(ids.data_ptr()) if ids is not None and n > 0 else None,
+                                           int(first_id), n, C.c_void_p(out.data_ptr()) if n > 0 else None))
+        return out
+
+    def scatter_ids(self, array, first_id, src):
+        n = int(src.shape[0])
+        src = src.contiguous()
+        self._check(self.lib.md_scatter_ids(self.h, ARRAY[array], int(first_id), n, C.c_void_p(src.data_ptr()) if n > 0 else None))
+
     def get_pairs(self) -> np.ndarray:
         """Half list as ORIGINAL-id pairs (lo, hi), int32 [E,2], unsorted."""
         n = C.c_int64(0)
@@ -343,3 +403,21 @@ class MDSystem:
         out = np.empty_like(a)
         out[ids] = a
         return out
+
+
+def dd_select(pos, lo: float, hi: float, axis: int = 0, stream=None):
+    """md_dd_select: int32 device tensor of the indices i (ascending) with lo <= pos[i, axis] < hi (fp32 comparisons).
+    pos: float32 [n,4] CUDA tensor."""
+    import torch
+    lib = load_library()
+    n = int(pos.shape[0])
+    pos = pos.contiguous()
+    st = stream if stream is not None else torch.cuda.current_stream(pos.device)
+    scratch = torch.empty(n // 1024 + 4, dtype=torch.int32, device=pos.device)
+    out = torch.empty(max(n, 1), dtype=torch.int32, device=pos.device)
+    cnt = C.c_int64(0)
+    rc = lib.md_dd_select(C.c_void_p(pos.data_ptr()), n, int(axis), float(lo), float(hi), C.c_void_p(out.data_ptr()), n,
+                          C.byref(cnt), C.c_void_p(scratch.data_ptr()), scratch.numel() * 4, C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise MDError(rc, "md_dd_select failed")
+    return out[:int(cnt.value)]

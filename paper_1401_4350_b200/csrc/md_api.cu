@@ -278,6 +278,8 @@ md_status sync_and_check(md_system* s, const char* where) {
 
 }  // namespace
 
+void md_drop_graphs(md_system* s) { drop_step_graph(s); }
+
 extern "C" {
 
 md_status md_workspace_bytes(int64_t N, const double box[3], double rcut, double skin, const md_potential* pot,
@@ -301,6 +303,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     md_system* s = (md_system*)calloc(1, sizeof(md_system));
     if (!s) return MD_ERR_INVALID;
     s->N = N;
+    s->N_capacity = N;
     s->stream = (cudaStream_t)cuda_stream;
     s->rcut = rcut; s->skin = skin;
     s->pot = *pot;
@@ -312,7 +315,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     carve((char*)workspace, N, g, rigid, &s->B);
 
     DevParams& P = s->P;
-    P.N = (int)N; P.ntiles = g.ntiles; P.cap = g.cap; P.capg = g.cap / 4;
+    P.N = (int)N; P.n_active = (int)N; P.ntiles = g.ntiles; P.cap = g.cap; P.capg = g.cap / 4;
     P.dLx = box[0]; P.dLy = box[1]; P.dLz = box[2];
     P.Lx = (float)box[0]; P.Ly = (float)box[1]; P.Lz = (float)box[2];
     P.hLx = 0.5f * P.Lx; P.hLy = 0.5f * P.Ly; P.hLz = 0.5f * P.Lz;
@@ -452,6 +455,7 @@ md_status md_set_precision(md_system* s, int32_t precision) {
     if (!s) return MD_ERR_INVALID;
     if (s->sticky) return (md_status)s->sticky;
     if (precision != MD_PREC_F32 && precision != MD_PREC_MIXED) return fail(s, MD_ERR_INVALID, "md_set_precision: unknown precision");
+    if (precision == MD_PREC_MIXED && s->P.n_active < s->P.N) return fail(s, MD_ERR_STATE, "md_set_precision: ghosts (md_set_active) need MD_PREC_F32");
     if (precision != s->precision) {
         s->precision = precision;
         s->shadow_valid = false;
@@ -861,6 +865,16 @@ md_status md_probe(md_system* s, int32_t kind, double* value) {
     }
     s->launches += 4;
     return check_cuda(s, "md_probe");
+}
+
+md_status md_rebuild_flag(md_system* s, int32_t* flag) {
+    if (!s || !flag) return MD_ERR_INVALID;
+    if (s->sticky) return (md_status)s->sticky;
+    DevCtrl c;
+    cudaMemcpyAsync(&c, s->B.ctrl, sizeof(c), cudaMemcpyDeviceToHost, s->stream);
+    md_status st = sync_and_check(s, "md_rebuild_flag");
+    *flag = c.rebuild != 0 ? 1 : 0;
+    return st;
 }
 
 md_status md_get_ids(md_system* s, int32_t* ids_host) {

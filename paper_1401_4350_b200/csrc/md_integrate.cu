@@ -15,14 +15,17 @@ __global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, f
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < P.N) {
-        const float hk = 0.5f * dt * P.inv_mass;
+        // ghosts of a space decomposition (md_set_active) are moved by the halo refresh only; their skin check still runs
+        const bool ghost = P.n_active < P.N && B.ids[i] >= P.n_active;
+        const float hk = ghost ? 0.0f : 0.5f * dt * P.inv_mass;
+        if (ghost) dt = 0.0f;
         float4 v = vel[i], f = force[i], x = pos[i];
         if (PRE) { v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z); }
         v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z);
         x.x = fmaf(dt, v.x, x.x); x.y = fmaf(dt, v.y, x.y); x.z = fmaf(dt, v.z, x.z);
         vel[i] = v;
         pos[i] = x;
-        if (RIGID) {
+        if (RIGID && !ghost) {
             float4 L = angmom[i], t = torque[i], q = quat[i];
             const float hd = 0.5f * dt;
             if (PRE) { L.x = fmaf(hd, t.x, L.x); L.y = fmaf(hd, t.y, L.y); L.z = fmaf(hd, t.z, L.z); }
@@ -53,10 +56,11 @@ __global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, f
 
 // second half: v += dt/2 F/m ; L += dt/2 tau
 template <bool RIGID>
-__global__ void __launch_bounds__(256) k_kick(DevParams P, float dt, float4* __restrict__ vel, const float4* __restrict__ force,
+__global__ void __launch_bounds__(256) k_kick(DevParams P, DevBuffers B, float dt, float4* __restrict__ vel, const float4* __restrict__ force,
                                               float4* __restrict__ angmom, const float4* __restrict__ torque) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.N) return;
+    if (P.n_active < P.N && B.ids[i] >= P.n_active) return;   // ghost (md_set_active)
     const float hk = 0.5f * dt * P.inv_mass;
     float4 v = vel[i], f = force[i];
     v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z);
@@ -223,8 +227,8 @@ void md_launch_kick(md_system* s, float dt) {
         s->launches += 1;
         return;
     }
-    if (s->rigid) k_kick<true><<<nb, 256, 0, s->stream>>>(s->P, dt, s->vel, s->force, s->angmom, s->torque);
-    else k_kick<false><<<nb, 256, 0, s->stream>>>(s->P, dt, s->vel, s->force, nullptr, nullptr);
+    if (s->rigid) k_kick<true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->vel, s->force, s->angmom, s->torque);
+    else k_kick<false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->vel, s->force, nullptr, nullptr);
     s->launches += 1;
 }
 
@@ -356,6 +360,7 @@ __global__ void __launch_bounds__(E_THREADS) k_energy_partial(DevParams P, DevBu
     __shared__ double sh[32];
     double u = 0.0, kt = 0.0, kr = 0.0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += gridDim.x * blockDim.x) {
+        if (P.n_active < P.N && B.ids[i] >= P.n_active) continue;   // ghosts belong to another rank's sums (md_set_active)
         u += (double)force[i].w;
         float4 v = vel[i];
         kt += (double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z;

@@ -58,6 +58,7 @@ struct BlkInfo {
 // Parameter block passed by value to every kernel.
 struct DevParams {
     int N, ntiles, cap, capg;          // capg = cap/4 (int4 groups per list row)
+    int n_active;                      // original ids >= n_active are ghosts of a space decomposition: not integrated, not in the energy (md_set_active)
     float Lx, Ly, Lz, hLx, hLy, hLz;   // box and half box (fp32, exactly the fp32 box of the fixtures)
     double dLx, dLy, dLz;              // same values in double (S:Q7)
     double rv2d, rc2d;                 // (rcut+skin)^2 and rcut^2 formed in double (S:O0, S:Q5)
@@ -142,6 +143,7 @@ struct md_system {
     DevBuffers B;
     cudaStream_t stream;
     int64_t N;
+    int64_t N_capacity;      // N at creation: md_resize may not exceed it (the workspace was carved for it)
     size_t ecap;
     size_t ucap;             // capacity of cl_units
     double rcut, skin;
@@ -200,6 +202,7 @@ void md_launch_count_in_cutoff(md_system* s);                             // ctr
 void md_staged_configure(md_system* s);                                   // per-device kernel attributes of md_staged.cu
 int md_staged_threads_per_particle(const md_system* s);                   // NS the staged LJ launch would use (0: rigid)
 bool md_run_probe(md_system* s, int kind, double* value);                 // md_probe.cu
+void md_drop_graphs(md_system* s);                                        // the captured step graphs (md_api.cu)
 // cluster list (md_cluster.cu)
 void md_cluster_configure(md_system* s);
 bool md_launch_build_cluster(md_system* s, bool gated, const float4* pos_src);
