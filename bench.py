@@ -412,6 +412,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--c5-max-log2n", type=int, default=20, help="C5: largest N of the sweep (configs[4] goes to 22)")
+    ap.add_argument("--no-graph", action="store_true",
+                    help="md_set_option(MD_OPT_NO_GRAPH): plain kernel launches instead of CUDA graphs, so that ncu lists every kernel")
     ap.add_argument("--dd", action="store_true", help="slab space decomposition of ONE system over the ranks instead of replicas")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -444,6 +446,8 @@ def main():
     N = w.N
     rigid = w.quat is not None
     s = MDSystem.from_workload(w, device=str(dev), order=args.order)
+    if args.no_graph:
+        s.set_option("no_graph", 1)
     vgather = "smem" if args.order != "none" else "l2"
     s.build_cells(); s.build_verlet(); s.forces("vertex", vgather)
     if args.melt_steps > 0:                       # untimed setup: melt the lattice (paper: thermalised states)
@@ -479,6 +483,7 @@ def main():
     E_in, units = sx["n_in_cutoff"], sx["n_cluster_units"]
     probes = {"ffma_tflops": s.probe("ffma"), "ffma2_tflops": s.probe("ffma2"), "mufu_tops": s.probe("mufu"),
               "red_v4_scatter_gops": s.probe("red_v4_scatter"), "red_v4_coalesced_gops": s.probe("red_v4_coalesced"),
+              "red_f32_scatter_gops": s.probe("red_f32_scatter"), "red_f32_coalesced_gops": s.probe("red_f32_coalesced"),
               "nominal_tflops": fp32_nominal_tflops()}
     if args.scatter is None:
         args.scatter = (vgather if args.strategy == "vertex" else best_edge[len("edge_"):])

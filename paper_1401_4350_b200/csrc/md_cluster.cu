@@ -51,10 +51,10 @@ __global__ void __launch_bounds__(32 * CLB_WARPS) k_build_cluster(DevParams P, D
     GATE(B, gated);
     extern __shared__ __align__(16) unsigned char smraw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const size_t per_warp = 16 * (size_t)MD_CLUSTER + 4 * (size_t)(CL_CELLCAP + MD_CLUSTER + 40) + 8 * (size_t)ucap_w;
+    const size_t per_warp = 32 * (size_t)MD_CLUSTER + 4 * (size_t)(CL_CELLCAP + MD_CLUSTER + 40) + 8 * (size_t)ucap_w;
     unsigned char* base = smraw + (size_t)w * ((per_warp + 15) / 16 * 16);
     float4* pi = reinterpret_cast<float4*>(base);                       // [16] owner positions
-    int* cells = reinterpret_cast<int*>(pi + MD_CLUSTER);               // [CL_CELLCAP] distinct candidate cells (ranks)
+    int* cells = reinterpret_cast<int*>(pi + 2 * MD_CLUSTER);           // [CL_CELLCAP] distinct candidate cells (ranks); pi[16..31] = raw owner positions
     int* own = cells + CL_CELLCAP;                                      // [16] distinct own cells
     int* hist = own + MD_CLUSTER;                                       // [17] popcount histogram, [17..33] cursors
     uint2* ubuf = reinterpret_cast<uint2*>(hist + 40);                  // [ucap_w] units in scan order
@@ -106,6 +106,43 @@ __global__ void __launch_bounds__(32 * CLB_WARPS) k_build_cluster(DevParams P, D
         L += __popc(kb);
         __syncwarp();
     }
+    // 3b. Can plain differences stand in for the minimum image?  Per axis: yes if the owners (+ r_v) stay clear of the
+    //     periodic face (mode 0), or, with the upper half of the box shifted down by L (exact in fp32: Sterbenz), clear of
+    //     the seam at +-L/2 (mode 1); else the cluster takes the robust minimum image for every pair (small boxes, storage
+    //     order NONE).  Shifted coordinates give bit-identical differences to min_image() for every pair within r_v.
+    float4 xo = lane < MD_CLUSTER ? pi[lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const bool live_o = lane < nown;
+    int mode[3];
+    {
+        const float Ls[3] = { P.Lx, P.Ly, P.Lz };
+        const float xs[3] = { xo.x, xo.y, xo.z };
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const float L = Ls[a], hL = 0.5f * L, rv = P.shift_margin;           // r_v + skin: a safe margin
+            const float v = xs[a], tv = v > hL ? v - L : v;
+            float lo = live_o ? v : 3.0e38f, hi = live_o ? v : -3.0e38f, tlo = live_o ? tv : 3.0e38f, thi = live_o ? tv : -3.0e38f;
+            for (int o = 16; o > 0; o >>= 1) {
+                lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, o)); hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+                tlo = fminf(tlo, __shfl_xor_sync(0xffffffffu, tlo, o)); thi = fmaxf(thi, __shfl_xor_sync(0xffffffffu, thi, o));
+            }
+            mode[a] = (lo - rv >= 0.0f && hi + rv < L) ? 0 : ((tlo - rv > -hL && thi + rv < hL) ? 1 : 2);
+        }
+    }
+    const bool fast = mode[0] < 2 && mode[1] < 2 && mode[2] < 2;
+    const float sLx = mode[0] == 1 ? P.Lx : 0.0f, sLy = mode[1] == 1 ? P.Ly : 0.0f, sLz = mode[2] == 1 ? P.Lz : 0.0f;
+    float4* pr = pi + MD_CLUSTER;                                         // raw owner positions (fp64 band decisions)
+    if (lane < MD_CLUSTER) {
+        pr[lane] = xo;
+        if (fast) {
+            int fl = 0;
+            if (xo.x > P.hLx && mode[0] == 1) { xo.x -= sLx; fl |= 1; }
+            if (xo.y > P.hLy && mode[1] == 1) { xo.y -= sLy; fl |= 2; }
+            if (xo.z > P.hLz && mode[2] == 1) { xo.z -= sLz; fl |= 4; }
+            xo.w = __int_as_float(fl);
+            pi[lane] = xo;
+        }
+    }
+    __syncwarp();
     // 4. candidates -> units
     int nunits = 0;
     unsigned long long npairs = 0ull;
@@ -113,25 +150,47 @@ __global__ void __launch_bounds__(32 * CLB_WARPS) k_build_cluster(DevParams P, D
     for (int ci = 0; ci < L; ++ci) {
         const int r = cells[ci];
         const int s0 = B.cell_start[r], n = B.cell_start[r + 1] - s0;
+        if (IDENT && s0 + n <= i0 + 1) continue;                         // half list: only j above the lowest owner can pair
         for (int t0 = 0; t0 < n; t0 += 32) {
             const int t = t0 + lane;
             unsigned int mask = 0u, img = 0u;
             int j = 0;
             if (t < n) {
                 j = IDENT ? s0 + t : B.items[s0 + t];
-                const float4 xj = pos[j];
+                const float4 xr = pos[j];
+                if (fast) {
+                    float4 xj = xr;
+                    int fj = 0;
+                    if (xj.x > P.hLx && mode[0] == 1) { xj.x -= sLx; fj |= 1; }
+                    if (xj.y > P.hLy && mode[1] == 1) { xj.y -= sLy; fj |= 2; }
+                    if (xj.z > P.hLz && mode[2] == 1) { xj.z -= sLz; fj |= 4; }
 #pragma unroll 4
-                for (int k = 0; k < MD_CLUSTER; ++k) {
-                    const float4 xi = pi[k];
-                    const float dx = min_image(xj.x, xi.x, P.Lx, P.hLx), dy = min_image(xj.y, xi.y, P.Ly, P.hLy),
-                                dz = min_image(xj.z, xi.z, P.Lz, P.hLz);
-                    const float tt = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) - P.rv2;
-                    bool in = tt < 0.0f;
-                    if (fabsf(tt) < P.band_rv) in = inside_fp64(xi, xj, P.dLx, P.dLy, P.dLz, P.rv2d);
-                    in = in && j > i0 + k && k < nown;                  // half list: slot of the owner < slot of j
-                    if (in) {
-                        mask |= 1u << k;
-                        img |= (fabsf(xj.x - xi.x) > P.hLx) | (fabsf(xj.y - xi.y) > P.hLy) | (fabsf(xj.z - xi.z) > P.hLz);
+                    for (int k = 0; k < MD_CLUSTER; ++k) {
+                        const float4 xi = pi[k];
+                        const float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
+                        const float tt = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) - P.rv2;
+                        bool in = tt < 0.0f;
+                        if (fabsf(tt) < P.band_rv) in = inside_fp64(pr[k], xr, P.dLx, P.dLy, P.dLz, P.rv2d);
+                        in = in && j > i0 + k && k < nown;              // half list: slot of the owner < slot of j
+                        if (in) {
+                            mask |= 1u << k;
+                            img |= (fj != __float_as_int(xi.w)) ? 1u : 0u;   // exactly one member was shifted on some axis: the pair crosses a face
+                        }
+                    }
+                } else {
+#pragma unroll 4
+                    for (int k = 0; k < MD_CLUSTER; ++k) {
+                        const float4 xi = pr[k];
+                        const float dx = min_image(xr.x, xi.x, P.Lx, P.hLx), dy = min_image(xr.y, xi.y, P.Ly, P.hLy),
+                                    dz = min_image(xr.z, xi.z, P.Lz, P.hLz);
+                        const float tt = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) - P.rv2;
+                        bool in = tt < 0.0f;
+                        if (fabsf(tt) < P.band_rv) in = inside_fp64(xi, xr, P.dLx, P.dLy, P.dLz, P.rv2d);
+                        in = in && j > i0 + k && k < nown;
+                        if (in) {
+                            mask |= 1u << k;
+                            img |= (fabsf(xr.x - xi.x) > P.hLx) | (fabsf(xr.y - xi.y) > P.hLy) | (fabsf(xr.z - xi.z) > P.hLz);
+                        }
                     }
                 }
             }
@@ -356,7 +415,7 @@ __global__ void __launch_bounds__(32 * CLF_WARPS) k_edge_cluster(DevParams P, De
 static int cluster_ucap_w(const md_system* s) { return (8 * s->P.cap + 31) / 32 * 32; }   // units one cluster may hold
 
 static size_t cluster_build_smem(const md_system* s) {
-    const size_t per_warp = 16 * (size_t)MD_CLUSTER + 4 * (size_t)(CL_CELLCAP + MD_CLUSTER + 40) + 8 * (size_t)cluster_ucap_w(s);
+    const size_t per_warp = 32 * (size_t)MD_CLUSTER + 4 * (size_t)(CL_CELLCAP + MD_CLUSTER + 40) + 8 * (size_t)cluster_ucap_w(s);
     return CLB_WARPS * ((per_warp + 15) / 16 * 16);
 }
 

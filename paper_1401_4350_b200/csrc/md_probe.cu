@@ -71,10 +71,11 @@ static bool probe_time(cudaStream_t st, F launch, float* ms) {
 
 // value: TFLOP/s (FFMA, FFMA2), Tops/s (MUFU), G lane-operations/s (the reductions).  false on a CUDA error.
 bool md_run_probe(md_system* s, int kind, double* value) {
-    const int nb = s->sm_count * 8;
-    float* out = reinterpret_cast<float*>(s->B.tmp4);                 // nb * 256 floats <= one plane for N >= 2^12 ... checked below
+    int nb = s->sm_count * 8;
+    float* out = reinterpret_cast<float*>(s->B.tmp4);                 // nb * 256 floats of the permutation scratch
     const size_t plane_bytes = 16 * (size_t)s->P.ntiles * MD_TILE * 7;
-    if ((size_t)nb * 256 * 4 > plane_bytes) return false;
+    if ((size_t)nb * 256 * 4 > plane_bytes) nb = (int)(plane_bytes / 1024);   // a small system: fewer blocks (the rates then read low)
+    if (nb < 1) return false;
     float ms = 0.f;
     const double winstr = (double)nb * 8 * PROBE_NIT * PROBE_CHAINS;   // warp instructions of the measured kind
     cudaStream_t st = s->stream;
