@@ -392,7 +392,7 @@ def test_mixed_precision_rigid_bodies_after_rebuilds(MD, oracle):
     pos, quat = s.in_id_order(s.pos), s.in_id_order(s.quat)
     assert np.abs(np.linalg.norm(quat.astype(np.float64), axis=1) - 1.0).max() < 1e-6
     o = oracle.forces(pos, w.box, dict(w.potential), quat=quat)
-    assert_forces(s, o, True)
+    assert_forces(s, o, True, ("patchy4096 mixed precision after 300 steps", "vertex_smem"))
     s.close()
 
 
@@ -437,7 +437,7 @@ def test_patchy_pp_short_trajectory(MD, oracle):
         s.integrate(w.dt, 100, strat, sc)
         pos, quat = s.in_id_order(s.pos), s.in_id_order(s.quat)
         snap = oracle.forces(pos, w.box, dict(w.potential), quat=quat)
-        assert_forces(s, snap, True)
+        assert_forces(s, snap, True, ("patchy_pp dimers after 100 steps", f"{strat}_{sc}"))
         dx = pos[:, :3].astype(np.float64) - o["pos"][:, :3]
         dx -= w.box * np.round(dx / w.box)
         assert np.abs(dx).max() < 1e-4
@@ -458,11 +458,11 @@ def test_blocks_over_the_launch_capacity_take_the_unstaged_path(MD, oracle, case
     s.set_option("stage_limit", 64)
     s.build_cells(); s.build_verlet(); s.forces("vertex", "smem")
     o = oracle.forces(w.pos, w.box, dict(w.potential), quat=w.quat)
-    assert_forces(s, o, w.quat is not None)
+    assert_forces(s, o, w.quat is not None, (f"{case} unstaged path", "vertex_smem"))
     s.integrate(w.dt, 20, "vertex", "smem")
     pos = s.in_id_order(s.pos)
     quat = s.in_id_order(s.quat) if w.quat is not None else None
-    assert_forces(s, oracle.forces(pos, w.box, dict(w.potential), quat=quat), quat is not None)
+    assert_forces(s, oracle.forces(pos, w.box, dict(w.potential), quat=quat), quat is not None, (f"{case} unstaged path after 20 steps", "vertex_smem"))
     s.close()
 
 
