@@ -163,7 +163,10 @@ __device__ __forceinline__ void scan_cell_bucket(const float4* __restrict__ cell
 template <bool SHIFT, bool SELF>
 __device__ __forceinline__ void scan_cell_fast(const float4* __restrict__ cellpos, int n, int t0, int me, float4 xi, float rv2,
                                                float hLx, float hLy, float hLz, float tLx, float tLy, float tLz,
-                                               unsigned short* tmp_blk, unsigned int& off, unsigned int offmax, float& bandmin) {
+                                               unsigned short* tmp_blk, unsigned int& off, unsigned int offmax, float& bandmin,
+                                               float near_gap) {
+    // near_gap = r_v^2 - r_c^2 for the rigid bodies (else a negative number: never near): bit 15 of the stored index marks a
+    // neighbour inside the CUTOFF at build time, so that the row can start with the pairs that will be evaluated
 #pragma unroll 8
     for (int k = 0; k < n; ++k) {
         float4 xj = __ldg(cellpos + k);
@@ -177,7 +180,8 @@ __device__ __forceinline__ void scan_cell_fast(const float4* __restrict__ cellpo
         bandmin = fminf(bandmin, fabsf(tt));
         int m = __float_as_int(tt) >> 31;                  // -1 inside r_v, 0 outside
         if (SELF) m = (t0 + k == me) ? 0 : m;
-        if (m) *reinterpret_cast<unsigned short*>(reinterpret_cast<char*>(tmp_blk) + off) = (unsigned short)(t0 + k);
+        const unsigned int nearbit = (tt + near_gap < 0.0f) ? 0x8000u : 0u;   // d2 < r_c^2
+        if (m) *reinterpret_cast<unsigned short*>(reinterpret_cast<char*>(tmp_blk) + off) = (unsigned short)((unsigned int)(t0 + k) | nearbit);
         off = min(off + ((unsigned int)m & (2u * MD_TB)), offmax);
     }
 }
@@ -449,6 +453,11 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     //    stencil cell, a bitmask of the candidates inside r_v (scan_cell_mask); pass B turns the masks into the row.
     int cnt = 0, lo_cnt = 0;
     bool bucketed = false, bucket_over = false;                   // dense cells: the scan already filled the column buckets
+    // Rigid bodies (few, expensive pairs; half of the listed pairs outside r_c): rows start with the neighbours that were
+    // inside the CUTOFF at build time, in scan order, instead of being scheduled by bank column (their 12-entry rows put no
+    // load on the shared-memory pipe).  The lanes of a warp then meet the pairs they evaluate at the same row positions
+    // and the in-cutoff branch of the force kernel diverges only where a pair has crossed r_c since the build.
+    const bool near_first = !MASKS && P.kind == MD_POT_PATCHY && P.row_schedule && P.stage_cap < 32768;
     unsigned long long pops_pre = 0ull;
     const int W = P.mask_words;                                   // 32-bit mask words per stencil cell
     constexpr bool use_masks = MASKS;                             // else: list form (few particles per cell)
@@ -465,6 +474,7 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
         float bandmin = maywrap ? 0.0f : 3.0e38f;                 // maywrap blocks go straight to the careful scan
         if (!maywrap && !use_masks) {
             const float rv2 = P.rv2;
+            const float near_gap = near_first ? P.rv2 - P.rc2 : -1.0f;
             unsigned int off = 2u * tid;
             const unsigned int offmax = (unsigned int)(P.cap + 1) * (2u * MD_TB) + 2u * tid;
             for (int sc = 0; sc < 27; ++sc) {
@@ -473,11 +483,11 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
                 const int t0 = ubase[u], n = ubase[u + 1] - t0;
                 const float4* cellpos = pos + ustart[u];
                 if (sc == 13) {                           // stencil entry 13 is the own cell: exclude the particle itself
-                    if (shift_ok) scan_cell_fast<true, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
-                    else scan_cell_fast<false, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
+                    if (shift_ok) scan_cell_fast<true, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin, near_gap);
+                    else scan_cell_fast<false, true>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin, near_gap);
                 } else {
-                    if (shift_ok) scan_cell_fast<true, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
-                    else scan_cell_fast<false, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin);
+                    if (shift_ok) scan_cell_fast<true, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin, near_gap);
+                    else scan_cell_fast<false, false>(cellpos, n, t0, me, xi, rv2, hLx, hLy, hLz, tLx, tLy, tLz, tmp_blk, off, offmax, bandmin, near_gap);
                 }
             }
             cnt = (int)((off - 2u * tid) / (2u * MD_TB));   // cap + 1 = overflow
@@ -546,7 +556,7 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     auto for_each_neighbour = [&](auto&& f) {
         if (!use_masks) {
             const int c2l = min(cnt, P.cap);
-            for (int k = 0; k < c2l; ++k) f((int)tmp[(size_t)k * MD_TB]);
+            for (int k = 0; k < c2l; ++k) f((int)(tmp[(size_t)k * MD_TB] & 0x7fffu));
             return;
         }
         for (int sc = 0; sc < 27; ++sc) {
@@ -580,13 +590,33 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
         unsigned long long pops = 0ull, rem8 = 0ull;
         int c2e = c2;                                      // entries to emit (0 after a bucket overflow)
         int lo_e = 0;                                      // neighbours with a lower slot, counted while emitting
-        if (c2 > 0 && !P.row_schedule && !use_masks) {
+        if (c2 > 0 && near_first) {
+            // two sweeps over the scan-order list: near neighbours first, then the rest (careful-path lists carry no flags: all "rest")
+            int kout = 0;
+            for (int pass = 0; pass < 2; ++pass) {
+                for (int k = 0; k < c2; ++k) {
+                    const unsigned int raw = tmp[(size_t)k * MD_TB];
+                    if (((raw >> 15) & 1u) == (unsigned int)pass) continue;      // pass 0 takes the flagged entries
+                    const unsigned int tq = raw & 0x7fffu;
+                    lo_e += (int)tq < me ? 1 : 0;
+                    w[kout & 3] = tq << rsh;
+                    if ((kout & 3) == 3) rowb[(size_t)(kout >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+                    ++kout;
+                }
+            }
+            if (kout & 3) {
+                for (int q = kout & 3; q < 4; ++q) w[q] = dummy;
+                rowb[(size_t)(kout >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+            }
+            lo_cnt = lo_e;
+            c2e = 0;                                       // nothing left for the scheduled emission below
+        } else if (c2 > 0 && !P.row_schedule && !use_masks) {
             // scan order, no column scheduling: the list the candidate scan left in scratch goes straight into the row
             for (int k0 = 0; k0 < c2; k0 += 4) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     const int k = k0 + q;
-                    const unsigned int tq = k < c2 ? (unsigned int)tmp[(size_t)k * MD_TB] : 0x7fffffffu;
+                    const unsigned int tq = k < c2 ? (unsigned int)(tmp[(size_t)k * MD_TB] & 0x7fffu) : 0x7fffffffu;
                     lo_e += (int)tq < me ? 1 : 0;
                     w[q] = k < c2 ? (tq << rsh) : dummy;
                 }
