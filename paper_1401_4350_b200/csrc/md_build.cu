@@ -237,7 +237,9 @@ void md_launch_build_cells(md_system* s, bool gated) {
     k_cell_rank_sort<<<nbN, 256, 0, s->stream>>>(P, s->B, g);
     s->launches += 2;
     if (s->order != MD_ORDER_NONE) {
-        float4* arrs[6] = { s->pos, s->vel, s->force, s->quat, s->angmom, s->torque };
+        // inside md_integrate (gated) the rebuild sits between the drift and the force evaluation: forces and torques are
+        // dead there and are recomputed in the new order right after, so they are not carried through the permutation
+        float4* arrs[6] = { s->pos, s->vel, gated ? nullptr : s->force, s->quat, s->angmom, gated ? nullptr : s->torque };
         StateArrays S;
         S.n = 0;
         for (int a = 0; a < 6; ++a) if (arrs[a]) S.a[S.n++] = arrs[a];
