@@ -195,6 +195,23 @@ def time_steps(torch, s, w, K, Wm, strategy, variant, dev, dist=None):
     return ms_total, 0.5 * (E0 + st1["n_edges"]), launches, st1["n_rebuilds"] - stw["n_rebuilds"], e_tot
 
 
+def in_situ_times(torch, s, w, strategy, variant, nsteps=10):
+    """The force kernel timed INSIDE real steps (back-to-back calls on fixed lists are the warm best case):
+    md_half_step(kick+drift) / md_forces / md_half_step(kick) with CUDA events around each call, `nsteps` steps right after
+    a list build (no rebuild can fall due that soon), median per call in microseconds."""
+    s.build_cells(); s.build_verlet(); s.forces(strategy, variant)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(nsteps)]
+    for k in range(nsteps):
+        ev[k][0].record(); s.half_step(w.dt, "kick_drift")
+        ev[k][1].record(); s.forces(strategy, variant)
+        ev[k][2].record(); s.half_step(w.dt, "kick")
+        ev[k][3].record()
+    torch.cuda.synchronize()
+    med = lambda a, b: statistics.median(ev[k][a].elapsed_time(ev[k][b]) * 1e3 for k in range(2, nsteps))
+    return {"kick_drift_us": med(0, 1), "force_us": med(1, 2), "kick_us": med(2, 3), "steps": nsteps - 2,
+            "what": "CUDA events around md_half_step / md_forces / md_half_step inside consecutive real steps (plain launches)"}
+
+
 def oracle_inputs(s, w):
     """The state the GPU holds, in original id order, as the oracle's input (identical input, S:8(d))."""
     pos = s.in_id_order(s.pos)
@@ -499,6 +516,8 @@ def main():
                                                    probes, args.workload)
     roofline = rooflines[f"{args.strategy}_{args.scatter}"]
     roofline["threads_per_particle"] = sx["threads_per_particle"]
+    situ = in_situ_times(torch, s, w, args.strategy, args.scatter)
+    roofline["in_situ"] = dict(situ, frac=roofline["frac"] * roofline["us_per_launch"] / situ["force_us"])
 
     # ---- whole-path steps: K x md_integrate(1 step) + one md_energy, device-resident state; both strategies ----
     ms_total, E_run, launches, rebuilds, e_tot = time_steps(torch, s, w, K, Wm, args.strategy, args.scatter, dev, dist)
