@@ -374,6 +374,13 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
         P.n_patches = pot->n_patches;
         for (int a = 0; a < MD_MAX_PATCH; ++a)
             for (int k = 0; k < 3; ++k) P.pdir[a][k] = a < pot->n_patches ? pot->patch_dir[a][k] : 0.0f;
+        {   // config 4's patch set (S:O4): b_1..b_4 = (1,1,1), (1,-1,-1), (-1,1,-1), (-1,-1,1) / sqrt(3), in this order
+            static const float tet[4][3] = { { 1, 1, 1 }, { 1, -1, -1 }, { -1, 1, -1 }, { -1, -1, 1 } };
+            P.tetra = pot->n_patches == 4 ? 1 : 0;
+            for (int a = 0; a < 4 && P.tetra; ++a)
+                for (int k = 0; k < 3; ++k)
+                    if (fabsf(pot->patch_dir[a][k] - tet[a][k] * 0.57735026918962576f) > 1e-6f) P.tetra = 0;
+        }
         P.eps_patch = pot->eps_patch;
         P.inv_sr2 = 1.0f / (pot->patch_sigma_r * pot->patch_sigma_r);
         P.inv_2sr2 = 0.5f * P.inv_sr2;
@@ -538,8 +545,7 @@ static void ensure_explicit(md_system* s) {
 // The (cluster, j) unit list of MD_SCATTER_CLUSTER for the current build, made on demand like the explicit lists.
 static md_status ensure_cluster(md_system* s) {
     if (s->cluster_valid) return MD_OK;
-    DevCtrl before;      // the build recounts E from its own units: the counters must come out the same
-    (void)before;
+    // (the build recounts E from its own units and rewrites the list counters: they must come out the same)
     if (!md_launch_build_cluster(s, false, s->B.pos_ref)) return fail(s, MD_ERR_CAPACITY, "MD_SCATTER_CLUSTER: max_neigh too large for the cluster build's shared memory");
     s->cluster_valid = true;
     return MD_OK;

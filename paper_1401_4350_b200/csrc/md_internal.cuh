@@ -85,6 +85,7 @@ struct DevParams {
     int chain_len;
     // patches
     int n_patches;
+    int tetra;                         // the patch set is config 4's tetrahedron in its canonical order: packed fast path (md_pair.cuh)
     float pdir[MD_MAX_PATCH][3];
     float eps_patch, inv_2sr2, inv_sr2, inv_w2, sigma, inv_inertia;
     // MD_POT_PATCHY_PP (the paper's own patchy model, S:8(f2)): runs on the rigid-body kernels with kind == MD_POT_PATCHY

@@ -106,6 +106,40 @@ __device__ __forceinline__ void patch_factor(const DevParams& P, const Rot& R, f
     Sz = P.inv_w2 * (R.m[2][0] * bx + R.m[2][1] * by + R.m[2][2] * bz);
 }
 
+// Both angular factors of a pair at once for the TETRAHEDRAL patch set of config 4 (B:10, S:O4: b_a = (+-1, +-1, +-1)/sqrt(3)
+// with an even number of minus signs), in packed f32x2: .x = particle i (direction +u), .y = particle j (direction -u).
+// The four dot products b_a.v need no multiplications (sums and differences of the components of v), and neither does
+// sum_a e_a b_a; 1/sqrt(3) is folded into the exponent scale and into the prefactor of S.  ~28 packed instructions + 8 MUFU
+// for both particles, against 2 x 45 scalar ones in patch_factor<4>.  R2[m][n] = (R_i[m][n], R_j[m][n]).
+__device__ __forceinline__ void patch_factor2_tetra(const DevParams& P, const float2 (&R2)[3][3], float ux, float uy, float uz,
+                                                    float2& A, float2& Sx, float2& Sy, float2& Sz) {
+    const float2 U0 = make_float2(ux, -ux), U1 = make_float2(uy, -uy), U2 = make_float2(uz, -uz);
+    // v = R^T dir
+    const float2 vx = __ffma2_rn(R2[2][0], U2, __ffma2_rn(R2[1][0], U1, __fmul2_rn(R2[0][0], U0)));
+    const float2 vy = __ffma2_rn(R2[2][1], U2, __ffma2_rn(R2[1][1], U1, __fmul2_rn(R2[0][1], U0)));
+    const float2 vz = __ffma2_rn(R2[2][2], U2, __ffma2_rn(R2[1][2], U1, __fmul2_rn(R2[0][2], U0)));
+    const float2 nvz = make_float2(-vz.x, -vz.y);
+    const float2 s = __fadd2_rn(vx, vy), d = __fadd2_rn(vx, make_float2(-vy.x, -vy.y));
+    // sqrt(3) b_a . v for b_1 = (1,1,1), b_2 = (1,-1,-1), b_3 = (-1,1,-1), b_4 = (-1,-1,1)
+    const float2 c1 = __fadd2_rn(s, vz), c2 = __fadd2_rn(d, nvz), c3 = __fadd2_rn(make_float2(-d.x, -d.y), nvz),
+                 c4 = __fadd2_rn(vz, make_float2(-s.x, -s.y));
+    const float k = P.inv_w2 * 1.4426950408889634f;                 // exp(x) = 2^(x log2 e)
+    const float2 ks = make_float2(k * 0.57735026918962576f, k * 0.57735026918962576f), nk = make_float2(-k, -k);
+    const float2 x1 = __ffma2_rn(c1, ks, nk), x2 = __ffma2_rn(c2, ks, nk), x3 = __ffma2_rn(c3, ks, nk), x4 = __ffma2_rn(c4, ks, nk);
+    const float2 e1 = make_float2(ex2_approx(x1.x), ex2_approx(x1.y)), e2 = make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
+    const float2 e3 = make_float2(ex2_approx(x3.x), ex2_approx(x3.y)), e4 = make_float2(ex2_approx(x4.x), ex2_approx(x4.y));
+    const float2 p12 = __fadd2_rn(e1, e2), p34 = __fadd2_rn(e3, e4);
+    const float2 m12 = __fadd2_rn(e1, make_float2(-e2.x, -e2.y)), m34 = __fadd2_rn(e3, make_float2(-e4.x, -e4.y));
+    A = __fadd2_rn(p12, p34);
+    // sqrt(3) sum_a e_a b_a = (e1 + e2 - e3 - e4, e1 - e2 + e3 - e4, e1 - e2 - e3 + e4)
+    const float2 bx = __fadd2_rn(p12, make_float2(-p34.x, -p34.y)), by = __fadd2_rn(m12, m34), bz = __fadd2_rn(m12, make_float2(-m34.x, -m34.y));
+    const float w = P.inv_w2 * 0.57735026918962576f;
+    const float2 w2 = make_float2(w, w);
+    Sx = __fmul2_rn(w2, __ffma2_rn(R2[0][2], bz, __ffma2_rn(R2[0][1], by, __fmul2_rn(R2[0][0], bx))));
+    Sy = __fmul2_rn(w2, __ffma2_rn(R2[1][2], bz, __ffma2_rn(R2[1][1], by, __fmul2_rn(R2[1][0], bx))));
+    Sz = __fmul2_rn(w2, __ffma2_rn(R2[2][2], bz, __ffma2_rn(R2[2][1], by, __fmul2_rn(R2[2][0], bx))));
+}
+
 // x^n for a small runtime integer n >= 1 by squaring (the paper's exponents: 100 = 200/2 and 5 = 10/2)
 __device__ __forceinline__ float ipow(float x, int n) {
     float r = 1.0f;
@@ -168,8 +202,19 @@ __device__ __forceinline__ void patchy_pair(const DevParams& P, float dx, float 
     float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
     float Ai, Six, Siy, Siz, Aj, Sjx, Sjy, Sjz;
     const Rot Rj = quat_to_rot(qj);
-    patch_factor<NP>(P, Ri, ux, uy, uz, Ai, Six, Siy, Siz);
-    patch_factor<NP>(P, Rj, -ux, -uy, -uz, Aj, Sjx, Sjy, Sjz);
+    if (NP == 4 && P.tetra) {       // config 4's tetrahedral patch set: both factors in packed f32x2
+        float2 R2[3][3];
+#pragma unroll
+        for (int m = 0; m < 3; ++m)
+#pragma unroll
+            for (int n = 0; n < 3; ++n) R2[m][n] = make_float2(Ri.m[m][n], Rj.m[m][n]);
+        float2 A, Sx, Sy, Sz;
+        patch_factor2_tetra(P, R2, ux, uy, uz, A, Sx, Sy, Sz);
+        Ai = A.x; Aj = A.y; Six = Sx.x; Sjx = Sx.y; Siy = Sy.x; Sjy = Sy.y; Siz = Sz.x; Sjz = Sz.y;
+    } else {
+        patch_factor<NP>(P, Ri, ux, uy, uz, Ai, Six, Siy, Siz);
+        patch_factor<NP>(P, Rj, -ux, -uy, -uz, Aj, Sjx, Sjy, Sjz);
+    }
     float dr = r - P.sigma;
     float G = ex2_approx(-dr * dr * P.inv_2sr2 * 1.4426950408889634f);
     float dG = -dr * P.inv_sr2 * G;

@@ -166,6 +166,31 @@ def test_step_graph_equals_plain_launches(MD):
     assert out[0][3] == (4 * 25 + 5 * 4) / 37 and out[1][3] > 4
 
 
+def test_options_row_schedule_and_unknown(MD, oracle):
+    """MD_OPT_ROW_SCHEDULE = 0 (Verlet rows in scan order instead of bank-column order: the measured alternative of
+    DESIGN.md section 10) changes the order of the row entries only: same pair set, forces within tolerance."""
+    from paper_1401_4350_b200 import MDError
+    w = W.lj_fluid(2 ** 14)
+    o = oracle.forces(w.pos, w.box, dict(w.potential))
+    s = MD.from_workload(w, order="hilbert")
+    for sched in (0, 1):
+        s.set_option("row_schedule", sched)
+        with pytest.raises(MDError) as e:
+            s.forces("vertex", "smem")                   # the option invalidates the lists
+        assert e.value.code == -2
+        s.build_cells(); s.build_verlet()
+        assert_pairs(s, oracle, s.in_id_order(s.pos), w.box, w.rcut, w.skin)
+        s.forces("vertex", "smem")
+        assert_forces(s, o, False, (f"lj16384 row_schedule={sched}", "vertex_smem"))
+    with pytest.raises(MDError) as e:
+        s.set_option(99, 1)
+    assert e.value.code == -1
+    with pytest.raises(MDError) as e:
+        s.set_option("no_graph", -1)
+    assert e.value.code == -1
+    s.close()
+
+
 def test_error_paths(MD):
     from paper_1401_4350_b200 import MDError
     w = W.config("C1")
