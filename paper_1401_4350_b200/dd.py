@@ -107,33 +107,35 @@ class LocalTransport:
 
 
 class DistTransport:
-    """One domain per process, torch.distributed point-to-point (backend nccl on GPUs, gloo on CPU)."""
+    """One domain per process, torch.distributed point-to-point: backend nccl moves device buffers GPU to GPU; with
+    `stage_host` the messages go through host memory (backend gloo: CPU tests, or several processes sharing one GPU)."""
 
-    def __init__(self, plan: SlabPlan, dist, device):
+    def __init__(self, plan: SlabPlan, dist, device, stage_host: bool = False):
         self.plan, self.dist, self.device = plan, dist, device
+        self.wire = "cpu" if stage_host else device        # where the buffers handed to torch.distributed live
         self.rank = dist.get_rank()
 
     def _sendrecv(self, send_to, send_msg, recv_from, like):
         import torch
         dist = self.dist
-        n_out = torch.tensor([send_msg[0].shape[0] if send_msg else 0], dtype=torch.int64, device=self.device)
-        n_in = torch.zeros(1, dtype=torch.int64, device=self.device)
+        n_out = torch.tensor([send_msg[0].shape[0] if send_msg else 0], dtype=torch.int64, device=self.wire)
+        n_in = torch.zeros(1, dtype=torch.int64, device=self.wire)
         ops = [dist.P2POp(dist.isend, n_out, send_to), dist.P2POp(dist.irecv, n_in, recv_from)]
         for w in dist.batch_isend_irecv(ops):
             w.wait()
         n = int(n_in.item())
-        recv = [torch.empty((n,) + tuple(t.shape[1:]), dtype=t.dtype, device=self.device) for t in like]
+        recv = [torch.empty((n,) + tuple(t.shape[1:]), dtype=t.dtype, device=self.wire) for t in like]
         ops = []
         for t in send_msg:
             if t.shape[0] > 0:
-                ops.append(dist.P2POp(dist.isend, t.contiguous(), send_to))
+                ops.append(dist.P2POp(dist.isend, t.contiguous().to(self.wire), send_to))
         for t in recv:
             if n > 0:
                 ops.append(dist.P2POp(dist.irecv, t, recv_from))
         if ops:
             for w in dist.batch_isend_irecv(ops):
                 w.wait()
-        return recv
+        return [r.to(self.device) for r in recv]
 
     def exchange(self, outgoing):
         r = self.rank
@@ -146,7 +148,7 @@ class DistTransport:
 
     def any_flag(self, flags) -> bool:
         import torch
-        t = torch.tensor([int(max(flags.values()))], dtype=torch.int32, device=self.device)
+        t = torch.tensor([int(max(flags.values()))], dtype=torch.int32, device=self.wire)
         self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
         return bool(t.item())
 

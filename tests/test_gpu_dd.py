@@ -137,3 +137,50 @@ def test_patchy_domains(oracle):
     assert np.abs(F[:, :3] - o["F"]).max() <= FTOL_REL * np.abs(o["F"]).max() + FTOL_ABS
     assert np.abs(T[:, :3] - o["T"]).max() <= FTOL_REL * np.abs(o["T"]).max() + FTOL_ABS
     sim.close()
+
+
+def _dd_worker(rank, world, port, out):
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    from paper_1401_4350_b200.dd import DDSimulation, DistTransport, Domain, SlabPlan
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = W.lj_fluid(2 ** 14, 2.5)
+    plan = SlabPlan(w.box, world, w.rcut + w.skin)
+    d = Domain(rank, plan, w.N, w.rcut, w.skin, w.potential, w.max_neigh, device="cuda:0", strategy="vertex", variant="smem")
+    d.load_initial(w.pos, w.vel)
+    sim = DDSimulation([d], DistTransport(plan, dist, torch.device("cuda:0"), stage_host=True))
+    sim.rebuild()
+    sim.run(w.dt, 60)
+    np.save(out + f".pos.{rank}.npy", sim.gather("pos", w.N))
+    np.save(out + f".force.{rank}.npy", sim.gather("force", w.N))
+    np.save(out + f".e.{rank}.npy", np.array(list(sim.energy()) + [d.n_rebuilds, d.n_own]))
+    sim.close()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_processes_over_torch_distributed(oracle, tmp_path):
+    """The real multi-process path: two ranks, each with its own md_system and its own process, exchanging migrants and
+    halos through torch.distributed (gloo, staged through host memory because both ranks share this one GPU; nothing
+    is timed and no kernel waits on a peer -- the processes block on the host).  bench.py --dd is this with nccl."""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    out = str(tmp_path / "dd2")
+    mp.spawn(_dd_worker, args=(2, port, out), nprocs=2, join=True)
+    w = W.lj_fluid(2 ** 14, 2.5)
+    pos = np.load(out + ".pos.0.npy"); F = np.load(out + ".force.0.npy")
+    p1 = np.load(out + ".pos.1.npy"); F1 = np.load(out + ".force.1.npy")
+    own0, own1 = ~np.isnan(pos[:, 0]), ~np.isnan(p1[:, 0])
+    assert (own0 ^ own1).all()                                       # every particle owned by exactly one rank
+    pos[own1] = p1[own1]; F[own1] = F1[own1]
+    e0, e1 = np.load(out + ".e.0.npy"), np.load(out + ".e.1.npy")
+    assert e0[3] >= 2 and e0[3] == e1[3] and e0[4] + e1[4] == w.N    # the ranks rebuilt together
+    o = oracle.forces(pos, w.box, dict(w.potential))
+    assert np.abs(F[:, :3] - o["F"]).max() <= FTOL_REL * np.abs(o["F"]).max() + FTOL_ABS
+    assert abs((e0[0] + e1[0]) - o["pe"].sum()) <= 1e-5 * abs(o["pe"].sum())
