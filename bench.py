@@ -323,6 +323,8 @@ def roofline_for(strategy, variant, t_us, Ef, E_in, N, rigid, units, probes, wor
     kname = knames[variant]
     if rigid:
         kname = kname.replace("_lj", "_patchy")
+        if variant == "warp" and Ef < 28 * N:      # short rows of rigid bodies: the compacting walk (launch_edge, md_forces.cu)
+            kname = "k_edge_warp_queue"
     traffic = None
     tf = ROOT / "profiles" / "roofline_traffic.csv"     # dram bytes per launch from the committed ncu --set full captures
     if tf.exists():
