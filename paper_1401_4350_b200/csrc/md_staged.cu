@@ -215,6 +215,13 @@ __device__ __noinline__ int scan_cell_slow(const float4* __restrict__ cellpos, i
 // ------------------------------------------------------------------------------------------------
 // S:A4 staged Verlet build.  One block per MD_TB slots, one thread per particle.
 // ------------------------------------------------------------------------------------------------
+#define TS_CB 16     // transposed scan: hit words (32 candidates each) per owner and pass
+#define TS_OC 32     // transposed scan: own cells per block it is sized for (more -> the per-thread scan)
+#define TS_ROW (MD_TB + 2 * TS_OC)   // hit words of one chunk: the owners of every own cell start at an even index
+#define TS_OFF_HITW (16 * MD_TB)     // after three planes of MD_TB + 2 floats
+#define TS_OFF_OWNF (TS_OFF_HITW + 4 * TS_CB * TS_ROW)
+#define TS_OFF_PCS (TS_OFF_OWNF + 2 * (3 * (TS_OC + 2) + 28 * TS_OC))
+#define TS_SMEM_BYTES (TS_OFF_PCS + 16 * MD_TB)
 template <bool MASKS>
 __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
                                                         int ncand_cap, int umax, int tbl_cap) {
@@ -227,7 +234,17 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     int* ubase = urank + umax;                                       // [umax + 1]
     int* ustart = ubase + umax + 1;                                  // [umax] first slot of the cell
     int* own_rank = ustart + umax;                                   // [MD_TB]
+    // transposed scan (MASKS variant): owners' positions, hit words, per-own-cell candidate prefixes
+    const int ts_off = (4 * ((tbl_cap >> 1) + 3 * umax + 1 + MD_TB) + 15) & ~15;     // byte offset from smraw: keeps the shared address space
+    float* xown = reinterpret_cast<float*>(smraw + ts_off);                           // [3][MD_TB + 2] owners' x, y, z planes (pairs of owners load as f32x2)
+    unsigned int* hitw = reinterpret_cast<unsigned int*>(smraw + ts_off + TS_OFF_HITW);   // [TS_CB][TS_ROW]
+    unsigned short* own_first = reinterpret_cast<unsigned short*>(smraw + ts_off + TS_OFF_OWNF);   // [TS_OC + 1] first thread of own cell oc
+    unsigned short* task_base = own_first + TS_OC + 2;               // [TS_OC + 1] chunks of 32 candidates before own cell oc
+    unsigned short* pbase = task_base + TS_OC + 2;                   // [TS_OC + 1] first hit-word index of own cell oc (even)
+    unsigned short* pref = pbase + TS_OC + 2;                        // [TS_OC][28] candidates before stencil cell sc of own cell oc
+    unsigned short* pcs = reinterpret_cast<unsigned short*>(smraw + ts_off + TS_OFF_PCS);   // [8][MD_TB] column populations of pass B
     __shared__ int sh_scan[33];
+    __shared__ int s_tsok;
     __shared__ int s_flags, s_err, s_own_base, s_U;
 
     const int b = blockIdx.x, tid = threadIdx.x;
@@ -467,12 +484,164 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     unsigned short* tmp = tmp_blk + tid;
     const short* __restrict__ mycells = reinterpret_cast<const short*>(cand) + max(myoc, 0) * 27;
     const int me = own_base + tid;
+    // 8a. TRANSPOSED scan (dense cells, no minimum image needed).  The per-thread scan below spends 58 issue slots per
+    //     candidate (lanes in different own cells diverge, ragged cell heads and tails, bucket bookkeeping on every
+    //     candidate).  Here a warp takes one own cell and 32 of the candidates of its stencil (enumerated across the 27
+    //     cells, so every lane holds one): the lane keeps ITS candidate in registers and the warp walks the owners of the
+    //     cell, whose position is one broadcast shared-memory load -- ~15 instructions per 32 tests, one ballot word per
+    //     (owner, 32 candidates).  Each owner thread then turns its hit words into the column buckets of pass B.  The band
+    //     decision (S:Q6) is taken in place, in fp64 on the raw coordinates, by the lanes that meet it.
+    bool tdone = false;
+    if (MASKS && !maywrap && nownc <= TS_OC) {
+        const int lane = tid & 31, wid = tid >> 5;
+        if (tid == 0) s_tsok = 1;
+        if (head) own_first[myoc] = (unsigned short)tid;
+        if (tid == 0) own_first[nownc] = (unsigned short)(i1 - i0);
+        { const float4 xo = live ? load_pos(i) : make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
+          xown[tid] = xo.x; xown[MD_TB + 2 + tid] = xo.y; xown[2 * (MD_TB + 2) + tid] = xo.z; }
+        if (tid < nownc) {
+            int sum = 0;
+            for (int sc = 0; sc < 27; ++sc) {
+                const int u = reinterpret_cast<const short*>(cand)[tid * 27 + sc];
+                pref[tid * 28 + sc] = (unsigned short)sum;
+                if (u >= 0) sum += ubase[u + 1] - ubase[u];
+            }
+            pref[tid * 28 + 27] = (unsigned short)sum;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int tb = 0, mx = 0, pb = 0;
+            for (int oc = 0; oc < nownc; ++oc) {
+                task_base[oc] = (unsigned short)tb;
+                pbase[oc] = (unsigned short)pb;
+                pb += (((int)own_first[oc + 1] + 1) & ~1) - ((int)own_first[oc] & ~1);      // owner pairs of the cell, from an even thread
+
+                const int ch = ((int)pref[oc * 28 + 27] + 31) >> 5;
+                tb += ch;
+                mx = max(mx, ch);
+            }
+            task_base[nownc] = (unsigned short)tb;
+            // the candidate lists (local index of candidate k of own cell oc) live in this block's part of the mask scratch
+            if ((size_t)tb * 32 > (size_t)2 * 27 * P.mask_words * MD_TB || tb > 65535) s_tsok = 0;
+            s_U = mx;       // most chunks of any own cell (s_U is free after step 3)
+        }
+        __syncthreads();
+        if (s_tsok) {
+            tdone = true;
+            const int ntask = task_base[nownc], maxch = s_U;
+            unsigned short* __restrict__ clist = reinterpret_cast<unsigned short*>(B.cmask + (size_t)b * 27 * P.mask_words * MD_TB);
+            const short* __restrict__ cand_s = reinterpret_cast<const short*>(cand);
+            const float rv2 = P.rv2, bandv = P.band_rv;
+            unsigned short* __restrict__ tmp2 = B.rows_tmp + (size_t)b * 8 * cap8 * MD_TB + tid;
+            const int plim = min(cap8, 255);
+            bool over = false;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) pcs[c * MD_TB + tid] = 0;
+            for (int cb0 = 0; cb0 < maxch; cb0 += TS_CB) {
+                if (cb0) __syncthreads();       // the hit words of the previous pass have been consumed
+                int oc = 0;
+                for (int tk = wid; tk < ntask; tk += MD_TB / 32) {
+                    while ((int)task_base[oc + 1] <= tk) ++oc;      // own cell of the task (tasks ascend)
+                    const int chunk = tk - (int)task_base[oc];
+                    if (chunk < cb0 || chunk >= cb0 + TS_CB) continue;
+                    // candidate k of the own cell's stencil -> (stencil cell, rank in it): binary search over the 27 prefixes,
+                    // held one per lane
+                    const int prl = pref[oc * 28 + min(lane, 27)];
+                    const int ktot = __shfl_sync(0xffffffffu, prl, 27);
+                    const int k = chunk * 32 + lane;
+                    const bool valid = k < ktot;
+                    int a = 0;
+#pragma unroll
+                    for (int st = 16; st > 0; st >>= 1) {
+                        const int pm = __shfl_sync(0xffffffffu, prl, min(a + st, 26));
+                        if (a + st <= 26 && pm <= k) a += st;
+                    }
+                    float4 xj = make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
+                    int slot = 0;
+                    const int pa = __shfl_sync(0xffffffffu, prl, a);
+                    if (valid) {
+                        const int u = cand_s[oc * 27 + a];          // pr[a] <= k < pr[a + 1]: cell a is not empty, so u >= 0
+                        const int r = k - pa;
+                        slot = ustart[u] + r;
+                        xj = load_pos(slot);
+                        clist[(size_t)tk * 32 + lane] = (unsigned short)(ubase[u] + r);
+                    }
+                    const int o0 = own_first[oc], o1 = own_first[oc + 1];
+                    unsigned int* __restrict__ hw = hitw + (chunk - cb0) * TS_ROW + (int)pbase[oc] - (o0 & ~1);   // hw[o]: words of owner thread o
+                    unsigned int* __restrict__ hwc = hw;
+                    // two owners per step in packed f32x2 (FADD2 / FMUL2 / FFMA2): pairs start at even threads, the owner
+                    // before o0 / after o1 - 1 of a ragged end is computed and not stored
+                    float bmin = 3.0e38f;
+                    const float2 nxjx = make_float2(-xj.x, -xj.x), nxjy = make_float2(-xj.y, -xj.y), nxjz = make_float2(-xj.z, -xj.z);   // (a - b)^2 == (b - a)^2 exactly
+                    const float2 nrv2 = make_float2(-rv2, -rv2);
+                    const float* __restrict__ xox = xown, * __restrict__ xoy = xown + MD_TB + 2, * __restrict__ xoz = xown + 2 * (MD_TB + 2);
+#pragma unroll 2
+                    for (int o = o0 & ~1; o < o1; o += 2) {
+                        const float2 ox = *reinterpret_cast<const float2*>(xox + o), oy = *reinterpret_cast<const float2*>(xoy + o),
+                                     oz = *reinterpret_cast<const float2*>(xoz + o);
+                        const float2 ddx = __fadd2_rn(ox, nxjx), ddy = __fadd2_rn(oy, nxjy), ddz = __fadd2_rn(oz, nxjz);
+                        const float2 d2 = __ffma2_rn(ddz, ddz, __ffma2_rn(ddy, ddy, __fmul2_rn(ddx, ddx)));
+                        const float2 tt = __fadd2_rn(d2, nrv2);
+                        bmin = fminf(fminf(bmin, fabsf(tt.x)), fabsf(tt.y));
+                        const unsigned int wa = __ballot_sync(0xffffffffu, tt.x < 0.0f);
+                        const unsigned int wb = __ballot_sync(0xffffffffu, tt.y < 0.0f);
+                        if (lane == 0) *reinterpret_cast<uint2*>(hwc + o) = make_uint2(wa, wb);   // padded layout: always in range
+                    }
+                    const bool banded = bmin < bandv;
+                    if (__any_sync(0xffffffffu, banded)) {          // rare: a pair inside the band -> fp64 on the raw coordinates (S:Q6)
+                        for (int o = o0; o < o1; ++o) {
+                            const float ddx = xj.x - xox[o], ddy = xj.y - xoy[o], ddz = xj.z - xoz[o];
+                            const float tt = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)) - rv2;
+                            bool in = tt < 0.0f;
+                            if (fabsf(tt) < bandv) in = inside_fp64(__ldg(pos + i0 + o), __ldg(pos + slot), P.dLx, P.dLy, P.dLz, P.rv2d);
+                            const unsigned int word = __ballot_sync(0xffffffffu, in);
+                            if (lane == 0) hw[o] = word;
+                        }
+                    }
+                }
+                __syncthreads();
+                if (live) {
+                    const int nw = min(TS_CB, (((int)pref[myoc * 28 + 27] + 31) >> 5) - cb0);
+                    const int myhw = (int)pbase[myoc] + tid - ((int)own_first[myoc] & ~1);
+                    const unsigned short* cl = clist + ((size_t)task_base[myoc] + cb0) * 32;
+                    // one flat loop over the set bits of all hit words (a loop per word would run at the pace of the lane with
+                    // the most hits in that word)
+                    int w = -1;
+                    unsigned int bits = 0u;
+                    for (;;) {
+                        if (bits == 0u) {
+                            if (++w >= nw) break;
+                            bits = hitw[w * TS_ROW + myhw];
+                            continue;
+                        }
+                        const int bit = __ffs(bits) - 1;
+                        bits &= bits - 1u;
+                        const int t = cl[w * 32 + bit];
+                        if (t == me) continue;
+                        const int c = t & 7;
+                        const int pp = (int)pcs[c * MD_TB + tid];
+                        if (pp < plim) { tmp2[(size_t)(c * cap8 + pp) * MD_TB] = (unsigned short)t; pcs[c * MD_TB + tid] = (unsigned short)(pp + 1); } else over = true;
+                    }
+                }
+            }
+            if (live) {
+                unsigned long long pops = 0ull;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) { const int pc1 = (int)pcs[c * MD_TB + tid]; cnt += pc1; pops |= (unsigned long long)pc1 << (8 * c); }
+                pops_pre = pops;
+                bucketed = true;
+                bucket_over = over;
+            }
+        }
+    }
     if (live) {
         const float4 xi_raw = __ldg(pos + i);
         const float4 xi = load_pos(i);
         const float hLx = P.hLx, hLy = P.hLy, hLz = P.hLz;
         float bandmin = maywrap ? 0.0f : 3.0e38f;                 // maywrap blocks go straight to the careful scan
-        if (!maywrap && !use_masks) {
+        if (tdone) {
+            // the transposed scan above has filled the buckets
+        } else if (!maywrap && !use_masks) {
             const float rv2 = P.rv2;
             const float near_gap = near_first ? P.rv2 - P.rc2 : -1.0f;
             unsigned int off = 2u * tid;
@@ -742,6 +911,8 @@ void md_launch_build_staged(md_system* s, bool gated) {
     // candidates are read through L1: with the small tables of dense cells leave it as large as the resident blocks allow
     // (measured at C2a: carveout 25 -> 1.96 ms, 50 -> 1.65, 75 -> 1.82, 100 -> 2.02); the 42 KB tables of sparse cells need
     // the shared memory itself (five resident blocks instead of two)
+    const bool tscan = P.use_masks && P.row_schedule;           // k_build_staged<true>: + the arrays of the transposed scan
+    if (tscan) smem += TS_SMEM_BYTES + 16;
     const int carve = smem > 30 * 1024 ? (int)cudaSharedmemCarveoutMaxShared : 50;
     if (carve != s->build_carve) {      // per handle = per device (function attributes are per device)
         cudaFuncSetAttribute(k_build_staged<true>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
@@ -749,7 +920,7 @@ void md_launch_build_staged(md_system* s, bool gated) {
         s->build_carve = carve;
     }
     k_staged_begin<<<1, 1, 0, s->stream>>>(s->B, g);
-    if (P.use_masks && P.row_schedule) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
+    if (tscan) k_build_staged<true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
     else k_build_staged<false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, g, s->pos, nc, um, tc);
     s->launches += 2;
 }
