@@ -315,8 +315,22 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     // 4. bitonic sort of the distinct ranks (ascending rank = ascending slot)
     int U2 = 32;
     while (U2 < U) U2 <<= 1;                          // U2 <= umax (a power of two)
-    for (int t = U + tid; t < U2; t += MD_TB) urank[t] = 0x7fffffff;
-    __syncthreads();
+    if (U <= MD_TB) {
+        // few distinct cells (dense cells: ~100): rank sort, one element per thread, two barriers instead of the ~30 of the
+        // bitonic network (the values are distinct: position = number of smaller ones)
+        int r = 0, p = 0;
+        if (tid < U) {
+            r = urank[tid];
+            for (int x = 0; x < U; ++x) p += urank[x] < r ? 1 : 0;
+        }
+        __syncthreads();
+        if (tid < U) urank[p] = r;
+        __syncthreads();
+        U2 = 0;                                        // skip the network below
+    } else {
+        for (int t = U + tid; t < U2; t += MD_TB) urank[t] = 0x7fffffff;
+        __syncthreads();
+    }
     for (int k = 2; k <= U2; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
             for (int t = tid; t < U2; t += MD_TB) {
@@ -605,22 +619,30 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
                     const int myhw = (int)pbase[myoc] + tid - ((int)own_first[myoc] & ~1);
                     const unsigned short* cl = clist + ((size_t)task_base[myoc] + cb0) * 32;
                     // one flat loop over the set bits of all hit words (a loop per word would run at the pace of the lane with
-                    // the most hits in that word)
+                    // the most hits in that word); the candidate-list entry of the NEXT hit is requested before the current one
+                    // is filed, so the two memory latencies overlap
                     int w = -1;
                     unsigned int bits = 0u;
-                    for (;;) {
-                        if (bits == 0u) {
-                            if (++w >= nw) break;
+                    auto next_hit = [&]() {
+                        while (bits == 0u) {
+                            if (++w >= nw) return -1;
                             bits = hitw[w * TS_ROW + myhw];
-                            continue;
                         }
                         const int bit = __ffs(bits) - 1;
                         bits &= bits - 1u;
-                        const int t = cl[w * 32 + bit];
-                        if (t == me) continue;
-                        const int c = t & 7;
-                        const int pp = (int)pcs[c * MD_TB + tid];
-                        if (pp < plim) { tmp2[(size_t)(c * cap8 + pp) * MD_TB] = (unsigned short)t; pcs[c * MD_TB + tid] = (unsigned short)(pp + 1); } else over = true;
+                        return w * 32 + bit;
+                    };
+                    int idx = next_hit();
+                    int tn = idx >= 0 ? (int)cl[idx] : me;
+                    while (idx >= 0) {
+                        const int t = tn;
+                        idx = next_hit();
+                        if (idx >= 0) tn = cl[idx];
+                        if (t != me) {
+                            const int c = t & 7;
+                            const int pp = (int)pcs[c * MD_TB + tid];
+                            if (pp < plim) { tmp2[(size_t)(c * cap8 + pp) * MD_TB] = (unsigned short)t; pcs[c * MD_TB + tid] = (unsigned short)(pp + 1); } else over = true;
+                        }
                     }
                 }
             }
