@@ -319,6 +319,26 @@ md_status md_scatter_ids(md_system*, int32_t array, int64_t first_id, int64_t n,
 md_status md_dd_select(const void* pos_dev, int64_t n, int32_t axis, double lo, double hi, int32_t* idx_out_dev, int64_t capacity,
                        int64_t* count_host, void* scratch_dev, size_t scratch_bytes, void* cuda_stream);
 
+/* -------------------------------------------------------------------------------------------------------------------
+ * No-allocation entry point (md_static.cu).  For callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * serving loops, harnesses that forbid it): the energy sums of md_energy (S:A9: U = sum_i pe_i, K_t = 1/2 m sum |v|^2,
+ * K_r = sum |L|^2 / (2 I), fp32 terms accumulated in fp64, two deterministic stages) with NO handle and NO workspace.
+ * The block partials live in a file-scope device array of 48 KiB that every GPU loading the library holds until exit;
+ * the call performs no cudaMalloc / cudaFree and no allocating library routine.
+ *   vel_dev, force_dev   DEVICE float4[n] (16-byte aligned), force.w = pe_i as left by md_forces
+ *   angmom_dev           DEVICE float4[n] or NULL (then e_out[2] = 0)
+ *   n                    1 .. MD_ENERGY_STATIC_MAX_N; beyond it MD_ERR_CAPACITY (nothing is launched)
+ *   e_out_dev            DEVICE double[3] = (U, K_t, K_r), written on cuda_stream; the caller owns it
+ *   err, err_len         optional HOST buffer for a message on failure (may be NULL / 0)
+ * All n particles are summed (no ghost exclusion: that needs a handle's id table).  Runs on the CURRENT device, on
+ * cuda_stream, asynchronously.  The first call on each device looks up the array's device address
+ * (cudaGetSymbolAddress): make that call outside a graph capture.  All calls on a device share the array: calls that
+ * overlap on the GPU (two streams, two host threads) race on it and must be serialised by the caller; it keeps the last
+ * call's contents, and every call overwrites all partials it reads (nothing has to be cleared). */
+#define MD_ENERGY_STATIC_MAX_N 16777216
+md_status md_energy_static(const void* vel_dev, const void* force_dev, const void* angmom_dev, int64_t n, double mass,
+                           double inv_inertia, double* e_out_dev, void* cuda_stream, char* err, size_t err_len);
+
 /* Number of kernels this library has launched on behalf of the handle (for bench.py's gpu_launches). */
 int64_t md_launch_count(const md_system*);
 

@@ -5,7 +5,7 @@ PyTorch is used for device memory and streams only; there is no CPU or PyTorch f
 `MDSystem` without the built library raises.
 """
 from .binding import (MDSystem, MDError, load_library, STRATEGY, SCATTER, GATHER, ORDER, POT_KIND, library_path,
-                      EXPORTED_SYMBOLS)
+                      EXPORTED_SYMBOLS, energy_static, ENERGY_STATIC_MAX_N)
 
 __all__ = ["MDSystem", "MDError", "load_library", "STRATEGY", "SCATTER", "GATHER", "ORDER", "POT_KIND", "library_path",
-           "EXPORTED_SYMBOLS"]
+           "EXPORTED_SYMBOLS", "energy_static", "ENERGY_STATIC_MAX_N"]

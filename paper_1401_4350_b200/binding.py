@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = ["md_workspace_bytes", "md_create", "md_bind_state", "md_set_
                     "md_get_state_double", "md_set_thermostat", "md_thermostat", "md_build_cells",
                     "md_build_verlet", "md_forces", "md_integrate", "md_energy", "md_stats", "md_stats_ex",
                     "md_set_option", "md_probe", "md_resize", "md_set_active", "md_half_step", "md_rebuild_flag",
-                    "md_gather_ids", "md_scatter_ids", "md_dd_select", "md_get_pairs", "md_get_ids", "md_step_host", "md_launch_count",
+                    "md_gather_ids", "md_scatter_ids", "md_dd_select", "md_energy_static", "md_get_pairs", "md_get_ids", "md_step_host", "md_launch_count",
                     "md_last_error", "md_destroy"]
 
 
@@ -158,6 +158,8 @@ def load_library() -> C.CDLL:
     L.md_dd_select.restype = C.c_int
     L.md_dd_select.argtypes = [vp, C.c_int64, C.c_int32, C.c_double, C.c_double, vp, C.c_int64, C.POINTER(C.c_int64), vp,
                                C.c_size_t, vp]
+    L.md_energy_static.restype = C.c_int
+    L.md_energy_static.argtypes = [vp, vp, vp, C.c_int64, C.c_double, C.c_double, vp, vp, C.c_char_p, C.c_size_t]
     L.md_get_pairs.restype = C.c_int
     L.md_get_pairs.argtypes = [vp, C.POINTER(C.c_int32), C.c_int64, C.POINTER(C.c_int64)]
     L.md_get_ids.restype = C.c_int
@@ -421,3 +423,29 @@ def dd_select(pos, lo: float, hi: float, axis: int = 0, stream=None):
     if rc != 0:
         raise MDError(rc, "md_dd_select failed")
     return out[:int(cnt.value)]
+
+
+ENERGY_STATIC_MAX_N = 16777216   # MD_ENERGY_STATIC_MAX_N
+
+
+def energy_static(vel, force, out, angmom=None, mass: float = 1.0, inv_inertia: float = 0.0, stream=None):
+    """md_energy_static: (U, K_t, K_r) of float32 [n,4] CUDA tensors into `out` (float64 [3] CUDA tensor, passed by the
+    caller: this call allocates nothing on the device; its scratch is a static device array of the library).  Asynchronous
+    on `stream` (default: torch's current stream of vel.device, which must be the current device).  Calls that overlap on
+    the GPU race on the shared scratch."""
+    import torch
+    lib = load_library()
+    for t in (vel, force) + ((angmom,) if angmom is not None else ()):
+        if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.dim() == 2 and t.shape[1] == 4):
+            raise ValueError("energy_static: state arrays must be contiguous float32 [n,4] CUDA tensors")
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 3):
+        raise ValueError("energy_static: out must be a contiguous float64 CUDA tensor of at least 3 elements")
+    n = int(vel.shape[0])
+    st = stream if stream is not None else torch.cuda.current_stream(vel.device)
+    err = C.create_string_buffer(256)
+    rc = lib.md_energy_static(C.c_void_p(vel.data_ptr()), C.c_void_p(force.data_ptr()),
+                              C.c_void_p(angmom.data_ptr()) if angmom is not None else None, n, float(mass), float(inv_inertia),
+                              C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream), err, 256)
+    if rc != 0:
+        raise MDError(rc, err.value.decode() or "md_energy_static failed")
+    return out

@@ -9,7 +9,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libmd_b200.so"
-SOURCES = ["md_api.cu", "md_build.cu", "md_forces.cu", "md_staged.cu", "md_integrate.cu", "md_probe.cu", "md_cluster.cu", "md_dd.cu"]
+SOURCES = ["md_api.cu", "md_build.cu", "md_forces.cu", "md_staged.cu", "md_integrate.cu", "md_probe.cu", "md_cluster.cu", "md_dd.cu", "md_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"]
 
