@@ -131,9 +131,13 @@ typedef enum {
     MD_OPT_NO_GRAPH = 1,    /* != 0: md_integrate launches its kernels one by one instead of replaying CUDA graphs
                                (profilers then list every kernel); same results bit for bit                          */
     MD_OPT_DEBUG = 2,       /* != 0: step-graph construction failures are printed on stderr                         */
-    MD_OPT_ROW_SCHEDULE = 3 /* staged Verlet rows: 1 (default) = entries ordered at build time by shared-memory bank column
+    MD_OPT_ROW_SCHEDULE = 3, /* staged Verlet rows: 1 (default) = entries ordered at build time by shared-memory bank column
                                so that the 128-bit gathers of the force kernels are conflict-free; 0 = scan order (a
                                cheaper build, more bank conflicts per force evaluation).  Invalidates the lists.      */
+    MD_OPT_BUILD_DIRECT = 4 /* staged Verlet build, dense cells: 1 (default) = the scheduled rows are emitted straight from the
+                               hit words of the transposed scan (candidates enumerated by bank column); 0 = through the
+                               column buckets in scratch memory (the form before it).  Same rows bit for bit.
+                               Invalidates the lists.                                                                */
 } md_option;
 
 /* md_probe kinds: machine ceilings other than HBM bandwidth that bound the force kernels (S:8(d)). */

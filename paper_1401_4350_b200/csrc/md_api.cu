@@ -332,6 +332,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.nblk = g.nblk; P.rcap = g.rcap; P.mask_words = g.mask_words;
     P.use_masks = ((double)N / (double)g.ncell >= 8.0) ? 1 : 0;
     P.row_schedule = 1;   // measured: masks win at 17.7 particles per cell, lists at 2.5-3
+    P.build_direct = 1;
     P.stage_cap = (int)((224 * 1024 - 16) / (rigid ? 32 : 16)) - 1;
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);
@@ -853,6 +854,11 @@ md_status md_set_option(md_system* s, int32_t option, int64_t value) {
     case MD_OPT_ROW_SCHEDULE:
         s->P.row_schedule = value != 0 ? 1 : 0;
         drop_step_graph(s);            // the graph bakes the parameter block in
+        s->lists_valid = s->staged_valid = s->legacy_valid = s->seg_valid = s->cluster_valid = false;
+        return MD_OK;
+    case MD_OPT_BUILD_DIRECT:
+        s->P.build_direct = value != 0 ? 1 : 0;
+        drop_step_graph(s);
         s->lists_valid = s->staged_valid = s->legacy_valid = s->seg_valid = s->cluster_valid = false;
         return MD_OK;
     case MD_OPT_DEBUG: s->debug = value != 0; return MD_OK;

@@ -70,6 +70,7 @@ struct DevParams {
     int nblk, stage_cap, rcap, mask_words;   // mask_words: 32-bit candidate-mask words per stencil cell (build scratch)
     int use_masks;                     // staged build: candidate masks (1) or index lists (0, few particles per cell)
     int row_schedule;                  // staged build: 1 = rows ordered by bank column (pass B buckets), 0 = scan order (MD_OPT_ROW_SCHEDULE)
+    int build_direct;                  // staged build, dense cells: 1 = rows emitted from the hit words (MD_OPT_BUILD_DIRECT)
     float skinf;
     float shift_margin;                // r_v + skin: see k_build_staged step 7c
     // pair potential

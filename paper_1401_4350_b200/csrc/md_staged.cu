@@ -215,13 +215,28 @@ __device__ __noinline__ int scan_cell_slow(const float4* __restrict__ cellpos, i
 // ------------------------------------------------------------------------------------------------
 // S:A4 staged Verlet build.  One block per MD_TB slots, one thread per particle.
 // ------------------------------------------------------------------------------------------------
-#define TS_CB 16     // transposed scan: hit words (32 candidates each) per owner and pass
+#define TS_CB 24     // transposed scan: hit words (32 candidates each) per owner and pass
 #define TS_OC 32     // transposed scan: own cells per block it is sized for (more -> the per-thread scan)
 #define TS_ROW (MD_TB + 2 * TS_OC)   // hit words of one chunk: the owners of every own cell start at an even index
 #define TS_OFF_HITW (16 * MD_TB)     // after three planes of MD_TB + 2 floats
 #define TS_OFF_OWNF (TS_OFF_HITW + 4 * TS_CB * TS_ROW)
-#define TS_OFF_PCS (TS_OFF_OWNF + 2 * (3 * (TS_OC + 2) + 28 * TS_OC))
-#define TS_SMEM_BYTES (TS_OFF_PCS + 16 * MD_TB)
+#define TS_OFF_PCS (TS_OFF_OWNF + 2 * (5 * (TS_OC + 2) + 28 * TS_OC) + 12)    // 16-byte aligned
+#define TS_OFF_CTAB (TS_OFF_PCS + 16 * MD_TB)                                  // direct form: per warp, 28 x 8 column prefixes (bytes)
+#define TS_OFF_PRE13 (TS_OFF_CTAB + (MD_TB / 32) * 28 * 8)
+#define TS_SMEM_BYTES (TS_OFF_PRE13 + 8 * TS_OC)
+static_assert(TS_OFF_PCS % 16 == 0 && TS_OFF_PRE13 % 8 == 0, "shared-memory layout of the transposed scan");
+
+// per-column populations (t & 7 == c, one byte each) of the local-index range [t0, t1)
+__device__ __forceinline__ unsigned long long col_counts8(int t0, int t1) {
+    unsigned long long r = 0ull;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const int f = t0 + ((c - t0) & 7);
+        const int n = f < t1 ? (t1 - f + 7) >> 3 : 0;
+        r |= (unsigned long long)n << (8 * c);
+    }
+    return r;
+}
 template <bool MASKS>
 __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffers B, int gated, const float4* __restrict__ pos,
                                                         int ncand_cap, int umax, int tbl_cap) {
@@ -241,10 +256,14 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     unsigned short* own_first = reinterpret_cast<unsigned short*>(smraw + ts_off + TS_OFF_OWNF);   // [TS_OC + 1] first thread of own cell oc
     unsigned short* task_base = own_first + TS_OC + 2;               // [TS_OC + 1] chunks of 32 candidates before own cell oc
     unsigned short* pbase = task_base + TS_OC + 2;                   // [TS_OC + 1] first hit-word index of own cell oc (even)
-    unsigned short* pref = pbase + TS_OC + 2;                        // [TS_OC][28] candidates before stencil cell sc of own cell oc
+    unsigned short* nchs = pbase + TS_OC + 2;                        // [TS_OC] direct form: chunks of own cell oc (column-sorted enumeration)
+    unsigned short* cbase = nchs + TS_OC + 2;                        // [TS_OC + 1] direct form: chunks before own cell oc
+    unsigned short* pref = cbase + TS_OC + 2;                        // [TS_OC][28] candidates before stencil cell sc of own cell oc
+    unsigned char* ctab = smraw + ts_off + TS_OFF_CTAB;              // [warps][28][8] direct form: candidates of column c before stencil cell a
+    unsigned long long* pre13 = reinterpret_cast<unsigned long long*>(smraw + ts_off + TS_OFF_PRE13);   // [TS_OC] per-column candidates before the own cell
     unsigned short* pcs = reinterpret_cast<unsigned short*>(smraw + ts_off + TS_OFF_PCS);   // [8][MD_TB] column populations of pass B
     __shared__ int sh_scan[33];
-    __shared__ int s_tsok;
+    __shared__ int s_tsok, s_direct;
     __shared__ int s_flags, s_err, s_own_base, s_U;
 
     const int b = blockIdx.x, tid = threadIdx.x;
@@ -506,6 +525,10 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     //     (owner, 32 candidates).  Each owner thread then turns its hit words into the column buckets of pass B.  The band
     //     decision (S:Q6) is taken in place, in fp64 on the raw coordinates, by the lanes that meet it.
     bool tdone = false;
+    bool tdirect = false;                   // direct form: rows emitted from the hit words (8b), no buckets
+    int d_myhw = 0, d_nch = 0;              // this thread's hit words: hitw[j * TS_ROW + d_myhw], j < d_nch
+    unsigned long long d_rem = 0ull;        // neighbours per column, one byte each
+    const unsigned short* d_cl = nullptr;   // candidate list of the thread's own cell: local index of (chunk j, lane l) at [j * 32 + l]
     if (MASKS && !maywrap && nownc <= TS_OC) {
         const int lane = tid & 31, wid = tid >> 5;
         if (tid == 0) s_tsok = 1;
@@ -515,12 +538,24 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
           xown[tid] = xo.x; xown[MD_TB + 2 + tid] = xo.y; xown[2 * (MD_TB + 2) + tid] = xo.z; }
         if (tid < nownc) {
             int sum = 0;
+            unsigned long long cc8 = 0ull, p13 = 0ull;          // per-column candidate counts, one byte each (direct form)
             for (int sc = 0; sc < 27; ++sc) {
                 const int u = reinterpret_cast<const short*>(cand)[tid * 27 + sc];
                 pref[tid * 28 + sc] = (unsigned short)sum;
-                if (u >= 0) sum += ubase[u + 1] - ubase[u];
+                if (sc == 13) p13 = cc8;
+                if (u >= 0) {
+                    const int t0 = ubase[u], t1 = ubase[u + 1];
+                    sum += t1 - t0;
+                    cc8 += col_counts8(t0, t1);
+                }
             }
             pref[tid * 28 + 27] = (unsigned short)sum;
+            int mx = 0;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) mx = max(mx, (int)((cc8 >> (8 * c)) & 255ull));
+            // a column holds at most total / 8 + 27 candidates: no byte of cc8 overflows while total <= 32 TS_CB
+            nchs[tid] = (unsigned short)(sum <= 32 * TS_CB ? (mx + 3) >> 2 : 0xffff);
+            pre13[tid] = p13;
         }
         __syncthreads();
         if (tid == 0) {
@@ -538,9 +573,137 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
             // the candidate lists (local index of candidate k of own cell oc) live in this block's part of the mask scratch
             if ((size_t)tb * 32 > (size_t)2 * 27 * P.mask_words * MD_TB || tb > 65535) s_tsok = 0;
             s_U = mx;       // most chunks of any own cell (s_U is free after step 3)
+            // direct form: every own cell fits one pass of hit words in its column-sorted enumeration
+            int direct = P.build_direct, cb = 0;
+            for (int oc = 0; oc < nownc; ++oc) {
+                cbase[oc] = (unsigned short)cb;
+                const int n = nchs[oc];
+                if (n > TS_CB) direct = 0; else cb += n;
+            }
+            if ((size_t)cb * 32 > (size_t)2 * 27 * P.mask_words * MD_TB) direct = 0;
+            s_direct = direct;
         }
         __syncthreads();
-        if (s_tsok) {
+        if (s_tsok && s_direct) {
+            // DIRECT form.  The candidates of an own cell's stencil are enumerated BY BANK COLUMN: lane l of chunk j holds
+            // candidate 4 j + (l & 3) of column l >> 2 (column = local index & 7), in stencil order within the column.  A hit
+            // word then holds one nibble per column; transposed per owner (below) the nibbles of a column form a bit string
+            // whose bit r is "candidate r of the column is a neighbour", and the scheduled emission of 8b takes "the next
+            // neighbour of column c" with one find-first-set: no buckets in scratch memory, no decode pass.  One warp takes a
+            // whole own cell, chunk after chunk.
+            tdone = true;
+            tdirect = true;
+            unsigned short* __restrict__ clist = reinterpret_cast<unsigned short*>(B.cmask + (size_t)b * 27 * P.mask_words * MD_TB);
+            const short* __restrict__ cand_s = reinterpret_cast<const short*>(cand);
+            const float rv2 = P.rv2, bandv = P.band_rv;
+            const float* __restrict__ xox = xown, * __restrict__ xoy = xown + MD_TB + 2, * __restrict__ xoz = xown + 2 * (MD_TB + 2);
+            unsigned char* __restrict__ tab = ctab + wid * (28 * 8);       // tab[a * 8 + c]
+            for (int oc = wid; oc < nownc; oc += MD_TB / 32) {
+                const int nch = nchs[oc];
+                const int o0 = own_first[oc], o1 = own_first[oc + 1];
+                const int c = lane >> 2, q = lane & 3;
+                // per-column prefix table of the 27 stencil cells: lane a takes cell a, an exclusive warp scan of the packed
+                // byte counts (no byte overflows: see nchs), one 64-bit store per cell
+                int ct0 = 0, cus = 0;
+                unsigned long long cc8 = 0ull;
+                if (lane < 27) {
+                    const int u = cand_s[oc * 27 + lane];
+                    if (u >= 0) { ct0 = ubase[u]; cc8 = col_counts8(ct0, ubase[u + 1]); cus = ustart[u] - ct0; }
+                }
+                unsigned long long inc = cc8;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const unsigned long long y = __shfl_up_sync(0xffffffffu, inc, d);
+                    if (lane >= d) inc += y;
+                }
+                __syncwarp();                                       // the table of the previous own cell is no longer read
+                if (lane < 28) *reinterpret_cast<unsigned long long*>(tab + lane * 8) = inc - cc8;
+                __syncwarp();
+                unsigned int* __restrict__ hw0 = hitw + (int)pbase[oc] - (o0 & ~1);
+                unsigned short* __restrict__ clo = clist + (size_t)cbase[oc] * 32;
+                const int ncol = tab[27 * 8 + c];                   // candidates of the lane's column
+                for (int j = 0; j < nch; ++j) {
+                    const int r = 4 * j + q;
+                    const bool valid = r < ncol;
+                    int a = 0;                                       // last cell whose prefix is <= r
+#pragma unroll
+                    for (int st = 16; st > 0; st >>= 1)
+                        if (a + st <= 26 && (int)tab[(a + st) * 8 + c] <= r) a += st;
+                    // the cell's first local index and slot offset come from the lane that holds cell a
+                    const int t0 = __shfl_sync(0xffffffffu, ct0, a), usl = __shfl_sync(0xffffffffu, cus, a);
+                    const int t = t0 + ((c - t0) & 7) + 8 * (r - (int)tab[a * 8 + c]);
+                    const int slot = valid ? usl + t : 0;
+                    float4 xj = make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
+                    if (valid) {
+                        xj = load_pos(slot);
+                        clo[j * 32 + lane] = (unsigned short)t;
+                    }
+                    unsigned int* __restrict__ hw = hw0 + j * TS_ROW;      // hw[o]: word of owner thread o
+                    float bmin = 3.0e38f;
+                    const float2 nxjx = make_float2(-xj.x, -xj.x), nxjy = make_float2(-xj.y, -xj.y), nxjz = make_float2(-xj.z, -xj.z);
+                    const float2 nrv2 = make_float2(-rv2, -rv2);
+#pragma unroll 2
+                    for (int o = o0 & ~1; o < o1; o += 2) {
+                        const float2 ox = *reinterpret_cast<const float2*>(xox + o), oy = *reinterpret_cast<const float2*>(xoy + o),
+                                     oz = *reinterpret_cast<const float2*>(xoz + o);
+                        const float2 ddx = __fadd2_rn(ox, nxjx), ddy = __fadd2_rn(oy, nxjy), ddz = __fadd2_rn(oz, nxjz);
+                        const float2 d2 = __ffma2_rn(ddz, ddz, __ffma2_rn(ddy, ddy, __fmul2_rn(ddx, ddx)));
+                        const float2 tt = __fadd2_rn(d2, nrv2);
+                        bmin = fminf(fminf(bmin, fabsf(tt.x)), fabsf(tt.y));
+                        const unsigned int wa = __ballot_sync(0xffffffffu, tt.x < 0.0f);
+                        const unsigned int wb = __ballot_sync(0xffffffffu, tt.y < 0.0f);
+                        if (lane == 0) *reinterpret_cast<uint2*>(hw + o) = make_uint2(wa, wb);   // padded layout: always in range
+                    }
+                    if (__any_sync(0xffffffffu, bmin < bandv)) {    // rare: a pair inside the band -> fp64 on the raw coordinates (S:Q6)
+                        for (int o = o0; o < o1; ++o) {
+                            const float ddx = xj.x - xox[o], ddy = xj.y - xoy[o], ddz = xj.z - xoz[o];
+                            const float tt = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)) - rv2;
+                            bool in = tt < 0.0f;
+                            if (fabsf(tt) < bandv) in = inside_fp64(__ldg(pos + i0 + o), __ldg(pos + slot), P.dLx, P.dLy, P.dLz, P.rv2d);
+                            const unsigned int word = __ballot_sync(0xffffffffu, in);
+                            if (lane == 0) hw[o] = word;
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+            if (live) {
+                d_nch = nchs[myoc];
+                d_myhw = (int)pbase[myoc] + tid - ((int)own_first[myoc] & ~1);
+                d_cl = clist + (size_t)cbase[myoc] * 32;
+                unsigned int* myw = hitw + d_myhw;
+                {   // the particle itself is a hit of its own column: clear it
+                    const int cme = me & 7;
+                    const int t0 = ubase[cand_s[myoc * 27 + 13]];
+                    const int f = t0 + ((cme - t0) & 7);
+                    const int rs = (int)((pre13[myoc] >> (8 * cme)) & 255ull) + ((me - f) >> 3);
+                    myw[(rs >> 2) * TS_ROW] &= ~(1u << (cme * 4 + (rs & 3)));
+                }
+                // transpose, in place, eight words at a time: word (8 g + c) becomes the bit string of column c over the chunks
+                // 8 g .. 8 g + 7 (bit 4 jj + q = candidate 4 (8 g + jj) + q of the column)
+                unsigned long long rem = 0ull;
+                for (int g = 0; 8 * g < d_nch; ++g) {
+                    unsigned int x[8];
+#pragma unroll
+                    for (int jj = 0; jj < 8; ++jj) x[jj] = 8 * g + jj < d_nch ? myw[(8 * g + jj) * TS_ROW] : 0u;
+                    // 8 x 8 nibble transpose: three butterfly stages (16-, 8-, 4-bit blocks)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) { const unsigned int t = ((x[i] >> 16) ^ x[i + 4]) & 0x0000ffffu; x[i + 4] ^= t; x[i] ^= t << 16; }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) if (!(i & 2)) { const unsigned int t = ((x[i] >> 8) ^ x[i + 2]) & 0x00ff00ffu; x[i + 2] ^= t; x[i] ^= t << 8; }
+#pragma unroll
+                    for (int i = 0; i < 8; i += 2) { const unsigned int t = ((x[i] >> 4) ^ x[i + 1]) & 0x0f0f0f0fu; x[i + 1] ^= t; x[i] ^= t << 4; }
+#pragma unroll
+                    for (int cc = 0; cc < 8; ++cc) {
+                        myw[(8 * g + cc) * TS_ROW] = x[cc];
+                        rem += (unsigned long long)__popc(x[cc]) << (8 * cc);
+                    }
+                }
+                d_rem = rem;
+#pragma unroll
+                for (int cc = 0; cc < 8; ++cc) cnt += (int)((rem >> (8 * cc)) & 255ull);
+            }
+        } else if (s_tsok) {
             tdone = true;
             const int ntask = task_base[nownc], maxch = s_U;
             unsigned short* __restrict__ clist = reinterpret_cast<unsigned short*>(B.cmask + (size_t)b * 27 * P.mask_words * MD_TB);
@@ -781,7 +944,50 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
         unsigned long long pops = 0ull, rem8 = 0ull;
         int c2e = c2;                                      // entries to emit (0 after a bucket overflow)
         int lo_e = 0;                                      // neighbours with a lower slot, counted while emitting
-        if (c2 > 0 && near_first) {
+        if (c2 > 0 && tdirect) {
+            // direct form: the schedule (column (k + p) mod 8 while it has one, else the fullest) takes "the next neighbour of
+            // column c" = the lowest set bit of the column's bit string (three 32-bit words per column, transposed above)
+            unsigned int* myw = hitw + d_myhw;
+            unsigned long long rem = d_rem;
+            const int ng = (d_nch + 7) >> 3;
+            for (int k0 = 0; k0 < c2; k0 += 4) {
+                int src[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int k = k0 + q;
+                    src[q] = -1;
+                    if (k < c2) {
+                        int c = (k + tid) & 7;
+                        int r = (int)((rem >> (8 * c)) & 255ull);
+                        if (r == 0) {                          // preferred column exhausted: take the fullest one
+#pragma unroll
+                            for (int cc = 0; cc < 8; ++cc) { const int v = (int)((rem >> (8 * cc)) & 255ull); if (v > r) { r = v; c = cc; } }
+                        }
+                        rem -= 1ull << (8 * c);
+                        unsigned int* pw = myw + c * TS_ROW;
+                        unsigned int bits = pw[0];
+                        int g = 0;
+                        if (bits == 0u && ng > 1) { pw += 8 * TS_ROW; bits = pw[0]; g = 1; }
+                        if (bits == 0u && ng > 2) { pw += 8 * TS_ROW; bits = pw[0]; g = 2; }
+                        if (bits) {                            // (always: the column has r > 0 neighbours left)
+                            const int bit = __ffs(bits) - 1;
+                            pw[0] = bits & (bits - 1u);
+                            const int rr = 32 * g + bit;        // rank of the candidate in its column
+                            src[q] = (rr >> 2) * 32 + c * 4 + (rr & 3);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const unsigned int tq = src[q] >= 0 ? (unsigned int)d_cl[src[q]] : 0x7fffffffu;
+                    lo_e += (int)tq < me ? 1 : 0;
+                    w[q] = src[q] >= 0 ? (tq << rsh) : dummy;
+                }
+                rowb[(size_t)(k0 >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+            }
+            lo_cnt = lo_e;
+            c2e = 0;                                       // nothing left for the scheduled emission below
+        } else if (c2 > 0 && near_first) {
             // two sweeps over the scan-order list: near neighbours first, then the rest (careful-path lists carry no flags: all "rest")
             int kout = 0;
             for (int pass = 0; pass < 2; ++pass) {
@@ -917,6 +1123,14 @@ static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, in
         um = want < um ? want : um;
         nc = 2 * um;
         region = nc > (27 * MD_TB + 1) / 2 ? nc : (27 * MD_TB + 1) / 2;
+    }
+    else {
+        // dense cells: the distinct-cell tables need no more than the sparse sizing gives (4x the cells of a compact block);
+        // the transposed scan wants the shared memory (four resident blocks)
+        const double side = cbrt(own) + 2.0;
+        int want = 256;
+        while (want < 4.0 * side * side * side && want < MD_UMAX) want <<= 1;
+        um = want < um ? want : um;
     }
     *ncand_cap = nc;
     *umax = um;

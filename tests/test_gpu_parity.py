@@ -191,6 +191,30 @@ def test_options_row_schedule_and_unknown(MD, oracle):
     s.close()
 
 
+def test_option_build_direct_same_rows(MD, oracle):
+    """MD_OPT_BUILD_DIRECT: the dense-cell Verlet build emits its scheduled rows straight from the hit words of the
+    transposed scan (1, default) or through column buckets in scratch memory (0).  Same pair set, and the SAME row order:
+    the VERTEX forces agree bit for bit.  Run on a melted fluid (ragged cells) and at r_c = 4.0 (blocks whose own cells
+    exceed one pass of hit words take the bucket form under either setting)."""
+    for rcut, melt in ((2.5, 150), (4.0, 0)):
+        w = W.lj_fluid(2 ** 14, rcut=rcut)
+        s = MD.from_workload(w, order="hilbert")
+        s.build_cells(); s.build_verlet(); s.forces("vertex", "smem")
+        if melt:
+            s.integrate(w.dt, melt, "vertex", "smem")
+        out = []
+        for direct in (1, 0, 1):
+            s.set_option("build_direct", direct)
+            s.build_cells(); s.build_verlet()
+            if direct == 0:
+                assert_pairs(s, oracle, s.in_id_order(s.pos), w.box, w.rcut, w.skin)
+            s.forces("vertex", "smem")
+            out.append((s.in_id_order(s.force).copy(), s.stats()["n_edges"]))
+        assert out[0][1] == out[1][1] == out[2][1]
+        assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][0], out[2][0])
+        s.close()
+
+
 def test_error_paths(MD):
     from paper_1401_4350_b200 import MDError
     w = W.config("C1")
