@@ -948,40 +948,52 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
             // direct form: the schedule (column (k + p) mod 8 while it has one, else the fullest) takes "the next neighbour of
             // column c" = the lowest set bit of the column's bit string (three 32-bit words per column, transposed above)
             unsigned int* myw = hitw + d_myhw;
-            unsigned long long rem = d_rem;
+            unsigned int rlo = (unsigned int)d_rem, rhi = (unsigned int)(d_rem >> 32);   // neighbours left per column, one byte each
             const int ng = (d_nch + 7) >> 3;
-            for (int k0 = 0; k0 < c2; k0 += 4) {
+            // one scheduled pick: returns the position of the neighbour in the candidate list
+            auto pick = [&](int k) {
+                int c = (k + tid) & 7;
+                if ((__byte_perm(rlo, rhi, c) & 0xffu) == 0u) {            // preferred column exhausted: the fullest one (first of equals)
+                    unsigned int m = __vmaxu4(rlo, rhi);
+                    m = __vmaxu4(m, m >> 16);
+                    m = max(m & 0xffu, (m >> 8) & 0xffu) * 0x01010101u;
+                    const unsigned int elo = __vcmpeq4(rlo, m), ehi = __vcmpeq4(rhi, m);
+                    c = elo ? (__ffs(elo) - 1) >> 3 : 4 + ((__ffs(ehi) - 1) >> 3);
+                }
+                const unsigned int dec = 1u << (8 * (c & 3));
+                if (c < 4) rlo -= dec; else rhi -= dec;
+                unsigned int* pw = myw + c * TS_ROW;
+                unsigned int bits = pw[0];
+                int g = 0;
+                if (bits == 0u && ng > 1) { pw += 8 * TS_ROW; bits = pw[0]; g = 1; }
+                if (bits == 0u && ng > 2) { pw += 8 * TS_ROW; bits = pw[0]; g = 2; }
+                const int bit = __ffs(bits) - 1;                            // (bits != 0: the column has neighbours left)
+                pw[0] = bits & (bits - 1u);
+                const int rr = 32 * g + bit;                                // rank of the candidate in its column
+                return (rr >> 2) * 32 + c * 4 + (rr & 3);
+            };
+            int k0 = 0;
+            for (; k0 + 4 <= c2; k0 += 4) {
                 int src[4];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const int k = k0 + q;
-                    src[q] = -1;
-                    if (k < c2) {
-                        int c = (k + tid) & 7;
-                        int r = (int)((rem >> (8 * c)) & 255ull);
-                        if (r == 0) {                          // preferred column exhausted: take the fullest one
-#pragma unroll
-                            for (int cc = 0; cc < 8; ++cc) { const int v = (int)((rem >> (8 * cc)) & 255ull); if (v > r) { r = v; c = cc; } }
-                        }
-                        rem -= 1ull << (8 * c);
-                        unsigned int* pw = myw + c * TS_ROW;
-                        unsigned int bits = pw[0];
-                        int g = 0;
-                        if (bits == 0u && ng > 1) { pw += 8 * TS_ROW; bits = pw[0]; g = 1; }
-                        if (bits == 0u && ng > 2) { pw += 8 * TS_ROW; bits = pw[0]; g = 2; }
-                        if (bits) {                            // (always: the column has r > 0 neighbours left)
-                            const int bit = __ffs(bits) - 1;
-                            pw[0] = bits & (bits - 1u);
-                            const int rr = 32 * g + bit;        // rank of the candidate in its column
-                            src[q] = (rr >> 2) * 32 + c * 4 + (rr & 3);
-                        }
-                    }
-                }
+                for (int q = 0; q < 4; ++q) src[q] = pick(k0 + q);
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const unsigned int tq = src[q] >= 0 ? (unsigned int)d_cl[src[q]] : 0x7fffffffu;
+                    const unsigned int tq = d_cl[src[q]];
                     lo_e += (int)tq < me ? 1 : 0;
-                    w[q] = src[q] >= 0 ? (tq << rsh) : dummy;
+                    w[q] = tq << rsh;
+                }
+                rowb[(size_t)(k0 >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
+            }
+            if (k0 < c2) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    w[q] = dummy;
+                    if (k0 + q < c2) {
+                        const unsigned int tq = d_cl[pick(k0 + q)];
+                        lo_e += (int)tq < me ? 1 : 0;
+                        w[q] = tq << rsh;
+                    }
                 }
                 rowb[(size_t)(k0 >> 2) * MD_TB] = make_uint2(w[0] | (w[1] << 16), w[2] | (w[3] << 16));
             }
