@@ -536,52 +536,65 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
         if (tid == 0) own_first[nownc] = (unsigned short)(i1 - i0);
         { const float4 xo = live ? load_pos(i) : make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
           xown[tid] = xo.x; xown[MD_TB + 2 + tid] = xo.y; xown[2 * (MD_TB + 2) + tid] = xo.z; }
-        if (tid < nownc) {
-            int sum = 0;
-            unsigned long long cc8 = 0ull, p13 = 0ull;          // per-column candidate counts, one byte each (direct form)
-            for (int sc = 0; sc < 27; ++sc) {
-                const int u = reinterpret_cast<const short*>(cand)[tid * 27 + sc];
-                pref[tid * 28 + sc] = (unsigned short)sum;
-                if (sc == 13) p13 = cc8;
-                if (u >= 0) {
-                    const int t0 = ubase[u], t1 = ubase[u + 1];
-                    sum += t1 - t0;
-                    cc8 += col_counts8(t0, t1);
-                }
+        // per own cell: candidates before every stencil cell (pref), per-column totals -> chunks of the direct form (nchs),
+        // per-column candidates before the own cell itself (pre13).  One warp per own cell, lane a = stencil cell a.
+        for (int oc = wid; oc < nownc; oc += MD_TB / 32) {
+            int n = 0;
+            unsigned long long cc8 = 0ull;                      // per-column candidate counts of the lane's cell, one byte each
+            if (lane < 27) {
+                const int u = reinterpret_cast<const short*>(cand)[oc * 27 + lane];
+                if (u >= 0) { const int t0 = ubase[u], t1 = ubase[u + 1]; n = t1 - t0; cc8 = col_counts8(t0, t1); }
             }
-            pref[tid * 28 + 27] = (unsigned short)sum;
-            int mx = 0;
+            int ninc = n;
+            unsigned long long cinc = cc8;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) mx = max(mx, (int)((cc8 >> (8 * c)) & 255ull));
-            // a column holds at most total / 8 + 27 candidates: no byte of cc8 overflows while total <= 32 TS_CB
-            nchs[tid] = (unsigned short)(sum <= 32 * TS_CB ? (mx + 3) >> 2 : 0xffff);
-            pre13[tid] = p13;
+            for (int d = 1; d < 32; d <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, ninc, d);
+                const unsigned long long z = __shfl_up_sync(0xffffffffu, cinc, d);
+                if (lane >= d) { ninc += y; cinc += z; }
+            }
+            if (lane < 28) pref[oc * 28 + lane] = (unsigned short)min(ninc - n, 65535);
+            if (lane == 13) pre13[oc] = cinc - cc8;
+            if (lane == 27) {
+                int mx = 0;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) mx = max(mx, (int)((cinc >> (8 * c)) & 255ull));
+                // a column holds at most total / 8 + 27 candidates: no byte overflows while total <= 32 TS_CB
+                nchs[oc] = (unsigned short)(ninc <= 32 * TS_CB ? (mx + 3) >> 2 : 0xffff);
+            }
         }
         __syncthreads();
-        if (tid == 0) {
-            int tb = 0, mx = 0, pb = 0;
-            for (int oc = 0; oc < nownc; ++oc) {
-                task_base[oc] = (unsigned short)tb;
-                pbase[oc] = (unsigned short)pb;
-                pb += (((int)own_first[oc + 1] + 1) & ~1) - ((int)own_first[oc] & ~1);      // owner pairs of the cell, from an even thread
-
-                const int ch = ((int)pref[oc * 28 + 27] + 31) >> 5;
-                tb += ch;
-                mx = max(mx, ch);
+        if (wid == 0) {
+            // exclusive prefixes over the own cells (nownc <= 32: lane = own cell): chunks of the bucket form (task_base), owner
+            // pairs from an even thread (pbase), chunks of the direct form (cbase)
+            const bool in = lane < nownc;
+            const int ch = in ? ((int)pref[lane * 28 + 27] + 31) >> 5 : 0;
+            const int pw2 = in ? (((int)own_first[lane + 1] + 1) & ~1) - ((int)own_first[lane] & ~1) : 0;
+            const int nd = in ? (int)nchs[lane] : 0;
+            const bool dok = nd <= TS_CB;
+            int a1 = ch, a2 = pw2, a3 = dok ? nd : 0;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int y1 = __shfl_up_sync(0xffffffffu, a1, d), y2 = __shfl_up_sync(0xffffffffu, a2, d), y3 = __shfl_up_sync(0xffffffffu, a3, d);
+                if (lane >= d) { a1 += y1; a2 += y2; a3 += y3; }
             }
-            task_base[nownc] = (unsigned short)tb;
-            // the candidate lists (local index of candidate k of own cell oc) live in this block's part of the mask scratch
-            if ((size_t)tb * 32 > (size_t)2 * 27 * P.mask_words * MD_TB || tb > 65535) s_tsok = 0;
-            s_U = mx;       // most chunks of any own cell (s_U is free after step 3)
-            // direct form: every own cell fits one pass of hit words in its column-sorted enumeration
-            int direct = P.build_direct, cb = 0;
-            for (int oc = 0; oc < nownc; ++oc) {
-                cbase[oc] = (unsigned short)cb;
-                const int n = nchs[oc];
-                if (n > TS_CB) direct = 0; else cb += n;
+            if (in) {
+                task_base[lane] = (unsigned short)min(a1 - ch, 65535);
+                pbase[lane] = (unsigned short)(a2 - pw2);
+                cbase[lane] = (unsigned short)(a3 - (dok ? nd : 0));
             }
-            if ((size_t)cb * 32 > (size_t)2 * 27 * P.mask_words * MD_TB) direct = 0;
-            s_direct = direct;
+            const int tb = __shfl_sync(0xffffffffu, a1, 31), cb = __shfl_sync(0xffffffffu, a3, 31);
+            const int mx = __reduce_max_sync(0xffffffffu, ch);
+            const bool alld = __all_sync(0xffffffffu, dok);
+            if (lane == 0) {
+                task_base[nownc] = (unsigned short)min(tb, 65535);
+                // the candidate lists (local index of candidate k of own cell oc) live in this block's part of the mask scratch
+                const size_t capu16 = (size_t)2 * 27 * P.mask_words * MD_TB;
+                if ((size_t)tb * 32 > capu16 || tb > 65535) s_tsok = 0;
+                s_U = mx;       // most chunks of any own cell (s_U is free after step 3)
+                // direct form: every own cell fits one pass of hit words in its column-sorted enumeration
+                s_direct = (P.build_direct && alld && (size_t)cb * 32 <= capu16) ? 1 : 0;
+            }
         }
         __syncthreads();
         if (s_tsok && s_direct) {
