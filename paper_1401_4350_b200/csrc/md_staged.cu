@@ -635,16 +635,16 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
                 unsigned int* __restrict__ hw0 = hitw + (int)pbase[oc] - (o0 & ~1);
                 unsigned short* __restrict__ clo = clist + (size_t)cbase[oc] * 32;
                 const int ncol = tab[27 * 8 + c];                   // candidates of the lane's column
+                // the lane's rank grows by 4 per chunk: it walks the cells of its column forwards (a = last cell whose
+                // prefix pa is <= r, pn = prefix of the next cell)
+                int a = 0, pa = 0, pn = tab[8 + c];
                 for (int j = 0; j < nch; ++j) {
                     const int r = 4 * j + q;
                     const bool valid = r < ncol;
-                    int a = 0;                                       // last cell whose prefix is <= r
-#pragma unroll
-                    for (int st = 16; st > 0; st >>= 1)
-                        if (a + st <= 26 && (int)tab[(a + st) * 8 + c] <= r) a += st;
+                    while (a < 26 && pn <= r) { ++a; pa = pn; pn = tab[(a + 1) * 8 + c]; }
                     // the cell's first local index and slot offset come from the lane that holds cell a
                     const int t0 = __shfl_sync(0xffffffffu, ct0, a), usl = __shfl_sync(0xffffffffu, cus, a);
-                    const int t = t0 + ((c - t0) & 7) + 8 * (r - (int)tab[a * 8 + c]);
+                    const int t = t0 + ((c - t0) & 7) + 8 * (r - pa);
                     const int slot = valid ? usl + t : 0;
                     float4 xj = make_float4(DUMMY_COORD, DUMMY_COORD, DUMMY_COORD, 0.f);
                     if (valid) {
