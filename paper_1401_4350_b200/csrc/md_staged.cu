@@ -652,6 +652,7 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
                         clo[j * 32 + lane] = (unsigned short)t;
                     }
                     unsigned int* __restrict__ hw = hw0 + j * TS_ROW;      // hw[o]: word of owner thread o
+                    unsigned int hp = smem_u32(hw + (o0 & ~1));             // running shared-memory address of the pair's two words
                     float bmin = 3.0e38f;
                     const float2 nxjx = make_float2(-xj.x, -xj.x), nxjy = make_float2(-xj.y, -xj.y), nxjz = make_float2(-xj.z, -xj.z);
                     const float2 nrv2 = make_float2(-rv2, -rv2);
@@ -665,7 +666,8 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
                         bmin = fminf(fminf(bmin, fabsf(tt.x)), fabsf(tt.y));
                         const unsigned int wa = __ballot_sync(0xffffffffu, tt.x < 0.0f);
                         const unsigned int wb = __ballot_sync(0xffffffffu, tt.y < 0.0f);
-                        if (lane == 0) *reinterpret_cast<uint2*>(hw + o) = make_uint2(wa, wb);   // padded layout: always in range
+                        if (lane == 0) asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(hp), "r"(wa), "r"(wb) : "memory");   // padded layout: always in range
+                        hp += 8u;
                     }
                     if (__any_sync(0xffffffffu, bmin < bandv)) {    // rare: a pair inside the band -> fp64 on the raw coordinates (S:Q6)
                         for (int o = o0; o < o1; ++o) {
