@@ -969,11 +969,14 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
             auto pick = [&](int k) {
                 int c = (k + tid) & 7;
                 if ((__byte_perm(rlo, rhi, c) & 0xffu) == 0u) {            // preferred column exhausted: the fullest one (first of equals)
-                    unsigned int m = __vmaxu4(rlo, rhi);
-                    m = __vmaxu4(m, m >> 16);
-                    m = max(m & 0xffu, (m >> 8) & 0xffu) * 0x01010101u;
-                    const unsigned int elo = __vcmpeq4(rlo, m), ehi = __vcmpeq4(rhi, m);
-                    c = elo ? (__ffs(elo) - 1) >> 3 : 4 + ((__ffs(ehi) - 1) >> 3);
+                    // key = count * 8 + (7 - column): the largest key is the fullest column, the lowest column among equals
+                    unsigned int best = 0u;
+#pragma unroll
+                    for (int cc = 0; cc < 8; ++cc) {
+                        const unsigned int bc = __byte_perm(cc < 4 ? rlo : rhi, 0u, 0x4440u | (unsigned int)(cc & 3));
+                        best = max(best, bc * 8u + (unsigned int)(7 - cc));
+                    }
+                    c = 7 - (int)(best & 7u);
                 }
                 const unsigned int dec = 1u << (8 * (c & 3));
                 if (c < 4) rlo -= dec; else rhi -= dec;
