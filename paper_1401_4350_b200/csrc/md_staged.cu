@@ -470,15 +470,19 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     if (tid == 0) s_flags = 0;   // from here on: bit a = axis a violates the margin criterion
     __syncthreads();
     if (wrap_axes) {
+        // tested per staged CELL (its coordinate interval, widened by 1 % of a cell for the rounding of the binning)
+        // instead of per staged position: a superset of the positions, 25x fewer tests
         int bad = 0;
-        for (int u = tid >> 5; u < U; u += MD_TB / 32) {
-            const int s0 = ustart[u], len = ubase[u + 1] - ubase[u];
-            for (int k = tid & 31; k < len; k += 32) {
-                const float4 x = pos[s0 + k];
-                if ((wrap_axes & 1) && fabsf(x.x - P.hLx) <= P.shift_margin) bad |= 1;
-                if ((wrap_axes & 2) && fabsf(x.y - P.hLy) <= P.shift_margin) bad |= 2;
-                if ((wrap_axes & 4) && fabsf(x.z - P.hLz) <= P.shift_margin) bad |= 4;
-            }
+        for (int u = tid; u < U; u += MD_TB) {
+            const int lin = B.cell_lin[urank[u]];
+            const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
+            auto near_half = [&](int c, double cscale, float hL) {
+                const float lo = (float)(((double)c - 0.01) / cscale), hi = (float)(((double)c + 1.01) / cscale);
+                return lo <= hL + P.shift_margin && hi >= hL - P.shift_margin;
+            };
+            if ((wrap_axes & 1) && near_half(cx, P.cscale_x, P.hLx)) bad |= 1;
+            if ((wrap_axes & 2) && near_half(cy, P.cscale_y, P.hLy)) bad |= 2;
+            if ((wrap_axes & 4) && near_half(cz, P.cscale_z, P.hLz)) bad |= 4;
         }
         if (bad) atomicOr(&s_flags, bad);
     }
