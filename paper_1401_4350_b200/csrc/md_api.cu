@@ -938,14 +938,35 @@ md_status md_step_host(md_system* s, void* pos_host, void* vel_host, void* force
     const size_t bytes = 16 * (size_t)s->N;
     reset_ids(s);   // host buffers are in ORIGINAL id order
     s->shadow_valid = false;
+    // Cells and lists need the positions only: velocities (and angular momenta) are uploaded on a second stream, into free
+    // planes of the permutation scratch, while the lists are built, and enter the slot order afterwards through ids[].
+    const size_t plane_in = (size_t)s->P.ntiles * MD_TILE;
+    float4* const vel_in = s->B.tmp4 + (size_t)(s->rigid ? 12 : 6) * plane_in;
+    float4* const ang_in = s->B.tmp4 + (size_t)13 * plane_in;     // rigid bodies only (14 planes)
+    bool split = s->order != MD_ORDER_NONE;
+    if (split && !s->aux_stream && cudaStreamCreateWithFlags(&s->aux_stream, cudaStreamNonBlocking) != cudaSuccess) split = false;
+    if (split && !s->ev_in && (cudaEventCreateWithFlags(&s->ev_in, cudaEventDisableTiming) != cudaSuccess ||
+                               cudaEventCreateWithFlags(&s->ev_vel, cudaEventDisableTiming) != cudaSuccess)) split = false;
+    if (!split) cudaGetLastError();
     cudaMemcpyAsync(s->pos, pos_host, bytes, cudaMemcpyHostToDevice, s->stream);
-    cudaMemcpyAsync(s->vel, vel_host, bytes, cudaMemcpyHostToDevice, s->stream);
-    if (s->rigid) {
-        cudaMemcpyAsync(s->quat, quat_host, bytes, cudaMemcpyHostToDevice, s->stream);
-        cudaMemcpyAsync(s->angmom, angmom_host, bytes, cudaMemcpyHostToDevice, s->stream);
+    if (split) {
+        cudaEventRecord(s->ev_in, s->stream);                       // the scratch planes are free once earlier work has drained
+        cudaStreamWaitEvent(s->aux_stream, s->ev_in, 0);
+        cudaMemcpyAsync(vel_in, vel_host, bytes, cudaMemcpyHostToDevice, s->aux_stream);
+        if (s->rigid) cudaMemcpyAsync(ang_in, angmom_host, bytes, cudaMemcpyHostToDevice, s->aux_stream);
+        cudaEventRecord(s->ev_vel, s->aux_stream);
+    } else {
+        cudaMemcpyAsync(s->vel, vel_host, bytes, cudaMemcpyHostToDevice, s->stream);
+        if (s->rigid) cudaMemcpyAsync(s->angmom, angmom_host, bytes, cudaMemcpyHostToDevice, s->stream);
     }
+    if (s->rigid) cudaMemcpyAsync(s->quat, quat_host, bytes, cudaMemcpyHostToDevice, s->stream);
     if ((st = md_build_cells(s)) != MD_OK) return st;
     if ((st = md_build_verlet(s)) != MD_OK) return st;
+    if (split) {
+        cudaStreamWaitEvent(s->stream, s->ev_vel, 0);
+        md_launch_permute_in(s, vel_in, s->vel);
+        if (s->rigid) md_launch_permute_in(s, ang_in, s->angmom);
+    }
     if ((st = md_forces(s, strategy, scatter)) != MD_OK) return st;
     if (nsteps > 0 && (st = md_integrate(s, dt, nsteps, strategy, scatter)) != MD_OK) return st;
     struct { float4* dev; void* host; } outs[6] = { { s->pos, pos_host }, { s->vel, vel_host }, { s->force, force_host },
@@ -972,6 +993,8 @@ const char* md_last_error(const md_system* s) { return s ? s->errmsg : "null han
 void md_destroy(md_system* s) {
     if (!s) return;
     drop_step_graph(s);
+    if (s->ev_in) cudaEventDestroy(s->ev_in);
+    if (s->ev_vel) cudaEventDestroy(s->ev_vel);
     if (s->aux_stream) cudaStreamDestroy(s->aux_stream);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     free(s);

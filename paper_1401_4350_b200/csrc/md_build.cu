@@ -438,6 +438,15 @@ __global__ void k_unpermute(DevParams P, DevBuffers B, const float4* src, float4
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < P.N) dst[B.ids[i]] = src[i];
 }
+// dst[s] = src[ids[s]]  (original id order -> slot order)
+__global__ void k_permute_in(DevParams P, DevBuffers B, const float4* __restrict__ src, float4* __restrict__ dst) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < P.N) dst[i] = src[B.ids[i]];
+}
+void md_launch_permute_in(md_system* s, const float4* src, float4* dst) {
+    k_permute_in<<<cdiv(s->P.N, 256), 256, 0, s->stream>>>(s->P, s->B, src, dst);
+    s->launches += 1;
+}
 void md_launch_unpermute(md_system* s, const float4* src, float4* dst) {
     k_unpermute<<<cdiv(s->P.N, 256), 256, 0, s->stream>>>(s->P, s->B, src, dst);
     s->launches += 1;

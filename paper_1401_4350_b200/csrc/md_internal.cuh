@@ -171,6 +171,7 @@ struct md_system {
     int* h_cell_rank;        // host copy (built at create)
     // one velocity-Verlet step as an executable CUDA graph: kick+drift, rebuild inside a conditional IF node that the
     // device-side skin flag drives, forces, kick (md_api.cu build_step_graph)
+    cudaEvent_t ev_in, ev_vel;               // md_step_host: ordering of the velocity upload on aux_stream
     cudaGraphExec_t step_exec, multi_exec;   // one step / MD_GRAPH_STEPS steps per launch
     cudaStream_t cap_stream, aux_stream; // internal capture streams: main sequence, conditional body
     int step_strategy, step_variant, step_stage, step_nodes, multi_nodes;   // *_nodes: kernels per launch outside the IF body
@@ -199,6 +200,7 @@ void md_launch_shadow_init(md_system* s);   // fp64 copies <- bound fp32 arrays
 void md_launch_energy(md_system* s);
 void md_launch_set_cond(md_system* s, unsigned long long cond_handle);   // conditional value = rebuild flag
 void md_launch_unpermute(md_system* s, const float4* src, float4* dst);   // dst[ids[s]] = src[s]
+void md_launch_permute_in(md_system* s, const float4* src, float4* dst);  // dst[s] = src[ids[s]]
 void md_launch_iota_ids(md_system* s);                                    // ids[s] = slot_of_id[s] = s
 void md_launch_count_in_cutoff(md_system* s);                             // ctrl->n_in from the explicit edge list
 void md_staged_configure(md_system* s);                                   // per-device kernel attributes of md_staged.cu
