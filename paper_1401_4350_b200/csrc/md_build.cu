@@ -207,19 +207,32 @@ __global__ void k_gather_state(DevParams P, DevBuffers B, int gated, StateArrays
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.N) return;
     const int o = B.items[i];
-    for (int k = 0; k < S.n; ++k) B.tmp4[k * plane + i] = S.a[k][o];
-    B.ids_tmp[i] = B.ids[o];
-    B.items_tmp[i] = B.cell_of[o];
+    const int id = B.ids[o], cell = B.cell_of[o];
+    for (int k0 = 0; k0 < S.n; k0 += 4) {        // four loads in flight before the first store (the arrays may alias for the compiler)
+        float4 v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) if (k0 + q < S.n) v[q] = S.a[k0 + q][o];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) if (k0 + q < S.n) B.tmp4[(k0 + q) * plane + i] = v[q];
+    }
+    B.ids_tmp[i] = id;
+    B.items_tmp[i] = cell;
 }
 __global__ void k_commit_state(DevParams P, DevBuffers B, int gated, StateArrays S, size_t plane) {
     GATE(B, gated);
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.N) return;
-    for (int k = 0; k < S.n; ++k) S.a[k][i] = B.tmp4[k * plane + i];
-    const int id = B.ids_tmp[i];
+    const int id = B.ids_tmp[i], cell = B.items_tmp[i];
+    for (int k0 = 0; k0 < S.n; k0 += 4) {
+        float4 v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) if (k0 + q < S.n) v[q] = B.tmp4[(k0 + q) * plane + i];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) if (k0 + q < S.n) S.a[k0 + q][i] = v[q];
+    }
     B.ids[i] = id;
     B.slot_of_id[id] = i;
-    B.cell_of[i] = B.items_tmp[i];
+    B.cell_of[i] = cell;
     B.items[i] = i;   // storage order == cell order from now on
 }
 
