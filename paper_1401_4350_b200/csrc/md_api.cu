@@ -177,6 +177,8 @@ void make_cell_rank(const int nc[3], int order, std::vector<int>& rank) {
 void drop_step_graph(md_system* s) {
     if (s->step_exec) { cudaGraphExecDestroy(s->step_exec); s->step_exec = nullptr; }
     if (s->multi_exec) { cudaGraphExecDestroy(s->multi_exec); s->multi_exec = nullptr; }
+    if (s->quad_exec) { cudaGraphExecDestroy(s->quad_exec); s->quad_exec = nullptr; }
+    if (s->pair_exec) { cudaGraphExecDestroy(s->pair_exec); s->pair_exec = nullptr; }
 }
 
 md_status fail(md_system* s, md_status code, const char* msg) {
@@ -758,14 +760,18 @@ static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t 
             s->step_dt_d != dt || s->step_stage != s->stage_launch) {
             drop_step_graph(s);
             if (!build_step_graph(s, fdt, strategy, scatter, staged, seg, 1, &s->step_exec, &s->step_nodes) ||
+                !build_step_graph(s, fdt, strategy, scatter, staged, seg, 2, &s->pair_exec, &s->pair_nodes) ||
+                !build_step_graph(s, fdt, strategy, scatter, staged, seg, 4, &s->quad_exec, &s->quad_nodes) ||
                 !build_step_graph(s, fdt, strategy, scatter, staged, seg, MD_GRAPH_STEPS, &s->multi_exec, &s->multi_nodes)) s->graphs_off = true;
         }
-        if (s->step_exec && s->multi_exec) {
-            while (k0 < nsteps) {      // MD_GRAPH_STEPS steps per launch while they fit, single steps for the rest
-                const bool multi = nsteps - k0 >= MD_GRAPH_STEPS;
-                if (cudaGraphLaunch(multi ? s->multi_exec : s->step_exec, s->stream) != cudaSuccess) break;
-                k0 += multi ? MD_GRAPH_STEPS : 1;
-                s->launches += multi ? s->multi_nodes : s->step_nodes;
+        if (s->step_exec && s->pair_exec && s->quad_exec && s->multi_exec) {
+            while (k0 < nsteps) {      // MD_GRAPH_STEPS steps per launch while they fit, then 4, 2, 1 for the rest
+                const int64_t left = nsteps - k0;
+                const int reps = left >= MD_GRAPH_STEPS ? MD_GRAPH_STEPS : left >= 4 ? 4 : left >= 2 ? 2 : 1;
+                cudaGraphExec_t ex = reps == MD_GRAPH_STEPS ? s->multi_exec : reps == 4 ? s->quad_exec : reps == 2 ? s->pair_exec : s->step_exec;
+                if (cudaGraphLaunch(ex, s->stream) != cudaSuccess) break;
+                k0 += reps;
+                s->launches += reps == MD_GRAPH_STEPS ? s->multi_nodes : reps == 4 ? s->quad_nodes : reps == 2 ? s->pair_nodes : s->step_nodes;
             }
         }
     }
