@@ -134,6 +134,10 @@ typedef enum {
     MD_OPT_ROW_SCHEDULE = 3, /* staged Verlet rows: 1 (default) = entries ordered at build time by shared-memory bank column
                                so that the 128-bit gathers of the force kernels are conflict-free; 0 = scan order (a
                                cheaper build, more bank conflicts per force evaluation).  Invalidates the lists.      */
+    MD_OPT_FUSE_STEPS = 5,  /* multi-step graphs of md_integrate, staged LJ / FENE VERTEX in fp32: 1 (default) = the force kernel of
+                               an inner step applies the kicks and the drift of the next step itself (no kick+drift kernel, no
+                               force store; positions alternate between the caller's array and a scratch plane inside the
+                               graph and end in the caller's array); 0 = separate kernels.  Same arithmetic, same results. */
     MD_OPT_BUILD_DIRECT = 4 /* staged Verlet build, dense cells: 1 (default) = the scheduled rows are emitted straight from the
                                hit words of the transposed scan (candidates enumerated by bank column); 0 = through the
                                column buckets in scratch memory (the form before it).  Same rows bit for bit.

@@ -17,7 +17,7 @@ ORDER = {"none": 0, "cell": 1, "hilbert": 2}
 PRECISION = {"f32": 0, "mixed": 1}
 ARRAY = {"pos": 0, "vel": 1, "force": 2, "quat": 3, "angmom": 4, "torque": 5}
 STEP_PART = {"kick_drift": 0, "kick": 1}
-OPTION = {"stage_limit": 0, "no_graph": 1, "debug": 2, "row_schedule": 3, "build_direct": 4}
+OPTION = {"stage_limit": 0, "no_graph": 1, "debug": 2, "row_schedule": 3, "build_direct": 4, "fuse_steps": 5}
 PROBE = {"ffma": 0, "ffma2": 1, "mufu": 2, "red_v4_scatter": 3, "red_f32_scatter": 4, "red_v4_coalesced": 5,
          "red_f32_coalesced": 6}
 POT_KIND = {"lj": 0, "fene_wca": 1, "patchy": 2, "patchy_pp": 3}

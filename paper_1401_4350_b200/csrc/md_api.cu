@@ -335,6 +335,7 @@ md_status md_create(md_system** out, int64_t N, const double box[3], double rcut
     P.use_masks = ((double)N / (double)g.ncell >= 8.0) ? 1 : 0;
     P.row_schedule = 1;   // measured: masks win at 17.7 particles per cell, lists at 2.5-3
     P.build_direct = 1;
+    s->fuse_steps = true;
     P.stage_cap = (int)((224 * 1024 - 16) / (rigid ? 32 : 16)) - 1;
     P.skinf = (float)skin;
     P.shift_margin = (float)(rv + skin);
@@ -613,12 +614,24 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     size_t ndeps = 0;
     int tail_nodes = 0, main_nodes = 0;
     bool aux_open = false;
+    // Fused step tails (multi-step graphs, staged LJ / FENE VERTEX, fp32, no ghosts): the force kernel of an inner step applies
+    // the kicks and the drift of the next step itself (FuseArgs), so steps 2..reps have no kick+drift kernel and no force
+    // store.  The new positions go to the other of two position arrays (the caller's and plane 6 of the permutation
+    // scratch); with the opening kick+drift of step 1 also written across there are `reps` (even) switches per graph and
+    // the state ends in the caller's array.  The rebuild chain of a step is captured on the array that is current there.
+    float4* const pos_user = s->pos;
+    float4* const pos_alt = s->B.tmp4 + (size_t)6 * s->P.ntiles * MD_TILE;
+    const bool fuse = s->fuse_steps && reps > 1 && reps % 2 == 0 && staged && !s->rigid && s->precision != MD_PREC_MIXED &&
+                      s->P.n_active >= s->P.N;
+    float4* cur = pos_user;
     for (int rep_i = 0; rep_i < reps && ok; ++rep_i) {   // `reps` consecutive steps in one graph, one IF node each
     cudaGraphConditionalHandle handle = 0;
     GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
     GCHK(cudaGraphConditionalHandleCreate(&handle, cg, 0, cudaGraphCondAssignDefault));
     if (ok) {
-        md_launch_kick_drift(s, fdt, rep_i > 0);   // sets the device rebuild flag (S:A5); carries the previous step's closing kick
+        if (!fuse) md_launch_kick_drift(s, fdt, rep_i > 0);   // sets the device rebuild flag (S:A5); carries the previous step's closing kick
+        else if (rep_i == 0) { float4* other = cur == pos_user ? pos_alt : pos_user; md_launch_kick_drift_to(s, fdt, other); cur = other; }
+        s->pos = cur;                              // everything below reads (and the rebuild permutes) the current array
         md_launch_set_cond(s, handle);
         GCHK(cudaStreamGetCaptureInfo(main_stream, &st, nullptr, &cg, &deps, &ndeps));
     }
@@ -653,12 +666,20 @@ static bool build_step_graph(md_system* s, float fdt, int32_t strategy, int32_t 
     }
     const int64_t before_tail = s->launches;
     if (ok) {
-        ok = launch_forces_any(s, strategy, scatter, rep_i == reps - 1) == MD_OK;   // md_energy sees the last step only
+        if (fuse && rep_i < reps - 1) {
+            float4* other = cur == pos_user ? pos_alt : pos_user;
+            ok = md_launch_forces_staged(s, false, FuseArgs{ s->vel, other, fdt });
+            cur = other;
+        } else {
+            ok = launch_forces_any(s, strategy, scatter, rep_i == reps - 1) == MD_OK;   // md_energy sees the last step only
+        }
         if (rep_i == reps - 1) md_launch_kick(s, fdt);   // inner steps: fused into the next kick+drift
     }
     tail_nodes = (int)(s->launches - before_tail);
-    main_nodes += 2 + tail_nodes;   // kernels outside the conditional body
+    main_nodes += ((fuse && rep_i > 0) ? 1 : 2) + tail_nodes;   // kernels outside the conditional body
     }
+    s->pos = pos_user;
+    if (fuse && cur != pos_user) ok = false;       // (cannot happen: reps is even)
     if (aux_open) {   // a failure while the body capture was open: close it, or aux_stream stays in capture mode for good
         cudaGraph_t tmp = nullptr;
         cudaStreamEndCapture(s->aux_stream, &tmp);
@@ -861,6 +882,10 @@ md_status md_set_option(md_system* s, int32_t option, int64_t value) {
         s->P.row_schedule = value != 0 ? 1 : 0;
         drop_step_graph(s);            // the graph bakes the parameter block in
         s->lists_valid = s->staged_valid = s->legacy_valid = s->seg_valid = s->cluster_valid = false;
+        return MD_OK;
+    case MD_OPT_FUSE_STEPS:
+        s->fuse_steps = value != 0;
+        drop_step_graph(s);
         return MD_OK;
     case MD_OPT_BUILD_DIRECT:
         s->P.build_direct = value != 0 ? 1 : 0;

@@ -9,9 +9,10 @@ static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 // PRE: the closing half kick of the previous step is applied first, in this kernel (same two roundings as k_kick
 // followed by this kernel: inside a multi-step graph the separate k_kick launch and its pass over vel/force are saved).
 template <bool RIGID, bool PRE>
-__global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, float dt, float4* __restrict__ pos, float4* __restrict__ vel,
+__global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, float dt, float4* pos, float4* __restrict__ vel,
                                                     const float4* __restrict__ force, float4* __restrict__ quat,
-                                                    float4* __restrict__ angmom, const float4* __restrict__ torque) {
+                                                    float4* __restrict__ angmom, const float4* __restrict__ torque,
+                                                    float4* pos_out) {      // == pos, or the other position array (fused steps)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < P.N) {
@@ -24,7 +25,7 @@ __global__ void __launch_bounds__(256) k_kick_drift(DevParams P, DevBuffers B, f
         v.x = fmaf(hk, f.x, v.x); v.y = fmaf(hk, f.y, v.y); v.z = fmaf(hk, f.z, v.z);
         x.x = fmaf(dt, v.x, x.x); x.y = fmaf(dt, v.y, x.y); x.z = fmaf(dt, v.z, x.z);
         vel[i] = v;
-        pos[i] = x;
+        pos_out[i] = x;
         if (RIGID && !ghost) {
             float4 L = angmom[i], t = torque[i], q = quat[i];
             const float hd = 0.5f * dt;
@@ -195,6 +196,11 @@ void md_launch_set_cond(md_system* s, unsigned long long cond_handle) {
     s->launches += 1;
 }
 
+void md_launch_kick_drift_to(md_system* s, float dt, float4* pos_out) {
+    k_kick_drift<false, false><<<cdiv(s->P.N, 256), 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr, pos_out);
+    s->launches += 1;
+}
+
 void md_launch_kick_drift(md_system* s, float dt, bool pre) {
     int nb = cdiv(s->P.N, 256);
     if (s->precision == MD_PREC_MIXED) {
@@ -210,11 +216,11 @@ void md_launch_kick_drift(md_system* s, float dt, bool pre) {
         return;
     }
     if (s->rigid) {
-        if (pre) k_kick_drift<true, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
-        else k_kick_drift<true, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque);
+        if (pre) k_kick_drift<true, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque, s->pos);
+        else k_kick_drift<true, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, s->quat, s->angmom, s->torque, s->pos);
     } else {
-        if (pre) k_kick_drift<false, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
-        else k_kick_drift<false, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr);
+        if (pre) k_kick_drift<false, true><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr, s->pos);
+        else k_kick_drift<false, false><<<nb, 256, 0, s->stream>>>(s->P, s->B, dt, s->pos, s->vel, s->force, nullptr, nullptr, nullptr, s->pos);
     }
     s->launches += 1;
 }

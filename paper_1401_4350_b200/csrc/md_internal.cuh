@@ -158,6 +158,7 @@ struct md_system {
     bool cluster_valid;                // the (cluster, j) unit list of MD_SCATTER_CLUSTER describes the current build
     int stage_limit;         // MD_OPT_STAGE_LIMIT: cap on the staged launch capacity (0 = none; tests of the unstaged path)
     bool no_graph, debug;    // MD_OPT_NO_GRAPH, MD_OPT_DEBUG
+    bool fuse_steps;         // MD_OPT_FUSE_STEPS: fused step tails in the multi-step graphs (default on)
     int device, sm_count;    // the device the handle was created on and its SM count (cudaDeviceProp)
     size_t smem_optin, smem_per_sm;   // largest opt-in dynamic shared memory per block / shared memory per SM of that device
     int build_carve;         // shared-memory carveout k_build_staged was last configured with on this device (-1 = none)
@@ -216,7 +217,13 @@ void md_launch_edge_cluster(md_system* s);                                // for
 // staged path (md_staged.cu)
 void md_launch_build_staged(md_system* s, bool gated);
 void md_launch_edges_from_rows(md_system* s);     // explicit (i, j) edge list from the staged rows (export / legacy EDGE variants)
-bool md_launch_forces_staged(md_system* s, bool energy);   // VERTEX on the staged rows; energy = false: force.w is not needed
+// Fused step tail of the staged LJ / FENE VERTEX kernel (inner steps of the multi-step graphs): instead of storing the force the
+// thread applies the closing half kick of its step and the opening half kick + drift of the next one (the arithmetic of
+// k_kick_drift<false, true>, same roundings), writes the new position to ANOTHER array -- other blocks still read the old
+// ones -- and runs the skin check.  vel == nullptr: off (the force is stored).
+struct FuseArgs { float4* vel; float4* pos_next; float dt; };
+bool md_launch_forces_staged(md_system* s, bool energy, FuseArgs fuse = FuseArgs{ nullptr, nullptr, 0.0f });   // VERTEX on the staged rows; energy = false: force.w is not needed
+void md_launch_kick_drift_to(md_system* s, float dt, float4* pos_out);   // fp32, point particles: opening half kick + drift, new positions to pos_out
 size_t md_staged_smem_bytes(const md_system* s, int stage_entries);
 
 #define MD_ERRBUF(s, ...) snprintf((s)->errmsg, sizeof((s)->errmsg), __VA_ARGS__)

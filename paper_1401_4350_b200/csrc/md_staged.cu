@@ -1479,11 +1479,29 @@ __device__ __forceinline__ void lj_chunk_s(const DevParams& P, unsigned int sp32
 // NS = threads per particle (1; 2 or 4 when the staged neighbourhood is so large that only one or two 256-particle blocks
 // fit on an SM: the block then runs 512 threads, thread h * 256 + p takes the row chunks c = h mod 2 of particle p and the
 // two partial sums meet in shared memory -- twice the warps for the same shared memory).  xch = exchange buffer (NS == 2).
+// fused step tail (FuseArgs, md_internal.cuh): v += hk f twice (closing kick of this step, opening kick of the next: two
+// roundings, as k_kick followed by k_kick_drift), x' = x + dt v into the other position array, skin check (S:Q4).
+// Not inlined: its registers must not compete with the row loop of the caller.
+__device__ __noinline__ void fuse_kick_drift(float hk, float dt, float half_skin2, float4* __restrict__ vel, const float4* __restrict__ pos,
+                                             float4* __restrict__ pos_next, const float4* __restrict__ pos_ref, int* __restrict__ rebuild,
+                                             int i, float fx, float fy, float fz) {
+    float4 v = vel[i];
+    float4 x = pos[i];                                      // raw position (the staged copy may be shift-transformed)
+    const float4 r = pos_ref[i];
+    v.x = fmaf(hk, fx, v.x); v.y = fmaf(hk, fy, v.y); v.z = fmaf(hk, fz, v.z);
+    v.x = fmaf(hk, fx, v.x); v.y = fmaf(hk, fy, v.y); v.z = fmaf(hk, fz, v.z);
+    x.x = fmaf(dt, v.x, x.x); x.y = fmaf(dt, v.y, x.y); x.z = fmaf(dt, v.z, x.z);
+    vel[i] = v;
+    pos_next[i] = x;
+    const float dx = x.x - r.x, dy = x.y - r.y, dz = x.z - r.z;
+    if ((dx * dx + dy * dy + dz * dz) > half_skin2) *rebuild = 1;     // S:Q4 strict '>'
+}
+
 template <bool IMG, int SH, bool UNIT, int NS, bool ENERGY>
 __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuffers& B, const BlkInfo bi, const Stage& st, int i,
                                                bool live, int cnt, const uint2* __restrict__ rowb, uint2 pkA, uint2 pkB, uint2 pkC,
                                                uint2 pkD, float* xch, const float4* __restrict__ pos, float4* __restrict__ force,
-                                               bool bonds) {
+                                               bool bonds, const FuseArgs& fuse) {
     const int tp = threadIdx.x % MD_TB, h = threadIdx.x / MD_TB;
     const float4 xi = st.spos[bi.own_base + (live ? tp : 0)];
     const unsigned int sp = smem_u32(st.spos);
@@ -1545,7 +1563,8 @@ __device__ __forceinline__ void vertex_lj_rows(const DevParams& P, const DevBuff
         fene_vertex_s(P, B, pos, i, a.fx, a.fy, a.fz, bpe);
         pe += 0.5f * bpe;
     }
-    force[i] = make_float4(a.fx, a.fy, a.fz, pe);
+    if (fuse.vel) fuse_kick_drift(0.5f * fuse.dt * P.inv_mass, fuse.dt, P.half_skin2, fuse.vel, pos, fuse.pos_next, B.pos_ref, &B.ctrl->rebuild, i, a.fx, a.fy, a.fz);
+    else force[i] = make_float4(a.fx, a.fy, a.fz, pe);
 }
 
 // Blocks whose neighbourhood does not fit the launch (it grew past the head room since the last synchronising call)
@@ -1565,7 +1584,8 @@ __device__ __forceinline__ int staged_slot_of_local(const int2* __restrict__ seg
 template <bool RIGID, bool PP>
 __device__ __forceinline__ void vertex_rows_unstaged(const DevParams& P, const DevBuffers& B, const BlkInfo bi, int b,
                                                   const float4* __restrict__ pos, const float4* __restrict__ quat,
-                                                  float4* __restrict__ force, float4* __restrict__ torque) {
+                                                  float4* __restrict__ force, float4* __restrict__ torque,
+                                                  const FuseArgs& fuse = FuseArgs{ nullptr, nullptr, 0.0f }) {
     if (threadIdx.x >= MD_TB) return;
     const int i = b * MD_TB + threadIdx.x;
     if (i >= P.N) return;
@@ -1601,6 +1621,7 @@ __device__ __forceinline__ void vertex_rows_unstaged(const DevParams& P, const D
         fene_vertex_s(P, B, pos, i, fx, fy, fz, bpe);
         pe += 0.5f * bpe;
     }
+    if (!RIGID && fuse.vel) { fuse_kick_drift(0.5f * fuse.dt * P.inv_mass, fuse.dt, P.half_skin2, fuse.vel, pos, fuse.pos_next, B.pos_ref, &B.ctrl->rebuild, i, fx, fy, fz); return; }
     force[i] = make_float4(fx, fy, fz, pe);
     if (RIGID) torque[i] = make_float4(tx, ty, tz, 0.f);
 }
@@ -1608,7 +1629,7 @@ __device__ __forceinline__ void vertex_rows_unstaged(const DevParams& P, const D
 template <int NS, bool ENERGY>
 __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k_vertex_lj_staged(DevParams P, DevBuffers B, int stage_entries,
                                                                                   const float4* __restrict__ pos,
-                                                                                  float4* __restrict__ force) {
+                                                                                  float4* __restrict__ force, FuseArgs fuse) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int b = blockIdx.x;
     const int tp = threadIdx.x % MD_TB, h = threadIdx.x / MD_TB;
@@ -1625,7 +1646,7 @@ __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k
     const BlkInfo bi = B.blk[b];
     if (bi.M <= 0) return;                         // the build failed for this block and latched the error: never guess
     if (bi.M + 1 > stage_entries) {                // launch sized too small for this block: slow path from global memory
-        vertex_rows_unstaged<false, false>(P, B, bi, b, pos, nullptr, force, nullptr);
+        vertex_rows_unstaged<false, false>(P, B, bi, b, pos, nullptr, force, nullptr, fuse);
         return;
     }
     const Stage st = stage_issue<false>(P, B, bi, b, stage_entries, pre, pos, nullptr, smraw);
@@ -1635,7 +1656,7 @@ __global__ void __launch_bounds__(MD_TB * NS, NS == 1 ? 4 : (NS == 2 ? 2 : 1)) k
     const bool bonds = P.kind == MD_POT_FENE_WCA;
     const bool img = (bi.flags & MD_BLK_WRAP) && !(bi.flags & MD_BLK_SHIFT_OK);
     const bool unit = P.sig2 == 1.0f;
-#define LJ_ROWS(IMG_, SH_, UNIT_, EN_) vertex_lj_rows<IMG_, SH_, UNIT_, NS, EN_>(P, B, bi, st, i, live, cnt, rowb, pkA, pkB, pkC, pkD, xch, pos, force, bonds)
+#define LJ_ROWS(IMG_, SH_, UNIT_, EN_) vertex_lj_rows<IMG_, SH_, UNIT_, NS, EN_>(P, B, bi, st, i, live, cnt, rowb, pkA, pkB, pkC, pkD, xch, pos, force, bonds, fuse)
     // (the energy-free form exists for the reduced-unit loop only: sigma == 1 in every config)
     if (bi.flags & MD_BLK_SH4) {
         if (unit) { if (img) LJ_ROWS(true, 4, true, ENERGY); else LJ_ROWS(false, 4, true, ENERGY); }
@@ -1770,7 +1791,7 @@ int md_staged_threads_per_particle(const md_system* s) {
 }
 
 // VERTEX on the staged rows.  Returns false if the neighbourhood does not fit in shared memory.
-bool md_launch_forces_staged(md_system* s, bool energy) {
+bool md_launch_forces_staged(md_system* s, bool energy, FuseArgs fuse) {
     const DevParams& P = s->P;
     const int se = staged_launch_entries(s);
     const size_t smem = md_staged_smem_bytes(s, se);
@@ -1780,13 +1801,13 @@ bool md_launch_forces_staged(md_system* s, bool energy) {
     else {
         const int ns = staged_lj_ns(s, smem);
         if (ns == 4)        // one block per SM: four threads per particle (1024-thread blocks, 32 warps on the SM)
-            { if (energy) k_vertex_lj_staged<4, true><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
-              else k_vertex_lj_staged<4, false><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force); }
+            { if (energy) k_vertex_lj_staged<4, true><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force, fuse);
+              else k_vertex_lj_staged<4, false><<<P.nblk, 4 * MD_TB, smem + 72 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force, fuse); }
         else if (ns == 2)   // <= 2 blocks per SM: two threads per particle
-            { if (energy) k_vertex_lj_staged<2, true><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force);
-              else k_vertex_lj_staged<2, false><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force); }
-        else if (energy) k_vertex_lj_staged<1, true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
-        else k_vertex_lj_staged<1, false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force);
+            { if (energy) k_vertex_lj_staged<2, true><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force, fuse);
+              else k_vertex_lj_staged<2, false><<<P.nblk, 2 * MD_TB, smem + 24 * MD_TB, s->stream>>>(P, s->B, se, s->pos, s->force, fuse); }
+        else if (energy) k_vertex_lj_staged<1, true><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force, fuse);
+        else k_vertex_lj_staged<1, false><<<P.nblk, MD_TB, smem, s->stream>>>(P, s->B, se, s->pos, s->force, fuse);
     }
     s->launches += 1;
     return true;
