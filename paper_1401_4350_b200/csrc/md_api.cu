@@ -177,6 +177,7 @@ void make_cell_rank(const int nc[3], int order, std::vector<int>& rank) {
 void drop_step_graph(md_system* s) {
     if (s->step_exec) { cudaGraphExecDestroy(s->step_exec); s->step_exec = nullptr; }
     if (s->multi_exec) { cudaGraphExecDestroy(s->multi_exec); s->multi_exec = nullptr; }
+    if (s->oct_exec) { cudaGraphExecDestroy(s->oct_exec); s->oct_exec = nullptr; }
     if (s->quad_exec) { cudaGraphExecDestroy(s->quad_exec); s->quad_exec = nullptr; }
     if (s->pair_exec) { cudaGraphExecDestroy(s->pair_exec); s->pair_exec = nullptr; }
 }
@@ -783,16 +784,17 @@ static md_status integrate_nve(md_system* s, double dt, int64_t nsteps, int32_t 
             if (!build_step_graph(s, fdt, strategy, scatter, staged, seg, 1, &s->step_exec, &s->step_nodes) ||
                 !build_step_graph(s, fdt, strategy, scatter, staged, seg, 2, &s->pair_exec, &s->pair_nodes) ||
                 !build_step_graph(s, fdt, strategy, scatter, staged, seg, 4, &s->quad_exec, &s->quad_nodes) ||
+                !build_step_graph(s, fdt, strategy, scatter, staged, seg, 8, &s->oct_exec, &s->oct_nodes) ||
                 !build_step_graph(s, fdt, strategy, scatter, staged, seg, MD_GRAPH_STEPS, &s->multi_exec, &s->multi_nodes)) s->graphs_off = true;
         }
-        if (s->step_exec && s->pair_exec && s->quad_exec && s->multi_exec) {
-            while (k0 < nsteps) {      // MD_GRAPH_STEPS steps per launch while they fit, then 4, 2, 1 for the rest
+        if (s->step_exec && s->pair_exec && s->quad_exec && s->oct_exec && s->multi_exec) {
+            while (k0 < nsteps) {      // MD_GRAPH_STEPS steps per launch while they fit, then 8, 4, 2, 1 for the rest
                 const int64_t left = nsteps - k0;
-                const int reps = left >= MD_GRAPH_STEPS ? MD_GRAPH_STEPS : left >= 4 ? 4 : left >= 2 ? 2 : 1;
-                cudaGraphExec_t ex = reps == MD_GRAPH_STEPS ? s->multi_exec : reps == 4 ? s->quad_exec : reps == 2 ? s->pair_exec : s->step_exec;
+                const int reps = left >= MD_GRAPH_STEPS ? MD_GRAPH_STEPS : left >= 8 ? 8 : left >= 4 ? 4 : left >= 2 ? 2 : 1;
+                cudaGraphExec_t ex = reps == MD_GRAPH_STEPS ? s->multi_exec : reps == 8 ? s->oct_exec : reps == 4 ? s->quad_exec : reps == 2 ? s->pair_exec : s->step_exec;
                 if (cudaGraphLaunch(ex, s->stream) != cudaSuccess) break;
                 k0 += reps;
-                s->launches += reps == MD_GRAPH_STEPS ? s->multi_nodes : reps == 4 ? s->quad_nodes : reps == 2 ? s->pair_nodes : s->step_nodes;
+                s->launches += reps == MD_GRAPH_STEPS ? s->multi_nodes : reps == 8 ? s->oct_nodes : reps == 4 ? s->quad_nodes : reps == 2 ? s->pair_nodes : s->step_nodes;
             }
         }
     }

@@ -8,7 +8,7 @@
 
 #define MD_TILE 32            // particles per list tile (one warp)
 #define MD_MAX_PATCH 8
-#define MD_GRAPH_STEPS 8        // steps per launch of the multi-step graph of md_integrate
+#define MD_GRAPH_STEPS 16       // steps per launch of the multi-step graph of md_integrate
 #define MD_CLUSTER 16           // owners per cluster of MD_SCATTER_CLUSTER (one 16-bit mask per (cluster, j) unit)
 
 // Device error bits latched in DevCtrl::err
@@ -174,8 +174,8 @@ struct md_system {
     // device-side skin flag drives, forces, kick (md_api.cu build_step_graph)
     cudaEvent_t ev_in, ev_vel;               // md_step_host: ordering of the velocity upload on aux_stream
     cudaGraphExec_t step_exec, multi_exec;   // one step / MD_GRAPH_STEPS steps per launch
-    cudaGraphExec_t quad_exec, pair_exec;    // 4 and 2 steps per launch: the tail of a call, with the fused closing kicks of the multi-step form
-    int quad_nodes, pair_nodes;
+    cudaGraphExec_t oct_exec, quad_exec, pair_exec;    // 8, 4 and 2 steps per launch: the tail of a call, with the fused closing kicks of the multi-step form
+    int oct_nodes, quad_nodes, pair_nodes;
     cudaStream_t cap_stream, aux_stream; // internal capture streams: main sequence, conditional body
     int step_strategy, step_variant, step_stage, step_nodes, multi_nodes;   // *_nodes: kernels per launch outside the IF body
     float step_dt;

@@ -162,9 +162,9 @@ def test_step_graph_equals_plain_launches(MD):
         s.close()
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
     assert out[0][2] == out[1][2] and out[0][2] >= 1
-    # graphs of 8, 4, 2 steps: kick+drift once, then condition + forces per step (the force kernel of an inner step carries
-    # the kicks and the drift of the next one), + the closing kick: 2 n + 2 kernels; a single step: 4.  37 = 4 x 8 + 4 + 1
-    assert out[0][3] == (4 * 18 + 10 + 4) / 37 and out[1][3] > 4
+    # graphs of 16, 8, 4, 2 steps: kick+drift once, then condition + forces per step (the force kernel of an inner step carries
+    # the kicks and the drift of the next one), + the closing kick: 2 n + 2 kernels; a single step: 4.  37 = 2 x 16 + 4 + 1
+    assert out[0][3] == (2 * 34 + 10 + 4) / 37 and out[1][3] > 4
 
 
 def test_options_row_schedule_and_unknown(MD, oracle):
