@@ -249,8 +249,9 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     int* ubase = urank + umax;                                       // [umax + 1]
     int* ustart = ubase + umax + 1;                                  // [umax] first slot of the cell
     int* own_rank = ustart + umax;                                   // [MD_TB]
+    int* own_xyz = own_rank + MD_TB;                                 // [MD_TB] packed cell coordinates of the own cells (pack_coord)
     // transposed scan (MASKS variant): owners' positions, hit words, per-own-cell candidate prefixes
-    const int ts_off = (4 * ((tbl_cap >> 1) + 3 * umax + 1 + MD_TB) + 15) & ~15;     // byte offset from smraw: keeps the shared address space
+    const int ts_off = (4 * ((tbl_cap >> 1) + 3 * umax + 1 + 2 * MD_TB) + 15) & ~15;     // byte offset from smraw: keeps the shared address space
     float* xown = reinterpret_cast<float*>(smraw + ts_off);                           // [3][MD_TB + 2] owners' x, y, z planes (pairs of owners load as f32x2)
     unsigned int* hitw = reinterpret_cast<unsigned int*>(smraw + ts_off + TS_OFF_HITW);   // [TS_CB][TS_ROW]
     unsigned short* own_first = reinterpret_cast<unsigned short*>(smraw + ts_off + TS_OFF_OWNF);   // [TS_OC + 1] first thread of own cell oc
@@ -272,12 +273,22 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     const bool live = i < i1;
     if (tid == 0) { s_flags = 0; s_err = 0; s_own_base = 0; s_U = 0; }
 
+    // cell coordinates of the own cells: three 10-bit fields when every axis has at most 1024 cells, else the linear index
+    const bool xyz_packed = P.ncx <= 1024 && P.ncy <= 1024 && P.ncz <= 1024;
+    auto cell_xyz = [&](int v, int& cx, int& cy, int& cz) {
+        if (xyz_packed) { cx = v & 1023; cy = (v >> 10) & 1023; cz = v >> 20; }
+        else { cz = v % P.ncz; cy = (v / P.ncz) % P.ncy; cx = v / (P.ncz * P.ncy); }
+    };
     // 1. the block's non-empty cells (storage ranks, ascending), compacted
     const int myrank = live ? B.cell_of[i] : -1;
     const int head = live && (tid == 0 || B.cell_of[i - 1] != myrank) ? 1 : 0;
     int nownc;
     const int oc_ex = blk_excl_scan(head, &nownc, sh_scan);
-    if (head) own_rank[oc_ex] = myrank;
+    if (head) {
+        own_rank[oc_ex] = myrank;
+        const int lin = B.cell_lin[myrank];      // the divisions by the cell counts happen once per own cell, not per stencil entry
+        own_xyz[oc_ex] = xyz_packed ? pack_coord(lin / (P.ncz * P.ncy), (lin / P.ncz) % P.ncy, lin % P.ncz) : lin;
+    }
     const int myoc = oc_ex + head - 1;       // ordinal of this thread's cell among the block's own cells
     __syncthreads();
 
@@ -295,9 +306,9 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     for (int t = tid; t < ncand_cap; t += MD_TB) cand[t] = 0x7fffffff;
     __syncthreads();
     for (int t = tid; t < n; t += MD_TB) {
-        const int lin = B.cell_lin[own_rank[t / 27]];
         const int s = t % 27;
-        const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
+        int cx, cy, cz;
+        cell_xyz(own_xyz[t / 27], cx, cy, cz);
         int ax = cx + s / 9 - 1, ay = cy + (s / 3) % 3 - 1, az = cz + s % 3 - 1;
         int wrapped = 0;   // bit a: the stencil crosses the periodic face of axis a
         if (ax < 0) { ax += P.ncx; wrapped |= 1; } else if (ax >= P.ncx) { ax -= P.ncx; wrapped |= 1; }
@@ -436,8 +447,9 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
     //     an empty cell / a cell already listed for this own cell (axes with fewer than 3 cells, S:Q8)
     {
         const bool small_axis = P.ncx < 3 || P.ncy < 3 || P.ncz < 3;
-        auto stencil_rank = [&](int lin, int st) {
-            const int cz = lin % P.ncz, cy = (lin / P.ncz) % P.ncy, cx = lin / (P.ncz * P.ncy);
+        auto stencil_rank = [&](int xyz, int st) {
+            int cx, cy, cz;
+            cell_xyz(xyz, cx, cy, cz);
             int ax = cx + st / 9 - 1, ay = cy + (st / 3) % 3 - 1, az = cz + st % 3 - 1;
             if (ax < 0) ax += P.ncx; else if (ax >= P.ncx) ax -= P.ncx;
             if (ay < 0) ay += P.ncy; else if (ay >= P.ncy) ay -= P.ncy;
@@ -446,7 +458,7 @@ __global__ void __launch_bounds__(MD_TB, 4) k_build_staged(DevParams P, DevBuffe
         };
         __syncthreads();   // cand[] is no longer read by the unique pass
         for (int t = tid; t < n; t += MD_TB) {
-            const int lin = B.cell_lin[own_rank[t / 27]];
+            const int lin = own_xyz[t / 27];
             const int st = t % 27;
             const int r = stencil_rank(lin, st);
             int lo = 0, hi = U - 1;
@@ -1169,7 +1181,7 @@ static void staged_build_sizes(const md_system* s, int* ncand_cap, int* umax, in
     *ncand_cap = nc;
     *umax = um;
     *tbl_cap = 2 * region;
-    *smem = 4 * ((size_t)region + 3 * (size_t)um + 1 + MD_TB) + 16;
+    *smem = 4 * ((size_t)region + 3 * (size_t)um + 1 + 2 * MD_TB) + 16;
 }
 
 void md_launch_build_staged(md_system* s, bool gated) {
