@@ -146,14 +146,16 @@ def test_vertex_and_segmented_are_bitwise_reproducible(MD):
 
 
 def test_step_graph_equals_plain_launches(MD):
-    """md_integrate replays a CUDA graph (rebuild inside a conditional node, 8 steps per launch); with
-    md_set_option(MD_OPT_NO_GRAPH, 1) it launches the same kernels one by one.  VERTEX is deterministic, so both give the same bits,
-    the same number of device-side rebuilds, and 37 steps exercise the multi-step graph and the single-step tail."""
+    """md_integrate replays CUDA graphs (rebuild inside a conditional node, 16 steps per launch, tails of 8, 4, 2, 1; the force
+    kernel of an inner step carries the kicks and the drift of the next one unless MD_OPT_FUSE_STEPS is 0); with
+    md_set_option(MD_OPT_NO_GRAPH, 1) it launches the plain kernels one by one.  VERTEX is deterministic, so all three give the
+    same bits and the same number of device-side rebuilds; 37 steps exercise the multi-step graphs and the single-step tail."""
     w = W.lj_fluid(2 ** 14)
     out = []
-    for no_graph in (False, True):
+    for no_graph, fuse in ((False, 1), (True, 1), (False, 0)):
         s = MD.from_workload(w, order="hilbert")
         s.set_option("no_graph", int(no_graph))
+        s.set_option("fuse_steps", fuse)
         s.build_cells(); s.build_verlet(); s.forces("vertex", "smem")
         l0 = s.launch_count()
         s.integrate(w.dt, 37, "vertex", "smem")
@@ -165,6 +167,9 @@ def test_step_graph_equals_plain_launches(MD):
     # graphs of 16, 8, 4, 2 steps: kick+drift once, then condition + forces per step (the force kernel of an inner step carries
     # the kicks and the drift of the next one), + the closing kick: 2 n + 2 kernels; a single step: 4.  37 = 2 x 16 + 4 + 1
     assert out[0][3] == (2 * 34 + 10 + 4) / 37 and out[1][3] > 4
+    # separate kernels inside the graphs: kick+drift, condition, forces per step + the closing kick: 3 n + 1
+    assert np.array_equal(out[0][0], out[2][0]) and np.array_equal(out[0][1], out[2][1]) and out[0][2] == out[2][2]
+    assert out[2][3] == (2 * 49 + 13 + 4) / 37
 
 
 def test_options_row_schedule_and_unknown(MD, oracle):
